@@ -1,0 +1,190 @@
+/* festina_eval.h — C ABI of libfestina_eval (sm_100a CUDA implementation).
+ *
+ * The batched, SLO-constrained energy argmin of Festina's control plane
+ * (arxiv/paper_2606_30391): global placement (§3.3, Eq. 2-3), per-GPU local
+ * configuration (§3.4, Fig. 8 step 3) and GPU x GPU consolidation scoring (§3.5).
+ * "P:NNN" cites a line of the paper text; "R:sNN" cites a reading listed in
+ * DESIGN.md ("Readings of the paper").
+ *
+ * Conventions common to every call
+ *   - Plain C types only.  Every bulk pointer of one call lives in the memory space named by
+ *     `space` (FS_HOST: ordinary or pinned host memory, FS_DEVICE: device memory of the
+ *     context's CUDA device).  Small descriptor structs (fs_dims, fs_params) are always host.
+ *   - The caller owns all in/out buffers.  Inputs are COPIED into context-owned device memory;
+ *     the caller may reuse them once `cuda_stream` has passed the call (FS_HOST inputs that are
+ *     not pinned are consumed before the call returns).  Outputs are written into the caller's
+ *     buffer; FS_HOST outputs are valid after the call returns, FS_DEVICE outputs after the
+ *     caller synchronises `cuda_stream`.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Return value: FS_OK (0) or a negative fs_status.  Nothing throws or aborts across the ABI.
+ *     Host-visible arguments are validated synchronously.  Device-resident data are
+ *     range-checked inside the kernels; a violation sets a sticky flag that the NEXT call
+ *     returns (and clears) as FS_ERR_RANGE.
+ *   - No feasible candidate: index fields are -1 and the value field is +INF
+ *     (the caller's cue to scale out).
+ *   - All arithmetic is IEEE-754 binary32, round-to-nearest-even, no FMA contraction, in the
+ *     bracketing DESIGN.md states; integer quantities are exact.
+ *   - One context per host thread / stream; calls on one context are not re-entrant.
+ *   - There is no CPU fallback: every entry point runs CUDA kernels on the context's device.
+ */
+#ifndef FESTINA_EVAL_H
+#define FESTINA_EVAL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fs_ctx fs_ctx; /* opaque: device copies of tables/state + scratch */
+
+typedef enum {
+  FS_OK = 0,
+  FS_ERR_ARG = -1,   /* NULL pointer, bad enum, bad count                       */
+  FS_ERR_SHAPE = -2, /* dims outside the supported range                        */
+  FS_ERR_STATE = -3, /* call order: profiles / GPU state not loaded yet         */
+  FS_ERR_RANGE = -4, /* an index / value inside device data was out of range    */
+  FS_ERR_CUDA = -5,  /* a CUDA runtime call failed (see fs_last_cuda_error)     */
+  FS_ERR_NOMEM = -6  /* device or host allocation failed                        */
+} fs_status;
+
+enum { FS_HOST = 0, FS_DEVICE = 1 };
+
+/* flags of fs_local_config: one objective bit and one split-mode bit (R:s8, R:s9) */
+enum {
+  FS_OBJ_ENERGY = 0,       /* slot cost = energy  t*POW ("lowest predicted energy") */
+  FS_OBJ_POWER = 1,        /* slot cost = power   POW   ("minimize power")           */
+  FS_SPLIT_EXHAUSTIVE = 0, /* all SM splits with sum == S                                  */
+  FS_SPLIT_MINSM = 2       /* per-task minimum SM, sum <= S (Fig. 8 step 3)         */
+};
+
+#define FS_RMAX 4   /* tenant slots per GPU (co-resident models)            */
+#define FS_PHASES 2 /* 0 = prefill (TTFT), 1 = decode (TBT) */
+
+/* Limits checked by fs_load_profiles (FS_ERR_SHAPE otherwise). */
+#define FS_MAX_M 32767
+#define FS_MAX_F 256
+#define FS_MAX_S 32
+#define FS_MAX_B 256
+
+/* Table axes: M models, F frequency levels (ascending MHz), S SM-share levels
+ * (index sigma <-> share (sigma+1)/S), B batch levels (index beta <-> batch beta+1).   */
+typedef struct { int32_t M, F, S, B; } fs_dims;
+
+/* Per model: weight-load (cold start) latency P:177; KV-cache MB per token (R:s13);
+ * weight footprint; energy of migrating the model.                              */
+typedef struct { float load_ms, kv_mb_per_token, weights_mb, mig_mj; } fs_model_info;
+
+/* Consolidation constants: idle power, horizon Delta, per-GPU memory
+ * capacity, safety margin delta in percent.                                      */
+typedef struct { float p_idle_w, horizon_ms, mem_cap_mb; int32_t delta_pct; } fs_params;
+
+/* One co-resident model ("tenant") of a GPU: its model id, its SM share index sigma
+ * (share = sigma+1 units), per phase the batch bucket beta, queued tokens q and the
+ * REMAINING SLO slack in ms (slo_ms[0] TTFT-like, slo_ms[1] TBT), and its memory use.    */
+typedef struct {
+  int16_t model; uint8_t sigma, _p0;
+  uint8_t beta[2], _p1[2];
+  uint32_t q[2];
+  float slo_ms[2];
+  float mem_used_mb;
+} fs_tenant; /* 28 bytes */
+
+/* Per-GPU state summary: number of tenants (0 = inactive GPU, never a
+ * candidate), current frequency index F_curr, earliest-available time T_avail, free memory. */
+typedef struct {
+  int32_t n_res, f_cur;
+  float t_avail_ms, mem_free_mb;
+  fs_tenant t[FS_RMAX];
+} fs_gpu_state; /* 128 bytes, 16-byte aligned */
+
+/* Request descriptor: model, prompt length L = Req_in, PREDICTED output length
+ * o_pred (the 5 % pad is applied inside), TTFT and TBT SLOs in ms, caller tag (echoed
+ * nowhere; free for the caller).                                                         */
+typedef struct {
+  int32_t model; uint32_t L, o_pred;
+  float slo_ttft_ms, slo_tbt_ms;
+  uint32_t tag, _pad[2];
+} fs_request; /* 32 bytes */
+
+/* Placement decision: GPU, granted share index sigma, frequency index phi, decode batch
+ * bucket beta the request joins, f_req = lowest feasible frequency index at (gpu, sigma),
+ * marginal energy Delta-E in mJ, TTFT and TBT estimates, flat = (gpu*S + sigma)*F + phi.  */
+typedef struct {
+  int32_t gpu; int16_t sigma, phi, beta, f_req;
+  float energy_mj, ttft_ms, tbt_ms;
+  uint32_t flat, _pad;
+} fs_placement; /* 32 bytes */
+
+/* Local configuration of one GPU: frequency, per tenant share index and per slot batch
+ * bucket, objective value, energy and power at the choice.                               */
+typedef struct {
+  int16_t phi, f_req;
+  uint8_t sigma[FS_RMAX];
+  uint8_t beta[FS_RMAX][2];
+  float cost, energy_mj, power_w;
+  uint32_t flat, _pad[4];
+} fs_local_cfg; /* 48 bytes */
+
+/* Consolidation result per source GPU: best destination, frequency index of the merged
+ * GPU, extra energy the destination pays, net saving of draining the source.             */
+typedef struct { int32_t dst, phi; float score_mj, saving_mj; } fs_consol_out; /* 16 bytes */
+
+/* Create / destroy a context bound to CUDA device `cuda_device`.
+ * fs_create: *out receives the context; FS_ERR_CUDA if the device cannot be used.        */
+int fs_create(fs_ctx** out, int cuda_device);
+int fs_destroy(fs_ctx* ctx);
+
+/* fs_load_profiles — the offline look-up table (§3.2.1; axes R:s1).
+ *   lat, pow : [M][2][F][S][B] fp32, row-major, beta fastest; latency in ms, power in W;
+ *              every entry finite and > 0.
+ *   freq_mhz : [F] ascending (informational; the arithmetic uses indices only).
+ *   models   : [M];  params: host struct.
+ * The library keeps its own copies (and a second, (sigma,phi)-plane-contiguous layout
+ * [M][2][B][S][F] built on the device).  Replaces any previously loaded profiles and
+ * invalidates the GPU state.  Errors: FS_ERR_ARG, FS_ERR_SHAPE, FS_ERR_NOMEM, FS_ERR_CUDA. */
+int fs_load_profiles(fs_ctx* ctx, const fs_dims* dims, const float* lat, const float* pow,
+                     const float* freq_mhz, const fs_model_info* models,
+                     const fs_params* params, int space, void* cuda_stream);
+
+/* fs_set_gpu_state — the per-GPU state summaries the global scheduler polls.
+ *   states : [K] records.  Invariants (FS_ERR_RANGE on the next call if violated; such a GPU
+ *            is treated as inactive): 0 <= n_res <= 4, model/sigma/beta/f_cur in range,
+ *            sum(sigma_i+1) <= S, q < 2^24.
+ * Launches the summary kernel: per GPU, per frequency and per "one more sequence on tenant j"
+ * variant, co-resident feasibility (the segmented max over co-residents)
+ * and the slot-order energy sum.                                     */
+int fs_set_gpu_state(fs_ctx* ctx, int32_t K, const fs_gpu_state* states, int space,
+                     void* cuda_stream);
+
+/* fs_place_batch — global dispatch (§3.3; Eq. 2-3; R:s2-s6).
+ * Every request is scored against the same state snapshot over all (GPU k, grant sigma,
+ * frequency phi); out[r] is the feasible candidate minimising (Delta-E, flat).
+ *   reqs : [R];  out : [R].  R = 0 is a no-op.                                            */
+int fs_place_batch(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* out,
+                   int space, void* cuda_stream);
+
+/* fs_local_config — per-GPU runtime resource allocation (§3.4, Fig. 8 step 3).
+ *   n, gpu_ids : the GPUs to configure; gpu_ids == NULL means GPUs 0..n-1 (n <= K).
+ *   flags      : FS_OBJ_* | FS_SPLIT_*.
+ *   out        : [n].                                                                      */
+int fs_local_config(fs_ctx* ctx, int32_t n, const int32_t* gpu_ids, uint32_t flags,
+                    fs_local_cfg* out, int space, void* cuda_stream);
+
+/* fs_consolidate — drain-one-source scoring over all GPU pairs (§3.5; margin
+ * P:351; idle power vs migration energy P:46; R:s17-s20).   out : [K].             */
+int fs_consolidate(fs_ctx* ctx, fs_consol_out* out, int space, void* cuda_stream);
+
+/* Diagnostics. */
+const char* fs_strerror(int code);
+int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed runtime call */
+/* Kernels launched by this context since creation (bench.py's gpu_launches counter).     */
+uint64_t fs_launch_count(const fs_ctx* ctx);
+/* Nominal work of the last fs_place_batch: eligible (request, GPU) pairs and candidates
+ * (sum of sm_free*F over them), counted on the device.  Valid after synchronising.        */
+int fs_last_place_stats(fs_ctx* ctx, uint64_t* pairs, uint64_t* candidates);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FESTINA_EVAL_H */

@@ -1,0 +1,99 @@
+"""CPU oracle of the Festina decision arithmetic — TEST INFRASTRUCTURE, not the product.
+
+ctypes wrapper around oracle/festina_oracle.cpp (plain C++17, written from PAPER.md; see that
+file's header for the pins).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+`--impl reference` legs may import this package; the CUDA path never does.  Inputs are numpy
+record arrays in the layout of include/festina_eval.h (the seeded generator
+paper_2606_30391_b200/synth.py produces them); outputs are numpy record arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+_PLACEMENT_DT = np.dtype(
+    [("gpu", "<i4"), ("sigma", "<i2"), ("phi", "<i2"), ("beta", "<i2"), ("f_req", "<i2"),
+     ("energy_mj", "<f4"), ("ttft_ms", "<f4"), ("tbt_ms", "<f4"), ("flat", "<u4"), ("_pad", "<u4")])
+_LOCAL_DT = np.dtype(
+    [("phi", "<i2"), ("f_req", "<i2"), ("sigma", "u1", (4,)), ("beta", "u1", (4, 2)),
+     ("cost", "<f4"), ("energy_mj", "<f4"), ("power_w", "<f4"), ("flat", "<u4"),
+     ("_pad", "<u4", (4,))])
+_CONSOL_DT = np.dtype([("dst", "<i4"), ("phi", "<i4"), ("score_mj", "<f4"), ("saving_mj", "<f4")])
+
+OBJ_ENERGY, OBJ_POWER, SPLIT_EXHAUSTIVE, SPLIT_MINSM = 0, 1, 0, 2
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.fo_slot.restype = C.c_int
+        _lib.fo_slot.argtypes = [C.c_int] * 4 + [C.c_void_p] * 2 + [C.c_int] * 5 + [C.c_uint32, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
+    return _lib
+
+
+def _p(a: np.ndarray):
+    assert a.flags["C_CONTIGUOUS"]
+    return C.c_void_p(a.ctypes.data)
+
+
+def _tables(lat: np.ndarray, pow_: np.ndarray):
+    assert lat.dtype == np.float32 and pow_.dtype == np.float32 and lat.shape == pow_.shape
+    M, P, F, S, B = lat.shape
+    assert P == 2
+    return (C.c_int(M), C.c_int(F), C.c_int(S), C.c_int(B), _p(lat), _p(pow_))
+
+
+def place_batch(lat, pow_, models, states, reqs, nthreads: int = 1) -> np.ndarray:
+    """fs_place_batch by definition (PAPER.md; readings s2-s6)."""
+    out = np.zeros(len(reqs), dtype=_PLACEMENT_DT)
+    lib().fo_place_batch(*_tables(lat, pow_), _p(models), C.c_int(len(states)), _p(states),
+                         C.c_int(len(reqs)), _p(reqs), _p(out), C.c_int(nthreads))
+    return out
+
+
+def local_config(lat, pow_, states, flags: int, gpu_ids=None, nthreads: int = 1) -> np.ndarray:
+    """fs_local_config by definition (Fig. 8 step 3)."""
+    if gpu_ids is None:
+        n, ids = len(states), C.c_void_p(0)
+    else:
+        gpu_ids = np.ascontiguousarray(gpu_ids, dtype=np.int32)
+        n, ids = len(gpu_ids), _p(gpu_ids)
+    out = np.zeros(n, dtype=_LOCAL_DT)
+    lib().fo_local_config(*_tables(lat, pow_), _p(states), C.c_int(n), ids, C.c_uint32(flags),
+                          _p(out), C.c_int(nthreads))
+    return out
+
+
+def consolidate(lat, pow_, models, states, p_idle_w, horizon_ms, mem_cap_mb, delta_pct,
+                nthreads: int = 1) -> np.ndarray:
+    """fs_consolidate by definition (PAPER.md, 623; readings s17-s20)."""
+    out = np.zeros(len(states), dtype=_CONSOL_DT)
+    lib().fo_consolidate(*_tables(lat, pow_), _p(models), C.c_int(len(states)), _p(states),
+                         C.c_float(p_idle_w), C.c_float(horizon_ms), C.c_float(mem_cap_mb),
+                         C.c_int(delta_pct), _p(out), C.c_int(nthreads))
+    return out
+
+
+def slot(lat, pow_, m, p, phi, sigma, beta, q, wait, slo):
+    """The shared slot rule: returns (ok, t, e)."""
+    t = C.c_float(0)
+    e = C.c_float(0)
+    ok = lib().fo_slot(*_tables(lat, pow_), m, p, phi, sigma, beta, C.c_uint32(q),
+                       C.c_float(wait), C.c_float(slo), C.byref(t), C.byref(e))
+    return bool(ok), np.float32(t.value), np.float32(e.value)
+
+
+def gpu_freq_floor(lat, pow_, state_rec: np.ndarray) -> int:
+    s = np.ascontiguousarray(state_rec).reshape(1)
+    return int(lib().fo_gpu_freq_floor(*_tables(lat, pow_), _p(s)))
+
+
+def tenant_fmin(lat, pow_, state_rec: np.ndarray, i: int) -> int:
+    s = np.ascontiguousarray(state_rec).reshape(1)
+    return int(lib().fo_tenant_fmin(*_tables(lat, pow_), _p(s), C.c_int(i)))

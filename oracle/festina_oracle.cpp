@@ -1,0 +1,413 @@
+// festina_oracle.cpp — TEST INFRASTRUCTURE, not the product.
+//
+// Plain, slow, obviously-correct CPU statement of what libfestina_eval computes, written from
+// the paper text (arxiv/paper_2606_30391; "P:NNN" = line of PAPER.md) and the readings listed
+// in DESIGN.md ("R:sNN").  Naive nested loops in the paper's order; no blocking, no hoisting,
+// no shared code with the CUDA path (own struct definitions, own arithmetic).  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.
+//
+// Each entry point returns an exact argmin over a finite candidate set under a fixed binary32
+// evaluation order, so the oracle is that definition written out.  Pins (tests/, -m "not gpu"):
+//   slot rule / energy .... Eq. 1-2 identity by hand, brute force
+//   placement ............. Eq. 2-3 special case, brute-force enumeration with an
+//                           independently written numpy evaluator, feasibility/optimality
+//                           invariants, duplicate-GPU / duplicate-frequency tie cases,
+//                           continuous optimum of the analytic generator
+//   local config .......... Fig. 8 step 3 worked table, brute force
+//   consolidation ......... brute force, C*_ab symmetry, empty-destination case,
+//                           App. G arithmetic
+// Nothing here is "parity unpinned".
+//
+// Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC (see oracle/build.py).
+// -ffp-contract=off matters: every fl(.) below is ONE binary32 rounding.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <thread>
+#include <vector>
+
+namespace {
+
+constexpr int RMAX = 4;
+const float INF = std::numeric_limits<float>::infinity();
+
+struct Tenant {  // 28 B, layout of the state record
+  int16_t model; uint8_t sigma, p0; uint8_t beta[2], p1[2];
+  uint32_t q[2]; float slo_ms[2]; float mem_used_mb;
+};
+struct GpuState { int32_t n_res, f_cur; float t_avail_ms, mem_free_mb; Tenant t[RMAX]; };
+struct Request { int32_t model; uint32_t L, o_pred; float slo_ttft_ms, slo_tbt_ms; uint32_t tag, pad[2]; };
+struct ModelInfo { float load_ms, kv_mb_per_token, weights_mb, mig_mj; };
+struct Placement { int32_t gpu; int16_t sigma, phi, beta, f_req; float energy_mj, ttft_ms, tbt_ms; uint32_t flat, pad; };
+struct LocalCfg { int16_t phi, f_req; uint8_t sigma[RMAX]; uint8_t beta[RMAX][2]; float cost, energy_mj, power_w; uint32_t flat, pad[4]; };
+struct ConsolOut { int32_t dst, phi; float score_mj, saving_mj; };
+static_assert(sizeof(Tenant) == 28 && sizeof(GpuState) == 128 && sizeof(Request) == 32, "layout");
+static_assert(sizeof(Placement) == 32 && sizeof(LocalCfg) == 48 && sizeof(ConsolOut) == 16, "layout");
+
+struct Tables {  // LUT[model][phase][freq][SM share][batch] (axes R:s1)
+  int M, F, S, B;
+  const float* lat; const float* pow;
+  size_t idx(int m, int p, int f, int s, int b) const {
+    return ((((size_t)m * 2 + p) * F + f) * S + s) * B + b;
+  }
+  float LAT(int m, int p, int f, int s, int b) const { return lat[idx(m, p, f, s, b)]; }
+  float POW(int m, int p, int f, int s, int b) const { return pow[idx(m, p, f, s, b)]; }
+};
+
+struct Slot { bool ok; float t, e; };
+
+// Shared slot rule.  Energy = Power x Time (Eq. 1); deadline check at a frequency
+// (P:216); "TBT for decode; TTFT for prefill" (R:s11):
+//   rounds = ceil(q/(beta+1));  t = fl(rounds*LAT);  e = fl(t*POW)
+//   prefill: fl(wait+t) <= slo     decode: LAT <= slo
+Slot slot_eval(const Tables& T, int m, int p, int phi, int sigma, int beta, uint32_t q,
+               float wait, float slo) {
+  if (q == 0) return {true, 0.0f, 0.0f};
+  uint32_t n = (uint32_t)beta + 1u;
+  uint32_t rounds = (q + n - 1u) / n;
+  float lat = T.LAT(m, p, phi, sigma, beta);
+  float t = (float)rounds * lat;
+  bool ok = (p == 0) ? ((wait + t) <= slo) : (lat <= slo);
+  float e = t * T.POW(m, p, phi, sigma, beta);
+  return {ok, t, e};
+}
+
+struct TenantEval { bool ok; float e; };
+
+// One co-resident at frequency phi with its own share sigma_i, wait = 0 (its slo is already
+// the remaining slack, R:s12).  bump = "one more sequence joins this tenant's decode batch":
+// the decode bucket moves to beta+1 when the decode queue is non-empty; past the table => not ok.
+TenantEval tenant_eval(const Tables& T, const Tenant& t, int phi, int sigma, bool bump) {
+  int b1 = t.beta[1] + ((bump && t.q[1] > 0) ? 1 : 0);
+  if (b1 >= T.B) return {false, INF};
+  Slot s0 = slot_eval(T, t.model, 0, phi, sigma, t.beta[0], t.q[0], 0.0f, t.slo_ms[0]);
+  Slot s1 = slot_eval(T, t.model, 1, phi, sigma, b1, t.q[1], 0.0f, t.slo_ms[1]);
+  return {s0.ok && s1.ok, s0.e + s1.e};
+}
+
+int sm_free_of(const GpuState& g, int S) {
+  int used = 0;
+  for (int i = 0; i < g.n_res; ++i) used += g.t[i].sigma + 1;
+  return S - used;
+}
+
+// ------------------------------------------------------------------------------------------
+// fs_place_batch: global dispatch.  Phase 1 feasibility, Phase 2
+// energy argmin (Eq. 2-3) generalised to (GPU, grant sigma, frequency phi)
+// (R:s2-s5); F_max retry is inside the swept phi set.  Tie: lowest flat (R:s6).
+void place_one(const Tables& T, const ModelInfo* mi, const GpuState* gs, int K,
+               const Request& rq, Placement& out) {
+  const int m = rq.model;
+  const uint32_t O = (21u * rq.o_pred + 19u) / 20u;        // ceil(1.05*o_pred), R:s14
+  const float mem = (float)(rq.L + O) * mi[m].kv_mb_per_token;  // Req_mem, R:s13
+  bool have = false;
+  float bestE = INF; uint32_t bestFlat = 0xFFFFFFFFu;
+  Placement best{}; best.gpu = -1; best.sigma = best.phi = best.beta = best.f_req = -1;
+  best.energy_mj = INF; best.ttft_ms = INF; best.tbt_ms = INF; best.flat = 0xFFFFFFFFu;
+
+  for (int k = 0; k < K; ++k) {
+    const GpuState& g = gs[k];
+    if (g.n_res < 1) continue;                             // inactive GPU (R:s16)
+    if (!(mem <= g.mem_free_mb)) continue;                 // memory must fit (R:s12)
+    const int smf = sm_free_of(g, T.S);
+    if (smf < 1) continue;
+    int j = -1;
+    for (int i = 0; i < g.n_res; ++i) if (g.t[i].model == m) { j = i; break; }
+    if (j < 0 && g.n_res >= RMAX) continue;                // no slot for a cold model
+    float wait = g.t_avail_ms;
+    if (j < 0) wait = wait + mi[m].load_ms;                // cold start: weight load
+    const int br0 = (int)(rq.L < (uint32_t)T.B ? rq.L : (uint32_t)T.B) - 1;
+    const int br1 = (j >= 0 && g.t[j].q[1] > 0) ? g.t[j].beta[1] + 1 : 0;
+    if (br1 >= T.B) continue;
+    // Ecur: energy of the GPU as it is now, at F_curr, slot-order sum (R:s4)
+    float Ecur = 0.0f;
+    for (int i = 0; i < g.n_res; ++i) {
+      TenantEval te = tenant_eval(T, g.t[i], g.f_cur, g.t[i].sigma, false);
+      Ecur = (i == 0) ? te.e : (Ecur + te.e);
+    }
+    for (int sg = 0; sg < smf; ++sg) {
+      int f_req = -1;
+      for (int phi = 0; phi < T.F; ++phi) {
+        bool ok_co = true; float A = 0.0f;
+        for (int i = 0; i < g.n_res; ++i) {
+          TenantEval te = tenant_eval(T, g.t[i], phi, g.t[i].sigma, i == j);
+          ok_co = ok_co && te.ok;
+          A = (i == 0) ? te.e : (A + te.e);
+        }
+        Slot s0 = slot_eval(T, m, 0, phi, sg, br0 < 0 ? 0 : br0, rq.L, wait, rq.slo_ttft_ms);
+        Slot s1 = slot_eval(T, m, 1, phi, sg, br1, O, 0.0f, rq.slo_tbt_ms);
+        if (!(ok_co && s0.ok && s1.ok)) continue;
+        float dE = (A + (s0.e + s1.e)) - Ecur;
+        if (!(dE < INF)) continue;                         // overflowed energy = infeasible (R:s23)
+        if (dE == 0.0f) dE = 0.0f;                         // -0 -> +0
+        if (f_req < 0) f_req = phi;
+        uint32_t flat = (uint32_t)((k * T.S + sg) * T.F + phi);
+        if (!have || dE < bestE) {                         // strict <: first (lowest flat) wins ties
+          have = true; bestE = dE; bestFlat = flat;
+          best.gpu = k; best.sigma = (int16_t)sg; best.phi = (int16_t)phi;
+          best.beta = (int16_t)br1; best.f_req = (int16_t)f_req;
+          best.energy_mj = dE; best.ttft_ms = wait + s0.t;
+          best.tbt_ms = T.LAT(m, 1, phi, sg, br1); best.flat = flat;
+        }
+      }
+    }
+  }
+  (void)bestFlat;
+  out = best;
+}
+
+// ------------------------------------------------------------------------------------------
+// fs_local_config: frequency sweep with per-task SM allocation (Fig. 8 step 3,
+// P:206-210); batching P:248; objective R:s8; split domain R:s9; one beta per slot R:s10.
+// Hierarchical definition: best beta per slot, then tenant sums, then the argmin.
+struct SlotBest { float g; int beta; float e; float pw; };
+
+SlotBest slot_search(const Tables& T, const Tenant& t, int p, int phi, int sigma, bool obj_power) {
+  if (t.q[p] == 0) return {0.0f, 0, 0.0f, 0.0f};
+  SlotBest b{INF, 0, 0.0f, 0.0f};
+  int nb = (int)(t.q[p] < (uint32_t)T.B ? t.q[p] : (uint32_t)T.B);
+  for (int beta = 0; beta < nb; ++beta) {
+    Slot s = slot_eval(T, t.model, p, phi, sigma, beta, t.q[p], 0.0f, t.slo_ms[p]);
+    if (!s.ok) continue;
+    float pw = T.POW(t.model, p, phi, sigma, beta);
+    float cost = obj_power ? pw : s.e;
+    if (cost < b.g) { b.g = cost; b.beta = beta; b.e = s.e; b.pw = pw; }
+  }
+  return b;
+}
+
+uint64_t binom(int n, int k) {
+  if (k < 0 || k > n) return 0;
+  uint64_t r = 1;
+  for (int i = 1; i <= k; ++i) r = r * (uint64_t)(n - k + i) / (uint64_t)i;
+  return r;
+}
+
+void local_one(const Tables& T, const GpuState& g, uint32_t flags, LocalCfg& out) {
+  const bool obj_power = flags & 1u, minsm = flags & 2u;
+  std::memset(&out, 0, sizeof(out));
+  out.phi = -1; out.f_req = -1; out.flat = 0xFFFFFFFFu;
+  const int n = g.n_res;
+  if (n < 1) { out.cost = 0.0f; return; }
+  out.cost = INF; out.energy_mj = INF; out.power_w = INF;
+  if (n > T.S) return;
+  const int F = T.F, S = T.S;
+  // G_i[phi][sigma] and the slot minima behind it
+  std::vector<SlotBest> sb((size_t)n * 2 * F * S);
+  std::vector<float> G((size_t)n * F * S);
+  auto SB = [&](int i, int p, int phi, int sg) -> SlotBest& { return sb[(((size_t)i * 2 + p) * F + phi) * S + sg]; };
+  auto GG = [&](int i, int phi, int sg) -> float& { return G[((size_t)i * F + phi) * S + sg]; };
+  for (int i = 0; i < n; ++i)
+    for (int phi = 0; phi < F; ++phi)
+      for (int sg = 0; sg < S; ++sg) {
+        SB(i, 0, phi, sg) = slot_search(T, g.t[i], 0, phi, sg, obj_power);
+        SB(i, 1, phi, sg) = slot_search(T, g.t[i], 1, phi, sg, obj_power);
+        GG(i, phi, sg) = SB(i, 0, phi, sg).g + SB(i, 1, phi, sg).g;
+      }
+  bool have = false; float bestC = INF; int bphi = -1; int bsig[RMAX] = {0, 0, 0, 0}; uint32_t bflat = 0;
+  int f_req = -1;
+  if (minsm) {
+    // the paper's rule: per frequency, each task's minimum SM meeting its deadline; sum <= budget
+    for (int phi = 0; phi < F; ++phi) {
+      int sig[RMAX]; bool all = true; int tot = 0;
+      for (int i = 0; i < n && all; ++i) {
+        sig[i] = -1;
+        for (int sg = 0; sg < S; ++sg) if (GG(i, phi, sg) < INF) { sig[i] = sg; break; }
+        if (sig[i] < 0) all = false; else tot += sig[i] + 1;
+      }
+      if (!all || tot > S) continue;                      // "<= budget": Fig. 8 accepts 100 % (R:s7)
+      float C = 0.0f;
+      for (int i = 0; i < n; ++i) C = (i == 0) ? GG(i, phi, sig[i]) : (C + GG(i, phi, sig[i]));
+      if (!(C < INF)) continue;
+      if (f_req < 0) f_req = phi;
+      if (!have || C < bestC) { have = true; bestC = C; bphi = phi; bflat = (uint32_t)phi; for (int i = 0; i < n; ++i) bsig[i] = sig[i]; }
+    }
+  } else {
+    const uint64_t NS = binom(S - 1, n - 1);
+    for (int phi = 0; phi < F; ++phi) {
+      // all compositions of S into n positive parts, lexicographic with sigma_0 most significant
+      int sig[RMAX] = {0, 0, 0, 0};
+      uint64_t rank = 0;
+      // plain nested loops over (sigma_0..sigma_3), keeping the tuples that sum to S (n <= 4)
+      for (int s0 = 0; s0 < S; ++s0) {
+        if (n == 1) { if (s0 + 1 != S) continue; }
+        for (int s1 = 0; s1 < (n >= 2 ? S : 1); ++s1) {
+          if (n == 2) { if (s0 + 1 + s1 + 1 != S) continue; }
+          for (int s2 = 0; s2 < (n >= 3 ? S : 1); ++s2) {
+            if (n == 3) { if (s0 + s1 + s2 + 3 != S) continue; }
+            for (int s3 = 0; s3 < (n >= 4 ? S : 1); ++s3) {
+              if (n == 4) { if (s0 + s1 + s2 + s3 + 4 != S) continue; }
+              sig[0] = s0; sig[1] = s1; sig[2] = s2; sig[3] = s3;
+              float C = 0.0f;
+              for (int i = 0; i < n; ++i) C = (i == 0) ? GG(i, phi, sig[i]) : (C + GG(i, phi, sig[i]));
+              uint64_t this_rank = rank++;
+              if (!(C < INF)) continue;
+              if (f_req < 0) f_req = phi;
+              if (!have || C < bestC) {
+                have = true; bestC = C; bphi = phi; bflat = (uint32_t)((uint64_t)phi * NS + this_rank);
+                for (int i = 0; i < n; ++i) bsig[i] = sig[i];
+              }
+            }
+          }
+        }
+      }
+    }
+  }
+  if (!have) return;
+  out.phi = (int16_t)bphi; out.f_req = (int16_t)f_req; out.cost = bestC; out.flat = bflat;
+  float E = 0.0f, PW = 0.0f;
+  for (int i = 0; i < n; ++i) {
+    const SlotBest& a = SB(i, 0, bphi, bsig[i]); const SlotBest& b = SB(i, 1, bphi, bsig[i]);
+    out.sigma[i] = (uint8_t)bsig[i]; out.beta[i][0] = (uint8_t)a.beta; out.beta[i][1] = (uint8_t)b.beta;
+    float ei = a.e + b.e, pi = a.pw + b.pw;
+    E = (i == 0) ? ei : (E + ei); PW = (i == 0) ? pi : (PW + pi);
+  }
+  out.energy_mj = E; out.power_w = PW;
+}
+
+// ------------------------------------------------------------------------------------------
+// fs_consolidate: drain-one-source scoring over all GPU pairs (R:s17).  Per-tenant minimum
+// feasible share per frequency (P:252 rule (1)), 5 % margin on SMs and memory,
+// idle power vs migration energy.
+struct GpuAgg { std::vector<int> need; std::vector<float> E; float mem; float Cstar; int n; };
+
+void consolidate_all(const Tables& T, const ModelInfo* mi, const GpuState* gs, int K,
+                     float p_idle_w, float horizon_ms, float mem_cap_mb, int delta_pct,
+                     ConsolOut* out, int nthreads) {
+  const int F = T.F, S = T.S;
+  const int NEED_INF = 1 << 20;
+  const int S_eff = (S * (100 - delta_pct)) / 100;
+  const float M_eff = (mem_cap_mb * (float)(100 - delta_pct)) / 100.0f;
+  std::vector<GpuAgg> agg(K);
+  for (int g = 0; g < K; ++g) {
+    GpuAgg& a = agg[g]; a.n = gs[g].n_res; a.need.assign(F, NEED_INF); a.E.assign(F, INF); a.mem = 0.0f; a.Cstar = INF;
+    if (a.n < 1) continue;
+    for (int i = 0; i < a.n; ++i) a.mem = (i == 0) ? gs[g].t[i].mem_used_mb : (a.mem + gs[g].t[i].mem_used_mb);
+    for (int phi = 0; phi < F; ++phi) {
+      int need = 0; float E = 0.0f; bool all = true;
+      for (int i = 0; i < a.n && all; ++i) {
+        int smin = -1; float ei = INF;
+        for (int sg = 0; sg < S; ++sg) {
+          TenantEval te = tenant_eval(T, gs[g].t[i], phi, sg, false);
+          if (te.ok) { smin = sg; ei = te.e; break; }
+        }
+        if (smin < 0) { all = false; break; }
+        need += smin + 1; E = (i == 0) ? ei : (E + ei);
+      }
+      if (all) { a.need[phi] = need; a.E[phi] = E; }
+      if (all && need <= S_eff && E < a.Cstar) a.Cstar = E;   // lowest phi on ties
+    }
+  }
+  auto work = [&](int a0, int a1) {
+    for (int a = a0; a < a1; ++a) {
+      ConsolOut o; o.dst = -1; o.phi = -1; o.score_mj = INF; o.saving_mj = -INF;
+      const GpuAgg& A = agg[a];
+      if (A.n >= 1) {
+        bool have = false;
+        for (int b = 0; b < K; ++b) {
+          const GpuAgg& Bg = agg[b];
+          if (b == a || Bg.n < 1) continue;
+          if (A.n + Bg.n > RMAX) continue;
+          if (!((A.mem + Bg.mem) <= M_eff)) continue;
+          if (!(Bg.Cstar < INF)) continue;
+          float Cab = INF; int phis = -1;
+          for (int phi = 0; phi < F; ++phi) {
+            if (A.need[phi] + Bg.need[phi] > S_eff) continue;
+            float e = Bg.E[phi] + A.E[phi];
+            if (e < Cab) { Cab = e; phis = phi; }
+          }
+          if (phis < 0) continue;
+          float score = Cab - Bg.Cstar;
+          if (!have || score < o.score_mj) { have = true; o.dst = b; o.phi = phis; o.score_mj = score; }
+        }
+        if (have) {
+          float mig = 0.0f;
+          for (int i = 0; i < A.n; ++i) mig = (i == 0) ? mi[gs[a].t[i].model].mig_mj : (mig + mi[gs[a].t[i].model].mig_mj);
+          o.saving_mj = ((p_idle_w * horizon_ms) + A.Cstar) - (o.score_mj + mig);
+        }
+      }
+      out[a] = o;
+    }
+  };
+  if (nthreads <= 1) { work(0, K); return; }
+  std::vector<std::thread> th;
+  for (int t = 0; t < nthreads; ++t) th.emplace_back(work, (int)((int64_t)K * t / nthreads), (int)((int64_t)K * (t + 1) / nthreads));
+  for (auto& x : th) x.join();
+}
+
+template <class Fn> void par_for(int n, int nthreads, Fn fn) {
+  if (nthreads <= 1) { for (int i = 0; i < n; ++i) fn(i); return; }
+  std::vector<std::thread> th;
+  for (int t = 0; t < nthreads; ++t)
+    th.emplace_back([=]() { for (int i = t; i < n; i += nthreads) fn(i); });
+  for (auto& x : th) x.join();
+}
+
+}  // namespace
+
+extern "C" {
+
+int fo_place_batch(int M, int F, int S, int B, const float* lat, const float* pow,
+                   const void* models, int K, const void* states, int R, const void* reqs,
+                   void* out, int nthreads) {
+  Tables T{M, F, S, B, lat, pow};
+  const ModelInfo* mi = (const ModelInfo*)models; const GpuState* gs = (const GpuState*)states;
+  const Request* rq = (const Request*)reqs; Placement* o = (Placement*)out;
+  par_for(R, nthreads, [&](int r) { place_one(T, mi, gs, K, rq[r], o[r]); });
+  return 0;
+}
+
+int fo_local_config(int M, int F, int S, int B, const float* lat, const float* pow,
+                    const void* states, int n, const int32_t* gpu_ids, uint32_t flags, void* out,
+                    int nthreads) {
+  Tables T{M, F, S, B, lat, pow};
+  const GpuState* gs = (const GpuState*)states; LocalCfg* o = (LocalCfg*)out;
+  par_for(n, nthreads, [&](int i) { local_one(T, gs[gpu_ids ? gpu_ids[i] : i], flags, o[i]); });
+  return 0;
+}
+
+int fo_consolidate(int M, int F, int S, int B, const float* lat, const float* pow,
+                   const void* models, int K, const void* states, float p_idle_w,
+                   float horizon_ms, float mem_cap_mb, int delta_pct, void* out, int nthreads) {
+  Tables T{M, F, S, B, lat, pow};
+  consolidate_all(T, (const ModelInfo*)models, (const GpuState*)states, K, p_idle_w, horizon_ms,
+                  mem_cap_mb, delta_pct, (ConsolOut*)out, nthreads);
+  return 0;
+}
+
+// Exposed for the pins: the slot rule and the per-GPU co-resident summary (segmented max).
+int fo_slot(int M, int F, int S, int B, const float* lat, const float* pow, int m, int p, int phi,
+            int sigma, int beta, uint32_t q, float wait, float slo, float* t, float* e) {
+  Tables T{M, F, S, B, lat, pow};
+  Slot s = slot_eval(T, m, p, phi, sigma, beta, q, wait, slo);
+  *t = s.t; *e = s.e; return s.ok ? 1 : 0;
+}
+
+// Lowest frequency index at which every co-resident of GPU g is feasible (-1 if none):
+// the "device-wide operating point" lower bound, max over co-residents of each one's lowest
+// feasible frequency when feasibility is monotone (R:s3).
+int fo_gpu_freq_floor(int M, int F, int S, int B, const float* lat, const float* pow,
+                      const void* state) {
+  Tables T{M, F, S, B, lat, pow};
+  const GpuState& g = *(const GpuState*)state;
+  for (int phi = 0; phi < F; ++phi) {
+    bool ok = true;
+    for (int i = 0; i < g.n_res; ++i) ok = ok && tenant_eval(T, g.t[i], phi, g.t[i].sigma, false).ok;
+    if (ok) return phi;
+  }
+  return -1;
+}
+
+// Per-tenant lowest feasible frequency (for the "max over co-residents" pin).
+int fo_tenant_fmin(int M, int F, int S, int B, const float* lat, const float* pow,
+                   const void* state, int i) {
+  Tables T{M, F, S, B, lat, pow};
+  const GpuState& g = *(const GpuState*)state;
+  for (int phi = 0; phi < F; ++phi)
+    if (tenant_eval(T, g.t[i], phi, g.t[i].sigma, false).ok) return phi;
+  return -1;
+}
+
+}  // extern "C"
