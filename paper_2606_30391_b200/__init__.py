@@ -1,0 +1,212 @@
+"""paper_2606_30391_b200 — thin Python binding of libfestina_eval (the sm_100a CUDA library).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels behind the C ABI
+declared in include/festina_eval.h.  There is no CPU fallback; importing the package without the
+built library, or creating a context without a CUDA device, fails loudly.
+
+Buffers may be numpy arrays (host; FS_HOST) or torch CUDA tensors (device; FS_DEVICE).  Record
+layouts are the numpy dtypes of `paper_2606_30391_b200.synth` (mirrors of the C structs).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import synth
+from .build import LIB as _LIB_PATH, build as build_library
+
+FS_OK, FS_ERR_ARG, FS_ERR_SHAPE, FS_ERR_STATE, FS_ERR_RANGE, FS_ERR_CUDA, FS_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
+FS_HOST, FS_DEVICE = 0, 1
+FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
+
+# every symbol include/festina_eval.h declares
+SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
+           "fs_local_config", "fs_consolidate", "fs_strerror", "fs_last_cuda_error",
+           "fs_launch_count", "fs_last_place_stats")
+
+
+class FsDims(C.Structure):
+    _fields_ = [("M", C.c_int32), ("F", C.c_int32), ("S", C.c_int32), ("B", C.c_int32)]
+
+
+class FsParams(C.Structure):
+    _fields_ = [("p_idle_w", C.c_float), ("horizon_ms", C.c_float), ("mem_cap_mb", C.c_float),
+                ("delta_pct", C.c_int32)]
+
+
+class FestinaError(RuntimeError):
+    def __init__(self, code: int, where: str, cuda: int = 0):
+        self.code = code
+        msg = lib().fs_strerror(code).decode()
+        super().__init__(f"{where}: {msg} (fs_status {code}" + (f", cudaError {cuda})" if cuda else ")"))
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libfestina_eval.so (built in-tree by build.py).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is not built: run `python -m paper_2606_30391_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    L = C.CDLL(_LIB_PATH)
+    vp, i32, u32 = C.c_void_p, C.c_int32, C.c_uint32
+    L.fs_create.argtypes = [C.POINTER(vp), C.c_int]
+    L.fs_destroy.argtypes = [vp]
+    L.fs_load_profiles.argtypes = [vp, C.POINTER(FsDims), vp, vp, vp, vp, C.POINTER(FsParams), C.c_int, vp]
+    L.fs_set_gpu_state.argtypes = [vp, i32, vp, C.c_int, vp]
+    L.fs_place_batch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
+    L.fs_local_config.argtypes = [vp, i32, vp, u32, vp, C.c_int, vp]
+    L.fs_consolidate.argtypes = [vp, vp, C.c_int, vp]
+    L.fs_strerror.argtypes = [C.c_int]
+    L.fs_strerror.restype = C.c_char_p
+    L.fs_last_cuda_error.argtypes = [vp]
+    L.fs_launch_count.argtypes = [vp]
+    L.fs_launch_count.restype = C.c_uint64
+    L.fs_last_place_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    for name in SYMBOLS:
+        getattr(L, name)   # AttributeError if the library does not export it
+    _lib = L
+    return L
+
+
+def _is_torch_cuda(x) -> bool:
+    return hasattr(x, "is_cuda") and bool(x.is_cuda)
+
+
+def _buf(x, nbytes: int | None = None):
+    """(pointer, space, keepalive) of a numpy array, a torch tensor (CPU or CUDA) or None."""
+    if x is None:
+        return C.c_void_p(0), None, None
+    if hasattr(x, "data_ptr"):                      # torch tensor
+        assert x.is_contiguous()
+        if nbytes is not None:
+            assert x.numel() * x.element_size() >= nbytes, "buffer too small"
+        return C.c_void_p(x.data_ptr()), (FS_DEVICE if x.is_cuda else FS_HOST), x
+    a = np.ascontiguousarray(x)
+    if nbytes is not None:
+        assert a.nbytes >= nbytes, "buffer too small"
+    return C.c_void_p(a.ctypes.data), FS_HOST, a
+
+
+def _stream_ptr(stream) -> C.c_void_p:
+    if stream is None:
+        return C.c_void_p(0)
+    if hasattr(stream, "cuda_stream"):
+        return C.c_void_p(stream.cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+class Festina:
+    """One libfestina_eval context on one CUDA device (not thread-safe, see festina_eval.h)."""
+
+    def __init__(self, device: int = 0):
+        self._h = C.c_void_p(0)
+        rc = lib().fs_create(C.byref(self._h), int(device))
+        if rc != FS_OK:
+            self._h = C.c_void_p(0)
+            raise FestinaError(rc, "fs_create")
+        self.device = device
+        self.dims = None
+        self.K = 0
+
+    def close(self):
+        if self._h:
+            lib().fs_destroy(self._h)
+            self._h = C.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int, where: str):
+        if rc != FS_OK:
+            raise FestinaError(rc, where, lib().fs_last_cuda_error(self._h))
+
+    # -- the five calls of the boundary ----------------------------------------------------
+    def load_profiles(self, lat, pow_, freq_mhz, models, params: synth.Params, stream=None):
+        M, P, F, S, B = tuple(lat.shape)
+        assert P == 2 and tuple(pow_.shape) == tuple(lat.shape)
+        n = M * 2 * F * S * B * 4
+        pl, sp, k1 = _buf(lat, n)
+        pp, sp2, k2 = _buf(pow_, n)
+        pf, sp3, k3 = _buf(freq_mhz, F * 4)
+        pm, sp4, k4 = _buf(models, M * 16)
+        assert sp == sp2 == sp3 == sp4, "all bulk pointers of one call live in one memory space"
+        dims = FsDims(M, F, S, B)
+        prm = FsParams(params.p_idle_w, params.horizon_ms, params.mem_cap_mb, params.delta_pct)
+        rc = lib().fs_load_profiles(self._h, C.byref(dims), pl, pp, pf, pm, C.byref(prm), sp,
+                                    _stream_ptr(stream))
+        self._check(rc, "fs_load_profiles")
+        self.dims = (M, F, S, B)
+        self.K = 0
+
+    def set_gpu_state(self, states, K: int | None = None, stream=None):
+        if K is None:
+            K = len(states) if not hasattr(states, "data_ptr") else states.numel() * states.element_size() // 128
+        ps, sp, keep = _buf(states, K * 128)
+        rc = lib().fs_set_gpu_state(self._h, K, ps, sp if sp is not None else FS_HOST, _stream_ptr(stream))
+        self._check(rc, "fs_set_gpu_state")
+        self.K = K
+
+    def place_batch(self, reqs, out=None, R: int | None = None, stream=None):
+        """Returns a numpy record array (host inputs) or writes into `out` (device tensors)."""
+        if R is None:
+            R = len(reqs) if not hasattr(reqs, "data_ptr") else reqs.numel() * reqs.element_size() // 32
+        pr, sp, keep = _buf(reqs, R * 32)
+        if sp is None:
+            sp = FS_HOST
+        if out is None:
+            assert sp == FS_HOST, "device inputs need a device `out` tensor"
+            out = np.zeros(R, dtype=synth.PLACEMENT_DT)
+        po, spo, keep2 = _buf(out, R * 32)
+        assert spo == sp or R == 0
+        rc = lib().fs_place_batch(self._h, R, pr, po, sp, _stream_ptr(stream))
+        self._check(rc, "fs_place_batch")
+        return out
+
+    def local_config(self, flags: int = 0, gpu_ids=None, n: int | None = None, out=None, stream=None):
+        if gpu_ids is not None and not hasattr(gpu_ids, "data_ptr"):
+            gpu_ids = np.ascontiguousarray(gpu_ids, dtype=np.int32)
+        if n is None:
+            n = self.K if gpu_ids is None else (len(gpu_ids) if not hasattr(gpu_ids, "data_ptr") else gpu_ids.numel())
+        pi, spi, keep = _buf(gpu_ids)
+        if out is None:
+            assert spi in (None, FS_HOST)
+            out = np.zeros(n, dtype=synth.LOCAL_CFG_DT)
+        po, spo, keep2 = _buf(out, n * 48)
+        assert spi is None or spi == spo
+        rc = lib().fs_local_config(self._h, n, pi, flags, po, spo, _stream_ptr(stream))
+        self._check(rc, "fs_local_config")
+        return out
+
+    def consolidate(self, out=None, stream=None):
+        if out is None:
+            out = np.zeros(self.K, dtype=synth.CONSOL_DT)
+        po, spo, keep = _buf(out, self.K * 16)
+        rc = lib().fs_consolidate(self._h, po, spo, _stream_ptr(stream))
+        self._check(rc, "fs_consolidate")
+        return out
+
+    # -- diagnostics -------------------------------------------------------------------------
+    @property
+    def launch_count(self) -> int:
+        return int(lib().fs_launch_count(self._h))
+
+    def last_place_stats(self):
+        a, b = C.c_uint64(0), C.c_uint64(0)
+        self._check(lib().fs_last_place_stats(self._h, C.byref(a), C.byref(b)), "fs_last_place_stats")
+        return int(a.value), int(b.value)
+
+    def load_cluster(self, cl: synth.Cluster, stream=None):
+        """Convenience: fs_load_profiles + fs_set_gpu_state from a synthetic cluster (host)."""
+        self.load_profiles(cl.lat, cl.pow, cl.freq_mhz, cl.models, cl.params, stream)
+        self.set_gpu_state(cl.states, stream=stream)
+        return self

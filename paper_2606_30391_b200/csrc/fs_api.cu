@@ -1,0 +1,347 @@
+// fs_api.cu — the C ABI of libfestina_eval (include/festina_eval.h): context, argument
+// validation, device-memory ownership, host<->device staging, kernel sequencing.
+// No arithmetic of the method lives here (kernels: fs_tables/fs_summary/fs_place/fs_local/
+// fs_consol .cu) and there is no CPU fallback: without a CUDA device every call fails.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "fs_kernels.h"
+
+struct fs_ctx {
+  int dev = 0;
+  fs_dims d{0, 0, 0, 0};
+  fs_params prm{0, 0, 0, 0};
+  bool have_prof = false, have_state = false;
+  // profiles
+  float *lat = nullptr, *pow = nullptr, *latT = nullptr, *powT = nullptr, *freq = nullptr;
+  fs_model_info* models = nullptr;
+  size_t table_cap = 0; int m_cap = 0, f_cap = 0;
+  uint32_t *comp = nullptr, *comp_n = nullptr; int ns_stride = 1; size_t comp_cap = 0;
+  // state + summaries
+  int K = 0, k_cap = 0;
+  fs_gpu_state* states = nullptr; FsGpuInfo* ginfo = nullptr; float* gA = nullptr; size_t gA_cap = 0;
+  int32_t *warm_off = nullptr, *warm_cursor = nullptr; uint32_t* warm_item = nullptr; int warm_m_cap = 0;
+  // placement scratch
+  int r_cap = 0; unsigned long long* keys = nullptr; unsigned long long* stats = nullptr;
+  fs_request* reqs_dev = nullptr; fs_placement* place_dev = nullptr;
+  // local scratch
+  size_t local_cap = 0; int n_cap = 0; float* G = nullptr; uint8_t* Bst = nullptr;
+  int32_t* ids_dev = nullptr; fs_local_cfg* local_dev = nullptr;
+  // consolidation scratch
+  size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
+  unsigned long long* ckeys = nullptr; fs_consol_out* consol_dev = nullptr;
+  // diagnostics
+  int* flag_host = nullptr; int* flag_dev = nullptr;
+  uint64_t launches = 0; int last_cuda = 0;
+};
+
+namespace {
+
+#define FS_CUDA(ctx, expr)                                   \
+  do {                                                       \
+    cudaError_t e_ = (expr);                                 \
+    if (e_ != cudaSuccess) {                                 \
+      (ctx)->last_cuda = (int)e_;                            \
+      cudaGetLastError();                                    \
+      return e_ == cudaErrorMemoryAllocation ? FS_ERR_NOMEM : FS_ERR_CUDA; \
+    }                                                        \
+  } while (0)
+
+template <class T> int grow(fs_ctx* c, T*& p, size_t n_elems) {
+  if (p) { cudaFree(p); p = nullptr; }
+  if (n_elems == 0) n_elems = 1;
+  FS_CUDA(c, cudaMalloc((void**)&p, n_elems * sizeof(T)));
+  return FS_OK;
+}
+#define FS_TRY(x) do { int r_ = (x); if (r_ != FS_OK) return r_; } while (0)
+
+// sticky device-side range errors of earlier calls: report once, then clear
+int take_flags(fs_ctx* c) {
+  int any = 0;
+  for (int i = 0; i < FS_NFLAGS; ++i) { any |= ((volatile int*)c->flag_host)[i]; c->flag_host[i] = 0; }
+  return any ? FS_ERR_RANGE : FS_OK;
+}
+
+int check_kernel(fs_ctx* c) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { c->last_cuda = (int)e; return FS_ERR_CUDA; }
+  return FS_OK;
+}
+
+FsView view_of(const fs_ctx* c) {
+  FsView v;
+  v.d = FsDimsDev{c->d.M, c->d.F, c->d.S, c->d.B};
+  v.lat = c->lat; v.pow = c->pow; v.latT = c->latT; v.powT = c->powT; v.models = c->models;
+  v.K = c->K; v.states = c->states; v.ginfo = c->ginfo; v.gA = c->gA; v.flag = c->flag_dev;
+  return v;
+}
+
+// all SM splits of S share units into n positive parts, lexicographic, sigma_0 most significant
+void build_splits(int S, std::vector<uint32_t>& comp, uint32_t comp_n[FS_RMAX], int& stride) {
+  std::vector<uint32_t> lists[FS_RMAX];
+  for (int n = 1; n <= FS_RMAX; ++n) {
+    int sg[FS_RMAX] = {0, 0, 0, 0};
+    // odometer over (sigma_0..sigma_{n-1}) in lexicographic order, keep sum(sigma_i+1) == S
+    while (true) {
+      int tot = 0;
+      for (int i = 0; i < n; ++i) tot += sg[i] + 1;
+      if (tot == S) {
+        uint32_t pk = 0;
+        for (int i = 0; i < n; ++i) pk |= (uint32_t)sg[i] << (8 * i);
+        lists[n - 1].push_back(pk);
+      }
+      int i = n - 1;
+      while (i >= 0 && ++sg[i] >= S) { sg[i] = 0; --i; }
+      if (i < 0) break;
+    }
+    comp_n[n - 1] = (uint32_t)lists[n - 1].size();
+  }
+  stride = 1;
+  for (int n = 0; n < FS_RMAX; ++n) if ((int)comp_n[n] > stride) stride = (int)comp_n[n];
+  comp.assign((size_t)stride * FS_RMAX, 0u);
+  for (int n = 0; n < FS_RMAX; ++n)
+    for (size_t r = 0; r < lists[n].size(); ++r) comp[(size_t)n * stride + r] = lists[n][r];
+}
+
+cudaMemcpyKind in_kind(int space) { return space == FS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice; }
+
+}  // namespace
+
+extern "C" {
+
+int fs_create(fs_ctx** out, int cuda_device) {
+  if (!out) return FS_ERR_ARG;
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
+    cudaGetLastError();
+    return FS_ERR_CUDA;   // no CUDA device: there is no CPU fallback
+  }
+  fs_ctx* c = new (std::nothrow) fs_ctx();
+  if (!c) return FS_ERR_NOMEM;
+  c->dev = cuda_device;
+  if (cudaSetDevice(cuda_device) != cudaSuccess ||
+      cudaHostAlloc((void**)&c->flag_host, sizeof(int) * FS_NFLAGS, cudaHostAllocMapped) != cudaSuccess ||
+      cudaHostGetDevicePointer((void**)&c->flag_dev, c->flag_host, 0) != cudaSuccess ||
+      cudaMalloc((void**)&c->stats, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+    cudaGetLastError();
+    delete c;
+    return FS_ERR_CUDA;
+  }
+  std::memset(c->flag_host, 0, sizeof(int) * FS_NFLAGS);
+  cudaMemset(c->stats, 0, 2 * sizeof(unsigned long long));
+  fsk_local_smem_attr();
+  *out = c;
+  return FS_OK;
+}
+
+int fs_destroy(fs_ctx* c) {
+  if (!c) return FS_ERR_ARG;
+  cudaSetDevice(c->dev);
+  cudaDeviceSynchronize();
+  void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
+                  c->ginfo, c->gA, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
+                  c->reqs_dev, c->place_dev, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
+                  c->agg, c->ckeys, c->consol_dev};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  if (c->flag_host) cudaFreeHost(c->flag_host);
+  cudaGetLastError();
+  delete c;
+  return FS_OK;
+}
+
+int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const float* pow,
+                     const float* freq_mhz, const fs_model_info* models, const fs_params* params,
+                     int space, void* cuda_stream) {
+  if (!c || !dims || !lat || !pow || !freq_mhz || !models || !params) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (dims->M < 1 || dims->M > FS_MAX_M || dims->F < 1 || dims->F > FS_MAX_F || dims->S < 1 ||
+      dims->S > FS_MAX_S || dims->B < 1 || dims->B > FS_MAX_B)
+    return FS_ERR_SHAPE;
+  if (params->delta_pct < 0 || params->delta_pct > 100) return FS_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  c->have_prof = false; c->have_state = false; c->K = 0; c->consol_cap = 0;
+  const size_t n = (size_t)dims->M * 2 * dims->F * dims->S * dims->B;
+  if (n > c->table_cap) {
+    FS_TRY(grow(c, c->lat, n)); FS_TRY(grow(c, c->pow, n));
+    FS_TRY(grow(c, c->latT, n)); FS_TRY(grow(c, c->powT, n));
+    c->table_cap = n;
+  }
+  if (dims->M > c->m_cap) { FS_TRY(grow(c, c->models, (size_t)dims->M)); c->m_cap = dims->M; }
+  if (dims->F > c->f_cap) { FS_TRY(grow(c, c->freq, (size_t)dims->F)); c->f_cap = dims->F; }
+  const cudaMemcpyKind kind = in_kind(space);
+  FS_CUDA(c, cudaMemcpyAsync(c->lat, lat, n * sizeof(float), kind, st));
+  FS_CUDA(c, cudaMemcpyAsync(c->pow, pow, n * sizeof(float), kind, st));
+  FS_CUDA(c, cudaMemcpyAsync(c->freq, freq_mhz, dims->F * sizeof(float), kind, st));
+  FS_CUDA(c, cudaMemcpyAsync(c->models, models, dims->M * sizeof(fs_model_info), kind, st));
+  c->d = *dims; c->prm = *params;
+  // SM-split enumeration table of fs_local_config (index bookkeeping only)
+  std::vector<uint32_t> comp; uint32_t comp_n[FS_RMAX]; int stride = 1;
+  build_splits(dims->S, comp, comp_n, stride);
+  if (comp.size() > c->comp_cap) { FS_TRY(grow(c, c->comp, comp.size())); c->comp_cap = comp.size(); }
+  if (!c->comp_n) FS_TRY(grow(c, c->comp_n, (size_t)FS_RMAX));
+  // synchronous copies: `comp` is a local that dies at return
+  FS_CUDA(c, cudaMemcpyAsync(c->comp, comp.data(), comp.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+  FS_CUDA(c, cudaMemcpyAsync(c->comp_n, comp_n, sizeof(comp_n), cudaMemcpyHostToDevice, st));
+  FS_CUDA(c, cudaStreamSynchronize(st));
+  c->ns_stride = stride;
+  c->launches += fsk_build_planes(c->lat, c->pow, c->latT, c->powT,
+                                  FsDimsDev{dims->M, dims->F, dims->S, dims->B}, c->flag_dev, st);
+  FS_TRY(check_kernel(c));
+  c->have_prof = true;
+  return pending;
+}
+
+int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space, void* cuda_stream) {
+  if (!c || K < 0 || (K > 0 && !states)) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof) return FS_ERR_STATE;
+  if ((unsigned long long)K * c->d.S * c->d.F >= 0xFFFFFFFFull) return FS_ERR_SHAPE;  // flat is 32-bit
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (K > c->k_cap) {
+    FS_TRY(grow(c, c->states, (size_t)K)); FS_TRY(grow(c, c->ginfo, (size_t)K));
+    FS_TRY(grow(c, c->warm_item, (size_t)K * FS_RMAX));
+    c->k_cap = K; c->consol_cap = 0;
+  }
+  const size_t na = (size_t)K * FS_NVAR * c->d.F;
+  if (na > c->gA_cap) { FS_TRY(grow(c, c->gA, na)); c->gA_cap = na; }
+  if (c->d.M > c->warm_m_cap) {
+    FS_TRY(grow(c, c->warm_off, (size_t)c->d.M + 1)); FS_TRY(grow(c, c->warm_cursor, (size_t)c->d.M));
+    c->warm_m_cap = c->d.M;
+  }
+  c->K = K; c->have_state = false;
+  if (K > 0) {
+    FS_CUDA(c, cudaMemcpyAsync(c->states, states, (size_t)K * sizeof(fs_gpu_state), in_kind(space), st));
+    FsView v = view_of(c);
+    c->launches += fsk_summary(v, c->ginfo, c->gA, st);
+    c->launches += fsk_build_warm_lists(v, c->warm_off, c->warm_cursor, c->warm_item, st);
+    FS_TRY(check_kernel(c));
+  }
+  c->have_state = true;
+  return pending;
+}
+
+int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out, int space,
+                   void* cuda_stream) {
+  if (!c || R < 0 || (R > 0 && (!reqs || !out))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (R == 0) return pending;
+  if (R > c->r_cap) {
+    FS_TRY(grow(c, c->keys, (size_t)R)); FS_TRY(grow(c, c->reqs_dev, (size_t)R));
+    FS_TRY(grow(c, c->place_dev, (size_t)R));
+    c->r_cap = R;
+  }
+  const fs_request* d_reqs = reqs; fs_placement* d_out = out;
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
+    d_reqs = c->reqs_dev; d_out = c->place_dev;
+  }
+  FsPlaceScratch sc{c->keys, c->stats, c->warm_off, c->warm_item};
+  c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,
+                    int space, void* cuda_stream) {
+  if (!c || n < 0 || (n > 0 && !out) || (flags & ~3u)) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
+  if (!gpu_ids && n > c->K) return FS_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (n == 0) return pending;
+  const size_t rows = (size_t)c->d.F * c->d.S;
+  const size_t need = (size_t)n * FS_RMAX * 2 * rows;
+  if (need > c->local_cap) { FS_TRY(grow(c, c->G, need)); FS_TRY(grow(c, c->Bst, need)); c->local_cap = need; }
+  if (n > c->n_cap) { FS_TRY(grow(c, c->ids_dev, (size_t)n)); FS_TRY(grow(c, c->local_dev, (size_t)n)); c->n_cap = n; }
+  const int32_t* d_ids = gpu_ids; fs_local_cfg* d_out = out;
+  if (space == FS_HOST) {
+    if (gpu_ids) {
+      FS_CUDA(c, cudaMemcpyAsync(c->ids_dev, gpu_ids, (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+      d_ids = c->ids_dev;
+    }
+    d_out = c->local_dev;
+  }
+  FsLocalScratch sc{c->G, c->Bst, c->comp, c->comp_n, c->ns_stride};
+  c->launches += fsk_local(view_of(c), n, d_ids, flags, d_out, sc, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(out, c->local_dev, (size_t)n * sizeof(fs_local_cfg), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) {
+  if (!c || (space != FS_HOST && space != FS_DEVICE)) return FS_ERR_ARG;
+  if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
+  if (c->K > 0 && !out) return FS_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (c->K == 0) return pending;
+  const size_t kf = (size_t)c->K * c->d.F;
+  if (kf > c->consol_cap) {
+    FS_TRY(grow(c, c->need, kf)); FS_TRY(grow(c, c->E, kf)); FS_TRY(grow(c, c->agg, (size_t)c->K));
+    FS_TRY(grow(c, c->ckeys, (size_t)c->K)); FS_TRY(grow(c, c->consol_dev, (size_t)c->K));
+    c->consol_cap = kf;
+  }
+  fs_consol_out* d_out = space == FS_HOST ? c->consol_dev : out;
+  FsConsolScratch sc{c->need, c->E, c->agg, c->ckeys};
+  c->launches += fsk_consolidate(view_of(c), c->prm, d_out, sc, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(out, c->consol_dev, (size_t)c->K * sizeof(fs_consol_out), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+const char* fs_strerror(int code) {
+  switch (code) {
+    case FS_OK: return "ok";
+    case FS_ERR_ARG: return "bad argument";
+    case FS_ERR_SHAPE: return "dims outside the supported range";
+    case FS_ERR_STATE: return "profiles or GPU state not loaded";
+    case FS_ERR_RANGE: return "index or value out of range in device data";
+    case FS_ERR_CUDA: return "CUDA runtime error";
+    case FS_ERR_NOMEM: return "out of memory";
+    default: return "unknown";
+  }
+}
+
+int fs_last_cuda_error(const fs_ctx* c) { return c ? c->last_cuda : 0; }
+uint64_t fs_launch_count(const fs_ctx* c) { return c ? c->launches : 0; }
+
+int fs_last_place_stats(fs_ctx* c, uint64_t* pairs, uint64_t* candidates) {
+  if (!c || !pairs || !candidates) return FS_ERR_ARG;
+  unsigned long long h[2] = {0, 0};
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  FS_CUDA(c, cudaMemcpy(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost));
+  *pairs = h[0]; *candidates = h[1];
+  return FS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,133 @@
+// fs_common.cuh — device-side building blocks of libfestina_eval (sm_100a).
+//
+// The product path.  Shares no code with oracle/ (own structs via include/festina_eval.h, own
+// arithmetic).  Every fl(.) of DESIGN.md "Numerics" is ONE binary32 round-to-nearest-even
+// operation: products and sums go through __fmul_rn/__fadd_rn/__fsub_rn, which nvcc never
+// contracts into FMA.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/festina_eval.h"
+
+#define FS_INF __int_as_float(0x7f800000)
+#define FS_NEED_INF 255          // "no feasible share" marker of the consolidation need[] bytes
+#define FS_NVAR (FS_RMAX + 1)    // co-resident energy variants: 0 = as is, 1+j = bump tenant j
+#define FS_KEY_NONE 0xFFFFFFFFFFFFFFFFull
+
+// Sticky range-error words: int[4] in mapped (zero-copy) host memory, one word per source.
+// Kernels only ever store 1 (plain store; no PCIe atomics needed); the next API call reads
+// and clears them on the host.
+enum { FS_FLAG_TABLE = 0, FS_FLAG_STATE = 1, FS_FLAG_REQUEST = 2, FS_FLAG_ARG = 3, FS_NFLAGS = 4 };
+__device__ __forceinline__ void fs_raise(int* flag, int which) {
+  *((volatile int*)flag + which) = 1;
+}
+
+// Per-GPU summary written by the summary kernel (fs_set_gpu_state) and read by placement.
+// 48 bytes, 16-byte aligned so that one GPU is three 128-bit loads.
+struct __align__(16) FsGpuInfo {
+  float t_avail_ms;     // T_avail
+  float mem_free_mb;    // free memory
+  float e_cur;          // Ecur: slot-order energy sum at F_curr, no bump (R:s4)
+  int32_t n_res;        // 0 = inactive or invalid record
+  int32_t sm_free;      // S - sum(sigma_i+1)
+  int32_t f_floor;      // lowest phi at which every co-resident is feasible (-1: none)
+  int16_t model[FS_RMAX];   // tenant models (-1 beyond n_res)
+  int16_t br1[FS_RMAX];     // decode bucket a joining request sees: beta_1+1 if q_1>0 else 0;
+                            // -1 = bucket past the table (candidate dropped)
+  uint32_t _pad[2];
+};
+static_assert(sizeof(FsGpuInfo) == 48, "FsGpuInfo layout");
+
+struct FsDimsDev { int M, F, S, B; };
+
+// ---- table addressing --------------------------------------------------------------------
+// logical layout  [M][2][F][S][B]  (beta fastest): the batch search of fs_local_config
+__device__ __forceinline__ size_t fs_idx(const FsDimsDev& d, int m, int p, int f, int s, int b) {
+  return ((((size_t)m * 2 + p) * d.F + f) * d.S + s) * d.B + b;
+}
+// plane layout    [M][2][B][S][F]  (phi fastest): one (sigma,phi) plane per (model,phase,beta)
+__device__ __forceinline__ size_t fs_plane(const FsDimsDev& d, int m, int p, int b) {
+  return (((size_t)m * 2 + p) * d.B + b) * (size_t)d.S * d.F;
+}
+
+// ---- arithmetic ---------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t fs_ceil_div(uint32_t q, uint32_t n) { return (q + n - 1u) / n; }
+
+// 64-bit argmin key: high word = order-preserving transform of the fp32 value, low word = flat
+// index (BASELINE north_star; SURVEY §8(c) "Numerics").  -0 is canonicalised to +0 first.
+__device__ __forceinline__ uint32_t fs_orderable(float v) {
+  if (v == 0.0f) v = 0.0f;
+  uint32_t u = __float_as_uint(v);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float fs_unorderable(uint32_t o) {
+  uint32_t u = (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o;
+  return __uint_as_float(u);
+}
+__device__ __forceinline__ unsigned long long fs_make_key(float v, uint32_t flat) {
+  return ((unsigned long long)fs_orderable(v) << 32) | flat;
+}
+__device__ __forceinline__ unsigned long long fs_warp_min_key(unsigned long long k) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    unsigned long long other = __shfl_xor_sync(0xffffffffu, k, o);
+    k = other < k ? other : k;
+  }
+  return k;
+}
+
+// The shared slot rule (Eq. 1; R:s11), given the two table values.
+//   rounds = ceil(q/(beta+1)); t = fl(rounds*lat); e = fl(t*pow)
+//   prefill (p==0): ok = fl(wait+t) <= slo;   decode: ok = lat <= slo
+struct FsSlot { bool ok; float t, e; };
+__device__ __forceinline__ FsSlot fs_slot(int p, float lat, float pw, uint32_t rounds, float wait,
+                                          float slo) {
+  FsSlot s;
+  s.t = __fmul_rn(__uint2float_rn(rounds), lat);
+  s.ok = (p == 0) ? (__fadd_rn(wait, s.t) <= slo) : (lat <= slo);
+  s.e = __fmul_rn(s.t, pw);
+  return s;
+}
+
+// ---- mbarrier + 1-D TMA bulk copy (global -> shared), sm_90+ PTX ---------------------------
+__device__ __forceinline__ uint32_t fs_smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void fs_mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(fs_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void fs_mbar_fence_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fs_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fs_smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void fs_mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(fs_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fs_mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(fs_smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// bytes must be a multiple of 16; src and dst 16-byte aligned
+__device__ __forceinline__ void fs_tma_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes,
+                                               uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+          "r"(fs_smem_u32(smem_dst)),
+      "l"(gsrc), "r"(bytes), "r"(fs_smem_u32(bar))
+      : "memory");
+}

@@ -1,0 +1,164 @@
+// fs_consol.cu — fs_consolidate: drain-one-source scoring over all GPU pairs (§3.5,
+// R:s17-s20).  Per tenant and frequency the minimum feasible share (P:252 rule (1));
+// 5 % safety margin on SMs and memory; idle power vs migration energy.
+//
+//   need_g[phi] = sum_i (sigma_i(phi)+1),  E_g[phi] = slot-order sum of e_i at those shares
+//   C*_g   = min_phi { E_g[phi] : need_g[phi] <= S_eff }
+//   C*_ab  = min_phi { fl(E_b[phi]+E_a[phi]) : need_a[phi]+need_b[phi] <= S_eff }  (lowest phi)
+//   score(a->b) = fl(C*_ab - C*_b);   dst(a) = argmin_b (score, b)  as one 64-bit key
+#include "fs_kernels.h"
+
+namespace {
+
+constexpr int TA = 8;          // sources per block of the pair kernel
+constexpr int PAIR_THREADS = 256;
+
+// ---- a9: per GPU, lanes over phi ------------------------------------------------------------
+__global__ void __launch_bounds__(128) consol_agg_kernel(FsView v, int S_eff,
+                                                        uint8_t* __restrict__ need,
+                                                        float* __restrict__ E,
+                                                        float4* __restrict__ agg) {
+  const int lane = threadIdx.x & 31;
+  const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (g >= v.K) return;
+  const FsDimsDev d = v.d;
+  const int n = v.ginfo[g].n_res;
+  const fs_gpu_state& st = v.states[g];
+  unsigned long long key = FS_KEY_NONE;
+  for (int phi = lane; phi < d.F; phi += 32) {
+    int nd = 0; float e = 0.0f; bool all = n >= 1;
+    for (int i = 0; i < n && all; ++i) {
+      int smin = -1; float ei = FS_INF;
+      for (int sg = 0; sg < d.S; ++sg) {
+        const TenantE te = tenant_eval(v, st.t[i], phi, sg, false);
+        if (te.ok) { smin = sg; ei = te.e; break; }
+      }
+      if (smin < 0) { all = false; break; }
+      nd += smin + 1;
+      e = (i == 0) ? ei : __fadd_rn(e, ei);
+    }
+    need[(size_t)phi * v.K + g] = all ? (uint8_t)nd : (uint8_t)FS_NEED_INF;
+    E[(size_t)phi * v.K + g] = all ? e : FS_INF;
+    if (all && nd <= S_eff && e < FS_INF) {
+      const unsigned long long kk = fs_make_key(e, (uint32_t)phi);
+      key = kk < key ? kk : key;
+    }
+  }
+  key = fs_warp_min_key(key);
+  if (lane == 0) {
+    float mem = 0.0f, mig = 0.0f;
+    for (int i = 0; i < n; ++i) {
+      mem = (i == 0) ? st.t[i].mem_used_mb : __fadd_rn(mem, st.t[i].mem_used_mb);
+      const float mg = v.models[st.t[i].model].mig_mj;
+      mig = (i == 0) ? mg : __fadd_rn(mig, mg);
+    }
+    const float cstar = key == FS_KEY_NONE ? FS_INF : fs_unorderable((uint32_t)(key >> 32));
+    agg[g] = make_float4(mem, cstar, mig, __int_as_float(n));
+  }
+}
+
+// ---- a10: pair scoring; one block = TA sources x all destinations ----------------------------
+__global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
+    FsView v, int S_eff, float M_eff, const uint8_t* __restrict__ need, const float* __restrict__ E,
+    const float4* __restrict__ agg, unsigned long long* __restrict__ keys) {
+  extern __shared__ unsigned char smem_raw[];
+  const int F = v.d.F, K = v.K;
+  float* sE = reinterpret_cast<float*>(smem_raw);                  // [F][TA]
+  int* sN = reinterpret_cast<int*>(smem_raw + sizeof(float) * F * TA);   // [F][TA]
+  __shared__ unsigned long long sred[TA][PAIR_THREADS / 32];
+  const int a0 = blockIdx.x * TA;
+  for (int x = threadIdx.x; x < F * TA; x += blockDim.x) {
+    const int phi = x / TA, a = a0 + x % TA;
+    sE[x] = a < K ? E[(size_t)phi * K + a] : FS_INF;
+    sN[x] = a < K ? need[(size_t)phi * K + a] : FS_NEED_INF;
+  }
+  __syncthreads();
+  float4 ag[TA];
+#pragma unroll
+  for (int t = 0; t < TA; ++t) ag[t] = a0 + t < K ? agg[a0 + t] : make_float4(0.f, FS_INF, 0.f, 0.f);
+  unsigned long long best[TA];
+#pragma unroll
+  for (int t = 0; t < TA; ++t) best[t] = FS_KEY_NONE;
+  for (int b = threadIdx.x; b < K; b += blockDim.x) {
+    float cab[TA];
+#pragma unroll
+    for (int t = 0; t < TA; ++t) cab[t] = FS_INF;
+    for (int phi = 0; phi < F; ++phi) {
+      const float eb = E[(size_t)phi * K + b];
+      const int nb = need[(size_t)phi * K + b];
+#pragma unroll
+      for (int t = 0; t < TA; ++t) {
+        const float e = __fadd_rn(eb, sE[phi * TA + t]);
+        if (sN[phi * TA + t] + nb <= S_eff) cab[t] = fminf(cab[t], e);   // INF never wins
+      }
+    }
+    const float4 gb = agg[b];
+    const int n_b = __float_as_int(gb.w);
+#pragma unroll
+    for (int t = 0; t < TA; ++t) {
+      const int a = a0 + t, n_a = __float_as_int(ag[t].w);
+      const bool ok = a < K && a != b && n_a >= 1 && n_b >= 1 && n_a + n_b <= FS_RMAX &&
+                      (__fadd_rn(ag[t].x, gb.x) <= M_eff) && gb.y < FS_INF && cab[t] < FS_INF;
+      if (ok) {
+        const unsigned long long kk = fs_make_key(__fsub_rn(cab[t], gb.y), (uint32_t)b);
+        best[t] = kk < best[t] ? kk : best[t];
+      }
+    }
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int t = 0; t < TA; ++t) {
+    const unsigned long long kk = fs_warp_min_key(best[t]);
+    if (lane == 0) sred[t][warp] = kk;
+  }
+  __syncthreads();
+  if (threadIdx.x < TA && a0 + threadIdx.x < K) {
+    unsigned long long kk = FS_KEY_NONE;
+    for (int w = 0; w < PAIR_THREADS / 32; ++w) kk = sred[threadIdx.x][w] < kk ? sred[threadIdx.x][w] : kk;
+    keys[a0 + threadIdx.x] = kk;
+  }
+}
+
+// ---- decode: dst, the merged GPU's frequency, score and net saving ---------------------------
+__global__ void consol_decode_kernel(FsView v, int S_eff, fs_params prm,
+                                     const uint8_t* __restrict__ need, const float* __restrict__ E,
+                                     const float4* __restrict__ agg,
+                                     const unsigned long long* __restrict__ keys,
+                                     fs_consol_out* __restrict__ out) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= v.K) return;
+  fs_consol_out o; o.dst = -1; o.phi = -1; o.score_mj = FS_INF; o.saving_mj = -FS_INF;
+  const unsigned long long key = keys[a];
+  if (key != FS_KEY_NONE) {
+    const int b = (int)(uint32_t)key;
+    float cab = FS_INF; int phis = -1;
+    for (int phi = 0; phi < v.d.F; ++phi) {
+      if ((int)need[(size_t)phi * v.K + a] + (int)need[(size_t)phi * v.K + b] > S_eff) continue;
+      const float e = __fadd_rn(E[(size_t)phi * v.K + b], E[(size_t)phi * v.K + a]);
+      if (e < cab) { cab = e; phis = phi; }            // strict: lowest phi on ties
+    }
+    const float4 ga = agg[a];
+    o.dst = b; o.phi = phis; o.score_mj = fs_unorderable((uint32_t)(key >> 32));
+    // saved idle energy over the horizon + the source's own optimum - what the destination
+    // pays extra - migration energy (R:s18)
+    o.saving_mj = __fsub_rn(__fadd_rn(__fmul_rn(prm.p_idle_w, prm.horizon_ms), ga.y),
+                            __fadd_rn(o.score_mj, ga.z));
+  }
+  out[a] = o;
+}
+
+}  // namespace
+
+int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
+                    const FsConsolScratch& sc, cudaStream_t st) {
+  if (v.K <= 0) return 0;
+  const int S_eff = (v.d.S * (100 - prm.delta_pct)) / 100;
+  const float M_eff = (prm.mem_cap_mb * (float)(100 - prm.delta_pct)) / 100.0f;
+  consol_agg_kernel<<<(v.K + 3) / 4, 128, 0, st>>>(v, S_eff, sc.need, sc.E, sc.agg);
+  const size_t smem = (sizeof(float) + sizeof(int)) * v.d.F * TA;
+  consol_pair_kernel<<<(v.K + TA - 1) / TA, PAIR_THREADS, smem, st>>>(v, S_eff, M_eff, sc.need,
+                                                                    sc.E, sc.agg, sc.keys);
+  consol_decode_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, S_eff, prm, sc.need, sc.E, sc.agg,
+                                                          sc.keys, out);
+  return 3;
+}

@@ -1,0 +1,91 @@
+// fs_kernels.h — host-side launchers of the CUDA kernels behind the C ABI (internal).
+// Each launcher enqueues on `st`, returns the number of kernels it launched, and never
+// synchronises.  Pointers are device pointers unless stated.
+#pragma once
+
+#include "fs_common.cuh"
+
+// device-resident view of everything fs_load_profiles / fs_set_gpu_state own
+struct FsView {
+  FsDimsDev d;
+  const float* lat;    // [M][2][F][S][B]
+  const float* pow;
+  const float* latT;   // [M][2][B][S][F]
+  const float* powT;
+  const fs_model_info* models;
+  int K;
+  const fs_gpu_state* states;
+  const FsGpuInfo* ginfo;   // [K]
+  const float* gA;          // [K][FS_NVAR][F]  co-resident energy per variant, INF = infeasible
+  int* flag;                // sticky range-error flag (mapped host memory)
+};
+
+// fs_tables.cu — validate (finite, > 0) and build the plane layout
+int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, FsDimsDev d,
+                     int* flag, cudaStream_t st);
+
+// fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st);
+
+// fs_place.cu — placement scoring + 64-bit-key argmin + decode
+struct FsPlaceScratch {
+  unsigned long long* keys;        // [R]
+  unsigned long long* stats;       // [2]: eligible pairs, candidates
+  // bucketing of GPUs by model (built by fs_set_gpu_state): warm lists
+  const int32_t* warm_off;         // [M+1]
+  const uint32_t* warm_item;       // [sum n_res]: k*4 + j
+};
+int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
+              const FsPlaceScratch& sc, cudaStream_t st);
+int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,
+                         uint32_t* warm_item /*[4K]*/, cudaStream_t st);
+
+// fs_local.cu — per-slot batch search + SM-split search
+struct FsLocalScratch {
+  float* G;               // [n][RMAX*2][F*S]  slot cost g_{i,p}[phi][sigma]
+  uint8_t* B;             // [n][RMAX*2][F*S]  best batch bucket beta* per slot row
+  const uint32_t* comp;   // [RMAX][ns_stride] SM splits in lexicographic order, sigma_i in byte i
+  const uint32_t* comp_n; // [RMAX] number of splits NS = C(S-1, n_res-1)
+  int ns_stride;
+};
+int fsk_local_smem_attr();   // raise the split kernel's dynamic shared memory limit (once)
+int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,
+              const FsLocalScratch& sc, cudaStream_t st);
+
+// fs_consol.cu — per-tenant minimum share, per-GPU aggregates, pair scoring
+struct FsConsolScratch {
+  uint8_t* need;     // [F][K]  sum of minimum shares per frequency, FS_NEED_INF = none
+  float* E;          // [F][K]  slot-order energy at those shares
+  float4* agg;       // [K]     {mem, C*, mig, n_res as float bits}
+  unsigned long long* keys;  // [K] per-source argmin key (score, dst)
+};
+int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
+                    const FsConsolScratch& sc, cudaStream_t st);
+
+#ifdef __CUDACC__
+// One co-resident ("tenant") at frequency phi with share sigma, wait = 0 because its slo is the
+// REMAINING slack (R:s12).  bump = one more sequence joins its decode batch: the decode bucket
+// moves to beta_1+1 when its decode queue is non-empty; past the table -> not ok, e = INF.
+// e = fl(e_prefill + e_decode) (Eq. 1); ok = both deadlines hold.
+struct TenantE { bool ok; float e; };
+__device__ __forceinline__ TenantE tenant_eval(const FsView& v, const fs_tenant& t, int phi,
+                                               int sigma, bool bump) {
+  const FsDimsDev& d = v.d;
+  const int b1 = t.beta[1] + ((bump && t.q[1] > 0) ? 1 : 0);
+  TenantE r;
+  if (b1 >= d.B) { r.ok = false; r.e = FS_INF; return r; }
+  bool ok = true; float e0 = 0.0f, e1 = 0.0f;
+  if (t.q[0] > 0) {
+    const size_t i = fs_plane(d, t.model, 0, t.beta[0]) + (size_t)sigma * d.F + phi;
+    FsSlot s = fs_slot(0, v.latT[i], v.powT[i], fs_ceil_div(t.q[0], t.beta[0] + 1u), 0.0f, t.slo_ms[0]);
+    ok = ok && s.ok; e0 = s.e;
+  }
+  if (t.q[1] > 0) {
+    const size_t i = fs_plane(d, t.model, 1, b1) + (size_t)sigma * d.F + phi;
+    FsSlot s = fs_slot(1, v.latT[i], v.powT[i], fs_ceil_div(t.q[1], b1 + 1u), 0.0f, t.slo_ms[1]);
+    ok = ok && s.ok; e1 = s.e;
+  }
+  r.ok = ok; r.e = __fadd_rn(e0, e1);
+  return r;
+}
+#endif

@@ -1,0 +1,153 @@
+// fs_summary.cu — per-GPU co-resident summary, run by fs_set_gpu_state.
+//
+// For every GPU k and every frequency phi it evaluates each co-resident ("tenant") with the
+// shared slot rule and reduces over the tenants of the GPU (the segment):
+//   ok_co[k][v][phi] = AND_i ok_i(phi; bump = (i == v-1))      -> f_floor = lowest phi with ok
+//   A[k][v][phi]     = ((e_0 + e_1) + ...) in slot order        (INF where !ok_co)
+// for the variants v = 0 ("as is") and v = 1+j ("one more sequence joins tenant j's decode
+// batch").  The shared frequency forces one operating point per device:
+// f_floor is the max over co-residents of each one's lowest feasible frequency when feasibility
+// is monotone, and is evaluated pointwise so it needs no monotonicity (R:s3).
+// Also Ecur[k] (energy now, at F_curr), free SMs, and the decode bucket a joining request sees.
+#include "fs_kernels.h"
+
+namespace {
+
+__device__ __forceinline__ bool state_valid(const fs_gpu_state& g, const FsDimsDev& d) {
+  if (g.n_res < 0 || g.n_res > FS_RMAX) return false;
+  if (g.n_res == 0) return true;
+  if (g.f_cur < 0 || g.f_cur >= d.F) return false;
+  int used = 0;
+  for (int i = 0; i < g.n_res; ++i) {
+    const fs_tenant& t = g.t[i];
+    if (t.model < 0 || t.model >= d.M || t.sigma >= d.S || t.beta[0] >= d.B || t.beta[1] >= d.B ||
+        t.q[0] >= (1u << 24) || t.q[1] >= (1u << 24))
+      return false;
+    used += t.sigma + 1;
+  }
+  return used <= d.S;
+}
+
+// one warp per GPU, lanes over phi
+__global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __restrict__ ginfo,
+                                                     float* __restrict__ gA) {
+  const int lane = threadIdx.x & 31;
+  const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (k >= v.K) return;
+  const FsDimsDev d = v.d;
+  const fs_gpu_state g = v.states[k];
+  const bool valid = state_valid(g, d);
+  const int n = valid ? g.n_res : 0;
+  float* A = gA + (size_t)k * FS_NVAR * d.F;
+  int f_floor = -1;
+  for (int base = 0; base < d.F; base += 32) {
+    const int phi = base + lane;
+    bool ok0 = false;
+    if (phi < d.F) {
+      float e_plain[FS_RMAX], e_bump[FS_RMAX]; bool ok_plain[FS_RMAX], ok_bump[FS_RMAX];
+#pragma unroll
+      for (int i = 0; i < FS_RMAX; ++i) {
+        if (i < n) {
+          TenantE a = tenant_eval(v, g.t[i], phi, g.t[i].sigma, false);
+          e_plain[i] = a.e; ok_plain[i] = a.ok;
+          if (g.t[i].q[1] > 0) {
+            TenantE b = tenant_eval(v, g.t[i], phi, g.t[i].sigma, true);
+            e_bump[i] = b.e; ok_bump[i] = b.ok;
+          } else { e_bump[i] = a.e; ok_bump[i] = a.ok; }
+        } else { e_plain[i] = e_bump[i] = 0.0f; ok_plain[i] = ok_bump[i] = true; }
+      }
+#pragma unroll
+      for (int var = 0; var < FS_NVAR; ++var) {
+        float acc = FS_INF; bool ok = (n >= 1) && (var <= n);
+        if (ok) {
+#pragma unroll
+          for (int i = 0; i < FS_RMAX; ++i) {
+            if (i < n) {
+              const bool bump = (i == var - 1);
+              const float e = bump ? e_bump[i] : e_plain[i];
+              ok = ok && (bump ? ok_bump[i] : ok_plain[i]);
+              acc = (i == 0) ? e : __fadd_rn(acc, e);   // slot-order sum
+            }
+          }
+        }
+        A[var * d.F + phi] = ok ? acc : FS_INF;
+        if (var == 0) ok0 = ok;
+      }
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, ok0);
+    if (f_floor < 0 && m) f_floor = base + __ffs(m) - 1;
+  }
+  if (lane == 0) {
+    FsGpuInfo gi;
+    gi.t_avail_ms = g.t_avail_ms; gi.mem_free_mb = g.mem_free_mb;
+    gi.n_res = n; gi.f_floor = f_floor; gi._pad[0] = gi._pad[1] = 0;
+    int used = 0; float ecur = 0.0f;
+    for (int i = 0; i < FS_RMAX; ++i) {
+      if (i < n) {
+        const fs_tenant& t = g.t[i];
+        used += t.sigma + 1;
+        gi.model[i] = t.model;
+        const int b = (t.q[1] > 0) ? t.beta[1] + 1 : 0;
+        gi.br1[i] = (int16_t)(b >= d.B ? -1 : b);
+        TenantE a = tenant_eval(v, t, g.f_cur, t.sigma, false);
+        ecur = (i == 0) ? a.e : __fadd_rn(ecur, a.e);
+      } else { gi.model[i] = -1; gi.br1[i] = -1; }
+    }
+    gi.e_cur = ecur; gi.sm_free = n ? d.S - used : 0;
+    ginfo[k] = gi;
+    if (!valid) fs_raise(v.flag, FS_FLAG_STATE);
+  }
+}
+
+// ---- warm lists: for every model, the (GPU, tenant slot) pairs that host it -----------------
+__global__ void warm_count_kernel(FsView v, int32_t* __restrict__ cnt /*[M+1], zeroed*/) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= v.K) return;
+  const FsGpuInfo gi = v.ginfo[k];
+  for (int i = 0; i < gi.n_res; ++i) {
+    bool first = true;   // only the LOWEST slot with this model is the join target
+    for (int j = 0; j < i; ++j) first = first && (gi.model[j] != gi.model[i]);
+    if (first) atomicAdd(&cnt[gi.model[i] + 1], 1);
+  }
+}
+__global__ void warm_scan_kernel(int32_t* off /*[M+1]*/, int32_t* cursor /*[M]*/, int M) {
+  // single thread: M <= 32767, run once per fs_set_gpu_state
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    int acc = 0; off[0] = 0;
+    for (int m = 0; m < M; ++m) { acc += off[m + 1]; off[m + 1] = acc; cursor[m] = 0; }
+  }
+}
+__global__ void warm_fill_kernel(FsView v, const int32_t* __restrict__ off,
+                                 int32_t* __restrict__ cursor, uint32_t* __restrict__ item) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= v.K) return;
+  const FsGpuInfo gi = v.ginfo[k];
+  for (int i = 0; i < gi.n_res; ++i) {
+    bool first = true;
+    for (int j = 0; j < i; ++j) first = first && (gi.model[j] != gi.model[i]);
+    if (first) {
+      const int m = gi.model[i];
+      const int pos = atomicAdd(&cursor[m], 1);
+      item[off[m] + pos] = (uint32_t)k * 4u + (uint32_t)i;
+    }
+  }
+}
+
+}  // namespace
+
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st) {
+  if (v.K <= 0) return 0;
+  const int wpb = 4;
+  summary_kernel<<<(v.K + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA);
+  return 1;
+}
+
+int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
+                         uint32_t* warm_item, cudaStream_t st) {
+  if (v.K <= 0) return 0;
+  cudaMemsetAsync(warm_off, 0, sizeof(int32_t) * (v.d.M + 1), st);
+  warm_count_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, warm_off);
+  warm_scan_kernel<<<1, 32, 0, st>>>(warm_off, warm_cursor, v.d.M);
+  warm_fill_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, warm_off, warm_cursor, warm_item);
+  return 3;
+}

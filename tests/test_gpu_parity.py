@@ -1,0 +1,230 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the
+same seeded inputs.  Everything here needs a B200: `-m gpu`."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import fs_compare as cmp
+import fs_util as U
+import oracle
+from paper_2606_30391_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+ALL_FLAGS = [0, 1, 2, 3]
+
+
+@pytest.fixture(scope="module")
+def ctx(fs):
+    c = fs.Festina(0)
+    yield c
+    c.close()
+
+
+def _oracle_place(cl, reqs=None, nthreads=8):
+    return oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests if reqs is None else reqs, nthreads)
+
+
+def _oracle_local(cl, flags, ids=None, nthreads=8):
+    return oracle.local_config(cl.lat, cl.pow, cl.states, flags, ids, nthreads)
+
+
+def _oracle_consol(cl, nthreads=8):
+    p = cl.params
+    return oracle.consolidate(cl.lat, cl.pow, cl.models, cl.states, p.p_idle_w, p.horizon_ms,
+                              p.mem_cap_mb, p.delta_pct, nthreads)
+
+
+def _check_all(ctx, cl, local=True, consol=True):
+    ctx.load_cluster(cl)
+    if cl.R:
+        got = ctx.place_batch(cl.requests)
+        cmp.assert_placement_equal(got, _oracle_place(cl))
+    if local:
+        for fl in ALL_FLAGS:
+            cmp.assert_local_equal(ctx.local_config(fl), _oracle_local(cl, fl))
+    if consol:
+        cmp.assert_consol_equal(ctx.consolidate(), _oracle_consol(cl))
+
+
+# ---- config 0 and ragged small clusters: everything, element by element ----------------------
+def test_tiny_config_all_entry_points(ctx):
+    cl = synth.make_cluster("tiny")
+    _check_all(ctx, cl)
+    got = ctx.place_batch(cl.requests)
+    assert (got["gpu"] >= 0).sum() > 200          # not a degenerate all-infeasible case
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_ragged_dims(ctx, seed):
+    """Dims that are not multiples of the warp / tile sizes, several tenants, ragged tails."""
+    st = synth.Stream(seed, "dims")
+    K = int(st.randint(1, 1, 70)[0]); M = int(st.randint(1, 1, 9)[0])
+    F = int(st.randint(1, 1, 70)[0]); S = int(st.randint(1, 1, 20)[0]); B = int(st.randint(1, 1, 40)[0])
+    cl = synth.make_custom(seed=100 + seed, K=K, M=M, F=F, S=S, B=B, R=97, lo=1, hi=4)
+    _check_all(ctx, cl)
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_tie_heavy_tables(ctx, seed):
+    """Tables quantised to a few powers of two: exact ties everywhere, lowest flat index wins."""
+    cl = U.tie_heavy(synth.make_custom(seed=200 + seed, K=9, M=3, F=12, S=6, B=5, R=64), seed)
+    cl.requests["slo_ttft_ms"] = 1e9
+    cl.requests["slo_tbt_ms"] = 1e9
+    cl.states["t"]["slo_ms"][...] = 1e9
+    _check_all(ctx, cl)
+
+
+def test_duplicate_models_on_one_gpu(ctx):
+    """The join target is the LOWEST slot holding the model."""
+    cl = synth.make_custom(seed=31, K=6, M=2, F=8, S=8, B=8, R=32, lo=2, hi=2)
+    cl.states["t"]["model"][:, 1] = cl.states["t"]["model"][:, 0]
+    _check_all(ctx, cl)
+
+
+def test_edge_cases(ctx):
+    cl = synth.make_custom(seed=41, K=12, M=3, F=10, S=8, B=8, R=40, lo=1, hi=4)
+    cl.states["n_res"][0] = 0                       # inactive GPU
+    cl.states["t"]["q"][1] = 0                      # all queues empty
+    cl.states["t"]["sigma"][2, :] = 1               # 4 tenants x 2 units = S: no free SMs
+    cl.states["n_res"][2] = 4
+    cl.states["t"]["model"][2] = [0, 1, 2, 0]
+    cl.states["t"]["beta"][3, :, 1] = cl.B - 1      # decode bucket already at the last level
+    cl.requests["L"][0] = 0
+    cl.requests["o_pred"][1] = 0
+    cl.requests["L"][2] = 1
+    cl.requests["slo_ttft_ms"][3] = 0.0             # nothing feasible
+    cl.requests["slo_tbt_ms"][4] = 0.0
+    cl.requests["L"][5] = 4096
+    cl.requests["o_pred"][5] = 4096
+    _check_all(ctx, cl)
+    got = ctx.place_batch(cl.requests)
+    assert got["gpu"][3] == -1 and np.isinf(got["energy_mj"][3]) and got["flat"][3] == 0xFFFFFFFF
+
+
+def test_empty_inputs(ctx):
+    cl = synth.make_custom(seed=5, K=4, M=2, F=4, S=4, B=4, R=8)
+    ctx.load_cluster(cl)
+    assert len(ctx.place_batch(cl.requests[:0])) == 0
+    assert len(ctx.local_config(0, gpu_ids=np.zeros(0, np.int32))) == 0
+    ctx.set_gpu_state(cl.states[:0])                # K = 0
+    got = ctx.place_batch(cl.requests)
+    assert (got["gpu"] == -1).all() and np.isinf(got["energy_mj"]).all()
+    assert len(ctx.consolidate()) == 0
+
+
+def test_local_gpu_id_subset(ctx):
+    cl = synth.make_custom(seed=6, K=20, M=4, F=16, S=8, B=16, R=0, lo=1, hi=4)
+    ctx.load_cluster(cl)
+    ids = np.array([19, 0, 7, 7, 3], dtype=np.int32)
+    for fl in ALL_FLAGS:
+        cmp.assert_local_equal(ctx.local_config(fl, gpu_ids=ids), _oracle_local(cl, fl, ids))
+
+
+def test_device_buffers_and_stream(ctx):
+    """FS_DEVICE pointers on a non-default torch stream give the same bytes as FS_HOST."""
+    import torch
+    cl = synth.make_cluster("tiny")
+    dev = torch.device("cuda:0")
+    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        lat, pw = torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev)
+        ctx.load_profiles(lat, pw, tb(cl.freq_mhz), tb(cl.models), cl.params, stream=s)
+        ctx.set_gpu_state(tb(cl.states), stream=s)
+        out = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+        ctx.place_batch(tb(cl.requests), out=out, stream=s)
+        lout = torch.empty(cl.K * 48, dtype=torch.uint8, device=dev)
+        ctx.local_config(0, n=cl.K, out=lout, stream=s)
+        cout = torch.empty(cl.K * 16, dtype=torch.uint8, device=dev)
+        ctx.consolidate(out=cout, stream=s)
+    s.synchronize()
+    cmp.assert_placement_equal(out.cpu().numpy().view(synth.PLACEMENT_DT), _oracle_place(cl))
+    cmp.assert_local_equal(lout.cpu().numpy().view(synth.LOCAL_CFG_DT), _oracle_local(cl, 0))
+    cmp.assert_consol_equal(cout.cpu().numpy().view(synth.CONSOL_DT), _oracle_consol(cl))
+
+
+# ---- error behaviour -------------------------------------------------------------------------
+def test_errors(fs):
+    c = fs.Festina(0)
+    cl = synth.make_custom(seed=8, K=4, M=2, F=4, S=4, B=4, R=8)
+    with pytest.raises(fs.FestinaError) as e:
+        c.set_gpu_state(cl.states)                  # before fs_load_profiles
+    assert e.value.code == fs.FS_ERR_STATE
+    c.load_profiles(cl.lat, cl.pow, cl.freq_mhz, cl.models, cl.params)
+    with pytest.raises(fs.FestinaError) as e:
+        c.place_batch(cl.requests)                  # before fs_set_gpu_state
+    assert e.value.code == fs.FS_ERR_STATE
+    bad = cl.states.copy()
+    bad["t"]["model"][1, 0] = 99                    # model index out of range
+    c.set_gpu_state(bad)
+    with pytest.raises(fs.FestinaError) as e:       # sticky flag surfaces on the next call
+        c.place_batch(cl.requests)
+    assert e.value.code == fs.FS_ERR_RANGE
+    # the invalid GPU is treated as inactive; results equal the oracle's on the cleaned state
+    clean = cl.states.copy()
+    clean["n_res"][1] = 0
+    got = c.place_batch(cl.requests)
+    ref = oracle.place_batch(cl.lat, cl.pow, cl.models, clean, cl.requests)
+    cmp.assert_placement_equal(got, ref)
+    breq = cl.requests.copy()
+    breq["model"][2] = -3
+    with pytest.raises(fs.FestinaError) as e:
+        c.place_batch(breq)
+    assert e.value.code == fs.FS_ERR_RANGE
+    with pytest.raises(fs.FestinaError) as e:
+        big = synth.make_custom(seed=8, K=1, M=1, F=2, S=40, B=2, R=0)   # S > FS_MAX_S
+        c.load_profiles(big.lat, big.pow, big.freq_mhz, big.models, big.params)
+    assert e.value.code == fs.FS_ERR_SHAPE
+    c.close()
+
+
+# ---- BASELINE.json configs at full size ----------------------------------------------------
+def test_rack_full(ctx):
+    cl = synth.make_cluster("rack")
+    ctx.load_cluster(cl)
+    got = ctx.place_batch(cl.requests)
+    cmp.assert_placement_equal(got, _oracle_place(cl))
+    # the Poisson dispatch ticks (variable R per call) give the same decisions as one call
+    ticks = synth.arrival_ticks(cl.seed, cl.R, 64)
+    parts, o = [], 0
+    for n in ticks:
+        parts.append(ctx.place_batch(cl.requests[o:o + n]))
+        o += n
+    cmp.assert_placement_equal(np.concatenate(parts), got)
+    for fl in ALL_FLAGS:
+        cmp.assert_local_equal(ctx.local_config(fl), _oracle_local(cl, fl))
+    cmp.assert_consol_equal(ctx.consolidate(), _oracle_consol(cl))
+
+
+def test_pod_full_size_sampled(ctx):
+    """configs[2] in the launch configuration bench.py times; the oracle recomputes a sample of
+    requests one by one, and every GPU's local config."""
+    cl = synth.make_cluster("pod")
+    ctx.load_cluster(cl)
+    got = ctx.place_batch(cl.requests)
+    idx = synth.Stream(7, "sample").randint(384, 0, cl.R - 1)
+    idx = np.unique(np.concatenate([idx, [0, cl.R - 1]]))
+    cmp.assert_placement_equal(got[idx], _oracle_place(cl, cl.requests[idx]))
+    assert (got["gpu"] >= 0).mean() > 0.9
+    for fl in (0, 2):
+        cmp.assert_local_equal(ctx.local_config(fl), _oracle_local(cl, fl))
+
+
+def test_local_sweep_full_size_sampled(ctx):
+    cl = synth.make_cluster("local")
+    ctx.load_cluster(cl)
+    ids = np.unique(synth.Stream(9, "sample").randint(96, 0, cl.K - 1)).astype(np.int32)
+    for fl in ALL_FLAGS:
+        got = ctx.local_config(fl)
+        assert len(got) == cl.K
+        cmp.assert_local_equal(got[ids], _oracle_local(cl, fl, ids))
+
+
+def test_consolidation_full_size(ctx):
+    cl = synth.make_cluster("consol")
+    ctx.load_cluster(cl)
+    got = ctx.consolidate()
+    cmp.assert_consol_equal(got, _oracle_consol(cl))
+    assert (got["dst"] >= 0).mean() > 0.5
