@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py — whole-hot-path throughput of libfestina_eval on N B200s (one process per GPU).
+
+A *step* is one pass of the hot path over one batch of synthetic input (BASELINE.json
+configs[2], "pod": K=1,024 GPUs, M=64 models, F=64, S=16, B=128, R=65,536 requests):
+    fs_set_gpu_state (co-resident summaries)  ->  fs_place_batch (R requests)
+    ->  fs_local_config on every GPU.
+`value` = nominal dense placement candidates (R*K*S*F) of all ranks / device time of the step,
+inputs resident in HBM.  `e2e` = the same through the C ABI with pinned HOST buffers (H2D of
+state + requests, D2H of placements + local configs inside the timed region).
+N > 1: tables and GPU state are replicated, every rank scores its own R requests (weak scaling,
+no data-path collective).
+`--impl reference` times the CPU oracle (test infrastructure) on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_30391_b200 import synth  # noqa: E402
+
+METRIC = "placement_candidate_evals_per_sec"
+UNIT = "candidates/s"
+# SURVEY §8(d) / DESIGN.md "Roofline": lane-operations the method needs per evaluated candidate
+OPS_PER_CANDIDATE = 13.0
+SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128   # 4 schedulers x 32 lanes (B300_MICROARCH "issue")
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thr = [], None, None
+        self.cmd = ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                    "-lms", "100"]
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(self.cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        self.thr = threading.Thread(target=pump, daemon=True)
+        self.thr.start()
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _dist():
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    lrank = int(os.environ.get("LOCAL_RANK", "0"))
+    return ws, rank, lrank
+
+
+def oracle_sample(cl, n_req: int, nthreads: int):
+    """One bounded pass of the hot path through the CPU oracle; returns (seconds, candidates)."""
+    import oracle
+    n_gpu = max(1, int(round(cl.K * n_req / cl.R)))
+    t0 = time.perf_counter()
+    oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests[:n_req], nthreads)
+    oracle.local_config(cl.lat, cl.pow, cl.states, 0, np.arange(n_gpu, dtype=np.int32), nthreads)
+    dt = time.perf_counter() - t0
+    return dt, n_req * cl.K * cl.S * cl.F, n_gpu
+
+
+def run_reference(args):
+    ws, rank, _ = _dist()
+    if rank != 0:
+        return
+    cl = synth.make_cluster(args.workload)
+    cores = os.cpu_count() or 1
+    n_req = args.ref_requests
+    for _ in range(args.warmup):
+        oracle_sample(cl, max(8, n_req // 8), cores)
+    tot, cand, n_gpu = 0.0, 0, 0
+    for _ in range(args.steps):
+        dt, c, n_gpu = oracle_sample(cl, n_req, cores)
+        tot += dt; cand += c
+    val = cand / tot
+    sample = (f"{n_req} of {cl.R} requests x all {cl.K} GPUs (fs_place_batch) + {n_gpu} GPUs "
+              f"(fs_local_config) per step")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": _config(cl, args),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def _config(cl, args):
+    return {"workload": f"{cl.name} (BASELINE.json configs[2]): K={cl.K} GPUs, M={cl.M}, F={cl.F}, S={cl.S}, "
+                        f"B={cl.B}, R={cl.R} requests per rank; step = fs_set_gpu_state + fs_place_batch + "
+                        f"fs_local_config(all GPUs, energy objective, exhaustive splits)",
+            "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B, "R_per_rank": cl.R,
+            "l2": "flushed between timed steps by overwriting a 256 MiB buffer",
+            "parallelism": f"replicated tables+state, requests sharded x{args.gpus}"}
+
+
+def run_ours(args):
+    import torch
+    import paper_2606_30391_b200 as fs
+
+    ws, rank, lrank = _dist()
+    dist = None
+    if ws > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(lrank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", lrank))
+    dev = torch.device("cuda", lrank)
+    torch.cuda.set_device(dev)
+    cl = synth.make_cluster(args.workload)
+    if rank > 0:   # every rank scores its own batch
+        cl.requests = synth.make_requests(cl.seed + 7919 * rank, cl.R, cl.M)
+    ctx = fs.Festina(lrank)
+    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+    # offline profile tables are loaded once (profiling is offline), not per step
+    ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                      tb(cl.models), cl.params)
+    d_states, d_reqs = tb(cl.states), tb(cl.requests)
+    d_place = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+    d_local = torch.empty(cl.K * 48, dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    ctx.set_timing(True)
+
+    def step_device():
+        ctx.set_gpu_state(d_states, stream=stream)
+        ctx.place_batch(d_reqs, out=d_place, stream=stream)
+        ctx.local_config(0, n=cl.K, out=d_local, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step_device()
+    barrier()
+    sampler = ClockSampler(lrank)
+    sampler.start()
+    l0 = ctx.launch_count
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kt = {}
+    barrier()
+    wall0 = time.perf_counter()
+    for a, b in evs:
+        flush.zero_()                      # L2 flush, outside the per-step events
+        a.record(stream)
+        step_device()
+        b.record(stream)
+        b.synchronize()
+        for k, v in ctx.get_timing().items():
+            kt.setdefault(k, []).append(v)
+    barrier()
+    wall = time.perf_counter() - wall0
+    launches = ctx.launch_count - l0
+    dev_ms = sum(a.elapsed_time(b) for a, b in evs)
+    pairs, cand_exec = ctx.last_place_stats()
+
+    # end to end through the C ABI with pinned host buffers
+    h_states = torch.from_numpy(cl.states.view(np.uint8).reshape(-1).copy()).pin_memory()
+    h_reqs = torch.from_numpy(cl.requests.view(np.uint8).reshape(-1).copy()).pin_memory()
+    h_place = torch.empty(cl.R * 32, dtype=torch.uint8).pin_memory()
+    h_local = torch.empty(cl.K * 48, dtype=torch.uint8).pin_memory()
+
+    def step_host():
+        ctx.set_gpu_state(h_states, stream=stream)
+        ctx.place_batch(h_reqs, out=h_place, stream=stream)
+        ctx.local_config(0, n=cl.K, out=h_local, stream=stream)
+
+    for _ in range(3):
+        step_host()
+    barrier()
+    e2e_t = 0.0
+    for _ in range(args.steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        step_host()
+        torch.cuda.synchronize()
+        e2e_t += time.perf_counter() - t0
+    clocks = sampler.stop()
+    assert np.array_equal(h_place.numpy(), d_place.cpu().numpy()), "host and device paths disagree"
+
+    t = torch.tensor([dev_ms, e2e_t * 1e3, wall * 1e3], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dev_ms, e2e_ms, wall_ms = (float(x) for x in t.cpu())
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    nominal = cl.R * cl.K * cl.S * cl.F
+    steps = args.steps
+    value = ws * nominal * steps / (dev_ms * 1e-3)
+    peaks, peak_src = _peaks()
+    sm_clk_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    alu_peak = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * sm_clk_hz          # lane-instructions / s
+    score_ms = float(np.mean(kt.get("place_score", [float("nan")])))
+    achieved = OPS_PER_CANDIDATE * cand_exec / (score_ms * 1e-3)
+    place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
+    ok = place["gpu"] >= 0
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": dev_ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": _config(cl, args),
+        "decisions_per_sec": ws * (cl.R + cl.K) * steps / (dev_ms * 1e-3),
+        "placement_decisions_per_sec": ws * cl.R * steps / (dev_ms * 1e-3),
+        "executed_candidates_per_step": cand_exec, "eligible_pairs_per_step": pairs,
+        "nominal_candidates_per_step": nominal,
+        "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
+        "wall_ms_per_step_incl_flush": wall_ms / steps,
+        "e2e": {"value": ws * nominal * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
+                "h2d_bytes_per_step": cl.K * 128 + cl.R * 32, "d2h_bytes_per_step": cl.R * 32 + cl.K * 48},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "fs_place_batch scorer", "achieved": achieved / 1e12,
+                     "peak": alu_peak / 1e12, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
+                     "traffic": None,
+                     "note": f"{OPS_PER_CANDIDATE:g} lane-ops per evaluated candidate (DESIGN.md) x "
+                             f"{cand_exec} candidates / {score_ms:.3f} ms; peak = 148 SMs x 128 lanes/clk x "
+                             f"{sm_clk_hz / 1e6:.0f} MHz ({peak_src} sm_max_mhz)"},
+        "degeneracy": {"placed_frac": float(ok.mean()),
+                       "top_phi_share": float(np.bincount(place["phi"][ok]).max() / max(ok.sum(), 1)),
+                       "distinct_gpus": int(len(np.unique(place["gpu"][ok])))},
+    }
+    if ws == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        dt, c, n_gpu = oracle_sample(cl, args.cpu_requests, cores)
+        line["cpu_baseline"] = {"value": c / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{args.cpu_requests} of {cl.R} requests x all {cl.K} GPUs + "
+                                          f"{n_gpu} GPUs local config, {dt:.1f} s"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="pod", choices=list(synth.CONFIGS))
+    ap.add_argument("--cpu-requests", type=int, default=1536, help="oracle sample of the cpu_baseline leg")
+    ap.add_argument("--ref-requests", type=int, default=256, help="oracle sample per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -24,7 +24,9 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
            "fs_local_config", "fs_consolidate", "fs_strerror", "fs_last_cuda_error",
-           "fs_launch_count", "fs_last_place_stats")
+           "fs_launch_count", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
+TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
+          "consol_pair")
 
 
 class FsDims(C.Structure):
@@ -69,6 +71,8 @@ def lib() -> C.CDLL:
     L.fs_launch_count.argtypes = [vp]
     L.fs_launch_count.restype = C.c_uint64
     L.fs_last_place_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.fs_set_timing.argtypes = [vp, C.c_int]
+    L.fs_get_timing.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
     for name in SYMBOLS:
         getattr(L, name)   # AttributeError if the library does not export it
     _lib = L
@@ -204,6 +208,15 @@ class Festina:
         a, b = C.c_uint64(0), C.c_uint64(0)
         self._check(lib().fs_last_place_stats(self._h, C.byref(a), C.byref(b)), "fs_last_place_stats")
         return int(a.value), int(b.value)
+
+    def set_timing(self, on: bool = True):
+        self._check(lib().fs_set_timing(self._h, int(on)), "fs_set_timing")
+
+    def get_timing(self) -> dict:
+        """Device time in ms of the most recent launch of each timed kernel (see fs_timer)."""
+        ms = (C.c_float * len(TIMERS))()
+        self._check(lib().fs_get_timing(self._h, ms, len(TIMERS)), "fs_get_timing")
+        return {k: float(ms[i]) for i, k in enumerate(TIMERS) if ms[i] >= 0}
 
     def load_cluster(self, cl: synth.Cluster, stream=None):
         """Convenience: fs_load_profiles + fs_set_gpu_state from a synthetic cluster (host)."""

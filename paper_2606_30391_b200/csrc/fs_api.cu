@@ -35,6 +35,7 @@ struct fs_ctx {
   // diagnostics
   int* flag_host = nullptr; int* flag_dev = nullptr;
   uint64_t launches = 0; int last_cuda = 0;
+  bool timing = false; bool have_events = false; FsTimers tm{};
 };
 
 namespace {
@@ -147,6 +148,8 @@ int fs_destroy(fs_ctx* c) {
                   c->agg, c->ckeys, c->consol_dev};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (c->flag_host) cudaFreeHost(c->flag_host);
+  if (c->have_events)
+    for (int i = 0; i < FS_T_COUNT; ++i) { cudaEventDestroy(c->tm.beg[i]); cudaEventDestroy(c->tm.end[i]); }
   cudaGetLastError();
   delete c;
   return FS_OK;
@@ -219,7 +222,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (K > 0) {
     FS_CUDA(c, cudaMemcpyAsync(c->states, states, (size_t)K * sizeof(fs_gpu_state), in_kind(space), st));
     FsView v = view_of(c);
-    c->launches += fsk_summary(v, c->ginfo, c->gA, st);
+    c->launches += fsk_summary(v, c->ginfo, c->gA, st, c->timing ? &c->tm : nullptr);
     c->launches += fsk_build_warm_lists(v, c->warm_off, c->warm_cursor, c->warm_item, st);
     FS_TRY(check_kernel(c));
   }
@@ -247,7 +250,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
   FsPlaceScratch sc{c->keys, c->stats, c->warm_off, c->warm_item};
-  c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st);
+  c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
@@ -281,7 +284,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
     d_out = c->local_dev;
   }
   FsLocalScratch sc{c->G, c->Bst, c->comp, c->comp_n, c->ns_stride};
-  c->launches += fsk_local(view_of(c), n, d_ids, flags, d_out, sc, st);
+  c->launches += fsk_local(view_of(c), n, d_ids, flags, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->local_dev, (size_t)n * sizeof(fs_local_cfg), cudaMemcpyDeviceToHost, st));
@@ -308,7 +311,7 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
   }
   fs_consol_out* d_out = space == FS_HOST ? c->consol_dev : out;
   FsConsolScratch sc{c->need, c->E, c->agg, c->ckeys};
-  c->launches += fsk_consolidate(view_of(c), c->prm, d_out, sc, st);
+  c->launches += fsk_consolidate(view_of(c), c->prm, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->consol_dev, (size_t)c->K * sizeof(fs_consol_out), cudaMemcpyDeviceToHost, st));
@@ -334,6 +337,33 @@ const char* fs_strerror(int code) {
 
 int fs_last_cuda_error(const fs_ctx* c) { return c ? c->last_cuda : 0; }
 uint64_t fs_launch_count(const fs_ctx* c) { return c ? c->launches : 0; }
+
+int fs_set_timing(fs_ctx* c, int on) {
+  if (!c) return FS_ERR_ARG;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  if (on && !c->have_events) {
+    for (int i = 0; i < FS_T_COUNT; ++i) {
+      FS_CUDA(c, cudaEventCreate(&c->tm.beg[i])); FS_CUDA(c, cudaEventCreate(&c->tm.end[i]));
+      c->tm.used[i] = false;
+    }
+    c->have_events = true;
+  }
+  c->timing = on != 0;
+  return FS_OK;
+}
+
+int fs_get_timing(fs_ctx* c, float* ms, int n) {
+  if (!c || !ms || n < 0) return FS_ERR_ARG;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  for (int i = 0; i < n; ++i) {
+    ms[i] = -1.0f;
+    if (i < FS_T_COUNT && c->have_events && c->tm.used[i]) {
+      FS_CUDA(c, cudaEventSynchronize(c->tm.end[i]));
+      FS_CUDA(c, cudaEventElapsedTime(&ms[i], c->tm.beg[i], c->tm.end[i]));
+    }
+  }
+  return FS_OK;
+}
 
 int fs_last_place_stats(fs_ctx* c, uint64_t* pairs, uint64_t* candidates) {
   if (!c || !pairs || !candidates) return FS_ERR_ARG;

@@ -150,14 +150,18 @@ __global__ void consol_decode_kernel(FsView v, int S_eff, fs_params prm,
 }  // namespace
 
 int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
-                    const FsConsolScratch& sc, cudaStream_t st) {
+                    const FsConsolScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int S_eff = (v.d.S * (100 - prm.delta_pct)) / 100;
   const float M_eff = (prm.mem_cap_mb * (float)(100 - prm.delta_pct)) / 100.0f;
+  fs_tm_beg(tm, FS_T_CONSOL_AGG, st);
   consol_agg_kernel<<<(v.K + 3) / 4, 128, 0, st>>>(v, S_eff, sc.need, sc.E, sc.agg);
+  fs_tm_end(tm, FS_T_CONSOL_AGG, st);
   const size_t smem = (sizeof(float) + sizeof(int)) * v.d.F * TA;
+  fs_tm_beg(tm, FS_T_CONSOL_PAIR, st);
   consol_pair_kernel<<<(v.K + TA - 1) / TA, PAIR_THREADS, smem, st>>>(v, S_eff, M_eff, sc.need,
                                                                     sc.E, sc.agg, sc.keys);
+  fs_tm_end(tm, FS_T_CONSOL_PAIR, st);
   consol_decode_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, S_eff, prm, sc.need, sc.E, sc.agg,
                                                           sc.keys, out);
   return 3;

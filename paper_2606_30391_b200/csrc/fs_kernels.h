@@ -5,6 +5,17 @@
 
 #include "fs_common.cuh"
 
+// Optional per-kernel timing (fs_set_timing): CUDA event pairs recorded on the caller's stream
+// around the kernels bench.py reports rooflines for.  NULL = no timing.
+enum { FS_T_PLACE_SCORE = 0, FS_T_PLACE_DECODE, FS_T_SUMMARY, FS_T_LOCAL_SLOT, FS_T_LOCAL_SPLIT,
+       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_COUNT };
+struct FsTimers {
+  cudaEvent_t beg[FS_T_COUNT], end[FS_T_COUNT];
+  bool used[FS_T_COUNT];
+};
+static inline void fs_tm_beg(FsTimers* t, int i, cudaStream_t st) { if (t) { cudaEventRecord(t->beg[i], st); } }
+static inline void fs_tm_end(FsTimers* t, int i, cudaStream_t st) { if (t) { cudaEventRecord(t->end[i], st); t->used[i] = true; } }
+
 // device-resident view of everything fs_load_profiles / fs_set_gpu_state own
 struct FsView {
   FsDimsDev d;
@@ -25,7 +36,7 @@ int fsk_build_planes(const float* lat, const float* pow, float* latT, float* pow
                      int* flag, cudaStream_t st);
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
-int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st);
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st, FsTimers* tm);
 
 // fs_place.cu — placement scoring + 64-bit-key argmin + decode
 struct FsPlaceScratch {
@@ -36,7 +47,7 @@ struct FsPlaceScratch {
   const uint32_t* warm_item;       // [sum n_res]: k*4 + j
 };
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
-              const FsPlaceScratch& sc, cudaStream_t st);
+              const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm);
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,
                          uint32_t* warm_item /*[4K]*/, cudaStream_t st);
 
@@ -50,7 +61,7 @@ struct FsLocalScratch {
 };
 int fsk_local_smem_attr();   // raise the split kernel's dynamic shared memory limit (once)
 int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,
-              const FsLocalScratch& sc, cudaStream_t st);
+              const FsLocalScratch& sc, cudaStream_t st, FsTimers* tm);
 
 // fs_consol.cu — per-tenant minimum share, per-GPU aggregates, pair scoring
 struct FsConsolScratch {
@@ -60,7 +71,7 @@ struct FsConsolScratch {
   unsigned long long* keys;  // [K] per-source argmin key (score, dst)
 };
 int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
-                    const FsConsolScratch& sc, cudaStream_t st);
+                    const FsConsolScratch& sc, cudaStream_t st, FsTimers* tm);
 
 #ifdef __CUDACC__
 // One co-resident ("tenant") at frequency phi with share sigma, wait = 0 because its slo is the

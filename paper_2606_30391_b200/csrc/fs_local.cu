@@ -231,12 +231,16 @@ int fsk_local_smem_attr() {
 }
 
 int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,
-              const FsLocalScratch& sc, cudaStream_t st) {
+              const FsLocalScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (n <= 0) return 0;
   const int rows = v.d.F * v.d.S;
+  fs_tm_beg(tm, FS_T_LOCAL_SLOT, st);
   local_slot_kernel<<<dim3(n, FS_RMAX * 2), 256, 0, st>>>(v, n, gpu_ids, flags, sc.G, sc.B);
+  fs_tm_end(tm, FS_T_LOCAL_SLOT, st);
   const size_t smem = sizeof(float) * FS_RMAX * rows;
+  fs_tm_beg(tm, FS_T_LOCAL_SPLIT, st);
   local_split_kernel<<<n, 256, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.B, sc.comp, sc.comp_n,
                                            sc.ns_stride, out);
+  fs_tm_end(tm, FS_T_LOCAL_SPLIT, st);
   return 2;
 }

@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
 }  // namespace
 
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
-              const FsPlaceScratch& sc, cudaStream_t st) {
+              const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (R <= 0) return 0;
   int launches = 0;
   cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
@@ -174,10 +174,14 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   nsplit = (v.K + kchunk - 1) / (kchunk > 0 ? kchunk : 1);
   if (nsplit < 1) nsplit = 1;
   const long long warps = (long long)R * nsplit;
+  fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
   place_generic_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(v, R, reqs, sc.keys, nsplit,
                                                                    kchunk, sc.stats);
+  fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   ++launches;
+  fs_tm_beg(tm, FS_T_PLACE_DECODE, st);
   place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
+  fs_tm_end(tm, FS_T_PLACE_DECODE, st);
   ++launches;
   return launches;
 }

@@ -135,10 +135,12 @@ __global__ void warm_fill_kernel(FsView v, const int32_t* __restrict__ off,
 
 }  // namespace
 
-int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st) {
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int wpb = 4;
+  fs_tm_beg(tm, FS_T_SUMMARY, st);
   summary_kernel<<<(v.K + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA);
+  fs_tm_end(tm, FS_T_SUMMARY, st);
   return 1;
 }
 
