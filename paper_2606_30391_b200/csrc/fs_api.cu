@@ -3,6 +3,7 @@
 // No arithmetic of the method lives here (kernels: fs_tables/fs_summary/fs_place/fs_local/
 // fs_consol .cu) and there is no CPU fallback: without a CUDA device every call fails.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -22,6 +23,7 @@ struct fs_ctx {
   // state + summaries
   int K = 0, k_cap = 0;
   fs_gpu_state* states = nullptr; FsGpuInfo* ginfo = nullptr; float* gA = nullptr; size_t gA_cap = 0;
+  FsGpuRec* grec = nullptr; float* gA0 = nullptr; size_t gA0_cap = 0; int Kpad = 0, FT = 32;
   int32_t *warm_off = nullptr, *warm_cursor = nullptr; uint32_t* warm_item = nullptr; int warm_m_cap = 0;
   // placement scratch
   int r_cap = 0; unsigned long long* keys = nullptr; unsigned long long* stats = nullptr;
@@ -36,6 +38,7 @@ struct fs_ctx {
   int* flag_host = nullptr; int* flag_dev = nullptr;
   uint64_t launches = 0; int last_cuda = 0;
   bool timing = false; bool have_events = false; FsTimers tm{};
+  int sm_count = 148; bool force_generic = false;
 };
 
 namespace {
@@ -76,6 +79,7 @@ FsView view_of(const fs_ctx* c) {
   v.d = FsDimsDev{c->d.M, c->d.F, c->d.S, c->d.B};
   v.lat = c->lat; v.pow = c->pow; v.latT = c->latT; v.powT = c->powT; v.models = c->models;
   v.K = c->K; v.states = c->states; v.ginfo = c->ginfo; v.gA = c->gA; v.flag = c->flag_dev;
+  v.grec = c->grec; v.gA0 = c->gA0; v.Kpad = c->Kpad; v.FT = c->FT;
   return v;
 }
 
@@ -134,6 +138,9 @@ int fs_create(fs_ctx** out, int cuda_device) {
   std::memset(c->flag_host, 0, sizeof(int) * FS_NFLAGS);
   cudaMemset(c->stats, 0, 2 * sizeof(unsigned long long));
   fsk_local_smem_attr();
+  fsk_place_smem_attr();
+  cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
+  if (const char* e = getenv("FS_FORCE_GENERIC")) c->force_generic = e[0] == '1';
   *out = c;
   return FS_OK;
 }
@@ -143,7 +150,7 @@ int fs_destroy(fs_ctx* c) {
   cudaSetDevice(c->dev);
   cudaDeviceSynchronize();
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
-                  c->ginfo, c->gA, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
+                  c->ginfo, c->gA, c->grec, c->gA0, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -209,11 +216,15 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   const int pending = take_flags(c);
   if (K > c->k_cap) {
     FS_TRY(grow(c, c->states, (size_t)K)); FS_TRY(grow(c, c->ginfo, (size_t)K));
+    FS_TRY(grow(c, c->grec, (size_t)K + FS_CHUNK));
     FS_TRY(grow(c, c->warm_item, (size_t)K * FS_RMAX));
     c->k_cap = K; c->consol_cap = 0;
   }
   const size_t na = (size_t)K * FS_NVAR * c->d.F;
   if (na > c->gA_cap) { FS_TRY(grow(c, c->gA, na)); c->gA_cap = na; }
+  c->Kpad = (K + FS_CHUNK - 1) / FS_CHUNK * FS_CHUNK; c->FT = (c->d.F + 31) / 32 * 32;
+  const size_t na0 = (size_t)c->Kpad * c->FT;
+  if (na0 > c->gA0_cap) { FS_TRY(grow(c, c->gA0, na0)); c->gA0_cap = na0; }
   if (c->d.M > c->warm_m_cap) {
     FS_TRY(grow(c, c->warm_off, (size_t)c->d.M + 1)); FS_TRY(grow(c, c->warm_cursor, (size_t)c->d.M));
     c->warm_m_cap = c->d.M;
@@ -222,7 +233,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (K > 0) {
     FS_CUDA(c, cudaMemcpyAsync(c->states, states, (size_t)K * sizeof(fs_gpu_state), in_kind(space), st));
     FsView v = view_of(c);
-    c->launches += fsk_summary(v, c->ginfo, c->gA, st, c->timing ? &c->tm : nullptr);
+    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0, st, c->timing ? &c->tm : nullptr);
     c->launches += fsk_build_warm_lists(v, c->warm_off, c->warm_cursor, c->warm_item, st);
     FS_TRY(check_kernel(c));
   }
@@ -249,7 +260,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
-  FsPlaceScratch sc{c->keys, c->stats, c->warm_off, c->warm_item};
+  FsPlaceScratch sc{c->keys, c->stats, c->warm_off, c->warm_item, c->sm_count, c->force_generic};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {

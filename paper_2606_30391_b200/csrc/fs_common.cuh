@@ -40,6 +40,16 @@ struct __align__(16) FsGpuInfo {
 };
 static_assert(sizeof(FsGpuInfo) == 48, "FsGpuInfo layout");
 
+// Compact per-GPU record the dense placement kernel stages with TMA (32 bytes).
+struct __align__(16) FsGpuRec {
+  float t_avail_ms, mem_free_mb, e_cur;
+  uint32_t meta;            // n_res | sm_free << 8   (n_res == 0: never a candidate)
+  int16_t model[FS_RMAX];
+  uint32_t _pad[2];
+};
+static_assert(sizeof(FsGpuRec) == 32, "FsGpuRec layout");
+#define FS_CHUNK 32         // GPUs per staged chunk (one per lane in the eligibility pass)
+
 struct FsDimsDev { int M, F, S, B; };
 
 // ---- table addressing --------------------------------------------------------------------

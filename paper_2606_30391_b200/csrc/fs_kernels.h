@@ -28,6 +28,10 @@ struct FsView {
   const fs_gpu_state* states;
   const FsGpuInfo* ginfo;   // [K]
   const float* gA;          // [K][FS_NVAR][F]  co-resident energy per variant, INF = infeasible
+  const FsGpuRec* grec;     // [Kpad]           compact records, Kpad = K rounded up to FS_CHUNK
+  const float* gA0;         // [Kpad][FT]       variant 0 of gA, row stride FT = F rounded up to 32,
+                            //                  padding = INF (what the dense kernel stages by TMA)
+  int Kpad, FT;
   int* flag;                // sticky range-error flag (mapped host memory)
 };
 
@@ -36,7 +40,8 @@ int fsk_build_planes(const float* lat, const float* pow, float* latT, float* pow
                      int* flag, cudaStream_t st);
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
-int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st, FsTimers* tm);
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
+                cudaStream_t st, FsTimers* tm);
 
 // fs_place.cu — placement scoring + 64-bit-key argmin + decode
 struct FsPlaceScratch {
@@ -45,7 +50,10 @@ struct FsPlaceScratch {
   // bucketing of GPUs by model (built by fs_set_gpu_state): warm lists
   const int32_t* warm_off;         // [M+1]
   const uint32_t* warm_item;       // [sum n_res]: k*4 + j
+  int sm_count;                    // SMs of the device (grid sizing)
+  bool force_generic;              // diagnostics: score with the generic kernel only
 };
+int fsk_place_smem_attr();
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
               const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm);
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,

@@ -120,6 +120,270 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
   }
 }
 
+
+// =============================================================================================
+// Dense scorer for COLD pairs (the request's model is not resident on the GPU), S <= 16, F <= 64.
+//
+// Factorisation (exact): for a cold pair the decode bucket is 0 and
+// the co-resident variant is 0, so everything that depends on (sigma, phi) is per REQUEST:
+//   t0[s][f] = fl(rounds0*LAT0)                    er[s][f] = fl(e0 + e1), INF where LAT1 > slo_tbt
+// and everything that depends on the GPU is per (k, phi):  A0[k][f], Ecur[k], wait_k, sm_free_k.
+// fl(A + x) and fl(x - Ecur) are monotone in x, hence
+//   min_s fl(fl(A0 + er[s]) - Ecur) = fl(fl(A0 + min_s er[s]) - Ecur)   over feasible s,
+// and fl(wait + t) <= slo  <=>  t <= T*(wait, slo) for the exactly computed threshold T*.
+// Per candidate that leaves one compare and one conditional min, on registers.
+//
+// Layout: one warp = one request, lane owns NPHI adjacent frequencies and all 16 shares
+// (2*16*NPHI registers).  A block walks the GPUs in chunks of 32 staged by 1-D TMA bulk copies
+// (records + A0 rows) through an mbarrier ring shared by its warps; each lane first evaluates
+// eligibility and T* for ONE GPU of the chunk, then the warp sweeps the eligible GPUs.
+// The lowest flat index among equal minima is recovered exactly at the end (see below).
+// =============================================================================================
+constexpr int DENSE_WARPS = 8;
+constexpr int DENSE_STAGES = 4;
+constexpr int DENSE_S = 16;
+
+// largest t >= 0 with fl(w + t) <= slo, or -1 if there is none.  fl(w + .) is monotone, so the
+// answer is characterised by g(T) <= slo < g(nextup(T)); a double-precision guess is verified
+// with the fp32 operation itself and a bit-pattern bisection covers whatever it misses.
+__device__ __forceinline__ float nextup_nonneg(float x) {       // x >= +0, finite or INF
+  return x < FS_INF ? __uint_as_float(__float_as_uint(x) + 1u) : x;
+}
+__device__ __noinline__ float tstar_bisect(float w, float slo) {
+  uint32_t lo = 0u, hi = 0x7F800000u;                            // g(lo) <= slo holds
+  if (__fadd_rn(w, FS_INF) <= slo) return FS_INF;
+  while (hi - lo > 1u) {
+    const uint32_t mid = lo + ((hi - lo) >> 1);
+    if (__fadd_rn(w, __uint_as_float(mid)) <= slo) lo = mid; else hi = mid;
+  }
+  return __uint_as_float(lo);
+}
+__device__ __forceinline__ float fs_tstar(float w, float slo) {
+  if (!(__fadd_rn(w, 0.0f) <= slo)) return -1.0f;                // also NaN
+  if (!(slo < FS_INF)) return FS_INF;
+  float s = slo; if (s == 0.0f) s = 0.0f;
+  const uint32_t sb = __float_as_uint(s);
+  const float up = __uint_as_float(s >= 0.0f ? sb + 1u : sb - 1u);   // next float above slo
+  const double U = 0.5 * ((double)s + (double)up);               // rounding boundary above slo
+  float T = __double2float_rd(U - (double)w);
+  if (!(T >= 0.0f)) T = 0.0f;
+  if (!(__fadd_rn(w, T) <= slo) && T > 0.0f) T = __uint_as_float(__float_as_uint(T) - 1u);
+  const bool ok_here = __fadd_rn(w, T) <= slo;
+  const bool ok_next = T < FS_INF && (__fadd_rn(w, nextup_nonneg(T)) <= slo);
+  if (ok_here && !ok_next) return T;
+  return tstar_bisect(w, slo);
+}
+
+struct DenseSmem {
+  alignas(128) float a0[DENSE_STAGES][FS_CHUNK * 64];   // [stage][gpu][FT] rows (FT = 32*NPHI)
+  alignas(16) FsGpuRec rec[DENSE_STAGES][FS_CHUNK];
+  alignas(16) float4 wb[DENSE_WARPS][FS_CHUNK];         // per warp: {T*, Ecur, sm_free, -}
+  alignas(8) uint64_t full[DENSE_STAGES];
+  alignas(8) uint64_t empty[DENSE_STAGES];
+};
+
+template <int NPHI>
+__global__ void __launch_bounds__(DENSE_WARPS * 32, 2)
+place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
+                   unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
+                   unsigned long long* __restrict__ stats) {
+  extern __shared__ __align__(128) unsigned char dense_smem_raw[];
+  DenseSmem& sm = *reinterpret_cast<DenseSmem*>(dense_smem_raw);
+  constexpr int FT = 32 * NPHI;
+  const FsDimsDev d = v.d;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nchunk_all = v.Kpad / FS_CHUNK;
+  const int slice = blockIdx.x % nslice;
+  const int c0 = slice * chunks_per_slice, c1 = min(nchunk_all, c0 + chunks_per_slice);
+  const int nchunk = c1 - c0;
+  const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS;
+  const int b_first = blockIdx.x / nslice, b_stride = gridDim.x / nslice;
+  const int my_batches = b_first < nbatch ? (nbatch - b_first + b_stride - 1) / b_stride : 0;
+  const long long total = (long long)my_batches * nchunk;
+  const uint32_t bytes_a0 = FS_CHUNK * FT * sizeof(float), bytes_rec = FS_CHUNK * sizeof(FsGpuRec);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < DENSE_STAGES; ++s) { fs_mbar_init(&sm.full[s], 1); fs_mbar_init(&sm.empty[s], DENSE_WARPS); }
+    fs_mbar_fence_init();
+  }
+  __syncthreads();
+  auto issue = [&](long long n) {          // producer: stage chunk number n of this block's stream
+    const int s = (int)(n % DENSE_STAGES);
+    fs_mbar_wait(&sm.empty[s], (uint32_t)(((n / DENSE_STAGES) & 1) ^ 1));
+    const int chunk = c0 + (int)(n % nchunk);
+    fs_mbar_expect_tx(&sm.full[s], bytes_a0 + bytes_rec);
+    fs_tma_load_1d(&sm.a0[s][0], v.gA0 + (size_t)chunk * FS_CHUNK * FT, bytes_a0, &sm.full[s]);
+    fs_tma_load_1d(&sm.rec[s][0], v.grec + (size_t)chunk * FS_CHUNK, bytes_rec, &sm.full[s]);
+  };
+  if (threadIdx.x == 0)
+    for (long long n = 0; n < total && n < DENSE_STAGES - 1; ++n) issue(n);
+
+  // per-request registers
+  float t0[DENSE_S][NPHI], er[DENSE_S][NPHI];
+  ReqCtx c; bool active = false; int r = -1;
+  float best = FS_INF; int bestk = -1;
+  unsigned long long npairs = 0, ncand = 0;
+
+  for (long long it = 0; it < total; ++it) {
+    const int ci = (int)(it % nchunk);
+    if (ci == 0) {
+      // ---- phase A: new request for this warp ------------------------------------------------
+      r = (b_first + (int)(it / nchunk) * b_stride) * DENSE_WARPS + warp;
+      active = r < R;
+      best = FS_INF; bestk = -1;
+      if (active) {
+        c = make_req(v, reqs[r]);
+        if (!c.valid) { active = false; if (lane == 0 && slice == 0) fs_raise(v.flag, FS_FLAG_REQUEST); }
+      }
+      if (active) {
+        const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
+        const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
+        const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
+#pragma unroll
+        for (int s = 0; s < DENSE_S; ++s)
+#pragma unroll
+          for (int i = 0; i < NPHI; ++i) {
+            const int phi = lane * NPHI + i;
+            float tt = FS_INF, ee = FS_INF;
+            if (s < d.S && phi < d.F) {
+              const int o = s * d.F + phi;
+              float e0 = 0.f, e1 = 0.f; bool ok1 = true; tt = 0.f;
+              if (c.L > 0) { tt = __fmul_rn(fr0, l0[o]); e0 = __fmul_rn(tt, p0[o]); }
+              if (c.O > 0) { const float la = l1[o]; ok1 = la <= c.slo_tbt; e1 = __fmul_rn(__fmul_rn(fO, la), p1[o]); }
+              ee = ok1 ? __fadd_rn(e0, e1) : FS_INF;
+            }
+            t0[s][i] = tt; er[s][i] = ee;
+          }
+      }
+    }
+    if (threadIdx.x == 0 && it + DENSE_STAGES - 1 < total) issue(it + DENSE_STAGES - 1);
+    __syncwarp();
+    const int st = (int)(it % DENSE_STAGES);
+    fs_mbar_wait(&sm.full[st], (uint32_t)((it / DENSE_STAGES) & 1));
+    if (active) {
+      // ---- eligibility + T*: lane <-> one GPU of the chunk ------------------------------------
+      const FsGpuRec g = sm.rec[st][lane];
+      const int n_res = g.meta & 0xFF, smf = (g.meta >> 8) & 0xFF;
+      bool el = n_res >= 1 && n_res < FS_RMAX && smf >= 1 && (c.mem <= g.mem_free_mb);
+#pragma unroll
+      for (int i = 0; i < FS_RMAX; ++i) el = el && (g.model[i] != c.m);   // resident -> warm path
+      float T = -1.0f;
+      if (el) {
+        T = c.L > 0 ? fs_tstar(__fadd_rn(g.t_avail_ms, c.load_ms), c.slo_ttft) : FS_INF;
+        npairs += 1; ncand += (unsigned long long)smf * d.F;
+      }
+      sm.wb[warp][lane] = make_float4(T, g.e_cur, __int_as_float(smf), 0.f);
+      unsigned mask = __ballot_sync(0xffffffffu, el && T >= 0.0f);
+      __syncwarp();
+      // ---- sweep the eligible GPUs of the chunk -------------------------------------------------
+      const int kbase = (c0 + ci) * FS_CHUNK;
+      while (mask) {
+        const int g_i = __ffs(mask) - 1; mask &= mask - 1;
+        const float4 w = sm.wb[warp][g_i];
+        const float Tst = w.x; const int sfree = __float_as_int(w.z);
+        float m[NPHI];
+#pragma unroll
+        for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
+#define FS_DENSE_STEP(s)                                                              \
+  _Pragma("unroll") for (int i = 0; i < NPHI; ++i)                                    \
+    asm("{.reg .pred p; setp.le.f32 p, %1, %2; @p min.f32 %0, %0, %3;}"               \
+        : "+f"(m[i]) : "f"(t0[s][i]), "f"(Tst), "f"(er[s][i]));
+        switch (sfree) {
+          default:
+          case 16: FS_DENSE_STEP(15) case 15: FS_DENSE_STEP(14) case 14: FS_DENSE_STEP(13)
+          case 13: FS_DENSE_STEP(12) case 12: FS_DENSE_STEP(11) case 11: FS_DENSE_STEP(10)
+          case 10: FS_DENSE_STEP(9)  case 9: FS_DENSE_STEP(8)   case 8: FS_DENSE_STEP(7)
+          case 7: FS_DENSE_STEP(6)   case 6: FS_DENSE_STEP(5)   case 5: FS_DENSE_STEP(4)
+          case 4: FS_DENSE_STEP(3)   case 3: FS_DENSE_STEP(2)   case 2: FS_DENSE_STEP(1)
+          case 1: FS_DENSE_STEP(0)
+        }
+#undef FS_DENSE_STEP
+        const float* arow = &sm.a0[st][g_i * FT + lane * NPHI];
+        float x = FS_INF;
+#pragma unroll
+        for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
+        const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
+        if (dE < best) { best = dE; bestk = kbase + g_i; }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) fs_mbar_arrive(&sm.empty[st]);
+
+    if (ci == nchunk - 1 && active) {
+      // ---- recovery: lowest flat index among the candidates that attain the minimum -----------
+      unsigned long long key = FS_KEY_NONE;
+      if (bestk >= 0) {
+        const FsGpuRec g = v.grec[bestk];
+        const int smf = (g.meta >> 8) & 0xFF;
+        const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
+        float a[NPHI];
+#pragma unroll
+        for (int i = 0; i < NPHI; ++i) a[i] = v.gA0[(size_t)bestk * FT + lane * NPHI + i];
+        bool found = false; uint32_t flat = 0xFFFFFFFFu;
+#pragma unroll
+        for (int s = 0; s < DENSE_S; ++s)
+#pragma unroll
+          for (int i = 0; i < NPHI; ++i) {
+            const bool feas = s < smf && (c.L == 0 || __fadd_rn(wait, t0[s][i]) <= c.slo_ttft);
+            const float dE = __fsub_rn(__fadd_rn(a[i], er[s][i]), g.e_cur);
+            if (!found && feas && dE == best) {
+              found = true; flat = (uint32_t)((bestk * d.S + s) * d.F + lane * NPHI + i);
+            }
+          }
+        if (found) key = fs_make_key(best, flat);
+      }
+      key = fs_warp_min_key(key);
+      if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
+    }
+  }
+  // work statistics (nominal candidates actually evaluated)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
+    ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
+  }
+  if (lane == 0 && stats && npairs) { atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand); }
+}
+
+// ---- warm pairs: the request's model is resident on the GPU (decode bucket and co-resident
+// variant depend on the GPU), evaluated candidate by candidate from the planes.  One warp per
+// request walks the (GPU, slot) list of its model; when `all_pairs` it walks every GPU instead.
+__global__ void __launch_bounds__(256) place_warm_kernel(FsView v, int R,
+                                                        const fs_request* __restrict__ reqs,
+                                                        unsigned long long* __restrict__ keys,
+                                                        const int32_t* __restrict__ warm_off,
+                                                        const uint32_t* __restrict__ warm_item,
+                                                        unsigned long long* __restrict__ stats) {
+  const int lane = threadIdx.x & 31;
+  const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (r >= R) return;
+  const ReqCtx c = make_req(v, reqs[r]);
+  if (!c.valid) return;                        // flagged by the dense kernel
+  const FsDimsDev d = v.d;
+  float best = FS_INF; uint32_t bflat = 0xFFFFFFFFu; bool have = false;
+  unsigned long long npairs = 0, ncand = 0;
+  // items of one model are unordered: compare (value, flat) in full
+  for (int it = warm_off[c.m]; it < warm_off[c.m + 1]; ++it) {
+    const int k = (int)(warm_item[it] >> 2);
+    const PairCtx p = make_pair(v, c, v.ginfo[k]);
+    if (!p.ok) continue;
+    npairs += 1; ncand += (unsigned long long)p.smf * d.F;
+    for (int sg = 0; sg < p.smf; ++sg)
+      for (int phi = lane; phi < d.F; phi += 32) {
+        const Cand cd = eval_cand(v, c, p, k, sg, phi);
+        float dE = cd.dE; if (dE == 0.0f) dE = 0.0f;
+        const uint32_t flat = (uint32_t)((k * d.S + sg) * d.F + phi);
+        if (cd.ok && (!have || dE < best || (dE == best && flat < bflat))) { have = true; best = dE; bflat = flat; }
+      }
+  }
+  unsigned long long key = have ? fs_make_key(best, bflat) : FS_KEY_NONE;
+  key = fs_warp_min_key(key);
+  if (lane == 0) {
+    if (key != FS_KEY_NONE) atomicMin(&keys[r], key);
+    if (stats && npairs) { atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand); }
+  }
+}
+
 // ---- decode: key -> fs_placement (one warp per request, lanes over phi for f_req) ----------
 __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
                                                           const fs_request* __restrict__ reqs,
@@ -155,6 +419,13 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
 
 }  // namespace
 
+int fsk_place_smem_attr() {
+  const int bytes = (int)sizeof(DenseSmem);
+  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  return e;
+}
+
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
               const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (R <= 0) return 0;
@@ -165,20 +436,40 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
   }
-  // split the GPUs of one request over several warps when R alone cannot fill 148 SMs
-  const long long want_warps = 148LL * 32;
-  int nsplit = 1;
-  if (R < want_warps) nsplit = (int)((want_warps + R - 1) / R);
-  if (nsplit > v.K) nsplit = v.K > 0 ? v.K : 1;
-  const int kchunk = (v.K + nsplit - 1) / nsplit;
-  nsplit = (v.K + kchunk - 1) / (kchunk > 0 ? kchunk : 1);
-  if (nsplit < 1) nsplit = 1;
-  const long long warps = (long long)R * nsplit;
+  const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= 64 && !sc.force_generic;
   fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
-  place_generic_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(v, R, reqs, sc.keys, nsplit,
-                                                                   kchunk, sc.stats);
+  if (dense_ok) {
+    // persistent blocks: 2 per SM; when the batch is small, slice the GPU chunks over blocks
+    const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS, nchunk = v.Kpad / FS_CHUNK;
+    const int max_blocks = sc.sm_count * 2;
+    int nslice = 1;
+    if (nbatch < max_blocks) nslice = min(nchunk, (max_blocks + nbatch - 1) / nbatch);
+    const int cps = (nchunk + nslice - 1) / nslice;
+    nslice = (nchunk + cps - 1) / cps;
+    int streams = min(nbatch, max(1, max_blocks / nslice));
+    const int grid = streams * nslice;
+    const size_t smem = sizeof(DenseSmem);
+    if (v.d.F <= 32)
+      place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.stats);
+    else
+      place_dense_kernel<2><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.stats);
+    ++launches;
+    place_warm_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, sc.warm_off, sc.warm_item, sc.stats);
+    ++launches;
+  } else {
+    // split the GPUs of one request over several warps when R alone cannot fill the SMs
+    const long long want_warps = (long long)sc.sm_count * 32;
+    int nsplit = 1;
+    if (R < want_warps) nsplit = (int)((want_warps + R - 1) / R);
+    if (nsplit > v.K) nsplit = v.K;
+    const int kchunk = (v.K + nsplit - 1) / nsplit;
+    nsplit = (v.K + kchunk - 1) / kchunk;
+    const long long warps = (long long)R * nsplit;
+    place_generic_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(v, R, reqs, sc.keys, nsplit,
+                                                                     kchunk, sc.stats);
+    ++launches;
+  }
   fs_tm_end(tm, FS_T_PLACE_SCORE, st);
-  ++launches;
   fs_tm_beg(tm, FS_T_PLACE_DECODE, st);
   place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
   fs_tm_end(tm, FS_T_PLACE_DECODE, st);

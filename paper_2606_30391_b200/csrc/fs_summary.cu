@@ -30,11 +30,23 @@ __device__ __forceinline__ bool state_valid(const fs_gpu_state& g, const FsDimsD
 
 // one warp per GPU, lanes over phi
 __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __restrict__ ginfo,
-                                                     float* __restrict__ gA) {
+                                                     float* __restrict__ gA,
+                                                     FsGpuRec* __restrict__ grec,
+                                                     float* __restrict__ gA0) {
   const int lane = threadIdx.x & 31;
   const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (k >= v.K) return;
+  if (k >= v.Kpad) return;
   const FsDimsDev d = v.d;
+  if (k >= v.K) {            // padding rows of the staged arrays: never a candidate
+    for (int phi = lane; phi < v.FT; phi += 32) gA0[(size_t)k * v.FT + phi] = FS_INF;
+    if (lane == 0) {
+      FsGpuRec r; r.t_avail_ms = r.mem_free_mb = r.e_cur = 0.f; r.meta = 0;
+      for (int i = 0; i < FS_RMAX; ++i) r.model[i] = -1;
+      r._pad[0] = r._pad[1] = 0;
+      grec[k] = r;
+    }
+    return;
+  }
   const fs_gpu_state g = v.states[k];
   const bool valid = state_valid(g, d);
   const int n = valid ? g.n_res : 0;
@@ -71,9 +83,9 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
           }
         }
         A[var * d.F + phi] = ok ? acc : FS_INF;
-        if (var == 0) ok0 = ok;
+        if (var == 0) { ok0 = ok; gA0[(size_t)k * v.FT + phi] = ok ? acc : FS_INF; }
       }
-    }
+    } else if (phi < v.FT) gA0[(size_t)k * v.FT + phi] = FS_INF;
     const unsigned m = __ballot_sync(0xffffffffu, ok0);
     if (f_floor < 0 && m) f_floor = base + __ffs(m) - 1;
   }
@@ -95,6 +107,11 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     }
     gi.e_cur = ecur; gi.sm_free = n ? d.S - used : 0;
     ginfo[k] = gi;
+    FsGpuRec r; r.t_avail_ms = gi.t_avail_ms; r.mem_free_mb = gi.mem_free_mb; r.e_cur = ecur;
+    r.meta = (uint32_t)n | ((uint32_t)gi.sm_free << 8);
+    for (int i = 0; i < FS_RMAX; ++i) r.model[i] = gi.model[i];
+    r._pad[0] = r._pad[1] = 0;
+    grec[k] = r;
     if (!valid) fs_raise(v.flag, FS_FLAG_STATE);
   }
 }
@@ -135,11 +152,12 @@ __global__ void warm_fill_kernel(FsView v, const int32_t* __restrict__ off,
 
 }  // namespace
 
-int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, cudaStream_t st, FsTimers* tm) {
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
+                cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int wpb = 4;
   fs_tm_beg(tm, FS_T_SUMMARY, st);
-  summary_kernel<<<(v.K + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA);
+  summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0);
   fs_tm_end(tm, FS_T_SUMMARY, st);
   return 1;
 }

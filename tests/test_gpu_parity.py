@@ -103,6 +103,32 @@ def test_edge_cases(ctx):
     assert got["gpu"][3] == -1 and np.isinf(got["energy_mj"][3]) and got["flat"][3] == 0xFFFFFFFF
 
 
+@pytest.mark.parametrize("seed", range(4))
+def test_ttft_deadline_on_the_rounding_boundary(ctx, seed):
+    """slo_ttft set to fl(wait + t0) of a real candidate, and to its float neighbours, so that the
+    deadline test sits exactly on a rounding boundary (the dense kernel's threshold T*)."""
+    cl = synth.make_custom(seed=300 + seed, K=40, M=6, F=48, S=12, B=16, R=192, lo=1, hi=3)
+    st = synth.Stream(seed, "boundary")
+    f32 = np.float32
+    for r in range(cl.R):
+        rq = cl.requests[r]
+        m, L = int(rq["model"]), int(rq["L"])
+        k = int(st.randint(1, 0, cl.K - 1)[0]); sg = int(st.randint(1, 0, cl.S - 1)[0])
+        phi = int(st.randint(1, 0, cl.F - 1)[0])
+        g = cl.states[k]
+        cold = m not in [int(g["t"][i]["model"]) for i in range(int(g["n_res"]))]
+        wait = f32(g["t_avail_ms"]) + (f32(cl.models["load_ms"][m]) if cold else f32(0))
+        b0 = min(L, cl.B) - 1
+        t0 = f32(-(-L // (b0 + 1))) * cl.lat[m, 0, phi, sg, b0]
+        edge = f32(f32(wait) + f32(t0))
+        which = r % 3
+        cl.requests["slo_ttft_ms"][r] = [edge, np.nextafter(edge, f32(-np.inf)), np.nextafter(edge, f32(np.inf))][which]
+        if r % 7 == 0:                                  # tiny waits: t0 dominates the sum
+            cl.states["t_avail_ms"][k] = f32(1e-6) * f32(r + 1)
+    cl.models["load_ms"][::2] = 0.0                     # wait can be exactly t_avail
+    _check_all(ctx, cl, local=False, consol=False)
+
+
 def test_empty_inputs(ctx):
     cl = synth.make_custom(seed=5, K=4, M=2, F=4, S=4, B=4, R=8)
     ctx.load_cluster(cl)
