@@ -206,7 +206,10 @@ def run_ours(args):
     wall = time.perf_counter() - wall0
     launches = ctx.launch_count - l0
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
-    pairs, cand_exec = ctx.last_place_stats()
+    pstats = ctx.last_place_stats()
+    pairs = pstats["dense_pairs"] + pstats["warm_pairs"]
+    cand_exec = pstats["dense_candidates"] + pstats["warm_candidates"]
+    cand_dense = pstats["dense_candidates"]
 
     # end to end through the C ABI with pinned host buffers
     h_states = torch.from_numpy(cl.states.view(np.uint8).reshape(-1).copy()).pin_memory()
@@ -248,7 +251,7 @@ def run_ours(args):
     sm_clk_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     alu_peak = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * sm_clk_hz          # lane-instructions / s
     score_ms = float(np.mean(kt.get("place_score", [float("nan")])))
-    achieved = OPS_PER_CANDIDATE * cand_exec / (score_ms * 1e-3)
+    achieved = OPS_PER_CANDIDATE * cand_dense / (score_ms * 1e-3)
     place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
     ok = place["gpu"] >= 0
     line = {
@@ -257,7 +260,7 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic", "config": _config(cl, args),
         "decisions_per_sec": ws * (cl.R + cl.K) * steps / (dev_ms * 1e-3),
         "placement_decisions_per_sec": ws * cl.R * steps / (dev_ms * 1e-3),
-        "executed_candidates_per_step": cand_exec, "eligible_pairs_per_step": pairs,
+        "executed_candidates_per_step": cand_exec, "eligible_pairs_per_step": pairs, "place_stats": pstats,
         "nominal_candidates_per_step": nominal,
         "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
         "wall_ms_per_step_incl_flush": wall_ms / steps,
@@ -269,7 +272,7 @@ def run_ours(args):
                      "peak": alu_peak / 1e12, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
                      "traffic": None,
                      "note": f"{OPS_PER_CANDIDATE:g} lane-ops per evaluated candidate (DESIGN.md) x "
-                             f"{cand_exec} candidates / {score_ms:.3f} ms; peak = 148 SMs x 128 lanes/clk x "
+                             f"{cand_dense} dense-kernel candidates / {score_ms:.3f} ms; peak = 148 SMs x 128 lanes/clk x "
                              f"{sm_clk_hz / 1e6:.0f} MHz ({peak_src} sm_max_mhz)"},
         "degeneracy": {"placed_frac": float(ok.mean()),
                        "top_phi_share": float(np.bincount(place["phi"][ok]).max() / max(ok.sum(), 1)),

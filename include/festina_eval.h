@@ -180,22 +180,25 @@ const char* fs_strerror(int code);
 int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed runtime call */
 /* Kernels launched by this context since creation (bench.py's gpu_launches counter).     */
 uint64_t fs_launch_count(const fs_ctx* ctx);
-/* Nominal work of the last fs_place_batch: eligible (request, GPU) pairs and candidates
- * (sum of sm_free*F over them), counted on the device.  Valid after synchronising.        */
-int fs_last_place_stats(fs_ctx* ctx, uint64_t* pairs, uint64_t* candidates);
+/* Work of the last fs_place_batch, counted on the device (valid after synchronising; this call
+ * synchronises the device): out[0] = eligible (request, GPU) pairs scored by the dense (cold)
+ * kernel or the generic kernel, out[1] = their candidates (sum of sm_free*F), out[2], out[3] =
+ * the same for the warm-pair kernel.                                                       */
+int fs_last_place_stats(fs_ctx* ctx, uint64_t out[4]);
 
 /* Per-kernel device timing for measurement (bench.py's roofline line).  fs_set_timing(ctx, 1)
  * makes every later call record CUDA event pairs on its stream around its kernels;
  * fs_get_timing waits for them and writes the duration in ms of the MOST RECENT launch of each
  * timed kernel into ms[0..n) (-1 = never launched), indexed by fs_timer.                    */
 typedef enum {
-  FS_TIMER_PLACE_SCORE = 0, /* candidate scoring + argmin of fs_place_batch          */
+  FS_TIMER_PLACE_SCORE = 0, /* fs_place_batch: dense candidate scoring + argmin       */
   FS_TIMER_PLACE_DECODE,    /* key -> fs_placement                                   */
   FS_TIMER_SUMMARY,         /* co-resident summary of fs_set_gpu_state               */
   FS_TIMER_LOCAL_SLOT,      /* per-slot batch search of fs_local_config              */
   FS_TIMER_LOCAL_SPLIT,     /* SM-split search of fs_local_config                    */
   FS_TIMER_CONSOL_AGG,      /* per-tenant minimum shares of fs_consolidate           */
   FS_TIMER_CONSOL_PAIR,     /* pair scoring of fs_consolidate                        */
+  FS_TIMER_PLACE_WARM,      /* fs_place_batch: pairs whose model is already resident */
   FS_TIMER_COUNT
 } fs_timer;
 int fs_set_timing(fs_ctx* ctx, int on);

@@ -26,7 +26,7 @@ SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "f
            "fs_local_config", "fs_consolidate", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
-          "consol_pair")
+          "consol_pair", "place_warm")
 
 
 class FsDims(C.Structure):
@@ -70,7 +70,7 @@ def lib() -> C.CDLL:
     L.fs_last_cuda_error.argtypes = [vp]
     L.fs_launch_count.argtypes = [vp]
     L.fs_launch_count.restype = C.c_uint64
-    L.fs_last_place_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.fs_last_place_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
     L.fs_set_timing.argtypes = [vp, C.c_int]
     L.fs_get_timing.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
     for name in SYMBOLS:
@@ -204,10 +204,12 @@ class Festina:
     def launch_count(self) -> int:
         return int(lib().fs_launch_count(self._h))
 
-    def last_place_stats(self):
-        a, b = C.c_uint64(0), C.c_uint64(0)
-        self._check(lib().fs_last_place_stats(self._h, C.byref(a), C.byref(b)), "fs_last_place_stats")
-        return int(a.value), int(b.value)
+    def last_place_stats(self) -> dict:
+        """Eligible pairs / candidates the last fs_place_batch evaluated, dense and warm kernels."""
+        o = (C.c_uint64 * 4)()
+        self._check(lib().fs_last_place_stats(self._h, o), "fs_last_place_stats")
+        return {"dense_pairs": int(o[0]), "dense_candidates": int(o[1]), "warm_pairs": int(o[2]),
+                "warm_candidates": int(o[3])}
 
     def set_timing(self, on: bool = True):
         self._check(lib().fs_set_timing(self._h, int(on)), "fs_set_timing")

@@ -27,6 +27,7 @@ struct fs_ctx {
   int32_t *warm_off = nullptr, *warm_cursor = nullptr; uint32_t* warm_item = nullptr; int warm_m_cap = 0;
   // placement scratch
   int r_cap = 0; unsigned long long* keys = nullptr; unsigned long long* stats = nullptr;
+  unsigned int* ctr = nullptr;
   fs_request* reqs_dev = nullptr; fs_placement* place_dev = nullptr;
   // local scratch
   size_t local_cap = 0; int n_cap = 0; float* G = nullptr; uint8_t* Bst = nullptr;
@@ -130,13 +131,13 @@ int fs_create(fs_ctx** out, int cuda_device) {
   if (cudaSetDevice(cuda_device) != cudaSuccess ||
       cudaHostAlloc((void**)&c->flag_host, sizeof(int) * FS_NFLAGS, cudaHostAllocMapped) != cudaSuccess ||
       cudaHostGetDevicePointer((void**)&c->flag_dev, c->flag_host, 0) != cudaSuccess ||
-      cudaMalloc((void**)&c->stats, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMalloc((void**)&c->stats, 4 * sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return FS_ERR_CUDA;
   }
   std::memset(c->flag_host, 0, sizeof(int) * FS_NFLAGS);
-  cudaMemset(c->stats, 0, 2 * sizeof(unsigned long long));
+  cudaMemset(c->stats, 0, 4 * sizeof(unsigned long long));
   fsk_local_smem_attr();
   fsk_place_smem_attr();
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
@@ -150,7 +151,7 @@ int fs_destroy(fs_ctx* c) {
   cudaSetDevice(c->dev);
   cudaDeviceSynchronize();
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
-                  c->ginfo, c->gA, c->grec, c->gA0, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
+                  c->ginfo, c->gA, c->grec, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -217,6 +218,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (K > c->k_cap) {
     FS_TRY(grow(c, c->states, (size_t)K)); FS_TRY(grow(c, c->ginfo, (size_t)K));
     FS_TRY(grow(c, c->grec, (size_t)K + FS_CHUNK));
+    FS_TRY(grow(c, c->ctr, (size_t)K / FS_CHUNK + 2));
     FS_TRY(grow(c, c->warm_item, (size_t)K * FS_RMAX));
     c->k_cap = K; c->consol_cap = 0;
   }
@@ -260,7 +262,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
-  FsPlaceScratch sc{c->keys, c->stats, c->warm_off, c->warm_item, c->sm_count, c->force_generic};
+  FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
@@ -376,12 +378,12 @@ int fs_get_timing(fs_ctx* c, float* ms, int n) {
   return FS_OK;
 }
 
-int fs_last_place_stats(fs_ctx* c, uint64_t* pairs, uint64_t* candidates) {
-  if (!c || !pairs || !candidates) return FS_ERR_ARG;
-  unsigned long long h[2] = {0, 0};
+int fs_last_place_stats(fs_ctx* c, uint64_t out[4]) {
+  if (!c || !out) return FS_ERR_ARG;
+  unsigned long long h[4] = {0, 0, 0, 0};
   FS_CUDA(c, cudaSetDevice(c->dev));
   FS_CUDA(c, cudaMemcpy(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost));
-  *pairs = h[0]; *candidates = h[1];
+  for (int i = 0; i < 4; ++i) out[i] = h[i];
   return FS_OK;
 }
 

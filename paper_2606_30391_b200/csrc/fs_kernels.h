@@ -8,7 +8,7 @@
 // Optional per-kernel timing (fs_set_timing): CUDA event pairs recorded on the caller's stream
 // around the kernels bench.py reports rooflines for.  NULL = no timing.
 enum { FS_T_PLACE_SCORE = 0, FS_T_PLACE_DECODE, FS_T_SUMMARY, FS_T_LOCAL_SLOT, FS_T_LOCAL_SPLIT,
-       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_COUNT };
+       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_PLACE_WARM, FS_T_COUNT };
 struct FsTimers {
   cudaEvent_t beg[FS_T_COUNT], end[FS_T_COUNT];
   bool used[FS_T_COUNT];
@@ -46,7 +46,8 @@ int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, fl
 // fs_place.cu — placement scoring + 64-bit-key argmin + decode
 struct FsPlaceScratch {
   unsigned long long* keys;        // [R]
-  unsigned long long* stats;       // [2]: eligible pairs, candidates
+  unsigned long long* stats;       // [4]: dense pairs, dense candidates, warm pairs, warm candidates
+  unsigned int* ctr;               // [nslice <= Kpad/32] dynamic request counters of the dense kernel
   // bucketing of GPUs by model (built by fs_set_gpu_state): warm lists
   const int32_t* warm_off;         // [M+1]
   const uint32_t* warm_item;       // [sum n_res]: k*4 + j

@@ -139,8 +139,8 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
 // eligibility and T* for ONE GPU of the chunk, then the warp sweeps the eligible GPUs.
 // The lowest flat index among equal minima is recovered exactly at the end (see below).
 // =============================================================================================
-constexpr int DENSE_WARPS = 8;
-constexpr int DENSE_STAGES = 4;
+constexpr int DENSE_WARPS = 16;
+constexpr int DENSE_SMEM_MAX = 200 * 1024;   // of the 227 KB a block may use
 constexpr int DENSE_S = 16;
 
 // largest t >= 0 with fl(w + t) <= slo, or -1 if there is none.  fl(w + .) is monotone, so the
@@ -174,95 +174,84 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
   return tstar_bisect(w, slo);
 }
 
-struct DenseSmem {
-  alignas(128) float a0[DENSE_STAGES][FS_CHUNK * 64];   // [stage][gpu][FT] rows (FT = 32*NPHI)
-  alignas(16) FsGpuRec rec[DENSE_STAGES][FS_CHUNK];
-  alignas(16) float4 wb[DENSE_WARPS][FS_CHUNK];         // per warp: {T*, Ecur, sm_free, -}
-  alignas(8) uint64_t full[DENSE_STAGES];
-  alignas(8) uint64_t empty[DENSE_STAGES];
-};
+// Shared memory of one block: its SLICE of the GPUs stays resident for the whole kernel, so the
+// warps never synchronise with each other after the initial TMA fill.
+//   a0  [KS][FT] floats   co-resident energy rows (variant 0), FT = 32*NPHI
+//   rec [KS]              compact GPU records
+//   wb  [DENSE_WARPS][32] per warp: {T*, Ecur, sm_free, -} of the chunk being swept
+__host__ __device__ inline size_t dense_smem_bytes(int KS, int FT) {
+  return (size_t)KS * FT * sizeof(float) + (size_t)KS * sizeof(FsGpuRec) +
+         (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) + 16;
+}
 
 template <int NPHI>
-__global__ void __launch_bounds__(DENSE_WARPS * 32, 2)
+__global__ void __launch_bounds__(DENSE_WARPS * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
-                   unsigned long long* __restrict__ stats) {
+                   unsigned int* __restrict__ ctr, unsigned long long* __restrict__ stats) {
   extern __shared__ __align__(128) unsigned char dense_smem_raw[];
-  DenseSmem& sm = *reinterpret_cast<DenseSmem*>(dense_smem_raw);
   constexpr int FT = 32 * NPHI;
   const FsDimsDev d = v.d;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int nchunk_all = v.Kpad / FS_CHUNK;
   const int slice = blockIdx.x % nslice;
   const int c0 = slice * chunks_per_slice, c1 = min(nchunk_all, c0 + chunks_per_slice);
-  const int nchunk = c1 - c0;
-  const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS;
-  const int b_first = blockIdx.x / nslice, b_stride = gridDim.x / nslice;
-  const int my_batches = b_first < nbatch ? (nbatch - b_first + b_stride - 1) / b_stride : 0;
-  const long long total = (long long)my_batches * nchunk;
-  const uint32_t bytes_a0 = FS_CHUNK * FT * sizeof(float), bytes_rec = FS_CHUNK * sizeof(FsGpuRec);
+  const int nchunk = c1 - c0, KS = nchunk * FS_CHUNK, KSmax = chunks_per_slice * FS_CHUNK;
+  float* s_a0 = reinterpret_cast<float*>(dense_smem_raw);
+  FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw + (size_t)KSmax * FT * sizeof(float));
+  float4* s_wb = reinterpret_cast<float4*>(dense_smem_raw + (size_t)KSmax * (FT * sizeof(float) + sizeof(FsGpuRec)));
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_wb + DENSE_WARPS * FS_CHUNK);
 
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < DENSE_STAGES; ++s) { fs_mbar_init(&sm.full[s], 1); fs_mbar_init(&sm.empty[s], DENSE_WARPS); }
-    fs_mbar_fence_init();
-  }
+  // ---- stage this block's GPU slice once: 1-D TMA bulk copies completing on one mbarrier --------
+  if (threadIdx.x == 0) { fs_mbar_init(s_bar, 1); fs_mbar_fence_init(); }
   __syncthreads();
-  auto issue = [&](long long n) {          // producer: stage chunk number n of this block's stream
-    const int s = (int)(n % DENSE_STAGES);
-    fs_mbar_wait(&sm.empty[s], (uint32_t)(((n / DENSE_STAGES) & 1) ^ 1));
-    const int chunk = c0 + (int)(n % nchunk);
-    fs_mbar_expect_tx(&sm.full[s], bytes_a0 + bytes_rec);
-    fs_tma_load_1d(&sm.a0[s][0], v.gA0 + (size_t)chunk * FS_CHUNK * FT, bytes_a0, &sm.full[s]);
-    fs_tma_load_1d(&sm.rec[s][0], v.grec + (size_t)chunk * FS_CHUNK, bytes_rec, &sm.full[s]);
-  };
-  if (threadIdx.x == 0)
-    for (long long n = 0; n < total && n < DENSE_STAGES - 1; ++n) issue(n);
+  if (threadIdx.x == 0) {
+    const uint32_t bytes_a0 = (uint32_t)KS * FT * sizeof(float), bytes_rec = (uint32_t)KS * sizeof(FsGpuRec);
+    fs_mbar_expect_tx(s_bar, bytes_a0 + bytes_rec);
+    const char* src = reinterpret_cast<const char*>(v.gA0 + (size_t)c0 * FS_CHUNK * FT);
+    char* dst = reinterpret_cast<char*>(s_a0);
+    for (uint32_t off = 0; off < bytes_a0; off += 32768u)
+      fs_tma_load_1d(dst + off, src + off, min(32768u, bytes_a0 - off), s_bar);
+    fs_tma_load_1d(s_rec, v.grec + (size_t)c0 * FS_CHUNK, bytes_rec, s_bar);
+  }
+  fs_mbar_wait(s_bar, 0);
 
-  // per-request registers
-  float t0[DENSE_S][NPHI], er[DENSE_S][NPHI];
-  ReqCtx c; bool active = false; int r = -1;
-  float best = FS_INF; int bestk = -1;
+  float4* wb = s_wb + warp * FS_CHUNK;
   unsigned long long npairs = 0, ncand = 0;
-
-  for (long long it = 0; it < total; ++it) {
-    const int ci = (int)(it % nchunk);
-    if (ci == 0) {
-      // ---- phase A: new request for this warp ------------------------------------------------
-      r = (b_first + (int)(it / nchunk) * b_stride) * DENSE_WARPS + warp;
-      active = r < R;
-      best = FS_INF; bestk = -1;
-      if (active) {
-        c = make_req(v, reqs[r]);
-        if (!c.valid) { active = false; if (lane == 0 && slice == 0) fs_raise(v.flag, FS_FLAG_REQUEST); }
-      }
-      if (active) {
-        const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
-        const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
-        const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
+  for (;;) {
+    // ---- next request of this slice: dynamic, one atomic per warp ----------------------------
+    int r = 0;
+    if (lane == 0) r = (int)atomicAdd(&ctr[slice], 1u);
+    r = __shfl_sync(0xffffffffu, r, 0);
+    if (r >= R) break;
+    const ReqCtx c = make_req(v, reqs[r]);
+    if (!c.valid) { if (lane == 0 && slice == 0) fs_raise(v.flag, FS_FLAG_REQUEST); continue; }
+    // ---- phase A: the request's (sigma, phi) tiles in registers -------------------------------
+    float t0[DENSE_S][NPHI], er[DENSE_S][NPHI];
+    {
+      const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
+      const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
+      const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
 #pragma unroll
-        for (int s = 0; s < DENSE_S; ++s)
+      for (int s = 0; s < DENSE_S; ++s)
 #pragma unroll
-          for (int i = 0; i < NPHI; ++i) {
-            const int phi = lane * NPHI + i;
-            float tt = FS_INF, ee = FS_INF;
-            if (s < d.S && phi < d.F) {
-              const int o = s * d.F + phi;
-              float e0 = 0.f, e1 = 0.f; bool ok1 = true; tt = 0.f;
-              if (c.L > 0) { tt = __fmul_rn(fr0, l0[o]); e0 = __fmul_rn(tt, p0[o]); }
-              if (c.O > 0) { const float la = l1[o]; ok1 = la <= c.slo_tbt; e1 = __fmul_rn(__fmul_rn(fO, la), p1[o]); }
-              ee = ok1 ? __fadd_rn(e0, e1) : FS_INF;
-            }
-            t0[s][i] = tt; er[s][i] = ee;
+        for (int i = 0; i < NPHI; ++i) {
+          const int phi = lane * NPHI + i;
+          float tt = FS_INF, ee = FS_INF;
+          if (s < d.S && phi < d.F) {
+            const int o = s * d.F + phi;
+            float e0 = 0.f, e1 = 0.f; bool ok1 = true; tt = 0.f;
+            if (c.L > 0) { tt = __fmul_rn(fr0, l0[o]); e0 = __fmul_rn(tt, p0[o]); }
+            if (c.O > 0) { const float la = l1[o]; ok1 = la <= c.slo_tbt; e1 = __fmul_rn(__fmul_rn(fO, la), p1[o]); }
+            ee = ok1 ? __fadd_rn(e0, e1) : FS_INF;
           }
-      }
+          t0[s][i] = tt; er[s][i] = ee;
+        }
     }
-    if (threadIdx.x == 0 && it + DENSE_STAGES - 1 < total) issue(it + DENSE_STAGES - 1);
-    __syncwarp();
-    const int st = (int)(it % DENSE_STAGES);
-    fs_mbar_wait(&sm.full[st], (uint32_t)((it / DENSE_STAGES) & 1));
-    if (active) {
+    float best = FS_INF; int bestk = -1;
+    for (int ci = 0; ci < nchunk; ++ci) {
       // ---- eligibility + T*: lane <-> one GPU of the chunk ------------------------------------
-      const FsGpuRec g = sm.rec[st][lane];
+      const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
       const int n_res = g.meta & 0xFF, smf = (g.meta >> 8) & 0xFF;
       bool el = n_res >= 1 && n_res < FS_RMAX && smf >= 1 && (c.mem <= g.mem_free_mb);
 #pragma unroll
@@ -272,14 +261,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         T = c.L > 0 ? fs_tstar(__fadd_rn(g.t_avail_ms, c.load_ms), c.slo_ttft) : FS_INF;
         npairs += 1; ncand += (unsigned long long)smf * d.F;
       }
-      sm.wb[warp][lane] = make_float4(T, g.e_cur, __int_as_float(smf), 0.f);
+      __syncwarp();
+      wb[lane] = make_float4(T, g.e_cur, __int_as_float(smf), 0.f);
       unsigned mask = __ballot_sync(0xffffffffu, el && T >= 0.0f);
       __syncwarp();
       // ---- sweep the eligible GPUs of the chunk -------------------------------------------------
-      const int kbase = (c0 + ci) * FS_CHUNK;
       while (mask) {
         const int g_i = __ffs(mask) - 1; mask &= mask - 1;
-        const float4 w = sm.wb[warp][g_i];
+        const float4 w = wb[g_i];
         const float Tst = w.x; const int sfree = __float_as_int(w.z);
         float m[NPHI];
 #pragma unroll
@@ -298,45 +287,38 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           case 1: FS_DENSE_STEP(0)
         }
 #undef FS_DENSE_STEP
-        const float* arow = &sm.a0[st][g_i * FT + lane * NPHI];
+        const float* arow = s_a0 + (size_t)(ci * FS_CHUNK + g_i) * FT + lane * NPHI;
         float x = FS_INF;
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
         const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
-        if (dE < best) { best = dE; bestk = kbase + g_i; }
+        if (dE < best) { best = dE; bestk = ci * FS_CHUNK + g_i; }
       }
     }
-    __syncwarp();
-    if (lane == 0) fs_mbar_arrive(&sm.empty[st]);
-
-    if (ci == nchunk - 1 && active) {
-      // ---- recovery: lowest flat index among the candidates that attain the minimum -----------
-      unsigned long long key = FS_KEY_NONE;
-      if (bestk >= 0) {
-        const FsGpuRec g = v.grec[bestk];
-        const int smf = (g.meta >> 8) & 0xFF;
-        const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
-        float a[NPHI];
+    // ---- recovery: lowest flat index among the candidates that attain the minimum -------------
+    unsigned long long key = FS_KEY_NONE;
+    if (bestk >= 0) {
+      const FsGpuRec g = s_rec[bestk];
+      const int smf = (g.meta >> 8) & 0xFF;
+      const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
+      const int kglob = c0 * FS_CHUNK + bestk;
+      bool found = false; uint32_t flat = 0xFFFFFFFFu;
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) a[i] = v.gA0[(size_t)bestk * FT + lane * NPHI + i];
-        bool found = false; uint32_t flat = 0xFFFFFFFFu;
+      for (int s = 0; s < DENSE_S; ++s)
 #pragma unroll
-        for (int s = 0; s < DENSE_S; ++s)
-#pragma unroll
-          for (int i = 0; i < NPHI; ++i) {
-            const bool feas = s < smf && (c.L == 0 || __fadd_rn(wait, t0[s][i]) <= c.slo_ttft);
-            const float dE = __fsub_rn(__fadd_rn(a[i], er[s][i]), g.e_cur);
-            if (!found && feas && dE == best) {
-              found = true; flat = (uint32_t)((bestk * d.S + s) * d.F + lane * NPHI + i);
-            }
+        for (int i = 0; i < NPHI; ++i) {
+          const bool feas = s < smf && (c.L == 0 || __fadd_rn(wait, t0[s][i]) <= c.slo_ttft);
+          const float dE = __fsub_rn(__fadd_rn(s_a0[(size_t)bestk * FT + lane * NPHI + i], er[s][i]), g.e_cur);
+          if (!found && feas && dE == best) {
+            found = true; flat = (uint32_t)((kglob * d.S + s) * d.F + lane * NPHI + i);
           }
-        if (found) key = fs_make_key(best, flat);
-      }
-      key = fs_warp_min_key(key);
-      if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
+        }
+      if (found) key = fs_make_key(best, flat);
     }
+    key = fs_warp_min_key(key);
+    if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
   }
-  // work statistics (nominal candidates actually evaluated)
+  // work statistics (eligible pairs and their candidates, by the oracle's definition)
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
@@ -380,7 +362,7 @@ __global__ void __launch_bounds__(256) place_warm_kernel(FsView v, int R,
   key = fs_warp_min_key(key);
   if (lane == 0) {
     if (key != FS_KEY_NONE) atomicMin(&keys[r], key);
-    if (stats && npairs) { atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand); }
+    if (stats && npairs) { atomicAdd(&stats[2], npairs); atomicAdd(&stats[3], ncand); }
   }
 }
 
@@ -420,9 +402,8 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
 }  // namespace
 
 int fsk_place_smem_attr() {
-  const int bytes = (int)sizeof(DenseSmem);
-  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   return e;
 }
 
@@ -431,7 +412,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   if (R <= 0) return 0;
   int launches = 0;
   cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-  cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 2, st);
+  cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 4, st);
   if (v.K <= 0) {
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
@@ -439,22 +420,30 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= 64 && !sc.force_generic;
   fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
   if (dense_ok) {
-    // persistent blocks: 2 per SM; when the batch is small, slice the GPU chunks over blocks
-    const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS, nchunk = v.Kpad / FS_CHUNK;
-    const int max_blocks = sc.sm_count * 2;
-    int nslice = 1;
-    if (nbatch < max_blocks) nslice = min(nchunk, (max_blocks + nbatch - 1) / nbatch);
+    // one persistent block per SM; each holds a slice of the GPUs in shared memory.  The number
+    // of slices is what the slice size forces, raised when R alone cannot occupy every SM.
+    const int FT = v.d.F <= 32 ? 32 : 64;
+    const int nchunk = v.Kpad / FS_CHUNK;
+    const size_t fixed = dense_smem_bytes(0, FT), per_chunk = dense_smem_bytes(FS_CHUNK, FT) - fixed;
+    const int max_cps = (int)((DENSE_SMEM_MAX - fixed) / per_chunk);
+    int nslice = (nchunk + max_cps - 1) / max_cps;
+    const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS;
+    if (nbatch * nslice < sc.sm_count) nslice = min(nchunk, (sc.sm_count + nbatch - 1) / nbatch);
     const int cps = (nchunk + nslice - 1) / nslice;
     nslice = (nchunk + cps - 1) / cps;
-    int streams = min(nbatch, max(1, max_blocks / nslice));
+    const int streams = max(1, min(nbatch, sc.sm_count / nslice));
     const int grid = streams * nslice;
-    const size_t smem = sizeof(DenseSmem);
-    if (v.d.F <= 32)
-      place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.stats);
+    const size_t smem = dense_smem_bytes(cps * FS_CHUNK, FT);
+    cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nslice, st);
+    if (FT == 32)
+      place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.stats);
     else
-      place_dense_kernel<2><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.stats);
+      place_dense_kernel<2><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.stats);
     ++launches;
+    fs_tm_end(tm, FS_T_PLACE_SCORE, st);
+    fs_tm_beg(tm, FS_T_PLACE_WARM, st);
     place_warm_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, sc.warm_off, sc.warm_item, sc.stats);
+    fs_tm_end(tm, FS_T_PLACE_WARM, st);
     ++launches;
   } else {
     // split the GPUs of one request over several warps when R alone cannot fill the SMs
@@ -468,8 +457,8 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     place_generic_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(v, R, reqs, sc.keys, nsplit,
                                                                      kchunk, sc.stats);
     ++launches;
+    fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   }
-  fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   fs_tm_beg(tm, FS_T_PLACE_DECODE, st);
   place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
   fs_tm_end(tm, FS_T_PLACE_DECODE, st);
