@@ -327,54 +327,219 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   if (lane == 0 && stats && npairs) { atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand); }
 }
 
-// ---- warm pairs: the request's model is resident on the GPU (decode bucket and co-resident
-// variant depend on the GPU), evaluated candidate by candidate from the planes.  One warp per
-// request walks the (GPU, slot) list of its model; when `all_pairs` it walks every GPU instead.
-__global__ void __launch_bounds__(256) place_warm_kernel(FsView v, int R,
-                                                        const fs_request* __restrict__ reqs,
-                                                        unsigned long long* __restrict__ keys,
-                                                        const int32_t* __restrict__ warm_off,
-                                                        const uint32_t* __restrict__ warm_item,
-                                                        unsigned long long* __restrict__ stats) {
-  const int lane = threadIdx.x & 31;
-  const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+// =============================================================================================
+// Warm pairs: the request's model is resident on the GPU, so the decode bucket (beta_j1+1), the
+// co-resident variant (1+j), wait (= T_avail, no weight load) and the decode plane depend on the
+// GPU.  Organised ITEM-major: an item is one (GPU k, slot j) of the per-model lists built by
+// fs_set_gpu_state.  A warp owns (item, block of 32 frequencies) and keeps the four plane columns
+// it needs in registers: LAT/POW of (m, decode, br1) and of (m, prefill, B-1) — the prefill bucket
+// of every request with L >= B; shorter prompts read their own prefill plane through L2.
+// It then walks the requests of model m (bucketed per call), 32 at a time: each lane prepares one
+// request (T*, rounds, eligibility), then the warp sweeps them.  Per candidate: 4 mul, 1 add,
+// 2 compares, 1 predicated min, all on registers.  Same monotone factorisation as the dense
+// kernel; the per-(item, request) minimum is reduced with redux.sync on the orderable value and
+// merged as (value, GPU) into wkeys[r] by atomicMin when it can still win; the decode kernel
+// turns the winning (request, GPU) into the lowest flat index.
+// =============================================================================================
+constexpr int WARM_WARPS = 4;
+constexpr int WARM_SLOTS = 4;      // warps that share the request list of one (item, phi block)
+
+struct __align__(16) WarmReq {     // what one request contributes, prepared by one lane
+  float T, fr0, fr1, tbt;          // T* for wait = T_avail; rounds as floats; slo_tbt (INF if O == 0)
+  int br0;                         // prefill bucket, -1 = the common plane B-1 held in registers
+  int r;                           // request index
+  uint32_t cur_hi;                 // high word of keys[r] when the chunk was prepared (pruning)
+  uint32_t _pad;
+};
+
+// bucket the requests of one call by model: counts -> offsets -> indices
+__global__ void req_count_kernel(const fs_request* __restrict__ reqs, int R, int M, int32_t* __restrict__ off) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= R) return;
-  const ReqCtx c = make_req(v, reqs[r]);
-  if (!c.valid) return;                        // flagged by the dense kernel
+  const int m = reqs[r].model;
+  if (m >= 0 && m < M) atomicAdd(&off[m + 1], 1);
+}
+// single-block inclusive scan of off[1..M] in place (off[0] = 0) and cursor[m] = 0
+__global__ void __launch_bounds__(1024) bucket_scan_kernel(int32_t* __restrict__ off, int32_t* __restrict__ cursor, int M) {
+  __shared__ int32_t part[1024];
+  const int t = threadIdx.x, per = (M + 1023) / 1024;
+  const int lo = min(M, t * per), hi = min(M, lo + per);
+  int32_t sum = 0;
+  for (int m = lo; m < hi; ++m) sum += off[m + 1];
+  part[t] = sum;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const int32_t add = t >= o ? part[t - o] : 0;
+    __syncthreads();
+    part[t] += add;
+    __syncthreads();
+  }
+  int32_t acc = part[t] - sum;
+  if (t == 0) off[0] = 0;
+  for (int m = lo; m < hi; ++m) { acc += off[m + 1]; off[m + 1] = acc; cursor[m] = 0; }
+}
+__global__ void req_fill_kernel(const fs_request* __restrict__ reqs, int R, int M,
+                                const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
+                                int32_t* __restrict__ idx) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= R) return;
+  const int m = reqs[r].model;
+  if (m >= 0 && m < M) idx[off[m] + atomicAdd(&cursor[m], 1)] = r;
+}
+
+__device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) {
+  uint32_t r;
+  asm volatile("redux.sync.min.u32 %0, %1, 0xffffffff;" : "=r"(r) : "r"(x));
+  return r;
+}
+
+__global__ void __launch_bounds__(WARM_WARPS * 32, 3)
+place_warm_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
+                  const unsigned long long* __restrict__ keys,
+                  unsigned long long* __restrict__ wkeys, const int32_t* __restrict__ warm_off,
+                  const uint32_t* __restrict__ warm_item, const int32_t* __restrict__ rb_off,
+                  const int32_t* __restrict__ rb_idx, int nphib,
+                  unsigned long long* __restrict__ stats) {
+  __shared__ WarmReq s_req[WARM_WARPS][32];
   const FsDimsDev d = v.d;
-  float best = FS_INF; uint32_t bflat = 0xFFFFFFFFu; bool have = false;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long gw = (long long)blockIdx.x * WARM_WARPS + warp;
+  const int slot = (int)(gw % WARM_SLOTS);
+  const int pb = (int)((gw / WARM_SLOTS) % nphib);
+  const long long item_i = gw / ((long long)WARM_SLOTS * nphib);
+  if (item_i >= warm_off[d.M]) return;
+  const uint32_t item = warm_item[item_i];
+  const int k = (int)(item >> 2), j = (int)(item & 3u);
+  const FsGpuInfo gi = v.ginfo[k];
+  const int m = gi.model[j], smf = gi.sm_free, br1 = gi.br1[j];
+  if (smf < 1 || br1 < 0) return;                       // no free SMs / decode bucket past the table
+  const int n_req = rb_off[m + 1] - rb_off[m];
+  if (n_req == 0) return;
+  const int phi = pb * 32 + lane;
+  const bool phi_ok = phi < d.F;
+  const int phic = phi_ok ? phi : 0;
+  // ---- item tiles in registers ------------------------------------------------------------------
+  float la0[DENSE_S], pw0[DENSE_S], la1[DENSE_S], pw1[DENSE_S];
+  {
+    const size_t o0 = fs_plane(d, m, 0, d.B - 1), o1 = fs_plane(d, m, 1, br1);
+#pragma unroll
+    for (int s = 0; s < DENSE_S; ++s) {
+      const bool in = s < smf && s < d.S;
+      const size_t o = (size_t)(in ? s : 0) * d.F + phic;
+      la0[s] = v.latT[o0 + o]; pw0[s] = v.powT[o0 + o];
+      la1[s] = v.latT[o1 + o]; pw1[s] = v.powT[o1 + o];
+    }
+  }
+  const float A = phi_ok ? v.gA[((size_t)k * FS_NVAR + 1 + j) * d.F + phic] : FS_INF;
+  const float ecur = gi.e_cur, kv = v.models[m].kv_mb_per_token;
+  WarmReq* wr = s_req[warp];
   unsigned long long npairs = 0, ncand = 0;
-  // items of one model are unordered: compare (value, flat) in full
-  for (int it = warm_off[c.m]; it < warm_off[c.m + 1]; ++it) {
-    const int k = (int)(warm_item[it] >> 2);
-    const PairCtx p = make_pair(v, c, v.ginfo[k]);
-    if (!p.ok) continue;
-    npairs += 1; ncand += (unsigned long long)p.smf * d.F;
-    for (int sg = 0; sg < p.smf; ++sg)
-      for (int phi = lane; phi < d.F; phi += 32) {
-        const Cand cd = eval_cand(v, c, p, k, sg, phi);
-        float dE = cd.dE; if (dE == 0.0f) dE = 0.0f;
-        const uint32_t flat = (uint32_t)((k * d.S + sg) * d.F + phi);
-        if (cd.ok && (!have || dE < best || (dE == best && flat < bflat))) { have = true; best = dE; bflat = flat; }
+
+  for (int cbase = slot * 32; cbase < n_req; cbase += WARM_SLOTS * 32) {
+    // ---- each lane prepares one request of the chunk ---------------------------------------------
+    bool el = false;
+    WarmReq q; q.T = -1.f; q.fr0 = q.fr1 = 0.f; q.tbt = 0.f; q.br0 = -1; q.r = -1; q.cur_hi = 0; q._pad = 0;
+    if (cbase + lane < n_req) {
+      const int r = rb_idx[rb_off[m] + cbase + lane];
+      const fs_request rq = reqs[r];
+      if (rq.L < (1u << 24) && rq.o_pred < (1u << 24)) {
+        const uint32_t O = (21u * rq.o_pred + 19u) / 20u;
+        const float mem = __fmul_rn(__uint2float_rn(rq.L + O), kv);
+        if (mem <= gi.mem_free_mb) {
+          el = true;
+          const uint32_t n0 = rq.L < (uint32_t)d.B ? rq.L : (uint32_t)d.B;
+          q.br0 = (n0 == (uint32_t)d.B || n0 == 0) ? -1 : (int)n0 - 1;
+          q.fr0 = n0 ? __uint2float_rn(fs_ceil_div(rq.L, n0)) : 0.0f;       // L == 0: t0 = e0 = 0
+          q.fr1 = __uint2float_rn(fs_ceil_div(O, (uint32_t)br1 + 1u));      // O == 0: e1 = 0
+          q.tbt = O > 0 ? rq.slo_tbt_ms : FS_INF;
+          q.T = rq.L > 0 ? fs_tstar(gi.t_avail_ms, rq.slo_ttft_ms) : FS_INF;
+          q.r = r; q.cur_hi = (uint32_t)(keys[r] >> 32);
+          if (pb == 0) { npairs += 1; ncand += (unsigned long long)smf * d.F; }
+        }
       }
+    }
+    __syncwarp();
+    wr[lane] = q;
+    unsigned mask = __ballot_sync(0xffffffffu, el && q.T >= 0.0f);
+    __syncwarp();
+    // ---- sweep the eligible requests -----------------------------------------------------------------
+    while (mask) {
+      const int qi = __ffs(mask) - 1; mask &= mask - 1;
+      const WarmReq w = wr[qi];
+      float mn = FS_INF;
+      if (w.br0 < 0) {
+#define FS_WARM_STEP(s) {                                                               \
+        const float t0 = __fmul_rn(w.fr0, la0[s]);                                      \
+        const float ee = __fadd_rn(__fmul_rn(t0, pw0[s]), __fmul_rn(__fmul_rn(w.fr1, la1[s]), pw1[s])); \
+        if (t0 <= w.T && la1[s] <= w.tbt) mn = fminf(mn, ee); }
+        switch (smf) {
+          default:
+          case 16: FS_WARM_STEP(15) case 15: FS_WARM_STEP(14) case 14: FS_WARM_STEP(13)
+          case 13: FS_WARM_STEP(12) case 12: FS_WARM_STEP(11) case 11: FS_WARM_STEP(10)
+          case 10: FS_WARM_STEP(9)  case 9: FS_WARM_STEP(8)   case 8: FS_WARM_STEP(7)
+          case 7: FS_WARM_STEP(6)   case 6: FS_WARM_STEP(5)   case 5: FS_WARM_STEP(4)
+          case 4: FS_WARM_STEP(3)   case 3: FS_WARM_STEP(2)   case 2: FS_WARM_STEP(1)
+          case 1: FS_WARM_STEP(0)
+        }
+#undef FS_WARM_STEP
+      } else {                                          // short prompt: its own prefill plane, via L2
+        const size_t o0 = fs_plane(d, m, 0, w.br0) + phic, o1 = fs_plane(d, m, 1, br1) + phic;
+#pragma unroll 1
+        for (int s = 0; s < smf; ++s) {
+          const float l1 = v.latT[o1 + (size_t)s * d.F];
+          const float t0 = __fmul_rn(w.fr0, v.latT[o0 + (size_t)s * d.F]);
+          const float ee = __fadd_rn(__fmul_rn(t0, v.powT[o0 + (size_t)s * d.F]),
+                                     __fmul_rn(__fmul_rn(w.fr1, l1), v.powT[o1 + (size_t)s * d.F]));
+          if (t0 <= w.T && l1 <= w.tbt) mn = fminf(mn, ee);
+        }
+      }
+      float dE = __fsub_rn(__fadd_rn(A, mn), ecur);     // monotone in mn
+      if (!(dE < FS_INF)) dE = FS_INF;                  // NaN / overflow: not a candidate
+      const uint32_t ord = fs_orderable(dE);
+      const uint32_t best = warp_min_u32(ord);
+      // (value, GPU) into the request's warm key: lowest k among equal minima, as the flat order
+      // wants; (sigma, phi) are recovered once per request by the decode kernel.
+      if (lane == 0 && best <= w.cur_hi && best < 0xFF800000u)
+        atomicMin(&wkeys[w.r], ((unsigned long long)best << 32) | (uint32_t)k);
+    }
   }
-  unsigned long long key = have ? fs_make_key(best, bflat) : FS_KEY_NONE;
-  key = fs_warp_min_key(key);
-  if (lane == 0) {
-    if (key != FS_KEY_NONE) atomicMin(&keys[r], key);
-    if (stats && npairs) { atomicAdd(&stats[2], npairs); atomicAdd(&stats[3], ncand); }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
+    ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
   }
+  if (lane == 0 && stats && npairs) { atomicAdd(&stats[2], npairs); atomicAdd(&stats[3], ncand); }
 }
 
 // ---- decode: key -> fs_placement (one warp per request, lanes over phi for f_req) ----------
 __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
                                                           const fs_request* __restrict__ reqs,
                                                           const unsigned long long* __restrict__ keys,
+                                                          const unsigned long long* __restrict__ wkeys,
                                                           fs_placement* __restrict__ out) {
   const int lane = threadIdx.x & 31;
   const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (r >= R) return;
-  const unsigned long long key = keys[r];
+  unsigned long long key = keys[r];
+  if (wkeys) {
+    // best warm pair (value, GPU): find its lowest (sigma, phi) and merge with the dense key
+    const unsigned long long wk = wkeys[r];
+    if (wk != FS_KEY_NONE && (uint32_t)(wk >> 32) <= (uint32_t)(key >> 32)) {
+      const FsDimsDev d = v.d;
+      const int k = (int)(uint32_t)wk; const uint32_t best = (uint32_t)(wk >> 32);
+      const ReqCtx c = make_req(v, reqs[r]);
+      const PairCtx p = make_pair(v, c, v.ginfo[k]);
+      uint32_t flat = 0xFFFFFFFFu;
+      for (int sg = 0; sg < p.smf && flat == 0xFFFFFFFFu; ++sg)
+        for (int phi = lane; phi < d.F; phi += 32) {
+          const Cand cd = eval_cand(v, c, p, k, sg, phi);
+          if (cd.ok && fs_orderable(cd.dE) == best) { flat = (uint32_t)((k * d.S + sg) * d.F + phi); break; }
+        }
+      unsigned long long cand = flat != 0xFFFFFFFFu ? (((unsigned long long)best << 32) | flat) : FS_KEY_NONE;
+      cand = fs_warp_min_key(cand);
+      key = cand < key ? cand : key;
+    }
+  }
   fs_placement o;
   o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
   o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
@@ -412,9 +577,10 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   if (R <= 0) return 0;
   int launches = 0;
   cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
+  cudaMemsetAsync(sc.wkeys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
   cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 4, st);
   if (v.K <= 0) {
-    place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
+    place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, nullptr, out);
     return 1;
   }
   const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= 64 && !sc.force_generic;
@@ -442,7 +608,17 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
     fs_tm_beg(tm, FS_T_PLACE_WARM, st);
-    place_warm_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, sc.warm_off, sc.warm_item, sc.stats);
+    {
+      cudaMemsetAsync(sc.rb_off, 0, sizeof(int32_t) * (size_t)(v.d.M + 1), st);
+      req_count_kernel<<<(R + 255) / 256, 256, 0, st>>>(reqs, R, v.d.M, sc.rb_off);
+      bucket_scan_kernel<<<1, 1024, 0, st>>>(sc.rb_off, sc.rb_cursor, v.d.M);
+      req_fill_kernel<<<(R + 255) / 256, 256, 0, st>>>(reqs, R, v.d.M, sc.rb_off, sc.rb_cursor, sc.rb_idx);
+      const int nphib = FT / 32;
+      const long long warps = (long long)v.K * FS_RMAX * nphib * WARM_SLOTS;   // upper bound on items
+      place_warm_kernel<<<(unsigned)((warps + WARM_WARPS - 1) / WARM_WARPS), WARM_WARPS * 32, 0, st>>>(
+          v, R, reqs, sc.keys, sc.wkeys, sc.warm_off, sc.warm_item, sc.rb_off, sc.rb_idx, nphib, sc.stats);
+      launches += 3;
+    }
     fs_tm_end(tm, FS_T_PLACE_WARM, st);
     ++launches;
   } else {
@@ -460,7 +636,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   }
   fs_tm_beg(tm, FS_T_PLACE_DECODE, st);
-  place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
+  place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, dense_ok ? sc.wkeys : nullptr, out);
   fs_tm_end(tm, FS_T_PLACE_DECODE, st);
   ++launches;
   return launches;
