@@ -261,22 +261,27 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         T = c.L > 0 ? fs_tstar(__fadd_rn(g.t_avail_ms, c.load_ms), c.slo_ttft) : FS_INF;
         npairs += 1; ncand += (unsigned long long)smf * d.F;
       }
+      // compact the eligible GPUs of the chunk, in ascending order, into the warp's list:
+      // {T*, Ecur, sm_free, byte offset of the GPU's A0 row}
+      const bool go = el && T >= 0.0f;
+      const unsigned mask = __ballot_sync(0xffffffffu, go);
       __syncwarp();
-      wb[lane] = make_float4(T, g.e_cur, __int_as_float(smf), 0.f);
-      unsigned mask = __ballot_sync(0xffffffffu, el && T >= 0.0f);
+      if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
+          make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((ci * FS_CHUNK + lane) * FT * (int)sizeof(float)));
       __syncwarp();
+      const int n_el = __popc(mask);
+      const char* a0_lane = reinterpret_cast<const char*>(s_a0 + lane * NPHI);
       // ---- sweep the eligible GPUs of the chunk -------------------------------------------------
-      while (mask) {
-        const int g_i = __ffs(mask) - 1; mask &= mask - 1;
-        const float4 w = wb[g_i];
+      for (int e = 0; e < n_el; ++e) {
+        const float4 w = wb[e];
         const float Tst = w.x; const int sfree = __float_as_int(w.z);
-        float m[NPHI];
+        float m[NPHI][2];                               // two min chains per frequency (ILP)
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
+        for (int i = 0; i < NPHI; ++i) m[i][0] = m[i][1] = FS_INF;
 #define FS_DENSE_STEP(s)                                                              \
   _Pragma("unroll") for (int i = 0; i < NPHI; ++i)                                    \
     asm("{.reg .pred p; setp.le.f32 p, %1, %2; @p min.f32 %0, %0, %3;}"               \
-        : "+f"(m[i]) : "f"(t0[s][i]), "f"(Tst), "f"(er[s][i]));
+        : "+f"(m[i][(s) & 1]) : "f"(t0[s][i]), "f"(Tst), "f"(er[s][i]));
         switch (sfree) {
           default:
           case 16: FS_DENSE_STEP(15) case 15: FS_DENSE_STEP(14) case 14: FS_DENSE_STEP(13)
@@ -287,14 +292,16 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           case 1: FS_DENSE_STEP(0)
         }
 #undef FS_DENSE_STEP
-        const float* arow = s_a0 + (size_t)(ci * FS_CHUNK + g_i) * FT + lane * NPHI;
+        const int row_off = __float_as_int(w.w);
+        const float* arow = reinterpret_cast<const float*>(a0_lane + row_off);
         float x = FS_INF;
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
+        for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], fminf(m[i][0], m[i][1])));
         const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
-        if (dE < best) { best = dE; bestk = ci * FS_CHUNK + g_i; }
+        if (dE < best) { best = dE; bestk = row_off; }
       }
     }
+    bestk = bestk >= 0 ? bestk / (FT * (int)sizeof(float)) : -1;
     // ---- recovery: lowest flat index among the candidates that attain the minimum -------------
     unsigned long long key = FS_KEY_NONE;
     if (bestk >= 0) {
@@ -484,13 +491,22 @@ place_warm_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
 #undef FS_WARM_STEP
       } else {                                          // short prompt: its own prefill plane, via L2
         const size_t o0 = fs_plane(d, m, 0, w.br0) + phic, o1 = fs_plane(d, m, 1, br1) + phic;
+        // four shares per trip so that the 16 loads of a trip are in flight together
 #pragma unroll 1
-        for (int s = 0; s < smf; ++s) {
-          const float l1 = v.latT[o1 + (size_t)s * d.F];
-          const float t0 = __fmul_rn(w.fr0, v.latT[o0 + (size_t)s * d.F]);
-          const float ee = __fadd_rn(__fmul_rn(t0, v.powT[o0 + (size_t)s * d.F]),
-                                     __fmul_rn(__fmul_rn(w.fr1, l1), v.powT[o1 + (size_t)s * d.F]));
-          if (t0 <= w.T && l1 <= w.tbt) mn = fminf(mn, ee);
+        for (int s4 = 0; s4 < smf; s4 += 4) {
+          float l0v[4], p0v[4], l1v[4], p1v[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const size_t so = (size_t)min(s4 + u, smf - 1) * d.F;
+            l0v[u] = v.latT[o0 + so]; p0v[u] = v.powT[o0 + so];
+            l1v[u] = v.latT[o1 + so]; p1v[u] = v.powT[o1 + so];
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const float t0 = __fmul_rn(w.fr0, l0v[u]);
+            const float ee = __fadd_rn(__fmul_rn(t0, p0v[u]), __fmul_rn(__fmul_rn(w.fr1, l1v[u]), p1v[u]));
+            if (s4 + u < smf && t0 <= w.T && l1v[u] <= w.tbt) mn = fminf(mn, ee);
+          }
         }
       }
       float dE = __fsub_rn(__fadd_rn(A, mn), ecur);     // monotone in mn
