@@ -33,6 +33,8 @@ struct fs_ctx {
   // local scratch
   size_t local_cap = 0; int n_cap = 0; float* G = nullptr; uint8_t* Bst = nullptr;
   int32_t* ids_dev = nullptr; fs_local_cfg* local_dev = nullptr;
+  int32_t *bin_off = nullptr, *bin_cursor = nullptr, *keylist = nullptr, *nkeys = nullptr; int bin_m_cap = 0;
+  uint4* lslots = nullptr;
   // consolidation scratch
   size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
   unsigned long long* ckeys = nullptr; fs_consol_out* consol_dev = nullptr;
@@ -153,7 +155,7 @@ int fs_destroy(fs_ctx* c) {
   cudaDeviceSynchronize();
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gA0, c->ctr, c->rb_off, c->rb_cursor, c->rb_idx, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->wkeys, c->stats,
-                  c->reqs_dev, c->place_dev, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
+                  c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (c->flag_host) cudaFreeHost(c->flag_host);
@@ -289,7 +291,16 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
   const size_t rows = (size_t)c->d.F * c->d.S;
   const size_t need = (size_t)n * FS_RMAX * 2 * rows;
   if (need > c->local_cap) { FS_TRY(grow(c, c->G, need)); FS_TRY(grow(c, c->Bst, need)); c->local_cap = need; }
-  if (n > c->n_cap) { FS_TRY(grow(c, c->ids_dev, (size_t)n)); FS_TRY(grow(c, c->local_dev, (size_t)n)); c->n_cap = n; }
+  if (n > c->n_cap) {
+    FS_TRY(grow(c, c->ids_dev, (size_t)n)); FS_TRY(grow(c, c->local_dev, (size_t)n));
+    FS_TRY(grow(c, c->lslots, (size_t)n * FS_RMAX * 2));
+    c->n_cap = n;
+  }
+  if (c->d.M > c->bin_m_cap) {
+    FS_TRY(grow(c, c->bin_off, (size_t)c->d.M * 16 + 1)); FS_TRY(grow(c, c->bin_cursor, (size_t)c->d.M * 16));
+    FS_TRY(grow(c, c->keylist, (size_t)c->d.M * 2)); FS_TRY(grow(c, c->nkeys, (size_t)1));
+    c->bin_m_cap = c->d.M;
+  }
   const int32_t* d_ids = gpu_ids; fs_local_cfg* d_out = out;
   if (space == FS_HOST) {
     if (gpu_ids) {
@@ -298,7 +309,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
     }
     d_out = c->local_dev;
   }
-  FsLocalScratch sc{c->G, c->Bst, c->comp, c->comp_n, c->ns_stride};
+  FsLocalScratch sc{c->G, c->Bst, c->comp, c->comp_n, c->ns_stride, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots};
   c->launches += fsk_local(view_of(c), n, d_ids, flags, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {

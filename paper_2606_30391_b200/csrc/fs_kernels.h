@@ -71,6 +71,12 @@ struct FsLocalScratch {
   const uint32_t* comp;   // [RMAX][ns_stride] SM splits in lexicographic order, sigma_i in byte i
   const uint32_t* comp_n; // [RMAX] number of splits NS = C(S-1, n_res-1)
   int ns_stride;
+  // per-call grouping of the live slots by (model, phase, q bucket)
+  int32_t* bin_off;       // [M*2*8 + 1]
+  int32_t* bin_cursor;    // [M*2*8]
+  int32_t* keylist;       // [M*2] non-empty (model, phase) keys
+  int32_t* nkeys;         // [1]
+  void* slots;            // [n*8] 16-byte slot records
 };
 int fsk_local_smem_attr();   // raise the split kernel's dynamic shared memory limit (once)
 int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,

@@ -58,6 +58,132 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
   }
 }
 
+// ---- step 1, table-major: slots grouped by (model, phase) so that every LUT row is read once ----
+// Per call the live slots (q > 0) are counting-sorted by bin = (model*2+phase)*QB + q-bucket.
+// A block takes one non-empty (model, phase) key and a tile of LS_TR consecutive (phi,sigma)
+// rows, stages their LAT/POW vectors over beta in shared memory (1-D TMA bulk copies; the rows of
+// a tile are contiguous in the caller's layout), and its warps walk the key's slots 32 at a
+// time: lane <-> slot, sequential over beta, LDS.128 broadcasts of four beta per row, rounds by
+// multiply-high with a per-beta magic constant (exact for q < 2^24, beta < 256).  Strict '<' in
+// ascending beta keeps the lowest beta on ties, as the definition wants.
+constexpr int LS_TR = 4;          // rows per tile
+constexpr int LS_QB = 8;          // q buckets per key (slots of similar depth share a warp)
+constexpr int LS_WARPS = 8;
+__constant__ uint32_t c_magic[FS_MAX_B];   // ceil(2^32 / (beta+1)), beta >= 1
+
+struct __align__(16) LocalSlot { int32_t gi; uint32_t q; float slo; uint32_t meta; };  // meta = slot | nb << 8
+
+__device__ __forceinline__ bool local_slot_of(const FsView& v, const int32_t* gpu_ids, int gi, int slot,
+                                              LocalSlot& o, int& bin) {
+  const int k = gpu_ids ? gpu_ids[gi] : gi;
+  if (k < 0 || k >= v.K) return false;
+  const int i = slot >> 1, p = slot & 1;
+  if (i >= v.ginfo[k].n_res) return false;
+  const fs_tenant& t = v.states[k].t[i];
+  const uint32_t q = t.q[p];
+  if (q == 0) return false;
+  const uint32_t nb = q < (uint32_t)v.d.B ? q : (uint32_t)v.d.B;
+  o.gi = gi; o.q = q; o.slo = t.slo_ms[p]; o.meta = (uint32_t)slot | (nb << 8);
+  bin = (t.model * 2 + p) * LS_QB + (int)(((nb - 1) * LS_QB) / (uint32_t)v.d.B);
+  return true;
+}
+__global__ void local_bin_count_kernel(FsView v, int n, const int32_t* __restrict__ gpu_ids, int32_t* __restrict__ off) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= n * FS_RMAX * 2) return;
+  LocalSlot o; int bin;
+  if (local_slot_of(v, gpu_ids, x >> 3, x & 7, o, bin)) atomicAdd(&off[bin + 1], 1);
+}
+__global__ void local_bin_fill_kernel(FsView v, int n, const int32_t* __restrict__ gpu_ids,
+                                      const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
+                                      LocalSlot* __restrict__ slots) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= n * FS_RMAX * 2) return;
+  LocalSlot o; int bin;
+  if (local_slot_of(v, gpu_ids, x >> 3, x & 7, o, bin)) slots[off[bin] + atomicAdd(&cursor[bin], 1)] = o;
+}
+__global__ void local_keys_kernel(const int32_t* __restrict__ off, int nkeys_all, int32_t* __restrict__ keylist,
+                                  int32_t* __restrict__ nkeys) {
+  const int key = blockIdx.x * blockDim.x + threadIdx.x;
+  if (key >= nkeys_all) return;
+  if (off[(key + 1) * LS_QB] > off[key * LS_QB]) keylist[atomicAdd(nkeys, 1)] = key;
+}
+
+template <int P, bool OBJ_POWER>
+__global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
+    FsView v, const int32_t* __restrict__ off, const int32_t* __restrict__ keylist,
+    const int32_t* __restrict__ nkeys, const LocalSlot* __restrict__ slots, float* __restrict__ Gs,
+    uint8_t* __restrict__ Bs) {
+  extern __shared__ __align__(128) unsigned char ls_smem[];
+  __shared__ __align__(8) uint64_t bar;
+  if ((int)blockIdx.x >= *nkeys) return;
+  const int key = keylist[blockIdx.x];
+  if ((key & 1) != P) return;
+  const FsDimsDev d = v.d;
+  const int B = d.B, rows = d.F * d.S;
+  const int r0 = blockIdx.y * LS_TR, tr = min(LS_TR, rows - r0);
+  float* sl = reinterpret_cast<float*>(ls_smem);            // [LS_TR][B]
+  float* sp = sl + LS_TR * B;                               // [LS_TR][B]
+  const size_t src = ((size_t)key * rows + r0) * B;
+  const uint32_t bytes = (uint32_t)tr * B * sizeof(float);
+  if (threadIdx.x == 0) { fs_mbar_init(&bar, 1); fs_mbar_fence_init(); }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    fs_mbar_expect_tx(&bar, 2 * bytes);
+    fs_tma_load_1d(sl, v.lat + src, bytes, &bar);
+    fs_tma_load_1d(sp, v.pow + src, bytes, &bar);
+  }
+  if (tr < LS_TR)   // ragged last tile: keep the unused rows finite
+    for (int x = threadIdx.x + tr * B; x < LS_TR * B; x += blockDim.x) { sl[x] = 1.0f; sp[x] = 1.0f; }
+  fs_mbar_wait(&bar, 0);
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int s0 = off[key * LS_QB], s1 = off[(key + 1) * LS_QB];
+  for (int base = s0 + warp * 32; base < s1; base += LS_WARPS * 32) {
+    const bool have = base + lane < s1;
+    LocalSlot sl_ = have ? slots[base + lane] : LocalSlot{0, 0u, 0.f, 0u};
+    const uint32_t nb = have ? (sl_.meta >> 8) : 0u;
+    uint32_t maxnb;
+    asm volatile("redux.sync.max.u32 %0, %1, 0xffffffff;" : "=r"(maxnb) : "r"(nb));
+    float best[LS_TR]; uint32_t bb[LS_TR];
+#pragma unroll
+    for (int r = 0; r < LS_TR; ++r) { best[r] = FS_INF; bb[r] = 0u; }
+    for (uint32_t b4 = 0; b4 < maxnb; b4 += 4) {
+      float4 L4[LS_TR], P4[LS_TR];
+#pragma unroll
+      for (int r = 0; r < LS_TR; ++r) {
+        L4[r] = *reinterpret_cast<const float4*>(sl + r * B + b4);
+        P4[r] = *reinterpret_cast<const float4*>(sp + r * B + b4);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const uint32_t beta = b4 + u;
+        const uint32_t rounds = beta == 0 ? sl_.q : __umulhi(sl_.q + beta, c_magic[beta]);
+        const float fr = __uint2float_rn(rounds);
+        const bool act = beta < nb;
+#pragma unroll
+        for (int r = 0; r < LS_TR; ++r) {
+          const float la = u == 0 ? L4[r].x : u == 1 ? L4[r].y : u == 2 ? L4[r].z : L4[r].w;
+          const float pw = u == 0 ? P4[r].x : u == 1 ? P4[r].y : u == 2 ? P4[r].z : P4[r].w;
+          const float t = __fmul_rn(fr, la);
+          const bool ok = P == 0 ? (t <= sl_.slo) : (la <= sl_.slo);
+          const float cost = OBJ_POWER ? pw : __fmul_rn(t, pw);
+          if (act && ok && cost < best[r]) { best[r] = cost; bb[r] = beta; }
+        }
+      }
+    }
+    if (have) {
+      const size_t o = ((size_t)sl_.gi * (FS_RMAX * 2) + (sl_.meta & 0xFF)) * rows + r0;
+      if (tr == LS_TR && (rows & 3) == 0) {
+        *reinterpret_cast<float4*>(Gs + o) = make_float4(best[0], best[1], best[2], best[3]);
+        *reinterpret_cast<uint32_t*>(Bs + o) = bb[0] | (bb[1] << 8) | (bb[2] << 16) | (bb[3] << 24);
+      } else {
+#pragma unroll
+        for (int r = 0; r < LS_TR; ++r) if (r < tr) { Gs[o + r] = best[r]; Bs[o + r] = (uint8_t)bb[r]; }
+      }
+    }
+  }
+}
+
 // ---- steps 2-3: tenant sums, split search, argmin; one block per GPU -----------------------
 __device__ __forceinline__ unsigned long long block_min_key(unsigned long long key,
                                                             unsigned long long* sred) {
@@ -108,7 +234,11 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
   const float* g_in = Gs + (size_t)gi * (FS_RMAX * 2) * rows;
   for (int x = threadIdx.x; x < n_res * rows; x += blockDim.x) {
     const int i = x / rows, row = x % rows;
-    sG[x] = __fadd_rn(g_in[(size_t)(i * 2) * rows + row], g_in[(size_t)(i * 2 + 1) * rows + row]);
+    // a slot with an empty queue costs 0 (the slot kernels do not visit it)
+    const fs_tenant& tt = v.states[k].t[i];
+    const float g0 = tt.q[0] ? g_in[(size_t)(i * 2) * rows + row] : 0.0f;
+    const float g1 = tt.q[1] ? g_in[(size_t)(i * 2 + 1) * rows + row] : 0.0f;
+    sG[x] = __fadd_rn(g0, g1);
   }
   __syncthreads();
   const bool minsm = flags & FS_SPLIT_MINSM;
@@ -202,10 +332,10 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
         o.sigma[i] = (uint8_t)sg;
         float e[2], pw[2];
         for (int p = 0; p < 2; ++p) {
-          const int beta = b_in[(size_t)(i * 2 + p) * rows + phi * d.S + sg];
+          const uint32_t q = g.t[i].q[p];
+          const int beta = q ? b_in[(size_t)(i * 2 + p) * rows + phi * d.S + sg] : 0;
           o.beta[i][p] = (uint8_t)beta;
           e[p] = 0.0f; pw[p] = 0.0f;
-          const uint32_t q = g.t[i].q[p];
           if (q > 0) {
             const size_t ix = fs_idx(d, g.t[i].model, p, phi, sg, beta);
             pw[p] = v.pow[ix];
@@ -225,22 +355,52 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
 }  // namespace
 
 int fsk_local_smem_attr() {
+  uint32_t magic[FS_MAX_B];
+  magic[0] = 0xFFFFFFFFu;   // unused (beta == 0: rounds = q)
+  for (uint32_t n = 2; n <= FS_MAX_B; ++n) magic[n - 1] = (uint32_t)(((1ull << 32) + n - 1) / n);
+  int e = (int)cudaMemcpyToSymbol(c_magic, magic, sizeof(magic));
   // [RMAX][F][S] floats at the largest supported dims = 128 KiB
-  return (int)cudaFuncSetAttribute(local_split_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)(sizeof(float) * FS_RMAX * FS_MAX_F * FS_MAX_S));
+  e |= (int)cudaFuncSetAttribute(local_split_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(sizeof(float) * FS_RMAX * FS_MAX_F * FS_MAX_S));
+  return e;
 }
 
 int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,
               const FsLocalScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (n <= 0) return 0;
   const int rows = v.d.F * v.d.S;
+  int launches = 0;
   fs_tm_beg(tm, FS_T_LOCAL_SLOT, st);
-  local_slot_kernel<<<dim3(n, FS_RMAX * 2), 256, 0, st>>>(v, n, gpu_ids, flags, sc.G, sc.B);
+  if (v.d.B % 4 == 0) {
+    const int nkeys_all = v.d.M * 2, nbins = nkeys_all * LS_QB, nslots = n * FS_RMAX * 2;
+    cudaMemsetAsync(sc.bin_off, 0, sizeof(int32_t) * (size_t)(nbins + 1), st);
+    cudaMemsetAsync(sc.nkeys, 0, sizeof(int32_t), st);
+    local_bin_count_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(v, n, gpu_ids, sc.bin_off);
+    fs_bucket_scan_kernel<<<1, 1024, 0, st>>>(sc.bin_off, sc.bin_cursor, nbins);
+    local_bin_fill_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(v, n, gpu_ids, sc.bin_off, sc.bin_cursor,
+                                                               reinterpret_cast<LocalSlot*>(sc.slots));
+    local_keys_kernel<<<(nkeys_all + 255) / 256, 256, 0, st>>>(sc.bin_off, nkeys_all, sc.keylist, sc.nkeys);
+    const dim3 grid(min(nkeys_all, nslots), (rows + LS_TR - 1) / LS_TR);
+    const size_t smem = sizeof(float) * 2 * LS_TR * v.d.B;
+    const LocalSlot* sl = reinterpret_cast<const LocalSlot*>(sc.slots);
+    // one launch per phase: the deadline rule differs (prefill: whole queue; decode: one step)
+    if (flags & FS_OBJ_POWER) {
+      local_slot_grouped_kernel<0, true><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
+      local_slot_grouped_kernel<1, true><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
+    } else {
+      local_slot_grouped_kernel<0, false><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
+      local_slot_grouped_kernel<1, false><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
+    }
+    launches += 6;
+  } else {
+    local_slot_kernel<<<dim3(n, FS_RMAX * 2), 256, 0, st>>>(v, n, gpu_ids, flags, sc.G, sc.B);
+    launches += 1;
+  }
   fs_tm_end(tm, FS_T_LOCAL_SLOT, st);
   const size_t smem = sizeof(float) * FS_RMAX * rows;
   fs_tm_beg(tm, FS_T_LOCAL_SPLIT, st);
   local_split_kernel<<<n, 256, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.B, sc.comp, sc.comp_n,
                                            sc.ns_stride, out);
   fs_tm_end(tm, FS_T_LOCAL_SPLIT, st);
-  return 2;
+  return launches + 1;
 }

@@ -366,25 +366,6 @@ __global__ void req_count_kernel(const fs_request* __restrict__ reqs, int R, int
   const int m = reqs[r].model;
   if (m >= 0 && m < M) atomicAdd(&off[m + 1], 1);
 }
-// single-block inclusive scan of off[1..M] in place (off[0] = 0) and cursor[m] = 0
-__global__ void __launch_bounds__(1024) bucket_scan_kernel(int32_t* __restrict__ off, int32_t* __restrict__ cursor, int M) {
-  __shared__ int32_t part[1024];
-  const int t = threadIdx.x, per = (M + 1023) / 1024;
-  const int lo = min(M, t * per), hi = min(M, lo + per);
-  int32_t sum = 0;
-  for (int m = lo; m < hi; ++m) sum += off[m + 1];
-  part[t] = sum;
-  __syncthreads();
-  for (int o = 1; o < 1024; o <<= 1) {
-    const int32_t add = t >= o ? part[t - o] : 0;
-    __syncthreads();
-    part[t] += add;
-    __syncthreads();
-  }
-  int32_t acc = part[t] - sum;
-  if (t == 0) off[0] = 0;
-  for (int m = lo; m < hi; ++m) { acc += off[m + 1]; off[m + 1] = acc; cursor[m] = 0; }
-}
 __global__ void req_fill_kernel(const fs_request* __restrict__ reqs, int R, int M,
                                 const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
                                 int32_t* __restrict__ idx) {
@@ -627,7 +608,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     {
       cudaMemsetAsync(sc.rb_off, 0, sizeof(int32_t) * (size_t)(v.d.M + 1), st);
       req_count_kernel<<<(R + 255) / 256, 256, 0, st>>>(reqs, R, v.d.M, sc.rb_off);
-      bucket_scan_kernel<<<1, 1024, 0, st>>>(sc.rb_off, sc.rb_cursor, v.d.M);
+      fs_bucket_scan_kernel<<<1, 1024, 0, st>>>(sc.rb_off, sc.rb_cursor, v.d.M);
       req_fill_kernel<<<(R + 255) / 256, 256, 0, st>>>(reqs, R, v.d.M, sc.rb_off, sc.rb_cursor, sc.rb_idx);
       const int nphib = FT / 32;
       const long long warps = (long long)v.K * FS_RMAX * nphib * WARM_SLOTS;   // upper bound on items

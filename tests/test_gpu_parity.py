@@ -129,6 +129,18 @@ def test_ttft_deadline_on_the_rounding_boundary(ctx, seed):
     _check_all(ctx, cl, local=False, consol=False)
 
 
+@pytest.mark.parametrize("B", [4, 12, 64, 256])
+def test_local_queue_depths_up_to_2_pow_24(ctx, B):
+    """rounds = ceil(q/(beta+1)) for q from 1 to 2^24-1 (the kernel divides by multiply-high)."""
+    cl = synth.make_custom(seed=500 + B, K=48, M=5, F=6, S=4, B=B, R=0, lo=1, hi=4)
+    st = synth.Stream(B, "bigq")
+    q = st.randint(cl.K * 8, 0, 24).reshape(cl.K, 4, 2)
+    q = (2 ** q.astype(np.int64)) - st.randint(cl.K * 8, 0, 3).reshape(cl.K, 4, 2)
+    cl.states["t"]["q"][...] = np.clip(q, 0, 2 ** 24 - 1).astype(np.uint32)
+    cl.states["t"]["slo_ms"][...] = 1e30
+    _check_all(ctx, cl, consol=False)
+
+
 def test_empty_inputs(ctx):
     cl = synth.make_custom(seed=5, K=4, M=2, F=4, S=4, B=4, R=8)
     ctx.load_cluster(cl)
