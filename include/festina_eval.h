@@ -180,11 +180,12 @@ const char* fs_strerror(int code);
 int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed runtime call */
 /* Kernels launched by this context since creation (bench.py's gpu_launches counter).     */
 uint64_t fs_launch_count(const fs_ctx* ctx);
-/* Work of the last fs_place_batch, counted on the device (valid after synchronising; this call
- * synchronises the device): out[0] = eligible (request, GPU) pairs scored by the dense (cold)
- * kernel or the generic kernel, out[1] = their candidates (sum of sm_free*F), out[2], out[3] =
- * the same for the warm-pair kernel.                                                       */
-int fs_last_place_stats(fs_ctx* ctx, uint64_t out[4]);
+/* Work of the last fs_place_batch, counted on the device (this call synchronises the device):
+ * out[0], out[1] = eligible (request, GPU) pairs of the dense (cold) kernel or the generic kernel and
+ * their candidates (sum of sm_free*F) by the method's definition; out[2], out[3] = the same for the
+ * warm-pair kernel; out[4], out[5] = pairs and candidates the dense kernel actually swept after its
+ * exact lower-bound pruning (<= out[0], out[1]).                                           */
+int fs_last_place_stats(fs_ctx* ctx, uint64_t out[6]);
 
 /* Per-kernel device timing for measurement (bench.py's roofline line).  fs_set_timing(ctx, 1)
  * makes every later call record CUDA event pairs on its stream around its kernels;

@@ -134,13 +134,13 @@ int fs_create(fs_ctx** out, int cuda_device) {
   if (cudaSetDevice(cuda_device) != cudaSuccess ||
       cudaHostAlloc((void**)&c->flag_host, sizeof(int) * FS_NFLAGS, cudaHostAllocMapped) != cudaSuccess ||
       cudaHostGetDevicePointer((void**)&c->flag_dev, c->flag_host, 0) != cudaSuccess ||
-      cudaMalloc((void**)&c->stats, 4 * sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMalloc((void**)&c->stats, 8 * sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return FS_ERR_CUDA;
   }
   std::memset(c->flag_host, 0, sizeof(int) * FS_NFLAGS);
-  cudaMemset(c->stats, 0, 4 * sizeof(unsigned long long));
+  cudaMemset(c->stats, 0, 8 * sizeof(unsigned long long));
   fsk_local_smem_attr();
   fsk_place_smem_attr();
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
@@ -391,12 +391,12 @@ int fs_get_timing(fs_ctx* c, float* ms, int n) {
   return FS_OK;
 }
 
-int fs_last_place_stats(fs_ctx* c, uint64_t out[4]) {
+int fs_last_place_stats(fs_ctx* c, uint64_t out[6]) {
   if (!c || !out) return FS_ERR_ARG;
-  unsigned long long h[4] = {0, 0, 0, 0};
+  unsigned long long h[6] = {0, 0, 0, 0, 0, 0};
   FS_CUDA(c, cudaSetDevice(c->dev));
   FS_CUDA(c, cudaMemcpy(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost));
-  for (int i = 0; i < 4; ++i) out[i] = h[i];
+  for (int i = 0; i < 6; ++i) out[i] = h[i];
   return FS_OK;
 }
 

@@ -45,7 +45,8 @@ struct __align__(16) FsGpuRec {
   float t_avail_ms, mem_free_mb, e_cur;
   uint32_t meta;            // n_res | sm_free << 8   (n_res == 0: never a candidate)
   int16_t model[FS_RMAX];
-  uint32_t _pad[2];
+  float a_min;              // min over phi of A0[k][phi] (+INF: co-residents never feasible)
+  uint32_t _pad;
 };
 static_assert(sizeof(FsGpuRec) == 32, "FsGpuRec layout");
 #define FS_CHUNK 32         // GPUs per staged chunk (one per lane in the eligibility pass)

@@ -143,6 +143,12 @@ constexpr int DENSE_WARPS = 16;
 constexpr int DENSE_SMEM_MAX = 200 * 1024;   // of the 227 KB a block may use
 constexpr int DENSE_S = 16;
 
+__device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) {
+  uint32_t r;
+  asm volatile("redux.sync.min.u32 %0, %1, 0xffffffff;" : "=r"(r) : "r"(x));
+  return r;
+}
+
 // largest t >= 0 with fl(w + t) <= slo, or -1 if there is none.  fl(w + .) is monotone, so the
 // answer is characterised by g(T) <= slo < g(nextup(T)); a double-precision guess is verified
 // with the fp32 operation itself and a bit-pattern bisection covers whatever it misses.
@@ -181,7 +187,7 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
 //   wb  [DENSE_WARPS][32] per warp: {T*, Ecur, sm_free, -} of the chunk being swept
 __host__ __device__ inline size_t dense_smem_bytes(int KS, int FT) {
   return (size_t)KS * FT * sizeof(float) + (size_t)KS * sizeof(FsGpuRec) +
-         (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) + 16;
+         (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) + (size_t)DENSE_WARPS * 2 * DENSE_S * sizeof(float) + 16;
 }
 
 template <int NPHI>
@@ -200,7 +206,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   float* s_a0 = reinterpret_cast<float*>(dense_smem_raw);
   FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw + (size_t)KSmax * FT * sizeof(float));
   float4* s_wb = reinterpret_cast<float4*>(dense_smem_raw + (size_t)KSmax * (FT * sizeof(float) + sizeof(FsGpuRec)));
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_wb + DENSE_WARPS * FS_CHUNK);
+  float* s_bnd = reinterpret_cast<float*>(s_wb + DENSE_WARPS * FS_CHUNK);   // [warp][2][16] prefix minima
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_bnd + DENSE_WARPS * 2 * DENSE_S);
 
   // ---- stage this block's GPU slice once: 1-D TMA bulk copies completing on one mbarrier --------
   if (threadIdx.x == 0) { fs_mbar_init(s_bar, 1); fs_mbar_fence_init(); }
@@ -217,7 +224,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   fs_mbar_wait(s_bar, 0);
 
   float4* wb = s_wb + warp * FS_CHUNK;
-  unsigned long long npairs = 0, ncand = 0;
+  float* bnd = s_bnd + warp * 2 * DENSE_S;      // [0][s]: min er over sigma <= s, all phi; [1][s]: same for t0
+  unsigned long long npairs = 0, ncand = 0, nswept = 0, ncswept = 0;
   for (;;) {
     // ---- next request of this slice: dynamic, one atomic per warp ----------------------------
     int r = 0;
@@ -248,8 +256,28 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           t0[s][i] = tt; er[s][i] = ee;
         }
     }
+    // ---- bounds for exact pruning: every candidate of a GPU with sm_free = s has
+    //   er >= bnd[0][s-1], t0 >= bnd[1][s-1]   hence   dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)
+    // (monotone rounding).  er, t0 >= +0, so their bit patterns order like unsigned integers.
+    {
+      uint32_t pe = 0x7F800000u, pt = 0x7F800000u;
+      __syncwarp();
+#pragma unroll
+      for (int s = 0; s < DENSE_S; ++s) {
+        uint32_t ue = 0x7F800000u, ut = 0x7F800000u;
+#pragma unroll
+        for (int i = 0; i < NPHI; ++i) {
+          ue = min(ue, __float_as_uint(er[s][i])); ut = min(ut, __float_as_uint(t0[s][i]));
+        }
+        pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut));
+        if (lane == 0) { bnd[s] = __uint_as_float(pe); bnd[DENSE_S + s] = __uint_as_float(pt); }
+      }
+      __syncwarp();
+    }
     float best = FS_INF; int bestk = -1;
     for (int ci = 0; ci < nchunk; ++ci) {
+      // best value found so far by any lane (all from GPUs with a lower index than this chunk's)
+      const float bestW = fs_unorderable(warp_min_u32(fs_orderable(best)));
       // ---- eligibility + T*: lane <-> one GPU of the chunk ------------------------------------
       const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
       const int n_res = g.meta & 0xFF, smf = (g.meta >> 8) & 0xFF;
@@ -258,8 +286,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       for (int i = 0; i < FS_RMAX; ++i) el = el && (g.model[i] != c.m);   // resident -> warm path
       float T = -1.0f;
       if (el) {
-        T = c.L > 0 ? fs_tstar(__fadd_rn(g.t_avail_ms, c.load_ms), c.slo_ttft) : FS_INF;
         npairs += 1; ncand += (unsigned long long)smf * d.F;
+        // prune: no candidate of this GPU can beat (or, having a higher index, tie) bestW
+        const float lb = __fsub_rn(__fadd_rn(g.a_min, bnd[smf - 1]), g.e_cur);
+        if (lb < bestW) {
+          T = c.L > 0 ? fs_tstar(__fadd_rn(g.t_avail_ms, c.load_ms), c.slo_ttft) : FS_INF;
+          if (!(bnd[DENSE_S + smf - 1] <= T)) T = -1.0f;       // no share meets the TTFT deadline
+        }
+        if (T >= 0.0f) { nswept += 1; ncswept += (unsigned long long)smf * d.F; }
       }
       // compact the eligible GPUs of the chunk, in ascending order, into the warp's list:
       // {T*, Ecur, sm_free, byte offset of the GPU's A0 row}
@@ -330,8 +364,13 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   for (int o = 16; o > 0; o >>= 1) {
     npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
     ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
+    nswept += __shfl_xor_sync(0xffffffffu, nswept, o);
+    ncswept += __shfl_xor_sync(0xffffffffu, ncswept, o);
   }
-  if (lane == 0 && stats && npairs) { atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand); }
+  if (lane == 0 && stats && npairs) {
+    atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand);
+    atomicAdd(&stats[4], nswept); atomicAdd(&stats[5], ncswept);
+  }
 }
 
 // =============================================================================================
@@ -375,11 +414,6 @@ __global__ void req_fill_kernel(const fs_request* __restrict__ reqs, int R, int 
   if (m >= 0 && m < M) idx[off[m] + atomicAdd(&cursor[m], 1)] = r;
 }
 
-__device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) {
-  uint32_t r;
-  asm volatile("redux.sync.min.u32 %0, %1, 0xffffffff;" : "=r"(r) : "r"(x));
-  return r;
-}
 
 __global__ void __launch_bounds__(WARM_WARPS * 32, 3)
 place_warm_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
@@ -575,7 +609,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   int launches = 0;
   cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
   cudaMemsetAsync(sc.wkeys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-  cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 4, st);
+  cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 8, st);
   if (v.K <= 0) {
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, nullptr, out);
     return 1;

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     if (lane == 0) {
       FsGpuRec r; r.t_avail_ms = r.mem_free_mb = r.e_cur = 0.f; r.meta = 0;
       for (int i = 0; i < FS_RMAX; ++i) r.model[i] = -1;
-      r._pad[0] = r._pad[1] = 0;
+      r.a_min = FS_INF; r._pad = 0;
       grec[k] = r;
     }
     return;
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
   const bool valid = state_valid(g, d);
   const int n = valid ? g.n_res : 0;
   float* A = gA + (size_t)k * FS_NVAR * d.F;
-  int f_floor = -1;
+  int f_floor = -1; float a_min = FS_INF;
   for (int base = 0; base < d.F; base += 32) {
     const int phi = base + lane;
     bool ok0 = false;
@@ -83,12 +83,14 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
           }
         }
         A[var * d.F + phi] = ok ? acc : FS_INF;
-        if (var == 0) { ok0 = ok; gA0[(size_t)k * v.FT + phi] = ok ? acc : FS_INF; }
+        if (var == 0) { ok0 = ok; gA0[(size_t)k * v.FT + phi] = ok ? acc : FS_INF; if (ok) a_min = fminf(a_min, acc); }
       }
     } else if (phi < v.FT) gA0[(size_t)k * v.FT + phi] = FS_INF;
     const unsigned m = __ballot_sync(0xffffffffu, ok0);
     if (f_floor < 0 && m) f_floor = base + __ffs(m) - 1;
   }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
   if (lane == 0) {
     FsGpuInfo gi;
     gi.t_avail_ms = g.t_avail_ms; gi.mem_free_mb = g.mem_free_mb;
@@ -110,7 +112,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     FsGpuRec r; r.t_avail_ms = gi.t_avail_ms; r.mem_free_mb = gi.mem_free_mb; r.e_cur = ecur;
     r.meta = (uint32_t)n | ((uint32_t)gi.sm_free << 8);
     for (int i = 0; i < FS_RMAX; ++i) r.model[i] = gi.model[i];
-    r._pad[0] = r._pad[1] = 0;
+    r.a_min = a_min; r._pad = 0;
     grec[k] = r;
     if (!valid) fs_raise(v.flag, FS_FLAG_STATE);
   }
