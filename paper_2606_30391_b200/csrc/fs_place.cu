@@ -180,14 +180,29 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
   return tstar_bisect(w, slo);
 }
 
-// Shared memory of one block: its SLICE of the GPUs stays resident for the whole kernel, so the
-// warps never synchronise with each other after the initial TMA fill.
-//   a0  [KS][FT] floats   co-resident energy rows (variant 0), FT = 32*NPHI
-//   rec [KS]              compact GPU records
-//   wb  [DENSE_WARPS][32] per warp: {T*, Ecur, sm_free, -} of the chunk being swept
-__host__ __device__ inline size_t dense_smem_bytes(int KS, int FT) {
-  return (size_t)KS * FT * sizeof(float) + (size_t)KS * sizeof(FsGpuRec) +
-         (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) + (size_t)DENSE_WARPS * 2 * DENSE_S * sizeof(float) + 16;
+// Shared memory of one block: the compact records of its SLICE of the GPUs stay resident for the
+// whole kernel (one TMA fill), so the warps never synchronise with each other afterwards.
+//   rec [KS]              compact GPU records (32 B each)
+//   wb  [DENSE_WARPS][32] per warp: {T*, Ecur, sm_free, GPU} of the chunk being swept
+//   bnd [DENSE_WARPS][32] per warp: prefix minima of er / t0 over shares (pruning bounds)
+// The A0 rows of the few GPUs that survive the pruning are read through L1/L2.
+__host__ __device__ inline size_t dense_smem_bytes(int KS) {
+  return (size_t)KS * sizeof(FsGpuRec) + (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) +
+         (size_t)DENSE_WARPS * 2 * DENSE_S * sizeof(float) + 16;
+}
+
+// NPHI adjacent values of row `o` for the lane whose first column is phi0 (columns clamped to the
+// row for padded lanes; the caller overrides those); one 64-bit load when the pair is aligned
+template <int NPHI>
+__device__ __forceinline__ void ld_cols(const float* __restrict__ base, int o, int phi0, int ncol, bool vec,
+                                        float (&x)[NPHI]) {
+  if (NPHI == 2 && vec) {
+    const float2 t = *reinterpret_cast<const float2*>(base + o + min(phi0, ncol - 2));
+    x[0] = t.x; x[NPHI - 1] = t.y;
+  } else {
+#pragma unroll
+    for (int i = 0; i < NPHI; ++i) x[i] = base[o + min(phi0 + i, ncol - 1)];
+  }
 }
 
 template <int NPHI>
@@ -203,29 +218,30 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const int slice = blockIdx.x % nslice;
   const int c0 = slice * chunks_per_slice, c1 = min(nchunk_all, c0 + chunks_per_slice);
   const int nchunk = c1 - c0, KS = nchunk * FS_CHUNK, KSmax = chunks_per_slice * FS_CHUNK;
-  float* s_a0 = reinterpret_cast<float*>(dense_smem_raw);
-  FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw + (size_t)KSmax * FT * sizeof(float));
-  float4* s_wb = reinterpret_cast<float4*>(dense_smem_raw + (size_t)KSmax * (FT * sizeof(float) + sizeof(FsGpuRec)));
+  FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw);
+  float4* s_wb = reinterpret_cast<float4*>(dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec));
   float* s_bnd = reinterpret_cast<float*>(s_wb + DENSE_WARPS * FS_CHUNK);   // [warp][2][16] prefix minima
   uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_bnd + DENSE_WARPS * 2 * DENSE_S);
+  const float* gA0 = v.gA0 + (size_t)c0 * FS_CHUNK * FT;   // rows of this slice
 
-  // ---- stage this block's GPU slice once: 1-D TMA bulk copies completing on one mbarrier --------
+  // ---- stage this block's GPU records once: 1-D TMA bulk copies completing on one mbarrier ------
   if (threadIdx.x == 0) { fs_mbar_init(s_bar, 1); fs_mbar_fence_init(); }
   __syncthreads();
   if (threadIdx.x == 0) {
-    const uint32_t bytes_a0 = (uint32_t)KS * FT * sizeof(float), bytes_rec = (uint32_t)KS * sizeof(FsGpuRec);
-    fs_mbar_expect_tx(s_bar, bytes_a0 + bytes_rec);
-    const char* src = reinterpret_cast<const char*>(v.gA0 + (size_t)c0 * FS_CHUNK * FT);
-    char* dst = reinterpret_cast<char*>(s_a0);
-    for (uint32_t off = 0; off < bytes_a0; off += 32768u)
-      fs_tma_load_1d(dst + off, src + off, min(32768u, bytes_a0 - off), s_bar);
-    fs_tma_load_1d(s_rec, v.grec + (size_t)c0 * FS_CHUNK, bytes_rec, s_bar);
+    const uint32_t bytes_rec = (uint32_t)KS * sizeof(FsGpuRec);
+    fs_mbar_expect_tx(s_bar, bytes_rec);
+    const char* src = reinterpret_cast<const char*>(v.grec + (size_t)c0 * FS_CHUNK);
+    char* dst = reinterpret_cast<char*>(s_rec);
+    for (uint32_t off = 0; off < bytes_rec; off += 32768u)
+      fs_tma_load_1d(dst + off, src + off, min(32768u, bytes_rec - off), s_bar);
   }
   fs_mbar_wait(s_bar, 0);
 
   float4* wb = s_wb + warp * FS_CHUNK;
   float* bnd = s_bnd + warp * 2 * DENSE_S;      // [0][s]: min er over sigma <= s, all phi; [1][s]: same for t0
   unsigned long long npairs = 0, ncand = 0, nswept = 0, ncswept = 0;
+  const bool vec = NPHI == 2 && (d.F & 1) == 0;
+  const int phi0 = lane * NPHI;
   for (;;) {
     // ---- next request of this slice: dynamic, one atomic per warp ----------------------------
     int r = 0;
@@ -235,26 +251,34 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     const ReqCtx c = make_req(v, reqs[r]);
     if (!c.valid) { if (lane == 0 && slice == 0) fs_raise(v.flag, FS_FLAG_REQUEST); continue; }
     // ---- phase A: the request's (sigma, phi) tiles in registers -------------------------------
+    // L == 0 / O == 0 need no branches: rounds = 0 gives t = e = +0 exactly (tables are finite),
+    // and an empty decode slot passes its deadline (threshold +INF).
     float t0[DENSE_S][NPHI], er[DENSE_S][NPHI];
     {
       const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
       const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
+      const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
 #pragma unroll
-      for (int s = 0; s < DENSE_S; ++s)
+      for (int s4 = 0; s4 < DENSE_S; s4 += 4) {
+        float a0[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) {
-          const int phi = lane * NPHI + i;
-          float tt = FS_INF, ee = FS_INF;
-          if (s < d.S && phi < d.F) {
-            const int o = s * d.F + phi;
-            float e0 = 0.f, e1 = 0.f; bool ok1 = true; tt = 0.f;
-            if (c.L > 0) { tt = __fmul_rn(fr0, l0[o]); e0 = __fmul_rn(tt, p0[o]); }
-            if (c.O > 0) { const float la = l1[o]; ok1 = la <= c.slo_tbt; e1 = __fmul_rn(__fmul_rn(fO, la), p1[o]); }
-            ee = ok1 ? __fadd_rn(e0, e1) : FS_INF;
-          }
-          t0[s][i] = tt; er[s][i] = ee;
+        for (int u = 0; u < 4; ++u) {                  // 16 independent loads in flight
+          const int o = min(s4 + u, d.S - 1) * d.F;
+          ld_cols<NPHI>(l0, o, phi0, d.F, vec, a0[u]); ld_cols<NPHI>(p0, o, phi0, d.F, vec, b0[u]);
+          ld_cols<NPHI>(l1, o, phi0, d.F, vec, a1[u]); ld_cols<NPHI>(p1, o, phi0, d.F, vec, b1[u]);
         }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+          for (int i = 0; i < NPHI; ++i) {
+            const float tt = __fmul_rn(fr0, a0[u][i]);
+            const float ee = __fadd_rn(__fmul_rn(tt, b0[u][i]), __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
+            const bool in = (s4 + u) < d.S && (phi0 + i) < d.F;
+            t0[s4 + u][i] = in ? tt : FS_INF;
+            er[s4 + u][i] = (in && a1[u][i] <= tbt) ? ee : FS_INF;
+          }
+      }
     }
     // ---- bounds for exact pruning: every candidate of a GPU with sm_free = s has
     //   er >= bnd[0][s-1], t0 >= bnd[1][s-1]   hence   dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)
@@ -301,10 +325,9 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       const unsigned mask = __ballot_sync(0xffffffffu, go);
       __syncwarp();
       if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
-          make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((ci * FS_CHUNK + lane) * FT * (int)sizeof(float)));
+          make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float(ci * FS_CHUNK + lane));
       __syncwarp();
       const int n_el = __popc(mask);
-      const char* a0_lane = reinterpret_cast<const char*>(s_a0 + lane * NPHI);
       // ---- sweep the eligible GPUs of the chunk -------------------------------------------------
       for (int e = 0; e < n_el; ++e) {
         const float4 w = wb[e];
@@ -326,16 +349,16 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           case 1: FS_DENSE_STEP(0)
         }
 #undef FS_DENSE_STEP
-        const int row_off = __float_as_int(w.w);
-        const float* arow = reinterpret_cast<const float*>(a0_lane + row_off);
+        const int kloc = __float_as_int(w.w);
+        float arow[NPHI];
+        ld_cols<NPHI>(gA0 + (size_t)kloc * FT, 0, phi0, FT, true, arow);   // rows are FT-padded: aligned
         float x = FS_INF;
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], fminf(m[i][0], m[i][1])));
         const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
-        if (dE < best) { best = dE; bestk = row_off; }
+        if (dE < best) { best = dE; bestk = kloc; }
       }
     }
-    bestk = bestk >= 0 ? bestk / (FT * (int)sizeof(float)) : -1;
     // ---- recovery: lowest flat index among the candidates that attain the minimum -------------
     unsigned long long key = FS_KEY_NONE;
     if (bestk >= 0) {
@@ -349,7 +372,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) {
           const bool feas = s < smf && (c.L == 0 || __fadd_rn(wait, t0[s][i]) <= c.slo_ttft);
-          const float dE = __fsub_rn(__fadd_rn(s_a0[(size_t)bestk * FT + lane * NPHI + i], er[s][i]), g.e_cur);
+          const float dE = __fsub_rn(__fadd_rn(gA0[(size_t)bestk * FT + lane * NPHI + i], er[s][i]), g.e_cur);
           if (!found && feas && dE == best) {
             found = true; flat = (uint32_t)((kglob * d.S + s) * d.F + lane * NPHI + i);
           }
@@ -621,7 +644,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     // of slices is what the slice size forces, raised when R alone cannot occupy every SM.
     const int FT = v.d.F <= 32 ? 32 : 64;
     const int nchunk = v.Kpad / FS_CHUNK;
-    const size_t fixed = dense_smem_bytes(0, FT), per_chunk = dense_smem_bytes(FS_CHUNK, FT) - fixed;
+    const size_t fixed = dense_smem_bytes(0), per_chunk = dense_smem_bytes(FS_CHUNK) - fixed;
     const int max_cps = (int)((DENSE_SMEM_MAX - fixed) / per_chunk);
     int nslice = (nchunk + max_cps - 1) / max_cps;
     const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS;
@@ -630,7 +653,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     nslice = (nchunk + cps - 1) / cps;
     const int streams = max(1, min(nbatch, sc.sm_count / nslice));
     const int grid = streams * nslice;
-    const size_t smem = dense_smem_bytes(cps * FS_CHUNK, FT);
+    const size_t smem = dense_smem_bytes(cps * FS_CHUNK);
     cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nslice, st);
     if (FT == 32)
       place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.stats);
