@@ -181,11 +181,11 @@ int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed run
 /* Kernels launched by this context since creation (bench.py's gpu_launches counter).     */
 uint64_t fs_launch_count(const fs_ctx* ctx);
 /* Work of the last fs_place_batch, counted on the device (this call synchronises the device):
- * out[0], out[1] = eligible (request, GPU) pairs of the dense (cold) kernel or the generic kernel and
- * their candidates (sum of sm_free*F) by the method's definition; out[2], out[3] = the same for the
- * warm-pair kernel; out[4], out[5] = pairs and candidates the dense kernel actually swept after its
- * exact lower-bound pruning (<= out[0], out[1]).                                           */
-int fs_last_place_stats(fs_ctx* ctx, uint64_t out[6]);
+ * out[0], out[1] = eligible COLD (request, GPU) pairs (model not resident; all pairs when the generic
+ * kernel ran) and their candidates (sum of sm_free*F) by the method's definition; out[2], out[3] =
+ * the same for WARM pairs (model resident); out[4..5] / out[6..7] = cold / warm pairs and candidates
+ * actually evaluated after the exact lower-bound pruning.                                  */
+int fs_last_place_stats(fs_ctx* ctx, uint64_t out[8]);
 
 /* Per-kernel device timing for measurement (bench.py's roofline line).  fs_set_timing(ctx, 1)
  * makes every later call record CUDA event pairs on its stream around its kernels;
@@ -199,7 +199,7 @@ typedef enum {
   FS_TIMER_LOCAL_SPLIT,     /* SM-split search of fs_local_config                    */
   FS_TIMER_CONSOL_AGG,      /* per-tenant minimum shares of fs_consolidate           */
   FS_TIMER_CONSOL_PAIR,     /* pair scoring of fs_consolidate                        */
-  FS_TIMER_PLACE_WARM,      /* fs_place_batch: pairs whose model is already resident */
+  FS_TIMER_PLACE_WARM,      /* (unused since the warm pairs moved into the scoring kernel) */
   FS_TIMER_COUNT
 } fs_timer;
 int fs_set_timing(fs_ctx* ctx, int on);

@@ -206,11 +206,12 @@ class Festina:
 
     def last_place_stats(self) -> dict:
         """Eligible pairs / candidates the last fs_place_batch evaluated, dense and warm kernels."""
-        o = (C.c_uint64 * 6)()
+        o = (C.c_uint64 * 8)()
         self._check(lib().fs_last_place_stats(self._h, o), "fs_last_place_stats")
         return {"dense_pairs": int(o[0]), "dense_candidates": int(o[1]), "warm_pairs": int(o[2]),
                 "warm_candidates": int(o[3]), "dense_swept_pairs": int(o[4]),
-                "dense_swept_candidates": int(o[5])}
+                "dense_swept_candidates": int(o[5]), "warm_swept_pairs": int(o[6]),
+                "warm_swept_candidates": int(o[7])}
 
     def set_timing(self, on: bool = True):
         self._check(lib().fs_set_timing(self._h, int(on)), "fs_set_timing")

@@ -24,11 +24,10 @@ struct fs_ctx {
   int K = 0, k_cap = 0;
   fs_gpu_state* states = nullptr; FsGpuInfo* ginfo = nullptr; float* gA = nullptr; size_t gA_cap = 0;
   FsGpuRec* grec = nullptr; float* gA0 = nullptr; size_t gA0_cap = 0; int Kpad = 0, FT = 32;
-  int32_t *warm_off = nullptr, *warm_cursor = nullptr; uint32_t* warm_item = nullptr; int warm_m_cap = 0;
+  int32_t *warm_off = nullptr, *warm_cursor = nullptr; FsWarmItem* warm_item = nullptr; int warm_m_cap = 0;
   // placement scratch
-  int r_cap = 0; unsigned long long* keys = nullptr; unsigned long long* wkeys = nullptr; unsigned long long* stats = nullptr;
+  int r_cap = 0; unsigned long long* keys = nullptr; unsigned long long* stats = nullptr;
   unsigned int* ctr = nullptr;
-  int32_t *rb_off = nullptr, *rb_cursor = nullptr, *rb_idx = nullptr;
   fs_request* reqs_dev = nullptr; fs_placement* place_dev = nullptr;
   // local scratch
   size_t local_cap = 0; int n_cap = 0; float* G = nullptr; uint8_t* Bst = nullptr;
@@ -154,7 +153,7 @@ int fs_destroy(fs_ctx* c) {
   cudaSetDevice(c->dev);
   cudaDeviceSynchronize();
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
-                  c->ginfo, c->gA, c->grec, c->gA0, c->ctr, c->rb_off, c->rb_cursor, c->rb_idx, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->wkeys, c->stats,
+                  c->ginfo, c->gA, c->grec, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -232,7 +231,6 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (na0 > c->gA0_cap) { FS_TRY(grow(c, c->gA0, na0)); c->gA0_cap = na0; }
   if (c->d.M > c->warm_m_cap) {
     FS_TRY(grow(c, c->warm_off, (size_t)c->d.M + 1)); FS_TRY(grow(c, c->warm_cursor, (size_t)c->d.M));
-    FS_TRY(grow(c, c->rb_off, (size_t)c->d.M + 1)); FS_TRY(grow(c, c->rb_cursor, (size_t)c->d.M));
     c->warm_m_cap = c->d.M;
   }
   c->K = K; c->have_state = false;
@@ -257,8 +255,8 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
   const int pending = take_flags(c);
   if (R == 0) return pending;
   if (R > c->r_cap) {
-    FS_TRY(grow(c, c->keys, (size_t)R)); FS_TRY(grow(c, c->wkeys, (size_t)R)); FS_TRY(grow(c, c->reqs_dev, (size_t)R));
-    FS_TRY(grow(c, c->place_dev, (size_t)R)); FS_TRY(grow(c, c->rb_idx, (size_t)R));
+    FS_TRY(grow(c, c->keys, (size_t)R)); FS_TRY(grow(c, c->reqs_dev, (size_t)R));
+    FS_TRY(grow(c, c->place_dev, (size_t)R));
     c->r_cap = R;
   }
   const fs_request* d_reqs = reqs; fs_placement* d_out = out;
@@ -266,7 +264,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
-  FsPlaceScratch sc{c->keys, c->wkeys, c->stats, c->ctr, c->warm_off, c->warm_item, c->rb_off, c->rb_cursor, c->rb_idx, c->sm_count, c->force_generic};
+  FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
@@ -391,12 +389,12 @@ int fs_get_timing(fs_ctx* c, float* ms, int n) {
   return FS_OK;
 }
 
-int fs_last_place_stats(fs_ctx* c, uint64_t out[6]) {
+int fs_last_place_stats(fs_ctx* c, uint64_t out[8]) {
   if (!c || !out) return FS_ERR_ARG;
-  unsigned long long h[6] = {0, 0, 0, 0, 0, 0};
+  unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   FS_CUDA(c, cudaSetDevice(c->dev));
   FS_CUDA(c, cudaMemcpy(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost));
-  for (int i = 0; i < 6; ++i) out[i] = h[i];
+  for (int i = 0; i < 8; ++i) out[i] = h[i];
   return FS_OK;
 }
 

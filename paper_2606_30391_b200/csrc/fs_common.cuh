@@ -49,6 +49,18 @@ struct __align__(16) FsGpuRec {
   uint32_t _pad;
 };
 static_assert(sizeof(FsGpuRec) == 32, "FsGpuRec layout");
+// One (GPU k, tenant slot j) that hosts a model: what a request of that model needs to bound and
+// to score the WARM pair (r, k) (48 bytes; built by fs_set_gpu_state, listed per model).
+struct __align__(16) FsWarmItem {
+  int32_t k, j;
+  int32_t br1;              // decode bucket the request joins (-1: past the table)
+  int32_t sm_free;
+  float t_avail_ms, mem_free_mb, e_cur;
+  float a_min;              // min over phi of A[k][1+j][phi]
+  float l1_min, p1_min;     // min of LAT / POW of plane (model, decode, br1) over sigma < sm_free, all phi
+  uint32_t _pad[2];
+};
+static_assert(sizeof(FsWarmItem) == 48, "FsWarmItem layout");
 #define FS_CHUNK 32         // GPUs per staged chunk (one per lane in the eligibility pass)
 
 struct FsDimsDev { int M, F, S, B; };

@@ -46,15 +46,11 @@ int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, fl
 // fs_place.cu — placement scoring + 64-bit-key argmin + decode
 struct FsPlaceScratch {
   unsigned long long* keys;        // [R]  (dE, flat) argmin keys
-  unsigned long long* wkeys;       // [R]  (dE, GPU) best warm pair per request
-  unsigned long long* stats;       // [4]: dense pairs, dense candidates, warm pairs, warm candidates
+  unsigned long long* stats;       // [8]: dense pairs, dense pairs/cands, warm pairs/cands, dense swept pairs/cands, warm swept pairs/cands
   unsigned int* ctr;               // [nslice <= Kpad/32] dynamic request counters of the dense kernel
   // bucketing of GPUs by model (built by fs_set_gpu_state): warm lists
   const int32_t* warm_off;         // [M+1]
-  const uint32_t* warm_item;       // [sum n_res]: k*4 + j
-  int32_t* rb_off;                 // [M+1] per-call request buckets by model
-  int32_t* rb_cursor;              // [M]
-  int32_t* rb_idx;                 // [R]
+  const FsWarmItem* witems;        // [<= 4K] items, grouped by model
   int sm_count;                    // SMs of the device (grid sizing)
   bool force_generic;              // diagnostics: score with the generic kernel only
 };
@@ -62,7 +58,7 @@ int fsk_place_smem_attr();
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
               const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm);
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,
-                         uint32_t* warm_item /*[4K]*/, cudaStream_t st);
+                         FsWarmItem* items /*[4K]*/, cudaStream_t st);
 
 // fs_local.cu — per-slot batch search + SM-split search
 struct FsLocalScratch {

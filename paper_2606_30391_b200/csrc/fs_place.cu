@@ -188,7 +188,7 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
 // The A0 rows of the few GPUs that survive the pruning are read through L1/L2.
 __host__ __device__ inline size_t dense_smem_bytes(int KS) {
   return (size_t)KS * sizeof(FsGpuRec) + (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) +
-         (size_t)DENSE_WARPS * 2 * DENSE_S * sizeof(float) + 16;
+         (size_t)DENSE_WARPS * 3 * DENSE_S * sizeof(float) + 16;
 }
 
 // NPHI adjacent values of row `o` for the lane whose first column is phi0 (columns clamped to the
@@ -209,7 +209,8 @@ template <int NPHI>
 __global__ void __launch_bounds__(DENSE_WARPS * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
-                   unsigned int* __restrict__ ctr, unsigned long long* __restrict__ stats) {
+                   unsigned int* __restrict__ ctr, const int32_t* __restrict__ warm_off,
+                   const FsWarmItem* __restrict__ witems, unsigned long long* __restrict__ stats) {
   extern __shared__ __align__(128) unsigned char dense_smem_raw[];
   constexpr int FT = 32 * NPHI;
   const FsDimsDev d = v.d;
@@ -221,7 +222,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw);
   float4* s_wb = reinterpret_cast<float4*>(dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec));
   float* s_bnd = reinterpret_cast<float*>(s_wb + DENSE_WARPS * FS_CHUNK);   // [warp][2][16] prefix minima
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_bnd + DENSE_WARPS * 2 * DENSE_S);
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_bnd + DENSE_WARPS * 3 * DENSE_S);
   const float* gA0 = v.gA0 + (size_t)c0 * FS_CHUNK * FT;   // rows of this slice
 
   // ---- stage this block's GPU records once: 1-D TMA bulk copies completing on one mbarrier ------
@@ -238,8 +239,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   fs_mbar_wait(s_bar, 0);
 
   float4* wb = s_wb + warp * FS_CHUNK;
-  float* bnd = s_bnd + warp * 2 * DENSE_S;      // [0][s]: min er over sigma <= s, all phi; [1][s]: same for t0
-  unsigned long long npairs = 0, ncand = 0, nswept = 0, ncswept = 0;
+  float* bnd = s_bnd + warp * 3 * DENSE_S;      // prefix minima over sigma <= s, all phi, of [0] er (cold), [1] t0, [2] e0
+  unsigned long long npairs = 0, ncand = 0, nswept = 0, ncswept = 0, wpairs = 0, wcand = 0, wswept = 0, wcswept = 0;
   const bool vec = NPHI == 2 && (d.F & 1) == 0;
   const int phi0 = lane * NPHI;
   for (;;) {
@@ -259,6 +260,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
       const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
+      uint32_t pe0 = 0x7F800000u;                       // running prefix min of e0 (bits; e0 >= +0)
+      __syncwarp();
 #pragma unroll
       for (int s4 = 0; s4 < DENSE_S; s4 += 4) {
         float a0[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
@@ -269,23 +272,28 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           ld_cols<NPHI>(l1, o, phi0, d.F, vec, a1[u]); ld_cols<NPHI>(p1, o, phi0, d.F, vec, b1[u]);
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int u = 0; u < 4; ++u) {
+          uint32_t ue0 = 0x7F800000u;
 #pragma unroll
           for (int i = 0; i < NPHI; ++i) {
             const float tt = __fmul_rn(fr0, a0[u][i]);
-            const float ee = __fadd_rn(__fmul_rn(tt, b0[u][i]), __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
+            const float e0 = __fmul_rn(tt, b0[u][i]);
+            const float ee = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
             const bool in = (s4 + u) < d.S && (phi0 + i) < d.F;
             t0[s4 + u][i] = in ? tt : FS_INF;
             er[s4 + u][i] = (in && a1[u][i] <= tbt) ? ee : FS_INF;
+            if (in) ue0 = min(ue0, __float_as_uint(e0));
           }
+          pe0 = min(pe0, warp_min_u32(ue0));
+          if (lane == 0) bnd[2 * DENSE_S + s4 + u] = __uint_as_float(pe0);
+        }
       }
     }
     // ---- bounds for exact pruning: every candidate of a GPU with sm_free = s has
-    //   er >= bnd[0][s-1], t0 >= bnd[1][s-1]   hence   dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)
-    // (monotone rounding).  er, t0 >= +0, so their bit patterns order like unsigned integers.
+    //   er >= bnd[0][s-1], t0 >= bnd[1][s-1], e0 >= bnd[2][s-1]
+    // hence, for a cold pair,  dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)   (monotone rounding).  er, t0 >= +0, so their bit patterns order like unsigned integers.
     {
       uint32_t pe = 0x7F800000u, pt = 0x7F800000u;
-      __syncwarp();
 #pragma unroll
       for (int s = 0; s < DENSE_S; ++s) {
         uint32_t ue = 0x7F800000u, ut = 0x7F800000u;
@@ -359,25 +367,68 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         if (dE < best) { best = dE; bestk = kloc; }
       }
     }
-    // ---- recovery: lowest flat index among the candidates that attain the minimum -------------
-    unsigned long long key = FS_KEY_NONE;
-    if (bestk >= 0) {
-      const FsGpuRec g = s_rec[bestk];
-      const int smf = (g.meta >> 8) & 0xFF;
-      const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
-      const int kglob = c0 * FS_CHUNK + bestk;
-      bool found = false; uint32_t flat = 0xFFFFFFFFu;
+    int bestkg = bestk >= 0 ? c0 * FS_CHUNK + bestk : 0x7FFFFFFF;    // global GPU index of the lane's best
+    // ---- warm pairs: GPUs that already host model m (decode bucket, variant and wait depend on
+    // the GPU).  Lane <-> item: bound  dE >= fl(fl(a_min + fl(e0min + e1min)) - Ecur)  with
+    // e1min = fl(fl(rounds1*l1_min)*p1_min); items that survive are scored candidate by candidate
+    // from the planes.  They come after GPUs with a higher index, so ties compare (dE, k) in full
+    // and the prune is strict.
+    for (int ib = warm_off[c.m]; ib < warm_off[c.m + 1]; ib += 32) {
+      uint32_t ordl = 0xFFFFFFFFu; int wk = 0, wsmf = 0;      // orderable bound of the lane's item
+      if (ib + lane < warm_off[c.m + 1]) {
+        const FsWarmItem it = witems[ib + lane];
+        const int kc = it.k / FS_CHUNK;
+        if (kc >= c0 && kc < c1 && it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
+          wpairs += 1; wcand += (unsigned long long)it.sm_free * d.F;
+          const float fr1 = __uint2float_rn(fs_ceil_div(c.O, (uint32_t)it.br1 + 1u));
+          const float e1lb = __fmul_rn(__fmul_rn(fr1, it.l1_min), it.p1_min);
+          const float lb = __fsub_rn(__fadd_rn(it.a_min, __fadd_rn(bnd[2 * DENSE_S + it.sm_free - 1], e1lb)), it.e_cur);
+          if (c.O == 0 || it.l1_min <= c.slo_tbt) {
+            const float T = c.L > 0 ? fs_tstar(it.t_avail_ms, c.slo_ttft) : FS_INF;
+            if (T >= 0.0f && bnd[DENSE_S + it.sm_free - 1] <= T) ordl = fs_orderable(lb);
+          }
+          wk = it.k; wsmf = it.sm_free;
+        }
+      }
+      // best-first: score the item with the lowest bound, tighten the incumbent, drop every item
+      // whose bound is now strictly above it (NaN bounds order above +INF and drop out too)
+      for (;;) {
+        const uint32_t mn = warp_min_u32(ordl);
+        const uint32_t inc = warp_min_u32(fs_orderable(best));
+        if (mn == 0xFFFFFFFFu || mn > inc) break;
+        const int src = __ffs(__ballot_sync(0xffffffffu, ordl == mn)) - 1;
+        if (lane == src) { ordl = 0xFFFFFFFFu; wswept += 1; wcswept += (unsigned long long)wsmf * d.F; }
+        const int k = __shfl_sync(0xffffffffu, wk, src);
+        const PairCtx p = make_pair(v, c, v.ginfo[k]);
+        if (!p.ok) continue;
+        for (int sg = 0; sg < p.smf; ++sg)
 #pragma unroll
-      for (int s = 0; s < DENSE_S; ++s)
+          for (int i = 0; i < NPHI; ++i) {
+            const int phi = phi0 + i;
+            if (phi < d.F) {
+              const Cand cd = eval_cand(v, c, p, k, sg, phi);
+              float dE = cd.dE; if (dE == 0.0f) dE = 0.0f;
+              if (cd.ok && (dE < best || (dE == best && k < bestkg))) { best = dE; bestkg = k; }
+            }
+          }
+      }
+    }
+    // ---- recovery: lowest flat index among the lane's candidates that attain its minimum, by the
+    // definition (eval_cand), at its best GPU ----------------------------------------------------
+    unsigned long long key = FS_KEY_NONE;
+    if (bestkg != 0x7FFFFFFF) {
+      const PairCtx p = make_pair(v, c, v.ginfo[bestkg]);
+      uint32_t flat = 0xFFFFFFFFu;
+      for (int sg = 0; sg < p.smf && flat == 0xFFFFFFFFu; ++sg)
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) {
-          const bool feas = s < smf && (c.L == 0 || __fadd_rn(wait, t0[s][i]) <= c.slo_ttft);
-          const float dE = __fsub_rn(__fadd_rn(gA0[(size_t)bestk * FT + lane * NPHI + i], er[s][i]), g.e_cur);
-          if (!found && feas && dE == best) {
-            found = true; flat = (uint32_t)((kglob * d.S + s) * d.F + lane * NPHI + i);
+          const int phi = phi0 + i;
+          if (phi < d.F && flat == 0xFFFFFFFFu) {
+            const Cand cd = eval_cand(v, c, p, bestkg, sg, phi);
+            if (cd.ok && cd.dE == best) flat = (uint32_t)((bestkg * d.S + sg) * d.F + phi);
           }
         }
-      if (found) key = fs_make_key(best, flat);
+      if (flat != 0xFFFFFFFFu) key = fs_make_key(best, flat);
     }
     key = fs_warp_min_key(key);
     if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
@@ -389,211 +440,28 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
     nswept += __shfl_xor_sync(0xffffffffu, nswept, o);
     ncswept += __shfl_xor_sync(0xffffffffu, ncswept, o);
+    wpairs += __shfl_xor_sync(0xffffffffu, wpairs, o);
+    wcand += __shfl_xor_sync(0xffffffffu, wcand, o);
+    wswept += __shfl_xor_sync(0xffffffffu, wswept, o);
+    wcswept += __shfl_xor_sync(0xffffffffu, wcswept, o);
   }
-  if (lane == 0 && stats && npairs) {
+  if (lane == 0 && stats && (npairs | wpairs)) {
     atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand);
+    atomicAdd(&stats[2], wpairs); atomicAdd(&stats[3], wcand);
     atomicAdd(&stats[4], nswept); atomicAdd(&stats[5], ncswept);
+    atomicAdd(&stats[6], wswept); atomicAdd(&stats[7], wcswept);
   }
-}
-
-// =============================================================================================
-// Warm pairs: the request's model is resident on the GPU, so the decode bucket (beta_j1+1), the
-// co-resident variant (1+j), wait (= T_avail, no weight load) and the decode plane depend on the
-// GPU.  Organised ITEM-major: an item is one (GPU k, slot j) of the per-model lists built by
-// fs_set_gpu_state.  A warp owns (item, block of 32 frequencies) and keeps the four plane columns
-// it needs in registers: LAT/POW of (m, decode, br1) and of (m, prefill, B-1) — the prefill bucket
-// of every request with L >= B; shorter prompts read their own prefill plane through L2.
-// It then walks the requests of model m (bucketed per call), 32 at a time: each lane prepares one
-// request (T*, rounds, eligibility), then the warp sweeps them.  Per candidate: 4 mul, 1 add,
-// 2 compares, 1 predicated min, all on registers.  Same monotone factorisation as the dense
-// kernel; the per-(item, request) minimum is reduced with redux.sync on the orderable value and
-// merged as (value, GPU) into wkeys[r] by atomicMin when it can still win; the decode kernel
-// turns the winning (request, GPU) into the lowest flat index.
-// =============================================================================================
-constexpr int WARM_WARPS = 4;
-constexpr int WARM_SLOTS = 4;      // warps that share the request list of one (item, phi block)
-
-struct __align__(16) WarmReq {     // what one request contributes, prepared by one lane
-  float T, fr0, fr1, tbt;          // T* for wait = T_avail; rounds as floats; slo_tbt (INF if O == 0)
-  int br0;                         // prefill bucket, -1 = the common plane B-1 held in registers
-  int r;                           // request index
-  uint32_t cur_hi;                 // high word of keys[r] when the chunk was prepared (pruning)
-  uint32_t _pad;
-};
-
-// bucket the requests of one call by model: counts -> offsets -> indices
-__global__ void req_count_kernel(const fs_request* __restrict__ reqs, int R, int M, int32_t* __restrict__ off) {
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= R) return;
-  const int m = reqs[r].model;
-  if (m >= 0 && m < M) atomicAdd(&off[m + 1], 1);
-}
-__global__ void req_fill_kernel(const fs_request* __restrict__ reqs, int R, int M,
-                                const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
-                                int32_t* __restrict__ idx) {
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= R) return;
-  const int m = reqs[r].model;
-  if (m >= 0 && m < M) idx[off[m] + atomicAdd(&cursor[m], 1)] = r;
-}
-
-
-__global__ void __launch_bounds__(WARM_WARPS * 32, 3)
-place_warm_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
-                  const unsigned long long* __restrict__ keys,
-                  unsigned long long* __restrict__ wkeys, const int32_t* __restrict__ warm_off,
-                  const uint32_t* __restrict__ warm_item, const int32_t* __restrict__ rb_off,
-                  const int32_t* __restrict__ rb_idx, int nphib,
-                  unsigned long long* __restrict__ stats) {
-  __shared__ WarmReq s_req[WARM_WARPS][32];
-  const FsDimsDev d = v.d;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long gw = (long long)blockIdx.x * WARM_WARPS + warp;
-  const int slot = (int)(gw % WARM_SLOTS);
-  const int pb = (int)((gw / WARM_SLOTS) % nphib);
-  const long long item_i = gw / ((long long)WARM_SLOTS * nphib);
-  if (item_i >= warm_off[d.M]) return;
-  const uint32_t item = warm_item[item_i];
-  const int k = (int)(item >> 2), j = (int)(item & 3u);
-  const FsGpuInfo gi = v.ginfo[k];
-  const int m = gi.model[j], smf = gi.sm_free, br1 = gi.br1[j];
-  if (smf < 1 || br1 < 0) return;                       // no free SMs / decode bucket past the table
-  const int n_req = rb_off[m + 1] - rb_off[m];
-  if (n_req == 0) return;
-  const int phi = pb * 32 + lane;
-  const bool phi_ok = phi < d.F;
-  const int phic = phi_ok ? phi : 0;
-  // ---- item tiles in registers ------------------------------------------------------------------
-  float la0[DENSE_S], pw0[DENSE_S], la1[DENSE_S], pw1[DENSE_S];
-  {
-    const size_t o0 = fs_plane(d, m, 0, d.B - 1), o1 = fs_plane(d, m, 1, br1);
-#pragma unroll
-    for (int s = 0; s < DENSE_S; ++s) {
-      const bool in = s < smf && s < d.S;
-      const size_t o = (size_t)(in ? s : 0) * d.F + phic;
-      la0[s] = v.latT[o0 + o]; pw0[s] = v.powT[o0 + o];
-      la1[s] = v.latT[o1 + o]; pw1[s] = v.powT[o1 + o];
-    }
-  }
-  const float A = phi_ok ? v.gA[((size_t)k * FS_NVAR + 1 + j) * d.F + phic] : FS_INF;
-  const float ecur = gi.e_cur, kv = v.models[m].kv_mb_per_token;
-  WarmReq* wr = s_req[warp];
-  unsigned long long npairs = 0, ncand = 0;
-
-  for (int cbase = slot * 32; cbase < n_req; cbase += WARM_SLOTS * 32) {
-    // ---- each lane prepares one request of the chunk ---------------------------------------------
-    bool el = false;
-    WarmReq q; q.T = -1.f; q.fr0 = q.fr1 = 0.f; q.tbt = 0.f; q.br0 = -1; q.r = -1; q.cur_hi = 0; q._pad = 0;
-    if (cbase + lane < n_req) {
-      const int r = rb_idx[rb_off[m] + cbase + lane];
-      const fs_request rq = reqs[r];
-      if (rq.L < (1u << 24) && rq.o_pred < (1u << 24)) {
-        const uint32_t O = (21u * rq.o_pred + 19u) / 20u;
-        const float mem = __fmul_rn(__uint2float_rn(rq.L + O), kv);
-        if (mem <= gi.mem_free_mb) {
-          el = true;
-          const uint32_t n0 = rq.L < (uint32_t)d.B ? rq.L : (uint32_t)d.B;
-          q.br0 = (n0 == (uint32_t)d.B || n0 == 0) ? -1 : (int)n0 - 1;
-          q.fr0 = n0 ? __uint2float_rn(fs_ceil_div(rq.L, n0)) : 0.0f;       // L == 0: t0 = e0 = 0
-          q.fr1 = __uint2float_rn(fs_ceil_div(O, (uint32_t)br1 + 1u));      // O == 0: e1 = 0
-          q.tbt = O > 0 ? rq.slo_tbt_ms : FS_INF;
-          q.T = rq.L > 0 ? fs_tstar(gi.t_avail_ms, rq.slo_ttft_ms) : FS_INF;
-          q.r = r; q.cur_hi = (uint32_t)(keys[r] >> 32);
-          if (pb == 0) { npairs += 1; ncand += (unsigned long long)smf * d.F; }
-        }
-      }
-    }
-    __syncwarp();
-    wr[lane] = q;
-    unsigned mask = __ballot_sync(0xffffffffu, el && q.T >= 0.0f);
-    __syncwarp();
-    // ---- sweep the eligible requests -----------------------------------------------------------------
-    while (mask) {
-      const int qi = __ffs(mask) - 1; mask &= mask - 1;
-      const WarmReq w = wr[qi];
-      float mn = FS_INF;
-      if (w.br0 < 0) {
-#define FS_WARM_STEP(s) {                                                               \
-        const float t0 = __fmul_rn(w.fr0, la0[s]);                                      \
-        const float ee = __fadd_rn(__fmul_rn(t0, pw0[s]), __fmul_rn(__fmul_rn(w.fr1, la1[s]), pw1[s])); \
-        if (t0 <= w.T && la1[s] <= w.tbt) mn = fminf(mn, ee); }
-        switch (smf) {
-          default:
-          case 16: FS_WARM_STEP(15) case 15: FS_WARM_STEP(14) case 14: FS_WARM_STEP(13)
-          case 13: FS_WARM_STEP(12) case 12: FS_WARM_STEP(11) case 11: FS_WARM_STEP(10)
-          case 10: FS_WARM_STEP(9)  case 9: FS_WARM_STEP(8)   case 8: FS_WARM_STEP(7)
-          case 7: FS_WARM_STEP(6)   case 6: FS_WARM_STEP(5)   case 5: FS_WARM_STEP(4)
-          case 4: FS_WARM_STEP(3)   case 3: FS_WARM_STEP(2)   case 2: FS_WARM_STEP(1)
-          case 1: FS_WARM_STEP(0)
-        }
-#undef FS_WARM_STEP
-      } else {                                          // short prompt: its own prefill plane, via L2
-        const size_t o0 = fs_plane(d, m, 0, w.br0) + phic, o1 = fs_plane(d, m, 1, br1) + phic;
-        // four shares per trip so that the 16 loads of a trip are in flight together
-#pragma unroll 1
-        for (int s4 = 0; s4 < smf; s4 += 4) {
-          float l0v[4], p0v[4], l1v[4], p1v[4];
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const size_t so = (size_t)min(s4 + u, smf - 1) * d.F;
-            l0v[u] = v.latT[o0 + so]; p0v[u] = v.powT[o0 + so];
-            l1v[u] = v.latT[o1 + so]; p1v[u] = v.powT[o1 + so];
-          }
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const float t0 = __fmul_rn(w.fr0, l0v[u]);
-            const float ee = __fadd_rn(__fmul_rn(t0, p0v[u]), __fmul_rn(__fmul_rn(w.fr1, l1v[u]), p1v[u]));
-            if (s4 + u < smf && t0 <= w.T && l1v[u] <= w.tbt) mn = fminf(mn, ee);
-          }
-        }
-      }
-      float dE = __fsub_rn(__fadd_rn(A, mn), ecur);     // monotone in mn
-      if (!(dE < FS_INF)) dE = FS_INF;                  // NaN / overflow: not a candidate
-      const uint32_t ord = fs_orderable(dE);
-      const uint32_t best = warp_min_u32(ord);
-      // (value, GPU) into the request's warm key: lowest k among equal minima, as the flat order
-      // wants; (sigma, phi) are recovered once per request by the decode kernel.
-      if (lane == 0 && best <= w.cur_hi && best < 0xFF800000u)
-        atomicMin(&wkeys[w.r], ((unsigned long long)best << 32) | (uint32_t)k);
-    }
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
-    ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
-  }
-  if (lane == 0 && stats && npairs) { atomicAdd(&stats[2], npairs); atomicAdd(&stats[3], ncand); }
 }
 
 // ---- decode: key -> fs_placement (one warp per request, lanes over phi for f_req) ----------
 __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
                                                           const fs_request* __restrict__ reqs,
                                                           const unsigned long long* __restrict__ keys,
-                                                          const unsigned long long* __restrict__ wkeys,
                                                           fs_placement* __restrict__ out) {
   const int lane = threadIdx.x & 31;
   const int r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (r >= R) return;
-  unsigned long long key = keys[r];
-  if (wkeys) {
-    // best warm pair (value, GPU): find its lowest (sigma, phi) and merge with the dense key
-    const unsigned long long wk = wkeys[r];
-    if (wk != FS_KEY_NONE && (uint32_t)(wk >> 32) <= (uint32_t)(key >> 32)) {
-      const FsDimsDev d = v.d;
-      const int k = (int)(uint32_t)wk; const uint32_t best = (uint32_t)(wk >> 32);
-      const ReqCtx c = make_req(v, reqs[r]);
-      const PairCtx p = make_pair(v, c, v.ginfo[k]);
-      uint32_t flat = 0xFFFFFFFFu;
-      for (int sg = 0; sg < p.smf && flat == 0xFFFFFFFFu; ++sg)
-        for (int phi = lane; phi < d.F; phi += 32) {
-          const Cand cd = eval_cand(v, c, p, k, sg, phi);
-          if (cd.ok && fs_orderable(cd.dE) == best) { flat = (uint32_t)((k * d.S + sg) * d.F + phi); break; }
-        }
-      unsigned long long cand = flat != 0xFFFFFFFFu ? (((unsigned long long)best << 32) | flat) : FS_KEY_NONE;
-      cand = fs_warp_min_key(cand);
-      key = cand < key ? cand : key;
-    }
-  }
+  const unsigned long long key = keys[r];
   fs_placement o;
   o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
   o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
@@ -631,10 +499,9 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   if (R <= 0) return 0;
   int launches = 0;
   cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-  cudaMemsetAsync(sc.wkeys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
   cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 8, st);
   if (v.K <= 0) {
-    place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, nullptr, out);
+    place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
   }
   const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= 64 && !sc.force_generic;
@@ -656,25 +523,11 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     const size_t smem = dense_smem_bytes(cps * FS_CHUNK);
     cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nslice, st);
     if (FT == 32)
-      place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.stats);
+      place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats);
     else
-      place_dense_kernel<2><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.stats);
+      place_dense_kernel<2><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats);
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
-    fs_tm_beg(tm, FS_T_PLACE_WARM, st);
-    {
-      cudaMemsetAsync(sc.rb_off, 0, sizeof(int32_t) * (size_t)(v.d.M + 1), st);
-      req_count_kernel<<<(R + 255) / 256, 256, 0, st>>>(reqs, R, v.d.M, sc.rb_off);
-      fs_bucket_scan_kernel<<<1, 1024, 0, st>>>(sc.rb_off, sc.rb_cursor, v.d.M);
-      req_fill_kernel<<<(R + 255) / 256, 256, 0, st>>>(reqs, R, v.d.M, sc.rb_off, sc.rb_cursor, sc.rb_idx);
-      const int nphib = FT / 32;
-      const long long warps = (long long)v.K * FS_RMAX * nphib * WARM_SLOTS;   // upper bound on items
-      place_warm_kernel<<<(unsigned)((warps + WARM_WARPS - 1) / WARM_WARPS), WARM_WARPS * 32, 0, st>>>(
-          v, R, reqs, sc.keys, sc.wkeys, sc.warm_off, sc.warm_item, sc.rb_off, sc.rb_idx, nphib, sc.stats);
-      launches += 3;
-    }
-    fs_tm_end(tm, FS_T_PLACE_WARM, st);
-    ++launches;
   } else {
     // split the GPUs of one request over several warps when R alone cannot fill the SMs
     const long long want_warps = (long long)sc.sm_count * 32;
@@ -690,7 +543,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   }
   fs_tm_beg(tm, FS_T_PLACE_DECODE, st);
-  place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, dense_ok ? sc.wkeys : nullptr, out);
+  place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
   fs_tm_end(tm, FS_T_PLACE_DECODE, st);
   ++launches;
   return launches;

@@ -129,26 +129,40 @@ __global__ void warm_count_kernel(FsView v, int32_t* __restrict__ cnt /*[M+1], z
     if (first) atomicAdd(&cnt[gi.model[i] + 1], 1);
   }
 }
-__global__ void warm_scan_kernel(int32_t* off /*[M+1]*/, int32_t* cursor /*[M]*/, int M) {
-  // single thread: M <= 32767, run once per fs_set_gpu_state
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
-    int acc = 0; off[0] = 0;
-    for (int m = 0; m < M; ++m) { acc += off[m + 1]; off[m + 1] = acc; cursor[m] = 0; }
-  }
-}
-__global__ void warm_fill_kernel(FsView v, const int32_t* __restrict__ off,
-                                 int32_t* __restrict__ cursor, uint32_t* __restrict__ item) {
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+// one warp per (GPU, slot): lanes over phi reduce the bounds the placement kernel prunes with
+__global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t* __restrict__ off,
+                                                       int32_t* __restrict__ cursor,
+                                                       FsWarmItem* __restrict__ items) {
+  const int lane = threadIdx.x & 31;
+  const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int k = w >> 2, i = w & 3;
   if (k >= v.K) return;
   const FsGpuInfo gi = v.ginfo[k];
-  for (int i = 0; i < gi.n_res; ++i) {
-    bool first = true;
-    for (int j = 0; j < i; ++j) first = first && (gi.model[j] != gi.model[i]);
-    if (first) {
-      const int m = gi.model[i];
-      const int pos = atomicAdd(&cursor[m], 1);
-      item[off[m] + pos] = (uint32_t)k * 4u + (uint32_t)i;
-    }
+  if (i >= gi.n_res) return;
+  for (int j = 0; j < i; ++j) if (gi.model[j] == gi.model[i]) return;   // not the join target
+  const FsDimsDev d = v.d;
+  const int m = gi.model[i], br1 = gi.br1[i];
+  float a_min = FS_INF, l1 = FS_INF, p1 = FS_INF;
+  for (int phi = lane; phi < d.F; phi += 32) {
+    a_min = fminf(a_min, v.gA[((size_t)k * FS_NVAR + 1 + i) * d.F + phi]);
+    if (br1 >= 0)
+      for (int sg = 0; sg < gi.sm_free; ++sg) {
+        const size_t o = fs_plane(d, m, 1, br1) + (size_t)sg * d.F + phi;
+        l1 = fminf(l1, v.latT[o]); p1 = fminf(p1, v.powT[o]);
+      }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
+    l1 = fminf(l1, __shfl_xor_sync(0xffffffffu, l1, o));
+    p1 = fminf(p1, __shfl_xor_sync(0xffffffffu, p1, o));
+  }
+  if (lane == 0) {
+    FsWarmItem it;
+    it.k = k; it.j = i; it.br1 = br1; it.sm_free = gi.sm_free;
+    it.t_avail_ms = gi.t_avail_ms; it.mem_free_mb = gi.mem_free_mb; it.e_cur = gi.e_cur;
+    it.a_min = a_min; it.l1_min = l1; it.p1_min = p1; it._pad[0] = it._pad[1] = 0;
+    items[off[m] + atomicAdd(&cursor[m], 1)] = it;
   }
 }
 
@@ -165,11 +179,11 @@ int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, fl
 }
 
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
-                         uint32_t* warm_item, cudaStream_t st) {
+                         FsWarmItem* items, cudaStream_t st) {
   if (v.K <= 0) return 0;
   cudaMemsetAsync(warm_off, 0, sizeof(int32_t) * (v.d.M + 1), st);
   warm_count_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, warm_off);
-  warm_scan_kernel<<<1, 32, 0, st>>>(warm_off, warm_cursor, v.d.M);
-  warm_fill_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, warm_off, warm_cursor, warm_item);
+  fs_bucket_scan_kernel<<<1, 1024, 0, st>>>(warm_off, warm_cursor, v.d.M);
+  warm_fill_kernel<<<(v.K * FS_RMAX + 3) / 4, 128, 0, st>>>(v, warm_off, warm_cursor, items);
   return 3;
 }
