@@ -31,8 +31,20 @@ from paper_2606_30391_b200 import synth  # noqa: E402
 
 METRIC = "placement_candidate_evals_per_sec"
 UNIT = "candidates/s"
-# SURVEY §8(d) / DESIGN.md "Roofline": lane-operations the method needs per evaluated candidate
-OPS_PER_CANDIDATE = 13.0
+# DESIGN.md §7 "Roofline": lane-operations (one 32-bit load / arithmetic / compare / select on one
+# lane) the method needs per unit of work, for the units the scoring kernel counts itself
+OPS_PER_CANDIDATE = 13.0   # dense definition: 8 fp32 arithmetic + 5 compare/select
+OPS_TILE = 14.0            # per (request, sigma, phi): 4 table loads, 5 fp32, 2 tests, 3 running minima
+OPS_PAIR_TEST = 18.0       # per (request, GPU) tested: 8-word record, 7 eligibility compares, bound (2 fp32 + compare)
+OPS_TSTAR = 12.0           # per swept pair: deadline threshold T*
+OPS_SWEEP = 2.0            # per swept candidate: compare + predicated min
+OPS_ROW = 4.0              # per swept (pair, phi): A0 load, add, min, subtract/compare share
+OPS_WARM_TEST = 20.0       # per warm pair tested: 12-word item, bound (5 fp32), 3 compares
+OPS_DEF = 14.0             # per candidate scored by the definition: 4 loads, 4 mul, 3 add/sub, 3 compares
+# dram bytes per launch of the scoring kernel and its issue utilisation, from the committed ncu
+# capture of this workload (profiles/; a profiler cannot run inside the timed bench)
+NCU_TRAFFIC_BYTES = 43.7e6
+NCU_NOTE = "profiles/r01_place_dense_ncu_full.md"
 SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128   # 4 schedulers x 32 lanes (B300_MICROARCH "issue")
 
 
@@ -206,10 +218,31 @@ def run_ours(args):
     wall = time.perf_counter() - wall0
     launches = ctx.launch_count - l0
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
+    # work counters: one untimed call of the counting instantiation (same input, same work)
+    ctx.set_work_stats(True)
+    ctx.place_batch(d_reqs, out=d_place, stream=stream)
     pstats = ctx.last_place_stats()
-    pairs = pstats["dense_pairs"] + pstats["warm_pairs"]
-    cand_exec = pstats["dense_candidates"] + pstats["warm_candidates"]
-    cand_dense = pstats["dense_candidates"]
+    ctx.set_work_stats(False)
+    useful_ops = (OPS_TILE * pstats["requests"] * cl.S * cl.F + OPS_PAIR_TEST * 32 * pstats["chunks_tested"]
+                  + OPS_TSTAR * pstats["cold_pairs_swept"] + OPS_SWEEP * pstats["cold_candidates_swept"]
+                  + OPS_ROW * cl.F * pstats["cold_pairs_swept"] + OPS_WARM_TEST * pstats["warm_pairs_tested"]
+                  + OPS_DEF * pstats["candidates_scored"])
+    # the dense definition's work: every eligible (request, GPU) pair x sm_free x F, counted by the
+    # generic kernel (no pruning) on a second context; also an on-GPU cross-check of the two kernels
+    os.environ["FS_FORCE_GENERIC"] = "1"
+    ctx_g = fs.Festina(lrank)
+    del os.environ["FS_FORCE_GENERIC"]
+    ctx_g.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                        tb(cl.models), cl.params)
+    ctx_g.set_gpu_state(d_states, stream=stream)
+    ctx_g.set_work_stats(True)
+    d_place_g = torch.empty_like(d_place)
+    ctx_g.place_batch(d_reqs, out=d_place_g, stream=stream)
+    gstats = ctx_g.last_place_stats()
+    torch.cuda.synchronize()
+    assert torch.equal(d_place_g, d_place), "generic and dense scoring kernels disagree"
+    ctx_g.close()
+    pairs, cand_def = gstats["cold_pairs_eligible"], gstats["candidates_scored"]
 
     # end to end through the C ABI with pinned host buffers
     h_states = torch.from_numpy(cl.states.view(np.uint8).reshape(-1).copy()).pin_memory()
@@ -244,14 +277,15 @@ def run_ours(args):
         if dist is not None:
             dist.destroy_process_group()
         return
-    nominal = cl.R * cl.K * cl.S * cl.F
+    grid_cands = cl.R * cl.K * cl.S * cl.F
     steps = args.steps
-    value = ws * nominal * steps / (dev_ms * 1e-3)
+    value = ws * grid_cands * steps / (dev_ms * 1e-3)
     peaks, peak_src = _peaks()
     sm_clk_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     alu_peak = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * sm_clk_hz          # lane-instructions / s
     score_ms = float(np.mean(kt.get("place_score", [float("nan")])))
-    achieved = OPS_PER_CANDIDATE * cand_dense / (score_ms * 1e-3)
+    achieved = useful_ops / (score_ms * 1e-3)
+    nominal = OPS_PER_CANDIDATE * cand_def / (score_ms * 1e-3)
     place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
     ok = place["gpu"] >= 0
     line = {
@@ -260,20 +294,26 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic", "config": _config(cl, args),
         "decisions_per_sec": ws * (cl.R + cl.K) * steps / (dev_ms * 1e-3),
         "placement_decisions_per_sec": ws * cl.R * steps / (dev_ms * 1e-3),
-        "executed_candidates_per_step": cand_exec, "eligible_pairs_per_step": pairs, "place_stats": pstats,
-        "nominal_candidates_per_step": nominal,
+        "nominal_candidates_per_step": grid_cands, "eligible_candidates_per_step": cand_def,
+        "eligible_pairs_per_step": pairs, "place_stats": pstats,
         "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
         "wall_ms_per_step_incl_flush": wall_ms / steps,
-        "e2e": {"value": ws * nominal * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
+        "e2e": {"value": ws * grid_cands * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
                 "h2d_bytes_per_step": cl.K * 128 + cl.R * 32, "d2h_bytes_per_step": cl.R * 32 + cl.K * 48},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": "fs_place_batch scorer", "achieved": achieved / 1e12,
-                     "peak": alu_peak / 1e12, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
-                     "traffic": None,
-                     "note": f"{OPS_PER_CANDIDATE:g} lane-ops per evaluated candidate (DESIGN.md) x "
-                             f"{cand_dense} dense-kernel candidates / {score_ms:.3f} ms; peak = 148 SMs x 128 lanes/clk x "
-                             f"{sm_clk_hz / 1e6:.0f} MHz ({peak_src} sm_max_mhz)"},
+        "roofline": {"bound": "alu", "kernel": "place_dense_kernel (fs_place_batch scoring + argmin)",
+                     "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tlane-op/s",
+                     "frac": achieved / alu_peak, "traffic": NCU_TRAFFIC_BYTES,
+                     "useful_lane_ops_per_launch": useful_ops, "kernel_ms": score_ms,
+                     "dense_definition": {"achieved": nominal / 1e12, "frac": nominal / alu_peak,
+                                          "note": f"{OPS_PER_CANDIDATE:g} lane-ops x {cand_def} eligible candidates "
+                                                  "(counted by the unpruned generic kernel); above 1 because "
+                                                  "exact pruning skips most of them"},
+                     "ncu": NCU_NOTE,
+                     "note": "achieved = lane-ops of the units the kernel counted itself (DESIGN.md section 7 "
+                             "per-unit figures) / CUDA-event time of the launch; peak = 148 SMs x 128 lanes/clk x "
+                             f"{sm_clk_hz / 1e6:.0f} MHz ({peak_src} sm_max_mhz); traffic from the committed ncu capture"},
         "degeneracy": {"placed_frac": float(ok.mean()),
                        "top_phi_share": float(np.bincount(place["phi"][ok]).max() / max(ok.sum(), 1)),
                        "distinct_gpus": int(len(np.unique(place["gpu"][ok])))},

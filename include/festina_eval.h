@@ -180,11 +180,17 @@ const char* fs_strerror(int code);
 int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed runtime call */
 /* Kernels launched by this context since creation (bench.py's gpu_launches counter).     */
 uint64_t fs_launch_count(const fs_ctx* ctx);
-/* Work of the last fs_place_batch, counted on the device (this call synchronises the device):
- * out[0], out[1] = eligible COLD (request, GPU) pairs (model not resident; all pairs when the generic
- * kernel ran) and their candidates (sum of sm_free*F) by the method's definition; out[2], out[3] =
- * the same for WARM pairs (model resident); out[4..5] / out[6..7] = cold / warm pairs and candidates
- * actually evaluated after the exact lower-bound pruning.                                  */
+/* Work counters of fs_place_batch (measurement only).  fs_set_work_stats(ctx, 1) makes later
+ * fs_place_batch calls run the counting instantiation of the scoring kernel (same results, a
+ * little slower); fs_last_place_stats copies the counters of the most recent such call
+ * (it synchronises the device):
+ *   out[0] chunks of 32 GPU records tested (lane <-> GPU: eligibility + lower bound)
+ *   out[1] cold (request, GPU) pairs found eligible      out[2] cold pairs swept after pruning
+ *   out[3] cold candidates swept (sum of sm_free*F)      out[4] warm (model resident) pairs tested
+ *   out[5] pairs scored candidate by candidate with the definition (warm pairs + tie recovery;
+ *          every eligible pair when the generic kernel ran)
+ *   out[6] candidates scored that way                    out[7] requests processed (x GPU slices) */
+int fs_set_work_stats(fs_ctx* ctx, int on);
 int fs_last_place_stats(fs_ctx* ctx, uint64_t out[8]);
 
 /* Per-kernel device timing for measurement (bench.py's roofline line).  fs_set_timing(ctx, 1)

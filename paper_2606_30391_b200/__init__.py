@@ -24,7 +24,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
            "fs_local_config", "fs_consolidate", "fs_strerror", "fs_last_cuda_error",
-           "fs_launch_count", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
+           "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm")
 
@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
     L.fs_last_cuda_error.argtypes = [vp]
     L.fs_launch_count.argtypes = [vp]
     L.fs_launch_count.restype = C.c_uint64
+    L.fs_set_work_stats.argtypes = [vp, C.c_int]
     L.fs_last_place_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
     L.fs_set_timing.argtypes = [vp, C.c_int]
     L.fs_get_timing.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
@@ -204,14 +205,16 @@ class Festina:
     def launch_count(self) -> int:
         return int(lib().fs_launch_count(self._h))
 
+    def set_work_stats(self, on: bool = True):
+        self._check(lib().fs_set_work_stats(self._h, int(on)), "fs_set_work_stats")
+
     def last_place_stats(self) -> dict:
-        """Eligible pairs / candidates the last fs_place_batch evaluated, dense and warm kernels."""
+        """Work counters of the last fs_place_batch run with set_work_stats(True) (festina_eval.h)."""
         o = (C.c_uint64 * 8)()
         self._check(lib().fs_last_place_stats(self._h, o), "fs_last_place_stats")
-        return {"dense_pairs": int(o[0]), "dense_candidates": int(o[1]), "warm_pairs": int(o[2]),
-                "warm_candidates": int(o[3]), "dense_swept_pairs": int(o[4]),
-                "dense_swept_candidates": int(o[5]), "warm_swept_pairs": int(o[6]),
-                "warm_swept_candidates": int(o[7])}
+        names = ("chunks_tested", "cold_pairs_eligible", "cold_pairs_swept", "cold_candidates_swept",
+                 "warm_pairs_tested", "pairs_scored", "candidates_scored", "requests")
+        return {n: int(o[i]) for i, n in enumerate(names)}
 
     def set_timing(self, on: bool = True):
         self._check(lib().fs_set_timing(self._h, int(on)), "fs_set_timing")

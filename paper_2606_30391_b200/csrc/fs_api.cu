@@ -23,7 +23,7 @@ struct fs_ctx {
   // state + summaries
   int K = 0, k_cap = 0;
   fs_gpu_state* states = nullptr; FsGpuInfo* ginfo = nullptr; float* gA = nullptr; size_t gA_cap = 0;
-  FsGpuRec* grec = nullptr; float* gA0 = nullptr; size_t gA0_cap = 0; int Kpad = 0, FT = 32;
+  FsGpuRec* grec = nullptr; FsGpuRec* gsort = nullptr; double *dsort = nullptr, *dsuf = nullptr; float* gA0 = nullptr; size_t gA0_cap = 0; int Kpad = 0, FT = 32;
   int32_t *warm_off = nullptr, *warm_cursor = nullptr; FsWarmItem* warm_item = nullptr; int warm_m_cap = 0;
   // placement scratch
   int r_cap = 0; unsigned long long* keys = nullptr; unsigned long long* stats = nullptr;
@@ -41,7 +41,7 @@ struct fs_ctx {
   int* flag_host = nullptr; int* flag_dev = nullptr;
   uint64_t launches = 0; int last_cuda = 0;
   bool timing = false; bool have_events = false; FsTimers tm{};
-  int sm_count = 148; bool force_generic = false;
+  int sm_count = 148; bool force_generic = false, count_work = false;
 };
 
 namespace {
@@ -82,7 +82,7 @@ FsView view_of(const fs_ctx* c) {
   v.d = FsDimsDev{c->d.M, c->d.F, c->d.S, c->d.B};
   v.lat = c->lat; v.pow = c->pow; v.latT = c->latT; v.powT = c->powT; v.models = c->models;
   v.K = c->K; v.states = c->states; v.ginfo = c->ginfo; v.gA = c->gA; v.flag = c->flag_dev;
-  v.grec = c->grec; v.gA0 = c->gA0; v.Kpad = c->Kpad; v.FT = c->FT;
+  v.grec = c->grec; v.gA0 = c->gA0; v.Kpad = c->Kpad; v.FT = c->FT; v.gsort = c->gsort; v.dsuf = c->dsuf;
   return v;
 }
 
@@ -153,7 +153,7 @@ int fs_destroy(fs_ctx* c) {
   cudaSetDevice(c->dev);
   cudaDeviceSynchronize();
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
-                  c->ginfo, c->gA, c->grec, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
+                  c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -219,7 +219,8 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   const int pending = take_flags(c);
   if (K > c->k_cap) {
     FS_TRY(grow(c, c->states, (size_t)K)); FS_TRY(grow(c, c->ginfo, (size_t)K));
-    FS_TRY(grow(c, c->grec, (size_t)K + FS_CHUNK));
+    FS_TRY(grow(c, c->grec, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->gsort, (size_t)K + FS_CHUNK));
+    FS_TRY(grow(c, c->dsort, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->dsuf, (size_t)K / FS_CHUNK + 4));
     FS_TRY(grow(c, c->ctr, (size_t)K / FS_CHUNK + 2));
     FS_TRY(grow(c, c->warm_item, (size_t)K * FS_RMAX));
     c->k_cap = K; c->consol_cap = 0;
@@ -237,7 +238,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (K > 0) {
     FS_CUDA(c, cudaMemcpyAsync(c->states, states, (size_t)K * sizeof(fs_gpu_state), in_kind(space), st));
     FsView v = view_of(c);
-    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0, st, c->timing ? &c->tm : nullptr);
+    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0, c->gsort, c->dsort, c->dsuf, st, c->timing ? &c->tm : nullptr);
     c->launches += fsk_build_warm_lists(v, c->warm_off, c->warm_cursor, c->warm_item, st);
     FS_TRY(check_kernel(c));
   }
@@ -264,7 +265,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
-  FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic};
+  FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic, c->count_work};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
@@ -386,6 +387,12 @@ int fs_get_timing(fs_ctx* c, float* ms, int n) {
       FS_CUDA(c, cudaEventElapsedTime(&ms[i], c->tm.beg[i], c->tm.end[i]));
     }
   }
+  return FS_OK;
+}
+
+int fs_set_work_stats(fs_ctx* c, int on) {
+  if (!c) return FS_ERR_ARG;
+  c->count_work = on != 0;
   return FS_OK;
 }
 

@@ -46,7 +46,7 @@ struct __align__(16) FsGpuRec {
   uint32_t meta;            // n_res | sm_free << 8   (n_res == 0: never a candidate)
   int16_t model[FS_RMAX];
   float a_min;              // min over phi of A0[k][phi] (+INF: co-residents never feasible)
-  uint32_t _pad;
+  uint32_t k;               // GPU index (the sorted copy is not in index order)
 };
 static_assert(sizeof(FsGpuRec) == 32, "FsGpuRec layout");
 // One (GPU k, tenant slot j) that hosts a model: what a request of that model needs to bound and

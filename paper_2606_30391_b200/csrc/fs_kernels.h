@@ -32,6 +32,8 @@ struct FsView {
   const float* gA0;         // [Kpad][FT]       variant 0 of gA, row stride FT = F rounded up to 32,
                             //                  padding = INF (what the dense kernel stages by TMA)
   int Kpad, FT;
+  const FsGpuRec* gsort;    // [Kpad]           grec in the dense kernel's scan order (fs_summary.cu)
+  const double* dsuf;       // [Kpad/32 + 2]    [0] magnitude bound, [1+c] suffix minimum of d from chunk c on
   int* flag;                // sticky range-error flag (mapped host memory)
 };
 
@@ -41,18 +43,21 @@ int fsk_build_planes(const float* lat, const float* pow, float* latT, float* pow
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
 int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
-                cudaStream_t st, FsTimers* tm);
+                FsGpuRec* gsort, double* dsort, double* dsuf, cudaStream_t st, FsTimers* tm);
 
 // fs_place.cu — placement scoring + 64-bit-key argmin + decode
 struct FsPlaceScratch {
   unsigned long long* keys;        // [R]  (dE, flat) argmin keys
-  unsigned long long* stats;       // [8]: dense pairs, dense pairs/cands, warm pairs/cands, dense swept pairs/cands, warm swept pairs/cands
+  unsigned long long* stats;       // [8] work counters of the last call: chunks of 32 GPUs tested, cold pairs
+                                   // eligible, cold pairs swept, cold candidates swept, warm items tested, pairs
+                                   // scored by the definition, candidates scored by the definition, requests
   unsigned int* ctr;               // [nslice <= Kpad/32] dynamic request counters of the dense kernel
   // bucketing of GPUs by model (built by fs_set_gpu_state): warm lists
   const int32_t* warm_off;         // [M+1]
   const FsWarmItem* witems;        // [<= 4K] items, grouped by model
   int sm_count;                    // SMs of the device (grid sizing)
   bool force_generic;              // diagnostics: score with the generic kernel only
+  bool count_work;                 // fill `stats` (fs_set_work_stats): a second instantiation of the kernel
 };
 int fsk_place_smem_attr();
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,

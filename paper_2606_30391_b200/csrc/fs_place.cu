@@ -116,31 +116,36 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
   key = fs_warp_min_key(key);
   if (lane == 0) {
     if (key != FS_KEY_NONE) atomicMin(&keys[r], key);
-    if (stats) { atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand); }
+    if (stats) { atomicAdd(&stats[1], npairs); atomicAdd(&stats[5], npairs); atomicAdd(&stats[6], ncand); }
   }
 }
 
 
 // =============================================================================================
-// Dense scorer for COLD pairs (the request's model is not resident on the GPU), S <= 16, F <= 64.
+// Dense scorer, S <= 16, F <= 64: one warp = one request, one persistent block per SM.
 //
-// Factorisation (exact): for a cold pair the decode bucket is 0 and
-// the co-resident variant is 0, so everything that depends on (sigma, phi) is per REQUEST:
+// Factorisation (exact).  For a COLD pair (the request's model is
+// not resident on the GPU) the decode bucket is 0 and the co-resident variant is 0, so everything
+// that depends on (sigma, phi) is per REQUEST:
 //   t0[s][f] = fl(rounds0*LAT0)                    er[s][f] = fl(e0 + e1), INF where LAT1 > slo_tbt
 // and everything that depends on the GPU is per (k, phi):  A0[k][f], Ecur[k], wait_k, sm_free_k.
 // fl(A + x) and fl(x - Ecur) are monotone in x, hence
 //   min_s fl(fl(A0 + er[s]) - Ecur) = fl(fl(A0 + min_s er[s]) - Ecur)   over feasible s,
 // and fl(wait + t) <= slo  <=>  t <= T*(wait, slo) for the exactly computed threshold T*.
-// Per candidate that leaves one compare and one conditional min, on registers.
 //
-// Layout: one warp = one request, lane owns NPHI adjacent frequencies and all 16 shares
-// (2*16*NPHI registers).  A block walks the GPUs in chunks of 32 staged by 1-D TMA bulk copies
-// (records + A0 rows) through an mbarrier ring shared by its warps; each lane first evaluates
-// eligibility and T* for ONE GPU of the chunk, then the warp sweeps the eligible GPUs.
-// The lowest flat index among equal minima is recovered exactly at the end (see below).
+// Per request the warp (a) builds the two tiles in its own shared-memory region, one row per
+// share, together with prefix minima over the shares (pruning bounds); (b) walks the GPUs in
+// ascending d = a_min - Ecur, lane <-> GPU: eligibility and the exact lower bound
+// fl(fl(a_min + bnd[sm_free]) - Ecur) against the incumbent; the few survivors are swept
+// (compare + predicated min per candidate); the walk stops when no later GPU can win;
+// (c) scores the WARM pairs (model resident: decode bucket, variant and wait depend on the GPU)
+// best bound first, candidate by candidate, and (d) re-scores the winning GPU once to recover the
+// lowest flat index attaining the minimum.  All loops are rolled and the tiles live in shared
+// memory so that the whole kernel stays inside the 32 KB instruction cache (profiles/: the
+// register-tiled, fully unrolled version spent 64 % of its stall samples on instruction fetch).
 // =============================================================================================
-constexpr int DENSE_WARPS = 16;
-constexpr int DENSE_SMEM_MAX = 200 * 1024;   // of the 227 KB a block may use
+constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102)
+constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
 constexpr int DENSE_S = 16;
 
 __device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) {
@@ -180,15 +185,16 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
   return tstar_bisect(w, slo);
 }
 
-// Shared memory of one block: the compact records of its SLICE of the GPUs stay resident for the
-// whole kernel (one TMA fill), so the warps never synchronise with each other afterwards.
-//   rec [KS]              compact GPU records (32 B each)
-//   wb  [DENSE_WARPS][32] per warp: {T*, Ecur, sm_free, GPU} of the chunk being swept
-//   bnd [DENSE_WARPS][32] per warp: prefix minima of er / t0 over shares (pruning bounds)
-// The A0 rows of the few GPUs that survive the pruning are read through L1/L2.
-__host__ __device__ inline size_t dense_smem_bytes(int KS) {
-  return (size_t)KS * sizeof(FsGpuRec) + (size_t)DENSE_WARPS * FS_CHUNK * sizeof(float4) +
-         (size_t)DENSE_WARPS * 3 * DENSE_S * sizeof(float) + 16;
+// Shared memory of one block:
+//   rec  [KS]            the block's slice of the SORTED compact GPU records (one TMA fill)
+//   tile [W][2][S][FT]   per warp: t0 rows, then er rows, of the request being scored
+//   wb   [W][32]         per warp: {T*, Ecur, sm_free, GPU} of the chunk's survivors
+//   bnd  [W][3][16]      per warp: prefix minima over sigma <= s, all phi, of er (cold), t0, e0
+__host__ __device__ inline size_t dense_warp_bytes(int S, int FT) {
+  return (size_t)2 * S * FT * sizeof(float) + FS_CHUNK * sizeof(float4) + 3 * DENSE_S * sizeof(float);
+}
+__host__ __device__ inline size_t dense_smem_bytes(int KS, int W, int S, int FT) {
+  return (size_t)KS * sizeof(FsGpuRec) + (size_t)W * dense_warp_bytes(S, FT) + 16;
 }
 
 // NPHI adjacent values of row `o` for the lane whose first column is phi0 (columns clamped to the
@@ -205,42 +211,78 @@ __device__ __forceinline__ void ld_cols(const float* __restrict__ base, int o, i
   }
 }
 
+// work statistics (what this launch actually did; bench.py turns them into lane-operations)
+__device__ __forceinline__ void flush_stats(unsigned long long* stats, uint32_t n_chunks, uint32_t n_elig,
+                                         uint32_t n_swept, uint32_t n_cswept, uint32_t n_witems,
+                                         uint32_t n_scored, uint32_t n_cscored, uint32_t n_req) {
+  if (!stats) return;
+  unsigned long long e = n_elig, w = n_witems;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    e += __shfl_xor_sync(0xffffffffu, e, o);
+    w += __shfl_xor_sync(0xffffffffu, w, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&stats[0], (unsigned long long)n_chunks); atomicAdd(&stats[1], e);
+    atomicAdd(&stats[2], (unsigned long long)n_swept); atomicAdd(&stats[3], (unsigned long long)n_cswept);
+    atomicAdd(&stats[4], w); atomicAdd(&stats[5], (unsigned long long)n_scored);
+    atomicAdd(&stats[6], (unsigned long long)n_cscored); atomicAdd(&stats[7], (unsigned long long)n_req);
+  }
+}
+
 template <int NPHI>
-__global__ void __launch_bounds__(DENSE_WARPS * 32, 1)
+__device__ __forceinline__ void ld_tile(const float* p, float (&x)[NPHI]) {
+  if (NPHI == 2) { const float2 t = *reinterpret_cast<const float2*>(p); x[0] = t.x; x[NPHI - 1] = t.y; }
+  else x[0] = p[0];
+}
+template <int NPHI>
+__device__ __forceinline__ void st_tile(float* p, const float (&x)[NPHI]) {
+  if (NPHI == 2) *reinterpret_cast<float2*>(p) = make_float2(x[0], x[NPHI - 1]);
+  else p[0] = x[0];
+}
+
+template <int NPHI, bool STATS>
+__global__ void __launch_bounds__(DENSE_MAXW * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
                    unsigned int* __restrict__ ctr, const int32_t* __restrict__ warm_off,
                    const FsWarmItem* __restrict__ witems, unsigned long long* __restrict__ stats) {
   extern __shared__ __align__(128) unsigned char dense_smem_raw[];
   constexpr int FT = 32 * NPHI;
+  constexpr uint32_t NONE32 = 0xFFFFFFFFu, INFBITS = 0x7F800000u;
+  constexpr int KNONE = 0x7FFFFFFF;
   const FsDimsDev d = v.d;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
   const int nchunk_all = v.Kpad / FS_CHUNK;
   const int slice = blockIdx.x % nslice;
   const int c0 = slice * chunks_per_slice, c1 = min(nchunk_all, c0 + chunks_per_slice);
   const int nchunk = c1 - c0, KS = nchunk * FS_CHUNK, KSmax = chunks_per_slice * FS_CHUNK;
   FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw);
-  float4* s_wb = reinterpret_cast<float4*>(dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec));
-  float* s_bnd = reinterpret_cast<float*>(s_wb + DENSE_WARPS * FS_CHUNK);   // [warp][2][16] prefix minima
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_bnd + DENSE_WARPS * 3 * DENSE_S);
-  const float* gA0 = v.gA0 + (size_t)c0 * FS_CHUNK * FT;   // rows of this slice
+  unsigned char* s_warp = dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec) + (size_t)warp * dense_warp_bytes(d.S, FT);
+  float* tl_t0 = reinterpret_cast<float*>(s_warp);
+  float* tl_er = tl_t0 + d.S * FT;
+  float4* wb = reinterpret_cast<float4*>(tl_er + d.S * FT);
+  float* bnd = reinterpret_cast<float*>(wb + FS_CHUNK);
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec) +
+                                                (size_t)W * dense_warp_bytes(d.S, FT));
 
-  // ---- stage this block's GPU records once: 1-D TMA bulk copies completing on one mbarrier ------
+  // ---- stage this block's slice of the SORTED GPU records once: 1-D TMA bulk copies on one mbarrier
   if (threadIdx.x == 0) { fs_mbar_init(s_bar, 1); fs_mbar_fence_init(); }
   __syncthreads();
   if (threadIdx.x == 0) {
     const uint32_t bytes_rec = (uint32_t)KS * sizeof(FsGpuRec);
     fs_mbar_expect_tx(s_bar, bytes_rec);
-    const char* src = reinterpret_cast<const char*>(v.grec + (size_t)c0 * FS_CHUNK);
+    const char* src = reinterpret_cast<const char*>(v.gsort + (size_t)c0 * FS_CHUNK);
     char* dst = reinterpret_cast<char*>(s_rec);
     for (uint32_t off = 0; off < bytes_rec; off += 32768u)
       fs_tma_load_1d(dst + off, src + off, min(32768u, bytes_rec - off), s_bar);
   }
   fs_mbar_wait(s_bar, 0);
 
-  float4* wb = s_wb + warp * FS_CHUNK;
-  float* bnd = s_bnd + warp * 3 * DENSE_S;      // prefix minima over sigma <= s, all phi, of [0] er (cold), [1] t0, [2] e0
-  unsigned long long npairs = 0, ncand = 0, nswept = 0, ncswept = 0, wpairs = 0, wcand = 0, wswept = 0, wcswept = 0;
+  const double* dsuf = v.dsuf + 1 + c0;
+  const double amax = v.dsuf[0];
+  // work counters (warp-uniform except n_elig / n_witems, which are per lane)
+  uint32_t n_chunks = 0, n_elig = 0, n_swept = 0, n_cswept = 0, n_witems = 0, n_scored = 0, n_cscored = 0, n_req = 0;
   const bool vec = NPHI == 2 && (d.F & 1) == 0;
   const int phi0 = lane * NPHI;
   for (;;) {
@@ -251,206 +293,196 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     if (r >= R) break;
     const ReqCtx c = make_req(v, reqs[r]);
     if (!c.valid) { if (lane == 0 && slice == 0) fs_raise(v.flag, FS_FLAG_REQUEST); continue; }
-    // ---- phase A: the request's (sigma, phi) tiles in registers -------------------------------
+    // ---- (a) the request's (sigma, phi) tiles, one row per share, and the pruning bounds:
+    // every candidate of a GPU with sm_free = s has  er >= bnd[0][s-1], t0 >= bnd[1][s-1],
+    // e0 >= bnd[2][s-1]; hence, for a cold pair,  dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)
+    // (monotone rounding).  er, t0, e0 >= +0, so their bit patterns order like unsigned integers.
     // L == 0 / O == 0 need no branches: rounds = 0 gives t = e = +0 exactly (tables are finite),
     // and an empty decode slot passes its deadline (threshold +INF).
-    float t0[DENSE_S][NPHI], er[DENSE_S][NPHI];
+    const float* pw0 = v.powT + fs_plane(d, c.m, 0, c.br0);
     {
-      const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
+      const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0);
       const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
       const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
-      uint32_t pe0 = 0x7F800000u;                       // running prefix min of e0 (bits; e0 >= +0)
+      uint32_t pe = INFBITS, pt = INFBITS, pe0 = INFBITS;   // running prefix minima (bits)
       __syncwarp();
-#pragma unroll
-      for (int s4 = 0; s4 < DENSE_S; s4 += 4) {
-        float a0[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {                  // 16 independent loads in flight
-          const int o = min(s4 + u, d.S - 1) * d.F;
-          ld_cols<NPHI>(l0, o, phi0, d.F, vec, a0[u]); ld_cols<NPHI>(p0, o, phi0, d.F, vec, b0[u]);
-          ld_cols<NPHI>(l1, o, phi0, d.F, vec, a1[u]); ld_cols<NPHI>(p1, o, phi0, d.F, vec, b1[u]);
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          uint32_t ue0 = 0x7F800000u;
-#pragma unroll
-          for (int i = 0; i < NPHI; ++i) {
-            const float tt = __fmul_rn(fr0, a0[u][i]);
-            const float e0 = __fmul_rn(tt, b0[u][i]);
-            const float ee = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
-            const bool in = (s4 + u) < d.S && (phi0 + i) < d.F;
-            t0[s4 + u][i] = in ? tt : FS_INF;
-            er[s4 + u][i] = (in && a1[u][i] <= tbt) ? ee : FS_INF;
-            if (in) ue0 = min(ue0, __float_as_uint(e0));
-          }
-          pe0 = min(pe0, warp_min_u32(ue0));
-          if (lane == 0) bnd[2 * DENSE_S + s4 + u] = __uint_as_float(pe0);
-        }
-      }
-    }
-    // ---- bounds for exact pruning: every candidate of a GPU with sm_free = s has
-    //   er >= bnd[0][s-1], t0 >= bnd[1][s-1], e0 >= bnd[2][s-1]
-    // hence, for a cold pair,  dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)   (monotone rounding).  er, t0 >= +0, so their bit patterns order like unsigned integers.
-    {
-      uint32_t pe = 0x7F800000u, pt = 0x7F800000u;
-#pragma unroll
-      for (int s = 0; s < DENSE_S; ++s) {
-        uint32_t ue = 0x7F800000u, ut = 0x7F800000u;
+#pragma unroll 2
+      for (int s = 0; s < d.S; ++s) {
+        float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI], tt[NPHI], ee[NPHI];
+        const int o = s * d.F;
+        ld_cols<NPHI>(l0, o, phi0, d.F, vec, a0); ld_cols<NPHI>(pw0, o, phi0, d.F, vec, b0);
+        ld_cols<NPHI>(l1, o, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, o, phi0, d.F, vec, b1);
+        uint32_t ue = INFBITS, ut = INFBITS, ue0 = INFBITS;
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) {
-          ue = min(ue, __float_as_uint(er[s][i])); ut = min(ut, __float_as_uint(t0[s][i]));
+          const float t = __fmul_rn(fr0, a0[i]);
+          const float e0 = __fmul_rn(t, b0[i]);
+          const float e = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[i]), b1[i]));
+          const bool in = (phi0 + i) < d.F;
+          tt[i] = in ? t : FS_INF;
+          ee[i] = (in && a1[i] <= tbt) ? e : FS_INF;
+          if (in) ue0 = min(ue0, __float_as_uint(e0));
+          ue = min(ue, __float_as_uint(ee[i])); ut = min(ut, __float_as_uint(tt[i]));
         }
-        pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut));
-        if (lane == 0) { bnd[s] = __uint_as_float(pe); bnd[DENSE_S + s] = __uint_as_float(pt); }
+        st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
+        pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut)); pe0 = min(pe0, warp_min_u32(ue0));
+        if (lane == 0) {
+          bnd[s] = __uint_as_float(pe); bnd[DENSE_S + s] = __uint_as_float(pt);
+          bnd[2 * DENSE_S + s] = __uint_as_float(pe0);
+        }
       }
       __syncwarp();
     }
-    float best = FS_INF; int bestk = -1;
-    for (int ci = 0; ci < nchunk; ++ci) {
-      // best value found so far by any lane (all from GPUs with a lower index than this chunk's)
+    // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scan is not in index order
+    float best = FS_INF; int bestk = KNONE;
+    // ---- (b) cold pairs: GPUs in ascending d = a_min - Ecur.  Every candidate of every GPU from
+    // chunk ci on has  dE >= fl(fl(a + b) - e)  with  a - e >= dsuf[ci],  b >= bmin,  a <= amax,
+    // and two roundings lose at most 2^-23 (a + b + |a + b - e|); the scan stops as soon as that
+    // (with twice the slack) exceeds the incumbent, strictly, so ties still meet every GPU.
+    const float bminf = bnd[d.S - 1];
+    const double bmin = (double)bminf;
+    for (int ci = 0; ci < nchunk && bminf < FS_INF; ++ci) {
       const float bestW = fs_unorderable(warp_min_u32(fs_orderable(best)));
-      // ---- eligibility + T*: lane <-> one GPU of the chunk ------------------------------------
+      const double ds = dsuf[ci];
+      if (!(ds < (double)FS_INF)) break;                 // sentinels only from here on
+      if (bestW < FS_INF) {
+        const double x = ds + bmin;
+        if (x - 0x1p-22 * (amax + bmin + fabs(x)) - 1e-37 > (double)bestW) break;
+      }
+      if (STATS) { n_chunks += 1; }
+      // ---- eligibility + bound: lane <-> one GPU of the chunk ---------------------------------
       const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
-      const int n_res = g.meta & 0xFF, smf = (g.meta >> 8) & 0xFF;
-      bool el = n_res >= 1 && n_res < FS_RMAX && smf >= 1 && (c.mem <= g.mem_free_mb);
-#pragma unroll
-      for (int i = 0; i < FS_RMAX; ++i) el = el && (g.model[i] != c.m);   // resident -> warm path
+      const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
+      const uint32_t mm = (uint32_t)c.m * 0x00010001u;
+      const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
+      const bool el = (c.mem <= g.mem_free_mb) && !(__vcmpeq2(gm[0], mm) | __vcmpeq2(gm[1], mm));
       float T = -1.0f;
       if (el) {
-        npairs += 1; ncand += (unsigned long long)smf * d.F;
-        // prune: no candidate of this GPU can beat (or, having a higher index, tie) bestW
+        if (STATS) { n_elig += 1; }
+        // prune: no candidate of this GPU can beat or tie the best found so far
         const float lb = __fsub_rn(__fadd_rn(g.a_min, bnd[smf - 1]), g.e_cur);
-        if (lb < bestW) {
-          T = c.L > 0 ? fs_tstar(__fadd_rn(g.t_avail_ms, c.load_ms), c.slo_ttft) : FS_INF;
-          if (!(bnd[DENSE_S + smf - 1] <= T)) T = -1.0f;       // no share meets the TTFT deadline
+        if (lb <= bestW && lb < FS_INF) {
+          const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
+          if (c.L == 0) T = FS_INF;
+          else if (__fadd_rn(wait, bnd[DENSE_S + smf - 1]) <= c.slo_ttft) T = fs_tstar(wait, c.slo_ttft);
         }
-        if (T >= 0.0f) { nswept += 1; ncswept += (unsigned long long)smf * d.F; }
       }
-      // compact the eligible GPUs of the chunk, in ascending order, into the warp's list:
-      // {T*, Ecur, sm_free, byte offset of the GPU's A0 row}
-      const bool go = el && T >= 0.0f;
+      // compact the surviving GPUs of the chunk into the warp's list: {T*, Ecur, sm_free, GPU}
+      const bool go = T >= 0.0f;
       const unsigned mask = __ballot_sync(0xffffffffu, go);
+      if (mask == 0u) continue;
       __syncwarp();
       if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
-          make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float(ci * FS_CHUNK + lane));
+          make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((int)g.k));
       __syncwarp();
       const int n_el = __popc(mask);
-      // ---- sweep the eligible GPUs of the chunk -------------------------------------------------
+      // ---- sweep the survivors: per candidate one compare and one predicated min ---------------
       for (int e = 0; e < n_el; ++e) {
         const float4 w = wb[e];
-        const float Tst = w.x; const int sfree = __float_as_int(w.z);
-        float m[NPHI][2];                               // two min chains per frequency (ILP)
+        const float Tst = w.x; const int sfree = __float_as_int(w.z); const int k = __float_as_int(w.w);
+        if (STATS) { n_swept += 1; n_cswept += (uint32_t)(sfree * d.F); }
+        float arow[NPHI], m[NPHI];
+        ld_cols<NPHI>(v.gA0 + (size_t)k * FT, 0, phi0, FT, true, arow);   // rows are FT-padded: aligned
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) m[i][0] = m[i][1] = FS_INF;
-#define FS_DENSE_STEP(s)                                                              \
-  _Pragma("unroll") for (int i = 0; i < NPHI; ++i)                                    \
-    asm("{.reg .pred p; setp.le.f32 p, %1, %2; @p min.f32 %0, %0, %3;}"               \
-        : "+f"(m[i][(s) & 1]) : "f"(t0[s][i]), "f"(Tst), "f"(er[s][i]));
-        switch (sfree) {
-          default:
-          case 16: FS_DENSE_STEP(15) case 15: FS_DENSE_STEP(14) case 14: FS_DENSE_STEP(13)
-          case 13: FS_DENSE_STEP(12) case 12: FS_DENSE_STEP(11) case 11: FS_DENSE_STEP(10)
-          case 10: FS_DENSE_STEP(9)  case 9: FS_DENSE_STEP(8)   case 8: FS_DENSE_STEP(7)
-          case 7: FS_DENSE_STEP(6)   case 6: FS_DENSE_STEP(5)   case 5: FS_DENSE_STEP(4)
-          case 4: FS_DENSE_STEP(3)   case 3: FS_DENSE_STEP(2)   case 2: FS_DENSE_STEP(1)
-          case 1: FS_DENSE_STEP(0)
+        for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
+#pragma unroll 4
+        for (int s = 0; s < sfree; ++s) {
+          float tt[NPHI], ee[NPHI];
+          ld_tile<NPHI>(tl_t0 + s * FT + phi0, tt); ld_tile<NPHI>(tl_er + s * FT + phi0, ee);
+#pragma unroll
+          for (int i = 0; i < NPHI; ++i) m[i] = tt[i] <= Tst ? fminf(m[i], ee[i]) : m[i];
         }
-#undef FS_DENSE_STEP
-        const int kloc = __float_as_int(w.w);
-        float arow[NPHI];
-        ld_cols<NPHI>(gA0 + (size_t)kloc * FT, 0, phi0, FT, true, arow);   // rows are FT-padded: aligned
         float x = FS_INF;
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], fminf(m[i][0], m[i][1])));
+        for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
         const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
-        if (dE < best) { best = dE; bestk = kloc; }
+        if (dE < best || (dE == best && k < bestk)) { best = dE; bestk = k; }
       }
     }
-    int bestkg = bestk >= 0 ? c0 * FS_CHUNK + bestk : 0x7FFFFFFF;    // global GPU index of the lane's best
-    // ---- warm pairs: GPUs that already host model m (decode bucket, variant and wait depend on
-    // the GPU).  Lane <-> item: bound  dE >= fl(fl(a_min + fl(e0min + e1min)) - Ecur)  with
-    // e1min = fl(fl(rounds1*l1_min)*p1_min); items that survive are scored candidate by candidate
-    // from the planes.  They come after GPUs with a higher index, so ties compare (dE, k) in full
-    // and the prune is strict.
-    for (int ib = warm_off[c.m]; ib < warm_off[c.m + 1]; ib += 32) {
-      uint32_t ordl = 0xFFFFFFFFu; int wk = 0, wsmf = 0;      // orderable bound of the lane's item
-      if (ib + lane < warm_off[c.m + 1]) {
-        const FsWarmItem it = witems[ib + lane];
-        const int kc = it.k / FS_CHUNK;
-        if (kc >= c0 && kc < c1 && it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
-          wpairs += 1; wcand += (unsigned long long)it.sm_free * d.F;
-          const float fr1 = __uint2float_rn(fs_ceil_div(c.O, (uint32_t)it.br1 + 1u));
-          const float e1lb = __fmul_rn(__fmul_rn(fr1, it.l1_min), it.p1_min);
-          const float lb = __fsub_rn(__fadd_rn(it.a_min, __fadd_rn(bnd[2 * DENSE_S + it.sm_free - 1], e1lb)), it.e_cur);
-          if (c.O == 0 || it.l1_min <= c.slo_tbt) {
-            const float T = c.L > 0 ? fs_tstar(it.t_avail_ms, c.slo_ttft) : FS_INF;
-            if (T >= 0.0f && bnd[DENSE_S + it.sm_free - 1] <= T) ordl = fs_orderable(lb);
-          }
-          wk = it.k; wsmf = it.sm_free;
-        }
-      }
-      // best-first: score the item with the lowest bound, tighten the incumbent, drop every item
-      // whose bound is now strictly above it (NaN bounds order above +INF and drop out too)
-      for (;;) {
+    // ---- (c), (d) the definition, pair by pair, from the t0 tile and the planes: first the WARM
+    // pairs (GPUs that already host model m), best bound first, then once more on the winning GPU
+    // to recover the lowest flat index attaining the minimum.  One code site serves both.
+    //   warm bound:  dE >= fl(fl(a_min + fl(e0min + e1min)) - Ecur),  e1min = fl(fl(rounds1*l1_min)*p1_min)
+    int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
+    uint32_t ordl = NONE32; int wk = 0;
+    bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32;
+    for (;;) {
+      int k = KNONE;
+      while (!recover) {
         const uint32_t mn = warp_min_u32(ordl);
         const uint32_t inc = warp_min_u32(fs_orderable(best));
-        if (mn == 0xFFFFFFFFu || mn > inc) break;
-        const int src = __ffs(__ballot_sync(0xffffffffu, ordl == mn)) - 1;
-        if (lane == src) { ordl = 0xFFFFFFFFu; wswept += 1; wcswept += (unsigned long long)wsmf * d.F; }
-        const int k = __shfl_sync(0xffffffffu, wk, src);
-        const PairCtx p = make_pair(v, c, v.ginfo[k]);
-        if (!p.ok) continue;
-        for (int sg = 0; sg < p.smf; ++sg)
-#pragma unroll
-          for (int i = 0; i < NPHI; ++i) {
-            const int phi = phi0 + i;
-            if (phi < d.F) {
-              const Cand cd = eval_cand(v, c, p, k, sg, phi);
-              float dE = cd.dE; if (dE == 0.0f) dE = 0.0f;
-              if (cd.ok && (dE < best || (dE == best && k < bestkg))) { best = dE; bestkg = k; }
-            }
-          }
-      }
-    }
-    // ---- recovery: lowest flat index among the lane's candidates that attain its minimum, by the
-    // definition (eval_cand), at its best GPU ----------------------------------------------------
-    unsigned long long key = FS_KEY_NONE;
-    if (bestkg != 0x7FFFFFFF) {
-      const PairCtx p = make_pair(v, c, v.ginfo[bestkg]);
-      uint32_t flat = 0xFFFFFFFFu;
-      for (int sg = 0; sg < p.smf && flat == 0xFFFFFFFFu; ++sg)
-#pragma unroll
-        for (int i = 0; i < NPHI; ++i) {
-          const int phi = phi0 + i;
-          if (phi < d.F && flat == 0xFFFFFFFFu) {
-            const Cand cd = eval_cand(v, c, p, bestkg, sg, phi);
-            if (cd.ok && cd.dE == best) flat = (uint32_t)((bestkg * d.S + sg) * d.F + phi);
+        if (mn != NONE32 && mn <= inc) {               // best-first: the item with the lowest bound
+          const int src = __ffs(__ballot_sync(0xffffffffu, ordl == mn)) - 1;
+          k = __shfl_sync(0xffffffffu, wk, src);
+          if (lane == src) ordl = NONE32;
+          break;
+        }
+        if (ib >= ie) {                                 // no item left that could beat the incumbent
+          const unsigned long long kk = fs_warp_min_key(((unsigned long long)fs_orderable(best) << 32) | (uint32_t)bestk);
+          recover = true; k = (int)(uint32_t)kk; bestW = fs_unorderable((uint32_t)(kk >> 32));
+          break;
+        }
+        ordl = NONE32;                                  // next 32 items: lane <-> item
+        const int ix = ib + lane;
+        if (ix < ie && ix % nslice == slice) {
+          const FsWarmItem it = witems[ix];
+          if (it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
+            if (STATS) { n_witems += 1; }
+            const float fr1 = __uint2float_rn(fs_ceil_div(c.O, (uint32_t)it.br1 + 1u));
+            const float e1lb = __fmul_rn(__fmul_rn(fr1, it.l1_min), it.p1_min);
+            const float lb = __fsub_rn(__fadd_rn(it.a_min, __fadd_rn(bnd[2 * DENSE_S + it.sm_free - 1], e1lb)), it.e_cur);
+            const bool tbt_ok = c.O == 0 || it.l1_min <= c.slo_tbt;
+            const bool ttft_ok = c.L == 0 || __fadd_rn(it.t_avail_ms, bnd[DENSE_S + it.sm_free - 1]) <= c.slo_ttft;
+            if (tbt_ok && ttft_ok && lb < FS_INF) ordl = fs_orderable(lb);
+            wk = it.k;
           }
         }
-      if (flat != 0xFFFFFFFFu) key = fs_make_key(best, flat);
+        ib += 32;
+      }
+      if (k == KNONE) break;                            // no feasible candidate at all
+      const PairCtx p = make_pair(v, c, v.ginfo[k]);
+      if (p.ok) {
+        if (STATS) { n_scored += 1; n_cscored += (uint32_t)(p.smf * d.F); }
+        const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
+        const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F;
+        const float fr1 = __uint2float_rn(p.rounds1);
+        float ar[NPHI];
+#pragma unroll
+        for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < d.F ? Ar[phi0 + i] : FS_INF;
+#pragma unroll 1
+        for (int s = 0; s < p.smf; ++s) {
+          float tt[NPHI], b0[NPHI], a1[NPHI], b1[NPHI];
+          ld_tile<NPHI>(tl_t0 + s * FT + phi0, tt);
+          ld_cols<NPHI>(pw0, s * d.F, phi0, d.F, vec, b0);
+          ld_cols<NPHI>(l1, s * d.F, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, s * d.F, phi0, d.F, vec, b1);
+#pragma unroll
+          for (int i = 0; i < NPHI; ++i) {
+            const float e0 = __fmul_rn(tt[i], b0[i]);
+            const float e1 = __fmul_rn(__fmul_rn(fr1, a1[i]), b1[i]);
+            float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);
+            if (dE == 0.0f) dE = 0.0f;
+            const bool ok = (c.L == 0 || __fadd_rn(p.wait, tt[i]) <= c.slo_ttft) &&
+                            (c.O == 0 || a1[i] <= c.slo_tbt) && dE < FS_INF;
+            if (recover) {
+              if (ok && dE == bestW && flat == NONE32) flat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
+            } else if (ok && (dE < best || (dE == best && k < bestk))) { best = dE; bestk = k; }
+          }
+          if (recover && __any_sync(0xffffffffu, flat != NONE32)) break;   // flat order is sigma-major
+        }
+      }
+      if (recover) break;
     }
+    unsigned long long key = flat != NONE32 ? fs_make_key(bestW, flat) : FS_KEY_NONE;
     key = fs_warp_min_key(key);
     if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
+    if (STATS) { n_req += 1; }
+    if (STATS && __any_sync(0xffffffffu, ((n_chunks | n_elig | n_swept | n_cswept | n_witems | n_scored | n_cscored | n_req) >> 30) != 0u)) {
+      flush_stats(stats, n_chunks, n_elig, n_swept, n_cswept, n_witems, n_scored, n_cscored, n_req);
+      n_chunks = n_elig = n_swept = n_cswept = n_witems = n_scored = n_cscored = n_req = 0;
+    }
   }
-  // work statistics (eligible pairs and their candidates, by the oracle's definition)
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
-    ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
-    nswept += __shfl_xor_sync(0xffffffffu, nswept, o);
-    ncswept += __shfl_xor_sync(0xffffffffu, ncswept, o);
-    wpairs += __shfl_xor_sync(0xffffffffu, wpairs, o);
-    wcand += __shfl_xor_sync(0xffffffffu, wcand, o);
-    wswept += __shfl_xor_sync(0xffffffffu, wswept, o);
-    wcswept += __shfl_xor_sync(0xffffffffu, wcswept, o);
-  }
-  if (lane == 0 && stats && (npairs | wpairs)) {
-    atomicAdd(&stats[0], npairs); atomicAdd(&stats[1], ncand);
-    atomicAdd(&stats[2], wpairs); atomicAdd(&stats[3], wcand);
-    atomicAdd(&stats[4], nswept); atomicAdd(&stats[5], ncswept);
-    atomicAdd(&stats[6], wswept); atomicAdd(&stats[7], wcswept);
-  }
+  if (STATS) flush_stats(stats, n_chunks, n_elig, n_swept, n_cswept, n_witems, n_scored, n_cscored, n_req);
 }
 
 // ---- decode: key -> fs_placement (one warp per request, lanes over phi for f_req) ----------
@@ -489,8 +521,10 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
 }  // namespace
 
 int fsk_place_smem_attr() {
-  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   return e;
 }
 
@@ -499,7 +533,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   if (R <= 0) return 0;
   int launches = 0;
   cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-  cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 8, st);
+  if (sc.count_work) cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 8, st);
   if (v.K <= 0) {
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
@@ -507,25 +541,30 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= 64 && !sc.force_generic;
   fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
   if (dense_ok) {
-    // one persistent block per SM; each holds a slice of the GPUs in shared memory.  The number
-    // of slices is what the slice size forces, raised when R alone cannot occupy every SM.
+    // one persistent block per SM; each holds a slice of the sorted GPU records in shared memory
+    // beside its warps' tiles.  Warps per block: as many as fit (registers cap them at DENSE_MAXW),
+    // fewer when R alone cannot occupy every SM; the number of slices is what the slice size
+    // forces, raised when the request batches alone cannot occupy every SM.
     const int FT = v.d.F <= 32 ? 32 : 64;
     const int nchunk = v.Kpad / FS_CHUNK;
-    const size_t fixed = dense_smem_bytes(0), per_chunk = dense_smem_bytes(FS_CHUNK) - fixed;
-    const int max_cps = (int)((DENSE_SMEM_MAX - fixed) / per_chunk);
+    const size_t pw = dense_warp_bytes(v.d.S, FT), per_chunk = (size_t)FS_CHUNK * sizeof(FsGpuRec);
+    int W = (int)((DENSE_SMEM_MAX - 16 - (size_t)min(nchunk, 64) * per_chunk) / pw);
+    W = max(1, min(min(DENSE_MAXW, W), (R + sc.sm_count - 1) / sc.sm_count));
+    const int max_cps = (int)((DENSE_SMEM_MAX - 16 - (size_t)W * pw) / per_chunk);
     int nslice = (nchunk + max_cps - 1) / max_cps;
-    const int nbatch = (R + DENSE_WARPS - 1) / DENSE_WARPS;
+    const int nbatch = (R + W - 1) / W;
     if (nbatch * nslice < sc.sm_count) nslice = min(nchunk, (sc.sm_count + nbatch - 1) / nbatch);
     const int cps = (nchunk + nslice - 1) / nslice;
     nslice = (nchunk + cps - 1) / cps;
     const int streams = max(1, min(nbatch, sc.sm_count / nslice));
     const int grid = streams * nslice;
-    const size_t smem = dense_smem_bytes(cps * FS_CHUNK);
+    const size_t smem = dense_smem_bytes(cps * FS_CHUNK, W, v.d.S, FT);
     cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nslice, st);
-    if (FT == 32)
-      place_dense_kernel<1><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats);
-    else
-      place_dense_kernel<2><<<grid, DENSE_WARPS * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats);
+#define FS_LAUNCH_DENSE(NP, ST) \
+  place_dense_kernel<NP, ST><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats)
+    if (FT == 32) { if (sc.count_work) FS_LAUNCH_DENSE(1, true); else FS_LAUNCH_DENSE(1, false); }
+    else          { if (sc.count_work) FS_LAUNCH_DENSE(2, true); else FS_LAUNCH_DENSE(2, false); }
+#undef FS_LAUNCH_DENSE
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   } else {
@@ -538,7 +577,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     nsplit = (v.K + kchunk - 1) / kchunk;
     const long long warps = (long long)R * nsplit;
     place_generic_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(v, R, reqs, sc.keys, nsplit,
-                                                                     kchunk, sc.stats);
+                                                                     kchunk, sc.count_work ? sc.stats : nullptr);
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
   }

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     if (lane == 0) {
       FsGpuRec r; r.t_avail_ms = r.mem_free_mb = r.e_cur = 0.f; r.meta = 0;
       for (int i = 0; i < FS_RMAX; ++i) r.model[i] = -1;
-      r.a_min = FS_INF; r._pad = 0;
+      r.a_min = FS_INF; r.k = 0;
       grec[k] = r;
     }
     return;
@@ -112,9 +112,99 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     FsGpuRec r; r.t_avail_ms = gi.t_avail_ms; r.mem_free_mb = gi.mem_free_mb; r.e_cur = ecur;
     r.meta = (uint32_t)n | ((uint32_t)gi.sm_free << 8);
     for (int i = 0; i < FS_RMAX; ++i) r.model[i] = gi.model[i];
-    r.a_min = a_min; r._pad = 0;
+    r.a_min = a_min; r.k = (uint32_t)k;
     grec[k] = r;
     if (!valid) fs_raise(v.flag, FS_FLAG_STATE);
+  }
+}
+
+
+// ---- scan order of the dense placement kernel --------------------------------------------------
+// GPUs that can take a COLD request at all (1 <= n_res < RMAX, sm_free >= 1, co-residents feasible
+// at some phi) in ascending order of d_k = a_min_k - Ecur_k, the request-independent part of the
+// pruning bound fl(fl(a_min + b) - Ecur); everything else follows as sentinels no request is
+// eligible for.  Placement results do not depend on this order (ties compare (dE, k) in full): it
+// only decides how soon a request meets its best GPUs and can stop scanning (fs_place.cu).
+__device__ __forceinline__ bool cold_capable(const FsGpuRec& r) {
+  const int n = r.meta & 0xFF, smf = (r.meta >> 8) & 0xFF;
+  return n >= 1 && n < FS_RMAX && smf >= 1 && r.a_min < FS_INF;
+}
+__device__ __forceinline__ float order_key(const FsGpuRec& r) {
+  float d = cold_capable(r) ? __fsub_rn(r.a_min, r.e_cur) : FS_INF;
+  return d == d ? d : FS_INF;
+}
+// rank of every record by (key, index): thread <-> record, keys walked through shared memory
+__global__ void __launch_bounds__(128) order_rank_kernel(const FsGpuRec* __restrict__ grec, int Kpad,
+                                                        FsGpuRec* __restrict__ gsort,
+                                                        double* __restrict__ dsort) {
+  __shared__ float tile[1024];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  FsGpuRec mine; float key = FS_INF;
+  if (i < Kpad) { mine = grec[i]; key = order_key(mine); }
+  int rank = 0;
+  for (int base = 0; base < Kpad; base += 1024) {
+    __syncthreads();
+    for (int x = threadIdx.x; x < 1024; x += blockDim.x)
+      tile[x] = base + x < Kpad ? order_key(grec[base + x]) : FS_INF;
+    __syncthreads();
+    const int n = min(1024, Kpad - base);
+    for (int x = 0; x < n; ++x) {
+      const float kj = tile[x];
+      rank += (kj < key || (kj == key && base + x < i)) ? 1 : 0;
+    }
+  }
+  if (i >= Kpad) return;
+  const bool cap = cold_capable(mine);
+  double dd = (double)FS_INF;
+  if (cap) { dd = (double)mine.a_min - (double)mine.e_cur; mine.k = (uint32_t)i; }
+  else {     // sentinel: mem_free = -INF fails every memory test
+    mine.t_avail_ms = 0.f; mine.mem_free_mb = -FS_INF; mine.e_cur = 0.f; mine.meta = 1u | (1u << 8);
+    for (int j = 0; j < FS_RMAX; ++j) mine.model[j] = -1;
+    mine.a_min = FS_INF; mine.k = 0u;
+  }
+  gsort[rank] = mine; dsort[rank] = dd;
+}
+// dsuf[0] = max over the capable GPUs of max(a_min, |Ecur|) (INF if any is huge: no early stop);
+// dsuf[1+c] = min of d over sorted positions >= 32*c   (exact suffix minimum, in double)
+__global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __restrict__ gsort,
+                                                           const double* __restrict__ dsort, int nchunk,
+                                                           double* __restrict__ dsuf) {
+  __shared__ double seg[1024];
+  __shared__ float smax[32];
+  const int t = threadIdx.x;
+  float amax = 0.0f;
+  for (int c = t; c < nchunk; c += 1024) {
+    double m = (double)FS_INF;
+    for (int x = 0; x < FS_CHUNK; ++x) {
+      const int pos = c * FS_CHUNK + x;
+      const double dv = dsort[pos];
+      m = dv < m ? dv : m;
+      if (dv < (double)FS_INF) amax = fmaxf(amax, fmaxf(gsort[pos].a_min, fabsf(gsort[pos].e_cur)));
+    }
+    dsuf[1 + c] = m;
+  }
+  __syncthreads();
+  const int per = (nchunk + 1023) / 1024;
+  const int lo = min(nchunk, t * per), hi = min(nchunk, lo + per);
+  double m = (double)FS_INF;
+  for (int c = lo; c < hi; ++c) { const double dv = dsuf[1 + c]; m = dv < m ? dv : m; }
+  seg[t] = m;
+  __syncthreads();
+  double carry = (double)FS_INF;                       // min over the segments after mine
+  for (int u = t + 1; u < 1024; ++u) { const double dv = seg[u]; carry = dv < carry ? dv : carry; }
+  for (int c = hi - 1; c >= lo; --c) {
+    const double dv = dsuf[1 + c];
+    carry = dv < carry ? dv : carry;
+    dsuf[1 + c] = carry;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+  if ((t & 31) == 0) smax[t >> 5] = amax;
+  __syncthreads();
+  if (t == 0) {
+    for (int w = 1; w < 32; ++w) amax = fmaxf(amax, smax[w]);
+    dsuf[0] = amax <= 1e37f ? (double)amax : (double)FS_INF;
+    dsuf[1 + nchunk] = (double)FS_INF;
   }
 }
 
@@ -169,13 +259,15 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
 }  // namespace
 
 int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
-                cudaStream_t st, FsTimers* tm) {
+                FsGpuRec* gsort, double* dsort, double* dsuf, cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int wpb = 4;
   fs_tm_beg(tm, FS_T_SUMMARY, st);
   summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0);
+  order_rank_kernel<<<(v.Kpad + 127) / 128, 128, 0, st>>>(grec, v.Kpad, gsort, dsort);
+  order_suffix_kernel<<<1, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf);
   fs_tm_end(tm, FS_T_SUMMARY, st);
-  return 1;
+  return 3;
 }
 
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
