@@ -133,30 +133,43 @@ __device__ __forceinline__ float order_key(const FsGpuRec& r) {
   float d = cold_capable(r) ? __fsub_rn(r.a_min, r.e_cur) : FS_INF;
   return d == d ? d : FS_INF;
 }
+// keys once, so that the ranking pass streams plain floats
+__global__ void order_key_kernel(const FsGpuRec* __restrict__ grec, int Kpad, float* __restrict__ okey) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < Kpad) okey[i] = order_key(grec[i]);
+}
 // rank of every record by (key, index): thread <-> record, keys walked through shared memory
-__global__ void __launch_bounds__(128) order_rank_kernel(const FsGpuRec* __restrict__ grec, int Kpad,
+__global__ void __launch_bounds__(128) order_rank_kernel(const FsGpuRec* __restrict__ grec,
+                                                        const float* __restrict__ okey, int Kpad,
                                                         FsGpuRec* __restrict__ gsort,
                                                         double* __restrict__ dsort) {
-  __shared__ float tile[1024];
+  __shared__ __align__(16) float tile[1024];
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  FsGpuRec mine; float key = FS_INF;
-  if (i < Kpad) { mine = grec[i]; key = order_key(mine); }
+  const float key = i < Kpad ? okey[i] : FS_INF;
   int rank = 0;
   for (int base = 0; base < Kpad; base += 1024) {
     __syncthreads();
-    for (int x = threadIdx.x; x < 1024; x += blockDim.x)
-      tile[x] = base + x < Kpad ? order_key(grec[base + x]) : FS_INF;
+    for (int x = threadIdx.x; x < 1024; x += blockDim.x) tile[x] = base + x < Kpad ? okey[base + x] : FS_INF;
     __syncthreads();
-    const int n = min(1024, Kpad - base);
-    for (int x = 0; x < n; ++x) {
-      const float kj = tile[x];
-      rank += (kj < key || (kj == key && base + x < i)) ? 1 : 0;
+    // j < i decides ties: entries before i count on <=, entries after on <
+    const int n = min(1024, Kpad - base), nle = max(0, min(n, i - base));
+    int x = 0;
+    for (; x + 4 <= nle; x += 4) {
+      const float4 t = *reinterpret_cast<const float4*>(tile + x);
+      rank += (t.x <= key) + (t.y <= key) + (t.z <= key) + (t.w <= key);
     }
+    for (; x < nle; ++x) rank += tile[x] <= key;
+    for (; x < n && (x & 3); ++x) rank += tile[x] < key;
+    for (; x + 4 <= n; x += 4) {
+      const float4 t = *reinterpret_cast<const float4*>(tile + x);
+      rank += (t.x < key) + (t.y < key) + (t.z < key) + (t.w < key);
+    }
+    for (; x < n; ++x) rank += tile[x] < key;
   }
   if (i >= Kpad) return;
-  const bool cap = cold_capable(mine);
+  FsGpuRec mine = grec[i];
   double dd = (double)FS_INF;
-  if (cap) { dd = (double)mine.a_min - (double)mine.e_cur; mine.k = (uint32_t)i; }
+  if (cold_capable(mine)) { dd = (double)mine.a_min - (double)mine.e_cur; mine.k = (uint32_t)i; }
   else {     // sentinel: mem_free = -INF fails every memory test
     mine.t_avail_ms = 0.f; mine.mem_free_mb = -FS_INF; mine.e_cur = 0.f; mine.meta = 1u | (1u << 8);
     for (int j = 0; j < FS_RMAX; ++j) mine.model[j] = -1;
@@ -171,17 +184,15 @@ __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __re
                                                            double* __restrict__ dsuf) {
   __shared__ double seg[1024];
   __shared__ float smax[32];
-  const int t = threadIdx.x;
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
   float amax = 0.0f;
-  for (int c = t; c < nchunk; c += 1024) {
-    double m = (double)FS_INF;
-    for (int x = 0; x < FS_CHUNK; ++x) {
-      const int pos = c * FS_CHUNK + x;
-      const double dv = dsort[pos];
-      m = dv < m ? dv : m;
-      if (dv < (double)FS_INF) amax = fmaxf(amax, fmaxf(gsort[pos].a_min, fabsf(gsort[pos].e_cur)));
-    }
-    dsuf[1 + c] = m;
+  for (int c = warp; c < nchunk; c += 32) {            // warp <-> chunk, lane <-> record
+    const int pos = c * FS_CHUNK + lane;
+    double m = dsort[pos];
+    if (m < (double)FS_INF) amax = fmaxf(amax, fmaxf(gsort[pos].a_min, fabsf(gsort[pos].e_cur)));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { const double u = __shfl_xor_sync(0xffffffffu, m, o); m = u < m ? u : m; }
+    if (lane == 0) dsuf[1 + c] = m;
   }
   __syncthreads();
   const int per = (nchunk + 1023) / 1024;
@@ -191,7 +202,7 @@ __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __re
   seg[t] = m;
   __syncthreads();
   double carry = (double)FS_INF;                       // min over the segments after mine
-  for (int u = t + 1; u < 1024; ++u) { const double dv = seg[u]; carry = dv < carry ? dv : carry; }
+  if (lo < hi) for (int u = t + 1; u < 1024; ++u) { const double dv = seg[u]; carry = dv < carry ? dv : carry; }
   for (int c = hi - 1; c >= lo; --c) {
     const double dv = dsuf[1 + c];
     carry = dv < carry ? dv : carry;
@@ -199,7 +210,7 @@ __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __re
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-  if ((t & 31) == 0) smax[t >> 5] = amax;
+  if (lane == 0) smax[warp] = amax;
   __syncthreads();
   if (t == 0) {
     for (int w = 1; w < 32; ++w) amax = fmaxf(amax, smax[w]);
@@ -264,10 +275,12 @@ int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, fl
   const int wpb = 4;
   fs_tm_beg(tm, FS_T_SUMMARY, st);
   summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0);
-  order_rank_kernel<<<(v.Kpad + 127) / 128, 128, 0, st>>>(grec, v.Kpad, gsort, dsort);
+  float* okey = reinterpret_cast<float*>(dsuf + v.Kpad / FS_CHUNK + 2);   // scratch behind dsuf
+  order_key_kernel<<<(v.Kpad + 255) / 256, 256, 0, st>>>(grec, v.Kpad, okey);
+  order_rank_kernel<<<(v.Kpad + 127) / 128, 128, 0, st>>>(grec, okey, v.Kpad, gsort, dsort);
   order_suffix_kernel<<<1, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf);
   fs_tm_end(tm, FS_T_SUMMARY, st);
-  return 3;
+  return 4;
 }
 
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
