@@ -23,6 +23,8 @@ _LOCAL_DT = np.dtype(
      ("_pad", "<u4", (4,))])
 _CONSOL_DT = np.dtype([("dst", "<i4"), ("phi", "<i4"), ("score_mj", "<f4"), ("saving_mj", "<f4")])
 
+_TASK_OUT_DT = np.dtype([("score", "<f4"), ("latency_ms", "<f4"), ("rank", "<i4"), ("admitted", "<i4")])
+
 OBJ_ENERGY, OBJ_POWER, SPLIT_EXHAUSTIVE, SPLIT_MINSM = 0, 1, 0, 2
 
 _lib = None
@@ -77,6 +79,21 @@ def consolidate(lat, pow_, models, states, p_idle_w, horizon_ms, mem_cap_mb, del
     lib().fo_consolidate(*_tables(lat, pow_), _p(models), C.c_int(len(states)), _p(states),
                          C.c_float(p_idle_w), C.c_float(horizon_ms), C.c_float(mem_cap_mb),
                          C.c_int(delta_pct), _p(out), C.c_int(nthreads))
+    return out
+
+
+def batch_tasks(lat, pow_, states, off, tasks, gpu_ids=None, nthreads: int = 1) -> np.ndarray:
+    """Local scheduler steps 1-2 by definition (Eq. 4, Fig. 8)."""
+    off = np.ascontiguousarray(off, dtype=np.int32)
+    n = len(off) - 1
+    ids = C.c_void_p(0)
+    if gpu_ids is not None:
+        gpu_ids = np.ascontiguousarray(gpu_ids, dtype=np.int32)
+        assert len(gpu_ids) == n
+        ids = _p(gpu_ids)
+    out = np.zeros(len(tasks), dtype=_TASK_OUT_DT)
+    lib().fo_batch_tasks(*_tables(lat, pow_), _p(states), C.c_int(n), ids, _p(off),
+                         _p(np.ascontiguousarray(tasks)), _p(out), C.c_int(nthreads))
     return out
 
 

@@ -16,6 +16,8 @@
 //   local config .......... Fig. 8 step 3 worked table, brute force
 //   consolidation ......... brute force, C*_ab symmetry, empty-destination case,
 //                           App. G arithmetic
+//   priority batching ..... Fig. 8 steps 1-2 worked table, independent numpy
+//                           restatement, budget / bypass invariants
 // Nothing here is "parity unpinned".
 //
 // Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC (see oracle/build.py).
@@ -345,6 +347,44 @@ template <class Fn> void par_for(int n, int nthreads, Fn fn) {
   for (auto& x : th) x.join();
 }
 
+// ---- local scheduler steps 1-2: unified priority score and priority-based task batching ------
+// Score_task = Latency(task) / (Slack_task - beta*Age_task), beta = 0 for decode, 1 for prefill
+// (Eq. 4); Latency(task) = the LUT entry of the scheduling unit at the GPU's current
+// frequency.  A task whose effective slack is used up (<= 0) is the most urgent: score +INF
+// (reading s26).  Batching (Fig. 8 steps 1-2): walk the tasks in descending score
+// (ties: lowest task index), admit a task iff its memory and SM share still fit, otherwise
+// bypass it and go on.  Budgets: all S share units, the GPU's free memory.
+struct Task { int16_t model; uint8_t phase, sigma, beta, p0[3]; float slack_ms, age_ms, mem_mb; uint32_t tag; };
+struct TaskOut { float score, latency_ms; int32_t rank, admitted; };
+static_assert(sizeof(Task) == 24 && sizeof(TaskOut) == 16, "layout");
+
+void batch_one(const Tables& T, const GpuState& g, const Task* tk, int n, TaskOut* out) {
+  std::vector<int> order(n);
+  for (int i = 0; i < n; ++i) {
+    const Task& t = tk[i];
+    float lat = T.LAT(t.model, t.phase, g.f_cur, t.sigma, t.beta);
+    float denom = (t.phase == 0) ? (t.slack_ms - t.age_ms) : t.slack_ms;
+    out[i].latency_ms = lat;
+    out[i].score = (denom > 0.0f) ? (lat / denom) : INF;
+    order[i] = i;
+  }
+  // insertion sort: descending score, stable (lowest index first among equals)
+  for (int a = 1; a < n; ++a) {
+    int x = order[a], b = a - 1;
+    while (b >= 0 && out[order[b]].score < out[x].score) { order[b + 1] = order[b]; --b; }
+    order[b + 1] = x;
+  }
+  int sm_left = T.S; float mem_left = g.mem_free_mb;
+  for (int pos = 0; pos < n; ++pos) {
+    const int i = order[pos]; const Task& t = tk[i];
+    out[i].rank = pos;
+    const int need = (int)t.sigma + 1;
+    if (need <= sm_left && t.mem_mb <= mem_left) {
+      out[i].admitted = 1; sm_left -= need; mem_left = mem_left - t.mem_mb;
+    } else out[i].admitted = 0;
+  }
+}
+
 }  // namespace
 
 extern "C" {
@@ -408,6 +448,18 @@ int fo_tenant_fmin(int M, int F, int S, int B, const float* lat, const float* po
   for (int phi = 0; phi < F; ++phi)
     if (tenant_eval(T, g.t[i], phi, g.t[i].sigma, false).ok) return phi;
   return -1;
+}
+
+// Steps 1-2 of the local scheduler for n GPUs; tasks of GPU i are tasks[off[i] .. off[i+1]).
+int fo_batch_tasks(int M, int F, int S, int B, const float* lat, const float* pow,
+                   const void* states, int n, const int32_t* gpu_ids, const int32_t* off,
+                   const void* tasks, void* out, int nthreads) {
+  Tables T{M, F, S, B, lat, pow};
+  const GpuState* gs = (const GpuState*)states; const Task* tk = (const Task*)tasks; TaskOut* o = (TaskOut*)out;
+  par_for(n, nthreads, [&](int i) {
+    batch_one(T, gs[gpu_ids ? gpu_ids[i] : i], tk + off[i], off[i + 1] - off[i], o + off[i]);
+  });
+  return 0;
 }
 
 }  // extern "C"

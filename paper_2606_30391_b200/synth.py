@@ -36,6 +36,10 @@ LOCAL_CFG_DT = np.dtype(
      ("cost", "<f4"), ("energy_mj", "<f4"), ("power_w", "<f4"), ("flat", "<u4"),
      ("_pad", "<u4", (4,))])
 CONSOL_DT = np.dtype([("dst", "<i4"), ("phi", "<i4"), ("score_mj", "<f4"), ("saving_mj", "<f4")])
+TASK_DT = np.dtype([("model", "<i2"), ("phase", "u1"), ("sigma", "u1"), ("beta", "u1"), ("_p0", "u1", (3,)),
+                    ("slack_ms", "<f4"), ("age_ms", "<f4"), ("mem_mb", "<f4"), ("tag", "<u4")])
+TASK_OUT_DT = np.dtype([("score", "<f4"), ("latency_ms", "<f4"), ("rank", "<i4"), ("admitted", "<i4")])
+assert TASK_DT.itemsize == 24 and TASK_OUT_DT.itemsize == 16
 
 assert TENANT_DT.itemsize == 28 and GPU_STATE_DT.itemsize == 128 and REQUEST_DT.itemsize == 32
 assert MODEL_INFO_DT.itemsize == 16 and PLACEMENT_DT.itemsize == 32
@@ -299,6 +303,31 @@ def make_requests(seed: int, R: int, M: int) -> np.ndarray:
     req["slo_tbt_ms"] = st.urange(R, 50.0, 150.0).astype(np.float32)
     req["tag"] = np.arange(R, dtype=np.uint32)
     return req
+
+
+def make_tasks(seed: int, K: int, M: int, S: int, B: int, lo: int, hi: int):
+    """Runnable tasks per GPU for the local scheduler's steps 1-2 (Eq. 4, Fig. 8): `lo..hi`
+    tasks per GPU (the paper's Table 3 measures 10-100 queued tasks), ~60 % decode steps with TBT
+    slack U[5,150] ms and ~40 % prefill units with TTFT slack U[50,2000] ms and age U[0,1.2*slack)
+    (so some prefills have used up their slack), SM demand 1..S/2 units, KV memory lognormal.
+    Returns (off [K+1] int32, tasks [off[K]] TASK_DT)."""
+    st = Stream(seed, "tasks")
+    n = st.randint(K, lo, hi).astype(np.int64)
+    off = np.zeros(K + 1, dtype=np.int32)
+    off[1:] = np.cumsum(n)
+    T = int(off[-1])
+    t = np.zeros(T, dtype=TASK_DT)
+    t["model"] = st.randint(T, 0, M - 1)
+    ph = (st.uniform(T) < 0.6).astype(np.uint8)          # 1 = decode
+    t["phase"] = ph
+    t["sigma"] = st.randint(T, 0, max(S // 2 - 1, 0))
+    t["beta"] = st.randint(T, 0, B - 1)
+    slack = np.where(ph == 1, st.urange(T, 5.0, 150.0), st.urange(T, 50.0, 2000.0))
+    t["slack_ms"] = slack.astype(np.float32)
+    t["age_ms"] = (st.uniform(T) * 1.2 * slack).astype(np.float32)
+    t["mem_mb"] = np.minimum(np.exp(5.5 + st.normal(T)), 8000.0).astype(np.float32)
+    t["tag"] = np.arange(T, dtype=np.uint32)
+    return off, t
 
 
 def arrival_ticks(seed: int, R: int, n_ticks: int, rho: float = 3.3) -> np.ndarray:
