@@ -130,6 +130,20 @@ typedef struct {
  * GPU, extra energy the destination pays, net saving of draining the source.             */
 typedef struct { int32_t dst, phi; float score_mj, saving_mj; } fs_consol_out; /* 16 bytes */
 
+/* One runnable task of the local scheduler's priority queue (Fig. 8 steps 1-2): a
+ * decode step or a prefill unit of `model`, run with `sigma`+1 SM share units at batch bucket
+ * `beta`.  slack_ms = remaining time to its SLO deadline (TBT for decode, TTFT for prefill),
+ * age_ms = time since it became runnable, mem_mb = memory it needs while running.  24 bytes. */
+typedef struct {
+  int16_t model; uint8_t phase, sigma, beta, _p0[3];
+  float slack_ms, age_ms, mem_mb; uint32_t tag;
+} fs_task;
+/* score = Eq. 4 (+INF when the effective slack is used up), latency_ms = the LUT entry it used,
+ * rank = position in descending-score order (ties: lowest index), admitted = 1 if the greedy
+ * walk put it into the batch.  rank = -1: the GPU's task list was rejected (FS_ERR_RANGE). 16 bytes. */
+typedef struct { float score, latency_ms; int32_t rank, admitted; } fs_task_out;
+#define FS_MAX_TASKS 1024  /* tasks per GPU in one fs_batch_tasks call */
+
 /* Create / destroy a context bound to CUDA device `cuda_device`.
  * fs_create: *out receives the context; FS_ERR_CUDA if the device cannot be used.        */
 int fs_create(fs_ctx** out, int cuda_device);
@@ -175,6 +189,17 @@ int fs_local_config(fs_ctx* ctx, int32_t n, const int32_t* gpu_ids, uint32_t fla
  * P:351; idle power vs migration energy P:46; R:s17-s20).   out : [K].             */
 int fs_consolidate(fs_ctx* ctx, fs_consol_out* out, int space, void* cuda_stream);
 
+/* Local scheduler steps 1-2 for n GPUs (Eq. 4, Fig. 8): unified priority
+ * score of every runnable task at the GPU's current frequency, then priority-based batching with
+ * bypass under the budgets "all S share units" and the GPU's free memory (fs_set_gpu_state).
+ * gpu_ids : [n] or NULL (= GPUs 0..n-1);  task_off : [n+1], tasks of entry i are
+ * tasks[task_off[i] .. task_off[i+1]) (at most FS_MAX_TASKS each);  tasks, out : [n_tasks].
+ * All bulk pointers live in `space`.  Invalid ids / fields raise FS_ERR_RANGE (sticky) and mark
+ * that GPU's outputs with rank = -1.                                                           */
+int fs_batch_tasks(fs_ctx* ctx, int32_t n, const int32_t* gpu_ids, const int32_t* task_off,
+                   const fs_task* tasks, fs_task_out* out, int32_t n_tasks, int space,
+                   void* cuda_stream);
+
 /* Diagnostics. */
 const char* fs_strerror(int code);
 int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed runtime call */
@@ -206,6 +231,7 @@ typedef enum {
   FS_TIMER_CONSOL_AGG,      /* per-tenant minimum shares of fs_consolidate           */
   FS_TIMER_CONSOL_PAIR,     /* pair scoring of fs_consolidate                        */
   FS_TIMER_PLACE_WARM,      /* (unused since the warm pairs moved into the scoring kernel) */
+  FS_TIMER_BATCH_TASKS,     /* fs_batch_tasks: priority score + batching            */
   FS_TIMER_COUNT
 } fs_timer;
 int fs_set_timing(fs_ctx* ctx, int on);

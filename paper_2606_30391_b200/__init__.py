@@ -23,10 +23,10 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_batch_tasks", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
-          "consol_pair", "place_warm")
+          "consol_pair", "place_warm", "batch_tasks")
 
 
 class FsDims(C.Structure):
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
     L.fs_place_batch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_local_config.argtypes = [vp, i32, vp, u32, vp, C.c_int, vp]
     L.fs_consolidate.argtypes = [vp, vp, C.c_int, vp]
+    L.fs_batch_tasks.argtypes = [vp, i32, vp, vp, vp, vp, i32, C.c_int, vp]
     L.fs_strerror.argtypes = [C.c_int]
     L.fs_strerror.restype = C.c_char_p
     L.fs_last_cuda_error.argtypes = [vp]
@@ -190,6 +191,30 @@ class Festina:
         assert spi is None or spi == spo
         rc = lib().fs_local_config(self._h, n, pi, flags, po, spo, _stream_ptr(stream))
         self._check(rc, "fs_local_config")
+        return out
+
+    def batch_tasks(self, task_off, tasks, gpu_ids=None, out=None, n: int | None = None,
+                    n_tasks: int | None = None, stream=None):
+        """fs_batch_tasks: priority score + batching with bypass for n GPUs (host arrays or device tensors)."""
+        host = not hasattr(tasks, "data_ptr")
+        if host:
+            task_off = np.ascontiguousarray(task_off, dtype=np.int32)
+            tasks = np.ascontiguousarray(tasks)
+            if gpu_ids is not None:
+                gpu_ids = np.ascontiguousarray(gpu_ids, dtype=np.int32)
+            n = len(task_off) - 1 if n is None else n
+            n_tasks = len(tasks) if n_tasks is None else n_tasks
+            if out is None:
+                out = np.zeros(n_tasks, dtype=synth.TASK_OUT_DT)
+        else:
+            assert out is not None and n is not None and n_tasks is not None
+        pi, _, k0 = _buf(gpu_ids)
+        pf, spf, k1 = _buf(task_off)
+        pt, spt, k2 = _buf(tasks, n_tasks * 24)
+        po, spo, k3 = _buf(out, n_tasks * 16)
+        sp = spf if spf is not None else FS_HOST
+        rc = lib().fs_batch_tasks(self._h, n, pi, pf, pt, po, n_tasks, sp, _stream_ptr(stream))
+        self._check(rc, "fs_batch_tasks")
         return out
 
     def consolidate(self, out=None, stream=None):

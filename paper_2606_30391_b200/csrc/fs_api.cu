@@ -34,6 +34,8 @@ struct fs_ctx {
   int32_t* ids_dev = nullptr; fs_local_cfg* local_dev = nullptr;
   int32_t *bin_off = nullptr, *bin_cursor = nullptr, *keylist = nullptr, *nkeys = nullptr; int bin_m_cap = 0;
   uint4* lslots = nullptr;
+  // task batching scratch (FS_HOST staging)
+  int bt_n_cap = 0, bt_t_cap = 0; int32_t *bt_ids = nullptr, *bt_off = nullptr; fs_task* bt_tasks = nullptr; fs_task_out* bt_out = nullptr;
   // consolidation scratch
   size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
   unsigned long long* ckeys = nullptr; fs_consol_out* consol_dev = nullptr;
@@ -155,7 +157,7 @@ int fs_destroy(fs_ctx* c) {
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
-                  c->agg, c->ckeys, c->consol_dev};
+                  c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (c->flag_host) cudaFreeHost(c->flag_host);
   if (c->have_events)
@@ -340,6 +342,36 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->consol_dev, (size_t)c->K * sizeof(fs_consol_out), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+int fs_batch_tasks(fs_ctx* c, int32_t n, const int32_t* gpu_ids, const int32_t* task_off,
+                   const fs_task* tasks, fs_task_out* out, int32_t n_tasks, int space, void* cuda_stream) {
+  if (!c || n < 0 || n_tasks < 0 || (n > 0 && !task_off) || (n_tasks > 0 && (!tasks || !out))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (n == 0) return pending;
+  const int32_t* d_ids = gpu_ids; const int32_t* d_off = task_off; const fs_task* d_tasks = tasks; fs_task_out* d_out = out;
+  if (space == FS_HOST) {
+    if (task_off[0] != 0 || task_off[n] != n_tasks) return FS_ERR_ARG;
+    if (n > c->bt_n_cap) { FS_TRY(grow(c, c->bt_ids, (size_t)n)); FS_TRY(grow(c, c->bt_off, (size_t)n + 1)); c->bt_n_cap = n; }
+    if (n_tasks > c->bt_t_cap) { FS_TRY(grow(c, c->bt_tasks, (size_t)n_tasks)); FS_TRY(grow(c, c->bt_out, (size_t)n_tasks)); c->bt_t_cap = n_tasks; }
+    if (gpu_ids) { FS_CUDA(c, cudaMemcpyAsync(c->bt_ids, gpu_ids, (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, st)); d_ids = c->bt_ids; }
+    FS_CUDA(c, cudaMemcpyAsync(c->bt_off, task_off, ((size_t)n + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (n_tasks > 0) FS_CUDA(c, cudaMemcpyAsync(c->bt_tasks, tasks, (size_t)n_tasks * sizeof(fs_task), cudaMemcpyHostToDevice, st));
+    d_off = c->bt_off; d_tasks = c->bt_tasks; d_out = c->bt_out;
+  }
+  c->launches += fsk_batch_tasks(view_of(c), n, d_ids, d_off, d_tasks, d_out, n_tasks, st, c->timing ? &c->tm : nullptr);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    if (n_tasks > 0) FS_CUDA(c, cudaMemcpyAsync(out, c->bt_out, (size_t)n_tasks * sizeof(fs_task_out), cudaMemcpyDeviceToHost, st));
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;

@@ -8,7 +8,7 @@
 // Optional per-kernel timing (fs_set_timing): CUDA event pairs recorded on the caller's stream
 // around the kernels bench.py reports rooflines for.  NULL = no timing.
 enum { FS_T_PLACE_SCORE = 0, FS_T_PLACE_DECODE, FS_T_SUMMARY, FS_T_LOCAL_SLOT, FS_T_LOCAL_SPLIT,
-       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_PLACE_WARM, FS_T_COUNT };
+       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_PLACE_WARM, FS_T_BATCH_TASKS, FS_T_COUNT };
 struct FsTimers {
   cudaEvent_t beg[FS_T_COUNT], end[FS_T_COUNT];
   bool used[FS_T_COUNT];
@@ -92,6 +92,10 @@ struct FsConsolScratch {
 };
 int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
                     const FsConsolScratch& sc, cudaStream_t st, FsTimers* tm);
+
+// fs_batch.cu — unified priority score + priority batching with bypass
+int fsk_batch_tasks(const FsView& v, int n, const int32_t* gpu_ids, const int32_t* off,
+                    const fs_task* tasks, fs_task_out* out, int n_tasks, cudaStream_t st, FsTimers* tm);
 
 #ifdef __CUDACC__
 // One co-resident ("tenant") at frequency phi with share sigma, wait = 0 because its slo is the

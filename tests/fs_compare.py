@@ -56,3 +56,11 @@ def assert_consol_equal(got, ref, exact=True):
         _int_equal(got[f], ref[f], f"consol.{f}")
     for f in ("score_mj", "saving_mj"):
         _float_close(got[f], ref[f], f"consol.{f}", exact)
+
+
+def assert_tasks_equal(got, ref):
+    assert len(got) == len(ref)
+    for f in ("rank", "admitted"):
+        _int_equal(got[f], ref[f], f"tasks.{f}")
+    for f in ("score", "latency_ms"):
+        _float_close(got[f], ref[f], f"tasks.{f}", True)

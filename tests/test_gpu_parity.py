@@ -266,3 +266,72 @@ def test_consolidation_full_size(ctx):
     got = ctx.consolidate()
     cmp.assert_consol_equal(got, _oracle_consol(cl))
     assert (got["dst"] >= 0).mean() > 0.5
+
+
+# ---- local scheduler steps 1-2: priority score + batching (fs_batch_tasks) --------------------
+def _oracle_tasks(cl, off, tasks, ids=None):
+    return oracle.batch_tasks(cl.lat, cl.pow, cl.states, off, tasks, ids, 8)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_batch_tasks_small_clusters(ctx, seed):
+    """0..130 tasks per GPU (empty lists, one task, non-powers of two, > 4 warps of tasks)."""
+    cl = synth.make_custom(seed=800 + seed, K=23, M=4, F=9, S=[4, 7, 10, 16][seed % 4], B=12, R=0)
+    off, tasks = synth.make_tasks(seed, cl.K, cl.M, cl.S, cl.B, 0, 130)
+    if seed % 2:                                    # heavy exact ties in the score
+        tasks["slack_ms"] = 64.0; tasks["age_ms"] = 0.0; tasks["beta"] = tasks["beta"] % 2
+        tasks["model"] = 0; tasks["sigma"] = tasks["sigma"] % 2
+    ctx.load_cluster(cl)
+    cmp.assert_tasks_equal(ctx.batch_tasks(off, tasks), _oracle_tasks(cl, off, tasks))
+
+
+def test_batch_tasks_limits_and_subset(ctx):
+    cl = synth.make_custom(seed=811, K=6, M=3, F=6, S=16, B=8, R=0)
+    off, tasks = synth.make_tasks(11, 3, cl.M, cl.S, cl.B, 1024, 1024)      # FS_MAX_TASKS per GPU
+    tasks["mem_mb"] *= 0.01                          # let many tasks fit the memory budget
+    ids = np.array([5, 0, 5], dtype=np.int32)
+    ctx.load_cluster(cl)
+    got = ctx.batch_tasks(off, tasks, gpu_ids=ids)
+    cmp.assert_tasks_equal(got, _oracle_tasks(cl, off, tasks, ids))
+    assert got["admitted"].sum() > 3
+    assert len(ctx.batch_tasks(np.zeros(1, np.int32), tasks[:0])) == 0      # no GPUs, no tasks
+
+
+def test_batch_tasks_fig8(ctx):
+    """The worked table of Fig. 8 steps 1-2 through the CUDA path."""
+    from test_oracle_batching import _fig8_cluster
+    lat, pw, st, tasks, names, fig = _fig8_cluster(mem_free=1e6)
+    M, _, F, S, B = lat.shape
+    models = np.zeros(M, dtype=synth.MODEL_INFO_DT)
+    ctx.load_profiles(lat, pw, np.ones(F, np.float32), models, synth.Params())
+    ctx.set_gpu_state(st)
+    out = ctx.batch_tasks([0, 6], tasks)
+    assert [names[i] for i in np.argsort(out["rank"])] == ["D1", "D3", "D2", "P1", "P3", "P2"]
+    assert {nm: int(out["admitted"][i]) for i, nm in enumerate(names)} == \
+        {"D1": 1, "D3": 1, "D2": 1, "P1": 0, "P3": 1, "P2": 0}
+
+
+def test_batch_tasks_errors(fs):
+    c = fs.Festina(0)
+    cl = synth.make_custom(seed=812, K=4, M=2, F=4, S=4, B=4, R=0)
+    off, tasks = synth.make_tasks(12, cl.K, cl.M, cl.S, cl.B, 3, 9)
+    c.load_cluster(cl)
+    bad = tasks.copy()
+    bad["sigma"][off[2]] = 9                         # share index out of range on GPU 2
+    with pytest.raises(fs.FestinaError) as e:
+        c.batch_tasks(off, bad)
+    assert e.value.code == fs.FS_ERR_RANGE
+    with pytest.raises(fs.FestinaError) as e:
+        c.batch_tasks(off, tasks, gpu_ids=np.array([0, 1, 99, 3], np.int32))
+    assert e.value.code == fs.FS_ERR_RANGE
+    got = c.batch_tasks(off, tasks)                  # clean call afterwards
+    cmp.assert_tasks_equal(got, oracle.batch_tasks(cl.lat, cl.pow, cl.states, off, tasks))
+    c.close()
+
+
+def test_batch_tasks_pod_size(ctx):
+    """1,024 GPUs x 10-100 queued tasks (the paper's Table 3 queue sizes), every task compared."""
+    cl = synth.make_cluster("pod")
+    off, tasks = synth.make_tasks(2, cl.K, cl.M, cl.S, cl.B, 10, 100)
+    ctx.load_cluster(cl)
+    cmp.assert_tasks_equal(ctx.batch_tasks(off, tasks), _oracle_tasks(cl, off, tasks))
