@@ -329,6 +329,134 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def _slot_evals(cl) -> int:
+    """Sum over live slots of F*S*min(B, q): the (slot, phi, sigma, beta) grid fs_local_config searches."""
+    q = cl.states["t"]["q"].astype(np.int64)
+    live = np.arange(4)[None, :] < cl.states["n_res"][:, None]
+    return int((np.minimum(q, cl.B) * live[:, :, None]).sum()) * cl.F * cl.S
+
+
+def run_aux(args):
+    """--workload local (BASELINE.json configs[3]) / consol (configs[4]): the other two entry points at
+    their own full-size configs, same JSON contract.  1 GPU."""
+    import torch
+    import paper_2606_30391_b200 as fs
+    import oracle
+    ws, rank, lrank = _dist()
+    assert ws == 1, "the local / consol workloads are single-GPU bench lines"
+    dev = torch.device("cuda", lrank)
+    torch.cuda.set_device(dev)
+    cl = synth.make_cluster(args.workload)
+    ctx = fs.Festina(lrank)
+    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+    ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                      tb(cl.models), cl.params)
+    d_states = tb(cl.states)
+    local = args.workload == "local"
+    rec = 48 if local else 16
+    d_out = torch.empty(cl.K * rec, dtype=torch.uint8, device=dev)
+    h_states = torch.from_numpy(cl.states.view(np.uint8).reshape(-1).copy()).pin_memory()
+    h_out = torch.empty(cl.K * rec, dtype=torch.uint8).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    ctx.set_timing(True)
+    flags = fs.FS_OBJ_POWER | fs.FS_SPLIT_EXHAUSTIVE      # configs[3]: "minimum-power feasible config"
+
+    def step(states, out):
+        ctx.set_gpu_state(states, stream=stream)
+        if local:
+            ctx.local_config(flags, n=cl.K, out=out, stream=stream)
+        else:
+            ctx.consolidate(out=out, stream=stream)
+
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        step(d_states, d_out)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(lrank)
+    sampler.start()
+    l0 = ctx.launch_count
+    kt, dev_ms = {}, 0.0
+    for _ in range(args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream); step(d_states, d_out); b.record(stream); b.synchronize()
+        dev_ms += a.elapsed_time(b)
+        for k, v in ctx.get_timing().items():
+            kt.setdefault(k, []).append(v)
+    launches = ctx.launch_count - l0
+    for _ in range(3):
+        step(h_states, h_out)
+    e2e_t = 0.0
+    for _ in range(args.steps):
+        flush.zero_(); torch.cuda.synchronize()
+        t0 = time.perf_counter(); step(h_states, h_out); torch.cuda.synchronize()
+        e2e_t += time.perf_counter() - t0
+    clocks = sampler.stop()
+    assert np.array_equal(h_out.numpy(), d_out.cpu().numpy()), "host and device paths disagree"
+    peaks, peak_src = _peaks()
+    alu_peak = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    cores = os.cpu_count() or 1
+    if local:
+        units, unit_name, metric = _slot_evals(cl), "slot evals/s", "local_slot_evals_per_sec"
+        kname, kms, ops = "local_slot_grouped_kernel (a7)", float(np.mean(kt["local_slot"])), 5.0
+        ops_note = ("5 lane-ops per (slot, phi, sigma, beta) under the power objective: 2 table values, "
+                    "rounds*LAT, deadline compare, cost compare/select (6 under the energy objective)")
+        res = d_out.cpu().numpy().view(synth.LOCAL_CFG_DT)
+        degeneracy = {"feasible_frac": float((res["phi"] >= 0).mean()),
+                      "top_phi_share": float(np.bincount(res["phi"][res["phi"] >= 0]).max() / max((res["phi"] >= 0).sum(), 1))}
+        n_s = args.cpu_gpus
+        t0 = time.perf_counter()
+        ref = oracle.local_config(cl.lat, cl.pow, cl.states, flags, np.arange(n_s, dtype=np.int32), cores)
+        dt = time.perf_counter() - t0
+        assert np.array_equal(ref["flat"], res["flat"][:n_s]), "CUDA and oracle disagree on the sample"
+        sub = synth.Cluster(**{**cl.__dict__, "states": cl.states[:n_s], "K": n_s})
+        cpu = {"value": _slot_evals(sub) / dt, "unit": unit_name, "cores": cores, "kind": "oracle",
+               "sample": f"GPUs 0..{n_s - 1} of {cl.K}, {dt:.1f} s"}
+        work = (f"local (BASELINE.json configs[3]): K={cl.K} GPUs, 2-4 co-residents, queue depths U{{0..256}}, "
+                f"F={cl.F} x all SM splits (S={cl.S}) x batch 1..{cl.B}; step = fs_set_gpu_state + "
+                "fs_local_config(all GPUs, power objective, exhaustive splits)")
+        decisions = cl.K
+    else:
+        units, unit_name, metric = cl.K * cl.K * cl.F, "pair-frequency evals/s", "consol_pair_freq_evals_per_sec"
+        kname, kms, ops = "consol_pair_kernel (a10)", float(np.mean(kt["consol_pair"])), 8.0
+        ops_note = ("8 lane-ops per (source, destination, phi): 2 fp32 + 2 small-int values, int add + compare, "
+                    "fp32 add, min (SURVEY 8(d))")
+        res = d_out.cpu().numpy().view(synth.CONSOL_DT)
+        degeneracy = {"has_destination_frac": float((res["dst"] >= 0).mean()),
+                      "distinct_destinations": int(len(np.unique(res["dst"][res["dst"] >= 0])))}
+        p = cl.params
+        t0 = time.perf_counter()
+        ref = oracle.consolidate(cl.lat, cl.pow, cl.models, cl.states, p.p_idle_w, p.horizon_ms, p.mem_cap_mb,
+                                 p.delta_pct, cores)
+        dt = time.perf_counter() - t0
+        assert np.array_equal(ref["dst"], res["dst"]), "CUDA and oracle disagree"
+        cpu = {"value": units / dt, "unit": unit_name, "cores": cores, "kind": "oracle",
+               "sample": f"the whole config ({cl.K} sources x {cl.K} destinations), {dt:.1f} s"}
+        work = (f"consol (BASELINE.json configs[4]): K={cl.K} GPUs, M={cl.M}, 1-2 tenants, load ~ Beta(2,5); "
+                f"step = fs_set_gpu_state + fs_consolidate ({cl.K * cl.K} pairs x {cl.F} frequencies)")
+        decisions = cl.K
+    steps = args.steps
+    achieved = ops * units / (kms * 1e-3)
+    line = {"metric": metric, "value": units * steps / (dev_ms * 1e-3), "unit": unit_name, "n_gpus": 1,
+            "steps": steps, "warmup": warm, "ms_per_step": dev_ms / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": work, "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B,
+                       "l2": "flushed between timed steps by overwriting a 256 MiB buffer"},
+            "decisions_per_sec": decisions * steps / (dev_ms * 1e-3),
+            "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
+            "e2e": {"value": units * steps / e2e_t, "unit": unit_name, "ms_per_step": 1e3 * e2e_t / steps,
+                    "h2d_bytes_per_step": cl.K * 128, "d2h_bytes_per_step": cl.K * rec},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": {"bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": alu_peak / 1e12,
+                         "unit": "Tlane-op/s", "frac": achieved / alu_peak, "traffic": None, "kernel_ms": kms,
+                         "note": ops_note + f"; x {units} units / CUDA-event time of the kernel; peak = 148 SMs x "
+                                 f"128 lanes/clk x sm_max_mhz ({peak_src})"},
+            "degeneracy": degeneracy, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -338,10 +466,13 @@ def main():
     ap.add_argument("--workload", default="pod", choices=list(synth.CONFIGS))
     ap.add_argument("--cpu-requests", type=int, default=1536, help="oracle sample of the cpu_baseline leg")
     ap.add_argument("--ref-requests", type=int, default=256, help="oracle sample per step of --impl reference")
+    ap.add_argument("--cpu-gpus", type=int, default=4096, help="oracle sample (GPUs) of --workload local")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload in ("local", "consol"):
+        run_aux(args)
     else:
         run_ours(args)
 
