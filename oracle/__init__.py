@@ -59,6 +59,14 @@ def place_batch(lat, pow_, models, states, reqs, nthreads: int = 1) -> np.ndarra
     return out
 
 
+def dispatch(lat, pow_, models, states, reqs, nthreads: int = 1) -> np.ndarray:
+    """The paper's three-phase dispatcher at (F_curr, SM_free) (Eq. 2-3)."""
+    out = np.zeros(len(reqs), dtype=_PLACEMENT_DT)
+    lib().fo_dispatch(*_tables(lat, pow_), _p(models), C.c_int(len(states)), _p(states),
+                      C.c_int(len(reqs)), _p(reqs), _p(out), C.c_int(nthreads))
+    return out
+
+
 def local_config(lat, pow_, states, flags: int, gpu_ids=None, nthreads: int = 1) -> np.ndarray:
     """fs_local_config by definition (Fig. 8 step 3)."""
     if gpu_ids is None:

@@ -16,6 +16,9 @@
 //   local config .......... Fig. 8 step 3 worked table, brute force
 //   consolidation ......... brute force, C*_ab symmetry, empty-destination case,
 //                           App. G arithmetic
+//   paper dispatcher ...... Eq. 2-3 by hand, Fig. 6-shaped toy, 2 % band
+//                           and tie-breaker cases, T_avail-ordered F_max retry and
+//                           scale-out, independent numpy restatement
 //   priority batching ..... Fig. 8 steps 1-2 worked table, independent numpy
 //                           restatement, budget / bypass invariants
 // Nothing here is "parity unpinned".
@@ -157,6 +160,97 @@ void place_one(const Tables& T, const ModelInfo* mi, const GpuState* gs, int K,
     }
   }
   (void)bestFlat;
+  out = best;
+}
+
+// ------------------------------------------------------------------------------------------
+// fs_dispatch: the paper's own three-phase dispatcher (Fig. 6), one operating point
+// per GPU: S_k = SM_free (all free share units), f_k = F_curr.
+//   Phase 1: GPU k is feasible iff the request, starting at T_avail with SM_free SMs,
+//     meets its deadlines at F_curr (plus memory / slot eligibility as in fs_place_batch).
+//   Phase 2 (Eq. 2-3): E^k = Power x Latency of the request's own prefill + decode
+//     work at (f_k, S_k); k* = argmin E^k.  Near-ties: among feasible GPUs with
+//     E^k <= fl(1.02*E_min) take the most free memory, then the largest SM_free, then lowest k.
+//   Phase 3: no feasible GPU -> walk the GPUs in ascending T_avail (ties: lowest k),
+//     evaluate at F_max (last frequency level), take the first feasible one.  Still none ->
+//     scale out: gpu = -1 and the energy-optimal feasible frequency of a fresh, empty GPU
+//     (all S units, wait = load_ms), "minimizing energy usage without violating SLOs".
+// Output: Placement with f_req reused as the phase that decided (1 = F_curr, 2 = F_max retry,
+// 3 = scale-out, -1 = nothing feasible even on a fresh GPU); flat = (k*S+sigma)*F+phi.
+struct OwnEval { bool ok; float e, ttft, tbt; };
+OwnEval own_eval(const Tables& T, const Request& rq, uint32_t O, int phi, int sg, int br1, float wait) {
+  const int m = rq.model;
+  const int br0 = (int)(rq.L < (uint32_t)T.B ? rq.L : (uint32_t)T.B) - 1;
+  Slot s0 = slot_eval(T, m, 0, phi, sg, br0 < 0 ? 0 : br0, rq.L, wait, rq.slo_ttft_ms);
+  Slot s1 = slot_eval(T, m, 1, phi, sg, br1, O, 0.0f, rq.slo_tbt_ms);
+  float e = s0.e + s1.e;
+  return {s0.ok && s1.ok && e < INF, e, wait + s0.t, T.LAT(m, 1, phi, sg, br1)};
+}
+
+void dispatch_one(const Tables& T, const ModelInfo* mi, const GpuState* gs, int K,
+                  const Request& rq, Placement& out) {
+  const int m = rq.model;
+  const uint32_t O = (21u * rq.o_pred + 19u) / 20u;
+  const float mem = (float)(rq.L + O) * mi[m].kv_mb_per_token;
+  Placement best{}; best.gpu = -1; best.sigma = best.phi = best.beta = best.f_req = -1;
+  best.energy_mj = INF; best.ttft_ms = INF; best.tbt_ms = INF; best.flat = 0xFFFFFFFFu;
+  struct Cand { bool elig; int smf, br1; float wait; };
+  std::vector<Cand> cd(K);
+  for (int k = 0; k < K; ++k) {                            // eligibility, as in fs_place_batch
+    const GpuState& g = gs[k]; Cand c{false, 0, 0, 0.0f};
+    if (g.n_res >= 1 && mem <= g.mem_free_mb) {
+      c.smf = sm_free_of(g, T.S);
+      int j = -1;
+      for (int i = 0; i < g.n_res; ++i) if (g.t[i].model == m) { j = i; break; }
+      c.wait = g.t_avail_ms;
+      if (j < 0) c.wait = c.wait + mi[m].load_ms;
+      c.br1 = (j >= 0 && g.t[j].q[1] > 0) ? g.t[j].beta[1] + 1 : 0;
+      c.elig = c.smf >= 1 && (j >= 0 || g.n_res < RMAX) && c.br1 < T.B;
+    }
+    cd[k] = c;
+  }
+  auto fill = [&](int k, int phi, const OwnEval& ev, int phase) {
+    best.gpu = k; best.sigma = (int16_t)(cd[k].smf - 1); best.phi = (int16_t)phi;
+    best.beta = (int16_t)cd[k].br1; best.f_req = (int16_t)phase; best.energy_mj = ev.e;
+    best.ttft_ms = ev.ttft; best.tbt_ms = ev.tbt;
+    best.flat = (uint32_t)((k * T.S + cd[k].smf - 1) * T.F + phi);
+  };
+  // Phase 1 + 2 at F_curr
+  float emin = INF;
+  for (int k = 0; k < K; ++k) if (cd[k].elig) {
+    OwnEval ev = own_eval(T, rq, O, gs[k].f_cur, cd[k].smf - 1, cd[k].br1, cd[k].wait);
+    if (ev.ok && ev.e < emin) emin = ev.e;
+  }
+  if (emin < INF) {
+    const float band = 1.02f * emin;
+    int bk = -1;
+    for (int k = 0; k < K; ++k) if (cd[k].elig) {
+      OwnEval ev = own_eval(T, rq, O, gs[k].f_cur, cd[k].smf - 1, cd[k].br1, cd[k].wait);
+      if (!(ev.ok && ev.e <= band)) continue;
+      if (bk < 0 || gs[k].mem_free_mb > gs[bk].mem_free_mb ||
+          (gs[k].mem_free_mb == gs[bk].mem_free_mb && cd[k].smf > cd[bk].smf)) {
+        bk = k; fill(k, gs[k].f_cur, ev, 1);
+      }
+    }
+    out = best; return;
+  }
+  // Phase 3: F_max retry in T_avail order
+  {
+    int bk = -1; OwnEval bev{};
+    for (int k = 0; k < K; ++k) if (cd[k].elig) {
+      OwnEval ev = own_eval(T, rq, O, T.F - 1, cd[k].smf - 1, cd[k].br1, cd[k].wait);
+      if (ev.ok && (bk < 0 || gs[k].t_avail_ms < gs[bk].t_avail_ms)) { bk = k; bev = ev; }
+    }
+    if (bk >= 0) { fill(bk, T.F - 1, bev, 2); out = best; return; }
+  }
+  // scale-out: best frequency of a fresh GPU
+  for (int phi = 0; phi < T.F; ++phi) {
+    OwnEval ev = own_eval(T, rq, O, phi, T.S - 1, 0, mi[m].load_ms);
+    if (ev.ok && ev.e < best.energy_mj) {
+      best.sigma = (int16_t)(T.S - 1); best.phi = (int16_t)phi; best.beta = 0; best.f_req = 3;
+      best.energy_mj = ev.e; best.ttft_ms = ev.ttft; best.tbt_ms = ev.tbt;
+    }
+  }
   out = best;
 }
 
@@ -396,6 +490,16 @@ int fo_place_batch(int M, int F, int S, int B, const float* lat, const float* po
   const ModelInfo* mi = (const ModelInfo*)models; const GpuState* gs = (const GpuState*)states;
   const Request* rq = (const Request*)reqs; Placement* o = (Placement*)out;
   par_for(R, nthreads, [&](int r) { place_one(T, mi, gs, K, rq[r], o[r]); });
+  return 0;
+}
+
+int fo_dispatch(int M, int F, int S, int B, const float* lat, const float* pow,
+                const void* models, int K, const void* states, int R, const void* reqs,
+                void* out, int nthreads) {
+  Tables T{M, F, S, B, lat, pow};
+  const ModelInfo* mi = (const ModelInfo*)models; const GpuState* gs = (const GpuState*)states;
+  const Request* rq = (const Request*)reqs; Placement* o = (Placement*)out;
+  par_for(R, nthreads, [&](int r) { dispatch_one(T, mi, gs, K, rq[r], o[r]); });
   return 0;
 }
 
