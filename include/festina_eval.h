@@ -189,6 +189,19 @@ int fs_local_config(fs_ctx* ctx, int32_t n, const int32_t* gpu_ids, uint32_t fla
  * P:351; idle power vs migration energy P:46; R:s17-s20).   out : [K].             */
 int fs_consolidate(fs_ctx* ctx, fs_consol_out* out, int space, void* cuda_stream);
 
+/* The paper's own dispatcher (Fig. 6): one operating point per GPU, S_k = SM_free and
+ * f_k = F_curr.  Phase 1: feasibility of the request at F_curr (same eligibility as
+ * fs_place_batch).  Phase 2: E^k = Power x Latency of the request's own work (Eq. 2), argmin
+ * (Eq. 3); among GPUs within 2 % of the minimum the most free memory wins, then the largest
+ * SM_free, then the lowest index.  Phase 3: if none is feasible, the first GPU in
+ * ascending T_avail that is feasible at F_max (last frequency level); else scale-out: gpu = -1
+ * and sigma = S-1, phi = the energy-optimal feasible frequency of a fresh GPU (wait = load_ms).
+ * Output records as fs_place_batch, except: energy_mj = E^k (not a marginal energy) and f_req =
+ * the phase that decided (1 = F_curr, 2 = F_max retry, 3 = scale-out, -1 = infeasible even on
+ * a fresh GPU).  Requires K < 2^24.  reqs : [R]; out : [R]; both in `space`.                  */
+int fs_dispatch(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* out, int space,
+                void* cuda_stream);
+
 /* Local scheduler steps 1-2 for n GPUs (Eq. 4, Fig. 8): unified priority
  * score of every runnable task at the GPU's current frequency, then priority-based batching with
  * bypass under the budgets "all S share units" and the GPU's free memory (fs_set_gpu_state).
@@ -232,6 +245,7 @@ typedef enum {
   FS_TIMER_CONSOL_PAIR,     /* pair scoring of fs_consolidate                        */
   FS_TIMER_PLACE_WARM,      /* (unused since the warm pairs moved into the scoring kernel) */
   FS_TIMER_BATCH_TASKS,     /* fs_batch_tasks: priority score + batching            */
+  FS_TIMER_DISPATCH,        /* fs_dispatch: the paper's three-phase dispatcher      */
   FS_TIMER_COUNT
 } fs_timer;
 int fs_set_timing(fs_ctx* ctx, int on);

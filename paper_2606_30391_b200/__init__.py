@@ -23,10 +23,10 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_batch_tasks", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
-          "consol_pair", "place_warm", "batch_tasks")
+          "consol_pair", "place_warm", "batch_tasks", "dispatch")
 
 
 class FsDims(C.Structure):
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
     L.fs_place_batch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_local_config.argtypes = [vp, i32, vp, u32, vp, C.c_int, vp]
     L.fs_consolidate.argtypes = [vp, vp, C.c_int, vp]
+    L.fs_dispatch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_batch_tasks.argtypes = [vp, i32, vp, vp, vp, vp, i32, C.c_int, vp]
     L.fs_strerror.argtypes = [C.c_int]
     L.fs_strerror.restype = C.c_char_p
@@ -176,6 +177,21 @@ class Festina:
         assert spo == sp or R == 0
         rc = lib().fs_place_batch(self._h, R, pr, po, sp, _stream_ptr(stream))
         self._check(rc, "fs_place_batch")
+        return out
+
+    def dispatch(self, reqs, out=None, R: int | None = None, stream=None):
+        """fs_dispatch: the paper's three-phase dispatcher at (F_curr, SM_free)."""
+        if R is None:
+            R = len(reqs) if not hasattr(reqs, "data_ptr") else reqs.numel() * reqs.element_size() // 32
+        pr, sp, keep = _buf(reqs, R * 32)
+        if sp is None:
+            sp = FS_HOST
+        if out is None:
+            assert sp == FS_HOST, "device inputs need a device `out` tensor"
+            out = np.zeros(R, dtype=synth.PLACEMENT_DT)
+        po, spo, keep2 = _buf(out, R * 32)
+        assert spo == sp or R == 0
+        self._check(lib().fs_dispatch(self._h, R, pr, po, sp, _stream_ptr(stream)), "fs_dispatch")
         return out
 
     def local_config(self, flags: int = 0, gpu_ids=None, n: int | None = None, out=None, stream=None):

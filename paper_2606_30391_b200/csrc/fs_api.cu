@@ -349,6 +349,37 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
   return pending;
 }
 
+int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out, int space,
+                void* cuda_stream) {
+  if (!c || R < 0 || (R > 0 && (!reqs || !out))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
+  if (c->K >= (1 << 24)) return FS_ERR_SHAPE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (R == 0) return pending;
+  if (R > c->r_cap) {
+    FS_TRY(grow(c, c->keys, (size_t)R)); FS_TRY(grow(c, c->reqs_dev, (size_t)R));
+    FS_TRY(grow(c, c->place_dev, (size_t)R));
+    c->r_cap = R;
+  }
+  const fs_request* d_reqs = reqs; fs_placement* d_out = out;
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
+    d_reqs = c->reqs_dev; d_out = c->place_dev;
+  }
+  c->launches += fsk_dispatch(view_of(c), R, d_reqs, d_out, st, c->timing ? &c->tm : nullptr);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
 int fs_batch_tasks(fs_ctx* c, int32_t n, const int32_t* gpu_ids, const int32_t* task_off,
                    const fs_task* tasks, fs_task_out* out, int32_t n_tasks, int space, void* cuda_stream) {
   if (!c || n < 0 || n_tasks < 0 || (n > 0 && !task_off) || (n_tasks > 0 && (!tasks || !out))) return FS_ERR_ARG;

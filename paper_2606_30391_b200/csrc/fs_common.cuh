@@ -36,7 +36,8 @@ struct __align__(16) FsGpuInfo {
   int16_t model[FS_RMAX];   // tenant models (-1 beyond n_res)
   int16_t br1[FS_RMAX];     // decode bucket a joining request sees: beta_1+1 if q_1>0 else 0;
                             // -1 = bucket past the table (candidate dropped)
-  uint32_t _pad[2];
+  int32_t f_cur;            // F_curr (0 for an inactive / invalid record)
+  uint32_t _pad;
 };
 static_assert(sizeof(FsGpuInfo) == 48, "FsGpuInfo layout");
 

@@ -8,7 +8,7 @@
 // Optional per-kernel timing (fs_set_timing): CUDA event pairs recorded on the caller's stream
 // around the kernels bench.py reports rooflines for.  NULL = no timing.
 enum { FS_T_PLACE_SCORE = 0, FS_T_PLACE_DECODE, FS_T_SUMMARY, FS_T_LOCAL_SLOT, FS_T_LOCAL_SPLIT,
-       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_PLACE_WARM, FS_T_BATCH_TASKS, FS_T_COUNT };
+       FS_T_CONSOL_AGG, FS_T_CONSOL_PAIR, FS_T_PLACE_WARM, FS_T_BATCH_TASKS, FS_T_DISPATCH, FS_T_COUNT };
 struct FsTimers {
   cudaEvent_t beg[FS_T_COUNT], end[FS_T_COUNT];
   bool used[FS_T_COUNT];
@@ -62,6 +62,8 @@ struct FsPlaceScratch {
 int fsk_place_smem_attr();
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
               const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm);
+// the paper's three-phase dispatcher at (F_curr, SM_free)
+int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* out, cudaStream_t st, FsTimers* tm);
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,
                          FsWarmItem* items /*[4K]*/, cudaStream_t st);
 

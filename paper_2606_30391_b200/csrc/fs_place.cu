@@ -518,6 +518,177 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
   if (lane == 0) out[r] = o;
 }
 
+// =============================================================================================
+// fs_dispatch: the paper's own three-phase dispatcher (Fig. 6), ONE operating point
+// per GPU: S_k = SM_free (sigma = sm_free-1), f_k = F_curr.
+//   Phase 1 feasibility at F_curr;  Phase 2 (Eq. 2-3) E^k = Power x Latency
+//   of the request's own work, argmin; 2 % band -> most free memory, largest SM_free, lowest k
+//   (P:229);  Phase 3 F_max retry, first feasible GPU in T_avail order; then scale-out:
+//   energy-optimal feasible frequency of a fresh GPU (all S units, wait = load_ms).
+// One warp = one request.  The warp builds the request's (sigma, phi) tiles t0 / er for the cold
+// case in shared memory once (as the S x F scorer does); a cold (request, GPU) pair is then two
+// shared-memory reads at (sm_free-1, F_curr), a warm pair (model resident: its own decode bucket)
+// reads the planes.  Lanes <-> GPUs; reductions by redux / 64-bit key shuffles.
+// =============================================================================================
+constexpr int DISP_WARPS = 8;
+
+struct OwnEval { bool ok; float e, ttft, tbt; };
+
+// the request's own prefill + decode work at (phi, sg) on pair p, from the planes (definition)
+__device__ __forceinline__ OwnEval own_eval_planes(const FsView& v, const ReqCtx& c, int br1, uint32_t rounds1,
+                                                   float wait, int sg, int phi) {
+  const FsDimsDev& d = v.d;
+  const size_t o = (size_t)sg * d.F + phi;
+  const size_t i0 = fs_plane(d, c.m, 0, c.br0) + o, i1 = fs_plane(d, c.m, 1, br1) + o;
+  const float lat1 = v.latT[i1];
+  bool ok = true; float t0 = 0.f, e0 = 0.f, e1 = 0.f;
+  if (c.L > 0) { FsSlot s = fs_slot(0, v.latT[i0], v.powT[i0], c.rounds0, wait, c.slo_ttft); ok = s.ok; t0 = s.t; e0 = s.e; }
+  if (c.O > 0) { FsSlot s = fs_slot(1, lat1, v.powT[i1], rounds1, 0.f, c.slo_tbt); ok = ok && s.ok; e1 = s.e; }
+  OwnEval r; r.e = __fadd_rn(e0, e1); r.ok = ok && r.e < FS_INF;
+  r.ttft = __fadd_rn(wait, t0); r.tbt = lat1;
+  return r;
+}
+
+struct DispPair { bool ok; float e; };
+// pair (request, GPU gi) at frequency phi: cold pairs from the tiles, warm pairs from the planes
+__device__ __forceinline__ DispPair disp_pair(const FsView& v, const ReqCtx& c, const PairCtx& p, int phi,
+                                              const float* tl_t0, const float* tl_er, int FT) {
+  DispPair r; r.ok = false; r.e = FS_INF;
+  if (!p.ok) return r;
+  const int sg = p.smf - 1;
+  if (p.j < 0 && tl_t0) {
+    const float t0 = tl_t0[sg * FT + phi];
+    r.e = tl_er[sg * FT + phi];
+    r.ok = (c.L == 0 || __fadd_rn(p.wait, t0) <= c.slo_ttft) && r.e < FS_INF;
+  } else {
+    const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, sg, phi);
+    r.ok = ev.ok; r.e = ev.e;
+  }
+  return r;
+}
+
+template <int NPHI>
+__global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int R,
+                                                                  const fs_request* __restrict__ reqs,
+                                                                  fs_placement* __restrict__ out, int use_tiles) {
+  extern __shared__ __align__(16) unsigned char disp_smem[];
+  constexpr int FT = 32 * NPHI;
+  const FsDimsDev d = v.d;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int r = blockIdx.x * DISP_WARPS + warp;
+  if (r >= R) return;
+  // F > 64: no tiles, every pair from the planes
+  float* tl_t0 = use_tiles ? reinterpret_cast<float*>(disp_smem) + (size_t)warp * 2 * d.S * FT : nullptr;
+  float* tl_er = tl_t0 + d.S * FT;
+  fs_placement o;
+  o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
+  o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
+  const ReqCtx c = make_req(v, reqs[r]);
+  if (!c.valid) { if (lane == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } return; }
+  // ---- the request's cold tiles: t0 = fl(rounds0*LAT0), er = fl(e0 + e1) (INF where LAT1 > slo_tbt)
+  if (use_tiles) {
+    const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
+    const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
+    const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
+    const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
+    const bool vec = NPHI == 2 && (d.F & 1) == 0;
+    const int phi0 = lane * NPHI;
+#pragma unroll 2
+    for (int s = 0; s < d.S; ++s) {
+      float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI], tt[NPHI], ee[NPHI];
+      const int ofs = s * d.F;
+      ld_cols<NPHI>(l0, ofs, phi0, d.F, vec, a0); ld_cols<NPHI>(p0, ofs, phi0, d.F, vec, b0);
+      ld_cols<NPHI>(l1, ofs, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, ofs, phi0, d.F, vec, b1);
+#pragma unroll
+      for (int i = 0; i < NPHI; ++i) {
+        const float t = __fmul_rn(fr0, a0[i]);
+        const float e = __fadd_rn(__fmul_rn(t, b0[i]), __fmul_rn(__fmul_rn(fO, a1[i]), b1[i]));
+        const bool in = (phi0 + i) < d.F;
+        tt[i] = in ? t : FS_INF;
+        ee[i] = (in && a1[i] <= tbt) ? e : FS_INF;
+      }
+      st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
+    }
+    __syncwarp();
+  }
+  // ---- Phase 1 + 2 at F_curr: E_min, then the 2 % band with the stability tie-breaker ----------
+  uint32_t emin_o = 0xFFFFFFFFu;
+  for (int base = 0; base < v.K; base += 32) {
+    const int k = base + lane;
+    if (k < v.K) {
+      const FsGpuInfo gi = v.ginfo[k];
+      const DispPair dp = disp_pair(v, c, make_pair(v, c, gi), gi.f_cur, tl_t0, tl_er, FT);
+      if (dp.ok) emin_o = min(emin_o, fs_orderable(dp.e));
+    }
+  }
+  emin_o = warp_min_u32(emin_o);
+  int phase = -1, kbest = -1, phibest = -1;
+  if (emin_o != 0xFFFFFFFFu) {
+    const float band = __fmul_rn(1.02f, fs_unorderable(emin_o));
+    unsigned long long key = FS_KEY_NONE;              // (most memory, largest SM_free, lowest k)
+    for (int base = 0; base < v.K; base += 32) {
+      const int k = base + lane;
+      if (k < v.K) {
+        const FsGpuInfo gi = v.ginfo[k];
+        const DispPair dp = disp_pair(v, c, make_pair(v, c, gi), gi.f_cur, tl_t0, tl_er, FT);
+        if (dp.ok && dp.e <= band) {
+          const unsigned long long kk = ((unsigned long long)(~fs_orderable(gi.mem_free_mb)) << 32) |
+                                        ((unsigned long long)(uint32_t)(d.S - gi.sm_free) << 24) | (uint32_t)k;
+          key = kk < key ? kk : key;
+        }
+      }
+    }
+    key = fs_warp_min_key(key);
+    kbest = (int)((uint32_t)key & 0xFFFFFFu); phase = 1;
+    phibest = v.ginfo[kbest].f_cur;
+  } else {
+    // ---- Phase 3: F_max retry, first feasible GPU in T_avail order ------------------------------
+    unsigned long long key = FS_KEY_NONE;
+    for (int base = 0; base < v.K; base += 32) {
+      const int k = base + lane;
+      if (k < v.K) {
+        const FsGpuInfo gi = v.ginfo[k];
+        const DispPair dp = disp_pair(v, c, make_pair(v, c, gi), d.F - 1, tl_t0, tl_er, FT);
+        if (dp.ok) {
+          const unsigned long long kk = ((unsigned long long)fs_orderable(gi.t_avail_ms) << 32) | (uint32_t)k;
+          key = kk < key ? kk : key;
+        }
+      }
+    }
+    key = fs_warp_min_key(key);
+    if (key != FS_KEY_NONE) { kbest = (int)(uint32_t)key; phase = 2; phibest = d.F - 1; }
+  }
+  if (kbest >= 0) {
+    const PairCtx p = make_pair(v, c, v.ginfo[kbest]);
+    const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, p.smf - 1, phibest);
+    o.gpu = kbest; o.sigma = (int16_t)(p.smf - 1); o.phi = (int16_t)phibest; o.beta = (int16_t)p.br1;
+    o.f_req = (int16_t)phase; o.energy_mj = ev.e; o.ttft_ms = ev.ttft; o.tbt_ms = ev.tbt;
+    o.flat = (uint32_t)((kbest * d.S + p.smf - 1) * d.F + phibest);
+  } else {
+    // ---- scale-out: energy-optimal feasible frequency of a fresh GPU (all S units, wait = load_ms)
+    unsigned long long key = FS_KEY_NONE;
+    for (int phi = lane; phi < d.F; phi += 32) {
+      bool ok; float e;
+      if (use_tiles) {
+        const float t0 = tl_t0[(d.S - 1) * FT + phi]; e = tl_er[(d.S - 1) * FT + phi];
+        ok = (c.L == 0 || __fadd_rn(c.load_ms, t0) <= c.slo_ttft) && e < FS_INF;
+      } else { const OwnEval ev = own_eval_planes(v, c, 0, c.O, c.load_ms, d.S - 1, phi); ok = ev.ok; e = ev.e; }
+      if (ok) {
+        const unsigned long long kk = fs_make_key(e, (uint32_t)phi);
+        key = kk < key ? kk : key;
+      }
+    }
+    key = fs_warp_min_key(key);
+    if (key != FS_KEY_NONE) {
+      const int phi = (int)(uint32_t)key;
+      const OwnEval ev = own_eval_planes(v, c, 0, c.O, c.load_ms, d.S - 1, phi);
+      o.sigma = (int16_t)(d.S - 1); o.phi = (int16_t)phi; o.beta = 0; o.f_req = 3;
+      o.energy_mj = ev.e; o.ttft_ms = ev.ttft; o.tbt_ms = ev.tbt;
+    }
+  }
+  if (lane == 0) out[r] = o;
+}
+
 }  // namespace
 
 int fsk_place_smem_attr() {
@@ -525,6 +696,8 @@ int fsk_place_smem_attr() {
   e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   e |= (int)cudaFuncSetAttribute(place_dense_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(dispatch_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 32 * 4);
+  e |= (int)cudaFuncSetAttribute(dispatch_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 64 * 4);
   return e;
 }
 
@@ -586,4 +759,16 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   fs_tm_end(tm, FS_T_PLACE_DECODE, st);
   ++launches;
   return launches;
+}
+
+int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* out, cudaStream_t st, FsTimers* tm) {
+  if (R <= 0) return 0;
+  const int use_tiles = v.d.F <= 64;
+  const int FT = v.d.F <= 32 ? 32 : 64;
+  const size_t smem = use_tiles ? (size_t)DISP_WARPS * 2 * v.d.S * FT * sizeof(float) : 0;
+  fs_tm_beg(tm, FS_T_DISPATCH, st);
+  if (FT == 32) dispatch_kernel<1><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles);
+  else          dispatch_kernel<2><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles);
+  fs_tm_end(tm, FS_T_DISPATCH, st);
+  return 1;
 }

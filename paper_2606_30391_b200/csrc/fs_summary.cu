@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
   if (lane == 0) {
     FsGpuInfo gi;
     gi.t_avail_ms = g.t_avail_ms; gi.mem_free_mb = g.mem_free_mb;
-    gi.n_res = n; gi.f_floor = f_floor; gi._pad[0] = gi._pad[1] = 0;
+    gi.n_res = n; gi.f_floor = f_floor; gi.f_cur = n ? g.f_cur : 0; gi._pad = 0;
     int used = 0; float ecur = 0.0f;
     for (int i = 0; i < FS_RMAX; ++i) {
       if (i < n) {

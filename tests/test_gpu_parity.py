@@ -335,3 +335,64 @@ def test_batch_tasks_pod_size(ctx):
     off, tasks = synth.make_tasks(2, cl.K, cl.M, cl.S, cl.B, 10, 100)
     ctx.load_cluster(cl)
     cmp.assert_tasks_equal(ctx.batch_tasks(off, tasks), _oracle_tasks(cl, off, tasks))
+
+
+# ---- the paper's three-phase dispatcher (fs_dispatch) ------------------------------------------
+def _oracle_dispatch(cl, reqs=None):
+    return oracle.dispatch(cl.lat, cl.pow, cl.models, cl.states, cl.requests if reqs is None else reqs, 8)
+
+
+def _mix_phases(cl, seed):
+    """Push part of the requests into phase 2 (F_max retry), phase 3 (scale-out) and 'infeasible'."""
+    u = synth.Stream(seed, "phases").uniform(cl.R)
+    cl.requests["slo_ttft_ms"] = np.where(u < 0.3, cl.requests["slo_ttft_ms"] * 0.03, cl.requests["slo_ttft_ms"]).astype(np.float32)
+    cl.requests["o_pred"] = np.where((u > 0.3) & (u < 0.4), 2 ** 20, cl.requests["o_pred"]).astype(np.uint32)   # fits no GPU's memory
+    cl.requests["slo_tbt_ms"] = np.where(u > 0.95, 1e-3, cl.requests["slo_tbt_ms"]).astype(np.float32)
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_dispatch_ragged_dims_all_phases(ctx, seed):
+    st = synth.Stream(seed, "ddims")
+    K = int(st.randint(1, 1, 90)[0]); M = int(st.randint(1, 1, 9)[0])
+    F = int(st.randint(1, 1, [64, 100][seed % 2])[0]); S = int(st.randint(1, 1, 20)[0]); B = int(st.randint(1, 1, 40)[0])
+    cl = synth.make_custom(seed=1000 + seed, K=K, M=M, F=F, S=S, B=B, R=150, lo=1, hi=4)
+    _mix_phases(cl, seed)
+    if seed % 3 == 0:                                 # equal free memory everywhere: the SM_free / index tie-breakers
+        cl.states["mem_free_mb"] = 30000.0
+    ctx.load_cluster(cl)
+    got = ctx.dispatch(cl.requests)
+    cmp.assert_placement_equal(got, _oracle_dispatch(cl))
+
+
+def test_dispatch_fig6(ctx):
+    """Fig. 6 through the CUDA path: timestamps 150 / 180 / 210 against the SLO of 200, 45 J vs 30 J."""
+    from test_oracle_dispatch import _toy, _gpu
+    lat, pw, models, st, rq = _toy(K=3)
+    for k, (t_avail, l, p) in enumerate([(100.0, 50.0, 900.0), (120.0, 60.0, 500.0), (150.0, 60.0, 100.0)]):
+        _gpu(st, k, 1, 2, k, t_avail, 1e6)
+        lat[0, 0, k, 1, 0] = l; pw[0, 0, k, 1, 0] = p
+    ctx.load_profiles(lat, pw, np.ones(3, np.float32), models, synth.Params())
+    ctx.set_gpu_state(st)
+    o = ctx.dispatch(rq)[0]
+    assert (o["gpu"], o["phi"], o["f_req"]) == (1, 1, 1) and o["energy_mj"] == np.float32(30000.0)
+
+
+def test_dispatch_tie_heavy(ctx):
+    cl = U.tie_heavy(synth.make_custom(seed=1020, K=40, M=3, F=12, S=6, B=5, R=96), 3)
+    cl.states["mem_free_mb"] = np.round(cl.states["mem_free_mb"] / 10000.0) * 10000.0
+    ctx.load_cluster(cl)
+    cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
+
+
+def test_dispatch_full_size(ctx):
+    """rack in full; pod at full size with a sample of requests recomputed by the oracle."""
+    cl = synth.make_cluster("rack")
+    ctx.load_cluster(cl)
+    cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
+    cl = synth.make_cluster("pod")
+    _mix_phases(cl, 5)
+    ctx.load_cluster(cl)
+    got = ctx.dispatch(cl.requests)
+    idx = np.unique(synth.Stream(11, "sample").randint(2048, 0, cl.R - 1))
+    cmp.assert_placement_equal(got[idx], _oracle_dispatch(cl, cl.requests[idx]))
+    assert set(np.unique(got["f_req"]).tolist()) >= {1, 2, 3}
