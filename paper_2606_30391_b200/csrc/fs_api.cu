@@ -369,7 +369,7 @@ int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out,
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
-  c->launches += fsk_dispatch(view_of(c), R, d_reqs, d_out, st, c->timing ? &c->tm : nullptr);
+  c->launches += fsk_dispatch(view_of(c), R, d_reqs, d_out, c->warm_off, c->warm_item, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));

@@ -44,7 +44,7 @@ static_assert(sizeof(FsGpuInfo) == 48, "FsGpuInfo layout");
 // Compact per-GPU record the dense placement kernel stages with TMA (32 bytes).
 struct __align__(16) FsGpuRec {
   float t_avail_ms, mem_free_mb, e_cur;
-  uint32_t meta;            // n_res | sm_free << 8   (n_res == 0: never a candidate)
+  uint32_t meta;            // n_res | sm_free << 8 | F_curr << 16   (n_res == 0: never a candidate)
   int16_t model[FS_RMAX];
   float a_min;              // min over phi of A0[k][phi] (+INF: co-residents never feasible)
   uint32_t k;               // GPU index (the sorted copy is not in index order)

@@ -531,6 +531,7 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
 // reads the planes.  Lanes <-> GPUs; reductions by redux / 64-bit key shuffles.
 // =============================================================================================
 constexpr int DISP_WARPS = 8;
+constexpr int DISP_NC = 4;                    // chunk minima kept per lane: GPUs beyond 32*32*DISP_NC are always revisited
 
 struct OwnEval { bool ok; float e, ttft, tbt; };
 
@@ -550,27 +551,50 @@ __device__ __forceinline__ OwnEval own_eval_planes(const FsView& v, const ReqCtx
 }
 
 struct DispPair { bool ok; float e; };
-// pair (request, GPU gi) at frequency phi: cold pairs from the tiles, warm pairs from the planes
-__device__ __forceinline__ DispPair disp_pair(const FsView& v, const ReqCtx& c, const PairCtx& p, int phi,
+// pair (request, GPU k with compact record g) at frequency phi (< 0: the GPU's F_curr).  Cold pairs
+// (model not resident: two packed 16-bit compares) read the tiles; warm pairs and the no-tile case
+// go through the full summary, make_pair and the planes.
+__device__ __forceinline__ DispPair disp_pair(const FsView& v, const ReqCtx& c, const FsGpuRec& g, int k, int phi,
                                               const float* tl_t0, const float* tl_er, int FT) {
   DispPair r; r.ok = false; r.e = FS_INF;
-  if (!p.ok) return r;
-  const int sg = p.smf - 1;
-  if (p.j < 0 && tl_t0) {
-    const float t0 = tl_t0[sg * FT + phi];
-    r.e = tl_er[sg * FT + phi];
-    r.ok = (c.L == 0 || __fadd_rn(p.wait, t0) <= c.slo_ttft) && r.e < FS_INF;
-  } else {
-    const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, sg, phi);
-    r.ok = ev.ok; r.e = ev.e;
+  const int n_res = g.meta & 0xFF, smf = (g.meta >> 8) & 0xFF;
+  if (phi < 0) phi = (g.meta >> 16) & 0xFFFF;
+  if (n_res < 1 || smf < 1 || !(c.mem <= g.mem_free_mb)) return r;
+  const uint32_t mm = (uint32_t)c.m * 0x00010001u;
+  const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
+  if (tl_t0) {
+    // resident model: a WARM pair, scored from the per-model list instead (a rare lane would make
+    // the whole warp take the slow path in almost every chunk)
+    if ((__vcmpeq2(gm[0], mm) | __vcmpeq2(gm[1], mm)) || n_res >= FS_RMAX) return r;
+    const int o = (smf - 1) * FT + phi;
+    r.e = tl_er[o];
+    r.ok = (c.L == 0 || __fadd_rn(__fadd_rn(g.t_avail_ms, c.load_ms), tl_t0[o]) <= c.slo_ttft) && r.e < FS_INF;
+    return r;
   }
+  const PairCtx p = make_pair(v, c, v.ginfo[k]);
+  if (!p.ok) return r;
+  const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, p.smf - 1, phi);
+  r.ok = ev.ok; r.e = ev.e;
+  return r;
+}
+
+// warm pair from the per-model list (phi < 0: the GPU's F_curr)
+__device__ __forceinline__ DispPair disp_warm(const FsView& v, const ReqCtx& c, const FsWarmItem& it, int phi) {
+  DispPair r; r.ok = false; r.e = FS_INF;
+  const FsGpuInfo gi = v.ginfo[it.k];
+  const PairCtx p = make_pair(v, c, gi);
+  if (!p.ok) return r;
+  const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, p.smf - 1, phi < 0 ? gi.f_cur : phi);
+  r.ok = ev.ok; r.e = ev.e;
   return r;
 }
 
 template <int NPHI>
 __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int R,
                                                                   const fs_request* __restrict__ reqs,
-                                                                  fs_placement* __restrict__ out, int use_tiles) {
+                                                                  fs_placement* __restrict__ out, int use_tiles,
+                                                                  const int32_t* __restrict__ warm_off,
+                                                                  const FsWarmItem* __restrict__ witems) {
   extern __shared__ __align__(16) unsigned char disp_smem[];
   constexpr int FT = 32 * NPHI;
   const FsDimsDev d = v.d;
@@ -612,30 +636,65 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
     __syncwarp();
   }
   // ---- Phase 1 + 2 at F_curr: E_min, then the 2 % band with the stability tie-breaker ----------
-  uint32_t emin_o = 0xFFFFFFFFu;
-  for (int base = 0; base < v.K; base += 32) {
-    const int k = base + lane;
-    if (k < v.K) {
-      const FsGpuInfo gi = v.ginfo[k];
-      const DispPair dp = disp_pair(v, c, make_pair(v, c, gi), gi.f_cur, tl_t0, tl_er, FT);
-      if (dp.ok) emin_o = min(emin_o, fs_orderable(dp.e));
-    }
+  // lane c keeps the minimum of chunk c (32 GPUs), c < 32*DISP_NC, so that the band scan only
+  // revisits chunks that hold a candidate inside the band
+  uint32_t emin_o = 0xFFFFFFFFu, cmin[DISP_NC];
+#pragma unroll
+  for (int u = 0; u < DISP_NC; ++u) cmin[u] = 0xFFFFFFFFu;
+  // grec is padded to a multiple of 32 records (n_res = 0); the next chunk's records are in flight
+  // while this one is scored
+  FsGpuRec nxt = v.grec[lane];
+  for (int base = 0; base < v.Kpad; base += 32) {
+    const FsGpuRec g = nxt;
+    if (base + 32 < v.Kpad) nxt = v.grec[base + 32 + lane];
+    uint32_t eo = 0xFFFFFFFFu;
+    const DispPair dp = disp_pair(v, c, g, base + lane, -1, tl_t0, tl_er, FT);
+    if (dp.ok) eo = fs_orderable(dp.e);
+    const uint32_t cm = warp_min_u32(eo);
+    const int ch = base >> 5;
+#pragma unroll
+    for (int u = 0; u < DISP_NC; ++u) if ((ch >> 5) == u && (ch & 31) == lane) cmin[u] = cm;
+    emin_o = min(emin_o, cm);
   }
-  emin_o = warp_min_u32(emin_o);
+  const int wb0 = use_tiles ? warm_off[c.m] : 0, wb1 = use_tiles ? warm_off[c.m + 1] : 0;
+  for (int ib = wb0; ib < wb1; ib += 32) {
+    uint32_t eo = 0xFFFFFFFFu;
+    if (ib + lane < wb1) {
+      const DispPair dp = disp_warm(v, c, witems[ib + lane], -1);
+      if (dp.ok) eo = fs_orderable(dp.e);
+    }
+    emin_o = min(emin_o, warp_min_u32(eo));
+  }
   int phase = -1, kbest = -1, phibest = -1;
   if (emin_o != 0xFFFFFFFFu) {
     const float band = __fmul_rn(1.02f, fs_unorderable(emin_o));
+    const uint32_t band_o = fs_orderable(band);
     unsigned long long key = FS_KEY_NONE;              // (most memory, largest SM_free, lowest k)
-    for (int base = 0; base < v.K; base += 32) {
+    for (int base = 0; base < v.Kpad; base += 32) {
+      const int ch = base >> 5;
+      if (ch < 32 * DISP_NC) {
+        uint32_t cm = 0xFFFFFFFFu;
+#pragma unroll
+        for (int u = 0; u < DISP_NC; ++u) if ((ch >> 5) == u) cm = cmin[u];
+        cm = __shfl_sync(0xffffffffu, cm, ch & 31);
+        if (cm > band_o) continue;                     // no candidate of this chunk is inside the band
+      }
       const int k = base + lane;
-      if (k < v.K) {
-        const FsGpuInfo gi = v.ginfo[k];
-        const DispPair dp = disp_pair(v, c, make_pair(v, c, gi), gi.f_cur, tl_t0, tl_er, FT);
-        if (dp.ok && dp.e <= band) {
-          const unsigned long long kk = ((unsigned long long)(~fs_orderable(gi.mem_free_mb)) << 32) |
-                                        ((unsigned long long)(uint32_t)(d.S - gi.sm_free) << 24) | (uint32_t)k;
-          key = kk < key ? kk : key;
-        }
+      const FsGpuRec g = v.grec[k];
+      const DispPair dp = disp_pair(v, c, g, k, -1, tl_t0, tl_er, FT);
+      if (dp.ok && dp.e <= band) {
+        const unsigned long long kk = ((unsigned long long)(~fs_orderable(g.mem_free_mb)) << 32) |
+                                      ((unsigned long long)(uint32_t)(d.S - (int)((g.meta >> 8) & 0xFF)) << 24) | (uint32_t)k;
+        key = kk < key ? kk : key;
+      }
+    }
+    for (int ib = wb0 + lane; ib < wb1; ib += 32) {
+      const FsWarmItem it = witems[ib];
+      const DispPair dp = disp_warm(v, c, it, -1);
+      if (dp.ok && dp.e <= band) {
+        const unsigned long long kk = ((unsigned long long)(~fs_orderable(it.mem_free_mb)) << 32) |
+                                      ((unsigned long long)(uint32_t)(d.S - it.sm_free) << 24) | (uint32_t)it.k;
+        key = kk < key ? kk : key;
       }
     }
     key = fs_warp_min_key(key);
@@ -644,15 +703,21 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
   } else {
     // ---- Phase 3: F_max retry, first feasible GPU in T_avail order ------------------------------
     unsigned long long key = FS_KEY_NONE;
-    for (int base = 0; base < v.K; base += 32) {
+    for (int base = 0; base < v.Kpad; base += 32) {
       const int k = base + lane;
-      if (k < v.K) {
-        const FsGpuInfo gi = v.ginfo[k];
-        const DispPair dp = disp_pair(v, c, make_pair(v, c, gi), d.F - 1, tl_t0, tl_er, FT);
-        if (dp.ok) {
-          const unsigned long long kk = ((unsigned long long)fs_orderable(gi.t_avail_ms) << 32) | (uint32_t)k;
-          key = kk < key ? kk : key;
-        }
+      const FsGpuRec g = v.grec[k];
+      const DispPair dp = disp_pair(v, c, g, k, d.F - 1, tl_t0, tl_er, FT);
+      if (dp.ok) {
+        const unsigned long long kk = ((unsigned long long)fs_orderable(g.t_avail_ms) << 32) | (uint32_t)k;
+        key = kk < key ? kk : key;
+      }
+    }
+    for (int ib = wb0 + lane; ib < wb1; ib += 32) {
+      const FsWarmItem it = witems[ib];
+      const DispPair dp = disp_warm(v, c, it, d.F - 1);
+      if (dp.ok) {
+        const unsigned long long kk = ((unsigned long long)fs_orderable(it.t_avail_ms) << 32) | (uint32_t)it.k;
+        key = kk < key ? kk : key;
       }
     }
     key = fs_warp_min_key(key);
@@ -761,14 +826,15 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
   return launches;
 }
 
-int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* out, cudaStream_t st, FsTimers* tm) {
+int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* out, const int32_t* warm_off,
+                 const FsWarmItem* witems, cudaStream_t st, FsTimers* tm) {
   if (R <= 0) return 0;
   const int use_tiles = v.d.F <= 64;
   const int FT = v.d.F <= 32 ? 32 : 64;
   const size_t smem = use_tiles ? (size_t)DISP_WARPS * 2 * v.d.S * FT * sizeof(float) : 0;
   fs_tm_beg(tm, FS_T_DISPATCH, st);
-  if (FT == 32) dispatch_kernel<1><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles);
-  else          dispatch_kernel<2><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles);
+  if (FT == 32) dispatch_kernel<1><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
+  else          dispatch_kernel<2><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
   fs_tm_end(tm, FS_T_DISPATCH, st);
   return 1;
 }

@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     gi.e_cur = ecur; gi.sm_free = n ? d.S - used : 0;
     ginfo[k] = gi;
     FsGpuRec r; r.t_avail_ms = gi.t_avail_ms; r.mem_free_mb = gi.mem_free_mb; r.e_cur = ecur;
-    r.meta = (uint32_t)n | ((uint32_t)gi.sm_free << 8);
+    r.meta = (uint32_t)n | ((uint32_t)gi.sm_free << 8) | ((uint32_t)gi.f_cur << 16);
     for (int i = 0; i < FS_RMAX; ++i) r.model[i] = gi.model[i];
     r.a_min = a_min; r.k = (uint32_t)k;
     grec[k] = r;
