@@ -222,7 +222,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (K > c->k_cap) {
     FS_TRY(grow(c, c->states, (size_t)K)); FS_TRY(grow(c, c->ginfo, (size_t)K));
     FS_TRY(grow(c, c->grec, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->gsort, (size_t)K + FS_CHUNK));
-    FS_TRY(grow(c, c->dsort, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->dsuf, (size_t)K / FS_CHUNK + 4 + ((size_t)K + FS_CHUNK) / 2 + 1));
+    FS_TRY(grow(c, c->dsort, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->dsuf, (size_t)K / FS_CHUNK + 8 + ((size_t)K + FS_CHUNK) / 2 + 1));
     FS_TRY(grow(c, c->ctr, (size_t)K / FS_CHUNK + 2));
     FS_TRY(grow(c, c->warm_item, (size_t)K * FS_RMAX));
     c->k_cap = K; c->consol_cap = 0;

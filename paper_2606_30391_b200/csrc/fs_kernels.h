@@ -33,7 +33,7 @@ struct FsView {
                             //                  padding = INF (what the dense kernel stages by TMA)
   int Kpad, FT;
   const FsGpuRec* gsort;    // [Kpad]           grec in the dense kernel's scan order (fs_summary.cu)
-  const double* dsuf;       // [Kpad/32 + 2]    [0] magnitude bound, [1+c] suffix minimum of d from chunk c on
+  const double* dsuf;       // [Kpad/32 + 3]    [0] magnitude bound, [1+c] suffix minimum of d from chunk c on, [last] earliest T_avail
   int* flag;                // sticky range-error flag (mapped host memory)
 };
 

@@ -281,6 +281,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
 
   const double* dsuf = v.dsuf + 1 + c0;
   const double amax = v.dsuf[0];
+  const float tmin = (float)v.dsuf[2 + nchunk_all];
   // work counters (warp-uniform except n_elig / n_witems, which are per lane)
   uint32_t n_chunks = 0, n_elig = 0, n_swept = 0, n_cswept = 0, n_witems = 0, n_scored = 0, n_cscored = 0, n_req = 0;
   const bool vec = NPHI == 2 && (d.F & 1) == 0;
@@ -334,72 +335,9 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       }
       __syncwarp();
     }
-    // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scan is not in index order
+    // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scans are not in index order
     float best = FS_INF; int bestk = KNONE;
-    // ---- (b) cold pairs: GPUs in ascending d = a_min - Ecur.  Every candidate of every GPU from
-    // chunk ci on has  dE >= fl(fl(a + b) - e)  with  a - e >= dsuf[ci],  b >= bmin,  a <= amax,
-    // and two roundings lose at most 2^-23 (a + b + |a + b - e|); the scan stops as soon as that
-    // (with twice the slack) exceeds the incumbent, strictly, so ties still meet every GPU.
-    const float bminf = bnd[d.S - 1];
-    const double bmin = (double)bminf;
-    for (int ci = 0; ci < nchunk && bminf < FS_INF; ++ci) {
-      const float bestW = fs_unorderable(warp_min_u32(fs_orderable(best)));
-      const double ds = dsuf[ci];
-      if (!(ds < (double)FS_INF)) break;                 // sentinels only from here on
-      if (bestW < FS_INF) {
-        const double x = ds + bmin;
-        if (x - 0x1p-22 * (amax + bmin + fabs(x)) - 1e-37 > (double)bestW) break;
-      }
-      if (STATS) { n_chunks += 1; }
-      // ---- eligibility + bound: lane <-> one GPU of the chunk ---------------------------------
-      const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
-      const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
-      const uint32_t mm = (uint32_t)c.m * 0x00010001u;
-      const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
-      const bool el = (c.mem <= g.mem_free_mb) && !(__vcmpeq2(gm[0], mm) | __vcmpeq2(gm[1], mm));
-      float T = -1.0f;
-      if (el) {
-        if (STATS) { n_elig += 1; }
-        // prune: no candidate of this GPU can beat or tie the best found so far
-        const float lb = __fsub_rn(__fadd_rn(g.a_min, bnd[smf - 1]), g.e_cur);
-        if (lb <= bestW && lb < FS_INF) {
-          const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
-          if (c.L == 0) T = FS_INF;
-          else if (__fadd_rn(wait, bnd[DENSE_S + smf - 1]) <= c.slo_ttft) T = fs_tstar(wait, c.slo_ttft);
-        }
-      }
-      // compact the surviving GPUs of the chunk into the warp's list: {T*, Ecur, sm_free, GPU}
-      const bool go = T >= 0.0f;
-      const unsigned mask = __ballot_sync(0xffffffffu, go);
-      if (mask == 0u) continue;
-      __syncwarp();
-      if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
-          make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((int)g.k));
-      __syncwarp();
-      const int n_el = __popc(mask);
-      // ---- sweep the survivors: per candidate one compare and one predicated min ---------------
-      for (int e = 0; e < n_el; ++e) {
-        const float4 w = wb[e];
-        const float Tst = w.x; const int sfree = __float_as_int(w.z); const int k = __float_as_int(w.w);
-        if (STATS) { n_swept += 1; n_cswept += (uint32_t)(sfree * d.F); }
-        float arow[NPHI], m[NPHI];
-        ld_cols<NPHI>(v.gA0 + (size_t)k * FT, 0, phi0, FT, true, arow);   // rows are FT-padded: aligned
-#pragma unroll
-        for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
-#pragma unroll 4
-        for (int s = 0; s < sfree; ++s) {
-          float tt[NPHI], ee[NPHI];
-          ld_tile<NPHI>(tl_t0 + s * FT + phi0, tt); ld_tile<NPHI>(tl_er + s * FT + phi0, ee);
-#pragma unroll
-          for (int i = 0; i < NPHI; ++i) m[i] = tt[i] <= Tst ? fminf(m[i], ee[i]) : m[i];
-        }
-        float x = FS_INF;
-#pragma unroll
-        for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
-        const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
-        if (dE < best || (dE == best && k < bestk)) { best = dE; bestk = k; }
-      }
-    }
+    uint32_t bflat = NONE32;   // flat index of the lane's incumbent when the definition body found it (warm pairs)
     // ---- (c), (d) the definition, pair by pair, from the t0 tile and the planes: first the WARM
     // pairs (GPUs that already host model m), best bound first, then once more on the winning GPU
     // to recover the lowest flat index attaining the minimum.  One code site serves both.
@@ -419,8 +357,82 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           break;
         }
         if (ib >= ie) {                                 // no item left that could beat the incumbent
+          // the cold scan comes AFTER the warm pairs: a cold start often cannot meet the TTFT deadline
+          // at all (load_ms against the SLO), and then only a warm incumbent lets the scan stop early
+          // ---- (b) cold pairs: GPUs in ascending d = a_min - Ecur.  Every candidate of every GPU from
+          // chunk ci on has  dE >= fl(fl(a + b) - e)  with  a - e >= dsuf[ci],  b >= bmin,  a <= amax,
+          // and two roundings lose at most 2^-23 (a + b + |a + b - e|); the scan stops as soon as that
+          // (with twice the slack) exceeds the incumbent, strictly, so ties still meet every GPU.
+          // No cold pair at all can meet the TTFT deadline if even the earliest T_avail plus the weight
+          // load plus the fastest prefill misses it (monotone rounding): then there is nothing to scan.
+          const float bminf = bnd[d.S - 1];
+          const double bmin = (double)bminf;
+          const bool cold_possible = bminf < FS_INF &&
+              (c.L == 0 || __fadd_rn(__fadd_rn(tmin, c.load_ms), bnd[DENSE_S + d.S - 1]) <= c.slo_ttft);
+          for (int ci = 0; ci < nchunk && cold_possible; ++ci) {
+            const float bestW = fs_unorderable(warp_min_u32(fs_orderable(best)));
+            const double ds = dsuf[ci];
+            if (!(ds < (double)FS_INF)) break;                 // sentinels only from here on
+            if (bestW < FS_INF) {
+              const double x = ds + bmin;
+              if (x - 0x1p-22 * (amax + bmin + fabs(x)) - 1e-37 > (double)bestW) break;
+            }
+            if (STATS) { n_chunks += 1; }
+            // ---- eligibility + bound: lane <-> one GPU of the chunk ---------------------------------
+            const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
+            const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
+            const uint32_t mm = (uint32_t)c.m * 0x00010001u;
+            const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
+            const bool el = (c.mem <= g.mem_free_mb) && !(__vcmpeq2(gm[0], mm) | __vcmpeq2(gm[1], mm));
+            float T = -1.0f;
+            if (el) {
+              if (STATS) { n_elig += 1; }
+              // prune: no candidate of this GPU can beat or tie the best found so far
+              const float lb = __fsub_rn(__fadd_rn(g.a_min, bnd[smf - 1]), g.e_cur);
+              if (lb <= bestW && lb < FS_INF) {
+                const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
+                if (c.L == 0) T = FS_INF;
+                else if (__fadd_rn(wait, bnd[DENSE_S + smf - 1]) <= c.slo_ttft) T = fs_tstar(wait, c.slo_ttft);
+              }
+            }
+            // compact the surviving GPUs of the chunk into the warp's list: {T*, Ecur, sm_free, GPU}
+            const bool go = T >= 0.0f;
+            const unsigned mask = __ballot_sync(0xffffffffu, go);
+            if (mask == 0u) continue;
+            __syncwarp();
+            if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
+                make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((int)g.k));
+            __syncwarp();
+            const int n_el = __popc(mask);
+            // ---- sweep the survivors: per candidate one compare and one predicated min ---------------
+            for (int e = 0; e < n_el; ++e) {
+              const float4 w = wb[e];
+              const float Tst = w.x; const int sfree = __float_as_int(w.z); const int k = __float_as_int(w.w);
+              if (STATS) { n_swept += 1; n_cswept += (uint32_t)(sfree * d.F); }
+              float arow[NPHI], m[NPHI];
+              ld_cols<NPHI>(v.gA0 + (size_t)k * FT, 0, phi0, FT, true, arow);   // rows are FT-padded: aligned
+      #pragma unroll
+              for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
+      #pragma unroll 4
+              for (int s = 0; s < sfree; ++s) {
+                float tt[NPHI], ee[NPHI];
+                ld_tile<NPHI>(tl_t0 + s * FT + phi0, tt); ld_tile<NPHI>(tl_er + s * FT + phi0, ee);
+      #pragma unroll
+                for (int i = 0; i < NPHI; ++i) m[i] = tt[i] <= Tst ? fminf(m[i], ee[i]) : m[i];
+              }
+              float x = FS_INF;
+      #pragma unroll
+              for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
+              const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
+              if (dE < best || (dE == best && k < bestk)) { best = dE; bestk = k; bflat = NONE32; }
+            }
+          }
           const unsigned long long kk = fs_warp_min_key(((unsigned long long)fs_orderable(best) << 32) | (uint32_t)bestk);
           recover = true; k = (int)(uint32_t)kk; bestW = fs_unorderable((uint32_t)(kk >> 32));
+          // a warm winner was scored by the definition in flat order: its lanes already hold their
+          // lowest flat index, nothing to recover (a GPU is warm or cold for a request, never both)
+          if (k != KNONE && best == bestW && bestk == k) flat = bflat;
+          if (__any_sync(0xffffffffu, flat != NONE32)) k = KNONE;
           break;
         }
         ordl = NONE32;                                  // next 32 items: lane <-> item
@@ -450,23 +462,34 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         float ar[NPHI];
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < d.F ? Ar[phi0 + i] : FS_INF;
+        // four share rows per trip: their 12 plane loads are issued before any of them is used
 #pragma unroll 1
-        for (int s = 0; s < p.smf; ++s) {
-          float tt[NPHI], b0[NPHI], a1[NPHI], b1[NPHI];
-          ld_tile<NPHI>(tl_t0 + s * FT + phi0, tt);
-          ld_cols<NPHI>(pw0, s * d.F, phi0, d.F, vec, b0);
-          ld_cols<NPHI>(l1, s * d.F, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, s * d.F, phi0, d.F, vec, b1);
+        for (int s4 = 0; s4 < p.smf; s4 += 4) {
+          float tt[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
 #pragma unroll
-          for (int i = 0; i < NPHI; ++i) {
-            const float e0 = __fmul_rn(tt[i], b0[i]);
-            const float e1 = __fmul_rn(__fmul_rn(fr1, a1[i]), b1[i]);
-            float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);
-            if (dE == 0.0f) dE = 0.0f;
-            const bool ok = (c.L == 0 || __fadd_rn(p.wait, tt[i]) <= c.slo_ttft) &&
-                            (c.O == 0 || a1[i] <= c.slo_tbt) && dE < FS_INF;
-            if (recover) {
-              if (ok && dE == bestW && flat == NONE32) flat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
-            } else if (ok && (dE < best || (dE == best && k < bestk))) { best = dE; bestk = k; }
+          for (int u = 0; u < 4; ++u) {
+            const int sr = min(s4 + u, p.smf - 1);
+            ld_cols<NPHI>(pw0, sr * d.F, phi0, d.F, vec, b0[u]);
+            ld_cols<NPHI>(l1, sr * d.F, phi0, d.F, vec, a1[u]); ld_cols<NPHI>(p1, sr * d.F, phi0, d.F, vec, b1[u]);
+            ld_tile<NPHI>(tl_t0 + sr * FT + phi0, tt[u]);
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int s = s4 + u;
+#pragma unroll
+            for (int i = 0; i < NPHI; ++i) {
+              const float e0 = __fmul_rn(tt[u][i], b0[u][i]);
+              const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
+              float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);
+              if (dE == 0.0f) dE = 0.0f;
+              const bool ok = s < p.smf && (c.L == 0 || __fadd_rn(p.wait, tt[u][i]) <= c.slo_ttft) &&
+                              (c.O == 0 || a1[u][i] <= c.slo_tbt) && dE < FS_INF;
+              if (recover) {
+                if (ok && dE == bestW && flat == NONE32) flat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
+              } else if (ok && (dE < best || (dE == best && k < bestk))) {
+                best = dE; bestk = k; bflat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
+              }
+            }
           }
           if (recover && __any_sync(0xffffffffu, flat != NONE32)) break;   // flat order is sigma-major
         }

@@ -178,18 +178,22 @@ __global__ void __launch_bounds__(128) order_rank_kernel(const FsGpuRec* __restr
   gsort[rank] = mine; dsort[rank] = dd;
 }
 // dsuf[0] = max over the capable GPUs of max(a_min, |Ecur|) (INF if any is huge: no early stop);
-// dsuf[1+c] = min of d over sorted positions >= 32*c   (exact suffix minimum, in double)
+// dsuf[1+c] = min of d over sorted positions >= 32*c   (exact suffix minimum, in double);
+// dsuf[2+nchunk] = the earliest T_avail among the capable GPUs
 __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __restrict__ gsort,
                                                            const double* __restrict__ dsort, int nchunk,
                                                            double* __restrict__ dsuf) {
   __shared__ double seg[1024];
-  __shared__ float smax[32];
+  __shared__ float smax[32], smin[32];
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-  float amax = 0.0f;
+  float amax = 0.0f, tmin = FS_INF;
   for (int c = warp; c < nchunk; c += 32) {            // warp <-> chunk, lane <-> record
     const int pos = c * FS_CHUNK + lane;
     double m = dsort[pos];
-    if (m < (double)FS_INF) amax = fmaxf(amax, fmaxf(gsort[pos].a_min, fabsf(gsort[pos].e_cur)));
+    if (m < (double)FS_INF) {
+      amax = fmaxf(amax, fmaxf(gsort[pos].a_min, fabsf(gsort[pos].e_cur)));
+      tmin = fminf(tmin, gsort[pos].t_avail_ms);
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { const double u = __shfl_xor_sync(0xffffffffu, m, o); m = u < m ? u : m; }
     if (lane == 0) dsuf[1 + c] = m;
@@ -209,13 +213,17 @@ __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __re
     dsuf[1 + c] = carry;
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-  if (lane == 0) smax[warp] = amax;
+  for (int o = 16; o > 0; o >>= 1) {
+    amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    tmin = fminf(tmin, __shfl_xor_sync(0xffffffffu, tmin, o));
+  }
+  if (lane == 0) { smax[warp] = amax; smin[warp] = tmin; }
   __syncthreads();
   if (t == 0) {
-    for (int w = 1; w < 32; ++w) amax = fmaxf(amax, smax[w]);
+    for (int w = 1; w < 32; ++w) { amax = fmaxf(amax, smax[w]); tmin = fminf(tmin, smin[w]); }
     dsuf[0] = amax <= 1e37f ? (double)amax : (double)FS_INF;
     dsuf[1 + nchunk] = (double)FS_INF;
+    dsuf[2 + nchunk] = (double)tmin;                   // earliest T_avail of a cold-capable GPU (NaN-free: min)
   }
 }
 
@@ -275,7 +283,7 @@ int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, fl
   const int wpb = 4;
   fs_tm_beg(tm, FS_T_SUMMARY, st);
   summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0);
-  float* okey = reinterpret_cast<float*>(dsuf + v.Kpad / FS_CHUNK + 2);   // scratch behind dsuf
+  float* okey = reinterpret_cast<float*>(dsuf + v.Kpad / FS_CHUNK + 4);   // scratch behind dsuf
   order_key_kernel<<<(v.Kpad + 255) / 256, 256, 0, st>>>(grec, v.Kpad, okey);
   order_rank_kernel<<<(v.Kpad + 127) / 128, 128, 0, st>>>(grec, okey, v.Kpad, gsort, dsort);
   order_suffix_kernel<<<1, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf);
