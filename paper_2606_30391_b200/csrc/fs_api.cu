@@ -30,7 +30,7 @@ struct fs_ctx {
   unsigned int* ctr = nullptr;
   fs_request* reqs_dev = nullptr; fs_placement* place_dev = nullptr;
   // local scratch
-  size_t local_cap = 0; int n_cap = 0; float* G = nullptr; uint8_t* Bst = nullptr;
+  size_t local_cap = 0; int n_cap = 0; float* G = nullptr;
   int32_t* ids_dev = nullptr; fs_local_cfg* local_dev = nullptr;
   int32_t *bin_off = nullptr, *bin_cursor = nullptr, *keylist = nullptr, *nkeys = nullptr; int bin_m_cap = 0;
   uint4* lslots = nullptr;
@@ -156,7 +156,7 @@ int fs_destroy(fs_ctx* c) {
   cudaDeviceSynchronize();
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
-                  c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->Bst, c->ids_dev, c->local_dev, c->need, c->E,
+                  c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (c->flag_host) cudaFreeHost(c->flag_host);
@@ -291,7 +291,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
   if (n == 0) return pending;
   const size_t rows = (size_t)c->d.F * c->d.S;
   const size_t need = (size_t)n * FS_RMAX * 2 * rows;
-  if (need > c->local_cap) { FS_TRY(grow(c, c->G, need)); FS_TRY(grow(c, c->Bst, need)); c->local_cap = need; }
+  if (need > c->local_cap) { FS_TRY(grow(c, c->G, need)); c->local_cap = need; }
   if (n > c->n_cap) {
     FS_TRY(grow(c, c->ids_dev, (size_t)n)); FS_TRY(grow(c, c->local_dev, (size_t)n));
     FS_TRY(grow(c, c->lslots, (size_t)n * FS_RMAX * 2));
@@ -310,7 +310,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
     }
     d_out = c->local_dev;
   }
-  FsLocalScratch sc{c->G, c->Bst, c->comp, c->comp_n, c->ns_stride, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots};
+  FsLocalScratch sc{c->G, c->comp, c->comp_n, c->ns_stride, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots};
   c->launches += fsk_local(view_of(c), n, d_ids, flags, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {

@@ -71,7 +71,6 @@ int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* 
 // fs_local.cu — per-slot batch search + SM-split search
 struct FsLocalScratch {
   float* G;               // [n][RMAX*2][F*S]  slot cost g_{i,p}[phi][sigma]
-  uint8_t* B;             // [n][RMAX*2][F*S]  best batch bucket beta* per slot row
   const uint32_t* comp;   // [RMAX][ns_stride] SM splits in lexicographic order, sigma_i in byte i
   const uint32_t* comp_n; // [RMAX] number of splits NS = C(S-1, n_res-1)
   int ns_stride;

@@ -17,14 +17,12 @@ namespace {
 // grid = (n GPUs, RMAX*2 slots); rows strided over the block's warps.
 __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
                                                         const int32_t* __restrict__ gpu_ids,
-                                                        uint32_t flags, float* __restrict__ Gs,
-                                                        uint8_t* __restrict__ Bs) {
+                                                        uint32_t flags, float* __restrict__ Gs) {
   const FsDimsDev d = v.d;
   const int gi = blockIdx.x, slot = blockIdx.y, i = slot >> 1, p = slot & 1;
   int k = gpu_ids ? gpu_ids[gi] : gi;
   const int rows = d.F * d.S;
   float* g_out = Gs + ((size_t)gi * (FS_RMAX * 2) + slot) * rows;
-  uint8_t* b_out = Bs + ((size_t)gi * (FS_RMAX * 2) + slot) * rows;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
   if (k < 0 || k >= v.K) return;                       // flagged by the split kernel
   const int n_res = v.ginfo[k].n_res;                  // 0 if the record was invalid
@@ -33,7 +31,7 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
   const uint32_t q = t.q[p];
   const bool obj_power = flags & FS_OBJ_POWER;
   if (q == 0) {
-    for (int row = threadIdx.x; row < rows; row += blockDim.x) { g_out[row] = 0.0f; b_out[row] = 0; }
+    for (int row = threadIdx.x; row < rows; row += blockDim.x) g_out[row] = 0.0f;
     return;
   }
   const float slo = t.slo_ms[p];
@@ -51,10 +49,7 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
       }
     }
     key = fs_warp_min_key(key);
-    if (lane == 0) {
-      g_out[row] = key == FS_KEY_NONE ? FS_INF : fs_unorderable((uint32_t)(key >> 32));
-      b_out[row] = key == FS_KEY_NONE ? 0 : (uint8_t)(uint32_t)key;
-    }
+    if (lane == 0) g_out[row] = key == FS_KEY_NONE ? FS_INF : fs_unorderable((uint32_t)(key >> 32));
   }
 }
 
@@ -111,8 +106,7 @@ __global__ void local_keys_kernel(const int32_t* __restrict__ off, int nkeys_all
 template <int P, bool OBJ_POWER>
 __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
     FsView v, const int32_t* __restrict__ off, const int32_t* __restrict__ keylist,
-    const int32_t* __restrict__ nkeys, const LocalSlot* __restrict__ slots, float* __restrict__ Gs,
-    uint8_t* __restrict__ Bs) {
+    const int32_t* __restrict__ nkeys, const LocalSlot* __restrict__ slots, float* __restrict__ Gs) {
   extern __shared__ __align__(128) unsigned char ls_smem[];
   __shared__ __align__(8) uint64_t bar;
   if ((int)blockIdx.x >= *nkeys) return;
@@ -144,9 +138,9 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
     const uint32_t nb = have ? (sl_.meta >> 8) : 0u;
     uint32_t maxnb;
     asm volatile("redux.sync.max.u32 %0, %1, 0xffffffff;" : "=r"(maxnb) : "r"(nb));
-    float best[LS_TR]; uint32_t bb[LS_TR];
+    float best[LS_TR];
 #pragma unroll
-    for (int r = 0; r < LS_TR; ++r) { best[r] = FS_INF; bb[r] = 0u; }
+    for (int r = 0; r < LS_TR; ++r) best[r] = FS_INF;
     for (uint32_t b4 = 0; b4 < maxnb; b4 += 4) {
       float4 L4[LS_TR], P4[LS_TR];
 #pragma unroll
@@ -167,7 +161,7 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
           const float t = __fmul_rn(fr, la);
           const bool ok = P == 0 ? (t <= sl_.slo) : (la <= sl_.slo);
           const float cost = OBJ_POWER ? pw : __fmul_rn(t, pw);
-          if (act && ok && cost < best[r]) { best[r] = cost; bb[r] = beta; }
+          if (act && ok) best[r] = fminf(best[r], cost);   // beta* is recovered for the chosen row only
         }
       }
     }
@@ -175,10 +169,9 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
       const size_t o = ((size_t)sl_.gi * (FS_RMAX * 2) + (sl_.meta & 0xFF)) * rows + r0;
       if (tr == LS_TR && (rows & 3) == 0) {
         *reinterpret_cast<float4*>(Gs + o) = make_float4(best[0], best[1], best[2], best[3]);
-        *reinterpret_cast<uint32_t*>(Bs + o) = bb[0] | (bb[1] << 8) | (bb[2] << 16) | (bb[3] << 24);
       } else {
 #pragma unroll
-        for (int r = 0; r < LS_TR; ++r) if (r < tr) { Gs[o + r] = best[r]; Bs[o + r] = (uint8_t)bb[r]; }
+        for (int r = 0; r < LS_TR; ++r) if (r < tr) Gs[o + r] = best[r];
       }
     }
   }
@@ -205,7 +198,6 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
                                                          const int32_t* __restrict__ gpu_ids,
                                                          uint32_t flags,
                                                          const float* __restrict__ Gs,
-                                                         const uint8_t* __restrict__ Bs,
                                                          const uint32_t* __restrict__ comp,   // [RMAX][NSmax] packed splits
                                                          const uint32_t* __restrict__ comp_n, // [RMAX] NS per n_res
                                                          int ns_stride,
@@ -313,18 +305,52 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
   }
   key = block_min_key(key, sred);
   fkey = block_min_key(fkey, sred);
+  // ---- outputs.  The slot kernels keep only the minimum cost per (slot, phi, sigma); the batch
+  // bucket beta* = lowest beta attaining it is recovered here, for the CHOSEN row of each slot only:
+  // warp <-> slot, lanes over beta, first feasible beta whose cost equals the stored minimum.
+  __shared__ int sbeta[FS_RMAX * 2];
+  uint32_t pk = 0; int phi = -1;
+  if (key != FS_KEY_NONE) {
+    const uint32_t flat = (uint32_t)key;
+    phi = minsm ? (int)flat : (int)(flat / NS);
+    if (minsm) {
+      for (int i = 0; i < n_res; ++i)
+        for (int s = 0; s < d.S; ++s) if (sG[i * rows + phi * d.S + s] < FS_INF) { pk |= (uint32_t)s << (8 * i); break; }
+    } else pk = comp[(size_t)(n_res - 1) * ns_stride + flat % NS];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31, i = w >> 1, p = w & 1;
+    if (w < FS_RMAX * 2) {
+      int bstar = 0;
+      const uint32_t q = i < n_res ? v.states[k].t[i].q[p] : 0u;
+      if (q > 0) {
+        const fs_tenant& tt = v.states[k].t[i];
+        const int sg = (pk >> (8 * i)) & 0xFF;
+        const float target = g_in[(size_t)(i * 2 + p) * rows + phi * d.S + sg], slo = tt.slo_ms[p];
+        const size_t base = fs_idx(d, tt.model, p, phi, sg, 0);
+        const int nb = (int)(q < (uint32_t)d.B ? q : (uint32_t)d.B);
+        const bool obj_power = flags & FS_OBJ_POWER;
+        bstar = -1;
+        for (int b0 = 0; b0 < nb && bstar < 0; b0 += 32) {
+          const int beta = b0 + lane;
+          bool hit = false;
+          if (beta < nb) {
+            const float la = v.lat[base + beta], pw = v.pow[base + beta];
+            const float t = __fmul_rn(__uint2float_rn(fs_ceil_div(q, (uint32_t)beta + 1u)), la);
+            const bool ok = p == 0 ? (t <= slo) : (la <= slo);
+            hit = ok && (obj_power ? pw : __fmul_rn(t, pw)) == target;
+          }
+          const unsigned m = __ballot_sync(0xffffffffu, hit);
+          if (m) bstar = b0 + __ffs(m) - 1;
+        }
+        if (bstar < 0) bstar = 0;
+      }
+      if (lane == 0) sbeta[w] = bstar;
+    }
+  }
+  __syncthreads();
   if (threadIdx.x == 0) {
     if (key != FS_KEY_NONE) {
-      const uint32_t flat = (uint32_t)key;
-      const int phi = minsm ? (int)flat : (int)(flat / NS);
-      o.phi = (int16_t)phi; o.f_req = (int16_t)(int)fkey; o.flat = flat;
+      o.phi = (int16_t)phi; o.f_req = (int16_t)(int)fkey; o.flat = (uint32_t)key;
       o.cost = fs_unorderable((uint32_t)(key >> 32));
-      uint32_t pk = 0;
-      if (minsm) {
-        for (int i = 0; i < n_res; ++i)
-          for (int s = 0; s < d.S; ++s) if (sG[i * rows + phi * d.S + s] < FS_INF) { pk |= (uint32_t)s << (8 * i); break; }
-      } else pk = comp[(size_t)(n_res - 1) * ns_stride + flat % NS];
-      const uint8_t* b_in = Bs + (size_t)gi * (FS_RMAX * 2) * rows;
       const fs_gpu_state& g = v.states[k];
       float E = 0.0f, PW = 0.0f;
       for (int i = 0; i < n_res; ++i) {
@@ -333,7 +359,7 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
         float e[2], pw[2];
         for (int p = 0; p < 2; ++p) {
           const uint32_t q = g.t[i].q[p];
-          const int beta = q ? b_in[(size_t)(i * 2 + p) * rows + phi * d.S + sg] : 0;
+          const int beta = q ? sbeta[i * 2 + p] : 0;
           o.beta[i][p] = (uint8_t)beta;
           e[p] = 0.0f; pw[p] = 0.0f;
           if (q > 0) {
@@ -385,21 +411,21 @@ int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs
     const LocalSlot* sl = reinterpret_cast<const LocalSlot*>(sc.slots);
     // one launch per phase: the deadline rule differs (prefill: whole queue; decode: one step)
     if (flags & FS_OBJ_POWER) {
-      local_slot_grouped_kernel<0, true><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
-      local_slot_grouped_kernel<1, true><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
+      local_slot_grouped_kernel<0, true><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G);
+      local_slot_grouped_kernel<1, true><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G);
     } else {
-      local_slot_grouped_kernel<0, false><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
-      local_slot_grouped_kernel<1, false><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G, sc.B);
+      local_slot_grouped_kernel<0, false><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G);
+      local_slot_grouped_kernel<1, false><<<grid, LS_WARPS * 32, smem, st>>>(v, sc.bin_off, sc.keylist, sc.nkeys, sl, sc.G);
     }
     launches += 6;
   } else {
-    local_slot_kernel<<<dim3(n, FS_RMAX * 2), 256, 0, st>>>(v, n, gpu_ids, flags, sc.G, sc.B);
+    local_slot_kernel<<<dim3(n, FS_RMAX * 2), 256, 0, st>>>(v, n, gpu_ids, flags, sc.G);
     launches += 1;
   }
   fs_tm_end(tm, FS_T_LOCAL_SLOT, st);
   const size_t smem = sizeof(float) * FS_RMAX * rows;
   fs_tm_beg(tm, FS_T_LOCAL_SPLIT, st);
-  local_split_kernel<<<n, 256, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.B, sc.comp, sc.comp_n,
+  local_split_kernel<<<n, 256, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.comp, sc.comp_n,
                                            sc.ns_stride, out);
   fs_tm_end(tm, FS_T_LOCAL_SPLIT, st);
   return launches + 1;
