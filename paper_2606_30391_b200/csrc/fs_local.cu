@@ -153,15 +153,18 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
         const uint32_t beta = b4 + u;
         const uint32_t rounds = beta == 0 ? sl_.q : __umulhi(sl_.q + beta, c_magic[beta]);
         const float fr = __uint2float_rn(rounds);
-        const bool act = beta < nb;
+        // beta past this slot's range: a deadline nothing meets (tables are > 0)
+        const float slo_b = beta < nb ? sl_.slo : -1.0f;
 #pragma unroll
         for (int r = 0; r < LS_TR; ++r) {
           const float la = u == 0 ? L4[r].x : u == 1 ? L4[r].y : u == 2 ? L4[r].z : L4[r].w;
           const float pw = u == 0 ? P4[r].x : u == 1 ? P4[r].y : u == 2 ? P4[r].z : P4[r].w;
           const float t = __fmul_rn(fr, la);
-          const bool ok = P == 0 ? (t <= sl_.slo) : (la <= sl_.slo);
           const float cost = OBJ_POWER ? pw : __fmul_rn(t, pw);
-          if (act && ok) best[r] = fminf(best[r], cost);   // beta* is recovered for the chosen row only
+          // one compare + one predicated min per candidate (the ALU pipe binds this kernel);
+          // beta* is recovered for the chosen row only (split kernel)
+          asm("{.reg .pred p; setp.le.f32 p, %1, %2; @p min.f32 %0, %0, %3;}"
+              : "+f"(best[r]) : "f"(P == 0 ? t : la), "f"(slo_b), "f"(cost));
         }
       }
     }
