@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
 // time: lane <-> slot, sequential over beta, LDS.128 broadcasts of four beta per row, rounds by
 // multiply-high with a per-beta magic constant (exact for q < 2^24, beta < 256).  Strict '<' in
 // ascending beta keeps the lowest beta on ties, as the definition wants.
-constexpr int LS_TR = 4;          // rows per tile
+constexpr int LS_TR = 8;          // rows per tile
 constexpr int LS_QB = 8;          // q buckets per key (slots of similar depth share a warp)
 constexpr int LS_WARPS = 8;
 __constant__ uint32_t c_magic[FS_MAX_B];   // ceil(2^32 / (beta+1)), beta >= 1
@@ -171,7 +171,9 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
     if (have) {
       const size_t o = ((size_t)sl_.gi * (FS_RMAX * 2) + (sl_.meta & 0xFF)) * rows + r0;
       if (tr == LS_TR && (rows & 3) == 0) {
-        *reinterpret_cast<float4*>(Gs + o) = make_float4(best[0], best[1], best[2], best[3]);
+#pragma unroll
+        for (int r = 0; r < LS_TR; r += 4)
+          *reinterpret_cast<float4*>(Gs + o + r) = make_float4(best[r], best[r + 1], best[r + 2], best[r + 3]);
       } else {
 #pragma unroll
         for (int r = 0; r < LS_TR; ++r) if (r < tr) Gs[o + r] = best[r];
