@@ -43,8 +43,8 @@ OPS_WARM_TEST = 20.0       # per warm pair tested: 12-word item, bound (5 fp32),
 OPS_DEF = 14.0             # per candidate scored by the definition: 4 loads, 4 mul, 3 add/sub, 3 compares
 # dram bytes per launch of the scoring kernel and its issue utilisation, from the committed ncu
 # capture of this workload (profiles/; a profiler cannot run inside the timed bench)
-NCU_TRAFFIC_BYTES = 43.05e6
-NCU_NOTE = "profiles/r01_place_dense_v5_ncu_full.md: sm__throughput 56.5 %, issue active 57.8 % of peak, 372.6 M warp instructions"
+NCU_TRAFFIC_BYTES = 43.24e6
+NCU_NOTE = "profiles/r01_final_pod.md: sm__throughput 58.7 %, issue active 64.7 % of peak, 242.6 M warp instructions"
 SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128   # 4 schedulers x 32 lanes (B300_MICROARCH "issue")
 
 
