@@ -23,6 +23,10 @@ _LOCAL_DT = np.dtype(
      ("_pad", "<u4", (4,))])
 _CONSOL_DT = np.dtype([("dst", "<i4"), ("phi", "<i4"), ("score_mj", "<f4"), ("saving_mj", "<f4")])
 
+_LLM_PROFILE_DT = np.dtype([("sigma_p", "<i2"), ("phi_p", "<i2"), ("sigma_d", "<i2"), ("phi_d", "<i2"),
+                            ("t_p_ms", "<f4"), ("t_d_ms", "<f4"), ("p_p_w", "<f4"), ("p_d_w", "<f4"),
+                            ("sm_units", "<f4"), ("need_units", "<i2"), ("phi_l", "<i2"), ("t_l_ms", "<f4"),
+                            ("e_l_mj", "<f4"), ("mem_mb", "<f4"), ("_pad", "<u4")])
 _TASK_OUT_DT = np.dtype([("score", "<f4"), ("latency_ms", "<f4"), ("rank", "<i4"), ("admitted", "<i4")])
 
 OBJ_ENERGY, OBJ_POWER, SPLIT_EXHAUSTIVE, SPLIT_MINSM = 0, 1, 0, 2
@@ -103,6 +107,25 @@ def batch_tasks(lat, pow_, states, off, tasks, gpu_ids=None, nthreads: int = 1) 
     lib().fo_batch_tasks(*_tables(lat, pow_), _p(states), C.c_int(n), ids, _p(off),
                          _p(np.ascontiguousarray(tasks)), _p(out), C.c_int(nthreads))
     return out
+
+
+def llm_profile(lat, pow_, models, llms, nthreads: int = 1) -> np.ndarray:
+    """Algorithm 1 phase 1 by definition (PAPER.md, 337-339, Eq. 8, Little's law)."""
+    out = np.zeros(len(llms), dtype=_LLM_PROFILE_DT)
+    lib().fo_llm_profile(*_tables(lat, pow_), _p(models), C.c_int(len(llms)), _p(np.ascontiguousarray(llms)),
+                         _p(out), C.c_int(nthreads))
+    return out
+
+
+def ewr(gpu_of, f_mhz, t_ms, K: int):
+    """Energy Waste Ratio, Eq. 5-7: returns (F_g [K], E_waste, E_optimal, EWR)."""
+    gpu_of = np.ascontiguousarray(gpu_of, dtype=np.int32)
+    f_mhz = np.ascontiguousarray(f_mhz, dtype=np.float32)
+    t_ms = np.ascontiguousarray(t_ms, dtype=np.float32)
+    fg = np.zeros(max(K, 1), dtype=np.float32)
+    out = np.zeros(3, dtype=np.float64)
+    lib().fo_ewr(C.c_int(len(gpu_of)), _p(gpu_of), _p(f_mhz), _p(t_ms), C.c_int(K), _p(fg), _p(out))
+    return fg[:K], float(out[0]), float(out[1]), float(out[2])
 
 
 def slot(lat, pow_, m, p, phi, sigma, beta, q, wait, slo):

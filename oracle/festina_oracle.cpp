@@ -19,6 +19,8 @@
 //   paper dispatcher ...... Eq. 2-3 by hand, Fig. 6-shaped toy, 2 % band
 //                           and tie-breaker cases, T_avail-ordered F_max retry and
 //                           scale-out, independent numpy restatement
+//   Alg. 1 phase 1 / EWR .. Eq. 8 and Little's law by hand, brute-force argmin restatement; EWR closed
+//                           forms (0 iff aligned, two-LLM case by hand)
 //   priority batching ..... Fig. 8 steps 1-2 worked table, independent numpy
 //                           restatement, budget / bypass invariants
 // Nothing here is "parity unpinned".
@@ -252,6 +254,80 @@ void dispatch_one(const Tables& T, const ModelInfo* mi, const GpuState* gs, int 
     }
   }
   out = best;
+}
+
+// ------------------------------------------------------------------------------------------
+// Algorithm 1, Phase 1: per active LLM, from its average input / output length:
+//   (SM_p, F_p), (SM_d, F_d) = the LUT configurations that minimise the prefill / decode energy
+//   while meeting the TTFT / TBT SLO (ties: lowest phi, then lowest sigma); T_p, T_d, P_p, P_d there;
+//   SM_l = (SM_p*T_p + SM_d*T_d) / (T_p + T_d)                                   (Eq. 8)
+//   l.S  = ceil(SM_l) share units;  l.F = the frequency that minimises the LLM's total energy at
+//   l.S units with both SLOs met (CalcFreq, Alg. 1 l.4; lowest phi on ties);
+//   M_l  = Weights + N_conc * Size_KV,  N_conc = lambda * W (Little's law), W = T_p + T_d at
+//   (l.S, l.F), Size_KV = (avg_in + avg_out) * kv_mb_per_token.
+// One sequence per decode step (batch bucket 0), the prefill batch bucket as in fs_place_batch.
+struct Llm { int32_t model; uint32_t avg_in, avg_out; float slo_ttft_ms, slo_tbt_ms, lambda_rps; uint32_t pad[2]; };
+struct LlmProfile {
+  int16_t sigma_p, phi_p, sigma_d, phi_d; float t_p_ms, t_d_ms, p_p_w, p_d_w;
+  float sm_units; int16_t need_units, phi_l; float t_l_ms, e_l_mj, mem_mb; uint32_t pad;
+};
+static_assert(sizeof(Llm) == 32 && sizeof(LlmProfile) == 48, "layout");
+
+void llm_profile_one(const Tables& T, const ModelInfo* mi, const Llm& l, LlmProfile& o) {
+  const int m = l.model;
+  const uint32_t L = l.avg_in, O = l.avg_out;
+  const int br0 = (int)(L < (uint32_t)T.B ? L : (uint32_t)T.B) - 1;
+  std::memset(&o, 0, sizeof(o));
+  o.sigma_p = o.phi_p = o.sigma_d = o.phi_d = o.need_units = o.phi_l = -1;
+  o.t_p_ms = o.t_d_ms = o.p_p_w = o.p_d_w = o.sm_units = o.t_l_ms = o.e_l_mj = o.mem_mb = INF;
+  float bp = INF, bd = INF;
+  for (int phi = 0; phi < T.F; ++phi)
+    for (int sg = 0; sg < T.S; ++sg) {
+      Slot p = slot_eval(T, m, 0, phi, sg, br0 < 0 ? 0 : br0, L, 0.0f, l.slo_ttft_ms);
+      if (p.ok && p.e < bp) {
+        bp = p.e; o.sigma_p = (int16_t)sg; o.phi_p = (int16_t)phi; o.t_p_ms = p.t;
+        o.p_p_w = L ? T.POW(m, 0, phi, sg, br0) : 0.0f;
+      }
+      Slot d = slot_eval(T, m, 1, phi, sg, 0, O, 0.0f, l.slo_tbt_ms);
+      if (d.ok && d.e < bd) {
+        bd = d.e; o.sigma_d = (int16_t)sg; o.phi_d = (int16_t)phi; o.t_d_ms = d.t;
+        o.p_d_w = O ? T.POW(m, 1, phi, sg, 0) : 0.0f;
+      }
+    }
+  if (o.phi_p < 0 || o.phi_d < 0) return;                 // one phase cannot meet its SLO anywhere
+  const float tsum = o.t_p_ms + o.t_d_ms;
+  o.sm_units = tsum > 0.0f ? (((float)(o.sigma_p + 1) * o.t_p_ms + (float)(o.sigma_d + 1) * o.t_d_ms) / tsum) : 1.0f;
+  int need = (int)std::ceil(o.sm_units);
+  if (need < 1) need = 1;
+  if (need > T.S) need = T.S;
+  o.need_units = (int16_t)need;
+  float be = INF;
+  for (int phi = 0; phi < T.F; ++phi) {
+    Slot p = slot_eval(T, m, 0, phi, need - 1, br0 < 0 ? 0 : br0, L, 0.0f, l.slo_ttft_ms);
+    Slot d = slot_eval(T, m, 1, phi, need - 1, 0, O, 0.0f, l.slo_tbt_ms);
+    const float e = p.e + d.e;
+    if (p.ok && d.ok && e < be) { be = e; o.phi_l = (int16_t)phi; o.t_l_ms = p.t + d.t; o.e_l_mj = e; }
+  }
+  if (o.phi_l < 0) return;
+  const float nconc = l.lambda_rps * (o.t_l_ms / 1000.0f);
+  const float kvsize = (float)(L + O) * mi[m].kv_mb_per_token;
+  o.mem_mb = mi[m].weights_mb + nconc * kvsize;
+}
+
+// Energy Waste Ratio (Eq. 5-7): F_g = highest preferred frequency among the LLMs on GPU g,
+//   E_waste = sum t_l (F_g^3 - F_l^3),  E_optimal = sum t_l F_l^3,  EWR = E_waste / E_optimal.
+// Plain left-to-right sums in binary64 over the LLMs in index order; gpu < 0 = not placed.
+void ewr_all(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, int K, float* fg, double out[3]) {
+  for (int g = 0; g < K; ++g) fg[g] = 0.0f;
+  for (int l = 0; l < n; ++l) if (gpu_of[l] >= 0 && f_mhz[l] > fg[gpu_of[l]]) fg[gpu_of[l]] = f_mhz[l];
+  double waste = 0.0, opt = 0.0;
+  for (int l = 0; l < n; ++l) {
+    if (gpu_of[l] < 0) continue;
+    const double F = fg[gpu_of[l]], f = f_mhz[l], t = t_ms[l];
+    waste += t * (F * F * F - f * f * f);
+    opt += t * (f * f * f);
+  }
+  out[0] = waste; out[1] = opt; out[2] = opt > 0.0 ? waste / opt : 0.0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -500,6 +576,19 @@ int fo_dispatch(int M, int F, int S, int B, const float* lat, const float* pow,
   const ModelInfo* mi = (const ModelInfo*)models; const GpuState* gs = (const GpuState*)states;
   const Request* rq = (const Request*)reqs; Placement* o = (Placement*)out;
   par_for(R, nthreads, [&](int r) { dispatch_one(T, mi, gs, K, rq[r], o[r]); });
+  return 0;
+}
+
+int fo_llm_profile(int M, int F, int S, int B, const float* lat, const float* pow, const void* models,
+                   int n, const void* llms, void* out, int nthreads) {
+  Tables T{M, F, S, B, lat, pow};
+  const ModelInfo* mi = (const ModelInfo*)models; const Llm* ll = (const Llm*)llms; LlmProfile* o = (LlmProfile*)out;
+  par_for(n, nthreads, [&](int i) { llm_profile_one(T, mi, ll[i], o[i]); });
+  return 0;
+}
+
+int fo_ewr(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, int K, float* fg, double* out3) {
+  ewr_all(n, gpu_of, f_mhz, t_ms, K, fg, out3);
   return 0;
 }
 

@@ -39,7 +39,14 @@ CONSOL_DT = np.dtype([("dst", "<i4"), ("phi", "<i4"), ("score_mj", "<f4"), ("sav
 TASK_DT = np.dtype([("model", "<i2"), ("phase", "u1"), ("sigma", "u1"), ("beta", "u1"), ("_p0", "u1", (3,)),
                     ("slack_ms", "<f4"), ("age_ms", "<f4"), ("mem_mb", "<f4"), ("tag", "<u4")])
 TASK_OUT_DT = np.dtype([("score", "<f4"), ("latency_ms", "<f4"), ("rank", "<i4"), ("admitted", "<i4")])
+LLM_DT = np.dtype([("model", "<i4"), ("avg_in", "<u4"), ("avg_out", "<u4"), ("slo_ttft_ms", "<f4"),
+                   ("slo_tbt_ms", "<f4"), ("lambda_rps", "<f4"), ("_pad", "<u4", (2,))])
+LLM_PROFILE_DT = np.dtype([("sigma_p", "<i2"), ("phi_p", "<i2"), ("sigma_d", "<i2"), ("phi_d", "<i2"),
+                           ("t_p_ms", "<f4"), ("t_d_ms", "<f4"), ("p_p_w", "<f4"), ("p_d_w", "<f4"),
+                           ("sm_units", "<f4"), ("need_units", "<i2"), ("phi_l", "<i2"), ("t_l_ms", "<f4"),
+                           ("e_l_mj", "<f4"), ("mem_mb", "<f4"), ("_pad", "<u4")])
 assert TASK_DT.itemsize == 24 and TASK_OUT_DT.itemsize == 16
+assert LLM_DT.itemsize == 32 and LLM_PROFILE_DT.itemsize == 48
 
 assert TENANT_DT.itemsize == 28 and GPU_STATE_DT.itemsize == 128 and REQUEST_DT.itemsize == 32
 assert MODEL_INFO_DT.itemsize == 16 and PLACEMENT_DT.itemsize == 32
@@ -328,6 +335,20 @@ def make_tasks(seed: int, K: int, M: int, S: int, B: int, lo: int, hi: int):
     t["mem_mb"] = np.minimum(np.exp(5.5 + st.normal(T)), 8000.0).astype(np.float32)
     t["tag"] = np.arange(T, dtype=np.uint32)
     return off, t
+
+
+def make_llms(seed: int, n: int, M: int) -> np.ndarray:
+    """Active LLMs for Algorithm 1 phase 1: average input / output lengths of the last window
+    (capped lognormals as for requests), SLOs in the paper's Table 2 ranges, arrival rate U[0.1, 5] req/s."""
+    st = Stream(seed, "llms")
+    l = np.zeros(n, dtype=LLM_DT)
+    l["model"] = st.randint(n, 0, M - 1)
+    l["avg_in"] = st.lognormal_len(n, 6.0, 1.0, 4096)
+    l["avg_out"] = st.lognormal_len(n, 5.0, 1.0, 4096)
+    l["slo_ttft_ms"] = st.urange(n, 250.0, 2000.0).astype(np.float32)
+    l["slo_tbt_ms"] = st.urange(n, 50.0, 150.0).astype(np.float32)
+    l["lambda_rps"] = st.urange(n, 0.1, 5.0).astype(np.float32)
+    return l
 
 
 def arrival_ticks(seed: int, R: int, n_ticks: int, rho: float = 3.3) -> np.ndarray:
