@@ -130,6 +130,21 @@ typedef struct {
  * GPU, extra energy the destination pays, net saving of draining the source.             */
 typedef struct { int32_t dst, phi; float score_mj, saving_mj; } fs_consol_out; /* 16 bytes */
 
+/* One active LLM for Algorithm 1, phase 1: its model, the average input / output length of
+ * the last window, its SLOs and its measured request arrival rate (requests per second).  32 bytes. */
+typedef struct {
+  int32_t model; uint32_t avg_in, avg_out; float slo_ttft_ms, slo_tbt_ms, lambda_rps; uint32_t _pad[2];
+} fs_llm;
+/* (sigma_p, phi_p), (sigma_d, phi_d): energy-optimal feasible LUT configuration of the prefill / decode
+ * phase, with its duration t_*_ms and power p_*_w; sm_units = Eq. 8 in share units, need_units =
+ * ceil(sm_units) = l.S; phi_l = l.F, the energy-optimal feasible frequency at l.S units, t_l_ms and
+ * e_l_mj the LLM's time and energy there; mem_mb = M_l by Little's law.  -1 / +INF where a
+ * phase (or l.F) has no feasible configuration.  48 bytes.                                      */
+typedef struct {
+  int16_t sigma_p, phi_p, sigma_d, phi_d; float t_p_ms, t_d_ms, p_p_w, p_d_w;
+  float sm_units; int16_t need_units, phi_l; float t_l_ms, e_l_mj, mem_mb; uint32_t _pad;
+} fs_llm_profile;
+
 /* One runnable task of the local scheduler's priority queue (Fig. 8 steps 1-2): a
  * decode step or a prefill unit of `model`, run with `sigma`+1 SM share units at batch bucket
  * `beta`.  slack_ms = remaining time to its SLO deadline (TBT for decode, TTFT for prefill),
@@ -212,6 +227,18 @@ int fs_dispatch(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* ou
 int fs_batch_tasks(fs_ctx* ctx, int32_t n, const int32_t* gpu_ids, const int32_t* task_off,
                    const fs_task* tasks, fs_task_out* out, int32_t n_tasks, int space,
                    void* cuda_stream);
+
+/* Algorithm 1, phase 1 (Eq. 8, Little's law) for n active LLMs: see
+ * fs_llm_profile.  Needs fs_load_profiles only.  llms, out : [n], in `space`.                   */
+int fs_llm_profiles(fs_ctx* ctx, int32_t n, const fs_llm* llms, fs_llm_profile* out, int space,
+                    void* cuda_stream);
+
+/* Energy Waste Ratio (Eq. 5-7) of a placement of n LLMs on K GPUs: gpu_of[l] = GPU of LLM l
+ * (< 0: not placed), f_mhz[l] = its preferred frequency F_l, t_ms[l] = its execution time t_l.
+ * f_gpu[g] = F_g = the highest F_l on GPU g (0 if empty); out3 = {E_waste, E_optimal, EWR} in
+ * binary64 (sums over the LLMs; EWR = 0 when E_optimal = 0).  All pointers in `space`.           */
+int fs_ewr(fs_ctx* ctx, int32_t n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms,
+           int32_t K, float* f_gpu, double* out3, int space, void* cuda_stream);
 
 /* Diagnostics. */
 const char* fs_strerror(int code);

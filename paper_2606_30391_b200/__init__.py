@@ -23,7 +23,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm", "batch_tasks", "dispatch")
@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
     L.fs_place_batch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_local_config.argtypes = [vp, i32, vp, u32, vp, C.c_int, vp]
     L.fs_consolidate.argtypes = [vp, vp, C.c_int, vp]
+    L.fs_llm_profiles.argtypes = [vp, i32, vp, vp, C.c_int, vp]
+    L.fs_ewr.argtypes = [vp, i32, vp, vp, vp, i32, vp, vp, C.c_int, vp]
     L.fs_dispatch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_batch_tasks.argtypes = [vp, i32, vp, vp, vp, vp, i32, C.c_int, vp]
     L.fs_strerror.argtypes = [C.c_int]
@@ -232,6 +234,33 @@ class Festina:
         rc = lib().fs_batch_tasks(self._h, n, pi, pf, pt, po, n_tasks, sp, _stream_ptr(stream))
         self._check(rc, "fs_batch_tasks")
         return out
+
+    def llm_profiles(self, llms, out=None, n: int | None = None, stream=None):
+        """fs_llm_profiles: Algorithm 1 phase 1 per active LLM (host arrays or device tensors)."""
+        if n is None:
+            n = len(llms) if not hasattr(llms, "data_ptr") else llms.numel() * llms.element_size() // 32
+        pi, sp, keep = _buf(llms, n * 32)
+        if sp is None:
+            sp = FS_HOST
+        if out is None:
+            assert sp == FS_HOST
+            out = np.zeros(n, dtype=synth.LLM_PROFILE_DT)
+        po, spo, keep2 = _buf(out, n * 48)
+        self._check(lib().fs_llm_profiles(self._h, n, pi, po, sp, _stream_ptr(stream)), "fs_llm_profiles")
+        return out
+
+    def ewr(self, gpu_of, f_mhz, t_ms, K: int, stream=None):
+        """fs_ewr on host arrays: returns (F_g [K], E_waste, E_optimal, EWR)."""
+        gpu_of = np.ascontiguousarray(gpu_of, dtype=np.int32)
+        f_mhz = np.ascontiguousarray(f_mhz, dtype=np.float32)
+        t_ms = np.ascontiguousarray(t_ms, dtype=np.float32)
+        fg = np.zeros(max(K, 1), dtype=np.float32)
+        out = np.zeros(3, dtype=np.float64)
+        p = lambda a: C.c_void_p(a.ctypes.data)
+        rc = lib().fs_ewr(self._h, len(gpu_of), p(gpu_of), p(f_mhz), p(t_ms), K, p(fg), p(out), FS_HOST,
+                          _stream_ptr(stream))
+        self._check(rc, "fs_ewr")
+        return fg[:K], float(out[0]), float(out[1]), float(out[2])
 
     def consolidate(self, out=None, stream=None):
         if out is None:

@@ -36,6 +36,8 @@ struct fs_ctx {
   uint4* lslots = nullptr;
   // task batching scratch (FS_HOST staging)
   int bt_n_cap = 0, bt_t_cap = 0; int32_t *bt_ids = nullptr, *bt_off = nullptr; fs_task* bt_tasks = nullptr; fs_task_out* bt_out = nullptr;
+  // Algorithm 1 / EWR scratch (FS_HOST staging)
+  size_t a1_cap = 0; unsigned char* a1_buf = nullptr;
   // consolidation scratch
   size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
   unsigned long long* ckeys = nullptr; fs_consol_out* consol_dev = nullptr;
@@ -157,7 +159,7 @@ int fs_destroy(fs_ctx* c) {
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
-                  c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out};
+                  c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (c->flag_host) cudaFreeHost(c->flag_host);
   if (c->have_events)
@@ -373,6 +375,71 @@ int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out,
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+static int a1_reserve(fs_ctx* c, size_t bytes) {
+  if (bytes > c->a1_cap) { FS_TRY(grow(c, c->a1_buf, bytes)); c->a1_cap = bytes; }
+  return FS_OK;
+}
+
+int fs_llm_profiles(fs_ctx* c, int32_t n, const fs_llm* llms, fs_llm_profile* out, int space, void* cuda_stream) {
+  if (!c || n < 0 || (n > 0 && (!llms || !out))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof) return FS_ERR_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (n == 0) return pending;
+  const fs_llm* d_in = llms; fs_llm_profile* d_out = out;
+  if (space == FS_HOST) {
+    FS_TRY(a1_reserve(c, (size_t)n * (sizeof(fs_llm) + sizeof(fs_llm_profile))));
+    d_in = reinterpret_cast<fs_llm*>(c->a1_buf);
+    d_out = reinterpret_cast<fs_llm_profile*>(c->a1_buf + (size_t)n * sizeof(fs_llm));
+    FS_CUDA(c, cudaMemcpyAsync(c->a1_buf, llms, (size_t)n * sizeof(fs_llm), cudaMemcpyHostToDevice, st));
+  }
+  c->launches += fsk_llm_profile(view_of(c), n, d_in, d_out, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(fs_llm_profile), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+int fs_ewr(fs_ctx* c, int32_t n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, int32_t K,
+           float* f_gpu, double* out3, int space, void* cuda_stream) {
+  if (!c || n < 0 || K < 0 || !out3 || (n > 0 && (!gpu_of || !f_mhz || !t_ms)) || (K > 0 && !f_gpu)) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  const int32_t* d_g = gpu_of; const float *d_f = f_mhz, *d_t = t_ms; float* d_fg = f_gpu; double* d_o = out3;
+  if (space == FS_HOST) {
+    const size_t nn = (size_t)n, kk = (size_t)K;
+    FS_TRY(a1_reserve(c, 32 + nn * 12 + kk * 4 + 16));
+    d_o = reinterpret_cast<double*>(c->a1_buf);                       // 3 doubles (32 bytes reserved)
+    d_g = reinterpret_cast<int32_t*>(c->a1_buf + 32);
+    d_f = reinterpret_cast<float*>(c->a1_buf + 32 + nn * 4);
+    d_t = reinterpret_cast<float*>(c->a1_buf + 32 + nn * 8);
+    d_fg = reinterpret_cast<float*>(c->a1_buf + 32 + nn * 12);
+    if (n > 0) {
+      FS_CUDA(c, cudaMemcpyAsync((void*)d_g, gpu_of, nn * 4, cudaMemcpyHostToDevice, st));
+      FS_CUDA(c, cudaMemcpyAsync((void*)d_f, f_mhz, nn * 4, cudaMemcpyHostToDevice, st));
+      FS_CUDA(c, cudaMemcpyAsync((void*)d_t, t_ms, nn * 4, cudaMemcpyHostToDevice, st));
+    }
+  }
+  c->launches += fsk_ewr(n, d_g, d_f, d_t, K, d_fg, d_o, c->flag_dev, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    if (K > 0) FS_CUDA(c, cudaMemcpyAsync(f_gpu, d_fg, (size_t)K * 4, cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaMemcpyAsync(out3, d_o, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;

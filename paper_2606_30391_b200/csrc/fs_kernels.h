@@ -99,6 +99,11 @@ int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
 int fsk_batch_tasks(const FsView& v, int n, const int32_t* gpu_ids, const int32_t* off,
                     const fs_task* tasks, fs_task_out* out, int n_tasks, cudaStream_t st, FsTimers* tm);
 
+// fs_alg1.cu — Algorithm 1 phase 1 and the Energy Waste Ratio (first part)
+int fsk_llm_profile(const FsView& v, int n, const fs_llm* llms, fs_llm_profile* out, cudaStream_t st);
+int fsk_ewr(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, int K, float* fg, double* out3,
+            int* flag, cudaStream_t st);
+
 #ifdef __CUDACC__
 // One co-resident ("tenant") at frequency phi with share sigma, wait = 0 because its slo is the
 // REMAINING slack (R:s12).  bump = one more sequence joins its decode batch: the decode bucket

@@ -396,3 +396,52 @@ def test_dispatch_full_size(ctx):
     idx = np.unique(synth.Stream(11, "sample").randint(2048, 0, cl.R - 1))
     cmp.assert_placement_equal(got[idx], _oracle_dispatch(cl, cl.requests[idx]))
     assert set(np.unique(got["f_req"]).tolist()) >= {1, 2, 3}
+
+
+# ---- Algorithm 1 phase 1 (fs_llm_profiles) and the Energy Waste Ratio (fs_ewr) --------------------
+def _assert_profiles_equal(got, ref):
+    for f in ("sigma_p", "phi_p", "sigma_d", "phi_d", "need_units", "phi_l"):
+        cmp._int_equal(got[f], ref[f], f"llm.{f}")
+    for f in ("t_p_ms", "t_d_ms", "p_p_w", "p_d_w", "sm_units", "t_l_ms", "e_l_mj", "mem_mb"):
+        cmp._float_close(got[f], ref[f], f"llm.{f}", True)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_llm_profiles(ctx, seed):
+    st = synth.Stream(seed, "ldims")
+    M = int(st.randint(1, 1, 9)[0]); F = int(st.randint(1, 1, 70)[0]); S = int(st.randint(1, 1, 20)[0]); B = int(st.randint(1, 1, 40)[0])
+    cl = synth.make_custom(seed=1200 + seed, K=2, M=M, F=F, S=S, B=B, R=0)
+    if seed % 2:
+        cl = U.tie_heavy(cl, seed)
+    llms = synth.make_llms(seed, 300, cl.M)
+    if seed % 4 == 1:
+        llms["slo_ttft_ms"] *= 0.02; llms["slo_tbt_ms"] *= 0.2
+    if seed % 4 == 2:
+        llms["avg_in"][::3] = 0; llms["avg_out"][1::3] = 0
+    ctx.load_cluster(cl)
+    _assert_profiles_equal(ctx.llm_profiles(llms), oracle.llm_profile(cl.lat, cl.pow, cl.models, llms, 8))
+
+
+def test_llm_profiles_pod_size(ctx):
+    cl = synth.make_cluster("pod")
+    llms = synth.make_llms(2, 4096, cl.M)
+    ctx.load_cluster(cl)
+    got = ctx.llm_profiles(llms)
+    _assert_profiles_equal(got, oracle.llm_profile(cl.lat, cl.pow, cl.models, llms, 8))
+    assert (got["phi_l"] >= 0).mean() > 0.9
+
+
+def test_ewr(ctx):
+    cl = synth.make_cluster("tiny")
+    ctx.load_cluster(cl)
+    st = synth.Stream(5, "ewr")
+    for n, K in ((0, 3), (1, 1), (5000, 300), (70000, 4096)):
+        g = st.randint(n, -1, K - 1).astype(np.int32); f = st.urange(n, 210, 1980).astype(np.float32)
+        t = st.urange(n, 1, 1e4).astype(np.float32)
+        fg, w, o, r = ctx.ewr(g, f, t, K)
+        rfg, rw, ro, rr = oracle.ewr(g, f, t, K)
+        assert np.array_equal(fg, rfg)
+        # binary64 sums in a different (tree) order: 1e-12 relative
+        assert abs(w - rw) <= 1e-12 * abs(rw) and abs(o - ro) <= 1e-12 * abs(ro) and abs(r - rr) <= 1e-12 * abs(rr)
+    fg, w, o, r = ctx.ewr([0, 0, 1, -1], [1000, 1500, 1200, 900], [1, 2, 3, 4], 2)
+    assert list(fg) == [1500.0, 1200.0] and w == 1500.0 ** 3 - 1000.0 ** 3 and r == w / o
