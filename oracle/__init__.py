@@ -128,6 +128,15 @@ def ewr(gpu_of, f_mhz, t_ms, K: int):
     return fg[:K], float(out[0]), float(out[1]), float(out[2])
 
 
+def replace_plan(llms, s_eff: int, m_eff: float):
+    """Algorithm 1 phases 2-3: returns (gpu_of [n], (N_sm, N_mem, N_min, N_active))."""
+    llms = np.ascontiguousarray(llms)
+    gpu_of = np.full(len(llms), -1, dtype=np.int32)
+    summ = np.zeros(4, dtype=np.int32)
+    lib().fo_replace_plan(C.c_int(len(llms)), _p(llms), C.c_int(s_eff), C.c_float(m_eff), _p(gpu_of), _p(summ))
+    return gpu_of, tuple(int(x) for x in summ)
+
+
 def slot(lat, pow_, m, p, phi, sigma, beta, q, wait, slo):
     """The shared slot rule: returns (ok, t, e)."""
     t = C.c_float(0)

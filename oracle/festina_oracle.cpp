@@ -21,6 +21,8 @@
 //                           scale-out, independent numpy restatement
 //   Alg. 1 phase 1 / EWR .. Eq. 8 and Little's law by hand, brute-force argmin restatement; EWR closed
 //                           forms (0 iff aligned, two-LLM case by hand)
+//   Alg. 1 phases 2-3 ..... BFD against brute-force optimal bin counts on tiny inputs (OPT <= BFD <=
+//                           11/9 OPT + 1), a Fig. 9-shaped swap case by hand, capacity invariants
 //   priority batching ..... Fig. 8 steps 1-2 worked table, independent numpy
 //                           restatement, budget / bypass invariants
 // Nothing here is "parity unpinned".
@@ -331,6 +333,127 @@ void ewr_all(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms
 }
 
 // ------------------------------------------------------------------------------------------
+// Algorithm 1, phases 2-3 (prose P:341-357): capacity planning by Best-Fit-Decreasing and the
+// EWR-minimising placement loop.  Readings: BFD sorts by decreasing size (ties: lower
+// index), puts an item into the open bin with the least remaining room that still fits (ties: lower
+// bin), else opens a bin; an LLM that exceeds a whole GPU is left unplaced (gpu = -1).  Phase 3 walks the
+// LLMs in ascending l.F (ties: lower index).  g.freq = highest l.F on g; the distance of an EMPTY GPU is
+// +INF (it is the last resort, so that similar frequencies group on the same GPU); ties: lower GPU.
+//   Target = closest GPU, Candidate = second closest.   Fits = SM units and memory both fit.
+//   1. Fits(target, l): assign.                                   (direct placement)
+//   2. else l_out = resident of target with the lowest l.F (ties: lower index); if Fits(cand, l_out) and
+//      Fits(target - l_out, l) and E_swap < E_curr: move l_out to cand, assign l to target, where
+//      E_curr = waste(target + l) + waste(cand), E_swap = waste(target - l_out + l) + waste(cand + l_out),
+//      waste(R) = sum_{r in R} t_r (F_R^3 - F_r^3), F_R = max F_r, binary64, residents in the order they
+//      joined, the hypothetical newcomer last.                    (EWR-driven swap, Alg. 1 l.16-21)
+//   3. else if Fits(cand, l): assign to cand (l.23-24); else the closest other GPU that fits (fallback,
+//      P:357); else activate a new GPU (l.26-27).
+struct PlanLlm { int32_t need_units; float mem_mb, f_mhz, t_ms; };
+static_assert(sizeof(PlanLlm) == 16, "layout");
+
+int bfd_units(const PlanLlm* L, int n, int cap) {
+  std::vector<int> order; for (int i = 0; i < n; ++i) if (L[i].need_units <= cap) order.push_back(i);
+  for (size_t a = 1; a < order.size(); ++a) {              // insertion sort, decreasing, stable
+    int x = order[a]; int b = (int)a - 1;
+    while (b >= 0 && L[order[b]].need_units < L[x].need_units) { order[b + 1] = order[b]; --b; }
+    order[b + 1] = x;
+  }
+  std::vector<int> rem;
+  for (int i : order) {
+    int best = -1;
+    for (size_t g = 0; g < rem.size(); ++g)
+      if (rem[g] >= L[i].need_units && (best < 0 || rem[g] < rem[best])) best = (int)g;
+    if (best < 0) { rem.push_back(cap); best = (int)rem.size() - 1; }
+    rem[best] -= L[i].need_units;
+  }
+  return (int)rem.size();
+}
+int bfd_mem(const PlanLlm* L, int n, float cap) {
+  std::vector<int> order; for (int i = 0; i < n; ++i) if (L[i].mem_mb <= cap) order.push_back(i);
+  for (size_t a = 1; a < order.size(); ++a) {
+    int x = order[a]; int b = (int)a - 1;
+    while (b >= 0 && L[order[b]].mem_mb < L[x].mem_mb) { order[b + 1] = order[b]; --b; }
+    order[b + 1] = x;
+  }
+  std::vector<float> rem;
+  for (int i : order) {
+    int best = -1;
+    for (size_t g = 0; g < rem.size(); ++g)
+      if (rem[g] >= L[i].mem_mb && (best < 0 || rem[g] < rem[best])) best = (int)g;
+    if (best < 0) { rem.push_back(cap); best = (int)rem.size() - 1; }
+    rem[best] = rem[best] - L[i].mem_mb;
+  }
+  return (int)rem.size();
+}
+
+struct PlanGpu { int sm_left; float mem_left; std::vector<int> res; };
+float plan_freq(const PlanLlm* L, const PlanGpu& g) {
+  float f = 0.0f; for (int r : g.res) if (L[r].f_mhz > f) f = L[r].f_mhz; return f;
+}
+// waste of the residents of g without `skip` (-1: none) plus `extra` (-1: none), extra last
+double plan_waste(const PlanLlm* L, const PlanGpu& g, int skip, int extra) {
+  float F = 0.0f;
+  for (int r : g.res) if (r != skip && L[r].f_mhz > F) F = L[r].f_mhz;
+  if (extra >= 0 && L[extra].f_mhz > F) F = L[extra].f_mhz;
+  const double F3 = (double)F * F * F;
+  double w = 0.0;
+  for (int r : g.res) if (r != skip) { const double f = L[r].f_mhz; w += (double)L[r].t_ms * (F3 - f * f * f); }
+  if (extra >= 0) { const double f = L[extra].f_mhz; w += (double)L[extra].t_ms * (F3 - f * f * f); }
+  return w;
+}
+
+void replace_plan(const PlanLlm* L, int n, int s_eff, float m_eff, int32_t* gpu_of, int32_t summary[4]) {
+  const int n_sm = bfd_units(L, n, s_eff), n_mem = bfd_mem(L, n, m_eff);
+  const int n_min = n_sm > n_mem ? n_sm : n_mem;
+  std::vector<PlanGpu> G(n_min, PlanGpu{s_eff, m_eff, {}});
+  std::vector<int> order(n);
+  for (int i = 0; i < n; ++i) { order[i] = i; gpu_of[i] = -1; }
+  for (int a = 1; a < n; ++a) {                             // ascending l.F, stable
+    int x = order[a], b = a - 1;
+    while (b >= 0 && L[order[b]].f_mhz > L[x].f_mhz) { order[b + 1] = order[b]; --b; }
+    order[b + 1] = x;
+  }
+  auto fits = [&](const PlanGpu& g, int l, int freed_units, float freed_mem, bool freed) {
+    const int sm = g.sm_left + freed_units;
+    const float mem = freed ? (g.mem_left + freed_mem) : g.mem_left;
+    return L[l].need_units <= sm && L[l].mem_mb <= mem;
+  };
+  auto put = [&](int g, int l) {
+    G[g].sm_left -= L[l].need_units; G[g].mem_left = G[g].mem_left - L[l].mem_mb; G[g].res.push_back(l); gpu_of[l] = g;
+  };
+  for (int l : order) {
+    if (L[l].need_units > s_eff || !(L[l].mem_mb <= m_eff)) continue;       // exceeds a whole GPU
+    auto dist = [&](int g) { return G[g].res.empty() ? INF : std::fabs(plan_freq(L, G[g]) - L[l].f_mhz); };
+    int tgt = -1, cand = -1;
+    for (int g = 0; g < (int)G.size(); ++g) if (tgt < 0 || dist(g) < dist(tgt)) tgt = g;
+    for (int g = 0; g < (int)G.size(); ++g) if (g != tgt && (cand < 0 || dist(g) < dist(cand))) cand = g;
+    bool done = false;
+    if (tgt >= 0 && fits(G[tgt], l, 0, 0.0f, false)) { put(tgt, l); done = true; }
+    if (!done && tgt >= 0 && cand >= 0 && !G[tgt].res.empty()) {
+      int lo = -1;
+      for (int r : G[tgt].res) if (lo < 0 || L[r].f_mhz < L[lo].f_mhz || (L[r].f_mhz == L[lo].f_mhz && r < lo)) lo = r;
+      const double e_curr = plan_waste(L, G[tgt], -1, l) + plan_waste(L, G[cand], -1, -1);
+      const double e_swap = plan_waste(L, G[tgt], lo, l) + plan_waste(L, G[cand], -1, lo);
+      if (fits(G[cand], lo, 0, 0.0f, false) && fits(G[tgt], l, L[lo].need_units, L[lo].mem_mb, true) && e_swap < e_curr) {
+        PlanGpu& t = G[tgt];
+        t.sm_left += L[lo].need_units; t.mem_left = t.mem_left + L[lo].mem_mb;
+        for (size_t x = 0; x < t.res.size(); ++x) if (t.res[x] == lo) { t.res.erase(t.res.begin() + x); break; }
+        put(cand, lo); put(tgt, l); done = true;
+      }
+    }
+    if (!done && cand >= 0 && fits(G[cand], l, 0, 0.0f, false)) { put(cand, l); done = true; }
+    if (!done) {
+      int fb = -1;
+      for (int g = 0; g < (int)G.size(); ++g)
+        if (g != tgt && g != cand && fits(G[g], l, 0, 0.0f, false) && (fb < 0 || dist(g) < dist(fb))) fb = g;
+      if (fb >= 0) { put(fb, l); done = true; }
+    }
+    if (!done) { G.push_back(PlanGpu{s_eff, m_eff, {}}); put((int)G.size() - 1, l); }
+  }
+  summary[0] = n_sm; summary[1] = n_mem; summary[2] = n_min; summary[3] = (int)G.size();
+}
+
+// ------------------------------------------------------------------------------------------
 // fs_local_config: frequency sweep with per-task SM allocation (Fig. 8 step 3,
 // P:206-210); batching P:248; objective R:s8; split domain R:s9; one beta per slot R:s10.
 // Hierarchical definition: best beta per slot, then tenant sums, then the argmin.
@@ -589,6 +712,11 @@ int fo_llm_profile(int M, int F, int S, int B, const float* lat, const float* po
 
 int fo_ewr(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, int K, float* fg, double* out3) {
   ewr_all(n, gpu_of, f_mhz, t_ms, K, fg, out3);
+  return 0;
+}
+
+int fo_replace_plan(int n, const void* llms, int s_eff, float m_eff, int32_t* gpu_of, int32_t* summary4) {
+  replace_plan((const PlanLlm*)llms, n, s_eff, m_eff, gpu_of, summary4);
   return 0;
 }
 

@@ -46,7 +46,8 @@ LLM_PROFILE_DT = np.dtype([("sigma_p", "<i2"), ("phi_p", "<i2"), ("sigma_d", "<i
                            ("sm_units", "<f4"), ("need_units", "<i2"), ("phi_l", "<i2"), ("t_l_ms", "<f4"),
                            ("e_l_mj", "<f4"), ("mem_mb", "<f4"), ("_pad", "<u4")])
 assert TASK_DT.itemsize == 24 and TASK_OUT_DT.itemsize == 16
-assert LLM_DT.itemsize == 32 and LLM_PROFILE_DT.itemsize == 48
+PLAN_LLM_DT = np.dtype([("need_units", "<i4"), ("mem_mb", "<f4"), ("f_mhz", "<f4"), ("t_ms", "<f4")])
+assert LLM_DT.itemsize == 32 and LLM_PROFILE_DT.itemsize == 48 and PLAN_LLM_DT.itemsize == 16
 
 assert TENANT_DT.itemsize == 28 and GPU_STATE_DT.itemsize == 128 and REQUEST_DT.itemsize == 32
 assert MODEL_INFO_DT.itemsize == 16 and PLACEMENT_DT.itemsize == 32
@@ -348,6 +349,18 @@ def make_llms(seed: int, n: int, M: int) -> np.ndarray:
     l["slo_ttft_ms"] = st.urange(n, 250.0, 2000.0).astype(np.float32)
     l["slo_tbt_ms"] = st.urange(n, 50.0, 150.0).astype(np.float32)
     l["lambda_rps"] = st.urange(n, 0.1, 5.0).astype(np.float32)
+    return l
+
+
+def make_plan_llms(seed: int, n: int, S: int, freq_mhz: np.ndarray, mem_cap: float = 80000.0) -> np.ndarray:
+    """LLM descriptors (l.S, l.M, l.F) for Algorithm 1 phases 2-3: SM demand 1..S/2 units, memory
+    6-40 % of a GPU (3-14 B parameter models plus KV), preferred frequency one of the table's levels."""
+    st = Stream(seed, "plan")
+    l = np.zeros(n, dtype=PLAN_LLM_DT)
+    l["need_units"] = st.randint(n, 1, max(S // 2, 1))
+    l["mem_mb"] = (st.urange(n, 0.06, 0.40) * mem_cap).astype(np.float32)
+    l["f_mhz"] = np.asarray(freq_mhz, dtype=np.float32)[st.randint(n, 0, len(freq_mhz) - 1)]
+    l["t_ms"] = st.urange(n, 50.0, 5000.0).astype(np.float32)
     return l
 
 
