@@ -145,6 +145,10 @@ typedef struct {
   float sm_units; int16_t need_units, phi_l; float t_l_ms, e_l_mj, mem_mb; uint32_t _pad;
 } fs_llm_profile;
 
+/* LLM descriptor of Algorithm 1: l.S = need_units (share units, >= 1), l.M = mem_mb,
+ * l.F = f_mhz (preferred frequency), t_ms = its execution time (the weight of Eq. 5).  16 bytes. */
+typedef struct { int32_t need_units; float mem_mb, f_mhz, t_ms; } fs_plan_llm;
+
 /* One runnable task of the local scheduler's priority queue (Fig. 8 steps 1-2): a
  * decode step or a prefill unit of `model`, run with `sigma`+1 SM share units at batch bucket
  * `beta`.  slack_ms = remaining time to its SLO deadline (TBT for decode, TTFT for prefill),
@@ -239,6 +243,19 @@ int fs_llm_profiles(fs_ctx* ctx, int32_t n, const fs_llm* llms, fs_llm_profile* 
  * binary64 (sums over the LLMs; EWR = 0 when E_optimal = 0).  All pointers in `space`.           */
 int fs_ewr(fs_ctx* ctx, int32_t n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms,
            int32_t K, float* f_gpu, double* out3, int space, void* cuda_stream);
+
+/* Algorithm 1, phases 2-3 for n active LLMs against the effective capacities
+ * s_eff (share units) and m_eff (MB) of one GPU ((1 - delta) of the real ones).
+ * Phase 2: summary[0] = N_sm, summary[1] = N_mem (Best-Fit-Decreasing bin counts), summary[2] =
+ * N_min = their maximum.  Phase 3: the LLMs in ascending f_mhz go to the GPU with the closest
+ * operating frequency (the highest f_mhz on it; an empty GPU is the last resort) if they fit;
+ * else the target's lowest-frequency resident moves to the second-closest GPU when that is
+ * resource-valid and lowers the waste of Eq. 5; else the second-closest GPU; else the closest other GPU
+ * that fits; else a new GPU.  gpu_of[l] = the GPU of LLM l (-1: it exceeds a whole GPU);
+ * summary[3] = GPUs in use or planned (>= N_min).  Ties: lower index everywhere.
+ * llms : [n]; gpu_of : [n]; summary : [4]; all in `space`.  need_units < 1 raises FS_ERR_RANGE.   */
+int fs_replace_plan(fs_ctx* ctx, int32_t n, const fs_plan_llm* llms, int32_t s_eff, float m_eff,
+                    int32_t* gpu_of, int32_t* summary, int space, void* cuda_stream);
 
 /* Diagnostics. */
 const char* fs_strerror(int code);

@@ -23,7 +23,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm", "batch_tasks", "dispatch")
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
     L.fs_place_batch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_local_config.argtypes = [vp, i32, vp, u32, vp, C.c_int, vp]
     L.fs_consolidate.argtypes = [vp, vp, C.c_int, vp]
+    L.fs_replace_plan.argtypes = [vp, i32, vp, i32, C.c_float, vp, vp, C.c_int, vp]
     L.fs_llm_profiles.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_ewr.argtypes = [vp, i32, vp, vp, vp, i32, vp, vp, C.c_int, vp]
     L.fs_dispatch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
@@ -261,6 +262,17 @@ class Festina:
                           _stream_ptr(stream))
         self._check(rc, "fs_ewr")
         return fg[:K], float(out[0]), float(out[1]), float(out[2])
+
+    def replace_plan(self, llms, s_eff: int, m_eff: float, stream=None):
+        """fs_replace_plan on host arrays: returns (gpu_of [n], (N_sm, N_mem, N_min, N_active))."""
+        llms = np.ascontiguousarray(llms)
+        gpu_of = np.full(max(len(llms), 1), -1, dtype=np.int32)
+        summ = np.zeros(4, dtype=np.int32)
+        p = lambda a: C.c_void_p(a.ctypes.data)
+        rc = lib().fs_replace_plan(self._h, len(llms), p(llms) if len(llms) else C.c_void_p(0), s_eff, m_eff,
+                                   p(gpu_of), p(summ), FS_HOST, _stream_ptr(stream))
+        self._check(rc, "fs_replace_plan")
+        return gpu_of[:len(llms)], tuple(int(x) for x in summ)
 
     def consolidate(self, out=None, stream=None):
         if out is None:

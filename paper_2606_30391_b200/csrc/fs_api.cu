@@ -37,7 +37,7 @@ struct fs_ctx {
   // task batching scratch (FS_HOST staging)
   int bt_n_cap = 0, bt_t_cap = 0; int32_t *bt_ids = nullptr, *bt_off = nullptr; fs_task* bt_tasks = nullptr; fs_task_out* bt_out = nullptr;
   // Algorithm 1 / EWR scratch (FS_HOST staging)
-  size_t a1_cap = 0; unsigned char* a1_buf = nullptr;
+  size_t a1_cap = 0; unsigned char* a1_buf = nullptr; size_t pl_cap = 0; unsigned char* pl_buf = nullptr;
   // consolidation scratch
   size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
   unsigned long long* ckeys = nullptr; fs_consol_out* consol_dev = nullptr;
@@ -159,7 +159,7 @@ int fs_destroy(fs_ctx* c) {
   void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
-                  c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf};
+                  c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf, c->pl_buf};
   for (void* p : ptrs) if (p) cudaFree(p);
   if (c->flag_host) cudaFreeHost(c->flag_host);
   if (c->have_events)
@@ -440,6 +440,36 @@ int fs_ewr(fs_ctx* c, int32_t n, const int32_t* gpu_of, const float* f_mhz, cons
   if (space == FS_HOST) {
     if (K > 0) FS_CUDA(c, cudaMemcpyAsync(f_gpu, d_fg, (size_t)K * 4, cudaMemcpyDeviceToHost, st));
     FS_CUDA(c, cudaMemcpyAsync(out3, d_o, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+int fs_replace_plan(fs_ctx* c, int32_t n, const fs_plan_llm* llms, int32_t s_eff, float m_eff,
+                    int32_t* gpu_of, int32_t* summary, int space, void* cuda_stream) {
+  if (!c || n < 0 || !summary || (n > 0 && (!llms || !gpu_of)) || s_eff < 1 || s_eff > FS_MAX_S) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  const size_t sb = fsk_plan_scratch_bytes(n);
+  if (sb > c->pl_cap) { FS_TRY(grow(c, c->pl_buf, sb)); c->pl_cap = sb; }
+  const fs_plan_llm* d_in = llms; int32_t* d_g = gpu_of; int32_t* d_s = summary;
+  if (space == FS_HOST) {
+    const size_t nn = (size_t)n;
+    FS_TRY(a1_reserve(c, 16 + nn * (sizeof(fs_plan_llm) + 4)));
+    d_s = reinterpret_cast<int32_t*>(c->a1_buf);
+    d_in = reinterpret_cast<fs_plan_llm*>(c->a1_buf + 16);
+    d_g = reinterpret_cast<int32_t*>(c->a1_buf + 16 + nn * sizeof(fs_plan_llm));
+    if (n > 0) FS_CUDA(c, cudaMemcpyAsync((void*)d_in, llms, nn * sizeof(fs_plan_llm), cudaMemcpyHostToDevice, st));
+  }
+  c->launches += fsk_replace_plan(n, d_in, s_eff, m_eff, c->pl_buf, d_g, d_s, c->flag_dev, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    if (n > 0) FS_CUDA(c, cudaMemcpyAsync(gpu_of, d_g, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaMemcpyAsync(summary, d_s, 16, cudaMemcpyDeviceToHost, st));
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;

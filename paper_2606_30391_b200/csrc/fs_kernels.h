@@ -104,6 +104,11 @@ int fsk_llm_profile(const FsView& v, int n, const fs_llm* llms, fs_llm_profile* 
 int fsk_ewr(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, int K, float* fg, double* out3,
             int* flag, cudaStream_t st);
 
+// fs_plan.cu — Algorithm 1 phases 2-3 (sequential part): one warp
+size_t fsk_plan_scratch_bytes(int n);
+int fsk_replace_plan(int n, const fs_plan_llm* llms, int s_eff, float m_eff, void* scratch, int32_t* gpu_of,
+                     int32_t* summary, int* flag, cudaStream_t st);
+
 #ifdef __CUDACC__
 // One co-resident ("tenant") at frequency phi with share sigma, wait = 0 because its slo is the
 // REMAINING slack (R:s12).  bump = one more sequence joins its decode batch: the decode bucket

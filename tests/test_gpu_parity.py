@@ -445,3 +445,50 @@ def test_ewr(ctx):
         assert abs(w - rw) <= 1e-12 * abs(rw) and abs(o - ro) <= 1e-12 * abs(ro) and abs(r - rr) <= 1e-12 * abs(rr)
     fg, w, o, r = ctx.ewr([0, 0, 1, -1], [1000, 1500, 1200, 900], [1, 2, 3, 4], 2)
     assert list(fg) == [1500.0, 1200.0] and w == 1500.0 ** 3 - 1000.0 ** 3 and r == w / o
+
+
+# ---- Algorithm 1 phases 2-3 (fs_replace_plan) ------------------------------------------------------
+@pytest.mark.parametrize("seed", range(10))
+def test_replace_plan(ctx, seed):
+    freq = np.linspace(210, 1980, [4, 16, 64][seed % 3]).astype(np.float32)
+    S = [8, 16, 32][seed % 3]
+    s_eff, m_eff = (S * 95) // 100, 76000.0
+    n = [0, 1, 7, 33, 100, 257, 600, 64, 31, 1000][seed]
+    l = synth.make_plan_llms(seed, n, S, freq)
+    if seed % 4 == 3 and n:
+        l["mem_mb"][::7] = 90000.0                  # exceed a whole GPU: stay unplaced
+        l["need_units"][3::11] = s_eff + 1
+    if seed == 4:
+        l["f_mhz"] = freq[0]                        # all frequencies equal: index tie-breaks everywhere
+    gpu_of, summ = ctx.replace_plan(l, s_eff, m_eff)
+    rg, rs = oracle.replace_plan(l, s_eff, m_eff)
+    assert summ == rs, (summ, rs)
+    assert np.array_equal(gpu_of, rg)
+
+
+def test_replace_plan_fig9(ctx):
+    """The hand-built swap case of tests/test_oracle_plan.py through the CUDA path."""
+    l = np.zeros(4, dtype=synth.PLAN_LLM_DT)
+    l["need_units"] = 1; l["mem_mb"] = [30, 30, 30, 40]; l["f_mhz"] = [900, 1000, 1400, 1500]; l["t_ms"] = 10
+    gpu_of, summ = ctx.replace_plan(l, 10, 100.0)
+    assert list(gpu_of) == [1, 0, 0, 0] and summ == (1, 2, 2, 2)
+    l["mem_mb"][3] = 50
+    assert list(ctx.replace_plan(l, 10, 100.0)[0]) == [0, 0, 0, 1]
+
+
+def test_replace_plan_from_profiles(ctx, fs):
+    """Phase 1 feeds phases 2-3: profiles of 512 LLMs on the rack tables -> plan -> EWR, all on the GPU path."""
+    cl = synth.make_cluster("rack")
+    ctx.load_cluster(cl)
+    llms = synth.make_llms(4, 512, cl.M)
+    pr = ctx.llm_profiles(llms)
+    ok = pr["phi_l"] >= 0
+    pl = np.zeros(int(ok.sum()), dtype=synth.PLAN_LLM_DT)
+    pl["need_units"] = pr["need_units"][ok]; pl["mem_mb"] = pr["mem_mb"][ok]
+    pl["f_mhz"] = cl.freq_mhz[pr["phi_l"][ok]]; pl["t_ms"] = pr["t_l_ms"][ok]
+    s_eff, m_eff = (cl.S * 95) // 100, 76000.0
+    gpu_of, summ = ctx.replace_plan(pl, s_eff, m_eff)
+    rg, rs = oracle.replace_plan(pl, s_eff, m_eff)
+    assert summ == rs and np.array_equal(gpu_of, rg)
+    fg, w, o, r = ctx.ewr(gpu_of, pl["f_mhz"], pl["t_ms"], summ[3])
+    assert abs(r - oracle.ewr(gpu_of, pl["f_mhz"], pl["t_ms"], summ[3])[3]) <= 1e-12 * max(r, 1e-300)
