@@ -137,6 +137,27 @@ def replace_plan(llms, s_eff: int, m_eff: float):
     return gpu_of, tuple(int(x) for x in summ)
 
 
+def assign(bytes_mb, bw_mb_per_ms):
+    """Minimum-cost source -> destination assignment, costs in whole microseconds."""
+    bytes_mb = np.ascontiguousarray(bytes_mb, dtype=np.float32)
+    bw = np.ascontiguousarray(bw_mb_per_ms, dtype=np.float32)
+    n = len(bytes_mb)
+    assert bw.shape == (n, n)
+    dst = np.full(max(n, 1), -1, dtype=np.int32)
+    tot = np.zeros(1, dtype=np.int64)
+    lib().fo_assign(C.c_int(n), _p(bytes_mb), _p(bw), _p(dst), _p(tot))
+    return dst[:n], int(tot[0])
+
+
+def migration_select(reqs):
+    """Finish locally vs migrate, tokens vs KV: returns (flags u8, migration ms)."""
+    reqs = np.ascontiguousarray(reqs)
+    out = np.zeros(max(len(reqs), 1), dtype=np.uint8)
+    ms = np.zeros(max(len(reqs), 1), dtype=np.float32)
+    lib().fo_migration_select(C.c_int(len(reqs)), _p(reqs), _p(out), _p(ms))
+    return out[:len(reqs)], ms[:len(reqs)]
+
+
 def slot(lat, pow_, m, p, phi, sigma, beta, q, wait, slo):
     """The shared slot rule: returns (ok, t, e)."""
     t = C.c_float(0)

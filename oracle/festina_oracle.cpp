@@ -23,6 +23,8 @@
 //                           forms (0 iff aligned, two-LLM case by hand)
 //   Alg. 1 phases 2-3 ..... BFD against brute-force optimal bin counts on tiny inputs (OPT <= BFD <=
 //                           11/9 OPT + 1), a Fig. 9-shaped swap case by hand, capacity invariants
+//   migration plan ........ brute force over all permutations (n <= 7), scipy's linear_sum_assignment,
+//                           hand-built rule cases
 //   priority batching ..... Fig. 8 steps 1-2 worked table, independent numpy
 //                           restatement, budget / bypass invariants
 // Nothing here is "parity unpinned".
@@ -454,6 +456,57 @@ void replace_plan(const PlanLlm* L, int n, int s_eff, float m_eff, int32_t* gpu_
 }
 
 // ------------------------------------------------------------------------------------------
+// Appendix E: transmission plan and selective request migration.
+//   e_uv = Bytes(u -> v) / BW(u, v); minimum-cost assignment of sources to destinations by the
+//   Kuhn-Munkres algorithm.  Costs are taken in whole microseconds, c_uv = rint(fl(fl(bytes_u / bw_uv) * 1000))
+//   with bytes in MB and bw in MB/ms (reading s33), so the optimum is an exact integer.
+//   Shortest-augmenting-path form with row / column potentials; ties: lowest column.
+void assign_min_cost(int n, const float* bytes_mb, const float* bw, int32_t* dst_of, int64_t* total_us) {
+  const int64_t BIG = (int64_t)1 << 60;
+  auto cost = [&](int u, int v) { return (int64_t)std::llrint((bytes_mb[u] / bw[(size_t)u * n + v]) * 1000.0f); };
+  std::vector<int64_t> pu(n + 1, 0), pv(n + 1, 0), minv(n + 1);
+  std::vector<int> p(n + 1, 0), way(n + 1, 0);               // p[j] = row matched to column j (1-based, 0 = none)
+  for (int i = 1; i <= n; ++i) {
+    p[0] = i; int j0 = 0;
+    std::vector<char> used(n + 1, 0);
+    for (int j = 0; j <= n; ++j) minv[j] = BIG;
+    do {
+      used[j0] = 1;
+      const int i0 = p[j0]; int64_t delta = BIG; int j1 = 0;
+      for (int j = 1; j <= n; ++j) if (!used[j]) {
+        const int64_t cur = cost(i0 - 1, j - 1) - pu[i0] - pv[j];
+        if (cur < minv[j]) { minv[j] = cur; way[j] = j0; }
+        if (minv[j] < delta) { delta = minv[j]; j1 = j; }
+      }
+      for (int j = 0; j <= n; ++j) {
+        if (used[j]) { pu[p[j]] += delta; pv[j] -= delta; } else minv[j] -= delta;
+      }
+      j0 = j1;
+    } while (p[j0] != 0);
+    do { const int j1 = way[j0]; p[j0] = p[j1]; j0 = j1; } while (j0);
+  }
+  int64_t tot = 0;
+  for (int j = 1; j <= n; ++j) { dst_of[p[j] - 1] = j - 1; }
+  for (int u = 0; u < n; ++u) tot += cost(u, dst_of[u]);
+  *total_us = tot;
+}
+
+// Per in-flight request: KV is transferred iff that is faster than recomputing it on the
+// destination; the request migrates iff its remaining computation on the source exceeds the migration
+// time; otherwise it finishes in place.  out: bit 0 = migrate, bit 1 = transfer KV (else tokens only).
+struct MigReq { float remaining_ms, tokens_mb, kv_mb, bw_mb_per_ms, recompute_ms; uint32_t pad[3]; };
+static_assert(sizeof(MigReq) == 32, "layout");
+void migration_select(int r, const MigReq* q, uint8_t* out, float* mig_ms) {
+  for (int i = 0; i < r; ++i) {
+    const float kv_tx = q[i].kv_mb / q[i].bw_mb_per_ms;
+    const bool kv = kv_tx < q[i].recompute_ms;
+    const float t = (q[i].tokens_mb / q[i].bw_mb_per_ms) + (kv ? kv_tx : q[i].recompute_ms);
+    mig_ms[i] = t;
+    out[i] = (uint8_t)((q[i].remaining_ms > t ? 1 : 0) | (kv ? 2 : 0));
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // fs_local_config: frequency sweep with per-task SM allocation (Fig. 8 step 3,
 // P:206-210); batching P:248; objective R:s8; split domain R:s9; one beta per slot R:s10.
 // Hierarchical definition: best beta per slot, then tenant sums, then the argmin.
@@ -717,6 +770,15 @@ int fo_ewr(int n, const int32_t* gpu_of, const float* f_mhz, const float* t_ms, 
 
 int fo_replace_plan(int n, const void* llms, int s_eff, float m_eff, int32_t* gpu_of, int32_t* summary4) {
   replace_plan((const PlanLlm*)llms, n, s_eff, m_eff, gpu_of, summary4);
+  return 0;
+}
+
+int fo_assign(int n, const float* bytes_mb, const float* bw, int32_t* dst_of, int64_t* total_us) {
+  assign_min_cost(n, bytes_mb, bw, dst_of, total_us);
+  return 0;
+}
+int fo_migration_select(int r, const void* reqs, uint8_t* out, float* mig_ms) {
+  migration_select(r, (const MigReq*)reqs, out, mig_ms);
   return 0;
 }
 

@@ -46,6 +46,9 @@ LLM_PROFILE_DT = np.dtype([("sigma_p", "<i2"), ("phi_p", "<i2"), ("sigma_d", "<i
                            ("sm_units", "<f4"), ("need_units", "<i2"), ("phi_l", "<i2"), ("t_l_ms", "<f4"),
                            ("e_l_mj", "<f4"), ("mem_mb", "<f4"), ("_pad", "<u4")])
 assert TASK_DT.itemsize == 24 and TASK_OUT_DT.itemsize == 16
+MIG_REQ_DT = np.dtype([("remaining_ms", "<f4"), ("tokens_mb", "<f4"), ("kv_mb", "<f4"), ("bw_mb_per_ms", "<f4"),
+                       ("recompute_ms", "<f4"), ("_pad", "<u4", (3,))])
+assert MIG_REQ_DT.itemsize == 32
 PLAN_LLM_DT = np.dtype([("need_units", "<i4"), ("mem_mb", "<f4"), ("f_mhz", "<f4"), ("t_ms", "<f4")])
 assert LLM_DT.itemsize == 32 and LLM_PROFILE_DT.itemsize == 48 and PLAN_LLM_DT.itemsize == 16
 
@@ -362,6 +365,25 @@ def make_plan_llms(seed: int, n: int, S: int, freq_mhz: np.ndarray, mem_cap: flo
     l["f_mhz"] = np.asarray(freq_mhz, dtype=np.float32)[st.randint(n, 0, len(freq_mhz) - 1)]
     l["t_ms"] = st.urange(n, 50.0, 5000.0).astype(np.float32)
     return l
+
+
+def make_migration(seed: int, n: int, r: int):
+    """State sizes and link bandwidths for the transmission plan (Appendix E): n sources with
+    6-60 GB of weights + KV, bandwidth 450 MB/ms inside a node of 8 (NVLink 5 class), 25-50 MB/ms across
+    nodes, a source mapped onto itself moves nothing faster (bw = 1e6); and r in-flight requests."""
+    st = Stream(seed, "migration")
+    bytes_mb = st.urange(n, 6000.0, 60000.0).astype(np.float32)
+    node = np.arange(n) // 8
+    same = node[:, None] == node[None, :]
+    bw = np.where(same, 450.0, st.urange(n * n, 25.0, 50.0).reshape(n, n)).astype(np.float32)
+    bw[np.arange(n), np.arange(n)] = 1e6
+    q = np.zeros(r, dtype=MIG_REQ_DT)
+    q["remaining_ms"] = np.exp(4.0 + 2.0 * st.normal(r)).astype(np.float32)
+    q["tokens_mb"] = st.urange(r, 0.001, 0.05).astype(np.float32)
+    q["kv_mb"] = st.urange(r, 10.0, 3000.0).astype(np.float32)
+    q["bw_mb_per_ms"] = np.where(st.uniform(r) < 0.5, 450.0, 40.0).astype(np.float32)
+    q["recompute_ms"] = st.urange(r, 5.0, 400.0).astype(np.float32)
+    return bytes_mb, bw, q
 
 
 def arrival_ticks(seed: int, R: int, n_ticks: int, rho: float = 3.3) -> np.ndarray:
