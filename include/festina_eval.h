@@ -149,6 +149,13 @@ typedef struct {
  * l.F = f_mhz (preferred frequency), t_ms = its execution time (the weight of Eq. 5).  16 bytes. */
 typedef struct { int32_t need_units; float mem_mb, f_mhz, t_ms; } fs_plan_llm;
 
+/* One in-flight request at reconfiguration time: remaining computation on the source,
+ * token state and KV-cache size, the bandwidth of its source -> destination link under the chosen
+ * mapping, and the time to recompute its KV cache on the destination.  32 bytes.               */
+typedef struct { float remaining_ms, tokens_mb, kv_mb, bw_mb_per_ms, recompute_ms; uint32_t _pad[3]; } fs_mig_req;
+#define FS_MIG_MIGRATE 1u   /* else: finish on the source */
+#define FS_MIG_KV 2u        /* transfer the KV cache; else tokens only and recompute */
+
 /* One runnable task of the local scheduler's priority queue (Fig. 8 steps 1-2): a
  * decode step or a prefill unit of `model`, run with `sigma`+1 SM share units at batch bucket
  * `beta`.  slack_ms = remaining time to its SLO deadline (TBT for decode, TTFT for prefill),
@@ -256,6 +263,18 @@ int fs_ewr(fs_ctx* ctx, int32_t n, const int32_t* gpu_of, const float* f_mhz, co
  * llms : [n]; gpu_of : [n]; summary : [4]; all in `space`.  need_units < 1 raises FS_ERR_RANGE.   */
 int fs_replace_plan(fs_ctx* ctx, int32_t n, const fs_plan_llm* llms, int32_t s_eff, float m_eff,
                     int32_t* gpu_of, int32_t* summary, int space, void* cuda_stream);
+
+/* Transmission plan: minimum-cost assignment of n sources to n destinations under
+ * e_uv = Bytes(u -> v) / BW(u, v), costs in whole microseconds rint(fl(fl(bytes_mb[u] / bw[u][v]) * 1000))
+ * (bytes in MB, bw in MB per ms, row-major [n][n], > 0), Kuhn-Munkres, exact in int64.
+ * dst_of[u] = destination of source u; *total_us = the minimum total cost.  n <= 1024.           */
+int fs_migration_plan(fs_ctx* ctx, int32_t n, const float* bytes_mb, const float* bw_mb_per_ms,
+                      int32_t* dst_of, int64_t* total_us, int space, void* cuda_stream);
+/* Selective request migration for r in-flight requests: flags[i] = FS_MIG_KV if sending the
+ * KV cache (kv_mb / bw) is faster than recomputing it, | FS_MIG_MIGRATE if the remaining computation on
+ * the source exceeds the migration time mig_ms[i] = tokens_mb / bw + min-option above.          */
+int fs_migration_select(fs_ctx* ctx, int32_t r, const fs_mig_req* reqs, uint8_t* flags, float* mig_ms,
+                        int space, void* cuda_stream);
 
 /* Diagnostics. */
 const char* fs_strerror(int code);

@@ -23,7 +23,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_migration_plan", "fs_migration_select", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm", "batch_tasks", "dispatch")
@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
     L.fs_place_batch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_local_config.argtypes = [vp, i32, vp, u32, vp, C.c_int, vp]
     L.fs_consolidate.argtypes = [vp, vp, C.c_int, vp]
+    L.fs_migration_plan.argtypes = [vp, i32, vp, vp, vp, vp, C.c_int, vp]
+    L.fs_migration_select.argtypes = [vp, i32, vp, vp, vp, C.c_int, vp]
     L.fs_replace_plan.argtypes = [vp, i32, vp, i32, C.c_float, vp, vp, C.c_int, vp]
     L.fs_llm_profiles.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_ewr.argtypes = [vp, i32, vp, vp, vp, i32, vp, vp, C.c_int, vp]
@@ -273,6 +275,29 @@ class Festina:
                                    p(gpu_of), p(summ), FS_HOST, _stream_ptr(stream))
         self._check(rc, "fs_replace_plan")
         return gpu_of[:len(llms)], tuple(int(x) for x in summ)
+
+    def migration_plan(self, bytes_mb, bw_mb_per_ms, stream=None):
+        """fs_migration_plan on host arrays: returns (dst_of [n], total cost in microseconds)."""
+        bytes_mb = np.ascontiguousarray(bytes_mb, dtype=np.float32)
+        bw = np.ascontiguousarray(bw_mb_per_ms, dtype=np.float32)
+        n = len(bytes_mb)
+        dst = np.full(max(n, 1), -1, dtype=np.int32)
+        tot = np.zeros(1, dtype=np.int64)
+        p = lambda a: C.c_void_p(a.ctypes.data)
+        rc = lib().fs_migration_plan(self._h, n, p(bytes_mb), p(bw), p(dst), p(tot), FS_HOST, _stream_ptr(stream))
+        self._check(rc, "fs_migration_plan")
+        return dst[:n], int(tot[0])
+
+    def migration_select(self, reqs, stream=None):
+        """fs_migration_select on host arrays: returns (flags u8, migration time ms)."""
+        reqs = np.ascontiguousarray(reqs)
+        r = len(reqs)
+        flags = np.zeros(max(r, 1), dtype=np.uint8)
+        ms = np.zeros(max(r, 1), dtype=np.float32)
+        p = lambda a: C.c_void_p(a.ctypes.data)
+        rc = lib().fs_migration_select(self._h, r, p(reqs), p(flags), p(ms), FS_HOST, _stream_ptr(stream))
+        self._check(rc, "fs_migration_select")
+        return flags[:r], ms[:r]
 
     def consolidate(self, out=None, stream=None):
         if out is None:

@@ -477,6 +477,66 @@ int fs_replace_plan(fs_ctx* c, int32_t n, const fs_plan_llm* llms, int32_t s_eff
   return pending;
 }
 
+int fs_migration_plan(fs_ctx* c, int32_t n, const float* bytes_mb, const float* bw, int32_t* dst_of,
+                      int64_t* total_us, int space, void* cuda_stream) {
+  if (!c || n < 0 || !total_us || (n > 0 && (!bytes_mb || !bw || !dst_of))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (n > 1024) return FS_ERR_SHAPE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  const float *d_b = bytes_mb, *d_w = bw; int32_t* d_d = dst_of; long long* d_t = reinterpret_cast<long long*>(total_us);
+  if (space == FS_HOST) {
+    const size_t nn = (size_t)n;
+    FS_TRY(a1_reserve(c, 16 + nn * 8 + nn * nn * 4));
+    d_t = reinterpret_cast<long long*>(c->a1_buf);
+    d_b = reinterpret_cast<float*>(c->a1_buf + 16); d_d = reinterpret_cast<int32_t*>(c->a1_buf + 16 + nn * 4);
+    d_w = reinterpret_cast<float*>(c->a1_buf + 16 + nn * 8);
+    if (n > 0) {
+      FS_CUDA(c, cudaMemcpyAsync((void*)d_b, bytes_mb, nn * 4, cudaMemcpyHostToDevice, st));
+      FS_CUDA(c, cudaMemcpyAsync((void*)d_w, bw, nn * nn * 4, cudaMemcpyHostToDevice, st));
+    }
+  }
+  c->launches += fsk_assign(n, d_b, d_w, d_d, d_t, c->flag_dev, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    if (n > 0) FS_CUDA(c, cudaMemcpyAsync(dst_of, d_d, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaMemcpyAsync(total_us, d_t, 8, cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
+int fs_migration_select(fs_ctx* c, int32_t r, const fs_mig_req* reqs, uint8_t* flags, float* mig_ms, int space,
+                        void* cuda_stream) {
+  if (!c || r < 0 || (r > 0 && (!reqs || !flags || !mig_ms))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (r == 0) return pending;
+  const fs_mig_req* d_q = reqs; uint8_t* d_f = flags; float* d_m = mig_ms;
+  if (space == FS_HOST) {
+    const size_t rr = (size_t)r;
+    FS_TRY(a1_reserve(c, rr * (sizeof(fs_mig_req) + 4 + 1) + 16));
+    d_q = reinterpret_cast<fs_mig_req*>(c->a1_buf); d_m = reinterpret_cast<float*>(c->a1_buf + rr * sizeof(fs_mig_req));
+    d_f = c->a1_buf + rr * (sizeof(fs_mig_req) + 4);
+    FS_CUDA(c, cudaMemcpyAsync((void*)d_q, reqs, rr * sizeof(fs_mig_req), cudaMemcpyHostToDevice, st));
+  }
+  c->launches += fsk_migration_select(r, d_q, d_f, d_m, st);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    FS_CUDA(c, cudaMemcpyAsync(flags, d_f, (size_t)r, cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaMemcpyAsync(mig_ms, d_m, (size_t)r * 4, cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
 int fs_batch_tasks(fs_ctx* c, int32_t n, const int32_t* gpu_ids, const int32_t* task_off,
                    const fs_task* tasks, fs_task_out* out, int32_t n_tasks, int space, void* cuda_stream) {
   if (!c || n < 0 || n_tasks < 0 || (n > 0 && !task_off) || (n_tasks > 0 && (!tasks || !out))) return FS_ERR_ARG;

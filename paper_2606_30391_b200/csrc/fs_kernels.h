@@ -109,6 +109,11 @@ size_t fsk_plan_scratch_bytes(int n);
 int fsk_replace_plan(int n, const fs_plan_llm* llms, int s_eff, float m_eff, void* scratch, int32_t* gpu_of,
                      int32_t* summary, int* flag, cudaStream_t st);
 
+// fs_migrate.cu — Appendix E: transmission plan (Kuhn-Munkres) and selective migration
+int fsk_assign(int n, const float* bytes_mb, const float* bw, int32_t* dst_of, long long* total_us, int* flag,
+               cudaStream_t st);
+int fsk_migration_select(int r, const fs_mig_req* q, uint8_t* out, float* mig_ms, cudaStream_t st);
+
 #ifdef __CUDACC__
 // One co-resident ("tenant") at frequency phi with share sigma, wait = 0 because its slo is the
 // REMAINING slack (R:s12).  bump = one more sequence joins its decode batch: the decode bucket

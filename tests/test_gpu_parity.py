@@ -492,3 +492,29 @@ def test_replace_plan_from_profiles(ctx, fs):
     assert summ == rs and np.array_equal(gpu_of, rg)
     fg, w, o, r = ctx.ewr(gpu_of, pl["f_mhz"], pl["t_ms"], summ[3])
     assert abs(r - oracle.ewr(gpu_of, pl["f_mhz"], pl["t_ms"], summ[3])[3]) <= 1e-12 * max(r, 1e-300)
+
+
+# ---- Appendix E: transmission plan and selective migration ------------------------------------------
+@pytest.mark.parametrize("n", [0, 1, 2, 7, 33, 120, 300])
+def test_migration_plan(ctx, n):
+    bytes_mb, bw, q = synth.make_migration(n, n, 10 * n)
+    if n == 33:
+        bw = np.round(bw / 25.0) * 25.0 + 25.0      # many equal costs: the tie rule decides the assignment
+    dst, tot = ctx.migration_plan(bytes_mb, bw)
+    rdst, rtot = oracle.assign(bytes_mb, bw)
+    assert tot == rtot and np.array_equal(dst, rdst)
+    assert sorted(dst) == list(range(n))            # a permutation whatever the tie-breaks
+    flags, ms = ctx.migration_select(q)
+    rflags, rms = oracle.migration_select(q)
+    assert np.array_equal(flags, rflags) and np.array_equal(ms.view(np.uint32), rms.view(np.uint32))
+
+
+def test_migration_plan_against_scipy(ctx):
+    """The total is unique even where the assignment is not: check the CUDA path against a library solver."""
+    from scipy.optimize import linear_sum_assignment
+    bytes_mb, bw, _ = synth.make_migration(77, 64, 0)
+    dst, tot = ctx.migration_plan(bytes_mb, bw)
+    t = (bytes_mb[:, None] / bw).astype(np.float32)
+    c = np.rint((t * np.float32(1000.0)).astype(np.float32)).astype(np.int64)
+    rows, cols = linear_sum_assignment(c)
+    assert tot == int(c[rows, cols].sum()) == int(c[np.arange(64), dst].sum())
