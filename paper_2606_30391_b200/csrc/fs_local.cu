@@ -240,6 +240,7 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
   __syncthreads();
   const bool minsm = flags & FS_SPLIT_MINSM;
   unsigned long long key = FS_KEY_NONE;
+  uint32_t fphi = 0xFFFFFFFFu;
   const uint32_t NS = minsm ? 1u : comp_n[n_res - 1];
   if (minsm) {
     for (int phi = threadIdx.x; phi < d.F; phi += blockDim.x) {
@@ -255,6 +256,7 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
       if (all && tot <= d.S && C < FS_INF) {
         const unsigned long long kk = fs_make_key(C, (uint32_t)phi);
         key = kk < key ? kk : key;
+        fphi = min(fphi, (uint32_t)phi);
       }
     }
   } else {
@@ -271,43 +273,12 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
       if (C < FS_INF) {
         const unsigned long long kk = fs_make_key(C, c);
         key = kk < key ? kk : key;
+        fphi = min(fphi, phi);
       }
     }
   }
-  // f_req = lowest phi with any feasible candidate: min over the low word / NS of feasible keys
-  // is not the key minimum, so reduce it separately as a key with value 0.
-  unsigned long long fkey = FS_KEY_NONE;
-  if (minsm) {
-    // feasible phis were exactly those that produced a key; recompute cheaply per thread
-    for (int phi = threadIdx.x; phi < d.F; phi += blockDim.x) {
-      int tot = 0; bool all = true; float C = 0.0f;
-      for (int i = 0; i < n_res; ++i) {
-        int sg = -1;
-        for (int s = 0; s < d.S; ++s) if (sG[i * rows + phi * d.S + s] < FS_INF) { sg = s; break; }
-        if (sg < 0) { all = false; break; }
-        tot += sg + 1;
-        const float g = sG[i * rows + phi * d.S + sg];
-        C = (i == 0) ? g : __fadd_rn(C, g);
-      }
-      if (all && tot <= d.S && C < FS_INF) { fkey = (unsigned long long)phi; break; }
-    }
-  } else {
-    const uint32_t* cp = comp + (size_t)(n_res - 1) * ns_stride;
-    for (int phi = 0; phi < d.F && fkey == FS_KEY_NONE; ++phi) {
-      // all threads scan the splits of this phi together
-      bool any = false;
-      for (uint32_t rank = threadIdx.x; rank < NS && !any; rank += blockDim.x) {
-        const uint32_t pk = cp[rank];
-        float C = 0.0f;
-        for (int i = 0; i < n_res; ++i) {
-          const float g = sG[i * rows + phi * d.S + ((pk >> (8 * i)) & 0xFF)];
-          C = (i == 0) ? g : __fadd_rn(C, g);
-        }
-        any = C < FS_INF;
-      }
-      if (__syncthreads_or(any)) fkey = (unsigned long long)phi;
-    }
-  }
+  // f_req = lowest phi with any feasible candidate: tracked beside the key, reduced as a key of its own
+  unsigned long long fkey = fphi == 0xFFFFFFFFu ? FS_KEY_NONE : (unsigned long long)fphi;
   key = block_min_key(key, sred);
   fkey = block_min_key(fkey, sred);
   // ---- outputs.  The slot kernels keep only the minimum cost per (slot, phi, sigma); the batch

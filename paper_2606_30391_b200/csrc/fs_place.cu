@@ -246,7 +246,8 @@ __global__ void __launch_bounds__(DENSE_MAXW * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
                    unsigned int* __restrict__ ctr, const int32_t* __restrict__ warm_off,
-                   const FsWarmItem* __restrict__ witems, unsigned long long* __restrict__ stats) {
+                   const FsWarmItem* __restrict__ witems, unsigned long long* __restrict__ stats,
+                   fs_placement* __restrict__ out) {
   extern __shared__ __align__(128) unsigned char dense_smem_raw[];
   constexpr int FT = 32 * NPHI;
   constexpr uint32_t NONE32 = 0xFFFFFFFFu, INFBITS = 0x7F800000u;
@@ -293,7 +294,17 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     r = __shfl_sync(0xffffffffu, r, 0);
     if (r >= R) break;
     const ReqCtx c = make_req(v, reqs[r]);
-    if (!c.valid) { if (lane == 0 && slice == 0) fs_raise(v.flag, FS_FLAG_REQUEST); continue; }
+    if (!c.valid) {
+      if (lane == 0 && slice == 0) {
+        fs_raise(v.flag, FS_FLAG_REQUEST);
+        if (out) {
+          fs_placement o; o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
+          o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
+          out[r] = o;
+        }
+      }
+      continue;
+    }
     // ---- (a) the request's (sigma, phi) tiles, one row per share, and the pruning bounds:
     // every candidate of a GPU with sm_free = s has  er >= bnd[0][s-1], t0 >= bnd[1][s-1],
     // e0 >= bnd[2][s-1]; hence, for a cold pair,  dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)
@@ -498,7 +509,44 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     }
     unsigned long long key = flat != NONE32 ? fs_make_key(bestW, flat) : FS_KEY_NONE;
     key = fs_warp_min_key(key);
-    if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
+    if (out == nullptr) {                              // several slices: merge by key, decode afterwards
+      if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
+    } else {
+      // one slice: this warp saw every GPU, so it writes the placement record itself: the chosen
+      // share row is evaluated once more across phi by the definition for f_req (lowest feasible
+      // phi of the chosen (GPU, share)) and the chosen candidate's TTFT / TBT
+      fs_placement o; o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
+      o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
+      if (key != FS_KEY_NONE) {
+        const uint32_t fl = (uint32_t)key;
+        const int phis = fl % d.F, sgs = (fl / d.F) % d.S, ks = fl / (d.F * d.S);
+        const PairCtx p = make_pair(v, c, v.ginfo[ks]);
+        const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
+        const float* Ar = v.gA + ((size_t)ks * FS_NVAR + p.var) * d.F;
+        const float fr1 = __uint2float_rn(p.rounds1);
+        float tt[NPHI], b0[NPHI], a1[NPHI], b1[NPHI];
+        ld_tile<NPHI>(tl_t0 + sgs * FT + phi0, tt);
+        ld_cols<NPHI>(pw0, sgs * d.F, phi0, d.F, vec, b0);
+        ld_cols<NPHI>(l1, sgs * d.F, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, sgs * d.F, phi0, d.F, vec, b1);
+        uint32_t fmin = NONE32; float ttft = 0.0f, tbt = 0.0f;
+#pragma unroll
+        for (int i = 0; i < NPHI; ++i) {
+          const int phi = phi0 + i;
+          const float ar = phi < d.F ? Ar[phi] : FS_INF;
+          const float dE = __fsub_rn(__fadd_rn(ar, __fadd_rn(__fmul_rn(tt[i], b0[i]), __fmul_rn(__fmul_rn(fr1, a1[i]), b1[i]))), p.ecur);
+          const bool ok = (c.L == 0 || __fadd_rn(p.wait, tt[i]) <= c.slo_ttft) && (c.O == 0 || a1[i] <= c.slo_tbt) && dE < FS_INF;
+          if (ok) fmin = min(fmin, (uint32_t)phi);
+          if (phi == phis) { ttft = __fadd_rn(p.wait, tt[i]); tbt = a1[i]; }
+        }
+        fmin = warp_min_u32(fmin);
+        const int owner = phis / NPHI;
+        ttft = __shfl_sync(0xffffffffu, ttft, owner); tbt = __shfl_sync(0xffffffffu, tbt, owner);
+        o.gpu = ks; o.sigma = (int16_t)sgs; o.phi = (int16_t)phis; o.beta = (int16_t)p.br1;
+        o.f_req = (int16_t)(int)fmin; o.energy_mj = fs_unorderable((uint32_t)(key >> 32));
+        o.ttft_ms = ttft; o.tbt_ms = tbt; o.flat = fl;
+      }
+      if (lane == 0) out[r] = o;
+    }
     if (STATS) { n_req += 1; }
     if (STATS && __any_sync(0xffffffffu, ((n_chunks | n_elig | n_swept | n_cswept | n_witems | n_scored | n_cscored | n_req) >> 30) != 0u)) {
       flush_stats(stats, n_chunks, n_elig, n_swept, n_cswept, n_witems, n_scored, n_cscored, n_req);
@@ -793,9 +841,9 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
               const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (R <= 0) return 0;
   int launches = 0;
-  cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
   if (sc.count_work) cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 8, st);
   if (v.K <= 0) {
+    cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
   }
@@ -821,14 +869,19 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     const int grid = streams * nslice;
     const size_t smem = dense_smem_bytes(cps * FS_CHUNK, W, v.d.S, FT);
     cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nslice, st);
+    // one slice: the scoring kernel writes the placement records itself (no key array, no decode launch)
+    fs_placement* direct = nslice == 1 ? out : nullptr;
+    if (!direct) cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
 #define FS_LAUNCH_DENSE(NP, ST) \
-  place_dense_kernel<NP, ST><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats)
+  place_dense_kernel<NP, ST><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats, direct)
     if (FT == 32) { if (sc.count_work) FS_LAUNCH_DENSE(1, true); else FS_LAUNCH_DENSE(1, false); }
     else          { if (sc.count_work) FS_LAUNCH_DENSE(2, true); else FS_LAUNCH_DENSE(2, false); }
 #undef FS_LAUNCH_DENSE
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
+    if (direct) return launches;
   } else {
+    cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
     // split the GPUs of one request over several warps when R alone cannot fill the SMs
     const long long want_warps = (long long)sc.sm_count * 32;
     int nsplit = 1;
