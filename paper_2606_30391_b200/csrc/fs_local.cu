@@ -229,13 +229,12 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
   o.cost = o.energy_mj = o.power_w = FS_INF;
   if (n_res > d.S) { if (threadIdx.x == 0) out[gi] = o; return; }
   const float* g_in = Gs + (size_t)gi * (FS_RMAX * 2) * rows;
-  for (int x = threadIdx.x; x < n_res * rows; x += blockDim.x) {
-    const int i = x / rows, row = x % rows;
+  for (int i = 0; i < n_res; ++i) {
     // a slot with an empty queue costs 0 (the slot kernels do not visit it)
-    const fs_tenant& tt = v.states[k].t[i];
-    const float g0 = tt.q[0] ? g_in[(size_t)(i * 2) * rows + row] : 0.0f;
-    const float g1 = tt.q[1] ? g_in[(size_t)(i * 2 + 1) * rows + row] : 0.0f;
-    sG[x] = __fadd_rn(g0, g1);
+    const bool q0 = v.states[k].t[i].q[0] != 0, q1 = v.states[k].t[i].q[1] != 0;
+    const float* ga = g_in + (size_t)(i * 2) * rows; const float* gb = ga + rows;
+    for (int row = threadIdx.x; row < rows; row += blockDim.x)
+      sG[i * rows + row] = __fadd_rn(q0 ? ga[row] : 0.0f, q1 ? gb[row] : 0.0f);
   }
   __syncthreads();
   const bool minsm = flags & FS_SPLIT_MINSM;
@@ -261,21 +260,27 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
     }
   } else {
     const uint32_t* cp = comp + (size_t)(n_res - 1) * ns_stride;
-    const uint32_t total = (uint32_t)d.F * NS;
-    for (uint32_t c = threadIdx.x; c < total; c += blockDim.x) {
-      const uint32_t phi = c / NS, rank = c % NS;
+    // thread <-> split (rank), inner loop over phi: no division per candidate, the four shared-memory
+    // offsets of a split are formed once; (cost, flat) compared in full because flat = phi*NS + rank is
+    // not visited in ascending order
+    float bestC = FS_INF; uint32_t bflat = 0xFFFFFFFFu;
+    for (uint32_t rank = threadIdx.x; rank < NS; rank += blockDim.x) {
       const uint32_t pk = cp[rank];
-      float C = 0.0f;
-      for (int i = 0; i < n_res; ++i) {
-        const float g = sG[i * rows + phi * d.S + ((pk >> (8 * i)) & 0xFF)];
-        C = (i == 0) ? g : __fadd_rn(C, g);
-      }
-      if (C < FS_INF) {
-        const unsigned long long kk = fs_make_key(C, c);
-        key = kk < key ? kk : key;
-        fphi = min(fphi, phi);
+      int off[FS_RMAX];
+#pragma unroll
+      for (int i = 0; i < FS_RMAX; ++i) off[i] = (i < n_res ? i : 0) * rows + (int)((pk >> (8 * i)) & 0xFF);
+      for (int phi = 0; phi < d.F; ++phi) {
+        float C = sG[off[0] + phi * d.S];
+#pragma unroll
+        for (int i = 1; i < FS_RMAX; ++i) if (i < n_res) C = __fadd_rn(C, sG[off[i] + phi * d.S]);
+        const uint32_t flat = (uint32_t)phi * NS + rank;
+        if (C < FS_INF) {
+          if (C < bestC || (C == bestC && flat < bflat)) { bestC = C; bflat = flat; }
+          fphi = min(fphi, (uint32_t)phi);
+        }
       }
     }
+    if (bflat != 0xFFFFFFFFu) key = fs_make_key(bestC, bflat);
   }
   // f_req = lowest phi with any feasible candidate: tracked beside the key, reduced as a key of its own
   unsigned long long fkey = fphi == 0xFFFFFFFFu ? FS_KEY_NONE : (unsigned long long)fphi;
