@@ -306,7 +306,7 @@ typedef enum {
   FS_TIMER_LOCAL_SPLIT,     /* SM-split search of fs_local_config                    */
   FS_TIMER_CONSOL_AGG,      /* per-tenant minimum shares of fs_consolidate           */
   FS_TIMER_CONSOL_PAIR,     /* pair scoring of fs_consolidate                        */
-  FS_TIMER_PLACE_WARM,      /* (unused since the warm pairs moved into the scoring kernel) */
+  FS_TIMER_PLACE_WARM,      /* scan order + warm lists, built by the first placement call after fs_set_gpu_state */
   FS_TIMER_BATCH_TASKS,     /* fs_batch_tasks: priority score + batching            */
   FS_TIMER_DISPATCH,        /* fs_dispatch: the paper's three-phase dispatcher      */
   FS_TIMER_COUNT

@@ -14,7 +14,7 @@ struct fs_ctx {
   int dev = 0;
   fs_dims d{0, 0, 0, 0};
   fs_params prm{0, 0, 0, 0};
-  bool have_prof = false, have_state = false;
+  bool have_prof = false, have_state = false, place_ready = false;
   // profiles
   float *lat = nullptr, *pow = nullptr, *latT = nullptr, *powT = nullptr, *freq = nullptr;
   fs_model_info* models = nullptr;
@@ -115,6 +115,16 @@ void build_splits(int S, std::vector<uint32_t>& comp, uint32_t comp_n[FS_RMAX], 
   comp.assign((size_t)stride * FS_RMAX, 0u);
   for (int n = 0; n < FS_RMAX; ++n)
     for (size_t r = 0; r < lists[n].size(); ++r) comp[(size_t)n * stride + r] = lists[n][r];
+}
+
+// scan order + warm lists of the placement kernels: once per fs_set_gpu_state, on first use
+int place_prepare(fs_ctx* c, cudaStream_t st) {
+  if (c->place_ready || c->K <= 0) return FS_OK;
+  c->launches += fsk_place_prepare(view_of(c), c->grec, c->gsort, c->dsort, c->dsuf, c->warm_off, c->warm_cursor,
+                                   c->warm_item, st, c->timing ? &c->tm : nullptr);
+  FS_TRY(check_kernel(c));
+  c->place_ready = true;
+  return FS_OK;
 }
 
 cudaMemcpyKind in_kind(int space) { return space == FS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice; }
@@ -238,12 +248,11 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
     FS_TRY(grow(c, c->warm_off, (size_t)c->d.M + 1)); FS_TRY(grow(c, c->warm_cursor, (size_t)c->d.M));
     c->warm_m_cap = c->d.M;
   }
-  c->K = K; c->have_state = false;
+  c->K = K; c->have_state = false; c->place_ready = false;
   if (K > 0) {
     FS_CUDA(c, cudaMemcpyAsync(c->states, states, (size_t)K * sizeof(fs_gpu_state), in_kind(space), st));
     FsView v = view_of(c);
-    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0, c->gsort, c->dsort, c->dsuf, st, c->timing ? &c->tm : nullptr);
-    c->launches += fsk_build_warm_lists(v, c->warm_off, c->warm_cursor, c->warm_item, st);
+    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0, st, c->timing ? &c->tm : nullptr);
     FS_TRY(check_kernel(c));
   }
   c->have_state = true;
@@ -269,6 +278,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
+  FS_TRY(place_prepare(c, st));
   FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic, c->count_work};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
@@ -371,6 +381,7 @@ int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out,
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
+  FS_TRY(place_prepare(c, st));
   c->launches += fsk_dispatch(view_of(c), R, d_reqs, d_out, c->warm_off, c->warm_item, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space == FS_HOST) {

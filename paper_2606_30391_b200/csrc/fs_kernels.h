@@ -43,7 +43,9 @@ int fsk_build_planes(const float* lat, const float* pow, float* latT, float* pow
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
 int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
-                FsGpuRec* gsort, double* dsort, double* dsuf, cudaStream_t st, FsTimers* tm);
+                cudaStream_t st, FsTimers* tm);
+int fsk_place_prepare(const FsView& v, const FsGpuRec* grec, FsGpuRec* gsort, double* dsort, double* dsuf,
+                      int32_t* warm_off, int32_t* warm_cursor, FsWarmItem* items, cudaStream_t st, FsTimers* tm);
 
 // fs_place.cu — placement scoring + 64-bit-key argmin + decode
 struct FsPlaceScratch {

@@ -278,17 +278,28 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
 }  // namespace
 
 int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
-                FsGpuRec* gsort, double* dsort, double* dsuf, cudaStream_t st, FsTimers* tm) {
+                cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int wpb = 4;
   fs_tm_beg(tm, FS_T_SUMMARY, st);
   summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0);
+  fs_tm_end(tm, FS_T_SUMMARY, st);
+  return 1;
+}
+
+// What only the placement entry points need (built lazily by their first call after fs_set_gpu_state):
+// the scan order of the scoring kernel and the per-model warm lists.
+int fsk_place_prepare(const FsView& v, const FsGpuRec* grec, FsGpuRec* gsort, double* dsort, double* dsuf,
+                      int32_t* warm_off, int32_t* warm_cursor, FsWarmItem* items, cudaStream_t st, FsTimers* tm) {
+  if (v.K <= 0) return 0;
+  fs_tm_beg(tm, FS_T_PLACE_WARM, st);
   float* okey = reinterpret_cast<float*>(dsuf + v.Kpad / FS_CHUNK + 4);   // scratch behind dsuf
   order_key_kernel<<<(v.Kpad + 255) / 256, 256, 0, st>>>(grec, v.Kpad, okey);
   order_rank_kernel<<<(v.Kpad + 127) / 128, 128, 0, st>>>(grec, okey, v.Kpad, gsort, dsort);
   order_suffix_kernel<<<1, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf);
-  fs_tm_end(tm, FS_T_SUMMARY, st);
-  return 4;
+  const int n = fsk_build_warm_lists(v, warm_off, warm_cursor, items, st);
+  fs_tm_end(tm, FS_T_PLACE_WARM, st);
+  return 3 + n;
 }
 
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
