@@ -252,7 +252,8 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (K > 0) {
     FS_CUDA(c, cudaMemcpyAsync(c->states, states, (size_t)K * sizeof(fs_gpu_state), in_kind(space), st));
     FsView v = view_of(c);
-    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0, st, c->timing ? &c->tm : nullptr);
+    c->launches += fsk_summary(v, c->ginfo, c->gA, c->grec, c->gA0,
+                               reinterpret_cast<float*>(c->dsuf + c->Kpad / FS_CHUNK + 4), st, c->timing ? &c->tm : nullptr);
     FS_TRY(check_kernel(c));
   }
   c->have_state = true;

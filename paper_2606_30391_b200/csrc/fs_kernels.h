@@ -42,7 +42,7 @@ int fsk_build_planes(const float* lat, const float* pow, float* latT, float* pow
                      int* flag, cudaStream_t st);
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
-int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0, float* okey,
                 cudaStream_t st, FsTimers* tm);
 int fsk_place_prepare(const FsView& v, const FsGpuRec* grec, FsGpuRec* gsort, double* dsort, double* dsuf,
                       int32_t* warm_off, int32_t* warm_cursor, FsWarmItem* items, cudaStream_t st, FsTimers* tm);

@@ -28,11 +28,20 @@ __device__ __forceinline__ bool state_valid(const fs_gpu_state& g, const FsDimsD
   return used <= d.S;
 }
 
+// the scan-order key of a compact record (see "scan order of the dense placement kernel" below)
+__device__ __forceinline__ bool cold_capable(const FsGpuRec& r) {
+  const int n = r.meta & 0xFF, smf = (r.meta >> 8) & 0xFF;
+  return n >= 1 && n < FS_RMAX && smf >= 1 && r.a_min < FS_INF;
+}
+__device__ __forceinline__ float order_key(const FsGpuRec& r) {
+  float d = cold_capable(r) ? __fsub_rn(r.a_min, r.e_cur) : FS_INF;
+  return d == d ? d : FS_INF;
+}
 // one warp per GPU, lanes over phi
 __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __restrict__ ginfo,
                                                      float* __restrict__ gA,
                                                      FsGpuRec* __restrict__ grec,
-                                                     float* __restrict__ gA0) {
+                                                     float* __restrict__ gA0, float* __restrict__ okey) {
   const int lane = threadIdx.x & 31;
   const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (k >= v.Kpad) return;
@@ -43,7 +52,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
       FsGpuRec r; r.t_avail_ms = r.mem_free_mb = r.e_cur = 0.f; r.meta = 0;
       for (int i = 0; i < FS_RMAX; ++i) r.model[i] = -1;
       r.a_min = FS_INF; r.k = 0;
-      grec[k] = r;
+      grec[k] = r; okey[k] = FS_INF;
     }
     return;
   }
@@ -113,7 +122,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     r.meta = (uint32_t)n | ((uint32_t)gi.sm_free << 8) | ((uint32_t)gi.f_cur << 16);
     for (int i = 0; i < FS_RMAX; ++i) r.model[i] = gi.model[i];
     r.a_min = a_min; r.k = (uint32_t)k;
-    grec[k] = r;
+    grec[k] = r; okey[k] = order_key(r);
     if (!valid) fs_raise(v.flag, FS_FLAG_STATE);
   }
 }
@@ -125,48 +134,24 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
 // pruning bound fl(fl(a_min + b) - Ecur); everything else follows as sentinels no request is
 // eligible for.  Placement results do not depend on this order (ties compare (dE, k) in full): it
 // only decides how soon a request meets its best GPUs and can stop scanning (fs_place.cu).
-__device__ __forceinline__ bool cold_capable(const FsGpuRec& r) {
-  const int n = r.meta & 0xFF, smf = (r.meta >> 8) & 0xFF;
-  return n >= 1 && n < FS_RMAX && smf >= 1 && r.a_min < FS_INF;
-}
-__device__ __forceinline__ float order_key(const FsGpuRec& r) {
-  float d = cold_capable(r) ? __fsub_rn(r.a_min, r.e_cur) : FS_INF;
-  return d == d ? d : FS_INF;
-}
-// keys once, so that the ranking pass streams plain floats
-__global__ void order_key_kernel(const FsGpuRec* __restrict__ grec, int Kpad, float* __restrict__ okey) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < Kpad) okey[i] = order_key(grec[i]);
-}
-// rank of every record by (key, index): thread <-> record, keys walked through shared memory
-__global__ void __launch_bounds__(128) order_rank_kernel(const FsGpuRec* __restrict__ grec,
+// rank of every record by (key, index): warp <-> record, lanes over the other records' keys
+// (written by the summary kernel), partial counts summed by shuffles
+__global__ void __launch_bounds__(256) order_rank_kernel(const FsGpuRec* __restrict__ grec,
                                                         const float* __restrict__ okey, int Kpad,
                                                         FsGpuRec* __restrict__ gsort,
                                                         double* __restrict__ dsort) {
-  __shared__ __align__(16) float tile[1024];
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const float key = i < Kpad ? okey[i] : FS_INF;
-  int rank = 0;
-  for (int base = 0; base < Kpad; base += 1024) {
-    __syncthreads();
-    for (int x = threadIdx.x; x < 1024; x += blockDim.x) tile[x] = base + x < Kpad ? okey[base + x] : FS_INF;
-    __syncthreads();
-    // j < i decides ties: entries before i count on <=, entries after on <
-    const int n = min(1024, Kpad - base), nle = max(0, min(n, i - base));
-    int x = 0;
-    for (; x + 4 <= nle; x += 4) {
-      const float4 t = *reinterpret_cast<const float4*>(tile + x);
-      rank += (t.x <= key) + (t.y <= key) + (t.z <= key) + (t.w <= key);
-    }
-    for (; x < nle; ++x) rank += tile[x] <= key;
-    for (; x < n && (x & 3); ++x) rank += tile[x] < key;
-    for (; x + 4 <= n; x += 4) {
-      const float4 t = *reinterpret_cast<const float4*>(tile + x);
-      rank += (t.x < key) + (t.y < key) + (t.z < key) + (t.w < key);
-    }
-    for (; x < n; ++x) rank += tile[x] < key;
-  }
+  const int lane = threadIdx.x & 31;
+  const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (i >= Kpad) return;
+  const float key = okey[i];
+  int rank = 0;
+  for (int j = lane; j < Kpad; j += 32) {
+    const float kj = okey[j];
+    rank += (kj < key || (kj == key && j < i)) ? 1 : 0;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) rank += __shfl_xor_sync(0xffffffffu, rank, o);
+  if (lane != 0) return;
   FsGpuRec mine = grec[i];
   double dd = (double)FS_INF;
   if (cold_capable(mine)) { dd = (double)mine.a_min - (double)mine.e_cur; mine.k = (uint32_t)i; }
@@ -205,8 +190,13 @@ __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __re
   for (int c = lo; c < hi; ++c) { const double dv = dsuf[1 + c]; m = dv < m ? dv : m; }
   seg[t] = m;
   __syncthreads();
-  double carry = (double)FS_INF;                       // min over the segments after mine
-  if (lo < hi) for (int u = t + 1; u < 1024; ++u) { const double dv = seg[u]; carry = dv < carry ? dv : carry; }
+  for (int off = 1; off < 1024; off <<= 1) {           // inclusive suffix-minimum scan of the segments
+    const double dv = t + off < 1024 ? seg[t + off] : (double)FS_INF;
+    __syncthreads();
+    if (dv < seg[t]) seg[t] = dv;
+    __syncthreads();
+  }
+  double carry = t + 1 < 1024 ? seg[t + 1] : (double)FS_INF;   // min over the segments after mine
   for (int c = hi - 1; c >= lo; --c) {
     const double dv = dsuf[1 + c];
     carry = dv < carry ? dv : carry;
@@ -277,12 +267,12 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
 
 }  // namespace
 
-int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0,
+int fsk_summary(const FsView& v, FsGpuInfo* ginfo, float* gA, FsGpuRec* grec, float* gA0, float* okey,
                 cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int wpb = 4;
   fs_tm_beg(tm, FS_T_SUMMARY, st);
-  summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0);
+  summary_kernel<<<(v.Kpad + wpb - 1) / wpb, wpb * 32, 0, st>>>(v, ginfo, gA, grec, gA0, okey);
   fs_tm_end(tm, FS_T_SUMMARY, st);
   return 1;
 }
@@ -293,13 +283,12 @@ int fsk_place_prepare(const FsView& v, const FsGpuRec* grec, FsGpuRec* gsort, do
                       int32_t* warm_off, int32_t* warm_cursor, FsWarmItem* items, cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   fs_tm_beg(tm, FS_T_PLACE_WARM, st);
-  float* okey = reinterpret_cast<float*>(dsuf + v.Kpad / FS_CHUNK + 4);   // scratch behind dsuf
-  order_key_kernel<<<(v.Kpad + 255) / 256, 256, 0, st>>>(grec, v.Kpad, okey);
-  order_rank_kernel<<<(v.Kpad + 127) / 128, 128, 0, st>>>(grec, okey, v.Kpad, gsort, dsort);
+  const float* okey = reinterpret_cast<const float*>(dsuf + v.Kpad / FS_CHUNK + 4);   // written by the summary kernel
+  order_rank_kernel<<<(v.Kpad + 7) / 8, 256, 0, st>>>(grec, okey, v.Kpad, gsort, dsort);
   order_suffix_kernel<<<1, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf);
   const int n = fsk_build_warm_lists(v, warm_off, warm_cursor, items, st);
   fs_tm_end(tm, FS_T_PLACE_WARM, st);
-  return 3 + n;
+  return 2 + n;
 }
 
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
