@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
 // ascending beta keeps the lowest beta on ties, as the definition wants.
 constexpr int LS_TR = 8;          // rows per tile
 constexpr int LS_QB = 8;          // q buckets per key (slots of similar depth share a warp)
-constexpr int LS_WARPS = 8;
+constexpr int LS_WARPS = 4;
 __constant__ uint32_t c_magic[FS_MAX_B];   // ceil(2^32 / (beta+1)), beta >= 1
 
 struct __align__(16) LocalSlot { int32_t gi; uint32_t q; float slo; uint32_t meta; };  // meta = slot | nb << 8
