@@ -518,3 +518,16 @@ def test_migration_plan_against_scipy(ctx):
     c = np.rint((t * np.float32(1000.0)).astype(np.float32)).astype(np.int64)
     rows, cols = linear_sum_assignment(c)
     assert tot == int(c[rows, cols].sum()) == int(c[np.arange(64), dst].sum())
+
+
+# ---- the paper's largest cluster size (Table 3: 10,000 GPUs): GPUs split over several slices ---------
+def test_ten_thousand_gpus_sampled(ctx):
+    cl = synth.make_custom(seed=77, K=10000, M=32, F=64, S=16, B=64, R=3000, lo=1, hi=4)
+    ctx.load_cluster(cl)
+    got = ctx.place_batch(cl.requests)
+    idx = np.unique(synth.Stream(13, "sample").randint(160, 0, cl.R - 1))
+    cmp.assert_placement_equal(got[idx], _oracle_place(cl, cl.requests[idx]))
+    one = ctx.place_batch(cl.requests[:1])            # a single arrival: the GPUs are split over the SMs
+    cmp.assert_placement_equal(one, got[:1])
+    dsp = ctx.dispatch(cl.requests)
+    cmp.assert_placement_equal(dsp[idx], _oracle_dispatch(cl, cl.requests[idx]))
