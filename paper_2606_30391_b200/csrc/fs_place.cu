@@ -660,26 +660,60 @@ __device__ __forceinline__ DispPair disp_warm(const FsView& v, const ReqCtx& c, 
   return r;
 }
 
-template <int NPHI>
+// reductions over the warps that share a request: the warp alone, or (BLOCK) all DISP_WARPS warps of the block
+template <bool BLOCK>
+__device__ __forceinline__ uint32_t disp_min_u32(uint32_t x, uint32_t* s_red, int warp, int lane) {
+  x = warp_min_u32(x);
+  if (BLOCK) {
+    __syncthreads();
+    if (lane == 0) s_red[warp] = x;
+    __syncthreads();
+    x = s_red[0];
+#pragma unroll
+    for (int w = 1; w < DISP_WARPS; ++w) x = min(x, s_red[w]);
+  }
+  return x;
+}
+template <bool BLOCK>
+__device__ __forceinline__ unsigned long long disp_min_key(unsigned long long k, unsigned long long* s_red, int warp, int lane) {
+  k = fs_warp_min_key(k);
+  if (BLOCK) {
+    __syncthreads();
+    if (lane == 0) s_red[warp] = k;
+    __syncthreads();
+    k = s_red[0];
+#pragma unroll
+    for (int w = 1; w < DISP_WARPS; ++w) k = s_red[w] < k ? s_red[w] : k;
+  }
+  return k;
+}
+
+// BLOCK = false: one warp per request (batches).  BLOCK = true: one block per request, its warps split
+// the GPUs (few requests, e.g. a single arrival against thousands of GPUs: the scan is the latency).
+template <int NPHI, bool BLOCK>
 __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int R,
                                                                   const fs_request* __restrict__ reqs,
                                                                   fs_placement* __restrict__ out, int use_tiles,
                                                                   const int32_t* __restrict__ warm_off,
                                                                   const FsWarmItem* __restrict__ witems) {
   extern __shared__ __align__(16) unsigned char disp_smem[];
+  __shared__ unsigned long long s_red[DISP_WARPS];
+  uint32_t* s_red32 = reinterpret_cast<uint32_t*>(s_red);
   constexpr int FT = 32 * NPHI;
+  constexpr int NW = BLOCK ? DISP_WARPS : 1;           // warps per request
   const FsDimsDev d = v.d;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int r = blockIdx.x * DISP_WARPS + warp;
+  const int sub = BLOCK ? warp : 0;
+  const int r = BLOCK ? (int)blockIdx.x : (int)blockIdx.x * DISP_WARPS + warp;
   if (r >= R) return;
   // F > 64: no tiles, every pair from the planes
-  float* tl_t0 = use_tiles ? reinterpret_cast<float*>(disp_smem) + (size_t)warp * 2 * d.S * FT : nullptr;
+  float* tl_t0 = use_tiles ? reinterpret_cast<float*>(disp_smem) + (size_t)(BLOCK ? 0 : warp) * 2 * d.S * FT : nullptr;
   float* tl_er = tl_t0 + d.S * FT;
   fs_placement o;
   o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
   o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
   const ReqCtx c = make_req(v, reqs[r]);
-  if (!c.valid) { if (lane == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } return; }
+  if (!c.valid) { if (lane == 0 && sub == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } return; }
   // ---- the request's cold tiles: t0 = fl(rounds0*LAT0), er = fl(e0 + e1) (INF where LAT1 > slo_tbt)
   if (use_tiles) {
     const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
@@ -689,7 +723,7 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
     const bool vec = NPHI == 2 && (d.F & 1) == 0;
     const int phi0 = lane * NPHI;
 #pragma unroll 2
-    for (int s = 0; s < d.S; ++s) {
+    for (int s = sub; s < d.S; s += NW) {
       float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI], tt[NPHI], ee[NPHI];
       const int ofs = s * d.F;
       ld_cols<NPHI>(l0, ofs, phi0, d.F, vec, a0); ld_cols<NPHI>(p0, ofs, phi0, d.F, vec, b0);
@@ -704,31 +738,33 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
       }
       st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
     }
-    __syncwarp();
+    if (BLOCK) __syncthreads(); else __syncwarp();
   }
   // ---- Phase 1 + 2 at F_curr: E_min, then the 2 % band with the stability tie-breaker ----------
-  // lane c keeps the minimum of chunk c (32 GPUs), c < 32*DISP_NC, so that the band scan only
-  // revisits chunks that hold a candidate inside the band
+  // This warp's chunks of 32 GPUs: sub, sub + NW, ...; lane j of cmin keeps the minimum of the warp's
+  // j-th chunk (j < 32*DISP_NC) so that the band scan only revisits chunks that hold a candidate
+  // inside the band.  grec is padded to a multiple of 32 records (n_res = 0); the next chunk's records
+  // are in flight while this one is scored.
+  const int nchunk = v.Kpad / 32;
   uint32_t emin_o = 0xFFFFFFFFu, cmin[DISP_NC];
 #pragma unroll
   for (int u = 0; u < DISP_NC; ++u) cmin[u] = 0xFFFFFFFFu;
-  // grec is padded to a multiple of 32 records (n_res = 0); the next chunk's records are in flight
-  // while this one is scored
-  FsGpuRec nxt = v.grec[lane];
-  for (int base = 0; base < v.Kpad; base += 32) {
-    const FsGpuRec g = nxt;
-    if (base + 32 < v.Kpad) nxt = v.grec[base + 32 + lane];
-    uint32_t eo = 0xFFFFFFFFu;
-    const DispPair dp = disp_pair(v, c, g, base + lane, -1, tl_t0, tl_er, FT);
-    if (dp.ok) eo = fs_orderable(dp.e);
-    const uint32_t cm = warp_min_u32(eo);
-    const int ch = base >> 5;
+  {
+    FsGpuRec nxt = v.grec[min(sub, nchunk - 1) * 32 + lane];
+    for (int ch = sub, j = 0; ch < nchunk; ch += NW, ++j) {
+      const FsGpuRec g = nxt;
+      if (ch + NW < nchunk) nxt = v.grec[(ch + NW) * 32 + lane];
+      uint32_t eo = 0xFFFFFFFFu;
+      const DispPair dp = disp_pair(v, c, g, ch * 32 + lane, -1, tl_t0, tl_er, FT);
+      if (dp.ok) eo = fs_orderable(dp.e);
+      const uint32_t cm = warp_min_u32(eo);
 #pragma unroll
-    for (int u = 0; u < DISP_NC; ++u) if ((ch >> 5) == u && (ch & 31) == lane) cmin[u] = cm;
-    emin_o = min(emin_o, cm);
+      for (int u = 0; u < DISP_NC; ++u) if ((j >> 5) == u && (j & 31) == lane) cmin[u] = cm;
+      emin_o = min(emin_o, cm);
+    }
   }
   const int wb0 = use_tiles ? warm_off[c.m] : 0, wb1 = use_tiles ? warm_off[c.m + 1] : 0;
-  for (int ib = wb0; ib < wb1; ib += 32) {
+  for (int ib = wb0 + sub * 32; ib < wb1; ib += 32 * NW) {
     uint32_t eo = 0xFFFFFFFFu;
     if (ib + lane < wb1) {
       const DispPair dp = disp_warm(v, c, witems[ib + lane], -1);
@@ -736,21 +772,21 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
     }
     emin_o = min(emin_o, warp_min_u32(eo));
   }
+  emin_o = disp_min_u32<BLOCK>(emin_o, s_red32, warp, lane);
   int phase = -1, kbest = -1, phibest = -1;
   if (emin_o != 0xFFFFFFFFu) {
     const float band = __fmul_rn(1.02f, fs_unorderable(emin_o));
     const uint32_t band_o = fs_orderable(band);
     unsigned long long key = FS_KEY_NONE;              // (most memory, largest SM_free, lowest k)
-    for (int base = 0; base < v.Kpad; base += 32) {
-      const int ch = base >> 5;
-      if (ch < 32 * DISP_NC) {
+    for (int ch = sub, j = 0; ch < nchunk; ch += NW, ++j) {
+      if (j < 32 * DISP_NC) {
         uint32_t cm = 0xFFFFFFFFu;
 #pragma unroll
-        for (int u = 0; u < DISP_NC; ++u) if ((ch >> 5) == u) cm = cmin[u];
-        cm = __shfl_sync(0xffffffffu, cm, ch & 31);
+        for (int u = 0; u < DISP_NC; ++u) if ((j >> 5) == u) cm = cmin[u];
+        cm = __shfl_sync(0xffffffffu, cm, j & 31);
         if (cm > band_o) continue;                     // no candidate of this chunk is inside the band
       }
-      const int k = base + lane;
+      const int k = ch * 32 + lane;
       const FsGpuRec g = v.grec[k];
       const DispPair dp = disp_pair(v, c, g, k, -1, tl_t0, tl_er, FT);
       if (dp.ok && dp.e <= band) {
@@ -759,7 +795,7 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
         key = kk < key ? kk : key;
       }
     }
-    for (int ib = wb0 + lane; ib < wb1; ib += 32) {
+    for (int ib = wb0 + sub * 32 + lane; ib < wb1; ib += 32 * NW) {
       const FsWarmItem it = witems[ib];
       const DispPair dp = disp_warm(v, c, it, -1);
       if (dp.ok && dp.e <= band) {
@@ -768,14 +804,14 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
         key = kk < key ? kk : key;
       }
     }
-    key = fs_warp_min_key(key);
+    key = disp_min_key<BLOCK>(key, s_red, warp, lane);
     kbest = (int)((uint32_t)key & 0xFFFFFFu); phase = 1;
     phibest = v.ginfo[kbest].f_cur;
   } else {
     // ---- Phase 3: F_max retry, first feasible GPU in T_avail order ------------------------------
     unsigned long long key = FS_KEY_NONE;
-    for (int base = 0; base < v.Kpad; base += 32) {
-      const int k = base + lane;
+    for (int ch = sub; ch < nchunk; ch += NW) {
+      const int k = ch * 32 + lane;
       const FsGpuRec g = v.grec[k];
       const DispPair dp = disp_pair(v, c, g, k, d.F - 1, tl_t0, tl_er, FT);
       if (dp.ok) {
@@ -783,7 +819,7 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
         key = kk < key ? kk : key;
       }
     }
-    for (int ib = wb0 + lane; ib < wb1; ib += 32) {
+    for (int ib = wb0 + sub * 32 + lane; ib < wb1; ib += 32 * NW) {
       const FsWarmItem it = witems[ib];
       const DispPair dp = disp_warm(v, c, it, d.F - 1);
       if (dp.ok) {
@@ -791,9 +827,10 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
         key = kk < key ? kk : key;
       }
     }
-    key = fs_warp_min_key(key);
+    key = disp_min_key<BLOCK>(key, s_red, warp, lane);
     if (key != FS_KEY_NONE) { kbest = (int)(uint32_t)key; phase = 2; phibest = d.F - 1; }
   }
+  if (sub != 0) return;                                // the request's first warp writes the record
   if (kbest >= 0) {
     const PairCtx p = make_pair(v, c, v.ginfo[kbest]);
     const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, p.smf - 1, phibest);
@@ -832,8 +869,8 @@ int fsk_place_smem_attr() {
   e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   e |= (int)cudaFuncSetAttribute(place_dense_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(dispatch_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 32 * 4);
-  e |= (int)cudaFuncSetAttribute(dispatch_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 64 * 4);
+  e |= (int)cudaFuncSetAttribute(dispatch_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 32 * 4);
+  e |= (int)cudaFuncSetAttribute(dispatch_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 64 * 4);
   return e;
 }
 
@@ -907,10 +944,18 @@ int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* o
   if (R <= 0) return 0;
   const int use_tiles = v.d.F <= 64;
   const int FT = v.d.F <= 32 ? 32 : 64;
-  const size_t smem = use_tiles ? (size_t)DISP_WARPS * 2 * v.d.S * FT * sizeof(float) : 0;
+  // few requests: one block per request, its warps split the GPUs; batches: one warp per request
+  const bool block_mode = (long long)R * DISP_WARPS <= 2LL * 148 * DISP_WARPS && v.Kpad >= 64 * DISP_WARPS;
+  const size_t smem = use_tiles ? (size_t)(block_mode ? 1 : DISP_WARPS) * 2 * v.d.S * FT * sizeof(float) : 0;
   fs_tm_beg(tm, FS_T_DISPATCH, st);
-  if (FT == 32) dispatch_kernel<1><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
-  else          dispatch_kernel<2><<<(R + DISP_WARPS - 1) / DISP_WARPS, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
+  const int grid = block_mode ? R : (R + DISP_WARPS - 1) / DISP_WARPS;
+  if (FT == 32) {
+    if (block_mode) dispatch_kernel<1, true><<<grid, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
+    else            dispatch_kernel<1, false><<<grid, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
+  } else {
+    if (block_mode) dispatch_kernel<2, true><<<grid, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
+    else            dispatch_kernel<2, false><<<grid, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
+  }
   fs_tm_end(tm, FS_T_DISPATCH, st);
   return 1;
 }

@@ -531,3 +531,10 @@ def test_ten_thousand_gpus_sampled(ctx):
     cmp.assert_placement_equal(one, got[:1])
     dsp = ctx.dispatch(cl.requests)
     cmp.assert_placement_equal(dsp[idx], _oracle_dispatch(cl, cl.requests[idx]))
+    # few arrivals: one block per request, its warps split the GPUs
+    few = cl.requests[:150].copy()
+    few["slo_ttft_ms"][::3] *= 0.03; few["o_pred"][1::5] = 2 ** 20; few["slo_tbt_ms"][2::7] = 1e-3
+    got_few = ctx.dispatch(few)
+    cmp.assert_placement_equal(got_few, _oracle_dispatch(cl, few))
+    assert set(np.unique(got_few["f_req"]).tolist()) >= {1, 2, 3}
+    cmp.assert_placement_equal(ctx.dispatch(few[:1]), got_few[:1])
