@@ -538,3 +538,25 @@ def test_ten_thousand_gpus_sampled(ctx):
     cmp.assert_placement_equal(got_few, _oracle_dispatch(cl, few))
     assert set(np.unique(got_few["f_req"]).tolist()) >= {1, 2, 3}
     cmp.assert_placement_equal(ctx.dispatch(few[:1]), got_few[:1])
+
+
+# ---- extreme magnitudes: the pruning bounds and the early stop must stay sound -----------------------
+@pytest.mark.parametrize("scale", [1e28, 1e-30, 1e-41])
+def test_extreme_energy_scales(ctx, scale):
+    """Power tables scaled so that energies sit near FLT_MAX, far below 1, and in the denormals."""
+    cl = synth.make_custom(seed=1300, K=96, M=5, F=24, S=10, B=12, R=160, lo=1, hi=4)
+    cl.pow = (cl.pow.astype(np.float64) * scale).astype(np.float32)
+    cl.pow[cl.pow == 0] = np.float32(1e-45)                   # tables must stay > 0
+    _check_all(ctx, cl, local=True, consol=True)
+    cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
+
+
+def test_negative_and_huge_waits(ctx):
+    cl = synth.make_custom(seed=1301, K=80, M=4, F=20, S=8, B=8, R=128, lo=1, hi=4)
+    cl.states["t_avail_ms"][::3] = -500.0                      # a GPU that has been free for a while
+    cl.states["t_avail_ms"][1::7] = 1e30
+    cl.models["load_ms"][0] = 0.0
+    cl.requests["slo_ttft_ms"][::5] = np.float32(np.inf)
+    cl.requests["slo_tbt_ms"][::4] = np.float32(np.inf)
+    _check_all(ctx, cl, local=False, consol=False)
+    cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
