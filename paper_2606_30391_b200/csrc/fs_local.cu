@@ -132,16 +132,28 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int s0 = off[key * LS_QB], s1 = off[(key + 1) * LS_QB];
-  for (int base = s0 + warp * 32; base < s1; base += LS_WARPS * 32) {
-    const bool have = base + lane < s1;
-    LocalSlot sl_ = have ? slots[base + lane] : LocalSlot{0, 0u, 0.f, 0u};
+  // Rounds of LS_WARPS*32 slots, lane <-> slot.  A last round of fewer than 64 slots spreads them evenly over
+  // the warps and, when a warp gets <= 16 of them, gives each slot G = 2, 4, ... lanes
+  // that split the beta range (groups of four beta, interleaved); their minima are merged by shuffles
+  // (min is exact in any order).  At pod a (model, phase) key has ~40 slots: without this most lanes idle.
+  for (int start = s0; start < s1; start += LS_WARPS * 32) {
+    const int n_round = min(LS_WARPS * 32, s1 - start);
+    int pad = 32, per = 32;
+    if (n_round < 64) {                                 // denser rounds keep lane <-> slot: splitting beta costs
+      per = (n_round + LS_WARPS - 1) / LS_WARPS;        // a second LDS wavefront per row, which only pays
+                                                        // when most lanes would idle otherwise
+      pad = 1; while (pad < per) pad <<= 1;
+    }
+    const int G = 32 / pad, grp = lane / pad, sl_ix = warp * per + (lane % pad);
+    const bool have = (lane % pad) < per && sl_ix < n_round;
+    LocalSlot sl_ = have ? slots[start + sl_ix] : LocalSlot{0, 0u, 0.f, 0u};
     const uint32_t nb = have ? (sl_.meta >> 8) : 0u;
     uint32_t maxnb;
     asm volatile("redux.sync.max.u32 %0, %1, 0xffffffff;" : "=r"(maxnb) : "r"(nb));
     float best[LS_TR];
 #pragma unroll
     for (int r = 0; r < LS_TR; ++r) best[r] = FS_INF;
-    for (uint32_t b4 = 0; b4 < maxnb; b4 += 4) {
+    for (uint32_t b4 = 4u * grp; b4 < maxnb; b4 += 4u * G) {
       float4 L4[LS_TR], P4[LS_TR];
 #pragma unroll
       for (int r = 0; r < LS_TR; ++r) {
@@ -168,7 +180,11 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
         }
       }
     }
-    if (have) {
+    for (int o2 = pad; o2 < 32; o2 <<= 1) {
+#pragma unroll
+      for (int r = 0; r < LS_TR; ++r) best[r] = fminf(best[r], __shfl_xor_sync(0xffffffffu, best[r], o2));
+    }
+    if (have && grp == 0) {
       const size_t o = ((size_t)sl_.gi * (FS_RMAX * 2) + (sl_.meta & 0xFF)) * rows + r0;
       if (tr == LS_TR && (rows & 3) == 0) {
 #pragma unroll
