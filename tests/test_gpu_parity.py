@@ -560,3 +560,24 @@ def test_negative_and_huge_waits(ctx):
     cl.requests["slo_tbt_ms"][::4] = np.float32(np.inf)
     _check_all(ctx, cl, local=False, consol=False)
     cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
+
+
+# ---- randomised sweep: dims, load shapes and SLO regimes, every entry point of the hot path ----------
+@pytest.mark.parametrize("block", range(4))
+def test_random_clusters_all_entry_points(ctx, block):
+    for seed in range(block * 30, block * 30 + 30):
+        st = synth.Stream(seed, "fuzz")
+        K = int(st.randint(1, 1, 400)[0]); M = int(st.randint(1, 1, 12)[0]); F = int(st.randint(1, 1, 64)[0])
+        S = int(st.randint(1, 1, 16)[0]); B = int(st.randint(1, 1, 48)[0]); R = int(st.randint(1, 1, 700)[0])
+        cl = synth.make_custom(seed=5000 + seed, K=K, M=M, F=F, S=S, B=B, R=R, lo=1, hi=4)
+        mode = seed % 5
+        if mode == 1:
+            cl = U.tie_heavy(cl, seed)
+        if mode == 2:                                   # many cold pairs can meet the TTFT deadline
+            cl.requests["slo_ttft_ms"] *= 3.0; cl.models["load_ms"] *= 0.1
+        if mode == 3:
+            cl.requests["slo_ttft_ms"] *= 0.05
+        if mode == 4:
+            cl.states["mem_free_mb"] *= 0.02
+        _check_all(ctx, cl)
+        cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
