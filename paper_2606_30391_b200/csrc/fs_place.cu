@@ -602,7 +602,8 @@ __global__ void __launch_bounds__(256) place_decode_kernel(FsView v, int R,
 // reads the planes.  Lanes <-> GPUs; reductions by redux / 64-bit key shuffles.
 // =============================================================================================
 constexpr int DISP_WARPS = 8;
-constexpr int DISP_NC = 4;                    // chunk minima kept per lane: GPUs beyond 32*32*DISP_NC are always revisited
+constexpr int DISP_NC = 4;                    // group minima kept per lane: GPUs beyond 32*32*DISP_GC*DISP_NC are always revisited
+constexpr int DISP_GC = 4;                    // chunks of 32 GPUs per group (one reduction, DISP_GC loads in flight)
 
 struct OwnEval { bool ok; float e, ttft, tbt; };
 
@@ -741,27 +742,32 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
     if (BLOCK) __syncthreads(); else __syncwarp();
   }
   // ---- Phase 1 + 2 at F_curr: E_min, then the 2 % band with the stability tie-breaker ----------
-  // This warp's chunks of 32 GPUs: sub, sub + NW, ...; lane j of cmin keeps the minimum of the warp's
-  // j-th chunk (j < 32*DISP_NC) so that the band scan only revisits chunks that hold a candidate
-  // inside the band.  grec is padded to a multiple of 32 records (n_res = 0); the next chunk's records
-  // are in flight while this one is scored.
+  // This warp's chunks of 32 GPUs: sub, sub + NW, ..., taken DISP_GC at a time; lane j of cmin keeps the
+  // minimum of the warp's j-th group so that the band scan only revisits groups that hold a candidate
+  // inside the band.  grec is padded to a multiple of 32 records (n_res = 0).
   const int nchunk = v.Kpad / 32;
   uint32_t emin_o = 0xFFFFFFFFu, cmin[DISP_NC];
 #pragma unroll
   for (int u = 0; u < DISP_NC; ++u) cmin[u] = 0xFFFFFFFFu;
-  {
-    FsGpuRec nxt = v.grec[min(sub, nchunk - 1) * 32 + lane];
-    for (int ch = sub, j = 0; ch < nchunk; ch += NW, ++j) {
-      const FsGpuRec g = nxt;
-      if (ch + NW < nchunk) nxt = v.grec[(ch + NW) * 32 + lane];
-      uint32_t eo = 0xFFFFFFFFu;
-      const DispPair dp = disp_pair(v, c, g, ch * 32 + lane, -1, tl_t0, tl_er, FT);
-      if (dp.ok) eo = fs_orderable(dp.e);
-      const uint32_t cm = warp_min_u32(eo);
+  for (int j0 = 0; sub + j0 * NW < nchunk; j0 += DISP_GC) {
+    FsGpuRec g4[DISP_GC];                              // DISP_GC independent record loads in flight
 #pragma unroll
-      for (int u = 0; u < DISP_NC; ++u) if ((j >> 5) == u && (j & 31) == lane) cmin[u] = cm;
-      emin_o = min(emin_o, cm);
+    for (int u = 0; u < DISP_GC; ++u) {
+      const int ch = sub + (j0 + u) * NW;
+      g4[u] = v.grec[min(ch, nchunk - 1) * 32 + lane];
+      if (ch >= nchunk) g4[u].meta = 0u;               // past the end: n_res = 0, never a candidate
     }
+    uint32_t eo = 0xFFFFFFFFu;
+#pragma unroll
+    for (int u = 0; u < DISP_GC; ++u) {
+      const DispPair dp = disp_pair(v, c, g4[u], (sub + (j0 + u) * NW) * 32 + lane, -1, tl_t0, tl_er, FT);
+      if (dp.ok) eo = min(eo, fs_orderable(dp.e));
+    }
+    const uint32_t cm = warp_min_u32(eo);
+    const int gj = j0 / DISP_GC;
+#pragma unroll
+    for (int u = 0; u < DISP_NC; ++u) if ((gj >> 5) == u && (gj & 31) == lane) cmin[u] = cm;
+    emin_o = min(emin_o, cm);
   }
   const int wb0 = use_tiles ? warm_off[c.m] : 0, wb1 = use_tiles ? warm_off[c.m + 1] : 0;
   for (int ib = wb0 + sub * 32; ib < wb1; ib += 32 * NW) {
@@ -778,21 +784,26 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
     const float band = __fmul_rn(1.02f, fs_unorderable(emin_o));
     const uint32_t band_o = fs_orderable(band);
     unsigned long long key = FS_KEY_NONE;              // (most memory, largest SM_free, lowest k)
-    for (int ch = sub, j = 0; ch < nchunk; ch += NW, ++j) {
-      if (j < 32 * DISP_NC) {
+    for (int j0 = 0; sub + j0 * NW < nchunk; j0 += DISP_GC) {
+      const int gj = j0 / DISP_GC;
+      if (gj < 32 * DISP_NC) {
         uint32_t cm = 0xFFFFFFFFu;
 #pragma unroll
-        for (int u = 0; u < DISP_NC; ++u) if ((j >> 5) == u) cm = cmin[u];
-        cm = __shfl_sync(0xffffffffu, cm, j & 31);
-        if (cm > band_o) continue;                     // no candidate of this chunk is inside the band
+        for (int u = 0; u < DISP_NC; ++u) if ((gj >> 5) == u) cm = cmin[u];
+        cm = __shfl_sync(0xffffffffu, cm, gj & 31);
+        if (cm > band_o) continue;                     // no candidate of this group is inside the band
       }
-      const int k = ch * 32 + lane;
-      const FsGpuRec g = v.grec[k];
-      const DispPair dp = disp_pair(v, c, g, k, -1, tl_t0, tl_er, FT);
-      if (dp.ok && dp.e <= band) {
-        const unsigned long long kk = ((unsigned long long)(~fs_orderable(g.mem_free_mb)) << 32) |
-                                      ((unsigned long long)(uint32_t)(d.S - (int)((g.meta >> 8) & 0xFF)) << 24) | (uint32_t)k;
-        key = kk < key ? kk : key;
+      for (int u = 0; u < DISP_GC; ++u) {
+        const int ch = sub + (j0 + u) * NW;
+        if (ch >= nchunk) break;
+        const int k = ch * 32 + lane;
+        const FsGpuRec g = v.grec[k];
+        const DispPair dp = disp_pair(v, c, g, k, -1, tl_t0, tl_er, FT);
+        if (dp.ok && dp.e <= band) {
+          const unsigned long long kk = ((unsigned long long)(~fs_orderable(g.mem_free_mb)) << 32) |
+                                        ((unsigned long long)(uint32_t)(d.S - (int)((g.meta >> 8) & 0xFF)) << 24) | (uint32_t)k;
+          key = kk < key ? kk : key;
+        }
       }
     }
     for (int ib = wb0 + sub * 32 + lane; ib < wb1; ib += 32 * NW) {
