@@ -470,6 +470,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
         const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F;
         const float fr1 = __uint2float_rn(p.rounds1);
+        // an empty prefill / decode slot passes its deadline whatever the wait (slot rule, q == 0)
+        const float wait_e = c.L ? p.wait : 0.0f, ttft_e = c.L ? c.slo_ttft : FS_INF, tbt_e = c.O ? c.slo_tbt : FS_INF;
         float ar[NPHI];
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < d.F ? Ar[phi0 + i] : FS_INF;
@@ -491,10 +493,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             for (int i = 0; i < NPHI; ++i) {
               const float e0 = __fmul_rn(tt[u][i], b0[u][i]);
               const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
-              float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);
-              if (dE == 0.0f) dE = 0.0f;
-              const bool ok = s < p.smf && (c.L == 0 || __fadd_rn(p.wait, tt[u][i]) <= c.slo_ttft) &&
-                              (c.O == 0 || a1[u][i] <= c.slo_tbt) && dE < FS_INF;
+              const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   // -0 == +0 in every compare below
+              const bool ok = s < p.smf && __fadd_rn(wait_e, tt[u][i]) <= ttft_e && a1[u][i] <= tbt_e && dE < FS_INF;
               if (recover) {
                 if (ok && dE == bestW && flat == NONE32) flat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
               } else if (ok && (dE < best || (dE == best && k < bestk))) {
