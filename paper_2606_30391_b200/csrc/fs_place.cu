@@ -475,7 +475,11 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         float ar[NPHI];
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < d.F ? Ar[phi0 + i] : FS_INF;
-        // four share rows per trip: their 12 plane loads are issued before any of them is used
+        // four share rows per trip: their 12 plane loads are issued before any of them is used.  Each lane
+        // keeps the minimum of ITS candidates of this pair and the first (lowest flat) candidate attaining
+        // it; merged into the incumbent afterwards, or, in the recovery pass, matched against the winner's
+        // value (the pair's minimum by the definition equals what the sweep found: monotone rounding).
+        float pb = FS_INF; uint32_t pflat = NONE32;
 #pragma unroll 1
         for (int s4 = 0; s4 < p.smf; s4 += 4) {
           float tt[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
@@ -494,16 +498,13 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
               const float e0 = __fmul_rn(tt[u][i], b0[u][i]);
               const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
               const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   // -0 == +0 in every compare below
-              const bool ok = s < p.smf && __fadd_rn(wait_e, tt[u][i]) <= ttft_e && a1[u][i] <= tbt_e && dE < FS_INF;
-              if (recover) {
-                if (ok && dE == bestW && flat == NONE32) flat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
-              } else if (ok && (dE < best || (dE == best && k < bestk))) {
-                best = dE; bestk = k; bflat = (uint32_t)((k * d.S + s) * d.F + phi0 + i);
-              }
+              const bool ok = s < p.smf && __fadd_rn(wait_e, tt[u][i]) <= ttft_e && a1[u][i] <= tbt_e;
+              if (ok && dE < pb) { pb = dE; pflat = (uint32_t)((k * d.S + s) * d.F + phi0 + i); }   // INF never enters
             }
           }
-          if (recover && __any_sync(0xffffffffu, flat != NONE32)) break;   // flat order is sigma-major
         }
+        if (recover) { if (pb == bestW) flat = pflat; }
+        else if (pb < best || (pb == best && k < bestk)) { best = pb; bestk = k; bflat = pflat; }
       }
       if (recover) break;
     }
