@@ -211,6 +211,22 @@ __device__ __forceinline__ void ld_cols(const float* __restrict__ base, int o, i
   }
 }
 
+// The same through per-lane pointers that already include the lane's (clamped) column: the address of a
+// row is then one widening multiply-add of an unsigned element offset instead of a chain of 64-bit adds.
+struct LanePtr { const float* a; const float* b; };
+template <int NPHI>
+__device__ __forceinline__ LanePtr lane_ptr(const float* base, int phi0, int ncol, bool vec) {
+  LanePtr p;
+  p.a = base + (NPHI == 2 && vec ? min(phi0, ncol - 2) : min(phi0, ncol - 1));
+  p.b = base + min(phi0 + NPHI - 1, ncol - 1);
+  return p;
+}
+template <int NPHI>
+__device__ __forceinline__ void ld_lane(const LanePtr& p, uint32_t o, bool vec, float (&x)[NPHI]) {
+  if (NPHI == 2 && vec) { const float2 t = *reinterpret_cast<const float2*>(p.a + o); x[0] = t.x; x[NPHI - 1] = t.y; }
+  else { x[0] = p.a[o]; if (NPHI == 2) x[NPHI - 1] = p.b[o]; }
+}
+
 // work statistics (what this launch actually did; bench.py turns them into lane-operations)
 __device__ __forceinline__ void flush_stats(unsigned long long* stats, uint32_t n_chunks, uint32_t n_elig,
                                          uint32_t n_swept, uint32_t n_cswept, uint32_t n_witems,
@@ -287,6 +303,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   uint32_t n_chunks = 0, n_elig = 0, n_swept = 0, n_cswept = 0, n_witems = 0, n_scored = 0, n_cscored = 0, n_req = 0;
   const bool vec = NPHI == 2 && (d.F & 1) == 0;
   const int phi0 = lane * NPHI;
+  const LanePtr q_a0 = lane_ptr<NPHI>(v.gA0, phi0, FT, true);
   for (;;) {
     // ---- next request of this slice: dynamic, one atomic per warp ----------------------------
     int r = 0;
@@ -311,10 +328,11 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     // (monotone rounding).  er, t0, e0 >= +0, so their bit patterns order like unsigned integers.
     // L == 0 / O == 0 need no branches: rounds = 0 gives t = e = +0 exactly (tables are finite),
     // and an empty decode slot passes its deadline (threshold +INF).
-    const float* pw0 = v.powT + fs_plane(d, c.m, 0, c.br0);
+    const LanePtr q_p0 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 0, c.br0), phi0, d.F, vec);
     {
-      const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0);
-      const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
+      const LanePtr q_l0 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 0, c.br0), phi0, d.F, vec);
+      const LanePtr q_l1 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 1, 0), phi0, d.F, vec);
+      const LanePtr q_p1 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 1, 0), phi0, d.F, vec);
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
       const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
       uint32_t pe = INFBITS, pt = INFBITS, pe0 = INFBITS;   // running prefix minima (bits)
@@ -323,8 +341,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       for (int s = 0; s < d.S; ++s) {
         float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI], tt[NPHI], ee[NPHI];
         const int o = s * d.F;
-        ld_cols<NPHI>(l0, o, phi0, d.F, vec, a0); ld_cols<NPHI>(pw0, o, phi0, d.F, vec, b0);
-        ld_cols<NPHI>(l1, o, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, o, phi0, d.F, vec, b1);
+        ld_lane<NPHI>(q_l0, o, vec, a0); ld_lane<NPHI>(q_p0, o, vec, b0);
+        ld_lane<NPHI>(q_l1, o, vec, a1); ld_lane<NPHI>(q_p1, o, vec, b1);
         uint32_t ue = INFBITS, ut = INFBITS, ue0 = INFBITS;
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) {
@@ -421,7 +439,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
               const float Tst = w.x; const int sfree = __float_as_int(w.z); const int k = __float_as_int(w.w);
               if (STATS) { n_swept += 1; n_cswept += (uint32_t)(sfree * d.F); }
               float arow[NPHI], m[NPHI];
-              ld_cols<NPHI>(v.gA0 + (size_t)k * FT, 0, phi0, FT, true, arow);   // rows are FT-padded: aligned
+              ld_lane<NPHI>(q_a0, (uint32_t)k * FT, true, arow);   // rows are FT-padded: aligned
       #pragma unroll
               for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
       #pragma unroll 4
@@ -468,6 +486,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       if (p.ok) {
         if (STATS) { n_scored += 1; n_cscored += (uint32_t)(p.smf * d.F); }
         const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
+        const LanePtr w_l1 = lane_ptr<NPHI>(l1, phi0, d.F, vec), w_p1 = lane_ptr<NPHI>(p1, phi0, d.F, vec);
         const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F;
         const float fr1 = __uint2float_rn(p.rounds1);
         // an empty prefill / decode slot passes its deadline whatever the wait (slot rule, q == 0)
@@ -486,8 +505,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int sr = min(s4 + u, p.smf - 1);
-            ld_cols<NPHI>(pw0, sr * d.F, phi0, d.F, vec, b0[u]);
-            ld_cols<NPHI>(l1, sr * d.F, phi0, d.F, vec, a1[u]); ld_cols<NPHI>(p1, sr * d.F, phi0, d.F, vec, b1[u]);
+            const uint32_t ro = (uint32_t)(sr * d.F);
+            ld_lane<NPHI>(q_p0, ro, vec, b0[u]); ld_lane<NPHI>(w_l1, ro, vec, a1[u]); ld_lane<NPHI>(w_p1, ro, vec, b1[u]);
             ld_tile<NPHI>(tl_t0 + sr * FT + phi0, tt[u]);
           }
 #pragma unroll
@@ -527,8 +546,9 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         const float fr1 = __uint2float_rn(p.rounds1);
         float tt[NPHI], b0[NPHI], a1[NPHI], b1[NPHI];
         ld_tile<NPHI>(tl_t0 + sgs * FT + phi0, tt);
-        ld_cols<NPHI>(pw0, sgs * d.F, phi0, d.F, vec, b0);
-        ld_cols<NPHI>(l1, sgs * d.F, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, sgs * d.F, phi0, d.F, vec, b1);
+        const LanePtr w_l1 = lane_ptr<NPHI>(l1, phi0, d.F, vec), w_p1 = lane_ptr<NPHI>(p1, phi0, d.F, vec);
+        const uint32_t ro = (uint32_t)(sgs * d.F);
+        ld_lane<NPHI>(q_p0, ro, vec, b0); ld_lane<NPHI>(w_l1, ro, vec, a1); ld_lane<NPHI>(w_p1, ro, vec, b1);
         uint32_t fmin = NONE32; float ttft = 0.0f, tbt = 0.0f;
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) {
