@@ -215,7 +215,7 @@ __device__ __forceinline__ unsigned long long block_min_key(unsigned long long k
   return sred[0];
 }
 
-__global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
+__global__ void __launch_bounds__(512) local_split_kernel(FsView v, int n,
                                                          const int32_t* __restrict__ gpu_ids,
                                                          uint32_t flags,
                                                          const float* __restrict__ Gs,
@@ -280,12 +280,15 @@ __global__ void __launch_bounds__(256) local_split_kernel(FsView v, int n,
     // offsets of a split are formed once; (cost, flat) compared in full because flat = phi*NS + rank is
     // not visited in ascending order
     float bestC = FS_INF; uint32_t bflat = 0xFFFFFFFFu;
-    for (uint32_t rank = threadIdx.x; rank < NS; rank += blockDim.x) {
+    // few splits (1 / 15 / 105 for 1-3 tenants): PG thread groups share them and divide the frequencies
+    const uint32_t PG = NS >= blockDim.x ? 1u : min((uint32_t)d.F, blockDim.x / NS);
+    const uint32_t pg = PG > 1 ? threadIdx.x / NS : 0u;
+    for (uint32_t rank = PG > 1 ? threadIdx.x % NS : threadIdx.x; rank < NS && pg < PG; rank += PG > 1 ? NS : blockDim.x) {
       const uint32_t pk = cp[rank];
       int off[FS_RMAX];
 #pragma unroll
       for (int i = 0; i < FS_RMAX; ++i) off[i] = (i < n_res ? i : 0) * rows + (int)((pk >> (8 * i)) & 0xFF);
-      for (int phi = 0; phi < d.F; ++phi) {
+      for (int phi = (int)pg; phi < d.F; phi += (int)PG) {
         float C = sG[off[0] + phi * d.S];
 #pragma unroll
         for (int i = 1; i < FS_RMAX; ++i) if (i < n_res) C = __fadd_rn(C, sG[off[i] + phi * d.S]);
@@ -422,7 +425,7 @@ int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs
   fs_tm_end(tm, FS_T_LOCAL_SLOT, st);
   const size_t smem = sizeof(float) * FS_RMAX * rows;
   fs_tm_beg(tm, FS_T_LOCAL_SPLIT, st);
-  local_split_kernel<<<n, 256, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.comp, sc.comp_n,
+  local_split_kernel<<<n, 512, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.comp, sc.comp_n,
                                            sc.ns_stride, out);
   fs_tm_end(tm, FS_T_LOCAL_SPLIT, st);
   return launches + 1;
