@@ -581,3 +581,20 @@ def test_random_clusters_all_entry_points(ctx, block):
             cl.states["mem_free_mb"] *= 0.02
         _check_all(ctx, cl)
         cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
+
+
+def test_fig8_step3_through_cuda(ctx):
+    """Fig. 8 step 3 (tests/golden/fig8_step3.txt) through fs_local_config."""
+    from test_oracle_pins import _fig8_cluster
+    from test_golden import _rows
+    rows = [[int(x) for x in r] for r in _rows("fig8_step3.txt")]
+    cl = _fig8_cluster()
+    ctx.load_profiles(cl.lat, cl.pow, np.array([r[0] for r in rows], np.float32), cl.models, synth.Params())
+    ctx.set_gpu_state(cl.states)
+    o = ctx.local_config(3 - 1)[0]                    # FS_OBJ_ENERGY | FS_SPLIT_MINSM
+    chosen = min([r for r in rows if r[5]], key=lambda r: r[6])
+    assert rows[int(o["phi"])][0] == chosen[0] == 1100
+    assert tuple((int(s) + 1) * 10 for s in o["sigma"]) == tuple(chosen[1:5])
+    assert o["energy_mj"] == np.float32(chosen[6] * 1000.0)
+    for fl in ALL_FLAGS:
+        cmp.assert_local_equal(ctx.local_config(fl), _oracle_local(cl, fl))
