@@ -466,8 +466,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="pod", choices=list(synth.CONFIGS))
-    ap.add_argument("--cpu-requests", type=int, default=1536, help="oracle sample of the cpu_baseline leg")
-    ap.add_argument("--ref-requests", type=int, default=256, help="oracle sample per step of --impl reference")
+    ap.add_argument("--cpu-requests", type=int, default=12288, help="oracle sample of the cpu_baseline leg")
+    ap.add_argument("--ref-requests", type=int, default=1024, help="oracle sample per step of --impl reference")
     ap.add_argument("--cpu-gpus", type=int, default=4096, help="oracle sample (GPUs) of --workload local")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
