@@ -148,6 +148,13 @@ constexpr int DENSE_MAXW = 20;                // warps per block at most (regist
 constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
 constexpr int DENSE_S = 16;
 
+// does any of the four 16-bit models packed in (w0, w1) equal m?  (exact "has a zero halfword" test on the
+// XOR; the SIMD-in-a-word video instructions are emulated on this architecture and cost ~30 instructions)
+__device__ __forceinline__ bool has_model(uint32_t w0, uint32_t w1, uint32_t mm) {
+  const uint32_t x0 = w0 ^ mm, x1 = w1 ^ mm;
+  return ((((x0 - 0x00010001u) & ~x0) | ((x1 - 0x00010001u) & ~x1)) & 0x80008000u) != 0u;
+}
+
 __device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) {
   uint32_t r;
   asm volatile("redux.sync.min.u32 %0, %1, 0xffffffff;" : "=r"(r) : "r"(x));
@@ -412,7 +419,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
             const uint32_t mm = (uint32_t)c.m * 0x00010001u;
             const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
-            const bool el = (c.mem <= g.mem_free_mb) && !(__vcmpeq2(gm[0], mm) | __vcmpeq2(gm[1], mm));
+            const bool el = (c.mem <= g.mem_free_mb) && !has_model(gm[0], gm[1], mm);
             float T = -1.0f;
             if (el) {
               if (STATS) { n_elig += 1; }
@@ -658,7 +665,7 @@ __device__ __forceinline__ DispPair disp_pair(const FsView& v, const ReqCtx& c, 
   if (tl_t0) {
     // resident model: a WARM pair, scored from the per-model list instead (a rare lane would make
     // the whole warp take the slow path in almost every chunk)
-    if ((__vcmpeq2(gm[0], mm) | __vcmpeq2(gm[1], mm)) || n_res >= FS_RMAX) return r;
+    if (has_model(gm[0], gm[1], mm) || n_res >= FS_RMAX) return r;
     const int o = (smf - 1) * FT + phi;
     r.e = tl_er[o];
     r.ok = (c.L == 0 || __fadd_rn(__fadd_rn(g.t_avail_ms, c.load_ms), tl_t0[o]) <= c.slo_ttft) && r.e < FS_INF;
