@@ -153,7 +153,7 @@ def run_reference(args):
 def _config(cl, args):
     return {"workload": f"{cl.name} (BASELINE.json configs[2]): K={cl.K} GPUs, M={cl.M}, F={cl.F}, S={cl.S}, "
                         f"B={cl.B}, R={cl.R} requests per rank; step = fs_set_gpu_state + fs_place_batch + "
-                        f"fs_local_config(all GPUs, energy objective, exhaustive splits)",
+                        f"fs_local_config(all GPUs, energy objective, exhaustive splits)" + ("; the two calls on two streams" if args.overlap else ""),
             "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B, "R_per_rank": cl.R,
             "l2": "flushed between timed steps by overwriting a 256 MiB buffer",
             "parallelism": f"replicated tables+state, requests sharded x{args.gpus}"}
@@ -187,10 +187,23 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     ctx.set_timing(True)
 
-    def step_device():
+    # fs_place_batch and fs_local_config both depend only on the state: the step issues them on two
+    # streams so that the slot search fills the issue slots the placement kernel leaves (same host thread)
+    side = torch.cuda.Stream(device=dev) if args.overlap else None
+    ev_state, ev_side = torch.cuda.Event(), torch.cuda.Event()
+
+    def step_device(serial=False):
         ctx.set_gpu_state(d_states, stream=stream)
+        if side is None or serial:
+            ctx.place_batch(d_reqs, out=d_place, stream=stream)
+            ctx.local_config(0, n=cl.K, out=d_local, stream=stream)
+            return
+        ev_state.record(stream)
+        side.wait_event(ev_state)
+        ctx.local_config(0, n=cl.K, out=d_local, stream=side)
         ctx.place_batch(d_reqs, out=d_place, stream=stream)
-        ctx.local_config(0, n=cl.K, out=d_local, stream=stream)
+        ev_side.record(side)
+        stream.wait_event(ev_side)
 
     def barrier():
         torch.cuda.synchronize()
@@ -214,12 +227,25 @@ def run_ours(args):
         step_device()
         b.record(stream)
         b.synchronize()
-        for k, v in ctx.get_timing().items():
-            kt.setdefault(k, []).append(v)
+        if side is None:
+            for k, v in ctx.get_timing().items():
+                kt.setdefault(k, []).append(v)
     barrier()
     wall = time.perf_counter() - wall0
     launches = ctx.launch_count - l0
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
+    # per-kernel durations need the kernels one after the other: when the timed steps overlap the two calls,
+    # the same K steps are run once more serially (same inputs, L2 flushed) for kernel_ms and the roofline
+    serial_ms = dev_ms
+    if side is not None:
+        serial_ms = 0.0
+        for _ in range(args.steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); step_device(serial=True); b.record(stream); b.synchronize()
+            serial_ms += a.elapsed_time(b)
+            for k, v in ctx.get_timing().items():
+                kt.setdefault(k, []).append(v)
     # work counters: one untimed call of the counting instantiation (same input, same work)
     ctx.set_work_stats(True)
     ctx.place_batch(d_reqs, out=d_place, stream=stream)
@@ -299,6 +325,10 @@ def run_ours(args):
         "nominal_candidates_per_step": grid_cands, "eligible_candidates_per_step": cand_def,
         "eligible_pairs_per_step": pairs, "place_stats": pstats,
         "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
+        "serial": {"ms_per_step": serial_ms / steps,
+                   "note": ("timed steps run fs_place_batch and fs_local_config on two streams; kernel_ms and the "
+                            "roofline come from the same steps run serially right after" if args.overlap else
+                            "timed steps are serial: kernel_ms comes from them")},
         "wall_ms_per_step_incl_flush": wall_ms / steps,
         "e2e": {"value": ws * grid_cands * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
                 "h2d_bytes_per_step": cl.K * 128 + cl.R * 32, "d2h_bytes_per_step": cl.R * 32 + cl.K * 48},
@@ -470,6 +500,7 @@ def main():
     ap.add_argument("--ref-requests", type=int, default=1024, help="oracle sample per step of --impl reference")
     ap.add_argument("--cpu-gpus", type=int, default=4096, help="oracle sample (GPUs) of --workload local")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--overlap", type=int, default=1, help="1: fs_local_config on a second stream beside fs_place_batch")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
