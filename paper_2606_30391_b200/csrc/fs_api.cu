@@ -16,7 +16,7 @@ struct fs_ctx {
   fs_params prm{0, 0, 0, 0};
   bool have_prof = false, have_state = false, place_ready = false;
   // profiles
-  float *lat = nullptr, *pow = nullptr, *latT = nullptr, *powT = nullptr, *freq = nullptr;
+  float *lat = nullptr, *pow = nullptr, *latT = nullptr, *powT = nullptr, *freq = nullptr; float2* dmin = nullptr; size_t dmin_cap = 0;
   fs_model_info* models = nullptr;
   size_t table_cap = 0; int m_cap = 0, f_cap = 0;
   uint32_t *comp = nullptr, *comp_n = nullptr; int ns_stride = 1; size_t comp_cap = 0;
@@ -84,7 +84,7 @@ int check_kernel(fs_ctx* c) {
 FsView view_of(const fs_ctx* c) {
   FsView v;
   v.d = FsDimsDev{c->d.M, c->d.F, c->d.S, c->d.B};
-  v.lat = c->lat; v.pow = c->pow; v.latT = c->latT; v.powT = c->powT; v.models = c->models;
+  v.lat = c->lat; v.pow = c->pow; v.latT = c->latT; v.powT = c->powT; v.dmin = c->dmin; v.models = c->models;
   v.K = c->K; v.states = c->states; v.ginfo = c->ginfo; v.gA = c->gA; v.flag = c->flag_dev;
   v.grec = c->grec; v.gA0 = c->gA0; v.Kpad = c->Kpad; v.FT = c->FT; v.gsort = c->gsort; v.dsuf = c->dsuf;
   return v;
@@ -166,7 +166,7 @@ int fs_destroy(fs_ctx* c) {
   if (!c) return FS_ERR_ARG;
   cudaSetDevice(c->dev);
   cudaDeviceSynchronize();
-  void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->freq, c->models, c->comp, c->comp_n, c->states,
+  void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->dmin, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf, c->pl_buf};
@@ -216,7 +216,9 @@ int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const flo
   FS_CUDA(c, cudaMemcpyAsync(c->comp_n, comp_n, sizeof(comp_n), cudaMemcpyHostToDevice, st));
   FS_CUDA(c, cudaStreamSynchronize(st));
   c->ns_stride = stride;
-  c->launches += fsk_build_planes(c->lat, c->pow, c->latT, c->powT,
+  { const size_t nd = (size_t)dims->M * dims->B * dims->S;
+    if (nd > c->dmin_cap) { FS_TRY(grow(c, c->dmin, nd)); c->dmin_cap = nd; } }
+  c->launches += fsk_build_planes(c->lat, c->pow, c->latT, c->powT, c->dmin,
                                   FsDimsDev{dims->M, dims->F, dims->S, dims->B}, c->flag_dev, st);
   FS_TRY(check_kernel(c));
   c->have_prof = true;

@@ -23,6 +23,7 @@ struct FsView {
   const float* pow;
   const float* latT;   // [M][2][B][S][F]
   const float* powT;
+  const float2* dmin;  // [M][B][S]  {min LAT, min POW} of the decode plane over shares <= s, all phi
   const fs_model_info* models;
   int K;
   const fs_gpu_state* states;
@@ -38,7 +39,7 @@ struct FsView {
 };
 
 // fs_tables.cu — validate (finite, > 0) and build the plane layout
-int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, FsDimsDev d,
+int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, float2* dmin, FsDimsDev d,
                      int* flag, cudaStream_t st);
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum

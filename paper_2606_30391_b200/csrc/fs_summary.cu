@@ -242,19 +242,12 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
   const FsDimsDev d = v.d;
   const int m = gi.model[i], br1 = gi.br1[i];
   float a_min = FS_INF, l1 = FS_INF, p1 = FS_INF;
-  for (int phi = lane; phi < d.F; phi += 32) {
-    a_min = fminf(a_min, v.gA[((size_t)k * FS_NVAR + 1 + i) * d.F + phi]);
-    if (br1 >= 0)
-      for (int sg = 0; sg < gi.sm_free; ++sg) {
-        const size_t o = fs_plane(d, m, 1, br1) + (size_t)sg * d.F + phi;
-        l1 = fminf(l1, v.latT[o]); p1 = fminf(p1, v.powT[o]);
-      }
-  }
+  for (int phi = lane; phi < d.F; phi += 32) a_min = fminf(a_min, v.gA[((size_t)k * FS_NVAR + 1 + i) * d.F + phi]);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
-    l1 = fminf(l1, __shfl_xor_sync(0xffffffffu, l1, o));
-    p1 = fminf(p1, __shfl_xor_sync(0xffffffffu, p1, o));
+  for (int o = 16; o > 0; o >>= 1) a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
+  if (br1 >= 0 && gi.sm_free >= 1) {                   // minima over shares < sm_free, all phi: one lookup
+    const float2 mn = v.dmin[((size_t)m * d.B + br1) * d.S + gi.sm_free - 1];
+    l1 = mn.x; p1 = mn.y;
   }
   if (lane == 0) {
     FsWarmItem it;

@@ -45,11 +45,34 @@ __global__ void __launch_bounds__(256) build_planes_kernel(const float* __restri
   if (bad) fs_raise(flag, FS_FLAG_TABLE);
 }
 
+// dmin[m][b][s] = { min LAT, min POW } of the decode plane (m, 1, b) over shares <= s and all phi: the
+// bounds l1_min / p1_min of a warm (GPU, slot) item are then one lookup at (model, bucket, sm_free - 1)
+__global__ void __launch_bounds__(128) decode_min_kernel(const float* __restrict__ latT, const float* __restrict__ powT,
+                                                        FsDimsDev d, float2* __restrict__ dmin) {
+  const int lane = threadIdx.x & 31;
+  const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (w >= d.M * d.B) return;
+  const int m = w / d.B, b = w % d.B;
+  const float* pl = latT + fs_plane(d, m, 1, b); const float* pp = powT + fs_plane(d, m, 1, b);
+  float ml = FS_INF, mp = FS_INF;
+  for (int s = 0; s < d.S; ++s) {
+    float l = FS_INF, p = FS_INF;
+    for (int phi = lane; phi < d.F; phi += 32) { l = fminf(l, pl[s * d.F + phi]); p = fminf(p, pp[s * d.F + phi]); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      l = fminf(l, __shfl_xor_sync(0xffffffffu, l, o)); p = fminf(p, __shfl_xor_sync(0xffffffffu, p, o));
+    }
+    ml = fminf(ml, l); mp = fminf(mp, p);
+    if (lane == 0) dmin[(size_t)w * d.S + s] = make_float2(ml, mp);
+  }
+}
+
 }  // namespace
 
-int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, FsDimsDev d,
+int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, float2* dmin, FsDimsDev d,
                      int* flag, cudaStream_t st) {
   const long long blocks = (long long)d.M * 2 * d.S * ((d.F + 31) / 32) * ((d.B + 31) / 32);
   build_planes_kernel<<<(unsigned)blocks, 256, 0, st>>>(lat, pow, latT, powT, d, flag);
-  return 1;
+  decode_min_kernel<<<(d.M * d.B + 3) / 4, 128, 0, st>>>(latT, powT, d, dmin);
+  return 2;
 }
