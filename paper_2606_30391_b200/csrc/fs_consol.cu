@@ -63,14 +63,13 @@ __global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
     const float4* __restrict__ agg, unsigned long long* __restrict__ keys) {
   extern __shared__ unsigned char smem_raw[];
   const int F = v.d.F, K = v.K;
-  float* sE = reinterpret_cast<float*>(smem_raw);                  // [F][TA]
-  int* sN = reinterpret_cast<int*>(smem_raw + sizeof(float) * F * TA);   // [F][TA]
+  float2* sEN = reinterpret_cast<float2*>(smem_raw);               // [F][TA] {E_a, need_a as int bits}: one LDS.64
   __shared__ unsigned long long sred[TA][PAIR_THREADS / 32];
   const int a0 = blockIdx.x * TA;
   for (int x = threadIdx.x; x < F * TA; x += blockDim.x) {
     const int phi = x / TA, a = a0 + x % TA;
-    sE[x] = a < K ? E[(size_t)phi * K + a] : FS_INF;
-    sN[x] = a < K ? need[(size_t)phi * K + a] : FS_NEED_INF;
+    sEN[x] = make_float2(a < K ? E[(size_t)phi * K + a] : FS_INF,
+                         __int_as_float(a < K ? (int)need[(size_t)phi * K + a] : FS_NEED_INF));
   }
   __syncthreads();
   float4 ag[TA];
@@ -79,29 +78,44 @@ __global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
   unsigned long long best[TA];
 #pragma unroll
   for (int t = 0; t < TA; ++t) best[t] = FS_KEY_NONE;
-  for (int b = threadIdx.x; b < K; b += blockDim.x) {
-    float cab[TA];
+  // two destinations per thread and trip: the broadcast read of a source's (E, need) serves both; per
+  // (source, destination, phi) one add, one integer compare and one predicated min
+  for (int b0 = threadIdx.x; b0 < K; b0 += 2 * blockDim.x) {
+    const int b1 = b0 + blockDim.x;
+    const bool two = b1 < K;
+    const int b1c = two ? b1 : b0;
+    float cab0[TA], cab1[TA];
 #pragma unroll
-    for (int t = 0; t < TA; ++t) cab[t] = FS_INF;
+    for (int t = 0; t < TA; ++t) cab0[t] = cab1[t] = FS_INF;
     for (int phi = 0; phi < F; ++phi) {
-      const float eb = E[(size_t)phi * K + b];
-      const int nb = need[(size_t)phi * K + b];
+      const float e0 = E[(size_t)phi * K + b0], e1 = E[(size_t)phi * K + b1c];
+      const int thr0 = S_eff - (int)need[(size_t)phi * K + b0], thr1 = S_eff - (int)need[(size_t)phi * K + b1c];
 #pragma unroll
       for (int t = 0; t < TA; ++t) {
-        const float e = __fadd_rn(eb, sE[phi * TA + t]);
-        if (sN[phi * TA + t] + nb <= S_eff) cab[t] = fminf(cab[t], e);   // INF never wins
+        const float2 en = sEN[phi * TA + t];
+        const int na = __float_as_int(en.y);
+        asm("{.reg .pred p; setp.le.s32 p, %1, %2; @p min.f32 %0, %0, %3;}"    // INF never wins
+            : "+f"(cab0[t]) : "r"(na), "r"(thr0), "f"(__fadd_rn(e0, en.x)));
+        asm("{.reg .pred p; setp.le.s32 p, %1, %2; @p min.f32 %0, %0, %3;}"
+            : "+f"(cab1[t]) : "r"(na), "r"(thr1), "f"(__fadd_rn(e1, en.x)));
       }
     }
-    const float4 gb = agg[b];
-    const int n_b = __float_as_int(gb.w);
 #pragma unroll
-    for (int t = 0; t < TA; ++t) {
-      const int a = a0 + t, n_a = __float_as_int(ag[t].w);
-      const bool ok = a < K && a != b && n_a >= 1 && n_b >= 1 && n_a + n_b <= FS_RMAX &&
-                      (__fadd_rn(ag[t].x, gb.x) <= M_eff) && gb.y < FS_INF && cab[t] < FS_INF;
-      if (ok) {
-        const unsigned long long kk = fs_make_key(__fsub_rn(cab[t], gb.y), (uint32_t)b);
-        best[t] = kk < best[t] ? kk : best[t];
+    for (int h = 0; h < 2; ++h) {
+      if (h == 1 && !two) break;
+      const int b = h ? b1 : b0;
+      const float4 gb = agg[b];
+      const int n_b = __float_as_int(gb.w);
+#pragma unroll
+      for (int t = 0; t < TA; ++t) {
+        const float cab = h ? cab1[t] : cab0[t];
+        const int a = a0 + t, n_a = __float_as_int(ag[t].w);
+        const bool ok = a < K && a != b && n_a >= 1 && n_b >= 1 && n_a + n_b <= FS_RMAX &&
+                        (__fadd_rn(ag[t].x, gb.x) <= M_eff) && gb.y < FS_INF && cab < FS_INF;
+        if (ok) {
+          const unsigned long long kk = fs_make_key(__fsub_rn(cab, gb.y), (uint32_t)b);
+          best[t] = kk < best[t] ? kk : best[t];
+        }
       }
     }
   }
@@ -157,7 +171,7 @@ int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
   fs_tm_beg(tm, FS_T_CONSOL_AGG, st);
   consol_agg_kernel<<<(v.K + 3) / 4, 128, 0, st>>>(v, S_eff, sc.need, sc.E, sc.agg);
   fs_tm_end(tm, FS_T_CONSOL_AGG, st);
-  const size_t smem = (sizeof(float) + sizeof(int)) * v.d.F * TA;
+  const size_t smem = sizeof(float2) * v.d.F * TA;
   fs_tm_beg(tm, FS_T_CONSOL_PAIR, st);
   consol_pair_kernel<<<(v.K + TA - 1) / TA, PAIR_THREADS, smem, st>>>(v, S_eff, M_eff, sc.need,
                                                                     sc.E, sc.agg, sc.keys);
