@@ -317,8 +317,8 @@ int fs_get_timing(fs_ctx* ctx, float* ms, int n);
 /* Measurement only: issue rates of the instruction classes the path is made of, in thread-instructions per
  * clock per SM at the SM clock `sm_mhz` (read it from nvidia-smi under load): out[0] FMUL, out[1] FADD,
  * out[2] FMNMX, out[3] FSETP + predicated FMNMX (per instruction), out[4] IMNMX, out[5] ISETP + SEL (per
- * instruction).  DESIGN.md section 7 checks the "alu" roofline peak (128 per clock per SM) against them.         */
-int fs_probe_pipe_rates(int cuda_device, double sm_mhz, double* out /*[6]*/);
+ * instruction), out[6] FSET mask + OR + unsigned min (per instruction).  DESIGN.md section 7 checks the "alu" roofline peak (128 per clock per SM) against them.         */
+int fs_probe_pipe_rates(int cuda_device, double sm_mhz, double* out /*[7]*/);
 
 #ifdef __cplusplus
 }

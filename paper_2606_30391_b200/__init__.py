@@ -40,11 +40,11 @@ class FsParams(C.Structure):
 
 def probe_pipe_rates(device: int = 0, sm_mhz: float = 1965.0) -> dict:
     """Issue rates (thread-instructions per clock per SM) of the path's instruction classes (measurement only)."""
-    o = (C.c_double * 6)()
+    o = (C.c_double * 7)()
     rc = lib().fs_probe_pipe_rates(device, sm_mhz, o)
     if rc != FS_OK:
         raise FestinaError(rc, "fs_probe_pipe_rates")
-    names = ("fmul", "fadd", "fmnmx", "fsetp_pred_fmnmx", "imnmx", "isetp_sel")
+    names = ("fmul", "fadd", "fmnmx", "fsetp_pred_fmnmx", "imnmx", "isetp_sel", "fset_or_umin")
     return {n: float(o[i]) for i, n in enumerate(names)}
 
 

@@ -25,6 +25,8 @@ __global__ void __launch_bounds__(1024) pipe_kernel(float* out, float seed) {
       if (OP == 4) asm volatile("min.s32 %0, %0, %1;" : "+r"(b[i]) : "r"(it));  // IMNMX
       if (OP == 5) asm volatile("{.reg .pred p; setp.le.s32 p, %0, %1; selp.s32 %0, %0, %2, p;}"
                                 : "+r"(b[i]) : "r"(it), "r"(i));                // ISETP + SEL
+      if (OP == 6) asm volatile("{.reg .u32 m; set.gt.u32.f32 m, %1, %2; or.b32 m, m, %3; min.u32 %0, %0, m;}"
+                                : "+r"(b[i]) : "f"(a[i]), "f"(c), "r"(it));     // FSET mask + LOP3 + unsigned min
     }
   }
   float s = 0.f;
@@ -51,7 +53,8 @@ double run_pipe(float* d_out, int sms, double sm_hz, int per_iter) {
 
 }  // namespace
 
-// out[6]: FMUL, FADD, FMNMX, FSETP+@FMNMX (per instruction), IMNMX, ISETP+SEL (per instruction)
+// out[7]: FMUL, FADD, FMNMX, FSETP+@FMNMX (per instruction), IMNMX, ISETP+SEL (per instruction),
+//         FSET mask + OR + unsigned min (per instruction)
 extern "C" int fs_probe_pipe_rates(int cuda_device, double sm_mhz, double* out) {
   if (!out || sm_mhz <= 0) return FS_ERR_ARG;
   if (cudaSetDevice(cuda_device) != cudaSuccess) { cudaGetLastError(); return FS_ERR_CUDA; }
@@ -63,6 +66,7 @@ extern "C" int fs_probe_pipe_rates(int cuda_device, double sm_mhz, double* out) 
   out[0] = run_pipe<0>(d_out, sms, hz, 1); out[1] = run_pipe<1>(d_out, sms, hz, 1);
   out[2] = run_pipe<2>(d_out, sms, hz, 1); out[3] = run_pipe<3>(d_out, sms, hz, 2);
   out[4] = run_pipe<4>(d_out, sms, hz, 1); out[5] = run_pipe<5>(d_out, sms, hz, 2);
+  out[6] = run_pipe<6>(d_out, sms, hz, 3);
   cudaFree(d_out);
   return cudaGetLastError() == cudaSuccess ? FS_OK : FS_ERR_CUDA;
 }
