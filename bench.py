@@ -153,7 +153,7 @@ def run_reference(args):
 def _config(cl, args):
     return {"workload": f"{cl.name} (BASELINE.json configs[2]): K={cl.K} GPUs, M={cl.M}, F={cl.F}, S={cl.S}, "
                         f"B={cl.B}, R={cl.R} requests per rank; step = fs_set_gpu_state + fs_place_batch + "
-                        f"fs_local_config(all GPUs, energy objective, exhaustive splits)" + ("; the two calls on two streams" if args.overlap else ""),
+                        f"fs_local_config(all GPUs, energy objective, exhaustive splits)" + ("; the two calls on two streams" if args.overlap else "") + ("; one CUDA graph per step" if args.graph else ""),
             "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B, "R_per_rank": cl.R,
             "l2": "flushed between timed steps by overwriting a 256 MiB buffer",
             "parallelism": f"replicated tables+state, requests sharded x{args.gpus}"}
@@ -192,18 +192,19 @@ def run_ours(args):
     side = torch.cuda.Stream(device=dev) if args.overlap else None
     ev_state, ev_side = torch.cuda.Event(), torch.cuda.Event()
 
-    def step_device(serial=False):
-        ctx.set_gpu_state(d_states, stream=stream)
+    def step_device(serial=False, st=None):
+        st = stream if st is None else st
+        ctx.set_gpu_state(d_states, stream=st)
         if side is None or serial:
-            ctx.place_batch(d_reqs, out=d_place, stream=stream)
-            ctx.local_config(0, n=cl.K, out=d_local, stream=stream)
+            ctx.place_batch(d_reqs, out=d_place, stream=st)
+            ctx.local_config(0, n=cl.K, out=d_local, stream=st)
             return
-        ev_state.record(stream)
+        ev_state.record(st)
         side.wait_event(ev_state)
         ctx.local_config(0, n=cl.K, out=d_local, stream=side)
-        ctx.place_batch(d_reqs, out=d_place, stream=stream)
+        ctx.place_batch(d_reqs, out=d_place, stream=st)
         ev_side.record(side)
-        stream.wait_event(ev_side)
+        st.wait_event(ev_side)
 
     def barrier():
         torch.cuda.synchronize()
@@ -213,6 +214,28 @@ def run_ours(args):
 
     for _ in range(max(args.warmup, 3)):
         step_device()
+    barrier()
+    # The calls are asynchronous and allocation-free after the first step, so a whole step (fork to the second
+    # stream and join included) can be captured into a CUDA graph and replayed: one launch per step for the host.
+    graph, launches_per_step = None, None
+    if args.graph:
+        try:
+            ctx.set_timing(False)                       # event records of the per-kernel timers are not capturable
+            cap = torch.cuda.Stream(device=dev)
+            cap.wait_stream(stream)
+            lc = ctx.launch_count
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=cap):
+                step_device(st=torch.cuda.current_stream())
+            launches_per_step = ctx.launch_count - lc
+            stream.wait_stream(cap)
+            for _ in range(3):
+                graph.replay()
+            torch.cuda.synchronize()
+        except Exception as e:                          # noqa: BLE001 - fall back to direct launches
+            print(f"bench.py: CUDA graph capture failed ({e}); timing direct launches", file=sys.stderr)
+            graph = None
+        ctx.set_timing(True)
     barrier()
     sampler = ClockSampler(lrank)
     sampler.start()
@@ -224,20 +247,23 @@ def run_ours(args):
     for a, b in evs:
         flush.zero_()                      # L2 flush, outside the per-step events
         a.record(stream)
-        step_device()
+        if graph is not None:
+            graph.replay()
+        else:
+            step_device()
         b.record(stream)
         b.synchronize()
-        if side is None:
+        if side is None and graph is None:
             for k, v in ctx.get_timing().items():
                 kt.setdefault(k, []).append(v)
     barrier()
     wall = time.perf_counter() - wall0
-    launches = ctx.launch_count - l0
+    launches = ctx.launch_count - l0 if graph is None else launches_per_step * args.steps
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
     # per-kernel durations need the kernels one after the other: when the timed steps overlap the two calls,
     # the same K steps are run once more serially (same inputs, L2 flushed) for kernel_ms and the roofline
     serial_ms = dev_ms
-    if side is not None:
+    if side is not None or graph is not None:
         serial_ms = 0.0
         for _ in range(args.steps):
             flush.zero_()
@@ -326,8 +352,10 @@ def run_ours(args):
         "eligible_pairs_per_step": pairs, "place_stats": pstats,
         "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
         "serial": {"ms_per_step": serial_ms / steps,
-                   "note": ("timed steps run fs_place_batch and fs_local_config on two streams; kernel_ms and the "
-                            "roofline come from the same steps run serially right after" if args.overlap else
+                   "note": ("timed steps run fs_place_batch and fs_local_config on two streams"
+                            + (", replayed from one CUDA graph per step" if graph is not None else "")
+                            + "; kernel_ms and the roofline come from the same steps run serially, launch by launch, "
+                              "right after" if (args.overlap or graph is not None) else
                             "timed steps are serial: kernel_ms comes from them")},
         "wall_ms_per_step_incl_flush": wall_ms / steps,
         "e2e": {"value": ws * grid_cands * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
@@ -500,6 +528,7 @@ def main():
     ap.add_argument("--ref-requests", type=int, default=1024, help="oracle sample per step of --impl reference")
     ap.add_argument("--cpu-gpus", type=int, default=4096, help="oracle sample (GPUs) of --workload local")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--graph", type=int, default=1, help="1: replay the device step from a CUDA graph")
     ap.add_argument("--overlap", type=int, default=1, help="1: fs_local_config on a second stream beside fs_place_batch")
     args = ap.parse_args()
     if args.impl == "reference":

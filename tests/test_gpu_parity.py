@@ -598,3 +598,38 @@ def test_fig8_step3_through_cuda(ctx):
     assert o["energy_mj"] == np.float32(chosen[6] * 1000.0)
     for fl in ALL_FLAGS:
         cmp.assert_local_equal(ctx.local_config(fl), _oracle_local(cl, fl))
+
+
+def test_step_is_capturable_into_a_cuda_graph(ctx):
+    """The device-buffer calls are asynchronous and allocation-free after the first step: a whole step with the
+    fork to a second stream and the join replays from one CUDA graph and gives the oracle's results."""
+    import torch
+    cl = synth.make_cluster("rack")
+    dev = torch.device("cuda:0")
+    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+    ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                      tb(cl.models), cl.params)
+    ds, dr = tb(cl.states), tb(cl.requests)
+    do = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+    dl = torch.empty(cl.K * 48, dtype=torch.uint8, device=dev)
+    side, ev0, ev1 = torch.cuda.Stream(), torch.cuda.Event(), torch.cuda.Event()
+
+    def step(st):
+        ctx.set_gpu_state(ds, stream=st)
+        ev0.record(st); side.wait_event(ev0)
+        ctx.local_config(0, n=cl.K, out=dl, stream=side)
+        ctx.place_batch(dr, out=do, stream=st)
+        ev1.record(side); st.wait_event(ev1)
+
+    warm = torch.cuda.Stream()
+    with torch.cuda.stream(warm):
+        step(warm)                                      # first call at these sizes allocates scratch
+    warm.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=warm):
+        step(torch.cuda.current_stream())
+    do.zero_(); dl.zero_()
+    g.replay(); g.replay()
+    torch.cuda.synchronize()
+    cmp.assert_placement_equal(do.cpu().numpy().view(synth.PLACEMENT_DT), _oracle_place(cl))
+    cmp.assert_local_equal(dl.cpu().numpy().view(synth.LOCAL_CFG_DT), _oracle_local(cl, 0))
