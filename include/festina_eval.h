@@ -24,7 +24,11 @@
  *     (the caller's cue to scale out).
  *   - All arithmetic is IEEE-754 binary32, round-to-nearest-even, no FMA contraction, in the
  *     bracketing DESIGN.md states; integer quantities are exact.
- *   - One context per host thread / stream; calls on one context are not re-entrant.
+ *   - One context per host thread; calls on one context are not re-entrant.  Calls that do not depend on
+ *     each other's outputs (fs_place_batch / fs_dispatch vs fs_local_config vs fs_consolidate, all after
+ *     fs_set_gpu_state) may be issued on different streams by that thread; the caller orders the streams.
+ *   - FS_DEVICE calls never synchronise and do not allocate once a call of the same sizes has run, so a
+ *     sequence of them can be captured into a CUDA graph (with fs_set_timing off) and replayed.
  *   - There is no CPU fallback: every entry point runs CUDA kernels on the context's device.
  */
 #ifndef FESTINA_EVAL_H
