@@ -633,3 +633,22 @@ def test_step_is_capturable_into_a_cuda_graph(ctx):
     torch.cuda.synchronize()
     cmp.assert_placement_equal(do.cpu().numpy().view(synth.PLACEMENT_DT), _oracle_place(cl))
     cmp.assert_local_equal(dl.cpu().numpy().view(synth.LOCAL_CFG_DT), _oracle_local(cl, 0))
+
+
+@pytest.mark.parametrize("variant", ["dynamic_power_x4", "cold_starts_feasible"])
+def test_pod_workload_variants_sampled(ctx, variant):
+    """configs[2] with a less degenerate shape: 4x the dynamic power (chosen frequencies spread over the levels)
+    or cheap weight loads (cold starts meet the TTFT deadline, so the sorted cold scan does the work)."""
+    cl = synth.make_cluster("pod")
+    if variant == "dynamic_power_x4":
+        cl.pow = (cl.pow + 3.0 * (cl.pow - cl.pow[:, :, :1])).astype(np.float32)
+    else:
+        cl.models["load_ms"] *= 0.05
+    ctx.load_cluster(cl)
+    got = ctx.place_batch(cl.requests)
+    idx = np.arange(0, cl.R, 256)
+    cmp.assert_placement_equal(got[idx], _oracle_place(cl, cl.requests[idx]))
+    ok = got["gpu"] >= 0
+    if variant == "dynamic_power_x4":
+        assert np.bincount(got["phi"][ok]).max() / ok.sum() < 0.5
+    cmp.assert_placement_equal(ctx.dispatch(cl.requests)[idx], _oracle_dispatch(cl, cl.requests[idx]))
