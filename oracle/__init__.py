@@ -71,6 +71,16 @@ def dispatch(lat, pow_, models, states, reqs, nthreads: int = 1) -> np.ndarray:
     return out
 
 
+def dispatch_commit(lat, pow_, models, states, reqs):
+    """The dispatcher with the sequential commit pass (reading s34 of PAPER.md lines 214-218):
+    returns (placements, the state records after the last commit)."""
+    out = np.zeros(len(reqs), dtype=_PLACEMENT_DT)
+    st = np.array(states, copy=True)
+    lib().fo_dispatch_commit(*_tables(lat, pow_), _p(models), C.c_int(len(st)), _p(st),
+                             C.c_int(len(reqs)), _p(reqs), _p(out))
+    return out, st
+
+
 def local_config(lat, pow_, states, flags: int, gpu_ids=None, nthreads: int = 1) -> np.ndarray:
     """fs_local_config by definition (Fig. 8 step 3)."""
     if gpu_ids is None:

@@ -260,6 +260,37 @@ void dispatch_one(const Tables& T, const ModelInfo* mi, const GpuState* gs, int 
   out = best;
 }
 
+// The sequential commit pass between the requests of one batch (reading R:s34 of
+// P:214-218): the requests are dispatched one after the other, in the caller's order, each against the
+// state the previous ones left.  A request sent to GPU k (phase 1 or 2) starts at its wait time with ALL
+// of SM_free_k units (Eq. 2: Latency(f_k, S_k, ...)) and holds them until it completes, so
+//   T_avail_k  <- fl(ttft + t_dec),  t_dec = fl(ceil(O/(beta+1)) * LAT1)   the earliest time the next
+//                                                                request can start there (SM_free as polled)
+//   mem_free_k <- fl(mem_free_k - Req_mem)      the memory stays reserved until the next poll
+//   F_curr_k   <- phi                           (phase 2 raised the clock to F_max; phase 1 leaves it)
+// A scale-out decision (gpu = -1) changes no record: activating a GPU is the caller's action.
+// The resident models of a GPU are those of the last poll (a second request of a model that was cold is
+// charged load_ms again: never an under-estimate of a TTFT).
+void dispatch_commit(const Tables& T, const ModelInfo* mi, GpuState* gs, int K, const Request* rq, int R,
+                     Placement* out) {
+  for (int r = 0; r < R; ++r) {
+    dispatch_one(T, mi, gs, K, rq[r], out[r]);
+    const Placement& p = out[r];
+    if (p.gpu < 0) continue;
+    const uint32_t O = (21u * rq[r].o_pred + 19u) / 20u;
+    const float mem = (float)(rq[r].L + O) * mi[rq[r].model].kv_mb_per_token;
+    float tdec = 0.0f;
+    if (O > 0) {
+      const uint32_t n = (uint32_t)p.beta + 1u;
+      tdec = (float)((O + n - 1u) / n) * p.tbt_ms;          // tbt_ms = LAT1 at the chosen point
+    }
+    GpuState& g = gs[p.gpu];
+    g.t_avail_ms = p.ttft_ms + tdec;
+    g.mem_free_mb = g.mem_free_mb - mem;
+    g.f_cur = p.phi;
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // Algorithm 1, Phase 1: per active LLM, from its average input / output length:
 //   (SM_p, F_p), (SM_d, F_d) = the LUT configurations that minimise the prefill / decode energy
@@ -752,6 +783,14 @@ int fo_dispatch(int M, int F, int S, int B, const float* lat, const float* pow,
   const ModelInfo* mi = (const ModelInfo*)models; const GpuState* gs = (const GpuState*)states;
   const Request* rq = (const Request*)reqs; Placement* o = (Placement*)out;
   par_for(R, nthreads, [&](int r) { dispatch_one(T, mi, gs, K, rq[r], o[r]); });
+  return 0;
+}
+
+// states is updated in place (the records after the last commit)
+int fo_dispatch_commit(int M, int F, int S, int B, const float* lat, const float* pow,
+                       const void* models, int K, void* states, int R, const void* reqs, void* out) {
+  Tables T{M, F, S, B, lat, pow};
+  dispatch_commit(T, (const ModelInfo*)models, (GpuState*)states, K, (const Request*)reqs, R, (Placement*)out);
   return 0;
 }
 
