@@ -153,6 +153,9 @@ typedef struct {
  * l.F = f_mhz (preferred frequency), t_ms = its execution time (the weight of Eq. 5).  16 bytes. */
 typedef struct { int32_t need_units; float mem_mb, f_mhz, t_ms; } fs_plan_llm;
 
+/* What the commit pass of fs_dispatch_commit changes in a GPU's record: 16 bytes. */
+typedef struct { float t_avail_ms, mem_free_mb; int32_t f_cur; uint32_t _pad; } fs_gpu_avail;
+
 /* One in-flight request at reconfiguration time: remaining computation on the source,
  * token state and KV-cache size, the bandwidth of its source -> destination link under the chosen
  * mapping, and the time to recompute its KV cache on the destination.  32 bytes.               */
@@ -231,6 +234,21 @@ int fs_consolidate(fs_ctx* ctx, fs_consol_out* out, int space, void* cuda_stream
  * a fresh GPU).  Requires K < 2^24.  reqs : [R]; out : [R]; both in `space`.                  */
 int fs_dispatch(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* out, int space,
                 void* cuda_stream);
+
+/* fs_dispatch with the sequential commit pass between the requests of one batch (
+ * R:s34 of P:214-218).  The requests are dispatched in the order given, each against the records the
+ * previous ones left.  A request sent to GPU k in phase 1 or 2 starts at its wait time with all of
+ * SM_free_k and holds it until it completes:
+ *   T_avail_k  <- fl(ttft + fl(ceil(O/(beta+1)) * tbt))   (its completion: when the next one can start)
+ *   mem_free_k <- fl(mem_free_k - Req_mem)                 (reserved until the next poll)
+ *   F_curr_k   <- phi                                       (the F_max retry leaves the GPU at F_max)
+ * Scale-out decisions (gpu = -1) change nothing; the resident models stay those of fs_set_gpu_state.
+ * The context's own GPU state is NOT modified: `after` ([K], may be NULL) receives the three fields of
+ * every GPU after the last commit; the caller feeds the next poll through fs_set_gpu_state.
+ * One thread block walks the requests (they are serial by definition); the GPUs are the parallel axis.
+ *   reqs : [R]; out : [R]; after : [K] or NULL; all in `space`.  Requires K < 2^24.              */
+int fs_dispatch_commit(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* out,
+                       fs_gpu_avail* after, int space, void* cuda_stream);
 
 /* Local scheduler steps 1-2 for n GPUs (Eq. 4, Fig. 8): unified priority
  * score of every runnable task at the GPU's current frequency, then priority-based batching with

@@ -23,7 +23,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_migration_plan", "fs_migration_select", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_dispatch_commit", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_migration_plan", "fs_migration_select", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_probe_pipe_rates", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm", "batch_tasks", "dispatch")
@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
     L.fs_llm_profiles.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_ewr.argtypes = [vp, i32, vp, vp, vp, i32, vp, vp, C.c_int, vp]
     L.fs_dispatch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
+    L.fs_dispatch_commit.argtypes = [vp, i32, vp, vp, vp, C.c_int, vp]
     L.fs_batch_tasks.argtypes = [vp, i32, vp, vp, vp, vp, i32, C.c_int, vp]
     L.fs_strerror.argtypes = [C.c_int]
     L.fs_strerror.restype = C.c_char_p
@@ -209,6 +210,24 @@ class Festina:
         assert spo == sp or R == 0
         self._check(lib().fs_dispatch(self._h, R, pr, po, sp, _stream_ptr(stream)), "fs_dispatch")
         return out
+
+    def dispatch_commit(self, reqs, out=None, after=None, R: int | None = None, stream=None):
+        """fs_dispatch_commit: the dispatcher with the sequential commit pass; returns (placements, the
+        (T_avail, free memory, F_curr) records after the last commit)."""
+        if R is None:
+            R = len(reqs) if not hasattr(reqs, "data_ptr") else reqs.numel() * reqs.element_size() // 32
+        pr, sp, keep = _buf(reqs, R * 32)
+        if sp is None:
+            sp = FS_HOST
+        if out is None:
+            assert sp == FS_HOST, "device inputs need device `out` / `after` tensors"
+            out = np.zeros(R, dtype=synth.PLACEMENT_DT)
+            after = np.zeros(self.K, dtype=synth.GPU_AVAIL_DT)
+        po, spo, keep2 = _buf(out, R * 32)
+        pa, spa, keep3 = _buf(after, self.K * 16)
+        assert (spo == sp or R == 0) and spa in (None, sp)
+        self._check(lib().fs_dispatch_commit(self._h, R, pr, po, pa, sp, _stream_ptr(stream)), "fs_dispatch_commit")
+        return out, after
 
     def local_config(self, flags: int = 0, gpu_ids=None, n: int | None = None, out=None, stream=None):
         if gpu_ids is not None and not hasattr(gpu_ids, "data_ptr"):

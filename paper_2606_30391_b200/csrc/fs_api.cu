@@ -401,6 +401,43 @@ static int a1_reserve(fs_ctx* c, size_t bytes) {
   return FS_OK;
 }
 
+int fs_dispatch_commit(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out, fs_gpu_avail* after,
+                       int space, void* cuda_stream) {
+  if (!c || R < 0 || (R > 0 && (!reqs || !out))) return FS_ERR_ARG;
+  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
+  if (c->K >= (1 << 24)) return FS_ERR_SHAPE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FS_CUDA(c, cudaSetDevice(c->dev));
+  const int pending = take_flags(c);
+  if (R == 0 && !after) return pending;
+  if (R > c->r_cap) {
+    FS_TRY(grow(c, c->keys, (size_t)R)); FS_TRY(grow(c, c->reqs_dev, (size_t)R));
+    FS_TRY(grow(c, c->place_dev, (size_t)R));
+    c->r_cap = R;
+  }
+  const fs_request* d_reqs = reqs; fs_placement* d_out = out; fs_gpu_avail* d_work = after;
+  const size_t wb = (size_t)(c->K > 0 ? c->K : 1) * sizeof(fs_gpu_avail);
+  if (space == FS_HOST || !after) {
+    FS_TRY(a1_reserve(c, wb));
+    d_work = reinterpret_cast<fs_gpu_avail*>(c->a1_buf);
+  }
+  if (space == FS_HOST && R > 0) {
+    FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
+    d_reqs = c->reqs_dev; d_out = c->place_dev;
+  }
+  c->launches += fsk_dispatch_commit(view_of(c), R, d_reqs, d_out, d_work, st, c->timing ? &c->tm : nullptr);
+  FS_TRY(check_kernel(c));
+  if (space == FS_HOST) {
+    if (R > 0) FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
+    if (after && c->K > 0) FS_CUDA(c, cudaMemcpyAsync(after, d_work, (size_t)c->K * sizeof(fs_gpu_avail), cudaMemcpyDeviceToHost, st));
+    FS_CUDA(c, cudaStreamSynchronize(st));
+    const int now = take_flags(c);
+    return pending != FS_OK ? pending : now;
+  }
+  return pending;
+}
+
 int fs_llm_profiles(fs_ctx* c, int32_t n, const fs_llm* llms, fs_llm_profile* out, int space, void* cuda_stream) {
   if (!c || n < 0 || (n > 0 && (!llms || !out))) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;

@@ -68,6 +68,8 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
 // the paper's three-phase dispatcher at (F_curr, SM_free)
 int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* out, const int32_t* warm_off,
                  const FsWarmItem* witems, cudaStream_t st, FsTimers* tm);
+int fsk_dispatch_commit(const FsView& v, int R, const fs_request* reqs, fs_placement* out, fs_gpu_avail* work,
+                        cudaStream_t st, FsTimers* tm);
 int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,
                          FsWarmItem* items /*[4K]*/, cudaStream_t st);
 

@@ -901,6 +901,126 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
   if (lane == 0) out[r] = o;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// fs_dispatch_commit: the dispatcher with the sequential commit pass between the requests of one batch
+// (the rest of NEXT-2; reading R:s34 of P:214-218).  The requests are inherently
+// serial (request r sees the records request r-1 left), so ONE block walks them in order; the parallel
+// axis is the GPUs: thread t owns GPUs t, t + blockDim, ... and is the only reader and writer of their
+// mutable record work[k] = (T_avail, free memory, F_curr).  Per request: one block-wide minimum for
+// E_min, one for the band's stability key (or the F_max retry's T_avail key); the owner of the winner
+// writes the decision and commits it.  Reductions alternate between two shared buffers: one barrier each.
+constexpr int CM_THREADS = 1024;
+
+__device__ __forceinline__ unsigned long long cm_block_min(unsigned long long x, unsigned long long (*buf)[CM_THREADS / 32],
+                                                           int& par, int nwarp, int warp, int lane) {
+  x = fs_warp_min_key(x);
+  if (lane == 0) buf[par][warp] = x;
+  __syncthreads();
+  unsigned long long y = lane < nwarp ? buf[par][lane] : FS_KEY_NONE;
+  par ^= 1;
+  return fs_warp_min_key(y);
+}
+
+struct CmEval { bool ok; PairCtx p; OwnEval ev; };
+// GPU k as the records stand now, at frequency phi (< 0: its F_curr)
+__device__ __forceinline__ CmEval cm_eval(const FsView& v, const ReqCtx& c, int k, const fs_gpu_avail& w, int phi) {
+  FsGpuInfo gi = v.ginfo[k];
+  gi.t_avail_ms = w.t_avail_ms; gi.mem_free_mb = w.mem_free_mb; gi.f_cur = w.f_cur;
+  CmEval r; r.p = make_pair(v, c, gi); r.ok = false;
+  if (!r.p.ok) return r;
+  r.ev = own_eval_planes(v, c, r.p.br1, r.p.rounds1, r.p.wait, r.p.smf - 1, phi < 0 ? gi.f_cur : phi);
+  r.ok = r.ev.ok;
+  return r;
+}
+
+__global__ void __launch_bounds__(CM_THREADS) dispatch_commit_kernel(FsView v, int R,
+                                                                     const fs_request* __restrict__ reqs,
+                                                                     fs_placement* __restrict__ out,
+                                                                     fs_gpu_avail* __restrict__ work) {
+  __shared__ unsigned long long s_buf[2][CM_THREADS / 32];
+  const FsDimsDev d = v.d;
+  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+  int par = 0;
+  for (int k = tid; k < v.K; k += nthr) {
+    const FsGpuInfo gi = v.ginfo[k];
+    fs_gpu_avail w; w.t_avail_ms = gi.t_avail_ms; w.mem_free_mb = gi.mem_free_mb; w.f_cur = gi.f_cur; w._pad = 0;
+    work[k] = w;
+  }
+  for (int r = 0; r < R; ++r) {
+    fs_placement o;
+    o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
+    o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
+    const ReqCtx c = make_req(v, reqs[r]);
+    if (!c.valid) { if (tid == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } continue; }
+    // ---- Phase 1 + 2 at F_curr: E_min over the feasible GPUs ------------------------------------
+    unsigned long long key = FS_KEY_NONE;
+    for (int k = tid; k < v.K; k += nthr) {
+      const CmEval e = cm_eval(v, c, k, work[k], -1);
+      if (e.ok) { const unsigned long long kk = fs_orderable(e.ev.e); key = kk < key ? kk : key; }
+    }
+    key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+    int kbest = -1, phase = -1, phibest = -1;
+    if (key != FS_KEY_NONE) {
+      const float band = __fmul_rn(1.02f, fs_unorderable((uint32_t)key));
+      key = FS_KEY_NONE;                                 // (most memory, largest SM_free, lowest k)
+      for (int k = tid; k < v.K; k += nthr) {
+        const fs_gpu_avail w = work[k];
+        const CmEval e = cm_eval(v, c, k, w, -1);
+        if (e.ok && e.ev.e <= band) {
+          const unsigned long long kk = ((unsigned long long)(~fs_orderable(w.mem_free_mb)) << 32) |
+                                        ((unsigned long long)(uint32_t)(d.S - e.p.smf) << 24) | (uint32_t)k;
+          key = kk < key ? kk : key;
+        }
+      }
+      key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+      kbest = (int)((uint32_t)key & 0xFFFFFFu); phase = 1;
+    } else {
+      // ---- Phase 3: F_max retry, first feasible GPU in T_avail order ----------------------------
+      for (int k = tid; k < v.K; k += nthr) {
+        const fs_gpu_avail w = work[k];
+        const CmEval e = cm_eval(v, c, k, w, d.F - 1);
+        if (e.ok) {
+          const unsigned long long kk = ((unsigned long long)fs_orderable(w.t_avail_ms) << 32) | (uint32_t)k;
+          key = kk < key ? kk : key;
+        }
+      }
+      key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+      if (key != FS_KEY_NONE) { kbest = (int)(uint32_t)key; phase = 2; phibest = d.F - 1; }
+    }
+    if (kbest >= 0) {
+      if (tid == kbest % nthr) {                         // the owner writes the decision and commits it
+        fs_gpu_avail w = work[kbest];
+        if (phase == 1) phibest = w.f_cur;
+        const CmEval e = cm_eval(v, c, kbest, w, phibest);
+        o.gpu = kbest; o.sigma = (int16_t)(e.p.smf - 1); o.phi = (int16_t)phibest; o.beta = (int16_t)e.p.br1;
+        o.f_req = (int16_t)phase; o.energy_mj = e.ev.e; o.ttft_ms = e.ev.ttft; o.tbt_ms = e.ev.tbt;
+        o.flat = (uint32_t)((kbest * d.S + e.p.smf - 1) * d.F + phibest);
+        out[r] = o;
+        const float tdec = c.O > 0 ? __fmul_rn(__uint2float_rn(e.p.rounds1), e.ev.tbt) : 0.f;
+        w.t_avail_ms = __fadd_rn(e.ev.ttft, tdec);
+        w.mem_free_mb = __fsub_rn(w.mem_free_mb, c.mem);
+        w.f_cur = phibest;
+        work[kbest] = w;
+      }
+    } else if (warp == 0) {
+      // ---- scale-out: energy-optimal feasible frequency of a fresh GPU; no record changes -------
+      key = FS_KEY_NONE;
+      for (int phi = lane; phi < d.F; phi += 32) {
+        const OwnEval ev = own_eval_planes(v, c, 0, c.O, c.load_ms, d.S - 1, phi);
+        if (ev.ok) { const unsigned long long kk = fs_make_key(ev.e, (uint32_t)phi); key = kk < key ? kk : key; }
+      }
+      key = fs_warp_min_key(key);
+      if (key != FS_KEY_NONE) {
+        const int phi = (int)(uint32_t)key;
+        const OwnEval ev = own_eval_planes(v, c, 0, c.O, c.load_ms, d.S - 1, phi);
+        o.sigma = (int16_t)(d.S - 1); o.phi = (int16_t)phi; o.beta = 0; o.f_req = 3;
+        o.energy_mj = ev.e; o.ttft_ms = ev.ttft; o.tbt_ms = ev.tbt;
+      }
+      if (lane == 0) out[r] = o;
+    }
+  }
+}
+
 }  // namespace
 
 int fsk_place_smem_attr() {
@@ -995,6 +1115,17 @@ int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* o
     if (block_mode) dispatch_kernel<2, true><<<grid, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
     else            dispatch_kernel<2, false><<<grid, DISP_WARPS * 32, smem, st>>>(v, R, reqs, out, use_tiles, warm_off, witems);
   }
+  fs_tm_end(tm, FS_T_DISPATCH, st);
+  return 1;
+}
+
+int fsk_dispatch_commit(const FsView& v, int R, const fs_request* reqs, fs_placement* out, fs_gpu_avail* work,
+                        cudaStream_t st, FsTimers* tm) {
+  if (R <= 0 && v.K <= 0) return 0;
+  int threads = ((v.K + 31) / 32) * 32;
+  threads = threads < 32 ? 32 : (threads > CM_THREADS ? CM_THREADS : threads);
+  fs_tm_beg(tm, FS_T_DISPATCH, st);
+  dispatch_commit_kernel<<<1, threads, 0, st>>>(v, R, reqs, out, work);
   fs_tm_end(tm, FS_T_DISPATCH, st);
   return 1;
 }

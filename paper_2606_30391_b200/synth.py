@@ -31,6 +31,7 @@ MODEL_INFO_DT = np.dtype(
 PLACEMENT_DT = np.dtype(
     [("gpu", "<i4"), ("sigma", "<i2"), ("phi", "<i2"), ("beta", "<i2"), ("f_req", "<i2"),
      ("energy_mj", "<f4"), ("ttft_ms", "<f4"), ("tbt_ms", "<f4"), ("flat", "<u4"), ("_pad", "<u4")])
+GPU_AVAIL_DT = np.dtype([("t_avail_ms", "<f4"), ("mem_free_mb", "<f4"), ("f_cur", "<i4"), ("_pad", "<u4")])
 LOCAL_CFG_DT = np.dtype(
     [("phi", "<i2"), ("f_req", "<i2"), ("sigma", "u1", (RMAX,)), ("beta", "u1", (RMAX, 2)),
      ("cost", "<f4"), ("energy_mj", "<f4"), ("power_w", "<f4"), ("flat", "<u4"),

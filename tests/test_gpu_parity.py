@@ -398,6 +398,92 @@ def test_dispatch_full_size(ctx):
     assert set(np.unique(got["f_req"]).tolist()) >= {1, 2, 3}
 
 
+# ---- the sequential commit pass (fs_dispatch_commit, reading s34) -------------------------------------
+def _assert_commit_equal(ctx, cl, reqs=None):
+    reqs = cl.requests if reqs is None else reqs
+    got, after = ctx.dispatch_commit(reqs)
+    ref, st = oracle.dispatch_commit(cl.lat, cl.pow, cl.models, cl.states, reqs)
+    cmp.assert_placement_equal(got, ref)
+    for f in ("t_avail_ms", "mem_free_mb", "f_cur"):
+        assert np.array_equal(after[f].view(np.uint32 if f != "f_cur" else np.int32),
+                              st[f].view(np.uint32 if f != "f_cur" else np.int32)), f"after.{f}"
+    return got
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_dispatch_commit_ragged_dims(ctx, seed):
+    st = synth.Stream(seed, "cdims")
+    K = int(st.randint(1, 1, [90, 2500][seed % 2])[0]); M = int(st.randint(1, 1, 9)[0])
+    F = int(st.randint(1, 1, [64, 100][seed % 3 == 0])[0]); S = int(st.randint(1, 1, 20)[0]); B = int(st.randint(1, 1, 40)[0])
+    cl = synth.make_custom(seed=1500 + seed, K=K, M=M, F=F, S=S, B=B, R=400, lo=1, hi=4)
+    if seed % 4 == 1:
+        cl.requests["slo_ttft_ms"] *= 0.1               # queues grow past the deadlines: phases 2 and 3
+    if seed % 4 == 2:
+        cl.states["mem_free_mb"] *= 0.01                # memory runs out during the batch
+    if seed % 4 == 3:
+        cl.states["mem_free_mb"] = 30000.0              # equal memory: the commit decides the tie-breaker
+    ctx.load_cluster(cl)
+    got = _assert_commit_equal(ctx, cl)
+    snap = ctx.dispatch(cl.requests)
+    assert got[0].tobytes() == snap[0].tobytes()
+    # the context's own state is untouched: the snapshot dispatcher gives the same answers afterwards
+    assert ctx.dispatch(cl.requests).tobytes() == snap.tobytes()
+
+
+def test_dispatch_commit_by_hand(ctx):
+    """tests/test_oracle_commit.py::test_commit_by_hand through the CUDA path."""
+    from test_oracle_dispatch import _toy, _gpu
+    lat, pw, models, st, rq = _toy(K=2, F=2)
+    rq = np.repeat(rq, 4); rq["o_pred"] = 20
+    for k, t_avail in enumerate([10.0, 0.0]):
+        _gpu(st, k, 1, 2, 0, t_avail, 1000.0)
+    lat[0, 0, 0, 1, 0] = 50.0; lat[0, 1, 0, 1, 0] = 2.0; pw[0, :, 0, 1, 0] = 1.0
+    lat[0, 0, 1, 1, 0] = 20.0; lat[0, 1, 1, 1, 0] = 1.0; pw[0, :, 1, 1, 0] = 9.0
+    st["mem_free_mb"][1] = 500.0
+    ctx.load_profiles(lat, pw, np.ones(2, np.float32), models, synth.Params())
+    ctx.set_gpu_state(st)
+    got, after = ctx.dispatch_commit(rq)
+    assert got["gpu"].tolist() == [0, 0, 1, 1] and got["ttft_ms"].tolist() == [60.0, 152.0, 50.0, 142.0]
+    assert after["t_avail_ms"].tolist() == [194.0, 184.0] and after["mem_free_mb"].tolist() == [956.0, 456.0]
+
+
+def test_dispatch_commit_edges(ctx):
+    import torch
+    cl = synth.make_custom(seed=1530, K=33, M=3, F=7, S=5, B=4, R=64, lo=1, hi=4)
+    ctx.load_cluster(cl)
+    got, after = ctx.dispatch_commit(cl.requests[:0])      # R = 0: the records as polled
+    assert len(got) == 0 and np.array_equal(after["t_avail_ms"], cl.states["t_avail_ms"])
+    assert np.array_equal(after["f_cur"], cl.states["f_cur"])
+    bad = cl.requests.copy(); bad["model"][5] = 99          # an invalid request is skipped, flagged on the next call
+    got = np.zeros(cl.R, dtype=synth.PLACEMENT_DT); aft = np.zeros(cl.K, dtype=synth.GPU_AVAIL_DT)
+    with pytest.raises(Exception):
+        ctx.dispatch_commit(bad, out=got, after=aft)
+    assert got["gpu"][5] == -1 and got["f_req"][5] == -1
+    ok = cl.requests.copy(); ok = np.delete(ok, 5)
+    ref, _ = oracle.dispatch_commit(cl.lat, cl.pow, cl.models, cl.states, ok)
+    cmp.assert_placement_equal(np.delete(got, 5), ref)
+    # device buffers
+    dreq = torch.from_numpy(cl.requests.view(np.uint8)).cuda()
+    dout = torch.zeros(cl.R * 32, dtype=torch.uint8, device="cuda"); daft = torch.zeros(cl.K * 16, dtype=torch.uint8, device="cuda")
+    ctx.dispatch_commit(dreq, out=dout, after=daft, R=cl.R)
+    torch.cuda.synchronize()
+    ref, st = oracle.dispatch_commit(cl.lat, cl.pow, cl.models, cl.states, cl.requests)
+    cmp.assert_placement_equal(dout.cpu().numpy().view(synth.PLACEMENT_DT), ref)
+    assert np.array_equal(daft.cpu().numpy().view(synth.GPU_AVAIL_DT)["t_avail_ms"], st["t_avail_ms"])
+
+
+def test_dispatch_commit_full_size(ctx):
+    """rack in full; the pod's 1,024 GPUs with its first 8,192 requests (the oracle replays them serially)."""
+    cl = synth.make_cluster("rack")
+    ctx.load_cluster(cl)
+    _assert_commit_equal(ctx, cl)
+    cl = synth.make_cluster("pod")
+    _mix_phases(cl, 5)
+    ctx.load_cluster(cl)
+    got = _assert_commit_equal(ctx, cl, cl.requests[:8192])
+    assert set(np.unique(got["f_req"]).tolist()) >= {1, 2}
+
+
 # ---- Algorithm 1 phase 1 (fs_llm_profiles) and the Energy Waste Ratio (fs_ewr) --------------------
 def _assert_profiles_equal(got, ref):
     for f in ("sigma_p", "phi_p", "sigma_d", "phi_d", "need_units", "phi_l"):
