@@ -636,18 +636,22 @@ constexpr int DISP_GC = 4;                    // chunks of 32 GPUs per group (on
 struct OwnEval { bool ok; float e, ttft, tbt; };
 
 // the request's own prefill + decode work at (phi, sg) on pair p, from the planes (definition)
+// the same from the four table entries (l0, p0: prefill; l1, p1: decode)
+__device__ __forceinline__ OwnEval own_eval_vals(const ReqCtx& c, uint32_t rounds1, float wait, float l0, float p0,
+                                                 float l1, float p1) {
+  bool ok = true; float t0 = 0.f, e0 = 0.f, e1 = 0.f;
+  if (c.L > 0) { FsSlot s = fs_slot(0, l0, p0, c.rounds0, wait, c.slo_ttft); ok = s.ok; t0 = s.t; e0 = s.e; }
+  if (c.O > 0) { FsSlot s = fs_slot(1, l1, p1, rounds1, 0.f, c.slo_tbt); ok = ok && s.ok; e1 = s.e; }
+  OwnEval r; r.e = __fadd_rn(e0, e1); r.ok = ok && r.e < FS_INF;
+  r.ttft = __fadd_rn(wait, t0); r.tbt = l1;
+  return r;
+}
 __device__ __forceinline__ OwnEval own_eval_planes(const FsView& v, const ReqCtx& c, int br1, uint32_t rounds1,
                                                    float wait, int sg, int phi) {
   const FsDimsDev& d = v.d;
   const size_t o = (size_t)sg * d.F + phi;
   const size_t i0 = fs_plane(d, c.m, 0, c.br0) + o, i1 = fs_plane(d, c.m, 1, br1) + o;
-  const float lat1 = v.latT[i1];
-  bool ok = true; float t0 = 0.f, e0 = 0.f, e1 = 0.f;
-  if (c.L > 0) { FsSlot s = fs_slot(0, v.latT[i0], v.powT[i0], c.rounds0, wait, c.slo_ttft); ok = s.ok; t0 = s.t; e0 = s.e; }
-  if (c.O > 0) { FsSlot s = fs_slot(1, lat1, v.powT[i1], rounds1, 0.f, c.slo_tbt); ok = ok && s.ok; e1 = s.e; }
-  OwnEval r; r.e = __fadd_rn(e0, e1); r.ok = ok && r.e < FS_INF;
-  r.ttft = __fadd_rn(wait, t0); r.tbt = lat1;
-  return r;
+  return own_eval_vals(c, rounds1, wait, v.latT[i0], v.powT[i0], v.latT[i1], v.powT[i1]);
 }
 
 struct DispPair { bool ok; float e; };
@@ -1021,6 +1025,148 @@ __global__ void __launch_bounds__(CM_THREADS) dispatch_commit_kernel(FsView v, i
   }
 }
 
+// The same pass with the GPUs in registers: thread t keeps the records of GPUs t, t + blockDim, ...
+// (KPT of them), so K <= KPT * blockDim.  The table entries of request r+1 at each GPU's F_curr are
+// requested right after request r has been scored and arrive while r's two reductions and its commit
+// run; a GPU whose F_curr the commit changed reloads its four entries.  What remains on the serial chain
+// of a request is arithmetic and two block-wide minima.
+struct CmPre { float l0, p0, l1, p1; int phi; };
+
+__device__ __forceinline__ CmPre cm_preload(const FsView& v, const ReqCtx& c, const FsGpuInfo& gi) {
+  CmPre q; q.l0 = q.p0 = q.l1 = q.p1 = 1.f; q.phi = -1;
+  if (!c.valid || gi.n_res < 1 || gi.sm_free < 1) return q;
+  const PairCtx p = make_pair(v, c, gi);                 // br1 depends on the tenants only
+  const FsDimsDev& d = v.d;
+  const size_t o = (size_t)(gi.sm_free - 1) * d.F + gi.f_cur;
+  const size_t i0 = fs_plane(d, c.m, 0, c.br0) + o, i1 = fs_plane(d, c.m, 1, p.br1) + o;
+  q.l0 = v.latT[i0]; q.p0 = v.powT[i0]; q.l1 = v.latT[i1]; q.p1 = v.powT[i1]; q.phi = gi.f_cur;
+  return q;
+}
+
+constexpr int CMR_THREADS = 512;                  // 128 registers per thread: the records of up to 4 GPUs
+template <int KPT>
+__global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView v, int R,
+                                                                         const fs_request* __restrict__ reqs,
+                                                                         fs_placement* __restrict__ out,
+                                                                         fs_gpu_avail* __restrict__ work) {
+  __shared__ unsigned long long s_buf[2][CM_THREADS / 32];
+  const FsDimsDev d = v.d;
+  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+  int par = 0;
+  FsGpuInfo gi[KPT]; CmPre pre[KPT];
+#pragma unroll
+  for (int u = 0; u < KPT; ++u) {
+    const int k = tid + u * nthr;
+    if (k < v.K) gi[u] = v.ginfo[k];
+    else { gi[u] = FsGpuInfo{}; gi[u].n_res = 0; }
+  }
+  fs_request rq_nx{};                                  // the raw request after the next one to be scored
+  if (R > 0) rq_nx = reqs[0];
+  ReqCtx cn = make_req(v, rq_nx);
+  if (R == 0) cn.valid = false;
+  if (R > 1) rq_nx = reqs[1];
+#pragma unroll
+  for (int u = 0; u < KPT; ++u) pre[u] = cm_preload(v, cn, gi[u]);
+  for (int r = 0; r < R; ++r) {
+    fs_placement o;
+    o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
+    o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
+    const ReqCtx c = cn;
+    // ---- score request r at F_curr from the entries requested one request ago --------------------
+    float ce[KPT], cttft[KPT], ctbt[KPT]; bool cok[KPT];
+    unsigned long long key = FS_KEY_NONE;
+#pragma unroll
+    for (int u = 0; u < KPT; ++u) {
+      cok[u] = false; ce[u] = FS_INF; cttft[u] = FS_INF; ctbt[u] = FS_INF;
+      if (!c.valid) continue;
+      const PairCtx p = make_pair(v, c, gi[u]);
+      if (!p.ok) continue;
+      if (pre[u].phi != gi[u].f_cur) pre[u] = cm_preload(v, c, gi[u]);   // the last commit moved this GPU's clock
+      const OwnEval ev = own_eval_vals(c, p.rounds1, p.wait, pre[u].l0, pre[u].p0, pre[u].l1, pre[u].p1);
+      cok[u] = ev.ok; ce[u] = ev.e; cttft[u] = ev.ttft; ctbt[u] = ev.tbt;
+      if (ev.ok) { const unsigned long long kk = fs_orderable(ev.e); key = kk < key ? kk : key; }
+    }
+    // ---- request r+1: its context, and its table entries on the way -------------------------------
+    if (r + 1 < R) {
+      cn = make_req(v, rq_nx);
+      if (r + 2 < R) rq_nx = reqs[r + 2];
+#pragma unroll
+      for (int u = 0; u < KPT; ++u) pre[u] = cm_preload(v, cn, gi[u]);
+    }
+    if (!c.valid) { if (tid == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } continue; }
+    key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+    int kbest = -1, phase = -1;
+    if (key != FS_KEY_NONE) {
+      const float band = __fmul_rn(1.02f, fs_unorderable((uint32_t)key));
+      key = FS_KEY_NONE;                                 // (most memory, largest SM_free, lowest k)
+#pragma unroll
+      for (int u = 0; u < KPT; ++u)
+        if (cok[u] && ce[u] <= band) {
+          const unsigned long long kk = ((unsigned long long)(~fs_orderable(gi[u].mem_free_mb)) << 32) |
+                                        ((unsigned long long)(uint32_t)(d.S - gi[u].sm_free) << 24) | (uint32_t)(tid + u * nthr);
+          key = kk < key ? kk : key;
+        }
+      key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+      kbest = (int)((uint32_t)key & 0xFFFFFFu); phase = 1;
+    } else {
+      // ---- Phase 3: F_max retry, first feasible GPU in T_avail order ----------------------------
+#pragma unroll
+      for (int u = 0; u < KPT; ++u) {
+        cok[u] = false;
+        const PairCtx p = make_pair(v, c, gi[u]);
+        if (!p.ok) continue;
+        const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, p.smf - 1, d.F - 1);
+        cok[u] = ev.ok; ce[u] = ev.e; cttft[u] = ev.ttft; ctbt[u] = ev.tbt;
+        if (ev.ok) {
+          const unsigned long long kk = ((unsigned long long)fs_orderable(gi[u].t_avail_ms) << 32) | (uint32_t)(tid + u * nthr);
+          key = kk < key ? kk : key;
+        }
+      }
+      key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+      if (key != FS_KEY_NONE) { kbest = (int)(uint32_t)key; phase = 2; }
+    }
+    if (kbest >= 0) {
+#pragma unroll
+      for (int u = 0; u < KPT; ++u)
+        if (kbest == tid + u * nthr) {                   // the owner writes the decision and commits it
+          const PairCtx p = make_pair(v, c, gi[u]);
+          const int phibest = phase == 1 ? gi[u].f_cur : d.F - 1;
+          o.gpu = kbest; o.sigma = (int16_t)(p.smf - 1); o.phi = (int16_t)phibest; o.beta = (int16_t)p.br1;
+          o.f_req = (int16_t)phase; o.energy_mj = ce[u]; o.ttft_ms = cttft[u]; o.tbt_ms = ctbt[u];
+          o.flat = (uint32_t)((kbest * d.S + p.smf - 1) * d.F + phibest);
+          out[r] = o;
+          const float tdec = c.O > 0 ? __fmul_rn(__uint2float_rn(p.rounds1), ctbt[u]) : 0.f;
+          gi[u].t_avail_ms = __fadd_rn(cttft[u], tdec);
+          gi[u].mem_free_mb = __fsub_rn(gi[u].mem_free_mb, c.mem);
+          gi[u].f_cur = phibest;
+        }
+    } else if (warp == 0) {
+      // ---- scale-out: energy-optimal feasible frequency of a fresh GPU; no record changes -------
+      key = FS_KEY_NONE;
+      for (int phi = lane; phi < d.F; phi += 32) {
+        const OwnEval ev = own_eval_planes(v, c, 0, c.O, c.load_ms, d.S - 1, phi);
+        if (ev.ok) { const unsigned long long kk = fs_make_key(ev.e, (uint32_t)phi); key = kk < key ? kk : key; }
+      }
+      key = fs_warp_min_key(key);
+      if (key != FS_KEY_NONE) {
+        const int phi = (int)(uint32_t)key;
+        const OwnEval ev = own_eval_planes(v, c, 0, c.O, c.load_ms, d.S - 1, phi);
+        o.sigma = (int16_t)(d.S - 1); o.phi = (int16_t)phi; o.beta = 0; o.f_req = 3;
+        o.energy_mj = ev.e; o.ttft_ms = ev.ttft; o.tbt_ms = ev.tbt;
+      }
+      if (lane == 0) out[r] = o;
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < KPT; ++u) {
+    const int k = tid + u * nthr;
+    if (k < v.K) {
+      fs_gpu_avail w; w.t_avail_ms = gi[u].t_avail_ms; w.mem_free_mb = gi[u].mem_free_mb; w.f_cur = gi[u].f_cur; w._pad = 0;
+      work[k] = w;
+    }
+  }
+}
+
 }  // namespace
 
 int fsk_place_smem_attr() {
@@ -1125,7 +1271,11 @@ int fsk_dispatch_commit(const FsView& v, int R, const fs_request* reqs, fs_place
   int threads = ((v.K + 31) / 32) * 32;
   threads = threads < 32 ? 32 : (threads > CM_THREADS ? CM_THREADS : threads);
   fs_tm_beg(tm, FS_T_DISPATCH, st);
-  dispatch_commit_kernel<<<1, threads, 0, st>>>(v, R, reqs, out, work);
+  const int tr = threads > CMR_THREADS ? CMR_THREADS : threads;
+  if (v.K <= CMR_THREADS) dispatch_commit_reg_kernel<1><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  else if (v.K <= 2 * CMR_THREADS) dispatch_commit_reg_kernel<2><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  else if (v.K <= 4 * CMR_THREADS) dispatch_commit_reg_kernel<4><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  else dispatch_commit_kernel<<<1, threads, 0, st>>>(v, R, reqs, out, work);
   fs_tm_end(tm, FS_T_DISPATCH, st);
   return 1;
 }
