@@ -52,7 +52,19 @@ typedef enum {
   FS_ERR_NOMEM = -6  /* device or host allocation failed                        */
 } fs_status;
 
-enum { FS_HOST = 0, FS_DEVICE = 1 };
+enum {
+  FS_HOST = 0,        /* host memory; the call returns when the outputs are in the caller's buffer          */
+  FS_DEVICE = 1,      /* device memory; the call returns after enqueueing its work on `cuda_stream`          */
+  FS_HOST_PINNED = 2  /* page-locked host memory, asynchronous: copies and kernels are enqueued on
+                         `cuda_stream` and the call returns without waiting.  Inputs must stay untouched and
+                         outputs are valid only after the caller synchronises the stream; range flags
+                         surface on the next call (as with FS_DEVICE).  fs_place_batch reads the requests and
+                         writes the records in place over PCIe when the buffers are mapped into the device's
+                         address space (cudaHostAlloc / cudaHostRegister; otherwise, or with FS_ZERO_COPY=0
+                         in the environment, by bulk copies).  Accepted by the calls of the serving
+                         loop: fs_set_gpu_state, fs_place_batch, fs_local_config, fs_consolidate, fs_dispatch;
+                         the others return FS_ERR_ARG.                                                       */
+};
 
 /* flags of fs_local_config: one objective bit and one split-mode bit (R:s8, R:s9) */
 enum {

@@ -18,7 +18,7 @@ from . import synth
 from .build import LIB as _LIB_PATH, build as build_library
 
 FS_OK, FS_ERR_ARG, FS_ERR_SHAPE, FS_ERR_STATE, FS_ERR_RANGE, FS_ERR_CUDA, FS_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
-FS_HOST, FS_DEVICE = 0, 1
+FS_HOST, FS_DEVICE, FS_HOST_PINNED = 0, 1, 2
 FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
@@ -118,6 +118,16 @@ def _buf(x, nbytes: int | None = None):
     return C.c_void_p(a.ctypes.data), FS_HOST, a
 
 
+def _pin(sp, pinned: bool, *bufs):
+    """FS_HOST -> FS_HOST_PINNED when the caller asks for the asynchronous page-locked host path."""
+    if not pinned:
+        return sp
+    assert sp == FS_HOST, "pinned=True is for host buffers"
+    for b in bufs:
+        assert b is None or (hasattr(b, "is_pinned") and b.is_pinned()), "pinned=True needs page-locked torch tensors"
+    return FS_HOST_PINNED
+
+
 def _stream_ptr(stream) -> C.c_void_p:
     if stream is None:
         return C.c_void_p(0)
@@ -172,16 +182,18 @@ class Festina:
         self.dims = (M, F, S, B)
         self.K = 0
 
-    def set_gpu_state(self, states, K: int | None = None, stream=None):
+    def set_gpu_state(self, states, K: int | None = None, stream=None, pinned: bool = False):
         if K is None:
             K = len(states) if not hasattr(states, "data_ptr") else states.numel() * states.element_size() // 128
         ps, sp, keep = _buf(states, K * 128)
-        rc = lib().fs_set_gpu_state(self._h, K, ps, sp if sp is not None else FS_HOST, _stream_ptr(stream))
+        sp = _pin(sp if sp is not None else FS_HOST, pinned, states)
+        rc = lib().fs_set_gpu_state(self._h, K, ps, sp, _stream_ptr(stream))
         self._check(rc, "fs_set_gpu_state")
         self.K = K
 
-    def place_batch(self, reqs, out=None, R: int | None = None, stream=None):
-        """Returns a numpy record array (host inputs) or writes into `out` (device tensors)."""
+    def place_batch(self, reqs, out=None, R: int | None = None, stream=None, pinned: bool = False):
+        """Returns a numpy record array (host inputs) or writes into `out` (device tensors).  pinned=True:
+        page-locked host tensors, asynchronous (FS_HOST_PINNED): synchronise `stream` before reading `out`."""
         if R is None:
             R = len(reqs) if not hasattr(reqs, "data_ptr") else reqs.numel() * reqs.element_size() // 32
         pr, sp, keep = _buf(reqs, R * 32)
@@ -192,6 +204,7 @@ class Festina:
             out = np.zeros(R, dtype=synth.PLACEMENT_DT)
         po, spo, keep2 = _buf(out, R * 32)
         assert spo == sp or R == 0
+        sp = _pin(sp, pinned, reqs, out)
         rc = lib().fs_place_batch(self._h, R, pr, po, sp, _stream_ptr(stream))
         self._check(rc, "fs_place_batch")
         return out
@@ -229,7 +242,7 @@ class Festina:
         self._check(lib().fs_dispatch_commit(self._h, R, pr, po, pa, sp, _stream_ptr(stream)), "fs_dispatch_commit")
         return out, after
 
-    def local_config(self, flags: int = 0, gpu_ids=None, n: int | None = None, out=None, stream=None):
+    def local_config(self, flags: int = 0, gpu_ids=None, n: int | None = None, out=None, stream=None, pinned: bool = False):
         if gpu_ids is not None and not hasattr(gpu_ids, "data_ptr"):
             gpu_ids = np.ascontiguousarray(gpu_ids, dtype=np.int32)
         if n is None:
@@ -240,6 +253,7 @@ class Festina:
             out = np.zeros(n, dtype=synth.LOCAL_CFG_DT)
         po, spo, keep2 = _buf(out, n * 48)
         assert spi is None or spi == spo
+        spo = _pin(spo, pinned, gpu_ids, out)
         rc = lib().fs_local_config(self._h, n, pi, flags, po, spo, _stream_ptr(stream))
         self._check(rc, "fs_local_config")
         return out

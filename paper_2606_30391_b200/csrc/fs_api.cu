@@ -37,6 +37,7 @@ struct fs_ctx {
   // task batching scratch (FS_HOST staging)
   int bt_n_cap = 0, bt_t_cap = 0; int32_t *bt_ids = nullptr, *bt_off = nullptr; fs_task* bt_tasks = nullptr; fs_task_out* bt_out = nullptr;
   // Algorithm 1 / EWR scratch (FS_HOST staging)
+  bool zero_copy = true;   // FS_ZERO_COPY=0 in the environment: bulk copies for FS_HOST_PINNED too
   size_t a1_cap = 0; unsigned char* a1_buf = nullptr; size_t pl_cap = 0; unsigned char* pl_buf = nullptr;
   // consolidation scratch
   size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
@@ -127,7 +128,9 @@ int place_prepare(fs_ctx* c, cudaStream_t st) {
   return FS_OK;
 }
 
-cudaMemcpyKind in_kind(int space) { return space == FS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice; }
+cudaMemcpyKind in_kind(int space) { return space != FS_DEVICE ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice; }
+// the calls of the serving loop also take page-locked host buffers without waiting for the stream
+bool space_ok(int space) { return space == FS_HOST || space == FS_DEVICE || space == FS_HOST_PINNED; }
 
 }  // namespace
 
@@ -158,6 +161,7 @@ int fs_create(fs_ctx** out, int cuda_device) {
   fsk_place_smem_attr();
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
   if (const char* e = getenv("FS_FORCE_GENERIC")) c->force_generic = e[0] == '1';
+  if (const char* e = getenv("FS_ZERO_COPY")) c->zero_copy = e[0] != '0';
   *out = c;
   return FS_OK;
 }
@@ -227,7 +231,7 @@ int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const flo
 
 int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space, void* cuda_stream) {
   if (!c || K < 0 || (K > 0 && !states)) return FS_ERR_ARG;
-  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof) return FS_ERR_STATE;
   if ((unsigned long long)K * c->d.S * c->d.F >= 0xFFFFFFFFull) return FS_ERR_SHAPE;  // flat is 32-bit
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -265,7 +269,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
 int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out, int space,
                    void* cuda_stream) {
   if (!c || R < 0 || (R > 0 && (!reqs || !out))) return FS_ERR_ARG;
-  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   FS_CUDA(c, cudaSetDevice(c->dev));
@@ -277,7 +281,22 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     c->r_cap = R;
   }
   const fs_request* d_reqs = reqs; fs_placement* d_out = out;
-  if (space == FS_HOST) {
+  // page-locked buffers are mapped into the device's address space: the scoring kernel reads each request
+  // and writes each record over PCIe itself (at pod 65,536 x 32 B each way hide behind the scoring; a bulk copy
+  // before and after the kernel would sit on the step's critical path)
+  bool zero_copy = false;
+  if (space == FS_HOST_PINNED && c->zero_copy) {
+    cudaPointerAttributes a_in{}, a_out{};
+    if (cudaPointerGetAttributes(&a_in, reqs) == cudaSuccess && cudaPointerGetAttributes(&a_out, out) == cudaSuccess &&
+        a_in.type == cudaMemoryTypeHost && a_out.type == cudaMemoryTypeHost && a_in.devicePointer && a_out.devicePointer) {
+      d_reqs = static_cast<const fs_request*>(a_in.devicePointer);
+      d_out = static_cast<fs_placement*>(a_out.devicePointer);
+      zero_copy = true;
+    } else {
+      (void)cudaGetLastError();
+    }
+  }
+  if (space != FS_DEVICE && !zero_copy) {
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
@@ -285,8 +304,10 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
   FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic, c->count_work};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
-  if (space == FS_HOST) {
+  if (zero_copy) return pending;
+  if (space != FS_DEVICE) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
+    if (space == FS_HOST_PINNED) return pending;   // the caller synchronises; flags surface on the next call
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;
@@ -297,7 +318,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
 int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags, fs_local_cfg* out,
                     int space, void* cuda_stream) {
   if (!c || n < 0 || (n > 0 && !out) || (flags & ~3u)) return FS_ERR_ARG;
-  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (!gpu_ids && n > c->K) return FS_ERR_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -318,7 +339,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
     c->bin_m_cap = c->d.M;
   }
   const int32_t* d_ids = gpu_ids; fs_local_cfg* d_out = out;
-  if (space == FS_HOST) {
+  if (space != FS_DEVICE) {
     if (gpu_ids) {
       FS_CUDA(c, cudaMemcpyAsync(c->ids_dev, gpu_ids, (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
       d_ids = c->ids_dev;
@@ -328,8 +349,9 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
   FsLocalScratch sc{c->G, c->comp, c->comp_n, c->ns_stride, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots};
   c->launches += fsk_local(view_of(c), n, d_ids, flags, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
-  if (space == FS_HOST) {
+  if (space != FS_DEVICE) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->local_dev, (size_t)n * sizeof(fs_local_cfg), cudaMemcpyDeviceToHost, st));
+    if (space == FS_HOST_PINNED) return pending;   // the caller synchronises; flags surface on the next call
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;
@@ -338,7 +360,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
 }
 
 int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) {
-  if (!c || (space != FS_HOST && space != FS_DEVICE)) return FS_ERR_ARG;
+  if (!c || !space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (c->K > 0 && !out) return FS_ERR_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -351,12 +373,13 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
     FS_TRY(grow(c, c->ckeys, (size_t)c->K)); FS_TRY(grow(c, c->consol_dev, (size_t)c->K));
     c->consol_cap = kf;
   }
-  fs_consol_out* d_out = space == FS_HOST ? c->consol_dev : out;
+  fs_consol_out* d_out = space != FS_DEVICE ? c->consol_dev : out;
   FsConsolScratch sc{c->need, c->E, c->agg, c->ckeys};
   c->launches += fsk_consolidate(view_of(c), c->prm, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
-  if (space == FS_HOST) {
+  if (space != FS_DEVICE) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->consol_dev, (size_t)c->K * sizeof(fs_consol_out), cudaMemcpyDeviceToHost, st));
+    if (space == FS_HOST_PINNED) return pending;   // the caller synchronises; flags surface on the next call
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;
@@ -367,7 +390,7 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
 int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out, int space,
                 void* cuda_stream) {
   if (!c || R < 0 || (R > 0 && (!reqs || !out))) return FS_ERR_ARG;
-  if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
+  if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (c->K >= (1 << 24)) return FS_ERR_SHAPE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -380,15 +403,16 @@ int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out,
     c->r_cap = R;
   }
   const fs_request* d_reqs = reqs; fs_placement* d_out = out;
-  if (space == FS_HOST) {
+  if (space != FS_DEVICE) {
     FS_CUDA(c, cudaMemcpyAsync(c->reqs_dev, reqs, (size_t)R * sizeof(fs_request), cudaMemcpyHostToDevice, st));
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
   FS_TRY(place_prepare(c, st));
   c->launches += fsk_dispatch(view_of(c), R, d_reqs, d_out, c->warm_off, c->warm_item, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
-  if (space == FS_HOST) {
+  if (space != FS_DEVICE) {
     FS_CUDA(c, cudaMemcpyAsync(out, c->place_dev, (size_t)R * sizeof(fs_placement), cudaMemcpyDeviceToHost, st));
+    if (space == FS_HOST_PINNED) return pending;   // the caller synchronises; flags surface on the next call
     FS_CUDA(c, cudaStreamSynchronize(st));
     const int now = take_flags(c);
     return pending != FS_OK ? pending : now;

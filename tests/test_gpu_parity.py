@@ -398,6 +398,30 @@ def test_dispatch_full_size(ctx):
     assert set(np.unique(got["f_req"]).tolist()) >= {1, 2, 3}
 
 
+def test_host_pinned_async_equals_host(ctx):
+    import paper_2606_30391_b200 as fs
+    """FS_HOST_PINNED: page-locked host buffers, the call does not wait; same bytes as the blocking FS_HOST calls."""
+    import torch
+    cl = synth.make_cluster("rack")
+    ctx.load_cluster(cl)
+    ref_p = ctx.place_batch(cl.requests); ref_l = ctx.local_config(0); ref_d = ctx.dispatch(cl.requests)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1).copy()).pin_memory()
+    h_st, h_rq = pin(cl.states), pin(cl.requests)
+    h_p = torch.zeros(cl.R * 32, dtype=torch.uint8).pin_memory(); h_l = torch.zeros(cl.K * 48, dtype=torch.uint8).pin_memory()
+    h_d = torch.zeros(cl.R * 32, dtype=torch.uint8).pin_memory()
+    s = torch.cuda.Stream()
+    ctx.set_gpu_state(h_st, stream=s, pinned=True)
+    ctx.place_batch(h_rq, out=h_p, stream=s, pinned=True)
+    ctx.local_config(0, n=cl.K, out=h_l, stream=s, pinned=True)
+    rc = fs.lib().fs_dispatch(ctx._h, cl.R, h_rq.data_ptr(), h_d.data_ptr(), fs.FS_HOST_PINNED, s.cuda_stream)
+    assert rc == 0
+    s.synchronize()
+    assert h_p.numpy().tobytes() == ref_p.tobytes() and h_l.numpy().tobytes() == ref_l.tobytes()
+    assert h_d.numpy().tobytes() == ref_d.tobytes()
+    # calls outside the serving loop reject the asynchronous space
+    assert fs.lib().fs_ewr(ctx._h, 0, None, None, None, 0, None, None, fs.FS_HOST_PINNED, None) == -1
+
+
 # ---- the sequential commit pass (fs_dispatch_commit, reading s34) -------------------------------------
 def _assert_commit_equal(ctx, cl, reqs=None):
     reqs = cl.requests if reqs is None else reqs
