@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
 
 
 // =============================================================================================
-// Dense scorer, S <= 16, F <= 64: one warp = one request, one persistent block per SM.
+// Dense scorer, S <= 32 (FS_MAX_S), F <= 64: one warp = one request, one persistent block per SM.
 //
 // Factorisation (exact).  For a COLD pair (the request's model is
 // not resident on the GPU) the decode bucket is 0 and the co-resident variant is 0, so everything
@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
 // =============================================================================================
 constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102)
 constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
-constexpr int DENSE_S = 16;
+constexpr int DENSE_S = FS_MAX_S;
 
 // does any of the four 16-bit models packed in (w0, w1) equal m?  (exact "has a zero halfword" test on the
 // XOR; the SIMD-in-a-word video instructions are emulated on this architecture and cost ~30 instructions)

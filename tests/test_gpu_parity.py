@@ -672,13 +672,31 @@ def test_negative_and_huge_waits(ctx):
     cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
 
 
+@pytest.mark.parametrize("S", [17, 24, 32])
+def test_dense_scoring_up_to_32_shares(ctx, S):
+    """The tiled scoring kernel covers every supported S (tiles of S rows per warp; fewer warps per block)."""
+    for mode, (K, F) in enumerate([(300, 64), (2500, 33), (64, 17)]):
+        cl = synth.make_custom(seed=1700 + S + mode, K=K, M=7, F=F, S=S, B=24, R=900, lo=1, hi=4)
+        if mode == 1:
+            cl.requests["slo_ttft_ms"] *= 3.0; cl.models["load_ms"] *= 0.1
+        if mode == 2:
+            cl = U.tie_heavy(cl, S)
+        ctx.load_cluster(cl)
+        ctx.set_work_stats(True)
+        got = ctx.place_batch(cl.requests)
+        stats = ctx.last_place_stats()
+        ctx.set_work_stats(False)
+        assert stats["chunks_tested"] > 0               # counted only by the tiled kernel's scan
+        cmp.assert_placement_equal(got, oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests, nthreads=16))
+
+
 # ---- randomised sweep: dims, load shapes and SLO regimes, every entry point of the hot path ----------
 @pytest.mark.parametrize("block", range(4))
 def test_random_clusters_all_entry_points(ctx, block):
     for seed in range(block * 30, block * 30 + 30):
         st = synth.Stream(seed, "fuzz")
         K = int(st.randint(1, 1, 400)[0]); M = int(st.randint(1, 1, 12)[0]); F = int(st.randint(1, 1, 64)[0])
-        S = int(st.randint(1, 1, 16)[0]); B = int(st.randint(1, 1, 48)[0]); R = int(st.randint(1, 1, 700)[0])
+        S = int(st.randint(1, 1, 32)[0]); B = int(st.randint(1, 1, 48)[0]); R = int(st.randint(1, 1, 700)[0])
         cl = synth.make_custom(seed=5000 + seed, K=K, M=M, F=F, S=S, B=B, R=R, lo=1, hi=4)
         mode = seed % 5
         if mode == 1:
