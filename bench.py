@@ -153,7 +153,7 @@ def run_reference(args):
 def _config(cl, args):
     return {"workload": f"{cl.name} (BASELINE.json configs[2]): K={cl.K} GPUs, M={cl.M}, F={cl.F}, S={cl.S}, "
                         f"B={cl.B}, R={cl.R} requests per rank; step = fs_set_gpu_state + fs_place_batch + "
-                        f"fs_local_config(all GPUs, energy objective, exhaustive splits)" + ("; the two calls on two streams" if args.overlap else "") + ("; one CUDA graph per step" if args.graph else ""),
+                        f"fs_local_config(all GPUs, energy objective, exhaustive splits" + (", then the minimum-SM split rule" if args.split_modes == "both" else "") + ")" + ("; the two calls on two streams" if args.overlap else "") + ("; one CUDA graph per step" if args.graph else ""),
             "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B, "R_per_rank": cl.R,
             "l2": "flushed between timed steps by overwriting a 256 MiB buffer",
             "parallelism": f"replicated tables+state, requests sharded x{args.gpus}"}
@@ -183,6 +183,8 @@ def run_ours(args):
     d_states, d_reqs = tb(cl.states), tb(cl.requests)
     d_place = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
     d_local = torch.empty(cl.K * 48, dtype=torch.uint8, device=dev)
+    both_splits = args.split_modes == "both"
+    d_local2 = torch.empty(cl.K * 48, dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
     ctx.set_timing(True)
@@ -198,10 +200,14 @@ def run_ours(args):
         if side is None or serial:
             ctx.place_batch(d_reqs, out=d_place, stream=st)
             ctx.local_config(0, n=cl.K, out=d_local, stream=st)
+            if both_splits:
+                ctx.local_config(2, n=cl.K, out=d_local2, stream=st)
             return
         ev_state.record(st)
         side.wait_event(ev_state)
         ctx.local_config(0, n=cl.K, out=d_local, stream=side)
+        if both_splits:
+            ctx.local_config(2, n=cl.K, out=d_local2, stream=side)
         ctx.place_batch(d_reqs, out=d_place, stream=st)
         ev_side.record(side)
         st.wait_event(ev_side)
@@ -303,6 +309,7 @@ def run_ours(args):
     h_reqs = torch.from_numpy(cl.requests.view(np.uint8).reshape(-1).copy()).pin_memory()
     h_place = torch.empty(cl.R * 32, dtype=torch.uint8).pin_memory()
     h_local = torch.empty(cl.K * 48, dtype=torch.uint8).pin_memory()
+    h_local2 = torch.empty(cl.K * 48, dtype=torch.uint8).pin_memory()
 
     # The same step as above with FS_HOST_PINNED buffers: every step copies its inputs (state records, requests)
     # from page-locked host memory and its results (placements, local configurations) back; the host waits for
@@ -313,10 +320,14 @@ def run_ours(args):
         if side is None:
             ctx.place_batch(h_reqs, out=h_place, stream=st, pinned=True)
             ctx.local_config(0, n=cl.K, out=h_local, stream=st, pinned=True)
+            if both_splits:
+                ctx.local_config(2, n=cl.K, out=h_local2, stream=st, pinned=True)
             return
         ev_state.record(st)
         side.wait_event(ev_state)
         ctx.local_config(0, n=cl.K, out=h_local, stream=side, pinned=True)
+        if both_splits:
+            ctx.local_config(2, n=cl.K, out=h_local2, stream=side, pinned=True)
         ctx.place_batch(h_reqs, out=h_place, stream=st, pinned=True)
         ev_side.record(side)
         st.wait_event(ev_side)
@@ -392,7 +403,7 @@ def run_ours(args):
                             "timed steps are serial: kernel_ms comes from them")},
         "wall_ms_per_step_incl_flush": wall_ms / steps,
         "e2e": {"value": ws * grid_cands * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
-                "h2d_bytes_per_step": cl.K * 128 + cl.R * 32, "d2h_bytes_per_step": cl.R * 32 + cl.K * 48,
+                "h2d_bytes_per_step": cl.K * 128 + cl.R * 32, "d2h_bytes_per_step": cl.R * 32 + cl.K * 48 * (2 if both_splits else 1),
                 "mode": "FS_HOST_PINNED buffers (page-locked host memory): state records and local configurations by "
                         "copy engine, requests read and placement records written over PCIe by the scoring kernel itself"
                         + (", two streams" if side is not None else "") + (", one CUDA graph per step" if hgraph is not None else "")
@@ -566,6 +577,8 @@ def main():
     ap.add_argument("--cpu-gpus", type=int, default=4096, help="oracle sample (GPUs) of --workload local")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--graph", type=int, default=1, help="1: replay the device step from a CUDA graph")
+    ap.add_argument("--split-modes", default="exhaustive", choices=["exhaustive", "both"],
+                    help="pod: fs_local_config once (all splits) or twice (all splits, then the per-task minimum-SM rule)")
     ap.add_argument("--overlap", type=int, default=1, help="1: fs_local_config on a second stream beside fs_place_batch")
     args = ap.parse_args()
     if args.impl == "reference":

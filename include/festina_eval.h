@@ -257,7 +257,8 @@ int fs_dispatch(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* ou
  * Scale-out decisions (gpu = -1) change nothing; the resident models stay those of fs_set_gpu_state.
  * The context's own GPU state is NOT modified: `after` ([K], may be NULL) receives the three fields of
  * every GPU after the last commit; the caller feeds the next poll through fs_set_gpu_state.
- * One thread block walks the requests (they are serial by definition); the GPUs are the parallel axis.
+ * One thread block (a cluster of up to 8 for 2,049..16,384 GPUs) walks the requests (they are serial by
+ * definition); the GPUs are the parallel axis.
  *   reqs : [R]; out : [R]; after : [K] or NULL; all in `space`.  Requires K < 2^24.              */
 int fs_dispatch_commit(fs_ctx* ctx, int32_t R, const fs_request* reqs, fs_placement* out,
                        fs_gpu_avail* after, int space, void* cuda_stream);

@@ -1030,6 +1030,35 @@ __global__ void __launch_bounds__(CM_THREADS) dispatch_commit_kernel(FsView v, i
 // requested right after request r has been scored and arrive while r's two reductions and its commit
 // run; a GPU whose F_curr the commit changed reloads its four entries.  What remains on the serial chain
 // of a request is arithmetic and two block-wide minima.
+// ---- thread-block cluster helpers (sm_90+ PTX): rank, size, a peer block's shared memory, barrier ----
+__device__ __forceinline__ uint32_t cl_rank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cl_size() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cl_store_u64(const void* local_smem, uint32_t peer, unsigned long long x) {
+  uint32_t remote;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(fs_smem_u32(local_smem)), "r"(peer));
+  asm volatile("st.shared::cluster.u64 [%0], %1;" ::"r"(remote), "l"(x) : "memory");
+}
+__device__ __forceinline__ void cl_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+constexpr int CM_MAXC = 8;                        // portable cluster size
+
+// minimum over the block and, with CLUSTER, over the blocks of the cluster: every block's leader warp
+// stores the block's minimum into slot [par][own rank] of every block (distributed shared memory), one
+// cluster barrier, every thread reads the slots of its own block
+template <bool CLUSTER>
+__device__ __forceinline__ unsigned long long cm_min_all(unsigned long long x, unsigned long long (*buf)[CM_THREADS / 32],
+                                                         unsigned long long (*cbuf)[CM_MAXC], int& par, int nwarp,
+                                                         int warp, int lane, uint32_t crank, uint32_t csize) {
+  if (!CLUSTER) return cm_block_min(x, buf, par, nwarp, warp, lane);
+  const int p = par;
+  x = cm_block_min(x, buf, par, nwarp, warp, lane);
+  if (warp == 0 && lane < (int)csize) cl_store_u64(&cbuf[p][crank], (uint32_t)lane, x);
+  cl_sync();
+  unsigned long long y = lane < (int)csize ? cbuf[p][lane] : FS_KEY_NONE;
+  return fs_warp_min_key(y);
+}
+
 struct CmPre { float l0, p0, l1, p1; int phi; };
 
 __device__ __forceinline__ CmPre cm_preload(const FsView& v, const ReqCtx& c, const FsGpuInfo& gi) {
@@ -1044,14 +1073,18 @@ __device__ __forceinline__ CmPre cm_preload(const FsView& v, const ReqCtx& c, co
 }
 
 constexpr int CMR_THREADS = 512;                  // 128 registers per thread: the records of up to 4 GPUs
-template <int KPT>
+template <int KPT, bool CLUSTER>
 __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView v, int R,
                                                                          const fs_request* __restrict__ reqs,
                                                                          fs_placement* __restrict__ out,
                                                                          fs_gpu_avail* __restrict__ work) {
   __shared__ unsigned long long s_buf[2][CM_THREADS / 32];
+  __shared__ unsigned long long s_cbuf[2][CM_MAXC];
   const FsDimsDev d = v.d;
-  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+  const uint32_t crank = CLUSTER ? cl_rank() : 0u, csize = CLUSTER ? cl_size() : 1u;
+  // thread `tid` of `nthr` across the cluster owns GPUs tid, tid + nthr, ...
+  const int tid = (int)crank * (int)blockDim.x + (int)threadIdx.x, nthr = (int)csize * (int)blockDim.x;
   int par = 0;
   FsGpuInfo gi[KPT]; CmPre pre[KPT];
 #pragma unroll
@@ -1094,7 +1127,7 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
       for (int u = 0; u < KPT; ++u) pre[u] = cm_preload(v, cn, gi[u]);
     }
     if (!c.valid) { if (tid == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } continue; }
-    key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+    key = cm_min_all<CLUSTER>(key, s_buf, s_cbuf, par, nwarp, warp, lane, crank, csize);
     int kbest = -1, phase = -1;
     if (key != FS_KEY_NONE) {
       const float band = __fmul_rn(1.02f, fs_unorderable((uint32_t)key));
@@ -1106,7 +1139,7 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
                                         ((unsigned long long)(uint32_t)(d.S - gi[u].sm_free) << 24) | (uint32_t)(tid + u * nthr);
           key = kk < key ? kk : key;
         }
-      key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+      key = cm_min_all<CLUSTER>(key, s_buf, s_cbuf, par, nwarp, warp, lane, crank, csize);
       kbest = (int)((uint32_t)key & 0xFFFFFFu); phase = 1;
     } else {
       // ---- Phase 3: F_max retry, first feasible GPU in T_avail order ----------------------------
@@ -1122,7 +1155,7 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
           key = kk < key ? kk : key;
         }
       }
-      key = cm_block_min(key, s_buf, par, nwarp, warp, lane);
+      key = cm_min_all<CLUSTER>(key, s_buf, s_cbuf, par, nwarp, warp, lane, crank, csize);
       if (key != FS_KEY_NONE) { kbest = (int)(uint32_t)key; phase = 2; }
     }
     if (kbest >= 0) {
@@ -1140,7 +1173,7 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
           gi[u].mem_free_mb = __fsub_rn(gi[u].mem_free_mb, c.mem);
           gi[u].f_cur = phibest;
         }
-    } else if (warp == 0) {
+    } else if (warp == 0 && crank == 0) {
       // ---- scale-out: energy-optimal feasible frequency of a fresh GPU; no record changes -------
       key = FS_KEY_NONE;
       for (int phi = lane; phi < d.F; phi += 32) {
@@ -1157,6 +1190,7 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
       if (lane == 0) out[r] = o;
     }
   }
+  if (CLUSTER) cl_sync();                              // no block leaves while a peer may still store into it
 #pragma unroll
   for (int u = 0; u < KPT; ++u) {
     const int k = tid + u * nthr;
@@ -1272,9 +1306,21 @@ int fsk_dispatch_commit(const FsView& v, int R, const fs_request* reqs, fs_place
   threads = threads < 32 ? 32 : (threads > CM_THREADS ? CM_THREADS : threads);
   fs_tm_beg(tm, FS_T_DISPATCH, st);
   const int tr = threads > CMR_THREADS ? CMR_THREADS : threads;
-  if (v.K <= CMR_THREADS) dispatch_commit_reg_kernel<1><<<1, tr, 0, st>>>(v, R, reqs, out, work);
-  else if (v.K <= 2 * CMR_THREADS) dispatch_commit_reg_kernel<2><<<1, tr, 0, st>>>(v, R, reqs, out, work);
-  else if (v.K <= 4 * CMR_THREADS) dispatch_commit_reg_kernel<4><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  if (v.K <= CMR_THREADS) dispatch_commit_reg_kernel<1, false><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  else if (v.K <= 2 * CMR_THREADS) dispatch_commit_reg_kernel<2, false><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  else if (v.K <= 4 * CMR_THREADS) dispatch_commit_reg_kernel<4, false><<<1, tr, 0, st>>>(v, R, reqs, out, work);
+  else if (v.K <= CM_MAXC * 4 * CMR_THREADS) {
+    // a thread-block cluster: up to 8 blocks x 512 threads x 4 GPUs in registers, minima through
+    // distributed shared memory
+    const int csize = (v.K + 4 * CMR_THREADS - 1) / (4 * CMR_THREADS);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)csize); cfg.blockDim = dim3(CMR_THREADS); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, dispatch_commit_reg_kernel<4, true>, v, R, reqs, out, work);
+  }
   else dispatch_commit_kernel<<<1, threads, 0, st>>>(v, R, reqs, out, work);
   fs_tm_end(tm, FS_T_DISPATCH, st);
   return 1;

@@ -454,6 +454,21 @@ def test_dispatch_commit_ragged_dims(ctx, seed):
     assert ctx.dispatch(cl.requests).tobytes() == snap.tobytes()
 
 
+@pytest.mark.parametrize("K", [2049, 5000, 16384, 16385])
+def test_dispatch_commit_many_gpus(ctx, K):
+    """2,049 .. 16,384 GPUs: a thread-block cluster (minima through distributed shared memory); more: the
+    single block with the records in global memory."""
+    cl = synth.make_custom(seed=1600 + K % 97, K=K, M=6, F=20, S=8, B=12, R=300, lo=1, hi=4)
+    u = synth.Stream(K, "cphase").uniform(cl.R)
+    cl.requests["slo_ttft_ms"] = np.where(u < 0.3, cl.requests["slo_ttft_ms"] * 0.02, cl.requests["slo_ttft_ms"]).astype(np.float32)
+    cl.requests["o_pred"] = np.where(u > 0.9, 2 ** 20, cl.requests["o_pred"]).astype(np.uint32)
+    if K == 5000:
+        cl.states["mem_free_mb"] = 30000.0              # every decision goes through the tie-breaker and the commit
+    ctx.load_cluster(cl)
+    got = _assert_commit_equal(ctx, cl)
+    assert set(np.unique(got["f_req"]).tolist()) >= {1, 3}
+
+
 def test_dispatch_commit_by_hand(ctx):
     """tests/test_oracle_commit.py::test_commit_by_hand through the CUDA path."""
     from test_oracle_dispatch import _toy, _gpu
