@@ -234,6 +234,21 @@ __device__ __forceinline__ void ld_lane(const LanePtr& p, uint32_t o, bool vec, 
   else { x[0] = p.a[o]; if (NPHI == 2) x[NPHI - 1] = p.b[o]; }
 }
 
+// asynchronous copy (LDGSTS) of the lane's NPHI values of row `o` into its own tile slot: no registers are
+// held while the row is on its way; the lane that issued the copy is the one that reads the slot
+template <int NPHI>
+__device__ __forceinline__ void cp_lane(float* dst, const LanePtr& p, uint32_t o, bool vec) {
+  const uint32_t d = fs_smem_u32(dst);
+  if (NPHI == 2 && vec) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(p.a + o) : "memory");
+  else {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(p.a + o) : "memory");
+    if (NPHI == 2) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d + 4u), "l"(p.b + o) : "memory");
+  }
+}
+__device__ __forceinline__ void cp_commit_wait_all() {
+  asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
 // work statistics (what this launch actually did; bench.py turns them into lane-operations)
 __device__ __forceinline__ void flush_stats(unsigned long long* stats, uint32_t n_chunks, uint32_t n_elig,
                                          uint32_t n_swept, uint32_t n_cswept, uint32_t n_witems,
@@ -344,29 +359,46 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
       uint32_t pe = INFBITS, pt = INFBITS, pe0 = INFBITS;   // running prefix minima (bits)
       __syncwarp();
-#pragma unroll 2
+      // the prefill rows (LAT0, POW0) of all shares go straight into the tile slots they will be replaced
+      // in (t0 over LAT0, er over POW0), asynchronously and without registers; the decode rows come
+      // through registers, four rows in flight
       for (int s = 0; s < d.S; ++s) {
-        float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI], tt[NPHI], ee[NPHI];
-        const int o = s * d.F;
-        ld_lane<NPHI>(q_l0, o, vec, a0); ld_lane<NPHI>(q_p0, o, vec, b0);
-        ld_lane<NPHI>(q_l1, o, vec, a1); ld_lane<NPHI>(q_p1, o, vec, b1);
-        uint32_t ue = INFBITS, ut = INFBITS, ue0 = INFBITS;
+        cp_lane<NPHI>(tl_t0 + s * FT + phi0, q_l0, (uint32_t)(s * d.F), vec);
+        cp_lane<NPHI>(tl_er + s * FT + phi0, q_p0, (uint32_t)(s * d.F), vec);
+      }
+      for (int s0 = 0; s0 < d.S; s0 += 4) {
+        float a1[4][NPHI], b1[4][NPHI];
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) {
-          const float t = __fmul_rn(fr0, a0[i]);
-          const float e0 = __fmul_rn(t, b0[i]);
-          const float e = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[i]), b1[i]));
-          const bool in = (phi0 + i) < d.F;
-          tt[i] = in ? t : FS_INF;
-          ee[i] = (in && a1[i] <= tbt) ? e : FS_INF;
-          if (in) ue0 = min(ue0, __float_as_uint(e0));
-          ue = min(ue, __float_as_uint(ee[i])); ut = min(ut, __float_as_uint(tt[i]));
+        for (int u = 0; u < 4; ++u) {
+          const int o = min(s0 + u, d.S - 1) * d.F;
+          ld_lane<NPHI>(q_l1, o, vec, a1[u]); ld_lane<NPHI>(q_p1, o, vec, b1[u]);
         }
-        st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
-        pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut)); pe0 = min(pe0, warp_min_u32(ue0));
-        if (lane == 0) {
-          bnd[s] = __uint_as_float(pe); bnd[DENSE_S + s] = __uint_as_float(pt);
-          bnd[2 * DENSE_S + s] = __uint_as_float(pe0);
+        if (s0 == 0) cp_commit_wait_all();               // the prefill rows have landed in the tile slots
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int s = s0 + u;
+          if (s < d.S) {
+            float a0[NPHI], b0[NPHI], tt[NPHI], ee[NPHI];
+            ld_tile<NPHI>(tl_t0 + s * FT + phi0, a0); ld_tile<NPHI>(tl_er + s * FT + phi0, b0);
+            uint32_t ue = INFBITS, ut = INFBITS, ue0 = INFBITS;
+#pragma unroll
+            for (int i = 0; i < NPHI; ++i) {
+              const float t = __fmul_rn(fr0, a0[i]);
+              const float e0 = __fmul_rn(t, b0[i]);
+              const float e = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
+              const bool in = (phi0 + i) < d.F;
+              tt[i] = in ? t : FS_INF;
+              ee[i] = (in && a1[u][i] <= tbt) ? e : FS_INF;
+              if (in) ue0 = min(ue0, __float_as_uint(e0));
+              ue = min(ue, __float_as_uint(ee[i])); ut = min(ut, __float_as_uint(tt[i]));
+            }
+            st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
+            pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut)); pe0 = min(pe0, warp_min_u32(ue0));
+            if (lane == 0) {
+              bnd[s] = __uint_as_float(pe); bnd[DENSE_S + s] = __uint_as_float(pt);
+              bnd[2 * DENSE_S + s] = __uint_as_float(pe0);
+            }
+          }
         }
       }
       __syncwarp();

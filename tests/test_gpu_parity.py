@@ -701,7 +701,8 @@ def test_dense_scoring_up_to_32_shares(ctx, S):
         got = ctx.place_batch(cl.requests)
         stats = ctx.last_place_stats()
         ctx.set_work_stats(False)
-        assert stats["chunks_tested"] > 0               # counted only by the tiled kernel's scan
+        # counted only by the tiled kernel (the cold scan alone can be empty: another slice's result may prune it)
+        assert stats["chunks_tested"] + stats["warm_pairs_tested"] > 0
         cmp.assert_placement_equal(got, oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests, nthreads=16))
 
 
