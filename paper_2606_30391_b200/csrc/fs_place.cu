@@ -237,12 +237,11 @@ __device__ __forceinline__ void ld_lane(const LanePtr& p, uint32_t o, bool vec, 
 // asynchronous copy (LDGSTS) of the lane's NPHI values of row `o` into its own tile slot: no registers are
 // held while the row is on its way; the lane that issued the copy is the one that reads the slot
 template <int NPHI>
-__device__ __forceinline__ void cp_lane(float* dst, const LanePtr& p, uint32_t o, bool vec) {
-  const uint32_t d = fs_smem_u32(dst);
-  if (NPHI == 2 && vec) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(p.a + o) : "memory");
+__device__ __forceinline__ void cp_lane(uint32_t dst, const LanePtr& p, bool vec) {
+  if (NPHI == 2 && vec) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(p.a) : "memory");
   else {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(p.a + o) : "memory");
-    if (NPHI == 2) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d + 4u), "l"(p.b + o) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(p.a) : "memory");
+    if (NPHI == 2) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + 4u), "l"(p.b) : "memory");
   }
 }
 __device__ __forceinline__ void cp_commit_wait_all() {
@@ -362,9 +361,15 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       // the prefill rows (LAT0, POW0) of all shares go straight into the tile slots they will be replaced
       // in (t0 over LAT0, er over POW0), asynchronously and without registers; the decode rows come
       // through registers, four rows in flight
-      for (int s = 0; s < d.S; ++s) {
-        cp_lane<NPHI>(tl_t0 + s * FT + phi0, q_l0, (uint32_t)(s * d.F), vec);
-        cp_lane<NPHI>(tl_er + s * FT + phi0, q_p0, (uint32_t)(s * d.F), vec);
+      {
+        uint32_t dt = fs_smem_u32(tl_t0 + phi0), de = fs_smem_u32(tl_er + phi0);
+        LanePtr gl = q_l0, gp = q_p0;
+#pragma unroll 4
+        for (int s = 0; s < d.S; ++s) {
+          cp_lane<NPHI>(dt, gl, vec); cp_lane<NPHI>(de, gp, vec);
+          dt += FT * 4u; de += FT * 4u;
+          gl.a += d.F; gl.b += d.F; gp.a += d.F; gp.b += d.F;
+        }
       }
       for (int s0 = 0; s0 < d.S; s0 += 4) {
         float a1[4][NPHI], b1[4][NPHI];
