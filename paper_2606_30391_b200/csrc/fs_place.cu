@@ -147,6 +147,7 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
 constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102)
 constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
 constexpr int DENSE_S = FS_MAX_S;
+constexpr int DENSE_TAIL = 4;                 // rounds of requests per warp handed out dynamically at the end
 
 // does any of the four 16-bit models packed in (w0, w1) equal m?  (exact "has a zero halfword" test on the
 // XOR; the SIMD-in-a-word video instructions are emulated on this architecture and cost ~30 instructions)
@@ -196,9 +197,10 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
 //   rec  [KS]            the block's slice of the SORTED compact GPU records (one TMA fill)
 //   tile [W][2][S][FT]   per warp: t0 rows, then er rows, of the request being scored
 //   wb   [W][32]         per warp: {T*, Ecur, sm_free, GPU} of the chunk's survivors
-//   bnd  [W][3][16]      per warp: prefix minima over sigma <= s, all phi, of er (cold), t0, e0
+//   bnd  [W][3][32]      per warp: prefix minima over sigma <= s, all phi, of er (cold), t0, e0
+//   req  [W]             per warp: the next statically assigned request, prefetched by cp.async
 __host__ __device__ inline size_t dense_warp_bytes(int S, int FT) {
-  return (size_t)2 * S * FT * sizeof(float) + FS_CHUNK * sizeof(float4) + 3 * DENSE_S * sizeof(float);
+  return (size_t)2 * S * FT * sizeof(float) + FS_CHUNK * sizeof(float4) + 3 * DENSE_S * sizeof(float) + sizeof(fs_request);
 }
 __host__ __device__ inline size_t dense_smem_bytes(int KS, int W, int S, int FT) {
   return (size_t)KS * sizeof(FsGpuRec) + (size_t)W * dense_warp_bytes(S, FT) + 16;
@@ -325,13 +327,37 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const bool vec = NPHI == 2 && (d.F & 1) == 0;
   const int phi0 = lane * NPHI;
   const LanePtr q_a0 = lane_ptr<NPHI>(v.gA0, phi0, FT, true);
+  // ---- which requests this warp scores: all but the last DENSE_TAIL rounds are assigned statically
+  // (warp w of the slice takes w, w + wps, ...), so the next request is known and fetched while the
+  // current one is scored (ticket -> request -> model info is otherwise a serial chain of three memory
+  // latencies at the head of every request); the tail is handed out dynamically, one atomic per warp,
+  // and evens out what the static part left uneven.
+  fs_request* s_req = reinterpret_cast<fs_request*>(bnd + 3 * DENSE_S);
+  const int wps = ((int)gridDim.x / nslice) * W, widx = ((int)blockIdx.x / nslice) * W + warp;
+  const int R0 = max(0, R - DENSE_TAIL * wps);
+  int r_static = widx;
+  bool fetched = false;                                  // s_req holds request r_static
   for (;;) {
-    // ---- next request of this slice: dynamic, one atomic per warp ----------------------------
     int r = 0;
-    if (lane == 0) r = (int)atomicAdd(&ctr[slice], 1u);
-    r = __shfl_sync(0xffffffffu, r, 0);
-    if (r >= R) break;
-    const ReqCtx c = make_req(v, reqs[r]);
+    fs_request rq;
+    if (r_static < R0) {
+      r = r_static; r_static += wps;
+      if (fetched) {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+        rq = *s_req;
+        __syncwarp();
+        fetched = false;
+      } else {
+        rq = reqs[r];
+      }
+    } else {
+      if (lane == 0) r = R0 + (int)atomicAdd(&ctr[slice], 1u);
+      r = __shfl_sync(0xffffffffu, r, 0);
+      if (r >= R) break;
+      rq = reqs[r];
+    }
+    const ReqCtx c = make_req(v, rq);
     if (!c.valid) {
       if (lane == 0 && slice == 0) {
         fs_raise(v.flag, FS_FLAG_REQUEST);
@@ -407,6 +433,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         }
       }
       __syncwarp();
+    }
+    if (r_static < R0) {                                 // the next static request, on its way during the scoring
+      if (lane < 2) {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(fs_smem_u32(s_req) + 16u * lane),
+                     "l"(reinterpret_cast<const char*>(reqs + r_static) + 16 * lane) : "memory");
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      fetched = true;
     }
     // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scans are not in index order
     float best = FS_INF; int bestk = KNONE;
