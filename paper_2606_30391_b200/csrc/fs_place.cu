@@ -451,9 +451,11 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     //   warm bound:  dE >= fl(fl(a_min + fl(e0min + e1min)) - Ecur),  e1min = fl(fl(rounds1*l1_min)*p1_min)
     int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
     uint32_t ordl = NONE32; int wk = 0;
+    uint32_t wpk = 0; float wta = 0.f, wec = 0.f;       // the lane's item: j | br1 << 8 | sm_free << 16, T_avail, Ecur
     bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32;
     for (;;) {
       int k = KNONE;
+      int wsrc = -1;                                    // lane that holds the chosen warm item
       while (!recover) {
         const uint32_t mn = warp_min_u32(ordl);
         const uint32_t inc = warp_min_u32(fs_orderable(best));
@@ -461,6 +463,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           const int src = __ffs(__ballot_sync(0xffffffffu, ordl == mn)) - 1;
           k = __shfl_sync(0xffffffffu, wk, src);
           if (lane == src) ordl = NONE32;
+          wsrc = src;
           break;
         }
         if (ib >= ie) {                                 // no item left that could beat the incumbent
@@ -554,13 +557,24 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             const bool tbt_ok = c.O == 0 || it.l1_min <= c.slo_tbt;
             const bool ttft_ok = c.L == 0 || __fadd_rn(it.t_avail_ms, bnd[DENSE_S + it.sm_free - 1]) <= c.slo_ttft;
             if (tbt_ok && ttft_ok && lb < FS_INF) ordl = fs_orderable(lb);
-            wk = it.k;
+            wk = it.k; wpk = (uint32_t)it.j | ((uint32_t)it.br1 << 8) | ((uint32_t)it.sm_free << 16);
+            wta = it.t_avail_ms; wec = it.e_cur;
           }
         }
         ib += 32;
       }
       if (k == KNONE) break;                            // no feasible candidate at all
-      const PairCtx p = make_pair(v, c, v.ginfo[k]);
+      // a warm pair's context comes from the item its lane holds (the item passed the memory, bucket and
+      // share tests when it was listed); only the recovery of a cold winner reads the GPU's summary
+      PairCtx p;
+      if (wsrc >= 0) {
+        const uint32_t pk = __shfl_sync(0xffffffffu, wpk, wsrc);
+        p.ok = true; p.j = (int)(pk & 0xFFu); p.var = p.j + 1; p.br1 = (int)((pk >> 8) & 0xFFu); p.smf = (int)(pk >> 16);
+        p.wait = __shfl_sync(0xffffffffu, wta, wsrc); p.ecur = __shfl_sync(0xffffffffu, wec, wsrc);
+        p.rounds1 = fs_ceil_div(c.O, (uint32_t)p.br1 + 1u);
+      } else {
+        p = make_pair(v, c, v.ginfo[k]);
+      }
       if (p.ok) {
         if (STATS) { n_scored += 1; n_cscored += (uint32_t)(p.smf * d.F); }
         const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
