@@ -417,11 +417,12 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
               const float t = __fmul_rn(fr0, a0[i]);
               const float e0 = __fmul_rn(t, b0[i]);
               const float e = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
-              const bool in = (phi0 + i) < d.F;
-              tt[i] = in ? t : FS_INF;
-              ee[i] = (in && a1[u][i] <= tbt) ? e : FS_INF;
-              if (in) ue0 = min(ue0, __float_as_uint(e0));
-              ue = min(ue, __float_as_uint(ee[i])); ut = min(ut, __float_as_uint(tt[i]));
+              // a padded lane (phi >= F) holds a copy of the row's last column(s): the minima are unchanged,
+              // and every consumer of the tiles adds an A row that is +INF there
+              tt[i] = t;
+              ee[i] = a1[u][i] <= tbt ? e : FS_INF;
+              ue0 = min(ue0, __float_as_uint(e0));
+              ue = min(ue, __float_as_uint(ee[i])); ut = min(ut, __float_as_uint(t));
             }
             st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
             pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut)); pe0 = min(pe0, warp_min_u32(ue0));
