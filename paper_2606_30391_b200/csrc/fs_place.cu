@@ -336,6 +336,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const int wps = ((int)gridDim.x / nslice) * W, widx = ((int)blockIdx.x / nslice) * W + warp;
   const int R0 = max(0, R - DENSE_TAIL * wps);
   int r_static = widx;
+  const bool req_aligned = (reinterpret_cast<unsigned long long>(reqs) & 15ull) == 0;   // 16-byte copies
   bool fetched = false;                                  // s_req holds request r_static
   for (;;) {
     int r = 0;
@@ -435,7 +436,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       }
       __syncwarp();
     }
-    if (r_static < R0) {                                 // the next static request, on its way during the scoring
+    if (r_static < R0 && req_aligned) {                  // the next static request, on its way during the scoring
       if (lane < 2) {
         asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(fs_smem_u32(s_req) + 16u * lane),
                      "l"(reinterpret_cast<const char*>(reqs + r_static) + 16 * lane) : "memory");

@@ -398,6 +398,24 @@ def test_dispatch_full_size(ctx):
     assert set(np.unique(got["f_req"]).tolist()) >= {1, 2, 3}
 
 
+def test_device_requests_at_a_4_byte_aligned_address(ctx):
+    """fs_request has 4-byte alignment: a device array that starts at any multiple of 4 must work
+    (the scoring kernel prefetches requests with 16-byte asynchronous copies only when it can)."""
+    import torch
+    cl = synth.make_cluster("rack")
+    ctx.load_cluster(cl)
+    ref = ctx.place_batch(cl.requests)
+    raw = torch.from_numpy(cl.requests.view(np.uint8).reshape(-1).copy())
+    for off in (4, 8, 20):
+        buf = torch.zeros(raw.numel() + 64, dtype=torch.uint8, device="cuda")
+        buf[off:off + raw.numel()] = raw.cuda()
+        out = torch.zeros(cl.R * 32 + 64, dtype=torch.uint8, device="cuda")
+        ctx.place_batch(buf[off:], out=out[off:], R=cl.R)
+        d = ctx.dispatch(buf[off:], out=torch.zeros(cl.R * 32, dtype=torch.uint8, device="cuda"), R=cl.R)
+        torch.cuda.synchronize()
+        assert out[off:off + cl.R * 32].cpu().numpy().tobytes() == ref.tobytes(), off
+
+
 def test_host_pinned_async_equals_host(ctx):
     import paper_2606_30391_b200 as fs
     """FS_HOST_PINNED: page-locked host buffers, the call does not wait; same bytes as the blocking FS_HOST calls."""
