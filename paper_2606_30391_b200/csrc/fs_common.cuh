@@ -106,6 +106,14 @@ __device__ __forceinline__ unsigned long long fs_warp_min_key(unsigned long long
 //   rounds = ceil(q/(beta+1)); t = fl(rounds*lat); e = fl(t*pow)
 //   prefill (p==0): ok = fl(wait+t) <= slo;   decode: ok = lat <= slo
 struct FsSlot { bool ok; float t, e; };
+// the same with the round count already converted (exact: rounds < 2^24)
+__device__ __forceinline__ FsSlot fs_slot_f(int p, float lat, float pw, float frounds, float wait, float slo) {
+  FsSlot s;
+  s.t = __fmul_rn(frounds, lat);
+  s.ok = (p == 0) ? (__fadd_rn(wait, s.t) <= slo) : (lat <= slo);
+  s.e = __fmul_rn(s.t, pw);
+  return s;
+}
 __device__ __forceinline__ FsSlot fs_slot(int p, float lat, float pw, uint32_t rounds, float wait,
                                           float slo) {
   FsSlot s;

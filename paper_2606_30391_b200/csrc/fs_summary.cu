@@ -60,23 +60,63 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
   const bool valid = state_valid(g, d);
   const int n = valid ? g.n_res : 0;
   float* A = gA + (size_t)k * FS_NVAR * d.F;
-  int f_floor = -1; float a_min = FS_INF;
+  int f_floor = -1; float a_min = FS_INF, ecur = 0.0f;
+  // per tenant, independent of phi: plane offsets and rounds of the prefill slot, the decode slot as it is
+  // and the decode slot with one more sequence (the integer divisions are done once, not per frequency)
+  size_t o0[FS_RMAX], o1[FS_RMAX], o1b[FS_RMAX]; float r0[FS_RMAX], r1[FS_RMAX], r1b[FS_RMAX];
+  bool has0[FS_RMAX], has1[FS_RMAX], bump_ok[FS_RMAX];
+#pragma unroll
+  for (int i = 0; i < FS_RMAX; ++i) {
+    o0[i] = o1[i] = o1b[i] = 0; r0[i] = r1[i] = r1b[i] = 0.f; has0[i] = has1[i] = false; bump_ok[i] = true;
+    if (i < n) {
+      const fs_tenant& t = g.t[i];
+      const int b1 = t.beta[1], b1b = b1 + (t.q[1] > 0 ? 1 : 0);
+      has0[i] = t.q[0] > 0; has1[i] = t.q[1] > 0; bump_ok[i] = b1b < d.B;
+      o0[i] = fs_plane(d, t.model, 0, t.beta[0]) + (size_t)t.sigma * d.F;
+      o1[i] = fs_plane(d, t.model, 1, b1) + (size_t)t.sigma * d.F;
+      o1b[i] = fs_plane(d, t.model, 1, min(b1b, d.B - 1)) + (size_t)t.sigma * d.F;
+      r0[i] = __uint2float_rn(fs_ceil_div(t.q[0], t.beta[0] + 1u));
+      r1[i] = __uint2float_rn(fs_ceil_div(t.q[1], b1 + 1u));
+      r1b[i] = __uint2float_rn(fs_ceil_div(t.q[1], (uint32_t)min(b1b, d.B - 1) + 1u));
+    }
+  }
   for (int base = 0; base < d.F; base += 32) {
-    const int phi = base + lane;
+    const int phi = base + lane, pc = min(phi, d.F - 1);
+    // every table entry of this frequency first (up to 24 independent loads in flight: the tables are
+    // cold in L2 at this point of a step, and one miss after the other is what this kernel would wait for)
+    float l0[FS_RMAX], p0[FS_RMAX], l1[FS_RMAX], p1[FS_RMAX], l1b[FS_RMAX], p1b[FS_RMAX];
+#pragma unroll
+    for (int i = 0; i < FS_RMAX; ++i) {
+      l0[i] = p0[i] = l1[i] = p1[i] = l1b[i] = p1b[i] = 1.0f;
+      if (i < n) {
+        l0[i] = v.latT[o0[i] + pc]; p0[i] = v.powT[o0[i] + pc];
+        l1[i] = v.latT[o1[i] + pc]; p1[i] = v.powT[o1[i] + pc];
+        l1b[i] = v.latT[o1b[i] + pc]; p1b[i] = v.powT[o1b[i] + pc];
+      }
+    }
+    float e_plain[FS_RMAX], e_bump[FS_RMAX]; bool ok_plain[FS_RMAX], ok_bump[FS_RMAX];
+    float esum = 0.0f;                                   // slot-order energy sum as it is (Ecur at F_curr)
+#pragma unroll
+    for (int i = 0; i < FS_RMAX; ++i) {
+      e_plain[i] = e_bump[i] = 0.0f; ok_plain[i] = ok_bump[i] = true;
+      if (i < n) {
+        const fs_tenant& t = g.t[i];
+        bool ok = true; float e0 = 0.0f, e1 = 0.0f, e1b = 0.0f; bool okb = true;
+        if (has0[i]) { const FsSlot sl = fs_slot_f(0, l0[i], p0[i], r0[i], 0.0f, t.slo_ms[0]); ok = sl.ok; e0 = sl.e; }
+        okb = ok;
+        if (has1[i]) {
+          const FsSlot sl = fs_slot_f(1, l1[i], p1[i], r1[i], 0.0f, t.slo_ms[1]); ok = ok && sl.ok; e1 = sl.e;
+          const FsSlot sb = fs_slot_f(1, l1b[i], p1b[i], r1b[i], 0.0f, t.slo_ms[1]); okb = okb && sb.ok; e1b = sb.e;
+        }
+        e_plain[i] = __fadd_rn(e0, e1); ok_plain[i] = ok;
+        if (has1[i]) { e_bump[i] = bump_ok[i] ? __fadd_rn(e0, e1b) : FS_INF; ok_bump[i] = bump_ok[i] && okb; }
+        else { e_bump[i] = e_plain[i]; ok_bump[i] = ok; }
+        esum = (i == 0) ? e_plain[i] : __fadd_rn(esum, e_plain[i]);
+      }
+    }
+    if (n >= 1 && base == (g.f_cur & ~31)) ecur = __shfl_sync(0xffffffffu, esum, g.f_cur & 31);
     bool ok0 = false;
     if (phi < d.F) {
-      float e_plain[FS_RMAX], e_bump[FS_RMAX]; bool ok_plain[FS_RMAX], ok_bump[FS_RMAX];
-#pragma unroll
-      for (int i = 0; i < FS_RMAX; ++i) {
-        if (i < n) {
-          TenantE a = tenant_eval(v, g.t[i], phi, g.t[i].sigma, false);
-          e_plain[i] = a.e; ok_plain[i] = a.ok;
-          if (g.t[i].q[1] > 0) {
-            TenantE b = tenant_eval(v, g.t[i], phi, g.t[i].sigma, true);
-            e_bump[i] = b.e; ok_bump[i] = b.ok;
-          } else { e_bump[i] = a.e; ok_bump[i] = a.ok; }
-        } else { e_plain[i] = e_bump[i] = 0.0f; ok_plain[i] = ok_bump[i] = true; }
-      }
 #pragma unroll
       for (int var = 0; var < FS_NVAR; ++var) {
         float acc = FS_INF; bool ok = (n >= 1) && (var <= n);
@@ -104,7 +144,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     FsGpuInfo gi;
     gi.t_avail_ms = g.t_avail_ms; gi.mem_free_mb = g.mem_free_mb;
     gi.n_res = n; gi.f_floor = f_floor; gi.f_cur = n ? g.f_cur : 0; gi._pad = 0;
-    int used = 0; float ecur = 0.0f;
+    int used = 0;
     for (int i = 0; i < FS_RMAX; ++i) {
       if (i < n) {
         const fs_tenant& t = g.t[i];
@@ -112,8 +152,6 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
         gi.model[i] = t.model;
         const int b = (t.q[1] > 0) ? t.beta[1] + 1 : 0;
         gi.br1[i] = (int16_t)(b >= d.B ? -1 : b);
-        TenantE a = tenant_eval(v, t, g.f_cur, t.sigma, false);
-        ecur = (i == 0) ? a.e : __fadd_rn(ecur, a.e);
       } else { gi.model[i] = -1; gi.br1[i] = -1; }
     }
     gi.e_cur = ecur; gi.sm_free = n ? d.S - used : 0;
