@@ -280,7 +280,9 @@ __device__ __forceinline__ void st_tile(float* p, const float (&x)[NPHI]) {
   else p[0] = x[0];
 }
 
-template <int NPHI, bool STATS>
+// VEC: the lane's two adjacent frequencies are one aligned 64-bit access (NPHI == 2 and F even); a template
+// parameter so that every row access is one instruction without a branch on the shape
+template <int NPHI, bool VEC, bool STATS>
 __global__ void __launch_bounds__(DENSE_MAXW * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
@@ -324,7 +326,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const float tmin = (float)v.dsuf[2 + nchunk_all];
   // work counters (warp-uniform except n_elig / n_witems, which are per lane)
   uint32_t n_chunks = 0, n_elig = 0, n_swept = 0, n_cswept = 0, n_witems = 0, n_scored = 0, n_cscored = 0, n_req = 0;
-  const bool vec = NPHI == 2 && (d.F & 1) == 0;
+  constexpr bool vec = VEC;
   const int phi0 = lane * NPHI;
   const LanePtr q_a0 = lane_ptr<NPHI>(v.gA0, phi0, FT, true);
   // ---- which requests this warp scores: all but the last DENSE_TAIL rounds are assigned statically
@@ -1291,10 +1293,12 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
 }  // namespace
 
 int fsk_place_smem_attr() {
-  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
   e |= (int)cudaFuncSetAttribute(dispatch_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 32 * 4);
   e |= (int)cudaFuncSetAttribute(dispatch_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 64 * 4);
   return e;
@@ -1335,10 +1339,12 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     // one slice: the scoring kernel writes the placement records itself (no key array, no decode launch)
     fs_placement* direct = nslice == 1 ? out : nullptr;
     if (!direct) cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-#define FS_LAUNCH_DENSE(NP, ST) \
-  place_dense_kernel<NP, ST><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats, direct)
-    if (FT == 32) { if (sc.count_work) FS_LAUNCH_DENSE(1, true); else FS_LAUNCH_DENSE(1, false); }
-    else          { if (sc.count_work) FS_LAUNCH_DENSE(2, true); else FS_LAUNCH_DENSE(2, false); }
+#define FS_LAUNCH_DENSE(NP, VC, ST) \
+  place_dense_kernel<NP, VC, ST><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats, direct)
+    const bool vec = FT == 64 && (v.d.F & 1) == 0;
+    if (FT == 32)  { if (sc.count_work) FS_LAUNCH_DENSE(1, false, true); else FS_LAUNCH_DENSE(1, false, false); }
+    else if (vec)  { if (sc.count_work) FS_LAUNCH_DENSE(2, true, true);  else FS_LAUNCH_DENSE(2, true, false); }
+    else           { if (sc.count_work) FS_LAUNCH_DENSE(2, false, true); else FS_LAUNCH_DENSE(2, false, false); }
 #undef FS_LAUNCH_DENSE
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);
