@@ -456,7 +456,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
     uint32_t ordl = NONE32; int wk = 0;
     uint32_t wpk = 0; float wta = 0.f, wec = 0.f;       // the lane's item: j | br1 << 8 | sm_free << 16, T_avail, Ecur
-    bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32;
+    bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32; int kwin = 0;
     for (;;) {
       int k = KNONE;
       int wsrc = -1;                                    // lane that holds the chosen warm item
@@ -542,7 +542,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             }
           }
           const unsigned long long kk = fs_warp_min_key(((unsigned long long)fs_orderable(best) << 32) | (uint32_t)bestk);
-          recover = true; k = (int)(uint32_t)kk; bestW = fs_unorderable((uint32_t)(kk >> 32));
+          recover = true; k = (int)(uint32_t)kk; kwin = k; bestW = fs_unorderable((uint32_t)(kk >> 32));
           // a warm winner was scored by the definition in flat order: its lanes already hold their
           // lowest flat index, nothing to recover (a GPU is warm or cold for a request, never both)
           if (k != KNONE && best == bestW && bestk == k) flat = bflat;
@@ -551,7 +551,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         }
         ordl = NONE32;                                  // next 32 items: lane <-> item
         const int ix = ib + lane;
-        if (ix < ie && ix % nslice == slice) {
+        if (ix < ie && (nslice == 1 || ix % nslice == slice)) {
           const FsWarmItem it = witems[ix];
           if (it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
             if (STATS) { n_witems += 1; }
@@ -635,7 +635,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
       if (key != FS_KEY_NONE) {
         const uint32_t fl = (uint32_t)key;
-        const int phis = fl % d.F, sgs = (fl / d.F) % d.S, ks = fl / (d.F * d.S);
+        // the winning GPU is known (kwin); one small division instead of three 32-bit ones
+        const int ks = kwin, rem = (int)(fl - (uint32_t)(ks * d.S * d.F)), sgs = rem / d.F, phis = rem - sgs * d.F;
         const PairCtx p = make_pair(v, c, v.ginfo[ks]);
         const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
         const float* Ar = v.gA + ((size_t)ks * FS_NVAR + p.var) * d.F;
