@@ -43,9 +43,9 @@ OPS_WARM_TEST = 20.0       # per warm pair tested: 12-word item, bound (5 fp32),
 OPS_DEF = 14.0             # per candidate scored by the definition: 4 loads, 4 mul, 3 add/sub, 3 compares
 # dram bytes per launch of the scoring kernel and its issue utilisation, from the committed ncu
 # capture of this workload (profiles/; a profiler cannot run inside the timed bench)
-NCU_TRAFFIC_BYTES = 42.56e6
+NCU_TRAFFIC_BYTES = 42.45e6
 NCU_NOTE = {"source": "profiles/r01_final_pod.md (ncu --set full of this kernel on this workload)",
-            "sm_throughput_pct_of_peak": 67.5, "issue_active_pct_of_peak": 72.3, "warp_instructions": 229.6e6,
+            "sm_throughput_pct_of_peak": 65.1, "issue_active_pct_of_peak": 70.4, "warp_instructions": 199.8e6,
             "note": "executed instructions; `frac` above counts only the lane-operations the method needs"}
 SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128   # 4 schedulers x 32 lanes (B300_MICROARCH "issue")
 
