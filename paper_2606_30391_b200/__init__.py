@@ -343,10 +343,11 @@ class Festina:
         self._check(rc, "fs_migration_select")
         return flags[:r], ms[:r]
 
-    def consolidate(self, out=None, stream=None):
+    def consolidate(self, out=None, stream=None, pinned: bool = False):
         if out is None:
             out = np.zeros(self.K, dtype=synth.CONSOL_DT)
         po, spo, keep = _buf(out, self.K * 16)
+        spo = _pin(spo, pinned, out)
         rc = lib().fs_consolidate(self._h, po, spo, _stream_ptr(stream))
         self._check(rc, "fs_consolidate")
         return out
