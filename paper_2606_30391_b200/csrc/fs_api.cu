@@ -241,13 +241,13 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
     FS_TRY(grow(c, c->states, (size_t)K)); FS_TRY(grow(c, c->ginfo, (size_t)K));
     FS_TRY(grow(c, c->grec, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->gsort, (size_t)K + FS_CHUNK));
     FS_TRY(grow(c, c->dsort, (size_t)K + FS_CHUNK)); FS_TRY(grow(c, c->dsuf, (size_t)K / FS_CHUNK + 8 + ((size_t)K + FS_CHUNK) / 2 + 1));
-    FS_TRY(grow(c, c->ctr, (size_t)K / FS_CHUNK + 2));
+    FS_TRY(grow(c, c->ctr, ((size_t)K / FS_CHUNK + 2) * ((FS_MAX_F + 63) / 64)));   // one counter per (slice, column block)
     FS_TRY(grow(c, c->warm_item, (size_t)K * FS_RMAX));
     c->k_cap = K; c->consol_cap = 0;
   }
   const size_t na = (size_t)K * FS_NVAR * c->d.F;
   if (na > c->gA_cap) { FS_TRY(grow(c, c->gA, na)); c->gA_cap = na; }
-  c->Kpad = (K + FS_CHUNK - 1) / FS_CHUNK * FS_CHUNK; c->FT = (c->d.F + 31) / 32 * 32;
+  c->Kpad = (K + FS_CHUNK - 1) / FS_CHUNK * FS_CHUNK; c->FT = c->d.F <= 64 ? (c->d.F + 31) / 32 * 32 : (c->d.F + 63) / 64 * 64;   // gA0 row stride: whole column blocks
   const size_t na0 = (size_t)c->Kpad * c->FT;
   if (na0 > c->gA0_cap) { FS_TRY(grow(c, c->gA0, na0)); c->gA0_cap = na0; }
   if (c->d.M > c->warm_m_cap) {

@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
 
 
 // =============================================================================================
-// Dense scorer, S <= 32 (FS_MAX_S), F <= 64: one warp = one request, one persistent block per SM.
+// Dense scorer, every supported shape (S <= 32; F <= 256 in column blocks of 64): one warp = one request, one persistent block per SM.
 //
 // Factorisation (exact).  For a COLD pair (the request's model is
 // not resident on the GPU) the decode bucket is 0 and the co-resident variant is 0, so everything
@@ -282,10 +282,14 @@ __device__ __forceinline__ void st_tile(float* p, const float (&x)[NPHI]) {
 
 // VEC: the lane's two adjacent frequencies are one aligned 64-bit access (NPHI == 2 and F even); a template
 // parameter so that every row access is one instruction without a branch on the shape
-template <int NPHI, bool VEC, bool STATS>
+// COLS: F > 64.  The frequencies are cut into blocks of 64 columns; a thread block scores every request on
+// (its slice of the GPUs) x (its column block), exactly like one more kind of slice: all row pointers are
+// shifted by the block's first column, the per-GPU bounds (minima over ALL frequencies) stay valid lower
+// bounds, and the results are merged by the 64-bit key (the record is then written by the decode kernel).
+template <int NPHI, bool VEC, bool STATS, bool COLS>
 __global__ void __launch_bounds__(DENSE_MAXW * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
-                   unsigned long long* __restrict__ keys, int nslice, int chunks_per_slice,
+                   unsigned long long* __restrict__ keys, int nslice, int ncb, int chunks_per_slice,
                    unsigned int* __restrict__ ctr, const int32_t* __restrict__ warm_off,
                    const FsWarmItem* __restrict__ witems, unsigned long long* __restrict__ stats,
                    fs_placement* __restrict__ out) {
@@ -296,7 +300,11 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const FsDimsDev d = v.d;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
   const int nchunk_all = v.Kpad / FS_CHUNK;
-  const int slice = blockIdx.x % nslice;
+  const int nsc = COLS ? nslice * ncb : nslice;         // (slice, column block) combinations
+  const int sci = blockIdx.x % nsc;
+  const int slice = COLS ? sci % nslice : sci;
+  const int cb0 = COLS ? (sci / nslice) * 64 : 0;        // first frequency of this block's columns
+  const int FA = COLS ? v.FT : FT;                       // row stride of gA0 (F rounded up to 64 when F > 64)
   const int c0 = slice * chunks_per_slice, c1 = min(nchunk_all, c0 + chunks_per_slice);
   const int nchunk = c1 - c0, KS = nchunk * FS_CHUNK, KSmax = chunks_per_slice * FS_CHUNK;
   FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw);
@@ -328,14 +336,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   uint32_t n_chunks = 0, n_elig = 0, n_swept = 0, n_cswept = 0, n_witems = 0, n_scored = 0, n_cscored = 0, n_req = 0;
   constexpr bool vec = VEC;
   const int phi0 = lane * NPHI;
-  const LanePtr q_a0 = lane_ptr<NPHI>(v.gA0, phi0, FT, true);
+  const LanePtr q_a0 = lane_ptr<NPHI>(v.gA0 + cb0, phi0, FT, true);
   // ---- which requests this warp scores: all but the last DENSE_TAIL rounds are assigned statically
   // (warp w of the slice takes w, w + wps, ...), so the next request is known and fetched while the
   // current one is scored (ticket -> request -> model info is otherwise a serial chain of three memory
   // latencies at the head of every request); the tail is handed out dynamically, one atomic per warp,
   // and evens out what the static part left uneven.
   fs_request* s_req = reinterpret_cast<fs_request*>(bnd + 3 * DENSE_S);
-  const int wps = ((int)gridDim.x / nslice) * W, widx = ((int)blockIdx.x / nslice) * W + warp;
+  const int wps = ((int)gridDim.x / nsc) * W, widx = ((int)blockIdx.x / nsc) * W + warp;
   const int R0 = max(0, R - DENSE_TAIL * wps);
   int r_static = widx;
   const bool req_aligned = (reinterpret_cast<unsigned long long>(reqs) & 15ull) == 0;   // 16-byte copies
@@ -355,14 +363,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         rq = reqs[r];
       }
     } else {
-      if (lane == 0) r = R0 + (int)atomicAdd(&ctr[slice], 1u);
+      if (lane == 0) r = R0 + (int)atomicAdd(&ctr[sci], 1u);
       r = __shfl_sync(0xffffffffu, r, 0);
       if (r >= R) break;
       rq = reqs[r];
     }
     const ReqCtx c = make_req(v, rq);
     if (!c.valid) {
-      if (lane == 0 && slice == 0) {
+      if (lane == 0 && sci == 0) {
         fs_raise(v.flag, FS_FLAG_REQUEST);
         if (out) {
           fs_placement o; o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
@@ -378,11 +386,12 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     // (monotone rounding).  er, t0, e0 >= +0, so their bit patterns order like unsigned integers.
     // L == 0 / O == 0 need no branches: rounds = 0 gives t = e = +0 exactly (tables are finite),
     // and an empty decode slot passes its deadline (threshold +INF).
-    const LanePtr q_p0 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 0, c.br0), phi0, d.F, vec);
+    const int Fc = d.F - cb0;                            // columns from this block's first one to the end of a row
+    const LanePtr q_p0 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 0, c.br0) + cb0, phi0, Fc, vec);
     {
-      const LanePtr q_l0 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 0, c.br0), phi0, d.F, vec);
-      const LanePtr q_l1 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 1, 0), phi0, d.F, vec);
-      const LanePtr q_p1 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 1, 0), phi0, d.F, vec);
+      const LanePtr q_l0 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 0, c.br0) + cb0, phi0, Fc, vec);
+      const LanePtr q_l1 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 1, 0) + cb0, phi0, Fc, vec);
+      const LanePtr q_p1 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 1, 0) + cb0, phi0, Fc, vec);
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
       const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
       uint32_t pe = INFBITS, pt = INFBITS, pe0 = INFBITS;   // running prefix minima (bits)
@@ -524,7 +533,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
               const float Tst = w.x; const int sfree = __float_as_int(w.z); const int k = __float_as_int(w.w);
               if (STATS) { n_swept += 1; n_cswept += (uint32_t)(sfree * d.F); }
               float arow[NPHI], m[NPHI];
-              ld_lane<NPHI>(q_a0, (uint32_t)k * FT, true, arow);   // rows are FT-padded: aligned
+              ld_lane<NPHI>(q_a0, (uint32_t)k * (uint32_t)FA, true, arow);   // rows are padded with +INF: aligned
       #pragma unroll
               for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
       #pragma unroll 4
@@ -582,14 +591,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       if (p.ok) {
         if (STATS) { n_scored += 1; n_cscored += (uint32_t)(p.smf * d.F); }
         const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
-        const LanePtr w_l1 = lane_ptr<NPHI>(l1, phi0, d.F, vec), w_p1 = lane_ptr<NPHI>(p1, phi0, d.F, vec);
-        const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F;
+        const LanePtr w_l1 = lane_ptr<NPHI>(l1 + cb0, phi0, Fc, vec), w_p1 = lane_ptr<NPHI>(p1 + cb0, phi0, Fc, vec);
+        const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F + cb0;
         const float fr1 = __uint2float_rn(p.rounds1);
         // an empty prefill / decode slot passes its deadline whatever the wait (slot rule, q == 0)
         const float wait_e = c.L ? p.wait : 0.0f, ttft_e = c.L ? c.slo_ttft : FS_INF, tbt_e = c.O ? c.slo_tbt : FS_INF;
         float ar[NPHI];
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < d.F ? Ar[phi0 + i] : FS_INF;
+        for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < Fc ? Ar[phi0 + i] : FS_INF;
         // four share rows per trip: their 12 plane loads are issued before any of them is used.  Each lane
         // keeps the minimum of ITS candidates of this pair and the first (lowest flat) candidate attaining
         // it; merged into the incumbent afterwards, or, in the recovery pass, matched against the winner's
@@ -614,7 +623,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
               const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
               const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   // -0 == +0 in every compare below
               const bool ok = s < p.smf && __fadd_rn(wait_e, tt[u][i]) <= ttft_e && a1[u][i] <= tbt_e;
-              if (ok && dE < pb) { pb = dE; pflat = (uint32_t)((k * d.S + s) * d.F + phi0 + i); }   // INF never enters
+              if (ok && dE < pb) { pb = dE; pflat = (uint32_t)((k * d.S + s) * d.F + cb0 + phi0 + i); }   // INF never enters
             }
           }
         }
@@ -625,7 +634,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     }
     unsigned long long key = flat != NONE32 ? fs_make_key(bestW, flat) : FS_KEY_NONE;
     key = fs_warp_min_key(key);
-    if (out == nullptr) {                              // several slices: merge by key, decode afterwards
+    if (COLS || out == nullptr) {                      // several slices / column blocks: merge by key, decode afterwards
       if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
     } else {
       // one slice: this warp saw every GPU, so it writes the placement record itself: the chosen
@@ -1294,12 +1303,15 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
 }  // namespace
 
 int fsk_place_smem_attr() {
-  int e = (int)cudaFuncSetAttribute(place_dense_kernel<1, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<2, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX);
+  int e = 0;
+#define FS_ATTR_DENSE(NP, VC, ST, CL) \
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<NP, VC, ST, CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX)
+  FS_ATTR_DENSE(1, false, false, false); FS_ATTR_DENSE(1, false, true, false);
+  FS_ATTR_DENSE(2, false, false, false); FS_ATTR_DENSE(2, false, true, false);
+  FS_ATTR_DENSE(2, true, false, false);  FS_ATTR_DENSE(2, true, true, false);
+  FS_ATTR_DENSE(2, false, false, true);  FS_ATTR_DENSE(2, false, true, true);
+  FS_ATTR_DENSE(2, true, false, true);   FS_ATTR_DENSE(2, true, true, true);
+#undef FS_ATTR_DENSE
   e |= (int)cudaFuncSetAttribute(dispatch_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 32 * 4);
   e |= (int)cudaFuncSetAttribute(dispatch_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 64 * 4);
   return e;
@@ -1315,7 +1327,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
   }
-  const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= 64 && !sc.force_generic;
+  const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= FS_MAX_F && !sc.force_generic;
   fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
   if (dense_ok) {
     // one persistent block per SM; each holds a slice of the sorted GPU records in shared memory
@@ -1323,6 +1335,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     // fewer when R alone cannot occupy every SM; the number of slices is what the slice size
     // forces, raised when the request batches alone cannot occupy every SM.
     const int FT = v.d.F <= 32 ? 32 : 64;
+    const int ncb = (v.d.F + 63) / 64;                 // column blocks of 64 frequencies (1 unless F > 64)
     const int nchunk = v.Kpad / FS_CHUNK;
     const size_t pw = dense_warp_bytes(v.d.S, FT), per_chunk = (size_t)FS_CHUNK * sizeof(FsGpuRec);
     int W = (int)((DENSE_SMEM_MAX - 16 - (size_t)min(nchunk, 64) * per_chunk) / pw);
@@ -1330,22 +1343,28 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     const int max_cps = (int)((DENSE_SMEM_MAX - 16 - (size_t)W * pw) / per_chunk);
     int nslice = (nchunk + max_cps - 1) / max_cps;
     const int nbatch = (R + W - 1) / W;
-    if (nbatch * nslice < sc.sm_count) nslice = min(nchunk, (sc.sm_count + nbatch - 1) / nbatch);
+    if (nbatch * nslice * ncb < sc.sm_count) nslice = min(nchunk, max(nslice, (sc.sm_count + nbatch * ncb - 1) / (nbatch * ncb)));
     const int cps = (nchunk + nslice - 1) / nslice;
     nslice = (nchunk + cps - 1) / cps;
-    const int streams = max(1, min(nbatch, sc.sm_count / nslice));
-    const int grid = streams * nslice;
+    const int nsc = nslice * ncb;
+    const int streams = max(1, min(nbatch, sc.sm_count / nsc));
+    const int grid = streams * nsc;
     const size_t smem = dense_smem_bytes(cps * FS_CHUNK, W, v.d.S, FT);
-    cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nslice, st);
+    cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nsc, st);
     // one slice: the scoring kernel writes the placement records itself (no key array, no decode launch)
-    fs_placement* direct = nslice == 1 ? out : nullptr;
+    fs_placement* direct = nsc == 1 ? out : nullptr;
     if (!direct) cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-#define FS_LAUNCH_DENSE(NP, VC, ST) \
-  place_dense_kernel<NP, VC, ST><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats, direct)
+#define FS_LAUNCH_DENSE(NP, VC, ST, CL) \
+  place_dense_kernel<NP, VC, ST, CL><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, ncb, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats, direct)
     const bool vec = FT == 64 && (v.d.F & 1) == 0;
-    if (FT == 32)  { if (sc.count_work) FS_LAUNCH_DENSE(1, false, true); else FS_LAUNCH_DENSE(1, false, false); }
-    else if (vec)  { if (sc.count_work) FS_LAUNCH_DENSE(2, true, true);  else FS_LAUNCH_DENSE(2, true, false); }
-    else           { if (sc.count_work) FS_LAUNCH_DENSE(2, false, true); else FS_LAUNCH_DENSE(2, false, false); }
+    if (FT == 32)      { if (sc.count_work) FS_LAUNCH_DENSE(1, false, true, false); else FS_LAUNCH_DENSE(1, false, false, false); }
+    else if (ncb == 1) {
+      if (vec) { if (sc.count_work) FS_LAUNCH_DENSE(2, true, true, false);  else FS_LAUNCH_DENSE(2, true, false, false); }
+      else     { if (sc.count_work) FS_LAUNCH_DENSE(2, false, true, false); else FS_LAUNCH_DENSE(2, false, false, false); }
+    } else {
+      if (vec) { if (sc.count_work) FS_LAUNCH_DENSE(2, true, true, true);  else FS_LAUNCH_DENSE(2, true, false, true); }
+      else     { if (sc.count_work) FS_LAUNCH_DENSE(2, false, true, true); else FS_LAUNCH_DENSE(2, false, false, true); }
+    }
 #undef FS_LAUNCH_DENSE
     ++launches;
     fs_tm_end(tm, FS_T_PLACE_SCORE, st);

@@ -138,6 +138,7 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     const unsigned m = __ballot_sync(0xffffffffu, ok0);
     if (f_floor < 0 && m) f_floor = base + __ffs(m) - 1;
   }
+  for (int phi = (d.F + 31) / 32 * 32 + lane; phi < v.FT; phi += 32) gA0[(size_t)k * v.FT + phi] = FS_INF;   // stride padding
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
   if (lane == 0) {

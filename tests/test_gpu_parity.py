@@ -724,12 +724,34 @@ def test_dense_scoring_up_to_32_shares(ctx, S):
         cmp.assert_placement_equal(got, oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests, nthreads=16))
 
 
+@pytest.mark.parametrize("F", [65, 96, 100, 128, 191, 256])
+def test_dense_scoring_more_than_64_frequencies(ctx, F):
+    """F > 64: the tiled kernel scores column blocks of 64 frequencies and merges them by key."""
+    for mode, (K, S) in enumerate([(200, 16), (1500, 7), (40, 32)]):
+        cl = synth.make_custom(seed=1800 + F + mode, K=K, M=6, F=F, S=S, B=20, R=500, lo=1, hi=4)
+        if mode == 1:
+            cl.requests["slo_ttft_ms"] *= 3.0; cl.models["load_ms"] *= 0.1
+        if mode == 2:
+            cl = U.tie_heavy(cl, F)
+        ctx.load_cluster(cl)
+        ctx.set_work_stats(True)
+        got = ctx.place_batch(cl.requests)
+        stats = ctx.last_place_stats()
+        ctx.set_work_stats(False)
+        assert stats["chunks_tested"] + stats["warm_pairs_tested"] > 0     # the tiled kernel ran
+        ref = oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests, nthreads=16)
+        cmp.assert_placement_equal(got, ref)
+        cmp.assert_placement_equal(ctx.place_batch(cl.requests), ref)        # the non-counting instantiation
+        if F >= 128 and mode < 2:                             # winners beyond the first column block do occur
+            assert (got["gpu"] >= 0).sum() > 50 and got["phi"].max() >= 64
+
+
 # ---- randomised sweep: dims, load shapes and SLO regimes, every entry point of the hot path ----------
 @pytest.mark.parametrize("block", range(4))
 def test_random_clusters_all_entry_points(ctx, block):
     for seed in range(block * 30, block * 30 + 30):
         st = synth.Stream(seed, "fuzz")
-        K = int(st.randint(1, 1, 400)[0]); M = int(st.randint(1, 1, 12)[0]); F = int(st.randint(1, 1, 64)[0])
+        K = int(st.randint(1, 1, 400)[0]); M = int(st.randint(1, 1, 12)[0]); F = int(st.randint(1, 1, [64, 64, 160][seed % 3])[0])
         S = int(st.randint(1, 1, 32)[0]); B = int(st.randint(1, 1, 48)[0]); R = int(st.randint(1, 1, 700)[0])
         cl = synth.make_custom(seed=5000 + seed, K=K, M=M, F=F, S=S, B=B, R=R, lo=1, hi=4)
         mode = seed % 5
