@@ -25,17 +25,49 @@ __global__ void __launch_bounds__(128) consol_agg_kernel(FsView v, int S_eff,
   const int n = v.ginfo[g].n_res;
   const fs_gpu_state& st = v.states[g];
   unsigned long long key = FS_KEY_NONE;
+  // per tenant, independent of (phi, sigma): plane offsets, round counts (the divisions once), deadlines
+  size_t o0[FS_RMAX], o1[FS_RMAX]; float r0[FS_RMAX], r1[FS_RMAX], slo0[FS_RMAX], slo1[FS_RMAX];
+  bool has0[FS_RMAX], has1[FS_RMAX];
+#pragma unroll
+  for (int i = 0; i < FS_RMAX; ++i) {
+    o0[i] = o1[i] = 0; r0[i] = r1[i] = 0.f; slo0[i] = slo1[i] = 0.f; has0[i] = has1[i] = false;
+    if (i < n) {
+      const fs_tenant& t = st.t[i];
+      has0[i] = t.q[0] > 0; has1[i] = t.q[1] > 0; slo0[i] = t.slo_ms[0]; slo1[i] = t.slo_ms[1];
+      o0[i] = fs_plane(d, t.model, 0, t.beta[0]); o1[i] = fs_plane(d, t.model, 1, t.beta[1]);
+      r0[i] = __uint2float_rn(fs_ceil_div(t.q[0], t.beta[0] + 1u));
+      r1[i] = __uint2float_rn(fs_ceil_div(t.q[1], t.beta[1] + 1u));
+    }
+  }
   for (int phi = lane; phi < d.F; phi += 32) {
     int nd = 0; float e = 0.0f; bool all = n >= 1;
-    for (int i = 0; i < n && all; ++i) {
-      int smin = -1; float ei = FS_INF;
-      for (int sg = 0; sg < d.S; ++sg) {
-        const TenantE te = tenant_eval(v, st.t[i], phi, sg, false);
-        if (te.ok) { smin = sg; ei = te.e; break; }
+#pragma unroll
+    for (int i = 0; i < FS_RMAX; ++i) {
+      if (i < n && all) {
+        // lowest feasible share of tenant i at phi: four shares' table entries are requested together
+        // (one memory latency per four shares instead of one per share), then tested in order
+        int smin = -1; float ei = FS_INF;
+        for (int sg0 = 0; sg0 < d.S && smin < 0; sg0 += 4) {
+          float l0[4], p0[4], l1[4], p1[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const size_t o = (size_t)min(sg0 + u, d.S - 1) * d.F + phi;
+            l0[u] = v.latT[o0[i] + o]; p0[u] = v.powT[o0[i] + o];
+            l1[u] = v.latT[o1[i] + o]; p1[u] = v.powT[o1[i] + o];
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (smin < 0 && sg0 + u < d.S) {
+              bool ok = true; float e0 = 0.0f, e1 = 0.0f;
+              if (has0[i]) { const FsSlot sl = fs_slot_f(0, l0[u], p0[u], r0[i], 0.0f, slo0[i]); ok = sl.ok; e0 = sl.e; }
+              if (has1[i]) { const FsSlot sl = fs_slot_f(1, l1[u], p1[u], r1[i], 0.0f, slo1[i]); ok = ok && sl.ok; e1 = sl.e; }
+              if (ok) { smin = sg0 + u; ei = __fadd_rn(e0, e1); }
+            }
+          }
+        }
+        if (smin < 0) all = false;
+        else { nd += smin + 1; e = (i == 0) ? ei : __fadd_rn(e, ei); }
       }
-      if (smin < 0) { all = false; break; }
-      nd += smin + 1;
-      e = (i == 0) ? ei : __fadd_rn(e, ei);
     }
     need[(size_t)phi * v.K + g] = all ? (uint8_t)nd : (uint8_t)FS_NEED_INF;
     E[(size_t)phi * v.K + g] = all ? e : FS_INF;
