@@ -27,7 +27,8 @@
  *   - One context per host thread; calls on one context are not re-entrant.  Calls that do not depend on
  *     each other's outputs (fs_place_batch / fs_dispatch vs fs_local_config vs fs_consolidate, all after
  *     fs_set_gpu_state) may be issued on different streams by that thread; the caller orders the streams.
- *   - FS_DEVICE calls never synchronise and do not allocate once a call of the same sizes has run, so a
+ *     fs_place_batch, fs_dispatch and fs_dispatch_commit share staging buffers: one of them at a time.
+ *   - FS_DEVICE and FS_HOST_PINNED calls never synchronise and do not allocate once a call of the same sizes has run, so a
  *     sequence of them can be captured into a CUDA graph (with fs_set_timing off) and replayed.
  *   - There is no CPU fallback: every entry point runs CUDA kernels on the context's device.
  */
