@@ -398,6 +398,17 @@ def test_dispatch_full_size(ctx):
     assert set(np.unique(got["f_req"]).tolist()) >= {1, 2, 3}
 
 
+@pytest.mark.parametrize("R", [1, 19, 2959, 11840, 11841, 14799, 20000])
+def test_request_counts_around_the_static_dynamic_boundary(ctx, R):
+    """The scoring kernel assigns all but the last four rounds of requests statically (148 blocks x 20 warps
+    = 2,960 requests per round) and hands out the tail dynamically: every request exactly once at any R."""
+    cl = synth.make_cluster("rack")
+    reqs = synth.make_requests(4242 + R, R, cl.M)
+    ctx.load_cluster(cl)
+    got = ctx.place_batch(reqs)
+    cmp.assert_placement_equal(got, oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, reqs, nthreads=16))
+
+
 def test_device_requests_at_a_4_byte_aligned_address(ctx):
     """fs_request has 4-byte alignment: a device array that starts at any multiple of 4 must work
     (the scoring kernel prefetches requests with 16-byte asynchronous copies only when it can)."""
