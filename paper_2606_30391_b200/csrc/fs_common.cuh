@@ -59,7 +59,8 @@ struct __align__(16) FsWarmItem {
   float t_avail_ms, mem_free_mb, e_cur;
   float a_min;              // min over phi of A[k][1+j][phi]
   float l1_min, p1_min;     // min of LAT / POW of plane (model, decode, br1) over sigma < sm_free, all phi
-  uint32_t _pad[2];
+  int32_t f_cur;            // F_curr of the GPU
+  uint32_t _pad;
 };
 static_assert(sizeof(FsWarmItem) == 48, "FsWarmItem layout");
 #define FS_CHUNK 32         // GPUs per staged chunk (one per lane in the eligibility pass)

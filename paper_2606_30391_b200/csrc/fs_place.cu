@@ -784,10 +784,11 @@ __device__ __forceinline__ DispPair disp_pair(const FsView& v, const ReqCtx& c, 
 // warm pair from the per-model list (phi < 0: the GPU's F_curr)
 __device__ __forceinline__ DispPair disp_warm(const FsView& v, const ReqCtx& c, const FsWarmItem& it, int phi) {
   DispPair r; r.ok = false; r.e = FS_INF;
-  const FsGpuInfo gi = v.ginfo[it.k];
-  const PairCtx p = make_pair(v, c, gi);
-  if (!p.ok) return r;
-  const OwnEval ev = own_eval_planes(v, c, p.br1, p.rounds1, p.wait, p.smf - 1, phi < 0 ? gi.f_cur : phi);
+  // the item carries what make_pair would read from the GPU's summary (listed items have n_res >= 1 and host
+  // the model in slot j): no dependent load before the table entries are requested
+  if (it.sm_free < 1 || it.br1 < 0 || !(c.mem <= it.mem_free_mb)) return r;
+  const OwnEval ev = own_eval_planes(v, c, it.br1, fs_ceil_div(c.O, (uint32_t)it.br1 + 1u), it.t_avail_ms,
+                                     it.sm_free - 1, phi < 0 ? it.f_cur : phi);
   r.ok = ev.ok; r.e = ev.e;
   return r;
 }

@@ -292,7 +292,7 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
     FsWarmItem it;
     it.k = k; it.j = i; it.br1 = br1; it.sm_free = gi.sm_free;
     it.t_avail_ms = gi.t_avail_ms; it.mem_free_mb = gi.mem_free_mb; it.e_cur = gi.e_cur;
-    it.a_min = a_min; it.l1_min = l1; it.p1_min = p1; it._pad[0] = it._pad[1] = 0;
+    it.a_min = a_min; it.l1_min = l1; it.p1_min = p1; it.f_cur = gi.f_cur; it._pad = 0;
     items[off[m] + atomicAdd(&cursor[m], 1)] = it;
   }
 }
