@@ -485,3 +485,153 @@ def test_consolidate_margin_delta():
     assert np.all(_consol(cl)["dst"] == -1)
     cl.states["t"]["mem_used_mb"][...] = 38000.0
     assert np.all(_consol(cl)["dst"] >= 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# Co-resident coupling BY HAND (P:44, P:127, P:265 shared operating point; DESIGN s4): a busy tenant of the
+# request's model (bump: its decode batch grows by the new sequence) and a busy tenant of another model.
+# Every number below is written out; none comes from fs_brute or from the oracle.
+def _coupled_cluster(beta1=0, q1=4, tenant0_tbt=1e9):
+    M, F, S, B = 2, 2, 4, 3
+    lat = np.full((M, 2, F, S, B), 1000.0, dtype=np.float32)
+    pw = np.full((M, 2, F, S, B), 1000.0, dtype=np.float32)
+    # model 0, decode, share sigma=0 (tenant 0's share; also the request's grant sigma=0)
+    lat[0, 1, 0, 0, 0], pw[0, 1, 0, 0, 0] = 10.0, 100.0     # phi 0, batch 1
+    lat[0, 1, 1, 0, 0], pw[0, 1, 1, 0, 0] = 5.0, 300.0      # phi 1, batch 1
+    lat[0, 1, 0, 0, 1], pw[0, 1, 0, 0, 1] = 12.0, 110.0     # phi 0, batch 2 (after the bump)
+    lat[0, 1, 1, 0, 1], pw[0, 1, 1, 0, 1] = 6.0, 320.0      # phi 1, batch 2
+    # model 0, decode, grant sigma=1
+    lat[0, 1, 0, 1, 1], pw[0, 1, 0, 1, 1] = 8.0, 120.0
+    lat[0, 1, 1, 1, 1], pw[0, 1, 1, 1, 1] = 4.0, 330.0
+    lat[0, 1, 0, 1, 0], pw[0, 1, 0, 1, 0] = 7.0, 105.0      # batch 1 at sigma=1 (the no-bump twin)
+    lat[0, 1, 1, 1, 0], pw[0, 1, 1, 1, 0] = 3.5, 310.0
+    # model 0, prefill at batch bucket min(L,B)-1 = 1
+    lat[0, 0, 0, 0, 1], pw[0, 0, 0, 0, 1] = 30.0, 100.0
+    lat[0, 0, 1, 0, 1], pw[0, 0, 1, 0, 1] = 15.0, 250.0
+    lat[0, 0, 0, 1, 1], pw[0, 0, 0, 1, 1] = 18.0, 120.0
+    lat[0, 0, 1, 1, 1], pw[0, 0, 1, 1, 1] = 9.0, 260.0
+    # model 1 (the other tenant), prefill, its share sigma=0, batch bucket 1
+    lat[1, 0, 0, 0, 1], pw[1, 0, 0, 0, 1] = 20.0, 50.0
+    lat[1, 0, 1, 0, 1], pw[1, 0, 1, 0, 1] = 10.0, 200.0
+    tenants = [dict(model=0, sigma=0, beta=(0, beta1), q=(0, q1), slo=(1e9, tenant0_tbt)),
+               dict(model=1, sigma=0, beta=(1, 0), q=(6, 0), slo=(1e9, 1e9))]
+    states = mk_states([mk_state(f_cur=1, t_avail=7.0, tenants=tenants)])
+    reqs = mk_requests([dict(model=0, L=2, o_pred=3)])       # O = ceil(1.05*3) = 4
+    return cluster_from(lat, pw, mk_models(M), states, reqs)
+
+
+def test_place_busy_coresidents_bump_and_negative_marginal_energy_by_hand():
+    """GPU now (F_curr = phi 1, nobody bumped): tenant 0 decodes 4 tokens one by one, 4 x 5 ms x 300 W = 6000 mJ;
+    tenant 1 prefills 6 tokens in batches of 2, 3 x 10 ms x 200 W = 6000 mJ: Ecur = 12000 mJ.
+    After the request joins tenant 0's decode batch (batch 2: 2 rounds) the co-residents cost
+      phi 0: 2 x 12 x 110 + 3 x 20 x 50 = 2640 + 3000 = 5640      phi 1: 2 x 6 x 320 + 3 x 10 x 200 = 9840
+    and the request itself (prefill 1 round of 2 tokens; decode O = 4 in its tenant's batch 2: 2 rounds)
+      (sigma 0, phi 0): 30 x 100 + 2 x 12 x 110 = 5640            (sigma 0, phi 1): 15 x 250 + 2 x 6 x 320 = 7590
+      (sigma 1, phi 0): 18 x 120 + 2 x 8 x 120 = 4080             (sigma 1, phi 1): 9 x 260 + 2 x 4 x 330 = 4980
+    dE = (A + e_r) - Ecur:  -720, 5430, -2280, 2820  ->  (sigma 1, phi 0) with a NEGATIVE marginal energy."""
+    cl = _coupled_cluster()
+    o = _place(cl)[0]
+    assert (o["gpu"], o["sigma"], o["phi"], o["beta"], o["f_req"]) == (0, 1, 0, 1, 0)
+    assert o["energy_mj"] == f32(-2280.0) and o["flat"] == (0 * 4 + 1) * 2 + 0
+    assert o["ttft_ms"] == f32(25.0) and o["tbt_ms"] == f32(8.0)        # 7 + 18; LAT1 at the chosen point
+    # request TBT SLO 7 ms: LAT1 = 12 / 8 at phi 0 miss it, 6 / 4 at phi 1 meet it -> (sigma 1, phi 1), 2820
+    cl.requests["slo_tbt_ms"] = 7.0
+    o = _place(cl)[0]
+    assert (o["sigma"], o["phi"], o["f_req"]) == (1, 1, 1) and o["energy_mj"] == f32(2820.0)
+    # request TTFT SLO 24 ms: 7+30, 7+18 miss, 7+15, 7+9 meet -> phi 1 again, (sigma 1) 2820
+    cl.requests["slo_tbt_ms"] = 1e9
+    cl.requests["slo_ttft_ms"] = 24.0
+    o = _place(cl)[0]
+    assert (o["sigma"], o["phi"]) == (1, 1) and o["ttft_ms"] == f32(16.0)
+    # the bump also decides the co-resident's own deadline: tenant 0 must keep TBT <= 11 ms; alone it runs at
+    # 10 ms (phi 0) but in batch 2 at 12 ms -> phi 0 is out for everyone (shared operating point, P:265)
+    cl = _coupled_cluster(tenant0_tbt=11.0)
+    o = _place(cl)[0]
+    assert (o["sigma"], o["phi"], o["f_req"]) == (1, 1, 1) and o["energy_mj"] == f32(2820.0)
+
+
+def test_place_bump_past_the_last_batch_level_drops_the_gpu():
+    """beta_1 = B-1: one more sequence does not fit the profiled batch range -> not a candidate (DESIGN s4)."""
+    cl = _coupled_cluster(beta1=2)
+    o = _place(cl)[0]
+    assert o["gpu"] == -1 and np.isinf(o["energy_mj"])
+
+
+def test_place_idle_decode_queue_means_no_bump():
+    """q_1 = 0: tenant 0 costs nothing now or later, the request opens batch 1 (bucket 0, 4 rounds):
+      Ecur = 0 + 6000;  A = (0 + 3000, 0 + 6000)
+      (0,0): 3000 + 4x10x100 = 7000 -> +3000 - 6000 = 4000      (0,1): 3750 + 4x5x300 = 9750 -> 9750
+      (1,0): 2160 + 4x7x105 = 5100 -> 2100                      (1,1): 2340 + 4x3.5x310 = 6680 -> 6680"""
+    cl = _coupled_cluster(q1=0)
+    o = _place(cl)[0]
+    assert (o["sigma"], o["phi"], o["beta"]) == (1, 0, 0)
+    assert o["energy_mj"] == f32(2100.0) and o["tbt_ms"] == f32(7.0)
+
+
+def test_place_cold_start_pays_the_weight_load():
+    """A GPU that does not host the model adds load_ms to the request's wait: 10 + 100 + 50 = 160 ms."""
+    M, F, S, B = 2, 1, 2, 1
+    lat = np.ones((M, 2, F, S, B), dtype=np.float32)
+    pw = np.ones_like(lat)
+    lat[1, 0, 0, 0, 0], pw[1, 0, 0, 0, 0] = 50.0, 10.0       # request's prefill on one share unit: 50 ms, 500 mJ
+    idle = dict(sigma=0, q=(0, 0))
+    states = mk_states([mk_state(t_avail=10.0, tenants=[dict(idle, model=0)]),    # cold for model 1
+                        mk_state(t_avail=130.0, tenants=[dict(idle, model=1)])])  # warm, but late: 130 + 50
+    reqs = mk_requests([dict(model=1, L=1, o_pred=0, ttft=160.0)])
+    cl = cluster_from(lat, pw, mk_models(M, load_ms=100.0), states, reqs)
+    o = _place(cl)[0]
+    assert o["gpu"] == 0 and o["ttft_ms"] == f32(160.0) and o["energy_mj"] == f32(500.0)
+    cl.requests["slo_ttft_ms"] = 159.0                        # would pass without the load (60 ms): it must not
+    assert _place(cl)[0]["gpu"] == -1
+    cl.requests["slo_ttft_ms"] = 180.0                        # both feasible, equal energy: lowest flat index
+    assert _place(cl)[0]["gpu"] == 0
+    cl.states[0]["mem_free_mb"] = -1.0
+    o = _place(cl)[0]
+    assert o["gpu"] == 1 and o["ttft_ms"] == f32(180.0)       # warm: no load added
+
+
+# ---------------------------------------------------------------------------------------------
+# FS_OBJ_POWER by hand on a 2 x 2 x 3 table (F, S, B) ("minimum-power feasible config", configs[3]; P:11)
+def _power_cluster():
+    F, S, B = 2, 2, 3
+    lat = np.zeros((1, 2, F, S, B), dtype=np.float32)
+    pw = np.zeros_like(lat)
+    # prefill queue of 3 tokens (rounds 3, 2, 1 at batch 1, 2, 3), TTFT slack 100 ms
+    lat[0, 0, 0, 0], pw[0, 0, 0, 0] = (40, 60, 120), (50, 45, 40)      # 120 ms at every batch: misses
+    lat[0, 0, 0, 1], pw[0, 0, 0, 1] = (30, 45, 98), (70, 66, 62)       # 90 / 90 / 98 ms
+    lat[0, 0, 1, 0], pw[0, 0, 1, 0] = (20, 30, 70), (120, 110, 130)    # 60 / 60 / 70 ms
+    lat[0, 0, 1, 1], pw[0, 0, 1, 1] = (10, 15, 35), (200, 190, 210)
+    # decode queue of 2 tokens (rounds 2, 1 at batch 1, 2; batch 3 > q is not a candidate), TBT slack 25 ms
+    lat[0, 1, 0, 0], pw[0, 1, 0, 0] = (20, 24, 1), (30, 35, 1)
+    lat[0, 1, 0, 1], pw[0, 1, 0, 1] = (15, 26, 1), (40, 20, 1)         # batch 2 is cheaper but misses 25 ms
+    lat[0, 1, 1, 0], pw[0, 1, 1, 0] = (10, 12, 1), (90, 80, 1)
+    lat[0, 1, 1, 1], pw[0, 1, 1, 1] = (5, 6, 1), (150, 140, 1)
+    states = mk_states([mk_state(tenants=[dict(model=0, sigma=0, q=(3, 2), slo=(100.0, 25.0))])])
+    return cluster_from(lat, pw, mk_models(1), states, mk_requests([]))
+
+
+def test_local_power_objective_by_hand():
+    cl = _power_cluster()
+    # minimum-SM rule, POWER: phi 0 needs share 2/2 (share 1/2 misses TTFT): 62 W (batch 3) + 40 W (batch 1) = 102 W;
+    # phi 1 runs on share 1/2: 110 W (batch 2) + 80 W (batch 2) = 190 W.  -> phi 0, 102 W, beta (2, 0);
+    # energy there = 98 x 62 + 2 x 15 x 40 = 6076 + 1200 = 7276 mJ
+    o = oracle.local_config(cl.lat, cl.pow, cl.states, oracle.OBJ_POWER | oracle.SPLIT_MINSM)[0]
+    assert (o["phi"], o["f_req"], o["sigma"][0]) == (0, 0, 1) and tuple(o["beta"][0]) == (2, 0)
+    assert o["cost"] == f32(102.0) and o["power_w"] == f32(102.0) and o["energy_mj"] == f32(7276.0)
+    # ENERGY on the same input picks batch 2 for the prefill: 2 x 45 x 66 = 5940 (< 6300, 6076) + 1200 = 7140 mJ
+    # against phi 1: min(7200, 6600, 9100) + min(1800, 960) = 7560 mJ; power there 66 + 40 = 106 W
+    o = oracle.local_config(cl.lat, cl.pow, cl.states, oracle.OBJ_ENERGY | oracle.SPLIT_MINSM)[0]
+    assert (o["phi"], o["sigma"][0]) == (0, 1) and tuple(o["beta"][0]) == (1, 0)
+    assert o["cost"] == f32(7140.0) and o["energy_mj"] == f32(7140.0) and o["power_w"] == f32(106.0)
+    # all splits summing to S: one tenant takes both units; phi 1 there costs 190 + 140 = 330 W -> phi 0 again
+    o = oracle.local_config(cl.lat, cl.pow, cl.states, oracle.OBJ_POWER | oracle.SPLIT_EXHAUSTIVE)[0]
+    assert (o["phi"], o["sigma"][0], o["flat"]) == (0, 1, 0) and o["cost"] == f32(102.0)
+    # tighten the TTFT slack to 95 ms: batch 3 at phi 0 (98 ms) drops out -> 66 W (batch 2) + 40 W = 106 W
+    cl.states[0]["t"][0]["slo_ms"][0] = 95.0
+    o = oracle.local_config(cl.lat, cl.pow, cl.states, oracle.OBJ_POWER | oracle.SPLIT_MINSM)[0]
+    assert o["cost"] == f32(106.0) and tuple(o["beta"][0]) == (1, 0)
+    # 85 ms: phi 0 is infeasible at every share and batch -> phi 1 on share 1/2, 190 W; f_req = 1
+    cl.states[0]["t"][0]["slo_ms"][0] = 85.0
+    o = oracle.local_config(cl.lat, cl.pow, cl.states, oracle.OBJ_POWER | oracle.SPLIT_MINSM)[0]
+    assert (o["phi"], o["f_req"], o["sigma"][0]) == (1, 1, 0) and o["cost"] == f32(190.0)
+    assert tuple(o["beta"][0]) == (1, 1) and o["energy_mj"] == f32(2 * 30 * 110 + 12 * 80)
