@@ -32,30 +32,30 @@ __global__ void __launch_bounds__(128) llm_profile_kernel(FsView v, int n, const
   const uint32_t n0 = L < (uint32_t)d.B ? L : (uint32_t)d.B;
   const int br0 = n0 ? (int)n0 - 1 : 0;
   const uint32_t rounds0 = n0 ? fs_ceil_div(L, n0) : 0u;
-  const float* l0 = v.latT + fs_plane(d, m, 0, br0); const float* p0 = v.powT + fs_plane(d, m, 0, br0);
-  const float* l1 = v.latT + fs_plane(d, m, 1, 0);   const float* p1 = v.powT + fs_plane(d, m, 1, 0);
+  const float2* lp0 = v.lpT + fs_plane(d, m, 0, br0);    // {LAT, POW} planes of the prefill bucket and of decode bucket 0
+  const float2* lp1 = v.lpT + fs_plane(d, m, 1, 0);
   // ---- preferred configuration per phase --------------------------------------------------------
   unsigned long long kp = FS_KEY_NONE, kd = FS_KEY_NONE;
   for (int x = lane; x < d.S * d.F; x += 32) {          // x = sigma*F + phi (plane order)
     const int sg = x / d.F, phi = x % d.F;
     const uint32_t flat = (uint32_t)(phi * d.S + sg);
     FsSlot a; a.ok = true; a.t = 0.f; a.e = 0.f;
-    if (L > 0) a = fs_slot(0, l0[x], p0[x], rounds0, 0.0f, l.slo_ttft_ms);
+    if (L > 0) a = fs_slot(0, lp0[x].x, lp0[x].y, rounds0, 0.0f, l.slo_ttft_ms);
     if (a.ok && a.e < FS_INF) { const unsigned long long k = fs_make_key(a.e, flat); kp = k < kp ? k : kp; }
     FsSlot b; b.ok = true; b.t = 0.f; b.e = 0.f;
-    if (O > 0) b = fs_slot(1, l1[x], p1[x], O, 0.0f, l.slo_tbt_ms);
+    if (O > 0) b = fs_slot(1, lp1[x].x, lp1[x].y, O, 0.0f, l.slo_tbt_ms);
     if (b.ok && b.e < FS_INF) { const unsigned long long k = fs_make_key(b.e, flat); kd = k < kd ? k : kd; }
   }
   kp = fs_warp_min_key(kp); kd = fs_warp_min_key(kd);
   if (kp != FS_KEY_NONE) {
     const int flat = (int)(uint32_t)kp, phi = flat / d.S, sg = flat % d.S, x = sg * d.F + phi;
     o.sigma_p = (int16_t)sg; o.phi_p = (int16_t)phi;
-    o.t_p_ms = L ? __fmul_rn(__uint2float_rn(rounds0), l0[x]) : 0.0f; o.p_p_w = L ? p0[x] : 0.0f;
+    o.t_p_ms = L ? __fmul_rn(__uint2float_rn(rounds0), lp0[x].x) : 0.0f; o.p_p_w = L ? lp0[x].y : 0.0f;
   }
   if (kd != FS_KEY_NONE) {
     const int flat = (int)(uint32_t)kd, phi = flat / d.S, sg = flat % d.S, x = sg * d.F + phi;
     o.sigma_d = (int16_t)sg; o.phi_d = (int16_t)phi;
-    o.t_d_ms = O ? __fmul_rn(__uint2float_rn(O), l1[x]) : 0.0f; o.p_d_w = O ? p1[x] : 0.0f;
+    o.t_d_ms = O ? __fmul_rn(__uint2float_rn(O), lp1[x].x) : 0.0f; o.p_d_w = O ? lp1[x].y : 0.0f;
   }
   if (kp != FS_KEY_NONE && kd != FS_KEY_NONE) {
     // ---- Eq. 8, l.S, l.F, Little's law -----------------------------------------------------------
@@ -70,17 +70,17 @@ __global__ void __launch_bounds__(128) llm_profile_kernel(FsView v, int n, const
     for (int phi = lane; phi < d.F; phi += 32) {
       const int x = (need - 1) * d.F + phi;
       FsSlot a; a.ok = true; a.t = 0.f; a.e = 0.f;
-      if (L > 0) a = fs_slot(0, l0[x], p0[x], rounds0, 0.0f, l.slo_ttft_ms);
+      if (L > 0) a = fs_slot(0, lp0[x].x, lp0[x].y, rounds0, 0.0f, l.slo_ttft_ms);
       FsSlot b; b.ok = true; b.t = 0.f; b.e = 0.f;
-      if (O > 0) b = fs_slot(1, l1[x], p1[x], O, 0.0f, l.slo_tbt_ms);
+      if (O > 0) b = fs_slot(1, lp1[x].x, lp1[x].y, O, 0.0f, l.slo_tbt_ms);
       const float e = __fadd_rn(a.e, b.e);
       if (a.ok && b.ok && e < FS_INF) { const unsigned long long k = fs_make_key(e, (uint32_t)phi); kl = k < kl ? k : kl; }
     }
     kl = fs_warp_min_key(kl);
     if (kl != FS_KEY_NONE) {
       const int phi = (int)(uint32_t)kl, x = (need - 1) * d.F + phi;
-      const float tp = L ? __fmul_rn(__uint2float_rn(rounds0), l0[x]) : 0.0f;
-      const float td = O ? __fmul_rn(__uint2float_rn(O), l1[x]) : 0.0f;
+      const float tp = L ? __fmul_rn(__uint2float_rn(rounds0), lp0[x].x) : 0.0f;
+      const float td = O ? __fmul_rn(__uint2float_rn(O), lp1[x].x) : 0.0f;
       o.phi_l = (int16_t)phi; o.t_l_ms = __fadd_rn(tp, td); o.e_l_mj = fs_unorderable((uint32_t)(kl >> 32));
       const float nconc = __fmul_rn(l.lambda_rps, __fdiv_rn(o.t_l_ms, 1000.0f));
       const float kvsize = __fmul_rn(__uint2float_rn(L + O), v.models[m].kv_mb_per_token);

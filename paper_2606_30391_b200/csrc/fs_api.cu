@@ -16,7 +16,7 @@ struct fs_ctx {
   fs_params prm{0, 0, 0, 0};
   bool have_prof = false, have_state = false, place_ready = false;
   // profiles
-  float *lat = nullptr, *pow = nullptr, *latT = nullptr, *powT = nullptr, *freq = nullptr; float2* dmin = nullptr; size_t dmin_cap = 0;
+  float *lat = nullptr, *pow = nullptr, *freq = nullptr; float2* lpT = nullptr; FsPlaneMin* pmin = nullptr; size_t pmin_cap = 0;
   fs_model_info* models = nullptr;
   size_t table_cap = 0; int m_cap = 0, f_cap = 0;
   uint32_t *comp = nullptr, *comp_n = nullptr; int ns_stride = 1; size_t comp_cap = 0;
@@ -46,7 +46,7 @@ struct fs_ctx {
   int* flag_host = nullptr; int* flag_dev = nullptr;
   uint64_t launches = 0; int last_cuda = 0;
   bool timing = false; bool have_events = false; FsTimers tm{};
-  int sm_count = 148; bool force_generic = false, count_work = false;
+  int sm_count = 148; bool count_work = false;
 };
 
 namespace {
@@ -85,7 +85,7 @@ int check_kernel(fs_ctx* c) {
 FsView view_of(const fs_ctx* c) {
   FsView v;
   v.d = FsDimsDev{c->d.M, c->d.F, c->d.S, c->d.B};
-  v.lat = c->lat; v.pow = c->pow; v.latT = c->latT; v.powT = c->powT; v.dmin = c->dmin; v.models = c->models;
+  v.lat = c->lat; v.pow = c->pow; v.lpT = c->lpT; v.pmin = c->pmin; v.models = c->models;
   v.K = c->K; v.states = c->states; v.ginfo = c->ginfo; v.gA = c->gA; v.flag = c->flag_dev;
   v.grec = c->grec; v.gA0 = c->gA0; v.Kpad = c->Kpad; v.FT = c->FT; v.gsort = c->gsort; v.dsuf = c->dsuf;
   return v;
@@ -160,7 +160,6 @@ int fs_create(fs_ctx** out, int cuda_device) {
   fsk_local_smem_attr();
   fsk_place_smem_attr();
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
-  if (const char* e = getenv("FS_FORCE_GENERIC")) c->force_generic = e[0] == '1';
   if (const char* e = getenv("FS_ZERO_COPY")) c->zero_copy = e[0] != '0';
   *out = c;
   return FS_OK;
@@ -170,7 +169,7 @@ int fs_destroy(fs_ctx* c) {
   if (!c) return FS_ERR_ARG;
   cudaSetDevice(c->dev);
   cudaDeviceSynchronize();
-  void* ptrs[] = {c->lat, c->pow, c->latT, c->powT, c->dmin, c->freq, c->models, c->comp, c->comp_n, c->states,
+  void* ptrs[] = {c->lat, c->pow, c->lpT, c->pmin, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf, c->pl_buf};
@@ -199,7 +198,7 @@ int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const flo
   const size_t n = (size_t)dims->M * 2 * dims->F * dims->S * dims->B;
   if (n > c->table_cap) {
     FS_TRY(grow(c, c->lat, n)); FS_TRY(grow(c, c->pow, n));
-    FS_TRY(grow(c, c->latT, n)); FS_TRY(grow(c, c->powT, n));
+    FS_TRY(grow(c, c->lpT, n));
     c->table_cap = n;
   }
   if (dims->M > c->m_cap) { FS_TRY(grow(c, c->models, (size_t)dims->M)); c->m_cap = dims->M; }
@@ -220,9 +219,9 @@ int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const flo
   FS_CUDA(c, cudaMemcpyAsync(c->comp_n, comp_n, sizeof(comp_n), cudaMemcpyHostToDevice, st));
   FS_CUDA(c, cudaStreamSynchronize(st));
   c->ns_stride = stride;
-  { const size_t nd = (size_t)dims->M * dims->B * dims->S;
-    if (nd > c->dmin_cap) { FS_TRY(grow(c, c->dmin, nd)); c->dmin_cap = nd; } }
-  c->launches += fsk_build_planes(c->lat, c->pow, c->latT, c->powT, c->dmin,
+  { const size_t nd = (size_t)dims->M * 2 * dims->B * dims->S;
+    if (nd > c->pmin_cap) { FS_TRY(grow(c, c->pmin, nd)); c->pmin_cap = nd; } }
+  c->launches += fsk_build_planes(c->lat, c->pow, c->lpT, c->pmin,
                                   FsDimsDev{dims->M, dims->F, dims->S, dims->B}, c->flag_dev, st);
   FS_TRY(check_kernel(c));
   c->have_prof = true;
@@ -301,7 +300,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
     d_reqs = c->reqs_dev; d_out = c->place_dev;
   }
   FS_TRY(place_prepare(c, st));
-  FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->force_generic, c->count_work};
+  FsPlaceScratch sc{c->keys, c->stats, c->ctr, c->warm_off, c->warm_item, c->sm_count, c->count_work};
   c->launches += fsk_place(view_of(c), R, d_reqs, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (zero_copy) return pending;

@@ -50,19 +50,28 @@ struct __align__(16) FsGpuRec {
   uint32_t k;               // GPU index (the sorted copy is not in index order)
 };
 static_assert(sizeof(FsGpuRec) == 32, "FsGpuRec layout");
+// Prefix minima of one plane (model, phase, batch bucket) over shares <= s and all phi (fs_tables.cu)
+struct __align__(16) FsPlaneMin {
+  double lp;                // min of the exact product LAT*POW
+  float lmin;               // min LAT
+  float pmax;               // max POW
+};
+static_assert(sizeof(FsPlaneMin) == 16, "FsPlaneMin layout");
 // One (GPU k, tenant slot j) that hosts a model: what a request of that model needs to bound and
-// to score the WARM pair (r, k) (48 bytes; built by fs_set_gpu_state, listed per model).
+// to score the WARM pair (r, k) (64 bytes; built by fs_set_gpu_state, listed per model).
 struct __align__(16) FsWarmItem {
   int32_t k, j;
   int32_t br1;              // decode bucket the request joins (-1: past the table)
   int32_t sm_free;
   float t_avail_ms, mem_free_mb, e_cur;
   float a_min;              // min over phi of A[k][1+j][phi]
-  float l1_min, p1_min;     // min of LAT / POW of plane (model, decode, br1) over sigma < sm_free, all phi
+  double lp1;               // FsPlaneMin of plane (model, decode, br1) at share sm_free - 1
+  float l1_min, p1_max;
   int32_t f_cur;            // F_curr of the GPU
-  uint32_t _pad;
+  uint32_t magic;           // ceil(2^32 / (br1+1)) for br1 >= 1 (0: br1 == 0): rounds by multiply-high
+  uint32_t _pad[2];
 };
-static_assert(sizeof(FsWarmItem) == 48, "FsWarmItem layout");
+static_assert(sizeof(FsWarmItem) == 64, "FsWarmItem layout");
 #define FS_CHUNK 32         // GPUs per staged chunk (one per lane in the eligibility pass)
 
 struct FsDimsDev { int M, F, S, B; };
@@ -101,6 +110,25 @@ __device__ __forceinline__ unsigned long long fs_warp_min_key(unsigned long long
     k = other < k ? other : k;
   }
   return k;
+}
+
+// ceil(q / n) for q < 2^24, 1 <= n <= 256 by multiply-high: magic = ceil(2^32 / n) for n >= 2 (0 stands for
+// n == 1).  floor((q-1)/n) = umulhi(q-1, magic) exactly, because (q-1) * (magic*n - 2^32) < 2^24 * 2^8 = 2^32.
+__host__ __device__ __forceinline__ uint32_t fs_magic(uint32_t n) {
+  return n <= 1u ? 0u : (uint32_t)((0x100000000ull + n - 1u) / n);
+}
+__device__ __forceinline__ uint32_t fs_ceil_div_magic(uint32_t q, uint32_t magic) {
+  return (magic == 0u || q == 0u) ? q : __umulhi(q - 1u, magic) + 1u;
+}
+
+// A lower bound on e = fl(fl(fr*LAT)*POW) of EVERY entry of a plane prefix, fr >= 0 an integer below 2^24:
+// with u = 2^-24, eta = 2^-150 one rounding obeys fl(z) >= z(1-u) - eta for every z >= 0 (half an ulp, normal
+// or subnormal), hence e >= fr*LAT*POW*(1-u)^2 - eta*(POW+1) >= fr*lp*(1-2u) - eta*(pmax+1).  Evaluated in
+// binary64 with twice that slack and rounded down; never negative.  Exactness of the kernel's results does not
+// depend on how tight this is, only on its being a lower bound.
+__device__ __forceinline__ float fs_energy_lb(float fr, double lp, float pmax) {
+  const double x = (double)fr * lp * (1.0 - 0x1p-22) - 0x1p-149 * ((double)pmax + 1.0);
+  return x > 0.0 ? __double2float_rd(x) : 0.0f;
 }
 
 // The shared slot rule (Eq. 1; R:s11), given the two table values.

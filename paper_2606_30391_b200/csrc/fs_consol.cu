@@ -52,8 +52,8 @@ __global__ void __launch_bounds__(128) consol_agg_kernel(FsView v, int S_eff,
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const size_t o = (size_t)min(sg0 + u, d.S - 1) * d.F + phi;
-            l0[u] = v.latT[o0[i] + o]; p0[u] = v.powT[o0[i] + o];
-            l1[u] = v.latT[o1[i] + o]; p1[u] = v.powT[o1[i] + o];
+            const float2 e0 = v.lpT[o0[i] + o], e1 = v.lpT[o1[i] + o];
+            l0[u] = e0.x; p0[u] = e0.y; l1[u] = e1.x; p1[u] = e1.y;
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {

@@ -21,9 +21,8 @@ struct FsView {
   FsDimsDev d;
   const float* lat;    // [M][2][F][S][B]
   const float* pow;
-  const float* latT;   // [M][2][B][S][F]
-  const float* powT;
-  const float2* dmin;  // [M][B][S]  {min LAT, min POW} of the decode plane over shares <= s, all phi
+  const float2* lpT;   // [M][2][B][S][F]  {LAT, POW}: the plane layout
+  const FsPlaneMin* pmin;  // [M][2][B][S]  prefix minima of every plane over shares <= s, all phi
   const fs_model_info* models;
   int K;
   const fs_gpu_state* states;
@@ -39,7 +38,7 @@ struct FsView {
 };
 
 // fs_tables.cu — validate (finite, > 0) and build the plane layout
-int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, float2* dmin, FsDimsDev d,
+int fsk_build_planes(const float* lat, const float* pow, float2* lpT, FsPlaneMin* pmin, FsDimsDev d,
                      int* flag, cudaStream_t st);
 
 // fs_summary.cu — per-GPU co-resident summary: segmented max / slot-order sum
@@ -59,8 +58,7 @@ struct FsPlaceScratch {
   const int32_t* warm_off;         // [M+1]
   const FsWarmItem* witems;        // [<= 4K] items, grouped by model
   int sm_count;                    // SMs of the device (grid sizing)
-  bool force_generic;              // diagnostics: score with the generic kernel only
-  bool count_work;                 // fill `stats` (fs_set_work_stats): a second instantiation of the kernel
+  bool count_work;                 // fill `stats` (fs_set_work_stats): the same kernel with its counters switched on
 };
 int fsk_place_smem_attr();
 int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
@@ -134,12 +132,14 @@ __device__ __forceinline__ TenantE tenant_eval(const FsView& v, const fs_tenant&
   bool ok = true; float e0 = 0.0f, e1 = 0.0f;
   if (t.q[0] > 0) {
     const size_t i = fs_plane(d, t.model, 0, t.beta[0]) + (size_t)sigma * d.F + phi;
-    FsSlot s = fs_slot(0, v.latT[i], v.powT[i], fs_ceil_div(t.q[0], t.beta[0] + 1u), 0.0f, t.slo_ms[0]);
+    const float2 e = v.lpT[i];
+    FsSlot s = fs_slot(0, e.x, e.y, fs_ceil_div(t.q[0], t.beta[0] + 1u), 0.0f, t.slo_ms[0]);
     ok = ok && s.ok; e0 = s.e;
   }
   if (t.q[1] > 0) {
     const size_t i = fs_plane(d, t.model, 1, b1) + (size_t)sigma * d.F + phi;
-    FsSlot s = fs_slot(1, v.latT[i], v.powT[i], fs_ceil_div(t.q[1], b1 + 1u), 0.0f, t.slo_ms[1]);
+    const float2 e = v.lpT[i];
+    FsSlot s = fs_slot(1, e.x, e.y, fs_ceil_div(t.q[1], b1 + 1u), 0.0f, t.slo_ms[1]);
     ok = ok && s.ok; e1 = s.e;
   }
   r.ok = ok; r.e = __fadd_rn(e0, e1);

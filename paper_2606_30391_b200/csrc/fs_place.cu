@@ -58,20 +58,21 @@ __device__ __forceinline__ PairCtx make_pair(const FsView& v, const ReqCtx& c, c
 
 struct Cand { bool ok; float dE, ttft, tbt; };
 
-// one candidate from the raw planes (used by the generic kernel and by the decode step)
+// one candidate from the raw planes (the decode step)
 __device__ __forceinline__ Cand eval_cand(const FsView& v, const ReqCtx& c, const PairCtx& p, int k,
                                           int sigma, int phi) {
   const FsDimsDev& d = v.d;
   const size_t o = (size_t)sigma * d.F + phi;
   const size_t i0 = fs_plane(d, c.m, 0, c.br0) + o, i1 = fs_plane(d, c.m, 1, p.br1) + o;
-  const float lat1 = v.latT[i1];
+  const float2 lp0 = v.lpT[i0], lp1 = v.lpT[i1];
+  const float lat1 = lp1.x;
   bool ok = true; float t0 = 0.f, e0 = 0.f, e1 = 0.f;
   if (c.L > 0) {
-    FsSlot s = fs_slot(0, v.latT[i0], v.powT[i0], c.rounds0, p.wait, c.slo_ttft);
+    FsSlot s = fs_slot(0, lp0.x, lp0.y, c.rounds0, p.wait, c.slo_ttft);
     ok = s.ok; t0 = s.t; e0 = s.e;
   }
   if (c.O > 0) {
-    FsSlot s = fs_slot(1, lat1, v.powT[i1], p.rounds1, 0.f, c.slo_tbt);
+    FsSlot s = fs_slot(1, lat1, lp1.y, p.rounds1, 0.f, c.slo_tbt);
     ok = ok && s.ok; e1 = s.e;
   }
   const float A = v.gA[((size_t)k * FS_NVAR + p.var) * d.F + phi];
@@ -82,72 +83,40 @@ __device__ __forceinline__ Cand eval_cand(const FsView& v, const ReqCtx& c, cons
   return r;
 }
 
-// ---- generic scorer: any dims, one warp per (request, GPU slice) ---------------------------
-__global__ void __launch_bounds__(256) place_generic_kernel(FsView v, int R,
-                                                           const fs_request* __restrict__ reqs,
-                                                           unsigned long long* __restrict__ keys,
-                                                           int nsplit, int kchunk,
-                                                           unsigned long long* __restrict__ stats) {
-  const int lane = threadIdx.x & 31;
-  const long long w = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (w >= (long long)R * nsplit) return;
-  const int r = (int)(w / nsplit), part = (int)(w % nsplit);
-  const ReqCtx c = make_req(v, reqs[r]);
-  if (!c.valid) { if (lane == 0) fs_raise(v.flag, FS_FLAG_REQUEST); return; }
-  const FsDimsDev d = v.d;
-  const int k0 = part * kchunk, k1 = min(v.K, k0 + kchunk);
-  float best = FS_INF; uint32_t bflat = 0xFFFFFFFFu; bool have = false;
-  unsigned long long npairs = 0, ncand = 0;
-  for (int k = k0; k < k1; ++k) {
-    const FsGpuInfo gi = v.ginfo[k];
-    const PairCtx p = make_pair(v, c, gi);
-    if (!p.ok) continue;
-    npairs += 1; ncand += (unsigned long long)p.smf * d.F;
-    for (int sg = 0; sg < p.smf; ++sg)
-      for (int phi = lane; phi < d.F; phi += 32) {
-        const Cand cd = eval_cand(v, c, p, k, sg, phi);
-        float dE = cd.dE; if (dE == 0.0f) dE = 0.0f;
-        if (cd.ok && (!have || dE < best)) {     // per-lane visiting order is ascending flat
-          have = true; best = dE; bflat = (uint32_t)((k * d.S + sg) * d.F + phi);
-        }
-      }
-  }
-  unsigned long long key = have ? fs_make_key(best, bflat) : FS_KEY_NONE;
-  key = fs_warp_min_key(key);
-  if (lane == 0) {
-    if (key != FS_KEY_NONE) atomicMin(&keys[r], key);
-    if (stats) { atomicAdd(&stats[1], npairs); atomicAdd(&stats[5], npairs); atomicAdd(&stats[6], ncand); }
-  }
-}
-
-
 // =============================================================================================
-// Dense scorer, every supported shape (S <= 32; F <= 256 in column blocks of 64): one warp = one request, one persistent block per SM.
+// Dense scorer, every supported shape (S <= 32; F <= 256 in column blocks of 64): one warp = one request,
+// one persistent block per SM, requests handed out by an atomic ticket two requests ahead (the next
+// request is already in shared memory, by cp.async, when the current one ends).
 //
-// Factorisation (exact).  For a COLD pair (the request's model is
-// not resident on the GPU) the decode bucket is 0 and the co-resident variant is 0, so everything
-// that depends on (sigma, phi) is per REQUEST:
+// Exact factorisation.  For a COLD pair (the request's model is not
+// resident on the GPU) the decode bucket is 0 and the co-resident variant is 0, so everything that
+// depends on (sigma, phi) is per REQUEST:
 //   t0[s][f] = fl(rounds0*LAT0)                    er[s][f] = fl(e0 + e1), INF where LAT1 > slo_tbt
 // and everything that depends on the GPU is per (k, phi):  A0[k][f], Ecur[k], wait_k, sm_free_k.
 // fl(A + x) and fl(x - Ecur) are monotone in x, hence
 //   min_s fl(fl(A0 + er[s]) - Ecur) = fl(fl(A0 + min_s er[s]) - Ecur)   over feasible s,
 // and fl(wait + t) <= slo  <=>  t <= T*(wait, slo) for the exactly computed threshold T*.
 //
-// Per request the warp (a) builds the two tiles in its own shared-memory region, one row per
-// share, together with prefix minima over the shares (pruning bounds); (b) walks the GPUs in
-// ascending d = a_min - Ecur, lane <-> GPU: eligibility and the exact lower bound
-// fl(fl(a_min + bnd[sm_free]) - Ecur) against the incumbent; the few survivors are swept
-// (compare + predicated min per candidate); the walk stops when no later GPU can win;
-// (c) scores the WARM pairs (model resident: decode bucket, variant and wait depend on the GPU)
-// best bound first, candidate by candidate, and (d) re-scores the winning GPU once to recover the
-// lowest flat index attaining the minimum.  All loops are rolled and the tiles live in shared
-// memory so that the whole kernel stays inside the 32 KB instruction cache (profiles/: the
-// register-tiled, fully unrolled version spent 64 % of its stall samples on instruction fetch).
+// Per request the warp
+//  (a) takes lower bounds on t0, e0 and er over every prefix of shares from the per-plane minima built
+//      with the tables (lane <-> share; fs_energy_lb): no table entry is touched for that;
+//  (b) scores the WARM pairs (model resident: decode bucket, variant and wait depend on the GPU; listed
+//      per model by fs_set_gpu_state), best bound first, candidate by candidate with the definition,
+//      straight from the {LAT, POW} planes (two 128-bit loads per share row and lane);
+//  (c) only if a cold pair could still win (deadline reachable after the weight load, bound of the best
+//      cold-capable GPU not above the incumbent) builds the (sigma, phi) tile {t0, er} in its own
+//      shared-memory region - the prefill plane arrives by ONE 1-D TMA bulk copy (cp.async.bulk on the
+//      warp's mbarrier; it is contiguous in the plane layout), the decode rows through registers - and
+//      walks the cold-capable GPUs in ascending d = a_min - Ecur, lane <-> GPU: eligibility and the exact
+//      lower bound fl(fl(a_min + bnd[sm_free]) - Ecur) against the incumbent; the survivors are swept
+//      (compare + predicated min per candidate); the walk stops when no later GPU can win;
+//  (d) re-scores a cold winner once with the definition to recover the lowest flat index attaining
+//      the minimum, and (one slice) writes the placement record.
+// All loops are rolled so that the kernel stays inside the instruction cache.
 // =============================================================================================
 constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102)
 constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
 constexpr int DENSE_S = FS_MAX_S;
-constexpr int DENSE_TAIL = 4;                 // rounds of requests per warp handed out dynamically at the end
 
 // does any of the four 16-bit models packed in (w0, w1) equal m?  (exact "has a zero halfword" test on the
 // XOR; the SIMD-in-a-word video instructions are emulated on this architecture and cost ~30 instructions)
@@ -194,99 +163,55 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
 }
 
 // Shared memory of one block:
-//   rec  [KS]            the block's slice of the SORTED compact GPU records (one TMA fill)
-//   tile [W][2][S][FT]   per warp: t0 rows, then er rows, of the request being scored
-//   wb   [W][32]         per warp: {T*, Ecur, sm_free, GPU} of the chunk's survivors
-//   bnd  [W][3][32]      per warp: prefix minima over sigma <= s, all phi, of er (cold), t0, e0
-//   req  [W]             per warp: the next statically assigned request, prefetched by cp.async
+//   rec  [KS]          the block's slice of the SORTED compact GPU records (one TMA fill)
+//   per warp:  tile [S][FT] of {t0, er} pairs (the prefill plane {LAT0, POW0} lands here first),
+//              wb [32] {T*, Ecur, sm_free, GPU} of the chunk's survivors, the next request (32 B),
+//              the warp's mbarrier, 8 work counters
 __host__ __device__ inline size_t dense_warp_bytes(int S, int FT) {
-  return (size_t)2 * S * FT * sizeof(float) + FS_CHUNK * sizeof(float4) + 3 * DENSE_S * sizeof(float) + sizeof(fs_request);
+  return (size_t)S * FT * sizeof(float2) + FS_CHUNK * sizeof(float4) + sizeof(fs_request) + 16 + 32;
 }
 __host__ __device__ inline size_t dense_smem_bytes(int KS, int W, int S, int FT) {
   return (size_t)KS * sizeof(FsGpuRec) + (size_t)W * dense_warp_bytes(S, FT) + 16;
 }
 
-// NPHI adjacent values of row `o` for the lane whose first column is phi0 (columns clamped to the
-// row for padded lanes; the caller overrides those); one 64-bit load when the pair is aligned
-template <int NPHI>
-__device__ __forceinline__ void ld_cols(const float* __restrict__ base, int o, int phi0, int ncol, bool vec,
-                                        float (&x)[NPHI]) {
-  if (NPHI == 2 && vec) {
-    const float2 t = *reinterpret_cast<const float2*>(base + o + min(phi0, ncol - 2));
-    x[0] = t.x; x[NPHI - 1] = t.y;
-  } else {
-#pragma unroll
-    for (int i = 0; i < NPHI; ++i) x[i] = base[o + min(phi0 + i, ncol - 1)];
-  }
-}
-
-// The same through per-lane pointers that already include the lane's (clamped) column: the address of a
-// row is then one widening multiply-add of an unsigned element offset instead of a chain of 64-bit adds.
-struct LanePtr { const float* a; const float* b; };
-template <int NPHI>
-__device__ __forceinline__ LanePtr lane_ptr(const float* base, int phi0, int ncol, bool vec) {
-  LanePtr p;
-  p.a = base + (NPHI == 2 && vec ? min(phi0, ncol - 2) : min(phi0, ncol - 1));
+// The lane's NPHI adjacent {LAT, POW} entries of a plane row.  Pointers already include the lane's column
+// (clamped to the row for padded lanes: they hold copies of the last columns, which no minimum notices,
+// and every consumer adds an A row that is +INF there).  VEC: the lane's two entries are one aligned
+// 128-bit access (NPHI == 2 and F even): a template parameter, so no branch on the shape at any load.
+struct LaneLP { const float2* a; const float2* b; };
+template <int NPHI, bool VEC>
+__device__ __forceinline__ LaneLP lane_lp(const float2* base, int phi0, int ncol) {
+  LaneLP p;
+  p.a = base + (NPHI == 2 && VEC ? min(phi0, ncol - 2) : min(phi0, ncol - 1));
   p.b = base + min(phi0 + NPHI - 1, ncol - 1);
   return p;
 }
-template <int NPHI>
-__device__ __forceinline__ void ld_lane(const LanePtr& p, uint32_t o, bool vec, float (&x)[NPHI]) {
-  if (NPHI == 2 && vec) { const float2 t = *reinterpret_cast<const float2*>(p.a + o); x[0] = t.x; x[NPHI - 1] = t.y; }
-  else { x[0] = p.a[o]; if (NPHI == 2) x[NPHI - 1] = p.b[o]; }
-}
-
-// asynchronous copy (LDGSTS) of the lane's NPHI values of row `o` into its own tile slot: no registers are
-// held while the row is on its way; the lane that issued the copy is the one that reads the slot
-template <int NPHI>
-__device__ __forceinline__ void cp_lane(uint32_t dst, const LanePtr& p, bool vec) {
-  if (NPHI == 2 && vec) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(p.a) : "memory");
-  else {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(p.a) : "memory");
-    if (NPHI == 2) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + 4u), "l"(p.b) : "memory");
+template <int NPHI, bool VEC>
+__device__ __forceinline__ void ld_lp(const LaneLP& p, uint32_t o, float (&l)[NPHI], float (&w)[NPHI]) {
+  if (NPHI == 2 && VEC) {
+    const float4 t = __ldg(reinterpret_cast<const float4*>(p.a + o));
+    l[0] = t.x; w[0] = t.y; l[NPHI - 1] = t.z; w[NPHI - 1] = t.w;
+  } else {
+    const float2 t = __ldg(p.a + o); l[0] = t.x; w[0] = t.y;
+    if (NPHI == 2) { const float2 u = __ldg(p.b + o); l[NPHI - 1] = u.x; w[NPHI - 1] = u.y; }
   }
 }
-__device__ __forceinline__ void cp_commit_wait_all() {
-  asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
-}
-
-// work statistics (what this launch actually did; bench.py turns them into lane-operations)
-__device__ __forceinline__ void flush_stats(unsigned long long* stats, uint32_t n_chunks, uint32_t n_elig,
-                                         uint32_t n_swept, uint32_t n_cswept, uint32_t n_witems,
-                                         uint32_t n_scored, uint32_t n_cscored, uint32_t n_req) {
-  if (!stats) return;
-  unsigned long long e = n_elig, w = n_witems;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    e += __shfl_xor_sync(0xffffffffu, e, o);
-    w += __shfl_xor_sync(0xffffffffu, w, o);
-  }
-  if ((threadIdx.x & 31) == 0) {
-    atomicAdd(&stats[0], (unsigned long long)n_chunks); atomicAdd(&stats[1], e);
-    atomicAdd(&stats[2], (unsigned long long)n_swept); atomicAdd(&stats[3], (unsigned long long)n_cswept);
-    atomicAdd(&stats[4], w); atomicAdd(&stats[5], (unsigned long long)n_scored);
-    atomicAdd(&stats[6], (unsigned long long)n_cscored); atomicAdd(&stats[7], (unsigned long long)n_req);
-  }
-}
-
+// the same from / to the warp's tile (the lane's slot is always aligned)
 template <int NPHI>
-__device__ __forceinline__ void ld_tile(const float* p, float (&x)[NPHI]) {
-  if (NPHI == 2) { const float2 t = *reinterpret_cast<const float2*>(p); x[0] = t.x; x[NPHI - 1] = t.y; }
-  else x[0] = p[0];
+__device__ __forceinline__ void ld_tile(const float2* p, float (&x)[NPHI], float (&y)[NPHI]) {
+  if (NPHI == 2) { const float4 t = *reinterpret_cast<const float4*>(p); x[0] = t.x; y[0] = t.y; x[NPHI - 1] = t.z; y[NPHI - 1] = t.w; }
+  else { const float2 t = *p; x[0] = t.x; y[0] = t.y; }
 }
 template <int NPHI>
-__device__ __forceinline__ void st_tile(float* p, const float (&x)[NPHI]) {
-  if (NPHI == 2) *reinterpret_cast<float2*>(p) = make_float2(x[0], x[NPHI - 1]);
-  else p[0] = x[0];
+__device__ __forceinline__ void st_tile(float2* p, const float (&x)[NPHI], const float (&y)[NPHI]) {
+  if (NPHI == 2) *reinterpret_cast<float4*>(p) = make_float4(x[0], y[0], x[NPHI - 1], y[NPHI - 1]);
+  else *p = make_float2(x[0], y[0]);
 }
 
-// VEC: the lane's two adjacent frequencies are one aligned 64-bit access (NPHI == 2 and F even); a template
-// parameter so that every row access is one instruction without a branch on the shape
-// COLS: F > 64.  The frequencies are cut into blocks of 64 columns; a thread block scores every request on
-// (its slice of the GPUs) x (its column block), exactly like one more kind of slice: all row pointers are
-// shifted by the block's first column, the per-GPU bounds (minima over ALL frequencies) stay valid lower
-// bounds, and the results are merged by the 64-bit key (the record is then written by the decode kernel).
-template <int NPHI, bool VEC, bool STATS, bool COLS>
+// work counters of a counting launch (fs_set_work_stats): per warp in shared memory, flushed per request
+enum { ST_CHUNKS = 0, ST_ELIG, ST_SWEPT, ST_CSWEPT, ST_WITEMS, ST_SCORED, ST_CSCORED, ST_REQ };
+
+template <int NPHI, bool VEC, bool COLS>
 __global__ void __launch_bounds__(DENSE_MAXW * 32, 1)
 place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    unsigned long long* __restrict__ keys, int nslice, int ncb, int chunks_per_slice,
@@ -295,7 +220,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                    fs_placement* __restrict__ out) {
   extern __shared__ __align__(128) unsigned char dense_smem_raw[];
   constexpr int FT = 32 * NPHI;
-  constexpr uint32_t NONE32 = 0xFFFFFFFFu, INFBITS = 0x7F800000u;
+  constexpr uint32_t NONE32 = 0xFFFFFFFFu, INFBITS = 0x7F800000u, FULL = 0xffffffffu;
   constexpr int KNONE = 0x7FFFFFFF;
   const FsDimsDev d = v.d;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
@@ -309,15 +234,18 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const int nchunk = c1 - c0, KS = nchunk * FS_CHUNK, KSmax = chunks_per_slice * FS_CHUNK;
   FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw);
   unsigned char* s_warp = dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec) + (size_t)warp * dense_warp_bytes(d.S, FT);
-  float* tl_t0 = reinterpret_cast<float*>(s_warp);
-  float* tl_er = tl_t0 + d.S * FT;
-  float4* wb = reinterpret_cast<float4*>(tl_er + d.S * FT);
-  float* bnd = reinterpret_cast<float*>(wb + FS_CHUNK);
+  float2* tile = reinterpret_cast<float2*>(s_warp);
+  float4* wb = reinterpret_cast<float4*>(tile + d.S * FT);
+  fs_request* s_req = reinterpret_cast<fs_request*>(wb + FS_CHUNK);
+  uint64_t* w_bar = reinterpret_cast<uint64_t*>(s_req + 1);
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(w_bar + 2);
   uint64_t* s_bar = reinterpret_cast<uint64_t*>(dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec) +
                                                 (size_t)W * dense_warp_bytes(d.S, FT));
 
   // ---- stage this block's slice of the SORTED GPU records once: 1-D TMA bulk copies on one mbarrier
-  if (threadIdx.x == 0) { fs_mbar_init(s_bar, 1); fs_mbar_fence_init(); }
+  if (threadIdx.x == 0) fs_mbar_init(s_bar, 1);
+  if (lane == 0) { fs_mbar_init(w_bar, 1); if (stats) { for (int i = 0; i < 8; ++i) s_cnt[i] = 0u; } }
+  if (threadIdx.x == 0) fs_mbar_fence_init();
   __syncthreads();
   if (threadIdx.x == 0) {
     const uint32_t bytes_rec = (uint32_t)KS * sizeof(FsGpuRec);
@@ -332,308 +260,311 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const double* dsuf = v.dsuf + 1 + c0;
   const double amax = v.dsuf[0];
   const float tmin = (float)v.dsuf[2 + nchunk_all];
-  // work counters (warp-uniform except n_elig / n_witems, which are per lane)
-  uint32_t n_chunks = 0, n_elig = 0, n_swept = 0, n_cswept = 0, n_witems = 0, n_scored = 0, n_cscored = 0, n_req = 0;
-  constexpr bool vec = VEC;
   const int phi0 = lane * NPHI;
-  const LanePtr q_a0 = lane_ptr<NPHI>(v.gA0 + cb0, phi0, FT, true);
-  // ---- which requests this warp scores: all but the last DENSE_TAIL rounds are assigned statically
-  // (warp w of the slice takes w, w + wps, ...), so the next request is known and fetched while the
-  // current one is scored (ticket -> request -> model info is otherwise a serial chain of three memory
-  // latencies at the head of every request); the tail is handed out dynamically, one atomic per warp,
-  // and evens out what the static part left uneven.
-  fs_request* s_req = reinterpret_cast<fs_request*>(bnd + 3 * DENSE_S);
-  const int wps = ((int)gridDim.x / nsc) * W, widx = ((int)blockIdx.x / nsc) * W + warp;
-  const int R0 = max(0, R - DENSE_TAIL * wps);
-  int r_static = widx;
+  const int Fc = d.F - cb0;                              // columns from this block's first one to the end of a row
+  const int ncol = min(FT, Fc);                          // columns of this block
+  const bool bulk = (d.F & 1) == 0;                      // rows are 16-byte multiples at 16-byte aligned addresses
+  const float* a0_lane = v.gA0 + cb0 + phi0;             // rows of gA0 are padded with +INF to FA columns: aligned
+  const int ls = min(lane, d.S - 1);                     // lane <-> share for the bounds
+  uint32_t tile_parity = 0;
+  // ---- request tickets: r_cur is being scored, r_nxt is on its way into s_req, the ticket after that is
+  // requested while r_cur is scored (ticket -> request -> model info would otherwise be a serial chain of
+  // three memory latencies at the head of every request)
   const bool req_aligned = (reinterpret_cast<unsigned long long>(reqs) & 15ull) == 0;   // 16-byte copies
-  bool fetched = false;                                  // s_req holds request r_static
-  for (;;) {
-    int r = 0;
-    fs_request rq;
-    if (r_static < R0) {
-      r = r_static; r_static += wps;
-      if (fetched) {
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncwarp();
-        rq = *s_req;
-        __syncwarp();
-        fetched = false;
-      } else {
-        rq = reqs[r];
+  int r_cur = 0, r_nxt = 0;
+  if (lane == 0) { r_cur = (int)atomicAdd(&ctr[sci], 1u); r_nxt = (int)atomicAdd(&ctr[sci], 1u); }
+  r_cur = __shfl_sync(FULL, r_cur, 0); r_nxt = __shfl_sync(FULL, r_nxt, 0);
+  fs_request rq;
+  if (r_cur < R) rq = reqs[r_cur];
+  while (r_cur < R) {
+    const int r = r_cur;
+    if (r_nxt < R) {
+      const char* src = reinterpret_cast<const char*>(reqs + r_nxt);
+      if (req_aligned) {
+        if (lane < 2) asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(fs_smem_u32(s_req) + 16u * lane), "l"(src + 16 * lane) : "memory");
+      } else if (lane < 8) {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(fs_smem_u32(s_req) + 4u * lane), "l"(src + 4 * lane) : "memory");
       }
-    } else {
-      if (lane == 0) r = R0 + (int)atomicAdd(&ctr[sci], 1u);
-      r = __shfl_sync(0xffffffffu, r, 0);
-      if (r >= R) break;
-      rq = reqs[r];
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    int r_nn = 0;
+    if (lane == 0) r_nn = (int)atomicAdd(&ctr[sci], 1u);
     const ReqCtx c = make_req(v, rq);
+    unsigned long long key = FS_KEY_NONE; int kwin = 0;
     if (!c.valid) {
-      if (lane == 0 && sci == 0) {
-        fs_raise(v.flag, FS_FLAG_REQUEST);
-        if (out) {
-          fs_placement o; o.gpu = -1; o.sigma = o.phi = o.beta = o.f_req = -1;
-          o.energy_mj = o.ttft_ms = o.tbt_ms = FS_INF; o.flat = 0xFFFFFFFFu; o._pad = 0;
-          out[r] = o;
-        }
-      }
-      continue;
-    }
-    // ---- (a) the request's (sigma, phi) tiles, one row per share, and the pruning bounds:
-    // every candidate of a GPU with sm_free = s has  er >= bnd[0][s-1], t0 >= bnd[1][s-1],
-    // e0 >= bnd[2][s-1]; hence, for a cold pair,  dE >= fl(fl(a_min + bnd[0][s-1]) - Ecur)
-    // (monotone rounding).  er, t0, e0 >= +0, so their bit patterns order like unsigned integers.
-    // L == 0 / O == 0 need no branches: rounds = 0 gives t = e = +0 exactly (tables are finite),
-    // and an empty decode slot passes its deadline (threshold +INF).
-    const int Fc = d.F - cb0;                            // columns from this block's first one to the end of a row
-    const LanePtr q_p0 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 0, c.br0) + cb0, phi0, Fc, vec);
-    {
-      const LanePtr q_l0 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 0, c.br0) + cb0, phi0, Fc, vec);
-      const LanePtr q_l1 = lane_ptr<NPHI>(v.latT + fs_plane(d, c.m, 1, 0) + cb0, phi0, Fc, vec);
-      const LanePtr q_p1 = lane_ptr<NPHI>(v.powT + fs_plane(d, c.m, 1, 0) + cb0, phi0, Fc, vec);
+      if (lane == 0 && sci == 0) fs_raise(v.flag, FS_FLAG_REQUEST);
+    } else {
+      // ---- (a) bounds over every prefix of shares (lane <-> share s: shares 0..s, all phi)
+      //   b_t0 = min t0 (exact: fl(fr0 * .) is monotone),  b_e0 <= min e0,  b_er <= min er of a cold pair
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
-      const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
-      uint32_t pe = INFBITS, pt = INFBITS, pe0 = INFBITS;   // running prefix minima (bits)
-      __syncwarp();
-      // the prefill rows (LAT0, POW0) of all shares go straight into the tile slots they will be replaced
-      // in (t0 over LAT0, er over POW0), asynchronously and without registers; the decode rows come
-      // through registers, four rows in flight
+      float b_t0, b_e0, b_er;
       {
-        uint32_t dt = fs_smem_u32(tl_t0 + phi0), de = fs_smem_u32(tl_er + phi0);
-        LanePtr gl = q_l0, gp = q_p0;
+        const FsPlaneMin pm0 = v.pmin[(((size_t)c.m * 2 + 0) * d.B + c.br0) * d.S + ls];
+        const FsPlaneMin pm1 = v.pmin[(((size_t)c.m * 2 + 1) * d.B + 0) * d.S + ls];
+        b_t0 = __fmul_rn(fr0, pm0.lmin);
+        b_e0 = fs_energy_lb(fr0, pm0.lp, pm0.pmax);
+        b_er = (c.O == 0 || pm1.lmin <= c.slo_tbt) ? __fadd_rn(b_e0, fs_energy_lb(fO, pm1.lp, pm1.pmax)) : FS_INF;
+      }
+      const LaneLP q_lp0 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 0, c.br0) + cb0, phi0, Fc);
+      // an empty prefill / decode slot passes its deadline whatever the wait (slot rule, q == 0)
+      const float ttft_e = c.L ? c.slo_ttft : FS_INF, tbt_e = c.O ? c.slo_tbt : FS_INF;
+      // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scans are not in index order
+      float best = FS_INF; int bestk = KNONE;
+      uint32_t bflat = NONE32;   // flat index of the lane's incumbent when the definition body found it (warm pairs)
+      // ---- (b), (d) the definition, pair by pair, from the planes: first the WARM pairs (GPUs that already
+      // host model m), best bound first, then once more on a cold winner to recover the lowest flat index
+      // attaining the minimum.  One code site serves both.
+      //   warm bound:  dE >= fl(fl(a_min + fl(b_e0[sm_free-1] + e1lb)) - Ecur),  e1lb = fs_energy_lb(rounds1, ...)
+      int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
+      uint32_t ordl = NONE32; int wk = 0;
+      uint32_t wpk = 0, wr1 = 0; float wta = 0.f, wec = 0.f;   // the lane's item: j | br1 << 8 | sm_free << 16, rounds1, T_avail, Ecur
+      bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32;
+      for (;;) {
+        int k = KNONE;
+        int wsrc = -1;                                    // lane that holds the chosen warm item
+        while (!recover) {
+          const uint32_t mn = warp_min_u32(ordl);
+          const uint32_t inc = warp_min_u32(fs_orderable(best));
+          if (mn != NONE32 && mn <= inc) {               // best-first: the item with the lowest bound
+            const int src = __ffs(__ballot_sync(FULL, ordl == mn)) - 1;
+            k = __shfl_sync(FULL, wk, src);
+            if (lane == src) ordl = NONE32;
+            wsrc = src;
+            break;
+          }
+          if (ib >= ie) {                                 // no item left that could beat the incumbent
+            // ---- (c) cold pairs, AFTER the warm ones: a cold start often cannot meet the TTFT deadline at
+            // all (load_ms against the SLO), and a warm incumbent lets the scan stop early.  GPUs in ascending
+            // d = a_min - Ecur: every candidate of every GPU from chunk ci on has dE >= fl(fl(a + b) - e) with
+            // a - e >= dsuf[ci], b >= bmin, a <= amax, and two roundings lose at most 2^-23 (a + b + |a + b - e|);
+            // the scan stops as soon as that (with twice the slack) exceeds the incumbent, strictly, so ties
+            // still meet every GPU.  No cold pair at all can meet the TTFT deadline if even the earliest
+            // T_avail plus the weight load plus the fastest prefill misses it (monotone rounding).
+            float bminf = __shfl_sync(FULL, b_er, d.S - 1);
+            const float t0min = __shfl_sync(FULL, b_t0, d.S - 1);
+            bool cold = bminf < FS_INF && nchunk > 0 &&
+                        (c.L == 0 || __fadd_rn(__fadd_rn(tmin, c.load_ms), t0min) <= c.slo_ttft);
+            float incW = fs_unorderable(inc);
+            if (cold) {                                   // the first chunk's stop test with the table bound
+              const double ds = dsuf[0];
+              if (!(ds < (double)FS_INF)) cold = false;
+              else if (incW < FS_INF) {
+                const double x = ds + (double)bminf;
+                if (x - 0x1p-22 * (amax + (double)bminf + fabs(x)) - 1e-37 > (double)incW) cold = false;
+              }
+            }
+            if (cold) {
+              // ---- the request's tile: {t0, er} per (share, frequency), and the EXACT prefix minima of er
+              const LaneLP q_lp1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, 0) + cb0, phi0, Fc);
+              __syncwarp();
+              if (bulk) {
+                // generic-proxy accesses of the last request's tile are ordered before the async-proxy writes
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) {
+                  const float2* src = v.lpT + fs_plane(d, c.m, 0, c.br0) + cb0;
+                  fs_mbar_expect_tx(w_bar, (uint32_t)(d.S * ncol) * 8u);
+                  if (ncol == FT && d.F == FT) fs_tma_load_1d(tile, src, (uint32_t)(d.S * FT) * 8u, w_bar);
+                  else for (int s = 0; s < d.S; ++s) fs_tma_load_1d(tile + s * FT, src + (size_t)s * d.F, (uint32_t)ncol * 8u, w_bar);
+                }
+              } else {
+                uint32_t dt = fs_smem_u32(tile + phi0);
+                LaneLP g = q_lp0;
+                for (int s = 0; s < d.S; ++s) {
+                  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dt), "l"(g.a) : "memory");
+                  if (NPHI == 2) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dt + 8u), "l"(g.b) : "memory");
+                  dt += FT * 8u; g.a += d.F; g.b += d.F;
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+              }
+              uint32_t pe = INFBITS;                      // running prefix minimum of er (bits: er >= +0)
+              for (int s0 = 0; s0 < d.S; s0 += 4) {
+                float a1[4][NPHI], b1[4][NPHI];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) ld_lp<NPHI, VEC>(q_lp1, (uint32_t)(min(s0 + u, d.S - 1) * d.F), a1[u], b1[u]);
+                if (s0 == 0) {                           // the prefill plane has landed in the tile
+                  if (bulk) { fs_mbar_wait(w_bar, tile_parity); tile_parity ^= 1u; }
+                  else { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+                  __syncwarp();
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                  const int s = s0 + u;
+                  if (s < d.S) {
+                    float a0[NPHI], b0[NPHI], tt[NPHI], ee[NPHI];
+                    ld_tile<NPHI>(tile + s * FT + phi0, a0, b0);
+                    uint32_t ue = INFBITS;
+#pragma unroll
+                    for (int i = 0; i < NPHI; ++i) {
+                      const float t = __fmul_rn(fr0, a0[i]);
+                      const float e = __fadd_rn(__fmul_rn(t, b0[i]), __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
+                      // columns past the row (phi >= F) hold whatever the tile held before: they are masked
+                      const bool in = !bulk || phi0 + i < ncol;
+                      tt[i] = in ? t : FS_INF;
+                      ee[i] = (in && a1[u][i] <= tbt_e) ? e : FS_INF;
+                      ue = min(ue, __float_as_uint(ee[i]));
+                    }
+                    st_tile<NPHI>(tile + s * FT + phi0, tt, ee);
+                    pe = min(pe, warp_min_u32(ue));
+                    if (lane == s) b_er = __uint_as_float(pe);
+                  }
+                }
+              }
+              __syncwarp();
+              bminf = __shfl_sync(FULL, b_er, d.S - 1);
+              const double bmin = (double)bminf;
+              for (int ci = 0; ci < nchunk && bminf < FS_INF; ++ci) {
+                incW = fs_unorderable(warp_min_u32(fs_orderable(best)));
+                const double ds = dsuf[ci];
+                if (!(ds < (double)FS_INF)) break;                 // sentinels only from here on
+                if (incW < FS_INF) {
+                  const double x = ds + bmin;
+                  if (x - 0x1p-22 * (amax + bmin + fabs(x)) - 1e-37 > (double)incW) break;
+                }
+                // ---- eligibility + bound: lane <-> one GPU of the chunk ---------------------------------
+                const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
+                const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
+                const uint32_t mm = (uint32_t)c.m * 0x00010001u;
+                const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
+                const bool el = (c.mem <= g.mem_free_mb) && !has_model(gm[0], gm[1], mm);
+                const float er_lb = __shfl_sync(FULL, b_er, smf - 1), t0_lb = __shfl_sync(FULL, b_t0, smf - 1);
+                float T = -1.0f;
+                if (el) {
+                  // prune: no candidate of this GPU can beat or tie the best found so far
+                  const float lb = __fsub_rn(__fadd_rn(g.a_min, er_lb), g.e_cur);
+                  if (lb <= incW && lb < FS_INF) {
+                    const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
+                    if (c.L == 0) T = FS_INF;
+                    else if (__fadd_rn(wait, t0_lb) <= c.slo_ttft) T = fs_tstar(wait, c.slo_ttft);
+                  }
+                }
+                // compact the surviving GPUs of the chunk into the warp's list: {T*, Ecur, sm_free, GPU}
+                const bool go = T >= 0.0f;
+                const unsigned mask = __ballot_sync(FULL, go);
+                if (stats) { const unsigned elm = __ballot_sync(FULL, el); if (lane == 0) { s_cnt[ST_CHUNKS] += 1u; s_cnt[ST_ELIG] += (uint32_t)__popc(elm); } }
+                if (mask == 0u) continue;
+                __syncwarp();
+                if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
+                    make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((int)g.k));
+                __syncwarp();
+                const int n_el = __popc(mask);
+                // ---- sweep the survivors: per candidate one compare and one predicated min ---------------
+                for (int e = 0; e < n_el; ++e) {
+                  const float4 w = wb[e];
+                  const float Tst = w.x; const int sfree = __float_as_int(w.z); const int kk = __float_as_int(w.w);
+                  if (stats && lane == 0) { s_cnt[ST_SWEPT] += 1u; s_cnt[ST_CSWEPT] += (uint32_t)(sfree * d.F); }
+                  float arow[NPHI], m[NPHI];
+                  {
+                    const float* ap = a0_lane + (size_t)kk * (size_t)FA;
+                    if (NPHI == 2) { const float2 t = *reinterpret_cast<const float2*>(ap); arow[0] = t.x; arow[NPHI - 1] = t.y; }
+                    else arow[0] = ap[0];
+                  }
+#pragma unroll
+                  for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
 #pragma unroll 4
-        for (int s = 0; s < d.S; ++s) {
-          cp_lane<NPHI>(dt, gl, vec); cp_lane<NPHI>(de, gp, vec);
-          dt += FT * 4u; de += FT * 4u;
-          gl.a += d.F; gl.b += d.F; gp.a += d.F; gp.b += d.F;
-        }
-      }
-      for (int s0 = 0; s0 < d.S; s0 += 4) {
-        float a1[4][NPHI], b1[4][NPHI];
+                  for (int s = 0; s < sfree; ++s) {
+                    float tt[NPHI], ee[NPHI];
+                    ld_tile<NPHI>(tile + s * FT + phi0, tt, ee);
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int o = min(s0 + u, d.S - 1) * d.F;
-          ld_lane<NPHI>(q_l1, o, vec, a1[u]); ld_lane<NPHI>(q_p1, o, vec, b1[u]);
-        }
-        if (s0 == 0) cp_commit_wait_all();               // the prefill rows have landed in the tile slots
+                    for (int i = 0; i < NPHI; ++i) m[i] = tt[i] <= Tst ? fminf(m[i], ee[i]) : m[i];
+                  }
+                  float x = FS_INF;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int s = s0 + u;
-          if (s < d.S) {
-            float a0[NPHI], b0[NPHI], tt[NPHI], ee[NPHI];
-            ld_tile<NPHI>(tl_t0 + s * FT + phi0, a0); ld_tile<NPHI>(tl_er + s * FT + phi0, b0);
-            uint32_t ue = INFBITS, ut = INFBITS, ue0 = INFBITS;
-#pragma unroll
-            for (int i = 0; i < NPHI; ++i) {
-              const float t = __fmul_rn(fr0, a0[i]);
-              const float e0 = __fmul_rn(t, b0[i]);
-              const float e = __fadd_rn(e0, __fmul_rn(__fmul_rn(fO, a1[u][i]), b1[u][i]));
-              // a padded lane (phi >= F) holds a copy of the row's last column(s): the minima are unchanged,
-              // and every consumer of the tiles adds an A row that is +INF there
-              tt[i] = t;
-              ee[i] = a1[u][i] <= tbt ? e : FS_INF;
-              ue0 = min(ue0, __float_as_uint(e0));
-              ue = min(ue, __float_as_uint(ee[i])); ut = min(ut, __float_as_uint(t));
-            }
-            st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
-            pe = min(pe, warp_min_u32(ue)); pt = min(pt, warp_min_u32(ut)); pe0 = min(pe0, warp_min_u32(ue0));
-            if (lane == 0) {
-              bnd[s] = __uint_as_float(pe); bnd[DENSE_S + s] = __uint_as_float(pt);
-              bnd[2 * DENSE_S + s] = __uint_as_float(pe0);
-            }
-          }
-        }
-      }
-      __syncwarp();
-    }
-    if (r_static < R0 && req_aligned) {                  // the next static request, on its way during the scoring
-      if (lane < 2) {
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(fs_smem_u32(s_req) + 16u * lane),
-                     "l"(reinterpret_cast<const char*>(reqs + r_static) + 16 * lane) : "memory");
-      }
-      asm volatile("cp.async.commit_group;" ::: "memory");
-      fetched = true;
-    }
-    // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scans are not in index order
-    float best = FS_INF; int bestk = KNONE;
-    uint32_t bflat = NONE32;   // flat index of the lane's incumbent when the definition body found it (warm pairs)
-    // ---- (c), (d) the definition, pair by pair, from the t0 tile and the planes: first the WARM
-    // pairs (GPUs that already host model m), best bound first, then once more on the winning GPU
-    // to recover the lowest flat index attaining the minimum.  One code site serves both.
-    //   warm bound:  dE >= fl(fl(a_min + fl(e0min + e1min)) - Ecur),  e1min = fl(fl(rounds1*l1_min)*p1_min)
-    int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
-    uint32_t ordl = NONE32; int wk = 0;
-    uint32_t wpk = 0; float wta = 0.f, wec = 0.f;       // the lane's item: j | br1 << 8 | sm_free << 16, T_avail, Ecur
-    bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32; int kwin = 0;
-    for (;;) {
-      int k = KNONE;
-      int wsrc = -1;                                    // lane that holds the chosen warm item
-      while (!recover) {
-        const uint32_t mn = warp_min_u32(ordl);
-        const uint32_t inc = warp_min_u32(fs_orderable(best));
-        if (mn != NONE32 && mn <= inc) {               // best-first: the item with the lowest bound
-          const int src = __ffs(__ballot_sync(0xffffffffu, ordl == mn)) - 1;
-          k = __shfl_sync(0xffffffffu, wk, src);
-          if (lane == src) ordl = NONE32;
-          wsrc = src;
-          break;
-        }
-        if (ib >= ie) {                                 // no item left that could beat the incumbent
-          // the cold scan comes AFTER the warm pairs: a cold start often cannot meet the TTFT deadline
-          // at all (load_ms against the SLO), and then only a warm incumbent lets the scan stop early
-          // ---- (b) cold pairs: GPUs in ascending d = a_min - Ecur.  Every candidate of every GPU from
-          // chunk ci on has  dE >= fl(fl(a + b) - e)  with  a - e >= dsuf[ci],  b >= bmin,  a <= amax,
-          // and two roundings lose at most 2^-23 (a + b + |a + b - e|); the scan stops as soon as that
-          // (with twice the slack) exceeds the incumbent, strictly, so ties still meet every GPU.
-          // No cold pair at all can meet the TTFT deadline if even the earliest T_avail plus the weight
-          // load plus the fastest prefill misses it (monotone rounding): then there is nothing to scan.
-          const float bminf = bnd[d.S - 1];
-          const double bmin = (double)bminf;
-          const bool cold_possible = bminf < FS_INF &&
-              (c.L == 0 || __fadd_rn(__fadd_rn(tmin, c.load_ms), bnd[DENSE_S + d.S - 1]) <= c.slo_ttft);
-          for (int ci = 0; ci < nchunk && cold_possible; ++ci) {
-            const float bestW = fs_unorderable(warp_min_u32(fs_orderable(best)));
-            const double ds = dsuf[ci];
-            if (!(ds < (double)FS_INF)) break;                 // sentinels only from here on
-            if (bestW < FS_INF) {
-              const double x = ds + bmin;
-              if (x - 0x1p-22 * (amax + bmin + fabs(x)) - 1e-37 > (double)bestW) break;
-            }
-            if (STATS) { n_chunks += 1; }
-            // ---- eligibility + bound: lane <-> one GPU of the chunk ---------------------------------
-            const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
-            const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
-            const uint32_t mm = (uint32_t)c.m * 0x00010001u;
-            const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
-            const bool el = (c.mem <= g.mem_free_mb) && !has_model(gm[0], gm[1], mm);
-            float T = -1.0f;
-            if (el) {
-              if (STATS) { n_elig += 1; }
-              // prune: no candidate of this GPU can beat or tie the best found so far
-              const float lb = __fsub_rn(__fadd_rn(g.a_min, bnd[smf - 1]), g.e_cur);
-              if (lb <= bestW && lb < FS_INF) {
-                const float wait = __fadd_rn(g.t_avail_ms, c.load_ms);
-                if (c.L == 0) T = FS_INF;
-                else if (__fadd_rn(wait, bnd[DENSE_S + smf - 1]) <= c.slo_ttft) T = fs_tstar(wait, c.slo_ttft);
+                  for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
+                  const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
+                  if (dE < best || (dE == best && kk < bestk)) { best = dE; bestk = kk; bflat = NONE32; }
+                }
               }
             }
-            // compact the surviving GPUs of the chunk into the warp's list: {T*, Ecur, sm_free, GPU}
-            const bool go = T >= 0.0f;
-            const unsigned mask = __ballot_sync(0xffffffffu, go);
-            if (mask == 0u) continue;
-            __syncwarp();
-            if (go) wb[__popc(mask & ((1u << lane) - 1u))] =
-                make_float4(T, g.e_cur, __int_as_float(smf), __int_as_float((int)g.k));
-            __syncwarp();
-            const int n_el = __popc(mask);
-            // ---- sweep the survivors: per candidate one compare and one predicated min ---------------
-            for (int e = 0; e < n_el; ++e) {
-              const float4 w = wb[e];
-              const float Tst = w.x; const int sfree = __float_as_int(w.z); const int k = __float_as_int(w.w);
-              if (STATS) { n_swept += 1; n_cswept += (uint32_t)(sfree * d.F); }
-              float arow[NPHI], m[NPHI];
-              ld_lane<NPHI>(q_a0, (uint32_t)k * (uint32_t)FA, true, arow);   // rows are padded with +INF: aligned
-      #pragma unroll
-              for (int i = 0; i < NPHI; ++i) m[i] = FS_INF;
-      #pragma unroll 4
-              for (int s = 0; s < sfree; ++s) {
-                float tt[NPHI], ee[NPHI];
-                ld_tile<NPHI>(tl_t0 + s * FT + phi0, tt); ld_tile<NPHI>(tl_er + s * FT + phi0, ee);
-      #pragma unroll
-                for (int i = 0; i < NPHI; ++i) m[i] = tt[i] <= Tst ? fminf(m[i], ee[i]) : m[i];
-              }
-              float x = FS_INF;
-      #pragma unroll
-              for (int i = 0; i < NPHI; ++i) x = fminf(x, __fadd_rn(arow[i], m[i]));
-              const float dE = __fsub_rn(x, w.y);          // monotone: min over the lane's phis first
-              if (dE < best || (dE == best && k < bestk)) { best = dE; bestk = k; bflat = NONE32; }
+            const unsigned long long kq = fs_warp_min_key(((unsigned long long)fs_orderable(best) << 32) | (uint32_t)bestk);
+            recover = true; k = (int)(uint32_t)kq; kwin = k; bestW = fs_unorderable((uint32_t)(kq >> 32));
+            // a warm winner was scored by the definition in flat order: its lanes already hold their
+            // lowest flat index, nothing to recover (a GPU is warm or cold for a request, never both)
+            if (k != KNONE && best == bestW && bestk == k) flat = bflat;
+            if (__any_sync(FULL, flat != NONE32)) k = KNONE;
+            break;
+          }
+          // next 32 items: lane <-> item
+          ordl = NONE32;
+          const int ix = ib + lane;
+          bool have = false; int sidx = 0; float e1lb = 0.f; FsWarmItem it;
+          if (ix < ie && (nslice == 1 || ix % nslice == slice)) {
+            it = witems[ix];
+            if (it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
+              have = true; sidx = it.sm_free - 1;
+              wr1 = fs_ceil_div_magic(c.O, it.magic);
+              e1lb = fs_energy_lb(__uint2float_rn(wr1), it.lp1, it.p1_max);
             }
           }
-          const unsigned long long kk = fs_warp_min_key(((unsigned long long)fs_orderable(best) << 32) | (uint32_t)bestk);
-          recover = true; k = (int)(uint32_t)kk; kwin = k; bestW = fs_unorderable((uint32_t)(kk >> 32));
-          // a warm winner was scored by the definition in flat order: its lanes already hold their
-          // lowest flat index, nothing to recover (a GPU is warm or cold for a request, never both)
-          if (k != KNONE && best == bestW && bestk == k) flat = bflat;
-          if (__any_sync(0xffffffffu, flat != NONE32)) k = KNONE;
-          break;
-        }
-        ordl = NONE32;                                  // next 32 items: lane <-> item
-        const int ix = ib + lane;
-        if (ix < ie && (nslice == 1 || ix % nslice == slice)) {
-          const FsWarmItem it = witems[ix];
-          if (it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
-            if (STATS) { n_witems += 1; }
-            const float fr1 = __uint2float_rn(fs_ceil_div(c.O, (uint32_t)it.br1 + 1u));
-            const float e1lb = __fmul_rn(__fmul_rn(fr1, it.l1_min), it.p1_min);
-            const float lb = __fsub_rn(__fadd_rn(it.a_min, __fadd_rn(bnd[2 * DENSE_S + it.sm_free - 1], e1lb)), it.e_cur);
+          const float e0lb = __shfl_sync(FULL, b_e0, sidx), t0lb = __shfl_sync(FULL, b_t0, sidx);
+          if (stats) { const uint32_t n = (uint32_t)__popc(__ballot_sync(FULL, have)); if (lane == 0) s_cnt[ST_WITEMS] += n; }
+          if (have) {
+            const float lb = __fsub_rn(__fadd_rn(it.a_min, __fadd_rn(e0lb, e1lb)), it.e_cur);
             const bool tbt_ok = c.O == 0 || it.l1_min <= c.slo_tbt;
-            const bool ttft_ok = c.L == 0 || __fadd_rn(it.t_avail_ms, bnd[DENSE_S + it.sm_free - 1]) <= c.slo_ttft;
+            const bool ttft_ok = c.L == 0 || __fadd_rn(it.t_avail_ms, t0lb) <= c.slo_ttft;
             if (tbt_ok && ttft_ok && lb < FS_INF) ordl = fs_orderable(lb);
             wk = it.k; wpk = (uint32_t)it.j | ((uint32_t)it.br1 << 8) | ((uint32_t)it.sm_free << 16);
             wta = it.t_avail_ms; wec = it.e_cur;
           }
+          ib += 32;
         }
-        ib += 32;
-      }
-      if (k == KNONE) break;                            // no feasible candidate at all
-      // a warm pair's context comes from the item its lane holds (the item passed the memory, bucket and
-      // share tests when it was listed); only the recovery of a cold winner reads the GPU's summary
-      PairCtx p;
-      if (wsrc >= 0) {
-        const uint32_t pk = __shfl_sync(0xffffffffu, wpk, wsrc);
-        p.ok = true; p.j = (int)(pk & 0xFFu); p.var = p.j + 1; p.br1 = (int)((pk >> 8) & 0xFFu); p.smf = (int)(pk >> 16);
-        p.wait = __shfl_sync(0xffffffffu, wta, wsrc); p.ecur = __shfl_sync(0xffffffffu, wec, wsrc);
-        p.rounds1 = fs_ceil_div(c.O, (uint32_t)p.br1 + 1u);
-      } else {
-        p = make_pair(v, c, v.ginfo[k]);
-      }
-      if (p.ok) {
-        if (STATS) { n_scored += 1; n_cscored += (uint32_t)(p.smf * d.F); }
-        const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
-        const LanePtr w_l1 = lane_ptr<NPHI>(l1 + cb0, phi0, Fc, vec), w_p1 = lane_ptr<NPHI>(p1 + cb0, phi0, Fc, vec);
-        const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F + cb0;
-        const float fr1 = __uint2float_rn(p.rounds1);
-        // an empty prefill / decode slot passes its deadline whatever the wait (slot rule, q == 0)
-        const float wait_e = c.L ? p.wait : 0.0f, ttft_e = c.L ? c.slo_ttft : FS_INF, tbt_e = c.O ? c.slo_tbt : FS_INF;
-        float ar[NPHI];
+        if (k == KNONE) break;                            // no feasible candidate at all, or a warm winner
+        // a warm pair's context comes from the item its lane holds (the item passed the memory, bucket and
+        // share tests when it was listed); only the recovery of a cold winner reads the GPU's summary
+        PairCtx p;
+        if (wsrc >= 0) {
+          const uint32_t pk = __shfl_sync(FULL, wpk, wsrc);
+          p.ok = true; p.j = (int)(pk & 0xFFu); p.var = p.j + 1; p.br1 = (int)((pk >> 8) & 0xFFu); p.smf = (int)(pk >> 16);
+          p.wait = __shfl_sync(FULL, wta, wsrc); p.ecur = __shfl_sync(FULL, wec, wsrc);
+          p.rounds1 = __shfl_sync(FULL, wr1, wsrc);
+        } else {
+          p = make_pair(v, c, v.ginfo[k]);
+        }
+        if (p.ok) {
+          if (stats && lane == 0) { s_cnt[ST_SCORED] += 1u; s_cnt[ST_CSCORED] += (uint32_t)(p.smf * d.F); }
+          const LaneLP w_lp1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, p.br1) + cb0, phi0, Fc);
+          const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F + cb0;
+          const float fr1 = __uint2float_rn(p.rounds1);
+          const float wait_e = c.L ? p.wait : 0.0f;
+          float ar[NPHI];
 #pragma unroll
-        for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < Fc ? Ar[phi0 + i] : FS_INF;
-        // four share rows per trip: their 12 plane loads are issued before any of them is used.  Each lane
-        // keeps the minimum of ITS candidates of this pair and the first (lowest flat) candidate attaining
-        // it; merged into the incumbent afterwards, or, in the recovery pass, matched against the winner's
-        // value (the pair's minimum by the definition equals what the sweep found: monotone rounding).
-        float pb = FS_INF; uint32_t pflat = NONE32;
+          for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < Fc ? Ar[phi0 + i] : FS_INF;
+          // four share rows per trip: their 8 plane loads are issued before any of them is used.  Each lane
+          // keeps the minimum of ITS candidates of this pair and the first (lowest flat) candidate attaining
+          // it; merged into the incumbent afterwards, or, in the recovery pass, matched against the winner's
+          // value (the pair's minimum by the definition equals what the sweep found: monotone rounding).
+          float pb = FS_INF; uint32_t pflat = NONE32;
+          const uint32_t flat0 = (uint32_t)(k * d.S * d.F + cb0 + phi0);
 #pragma unroll 1
-        for (int s4 = 0; s4 < p.smf; s4 += 4) {
-          float tt[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
+          for (int s4 = 0; s4 < p.smf; s4 += 4) {
+            float a0[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int sr = min(s4 + u, p.smf - 1);
-            const uint32_t ro = (uint32_t)(sr * d.F);
-            ld_lane<NPHI>(q_p0, ro, vec, b0[u]); ld_lane<NPHI>(w_l1, ro, vec, a1[u]); ld_lane<NPHI>(w_p1, ro, vec, b1[u]);
-            ld_tile<NPHI>(tl_t0 + sr * FT + phi0, tt[u]);
-          }
+            for (int u = 0; u < 4; ++u) {
+              const uint32_t ro = (uint32_t)(min(s4 + u, p.smf - 1) * d.F);
+              ld_lp<NPHI, VEC>(q_lp0, ro, a0[u], b0[u]); ld_lp<NPHI, VEC>(w_lp1, ro, a1[u], b1[u]);
+            }
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int s = s4 + u;
+            for (int u = 0; u < 4; ++u) {
+              const int s = s4 + u;
 #pragma unroll
-            for (int i = 0; i < NPHI; ++i) {
-              const float e0 = __fmul_rn(tt[u][i], b0[u][i]);
-              const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
-              const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   // -0 == +0 in every compare below
-              const bool ok = s < p.smf && __fadd_rn(wait_e, tt[u][i]) <= ttft_e && a1[u][i] <= tbt_e;
-              if (ok && dE < pb) { pb = dE; pflat = (uint32_t)((k * d.S + s) * d.F + cb0 + phi0 + i); }   // INF never enters
+              for (int i = 0; i < NPHI; ++i) {
+                const float t0 = __fmul_rn(fr0, a0[u][i]);
+                const float e0 = __fmul_rn(t0, b0[u][i]);
+                const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
+                const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   // -0 == +0 in every compare below
+                const bool ok = s < p.smf && __fadd_rn(wait_e, t0) <= ttft_e && a1[u][i] <= tbt_e;
+                if (ok && dE < pb) { pb = dE; pflat = flat0 + (uint32_t)(s * d.F + i); }   // INF never enters
+              }
             }
           }
+          if (recover) { if (pb == bestW) flat = pflat; }
+          else if (pb < best || (pb == best && k < bestk)) { best = pb; bestk = k; bflat = pflat; }
         }
-        if (recover) { if (pb == bestW) flat = pflat; }
-        else if (pb < best || (pb == best && k < bestk)) { best = pb; bestk = k; bflat = pflat; }
+        if (recover) break;
       }
-      if (recover) break;
+      key = flat != NONE32 ? fs_make_key(bestW, flat) : FS_KEY_NONE;
+      key = fs_warp_min_key(key);
     }
-    unsigned long long key = flat != NONE32 ? fs_make_key(bestW, flat) : FS_KEY_NONE;
-    key = fs_warp_min_key(key);
     if (COLS || out == nullptr) {                      // several slices / column blocks: merge by key, decode afterwards
       if (lane == 0 && key != FS_KEY_NONE) atomicMin(&keys[r], key);
     } else {
@@ -647,40 +578,45 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         // the winning GPU is known (kwin); one small division instead of three 32-bit ones
         const int ks = kwin, rem = (int)(fl - (uint32_t)(ks * d.S * d.F)), sgs = rem / d.F, phis = rem - sgs * d.F;
         const PairCtx p = make_pair(v, c, v.ginfo[ks]);
-        const float* l1 = v.latT + fs_plane(d, c.m, 1, p.br1); const float* p1 = v.powT + fs_plane(d, c.m, 1, p.br1);
+        const LaneLP q0 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 0, c.br0), phi0, d.F);
+        const LaneLP q1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, p.br1), phi0, d.F);
         const float* Ar = v.gA + ((size_t)ks * FS_NVAR + p.var) * d.F;
-        const float fr1 = __uint2float_rn(p.rounds1);
-        float tt[NPHI], b0[NPHI], a1[NPHI], b1[NPHI];
-        ld_tile<NPHI>(tl_t0 + sgs * FT + phi0, tt);
-        const LanePtr w_l1 = lane_ptr<NPHI>(l1, phi0, d.F, vec), w_p1 = lane_ptr<NPHI>(p1, phi0, d.F, vec);
+        const float fr0 = __uint2float_rn(c.rounds0), fr1 = __uint2float_rn(p.rounds1);
+        float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI];
         const uint32_t ro = (uint32_t)(sgs * d.F);
-        ld_lane<NPHI>(q_p0, ro, vec, b0); ld_lane<NPHI>(w_l1, ro, vec, a1); ld_lane<NPHI>(w_p1, ro, vec, b1);
+        ld_lp<NPHI, VEC>(q0, ro, a0, b0); ld_lp<NPHI, VEC>(q1, ro, a1, b1);
         uint32_t fmin = NONE32; float ttft = 0.0f, tbt = 0.0f;
 #pragma unroll
         for (int i = 0; i < NPHI; ++i) {
           const int phi = phi0 + i;
           const float ar = phi < d.F ? Ar[phi] : FS_INF;
-          const float dE = __fsub_rn(__fadd_rn(ar, __fadd_rn(__fmul_rn(tt[i], b0[i]), __fmul_rn(__fmul_rn(fr1, a1[i]), b1[i]))), p.ecur);
-          const bool ok = (c.L == 0 || __fadd_rn(p.wait, tt[i]) <= c.slo_ttft) && (c.O == 0 || a1[i] <= c.slo_tbt) && dE < FS_INF;
+          const float t0 = __fmul_rn(fr0, a0[i]);
+          const float dE = __fsub_rn(__fadd_rn(ar, __fadd_rn(__fmul_rn(t0, b0[i]), __fmul_rn(__fmul_rn(fr1, a1[i]), b1[i]))), p.ecur);
+          const bool ok = (c.L == 0 || __fadd_rn(p.wait, t0) <= c.slo_ttft) && (c.O == 0 || a1[i] <= c.slo_tbt) && dE < FS_INF;
           if (ok) fmin = min(fmin, (uint32_t)phi);
-          if (phi == phis) { ttft = __fadd_rn(p.wait, tt[i]); tbt = a1[i]; }
+          if (phi == phis) { ttft = __fadd_rn(p.wait, t0); tbt = a1[i]; }
         }
         fmin = warp_min_u32(fmin);
         const int owner = phis / NPHI;
-        ttft = __shfl_sync(0xffffffffu, ttft, owner); tbt = __shfl_sync(0xffffffffu, tbt, owner);
+        ttft = __shfl_sync(FULL, ttft, owner); tbt = __shfl_sync(FULL, tbt, owner);
         o.gpu = ks; o.sigma = (int16_t)sgs; o.phi = (int16_t)phis; o.beta = (int16_t)p.br1;
         o.f_req = (int16_t)(int)fmin; o.energy_mj = fs_unorderable((uint32_t)(key >> 32));
         o.ttft_ms = ttft; o.tbt_ms = tbt; o.flat = fl;
       }
       if (lane == 0) out[r] = o;
     }
-    if (STATS) { n_req += 1; }
-    if (STATS && __any_sync(0xffffffffu, ((n_chunks | n_elig | n_swept | n_cswept | n_witems | n_scored | n_cscored | n_req) >> 30) != 0u)) {
-      flush_stats(stats, n_chunks, n_elig, n_swept, n_cswept, n_witems, n_scored, n_cscored, n_req);
-      n_chunks = n_elig = n_swept = n_cswept = n_witems = n_scored = n_cscored = n_req = 0;
+    if (stats) {
+      __syncwarp();
+      if (lane < 8) { const uint32_t x = lane == ST_REQ ? 1u : s_cnt[lane]; if (x) atomicAdd(&stats[lane], (unsigned long long)x); s_cnt[lane] = 0u; }
+      __syncwarp();
     }
+    // ---- advance: the next request has landed in s_req
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
+    if (r_nxt < R) rq = *s_req;
+    __syncwarp();
+    r_cur = r_nxt; r_nxt = __shfl_sync(FULL, r_nn, 0);
   }
-  if (STATS) flush_stats(stats, n_chunks, n_elig, n_swept, n_cswept, n_witems, n_scored, n_cscored, n_req);
 }
 
 // ---- decode: key -> fs_placement (one warp per request, lanes over phi for f_req) ----------
@@ -750,7 +686,8 @@ __device__ __forceinline__ OwnEval own_eval_planes(const FsView& v, const ReqCtx
   const FsDimsDev& d = v.d;
   const size_t o = (size_t)sg * d.F + phi;
   const size_t i0 = fs_plane(d, c.m, 0, c.br0) + o, i1 = fs_plane(d, c.m, 1, br1) + o;
-  return own_eval_vals(c, rounds1, wait, v.latT[i0], v.powT[i0], v.latT[i1], v.powT[i1]);
+  const float2 a = v.lpT[i0], b = v.lpT[i1];
+  return own_eval_vals(c, rounds1, wait, a.x, a.y, b.x, b.y);
 }
 
 struct DispPair { bool ok; float e; };
@@ -849,27 +786,24 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
   if (!c.valid) { if (lane == 0 && sub == 0) { fs_raise(v.flag, FS_FLAG_REQUEST); out[r] = o; } return; }
   // ---- the request's cold tiles: t0 = fl(rounds0*LAT0), er = fl(e0 + e1) (INF where LAT1 > slo_tbt)
   if (use_tiles) {
-    const float* l0 = v.latT + fs_plane(d, c.m, 0, c.br0); const float* p0 = v.powT + fs_plane(d, c.m, 0, c.br0);
-    const float* l1 = v.latT + fs_plane(d, c.m, 1, 0);     const float* p1 = v.powT + fs_plane(d, c.m, 1, 0);
+    const float2* lp0 = v.lpT + fs_plane(d, c.m, 0, c.br0);   // {LAT, POW} planes: prefill bucket, decode bucket 0
+    const float2* lp1 = v.lpT + fs_plane(d, c.m, 1, 0);
     const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
     const float tbt = c.O > 0 ? c.slo_tbt : FS_INF;
-    const bool vec = NPHI == 2 && (d.F & 1) == 0;
     const int phi0 = lane * NPHI;
 #pragma unroll 2
     for (int s = sub; s < d.S; s += NW) {
-      float a0[NPHI], b0[NPHI], a1[NPHI], b1[NPHI], tt[NPHI], ee[NPHI];
       const int ofs = s * d.F;
-      ld_cols<NPHI>(l0, ofs, phi0, d.F, vec, a0); ld_cols<NPHI>(p0, ofs, phi0, d.F, vec, b0);
-      ld_cols<NPHI>(l1, ofs, phi0, d.F, vec, a1); ld_cols<NPHI>(p1, ofs, phi0, d.F, vec, b1);
 #pragma unroll
       for (int i = 0; i < NPHI; ++i) {
-        const float t = __fmul_rn(fr0, a0[i]);
-        const float e = __fadd_rn(__fmul_rn(t, b0[i]), __fmul_rn(__fmul_rn(fO, a1[i]), b1[i]));
         const bool in = (phi0 + i) < d.F;
-        tt[i] = in ? t : FS_INF;
-        ee[i] = (in && a1[i] <= tbt) ? e : FS_INF;
+        const int col = min(phi0 + i, d.F - 1);
+        const float2 x0 = lp0[ofs + col], x1 = lp1[ofs + col];
+        const float t = __fmul_rn(fr0, x0.x);
+        const float e = __fadd_rn(__fmul_rn(t, x0.y), __fmul_rn(__fmul_rn(fO, x1.x), x1.y));
+        tl_t0[s * FT + phi0 + i] = in ? t : FS_INF;
+        tl_er[s * FT + phi0 + i] = (in && x1.x <= tbt) ? e : FS_INF;
       }
-      st_tile<NPHI>(tl_t0 + s * FT + phi0, tt); st_tile<NPHI>(tl_er + s * FT + phi0, ee);
     }
     if (BLOCK) __syncthreads(); else __syncwarp();
   }
@@ -901,7 +835,10 @@ __global__ void __launch_bounds__(DISP_WARPS * 32) dispatch_kernel(FsView v, int
     for (int u = 0; u < DISP_NC; ++u) if ((gj >> 5) == u && (gj & 31) == lane) cmin[u] = cm;
     emin_o = min(emin_o, cm);
   }
-  const int wb0 = use_tiles ? warm_off[c.m] : 0, wb1 = use_tiles ? warm_off[c.m + 1] : 0;
+  // no GPUs (K = 0): the warm lists were not rebuilt for this state (they may hold the previous poll's items, or
+  // nothing at all on a fresh context) and must not be read
+  const bool warm = use_tiles && v.K > 0;
+  const int wb0 = warm ? warm_off[c.m] : 0, wb1 = warm ? warm_off[c.m + 1] : 0;
   for (int ib = wb0 + sub * 32; ib < wb1; ib += 32 * NW) {
     uint32_t eo = 0xFFFFFFFFu;
     if (ib + lane < wb1) {
@@ -1168,7 +1105,8 @@ __device__ __forceinline__ CmPre cm_preload(const FsView& v, const ReqCtx& c, co
   const FsDimsDev& d = v.d;
   const size_t o = (size_t)(gi.sm_free - 1) * d.F + gi.f_cur;
   const size_t i0 = fs_plane(d, c.m, 0, c.br0) + o, i1 = fs_plane(d, c.m, 1, p.br1) + o;
-  q.l0 = v.latT[i0]; q.p0 = v.powT[i0]; q.l1 = v.latT[i1]; q.p1 = v.powT[i1]; q.phi = gi.f_cur;
+  const float2 a = v.lpT[i0], b = v.lpT[i1];
+  q.l0 = a.x; q.p0 = a.y; q.l1 = b.x; q.p1 = b.y; q.phi = gi.f_cur;
   return q;
 }
 
@@ -1305,13 +1243,10 @@ __global__ void __launch_bounds__(CMR_THREADS) dispatch_commit_reg_kernel(FsView
 
 int fsk_place_smem_attr() {
   int e = 0;
-#define FS_ATTR_DENSE(NP, VC, ST, CL) \
-  e |= (int)cudaFuncSetAttribute(place_dense_kernel<NP, VC, ST, CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX)
-  FS_ATTR_DENSE(1, false, false, false); FS_ATTR_DENSE(1, false, true, false);
-  FS_ATTR_DENSE(2, false, false, false); FS_ATTR_DENSE(2, false, true, false);
-  FS_ATTR_DENSE(2, true, false, false);  FS_ATTR_DENSE(2, true, true, false);
-  FS_ATTR_DENSE(2, false, false, true);  FS_ATTR_DENSE(2, false, true, true);
-  FS_ATTR_DENSE(2, true, false, true);   FS_ATTR_DENSE(2, true, true, true);
+#define FS_ATTR_DENSE(NP, VC, CL) \
+  e |= (int)cudaFuncSetAttribute(place_dense_kernel<NP, VC, CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, DENSE_SMEM_MAX)
+  FS_ATTR_DENSE(1, false, false); FS_ATTR_DENSE(2, false, false); FS_ATTR_DENSE(2, true, false);
+  FS_ATTR_DENSE(2, false, true);  FS_ATTR_DENSE(2, true, true);
 #undef FS_ATTR_DENSE
   e |= (int)cudaFuncSetAttribute(dispatch_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 32 * 4);
   e |= (int)cudaFuncSetAttribute(dispatch_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DISP_WARPS * 2 * FS_MAX_S * 64 * 4);
@@ -1328,63 +1263,42 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
     return 1;
   }
-  const bool dense_ok = v.d.S <= DENSE_S && v.d.F <= FS_MAX_F && !sc.force_generic;
   fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
-  if (dense_ok) {
-    // one persistent block per SM; each holds a slice of the sorted GPU records in shared memory
-    // beside its warps' tiles.  Warps per block: as many as fit (registers cap them at DENSE_MAXW),
-    // fewer when R alone cannot occupy every SM; the number of slices is what the slice size
-    // forces, raised when the request batches alone cannot occupy every SM.
-    const int FT = v.d.F <= 32 ? 32 : 64;
-    const int ncb = (v.d.F + 63) / 64;                 // column blocks of 64 frequencies (1 unless F > 64)
-    const int nchunk = v.Kpad / FS_CHUNK;
-    const size_t pw = dense_warp_bytes(v.d.S, FT), per_chunk = (size_t)FS_CHUNK * sizeof(FsGpuRec);
-    int W = (int)((DENSE_SMEM_MAX - 16 - (size_t)min(nchunk, 64) * per_chunk) / pw);
-    W = max(1, min(min(DENSE_MAXW, W), (R + sc.sm_count - 1) / sc.sm_count));
-    const int max_cps = (int)((DENSE_SMEM_MAX - 16 - (size_t)W * pw) / per_chunk);
-    int nslice = (nchunk + max_cps - 1) / max_cps;
-    const int nbatch = (R + W - 1) / W;
-    if (nbatch * nslice * ncb < sc.sm_count) nslice = min(nchunk, max(nslice, (sc.sm_count + nbatch * ncb - 1) / (nbatch * ncb)));
-    const int cps = (nchunk + nslice - 1) / nslice;
-    nslice = (nchunk + cps - 1) / cps;
-    const int nsc = nslice * ncb;
-    const int streams = max(1, min(nbatch, sc.sm_count / nsc));
-    const int grid = streams * nsc;
-    const size_t smem = dense_smem_bytes(cps * FS_CHUNK, W, v.d.S, FT);
-    cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nsc, st);
-    // one slice: the scoring kernel writes the placement records itself (no key array, no decode launch)
-    fs_placement* direct = nsc == 1 ? out : nullptr;
-    if (!direct) cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-#define FS_LAUNCH_DENSE(NP, VC, ST, CL) \
-  place_dense_kernel<NP, VC, ST, CL><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, ncb, cps, sc.ctr, sc.warm_off, sc.witems, sc.stats, direct)
-    const bool vec = FT == 64 && (v.d.F & 1) == 0;
-    if (FT == 32)      { if (sc.count_work) FS_LAUNCH_DENSE(1, false, true, false); else FS_LAUNCH_DENSE(1, false, false, false); }
-    else if (ncb == 1) {
-      if (vec) { if (sc.count_work) FS_LAUNCH_DENSE(2, true, true, false);  else FS_LAUNCH_DENSE(2, true, false, false); }
-      else     { if (sc.count_work) FS_LAUNCH_DENSE(2, false, true, false); else FS_LAUNCH_DENSE(2, false, false, false); }
-    } else {
-      if (vec) { if (sc.count_work) FS_LAUNCH_DENSE(2, true, true, true);  else FS_LAUNCH_DENSE(2, true, false, true); }
-      else     { if (sc.count_work) FS_LAUNCH_DENSE(2, false, true, true); else FS_LAUNCH_DENSE(2, false, false, true); }
-    }
+  // one persistent block per SM; each holds a slice of the sorted GPU records in shared memory
+  // beside its warps' tiles.  Warps per block: as many as fit (registers cap them at DENSE_MAXW),
+  // fewer when R alone cannot occupy every SM; the number of slices is what the slice size
+  // forces, raised when the request batches alone cannot occupy every SM.
+  const int FT = v.d.F <= 32 ? 32 : 64;
+  const int ncb = (v.d.F + 63) / 64;                 // column blocks of 64 frequencies (1 unless F > 64)
+  const int nchunk = v.Kpad / FS_CHUNK;
+  const size_t pw = dense_warp_bytes(v.d.S, FT), per_chunk = (size_t)FS_CHUNK * sizeof(FsGpuRec);
+  int W = (int)((DENSE_SMEM_MAX - 16 - (size_t)min(nchunk, 64) * per_chunk) / pw);
+  W = max(1, min(min(DENSE_MAXW, W), (R + sc.sm_count - 1) / sc.sm_count));
+  const int max_cps = (int)((DENSE_SMEM_MAX - 16 - (size_t)W * pw) / per_chunk);
+  int nslice = (nchunk + max_cps - 1) / max_cps;
+  const int nbatch = (R + W - 1) / W;
+  if (nbatch * nslice * ncb < sc.sm_count) nslice = min(nchunk, max(nslice, (sc.sm_count + nbatch * ncb - 1) / (nbatch * ncb)));
+  const int cps = (nchunk + nslice - 1) / nslice;
+  nslice = (nchunk + cps - 1) / cps;
+  const int nsc = nslice * ncb;
+  const int streams = max(1, min(nbatch, sc.sm_count / nsc));
+  const int grid = streams * nsc;
+  const size_t smem = dense_smem_bytes(cps * FS_CHUNK, W, v.d.S, FT);
+  cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nsc, st);
+  // one slice: the scoring kernel writes the placement records itself (no key array, no decode launch)
+  fs_placement* direct = nsc == 1 ? out : nullptr;
+  if (!direct) cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
+  unsigned long long* stats = sc.count_work ? sc.stats : nullptr;
+#define FS_LAUNCH_DENSE(NP, VC, CL) \
+  place_dense_kernel<NP, VC, CL><<<grid, W * 32, smem, st>>>(v, R, reqs, sc.keys, nslice, ncb, cps, sc.ctr, sc.warm_off, sc.witems, stats, direct)
+  const bool vec = FT == 64 && (v.d.F & 1) == 0;
+  if (FT == 32) FS_LAUNCH_DENSE(1, false, false);
+  else if (ncb == 1) { if (vec) FS_LAUNCH_DENSE(2, true, false); else FS_LAUNCH_DENSE(2, false, false); }
+  else               { if (vec) FS_LAUNCH_DENSE(2, true, true);  else FS_LAUNCH_DENSE(2, false, true); }
 #undef FS_LAUNCH_DENSE
-    ++launches;
-    fs_tm_end(tm, FS_T_PLACE_SCORE, st);
-    if (direct) return launches;
-  } else {
-    cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
-    // split the GPUs of one request over several warps when R alone cannot fill the SMs
-    const long long want_warps = (long long)sc.sm_count * 32;
-    int nsplit = 1;
-    if (R < want_warps) nsplit = (int)((want_warps + R - 1) / R);
-    if (nsplit > v.K) nsplit = v.K;
-    const int kchunk = (v.K + nsplit - 1) / nsplit;
-    nsplit = (v.K + kchunk - 1) / kchunk;
-    const long long warps = (long long)R * nsplit;
-    place_generic_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(v, R, reqs, sc.keys, nsplit,
-                                                                     kchunk, sc.count_work ? sc.stats : nullptr);
-    ++launches;
-    fs_tm_end(tm, FS_T_PLACE_SCORE, st);
-  }
+  ++launches;
+  fs_tm_end(tm, FS_T_PLACE_SCORE, st);
+  if (direct) return launches;
   fs_tm_beg(tm, FS_T_PLACE_DECODE, st);
   place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);
   fs_tm_end(tm, FS_T_PLACE_DECODE, st);

@@ -89,9 +89,8 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
     for (int i = 0; i < FS_RMAX; ++i) {
       l0[i] = p0[i] = l1[i] = p1[i] = l1b[i] = p1b[i] = 1.0f;
       if (i < n) {
-        l0[i] = v.latT[o0[i] + pc]; p0[i] = v.powT[o0[i] + pc];
-        l1[i] = v.latT[o1[i] + pc]; p1[i] = v.powT[o1[i] + pc];
-        l1b[i] = v.latT[o1b[i] + pc]; p1b[i] = v.powT[o1b[i] + pc];
+        const float2 a = v.lpT[o0[i] + pc], b = v.lpT[o1[i] + pc], c = v.lpT[o1b[i] + pc];
+        l0[i] = a.x; p0[i] = a.y; l1[i] = b.x; p1[i] = b.y; l1b[i] = c.x; p1b[i] = c.y;
       }
     }
     float e_plain[FS_RMAX], e_bump[FS_RMAX]; bool ok_plain[FS_RMAX], ok_bump[FS_RMAX];
@@ -280,19 +279,20 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
   for (int j = 0; j < i; ++j) if (gi.model[j] == gi.model[i]) return;   // not the join target
   const FsDimsDev d = v.d;
   const int m = gi.model[i], br1 = gi.br1[i];
-  float a_min = FS_INF, l1 = FS_INF, p1 = FS_INF;
+  float a_min = FS_INF;
+  FsPlaneMin pm; pm.lp = (double)FS_INF; pm.lmin = FS_INF; pm.pmax = 0.0f;
   for (int phi = lane; phi < d.F; phi += 32) a_min = fminf(a_min, v.gA[((size_t)k * FS_NVAR + 1 + i) * d.F + phi]);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
   if (br1 >= 0 && gi.sm_free >= 1) {                   // minima over shares < sm_free, all phi: one lookup
-    const float2 mn = v.dmin[((size_t)m * d.B + br1) * d.S + gi.sm_free - 1];
-    l1 = mn.x; p1 = mn.y;
+    pm = v.pmin[(((size_t)m * 2 + 1) * d.B + br1) * d.S + gi.sm_free - 1];
   }
   if (lane == 0) {
     FsWarmItem it;
     it.k = k; it.j = i; it.br1 = br1; it.sm_free = gi.sm_free;
     it.t_avail_ms = gi.t_avail_ms; it.mem_free_mb = gi.mem_free_mb; it.e_cur = gi.e_cur;
-    it.a_min = a_min; it.l1_min = l1; it.p1_min = p1; it.f_cur = gi.f_cur; it._pad = 0;
+    it.a_min = a_min; it.lp1 = pm.lp; it.l1_min = pm.lmin; it.p1_max = pm.pmax; it.f_cur = gi.f_cur;
+    it.magic = fs_magic((uint32_t)max(br1, 0) + 1u); it._pad[0] = it._pad[1] = 0;
     items[off[m] + atomicAdd(&cursor[m], 1)] = it;
   }
 }

@@ -1,6 +1,7 @@
 // fs_tables.cu — fs_load_profiles device work: validate the LUT and build the
-// plane layout [M][2][B][S][F] in which the (sigma,phi) plane of one (model, phase, batch
-// bucket) is one contiguous S*F*4-byte block (what placement stages per request).
+// plane layout [M][2][B][S][F] of {LAT, POW} pairs in which the (sigma,phi) plane of one (model,
+// phase, batch bucket) is one contiguous S*F*8-byte block (what placement stages per request with
+// one TMA bulk copy), and the per-plane prefix minima the placement bounds are made of.
 #include "fs_kernels.h"
 
 namespace {
@@ -9,8 +10,7 @@ namespace {
 // tables.  Reads are coalesced along beta, writes along phi.
 __global__ void __launch_bounds__(256) build_planes_kernel(const float* __restrict__ lat,
                                                           const float* __restrict__ pow,
-                                                          float* __restrict__ latT,
-                                                          float* __restrict__ powT, FsDimsDev d,
+                                                          float2* __restrict__ lpT, FsDimsDev d,
                                                           int* flag) {
   __shared__ float tl[32][33];
   __shared__ float tp[32][33];
@@ -38,41 +38,45 @@ __global__ void __launch_bounds__(256) build_planes_kernel(const float* __restri
     const int b = tb * 32 + r, f = tf * 32 + tx;
     if (f < d.F && b < d.B) {
       const size_t o = (((size_t)mp * d.B + b) * d.S + s) * d.F + f;
-      latT[o] = tl[tx][r];
-      powT[o] = tp[tx][r];
+      lpT[o] = make_float2(tl[tx][r], tp[tx][r]);
     }
   }
   if (bad) fs_raise(flag, FS_FLAG_TABLE);
 }
 
-// dmin[m][b][s] = { min LAT, min POW } of the decode plane (m, 1, b) over shares <= s and all phi: the
-// bounds l1_min / p1_min of a warm (GPU, slot) item are then one lookup at (model, bucket, sm_free - 1)
-__global__ void __launch_bounds__(128) decode_min_kernel(const float* __restrict__ latT, const float* __restrict__ powT,
-                                                        FsDimsDev d, float2* __restrict__ dmin) {
+// pmin[m][p][b][s] over the plane (m, p, b), shares <= s and all phi: the minimum of the exact product
+// LAT*POW (binary64 holds the product of two binary32 values exactly), the minimum LAT and the maximum POW.
+// fs_energy_lb (fs_common.cuh) turns them into a lower bound on fl(fl(rounds*LAT)*POW) of every such entry.
+__global__ void __launch_bounds__(128) plane_min_kernel(const float2* __restrict__ lpT, FsDimsDev d,
+                                                       FsPlaneMin* __restrict__ pmin) {
   const int lane = threadIdx.x & 31;
-  const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (w >= d.M * d.B) return;
-  const int m = w / d.B, b = w % d.B;
-  const float* pl = latT + fs_plane(d, m, 1, b); const float* pp = powT + fs_plane(d, m, 1, b);
-  float ml = FS_INF, mp = FS_INF;
+  const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);     // (m*2+p)*B + b
+  if (w >= d.M * 2 * d.B) return;
+  const float2* pl = lpT + (size_t)w * d.S * d.F;
+  double mlp = (double)FS_INF; float ml = FS_INF, xp = 0.0f;
   for (int s = 0; s < d.S; ++s) {
-    float l = FS_INF, p = FS_INF;
-    for (int phi = lane; phi < d.F; phi += 32) { l = fminf(l, pl[s * d.F + phi]); p = fminf(p, pp[s * d.F + phi]); }
+    double lp = (double)FS_INF; float l = FS_INF, p = 0.0f;
+    for (int phi = lane; phi < d.F; phi += 32) {
+      const float2 e = pl[s * d.F + phi];
+      const double pr = (double)e.x * (double)e.y;
+      lp = pr < lp ? pr : lp; l = fminf(l, e.x); p = fmaxf(p, e.y);
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      l = fminf(l, __shfl_xor_sync(0xffffffffu, l, o)); p = fminf(p, __shfl_xor_sync(0xffffffffu, p, o));
+      const double u = __shfl_xor_sync(0xffffffffu, lp, o); lp = u < lp ? u : lp;
+      l = fminf(l, __shfl_xor_sync(0xffffffffu, l, o)); p = fmaxf(p, __shfl_xor_sync(0xffffffffu, p, o));
     }
-    ml = fminf(ml, l); mp = fminf(mp, p);
-    if (lane == 0) dmin[(size_t)w * d.S + s] = make_float2(ml, mp);
+    mlp = lp < mlp ? lp : mlp; ml = fminf(ml, l); xp = fmaxf(xp, p);
+    if (lane == 0) { FsPlaneMin o; o.lp = mlp; o.lmin = ml; o.pmax = xp; pmin[(size_t)w * d.S + s] = o; }
   }
 }
 
 }  // namespace
 
-int fsk_build_planes(const float* lat, const float* pow, float* latT, float* powT, float2* dmin, FsDimsDev d,
+int fsk_build_planes(const float* lat, const float* pow, float2* lpT, FsPlaneMin* pmin, FsDimsDev d,
                      int* flag, cudaStream_t st) {
   const long long blocks = (long long)d.M * 2 * d.S * ((d.F + 31) / 32) * ((d.B + 31) / 32);
-  build_planes_kernel<<<(unsigned)blocks, 256, 0, st>>>(lat, pow, latT, powT, d, flag);
-  decode_min_kernel<<<(d.M * d.B + 3) / 4, 128, 0, st>>>(latT, powT, d, dmin);
+  build_planes_kernel<<<(unsigned)blocks, 256, 0, st>>>(lat, pow, lpT, d, flag);
+  plane_min_kernel<<<(d.M * 2 * d.B + 3) / 4, 128, 0, st>>>(lpT, d, pmin);
   return 2;
 }
