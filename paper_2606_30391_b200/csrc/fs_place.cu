@@ -114,7 +114,7 @@ __device__ __forceinline__ Cand eval_cand(const FsView& v, const ReqCtx& c, cons
 //      the minimum, and (one slice) writes the placement record.
 // All loops are rolled so that the kernel stays inside the instruction cache.
 // =============================================================================================
-constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102)
+constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102 -> 96)
 constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
 constexpr int DENSE_S = FS_MAX_S;
 
@@ -162,16 +162,17 @@ __device__ __forceinline__ float fs_tstar(float w, float slo) {
   return tstar_bisect(w, slo);
 }
 
-// Shared memory of one block:
-//   rec  [KS]          the block's slice of the SORTED compact GPU records (one TMA fill)
-//   per warp:  tile [S][FT] of {t0, er} pairs (the prefill plane {LAT0, POW0} lands here first),
-//              wb [32] {T*, Ecur, sm_free, GPU} of the chunk's survivors, the next request (32 B),
-//              the warp's mbarrier, 8 work counters
+// Shared memory of one block, per warp:  wb [32] {T*, Ecur, sm_free, GPU} of the chunk's survivors, the next
+// request (32 B), the warp's mbarrier, 8 work counters, then the tile [S][FT] of {t0, er} pairs (the prefill
+// plane {LAT0, POW0} lands there first, by one TMA bulk copy, when the request has cold pairs to sweep).
+// The sorted compact GPU records are streamed from global memory (L2) with two 128-bit loads per lane and
+// chunk: at pod a request looks at 0.3 chunks.
+constexpr int DENSE_WB_OFF = 0, DENSE_REQ_OFF = 512, DENSE_BAR_OFF = 544, DENSE_CNT_OFF = 560, DENSE_TILE_OFF = 640;
 __host__ __device__ inline size_t dense_warp_bytes(int S, int FT) {
-  return (size_t)S * FT * sizeof(float2) + FS_CHUNK * sizeof(float4) + sizeof(fs_request) + 16 + 32;
+  return (size_t)DENSE_TILE_OFF + (size_t)S * FT * sizeof(float2);
 }
-__host__ __device__ inline size_t dense_smem_bytes(int KS, int W, int S, int FT) {
-  return (size_t)KS * sizeof(FsGpuRec) + (size_t)W * dense_warp_bytes(S, FT) + 16;
+__host__ __device__ inline size_t dense_smem_bytes(int W, int S, int FT) {
+  return (size_t)W * dense_warp_bytes(S, FT);
 }
 
 // The lane's NPHI adjacent {LAT, POW} entries of a plane row.  Pointers already include the lane's column
@@ -223,7 +224,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   constexpr uint32_t NONE32 = 0xFFFFFFFFu, INFBITS = 0x7F800000u, FULL = 0xffffffffu;
   constexpr int KNONE = 0x7FFFFFFF;
   const FsDimsDev d = v.d;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int nchunk_all = v.Kpad / FS_CHUNK;
   const int nsc = COLS ? nslice * ncb : nslice;         // (slice, column block) combinations
   const int sci = blockIdx.x % nsc;
@@ -231,31 +232,16 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const int cb0 = COLS ? (sci / nslice) * 64 : 0;        // first frequency of this block's columns
   const int FA = COLS ? v.FT : FT;                       // row stride of gA0 (F rounded up to 64 when F > 64)
   const int c0 = slice * chunks_per_slice, c1 = min(nchunk_all, c0 + chunks_per_slice);
-  const int nchunk = c1 - c0, KS = nchunk * FS_CHUNK, KSmax = chunks_per_slice * FS_CHUNK;
-  FsGpuRec* s_rec = reinterpret_cast<FsGpuRec*>(dense_smem_raw);
-  unsigned char* s_warp = dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec) + (size_t)warp * dense_warp_bytes(d.S, FT);
-  float2* tile = reinterpret_cast<float2*>(s_warp);
-  float4* wb = reinterpret_cast<float4*>(tile + d.S * FT);
-  fs_request* s_req = reinterpret_cast<fs_request*>(wb + FS_CHUNK);
-  uint64_t* w_bar = reinterpret_cast<uint64_t*>(s_req + 1);
-  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(w_bar + 2);
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(dense_smem_raw + (size_t)KSmax * sizeof(FsGpuRec) +
-                                                (size_t)W * dense_warp_bytes(d.S, FT));
-
-  // ---- stage this block's slice of the SORTED GPU records once: 1-D TMA bulk copies on one mbarrier
-  if (threadIdx.x == 0) fs_mbar_init(s_bar, 1);
-  if (lane == 0) { fs_mbar_init(w_bar, 1); if (stats) { for (int i = 0; i < 8; ++i) s_cnt[i] = 0u; } }
-  if (threadIdx.x == 0) fs_mbar_fence_init();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    const uint32_t bytes_rec = (uint32_t)KS * sizeof(FsGpuRec);
-    fs_mbar_expect_tx(s_bar, bytes_rec);
-    const char* src = reinterpret_cast<const char*>(v.gsort + (size_t)c0 * FS_CHUNK);
-    char* dst = reinterpret_cast<char*>(s_rec);
-    for (uint32_t off = 0; off < bytes_rec; off += 32768u)
-      fs_tma_load_1d(dst + off, src + off, min(32768u, bytes_rec - off), s_bar);
-  }
-  fs_mbar_wait(s_bar, 0);
+  const int nchunk = c1 - c0;
+  const FsGpuRec* __restrict__ g_rec = v.gsort + (size_t)c0 * FS_CHUNK;     // this block's slice of the SORTED records
+  unsigned char* s_warp = dense_smem_raw + (size_t)warp * dense_warp_bytes(d.S, FT);
+  float4* wb = reinterpret_cast<float4*>(s_warp + DENSE_WB_OFF);
+  fs_request* s_req = reinterpret_cast<fs_request*>(s_warp + DENSE_REQ_OFF);
+  uint64_t* w_bar = reinterpret_cast<uint64_t*>(s_warp + DENSE_BAR_OFF);
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp + DENSE_CNT_OFF);
+  float2* tile = reinterpret_cast<float2*>(s_warp + DENSE_TILE_OFF);
+  if (lane == 0) { fs_mbar_init(w_bar, 1); fs_mbar_fence_init(); if (stats) { for (int i = 0; i < 8; ++i) s_cnt[i] = 0u; } }
+  __syncwarp();
 
   const double* dsuf = v.dsuf + 1 + c0;
   const double amax = v.dsuf[0];
@@ -361,12 +347,11 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                 // generic-proxy accesses of the last request's tile are ordered before the async-proxy writes
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
-                if (lane == 0) {
-                  const float2* src = v.lpT + fs_plane(d, c.m, 0, c.br0) + cb0;
-                  fs_mbar_expect_tx(w_bar, (uint32_t)(d.S * ncol) * 8u);
-                  if (ncol == FT && d.F == FT) fs_tma_load_1d(tile, src, (uint32_t)(d.S * FT) * 8u, w_bar);
-                  else for (int s = 0; s < d.S; ++s) fs_tma_load_1d(tile + s * FT, src + (size_t)s * d.F, (uint32_t)ncol * 8u, w_bar);
-                }
+                const float2* src = v.lpT + fs_plane(d, c.m, 0, c.br0) + cb0;
+                if (lane == 0) fs_mbar_expect_tx(w_bar, (uint32_t)(d.S * ncol) * 8u);
+                __syncwarp();
+                if (ncol == FT && d.F == FT) { if (lane == 0) fs_tma_load_1d(tile, src, (uint32_t)(d.S * FT) * 8u, w_bar); }
+                else if (lane < d.S) fs_tma_load_1d(tile + lane * FT, src + (size_t)lane * d.F, (uint32_t)ncol * 8u, w_bar);
               } else {
                 uint32_t dt = fs_smem_u32(tile + phi0);
                 LaneLP g = q_lp0;
@@ -422,7 +407,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
                   if (x - 0x1p-22 * (amax + bmin + fabs(x)) - 1e-37 > (double)incW) break;
                 }
                 // ---- eligibility + bound: lane <-> one GPU of the chunk ---------------------------------
-                const FsGpuRec g = s_rec[ci * FS_CHUNK + lane];
+                const FsGpuRec g = g_rec[ci * FS_CHUNK + lane];
                 const int smf = (g.meta >> 8) & 0xFF;              // >= 1 (sentinels included)
                 const uint32_t mm = (uint32_t)c.m * 0x00010001u;
                 const uint32_t* gm = reinterpret_cast<const uint32_t*>(g.model);
@@ -529,34 +514,43 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           float ar[NPHI];
 #pragma unroll
           for (int i = 0; i < NPHI; ++i) ar[i] = (phi0 + i) < Fc ? Ar[phi0 + i] : FS_INF;
-          // four share rows per trip: their 8 plane loads are issued before any of them is used.  Each lane
-          // keeps the minimum of ITS candidates of this pair and the first (lowest flat) candidate attaining
-          // it; merged into the incumbent afterwards, or, in the recovery pass, matched against the winner's
-          // value (the pair's minimum by the definition equals what the sweep found: monotone rounding).
+          // two share rows per stage, software-pipelined: the four plane loads of the NEXT stage are issued
+          // before the current one is scored, so a stage's latency hides behind the arithmetic of the one
+          // before it.  Each lane keeps the minimum of ITS candidates of this pair and the first (lowest flat)
+          // candidate attaining it; merged into the incumbent afterwards, or, in the recovery pass, matched
+          // against the winner's value (the pair's minimum by the definition equals what the sweep found:
+          // monotone rounding).
           float pb = FS_INF; uint32_t pflat = NONE32;
           const uint32_t flat0 = (uint32_t)(k * d.S * d.F + cb0 + phi0);
+          float a0[2][2][NPHI], b0[2][2][NPHI], a1[2][2][NPHI], b1[2][2][NPHI];   // [stage buffer][row][phi]
+#define FS_BODY_LOAD(BUF, S0)                                                                          \
+  _Pragma("unroll") for (int u = 0; u < 2; ++u) {                                                      \
+    const uint32_t ro = (uint32_t)(min((S0) + u, p.smf - 1) * d.F);                                    \
+    ld_lp<NPHI, VEC>(q_lp0, ro, a0[BUF][u], b0[BUF][u]); ld_lp<NPHI, VEC>(w_lp1, ro, a1[BUF][u], b1[BUF][u]); \
+  }
+#define FS_BODY_SCORE(BUF, S0)                                                                         \
+  _Pragma("unroll") for (int u = 0; u < 2; ++u) {                                                      \
+    const int s = (S0) + u;                                                                            \
+    _Pragma("unroll") for (int i = 0; i < NPHI; ++i) {                                                 \
+      const float t0 = __fmul_rn(fr0, a0[BUF][u][i]);                                                  \
+      const float e0 = __fmul_rn(t0, b0[BUF][u][i]);                                                   \
+      const float e1 = __fmul_rn(__fmul_rn(fr1, a1[BUF][u][i]), b1[BUF][u][i]);                        \
+      const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   /* -0 == +0 in every compare below */ \
+      const bool ok = s < p.smf && __fadd_rn(wait_e, t0) <= ttft_e && a1[BUF][u][i] <= tbt_e;          \
+      if (ok && dE < pb) { pb = dE; pflat = flat0 + (uint32_t)(s * d.F + i); }   /* INF never enters */ \
+    }                                                                                                  \
+  }
+          FS_BODY_LOAD(0, 0)
 #pragma unroll 1
           for (int s4 = 0; s4 < p.smf; s4 += 4) {
-            float a0[4][NPHI], b0[4][NPHI], a1[4][NPHI], b1[4][NPHI];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-              const uint32_t ro = (uint32_t)(min(s4 + u, p.smf - 1) * d.F);
-              ld_lp<NPHI, VEC>(q_lp0, ro, a0[u], b0[u]); ld_lp<NPHI, VEC>(w_lp1, ro, a1[u], b1[u]);
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-              const int s = s4 + u;
-#pragma unroll
-              for (int i = 0; i < NPHI; ++i) {
-                const float t0 = __fmul_rn(fr0, a0[u][i]);
-                const float e0 = __fmul_rn(t0, b0[u][i]);
-                const float e1 = __fmul_rn(__fmul_rn(fr1, a1[u][i]), b1[u][i]);
-                const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   // -0 == +0 in every compare below
-                const bool ok = s < p.smf && __fadd_rn(wait_e, t0) <= ttft_e && a1[u][i] <= tbt_e;
-                if (ok && dE < pb) { pb = dE; pflat = flat0 + (uint32_t)(s * d.F + i); }   // INF never enters
-              }
-            }
+            FS_BODY_LOAD(1, s4 + 2)
+            FS_BODY_SCORE(0, s4)
+            if (s4 + 2 >= p.smf) break;
+            FS_BODY_LOAD(0, s4 + 4)
+            FS_BODY_SCORE(1, s4 + 2)
           }
+#undef FS_BODY_LOAD
+#undef FS_BODY_SCORE
           if (recover) { if (pb == bestW) flat = pflat; }
           else if (pb < best || (pb == best && k < bestk)) { best = pb; bestk = k; bflat = pflat; }
         }
@@ -615,7 +609,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     __syncwarp();
     if (r_nxt < R) rq = *s_req;
     __syncwarp();
-    r_cur = r_nxt; r_nxt = __shfl_sync(FULL, r_nn, 0);
+    r_cur = r_nxt;
+    asm volatile("shfl.sync.idx.b32 %0, %1, 0, 31, 0xffffffff;" : "=r"(r_nxt) : "r"(r_nn) : "memory");
   }
 }
 
@@ -1264,26 +1259,24 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
     return 1;
   }
   fs_tm_beg(tm, FS_T_PLACE_SCORE, st);
-  // one persistent block per SM; each holds a slice of the sorted GPU records in shared memory
-  // beside its warps' tiles.  Warps per block: as many as fit (registers cap them at DENSE_MAXW),
-  // fewer when R alone cannot occupy every SM; the number of slices is what the slice size
-  // forces, raised when the request batches alone cannot occupy every SM.
+  // one persistent block per SM.  Warps per block: as many as fit (shared memory: one tile per warp;
+  // registers cap them at DENSE_MAXW), fewer when R alone cannot occupy every SM.
   const int FT = v.d.F <= 32 ? 32 : 64;
   const int ncb = (v.d.F + 63) / 64;                 // column blocks of 64 frequencies (1 unless F > 64)
   const int nchunk = v.Kpad / FS_CHUNK;
-  const size_t pw = dense_warp_bytes(v.d.S, FT), per_chunk = (size_t)FS_CHUNK * sizeof(FsGpuRec);
-  int W = (int)((DENSE_SMEM_MAX - 16 - (size_t)min(nchunk, 64) * per_chunk) / pw);
+  const size_t pw = dense_warp_bytes(v.d.S, FT);
+  int W = (int)(DENSE_SMEM_MAX / pw);
   W = max(1, min(min(DENSE_MAXW, W), (R + sc.sm_count - 1) / sc.sm_count));
-  const int max_cps = (int)((DENSE_SMEM_MAX - 16 - (size_t)W * pw) / per_chunk);
-  int nslice = (nchunk + max_cps - 1) / max_cps;
+  // the GPUs are cut into slices only when the requests alone cannot occupy every SM
+  int nslice = 1;
   const int nbatch = (R + W - 1) / W;
-  if (nbatch * nslice * ncb < sc.sm_count) nslice = min(nchunk, max(nslice, (sc.sm_count + nbatch * ncb - 1) / (nbatch * ncb)));
+  if (nbatch * ncb < sc.sm_count) nslice = min(nchunk, (sc.sm_count + nbatch * ncb - 1) / (nbatch * ncb));
   const int cps = (nchunk + nslice - 1) / nslice;
   nslice = (nchunk + cps - 1) / cps;
   const int nsc = nslice * ncb;
   const int streams = max(1, min(nbatch, sc.sm_count / nsc));
   const int grid = streams * nsc;
-  const size_t smem = dense_smem_bytes(cps * FS_CHUNK, W, v.d.S, FT);
+  const size_t smem = dense_smem_bytes(W, v.d.S, FT);
   cudaMemsetAsync(sc.ctr, 0, sizeof(unsigned int) * (size_t)nsc, st);
   // one slice: the scoring kernel writes the placement records itself (no key array, no decode launch)
   fs_placement* direct = nsc == 1 ? out : nullptr;
