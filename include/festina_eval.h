@@ -19,7 +19,10 @@
  *   - Return value: FS_OK (0) or a negative fs_status.  Nothing throws or aborts across the ABI.
  *     Host-visible arguments are validated synchronously.  Device-resident data are
  *     range-checked inside the kernels; a violation sets a sticky flag that the NEXT call
- *     returns (and clears) as FS_ERR_RANGE.
+ *     returns (and clears) as FS_ERR_RANGE.  FS_HOST calls wait for their own kernels and report their own
+ *     flags; for FS_DEVICE / FS_HOST_PINNED calls the flag is reported by the first later call on the context
+ *     (whichever it is): FS_ERR_RANGE then says that SOME earlier asynchronous call saw bad data, and the
+ *     records it affected carry gpu / phi / dst = -1.
  *   - No feasible candidate: index fields are -1 and the value field is +INF
  *     (the caller's cue to scale out).
  *   - All arithmetic is IEEE-754 binary32, round-to-nearest-even, no FMA contraction, in the
@@ -29,7 +32,10 @@
  *     fs_set_gpu_state) may be issued on different streams by that thread; the caller orders the streams.
  *     fs_place_batch, fs_dispatch and fs_dispatch_commit share staging buffers: one of them at a time.
  *   - FS_DEVICE and FS_HOST_PINNED calls never synchronise and do not allocate once a call of the same sizes has run, so a
- *     sequence of them can be captured into a CUDA graph (with fs_set_timing off) and replayed.
+ *     sequence of them can be captured into a CUDA graph (with fs_set_timing off) and replayed.  The scan order
+ *     and the per-model lists of the placement calls are built by the FIRST fs_place_batch / fs_dispatch after
+ *     an fs_set_gpu_state: capture fs_set_gpu_state in the same graph as the placement calls that follow it (a
+ *     graph holding only a placement call would replay against the lists of the state it was captured with).
  *   - There is no CPU fallback: every entry point runs CUDA kernels on the context's device.
  */
 #ifndef FESTINA_EVAL_H
@@ -318,14 +324,13 @@ int fs_last_cuda_error(const fs_ctx* ctx); /* cudaError_t of the last failed run
 /* Kernels launched by this context since creation (bench.py's gpu_launches counter).     */
 uint64_t fs_launch_count(const fs_ctx* ctx);
 /* Work counters of fs_place_batch (measurement only).  fs_set_work_stats(ctx, 1) makes later
- * fs_place_batch calls run the counting instantiation of the scoring kernel (same results, a
- * little slower); fs_last_place_stats copies the counters of the most recent such call
+ * fs_place_batch calls run the scoring kernel with its work counters switched on (same kernel, same
+ * results, a little slower); fs_last_place_stats copies the counters of the most recent such call
  * (it synchronises the device):
  *   out[0] chunks of 32 GPU records tested (lane <-> GPU: eligibility + lower bound)
  *   out[1] cold (request, GPU) pairs found eligible      out[2] cold pairs swept after pruning
  *   out[3] cold candidates swept (sum of sm_free*F)      out[4] warm (model resident) pairs tested
- *   out[5] pairs scored candidate by candidate with the definition (warm pairs + tie recovery;
- *          every eligible pair when the generic kernel ran)
+ *   out[5] pairs scored candidate by candidate with the definition (warm pairs + tie recovery)
  *   out[6] candidates scored that way                    out[7] requests processed (x GPU slices) */
 int fs_set_work_stats(fs_ctx* ctx, int on);
 int fs_last_place_stats(fs_ctx* ctx, uint64_t out[8]);
@@ -349,12 +354,6 @@ typedef enum {
 } fs_timer;
 int fs_set_timing(fs_ctx* ctx, int on);
 int fs_get_timing(fs_ctx* ctx, float* ms, int n);
-
-/* Measurement only: issue rates of the instruction classes the path is made of, in thread-instructions per
- * clock per SM at the SM clock `sm_mhz` (read it from nvidia-smi under load): out[0] FMUL, out[1] FADD,
- * out[2] FMNMX, out[3] FSETP + predicated FMNMX (per instruction), out[4] IMNMX, out[5] ISETP + SEL (per
- * instruction), out[6] FSET mask + OR + unsigned min (per instruction).  DESIGN.md section 7 checks the "alu" roofline peak (128 per clock per SM) against them.         */
-int fs_probe_pipe_rates(int cuda_device, double sm_mhz, double* out /*[7]*/);
 
 #ifdef __cplusplus
 }

@@ -24,7 +24,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
            "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_dispatch_commit", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_migration_plan", "fs_migration_select", "fs_strerror", "fs_last_cuda_error",
-           "fs_launch_count", "fs_probe_pipe_rates", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
+           "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm", "batch_tasks", "dispatch")
 
@@ -36,16 +36,6 @@ class FsDims(C.Structure):
 class FsParams(C.Structure):
     _fields_ = [("p_idle_w", C.c_float), ("horizon_ms", C.c_float), ("mem_cap_mb", C.c_float),
                 ("delta_pct", C.c_int32)]
-
-
-def probe_pipe_rates(device: int = 0, sm_mhz: float = 1965.0) -> dict:
-    """Issue rates (thread-instructions per clock per SM) of the path's instruction classes (measurement only)."""
-    o = (C.c_double * 7)()
-    rc = lib().fs_probe_pipe_rates(device, sm_mhz, o)
-    if rc != FS_OK:
-        raise FestinaError(rc, "fs_probe_pipe_rates")
-    names = ("fmul", "fadd", "fmnmx", "fsetp_pred_fmnmx", "imnmx", "isetp_sel", "fset_or_umin")
-    return {n: float(o[i]) for i, n in enumerate(names)}
 
 
 class FestinaError(RuntimeError):
@@ -88,7 +78,6 @@ def lib() -> C.CDLL:
     L.fs_last_cuda_error.argtypes = [vp]
     L.fs_launch_count.argtypes = [vp]
     L.fs_launch_count.restype = C.c_uint64
-    L.fs_probe_pipe_rates.argtypes = [C.c_int, C.c_double, C.POINTER(C.c_double)]
     L.fs_set_work_stats.argtypes = [vp, C.c_int]
     L.fs_last_place_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
     L.fs_set_timing.argtypes = [vp, C.c_int]

@@ -61,18 +61,29 @@ namespace {
     }                                                        \
   } while (0)
 
+// The new buffer is allocated before the old one is released: after a failed allocation the pointer and the
+// caller's capacity field still describe a valid (old) buffer, and the next call simply tries again.
 template <class T> int grow(fs_ctx* c, T*& p, size_t n_elems) {
-  if (p) { cudaFree(p); p = nullptr; }
   if (n_elems == 0) n_elems = 1;
-  FS_CUDA(c, cudaMalloc((void**)&p, n_elems * sizeof(T)));
+  T* fresh = nullptr;
+  FS_CUDA(c, cudaMalloc((void**)&fresh, n_elems * sizeof(T)));
+  if (p) {
+    // kernels of earlier calls may still read the old buffer on the caller's streams
+    FS_CUDA(c, cudaDeviceSynchronize());
+    FS_CUDA(c, cudaFree(p));
+  }
+  p = fresh;
   return FS_OK;
 }
 #define FS_TRY(x) do { int r_ = (x); if (r_ != FS_OK) return r_; } while (0)
 
 // sticky device-side range errors of earlier calls: report once, then clear
 int take_flags(fs_ctx* c) {
+  // one atomic exchange per word: a flag a running kernel raises is either seen by this call or left for the
+  // next one, never lost between a read and a clear.  (A flag is reported by the first call that sees it, which
+  // for FS_DEVICE / FS_HOST_PINNED calls is a later call than the one that caused it: festina_eval.h.)
   int any = 0;
-  for (int i = 0; i < FS_NFLAGS; ++i) { any |= ((volatile int*)c->flag_host)[i]; c->flag_host[i] = 0; }
+  for (int i = 0; i < FS_NFLAGS; ++i) any |= __atomic_exchange_n(&c->flag_host[i], 0, __ATOMIC_ACQ_REL);
   return any ? FS_ERR_RANGE : FS_OK;
 }
 
@@ -173,13 +184,16 @@ int fs_destroy(fs_ctx* c) {
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
                   c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf, c->pl_buf};
-  for (void* p : ptrs) if (p) cudaFree(p);
-  if (c->flag_host) cudaFreeHost(c->flag_host);
+  bool ok = true;
+  for (void* p : ptrs) if (p) ok = (cudaFree(p) == cudaSuccess) && ok;
+  if (c->flag_host) ok = (cudaFreeHost(c->flag_host) == cudaSuccess) && ok;
   if (c->have_events)
-    for (int i = 0; i < FS_T_COUNT; ++i) { cudaEventDestroy(c->tm.beg[i]); cudaEventDestroy(c->tm.end[i]); }
+    for (int i = 0; i < FS_T_COUNT; ++i) {
+      ok = (cudaEventDestroy(c->tm.beg[i]) == cudaSuccess) && ok; ok = (cudaEventDestroy(c->tm.end[i]) == cudaSuccess) && ok;
+    }
   cudaGetLastError();
   delete c;
-  return FS_OK;
+  return ok ? FS_OK : FS_ERR_CUDA;
 }
 
 int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const float* pow,

@@ -91,9 +91,11 @@ __global__ void __launch_bounds__(128) consol_agg_kernel(FsView v, int S_eff,
 
 // ---- a10: pair scoring; one block = TA sources x all destinations ----------------------------
 __global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
-    FsView v, int S_eff, float M_eff, const uint8_t* __restrict__ need, const float* __restrict__ E,
+    FsView v, int S_eff, float mem_cap_mb, int delta_pct, const uint8_t* __restrict__ need, const float* __restrict__ E,
     const float4* __restrict__ agg, unsigned long long* __restrict__ keys) {
   extern __shared__ unsigned char smem_raw[];
+  // M_eff = fl(fl(cap * (100 - delta)) / 100): the 5 % margin on memory (R:s19)
+  const float M_eff = __fdiv_rn(__fmul_rn(mem_cap_mb, (float)(100 - delta_pct)), 100.0f);
   const int F = v.d.F, K = v.K;
   float2* sEN = reinterpret_cast<float2*>(smem_raw);               // [F][TA] {E_a, need_a as int bits}: one LDS.64
   __shared__ unsigned long long sred[TA][PAIR_THREADS / 32];
@@ -199,14 +201,13 @@ int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
                     const FsConsolScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (v.K <= 0) return 0;
   const int S_eff = (v.d.S * (100 - prm.delta_pct)) / 100;
-  const float M_eff = (prm.mem_cap_mb * (float)(100 - prm.delta_pct)) / 100.0f;
   fs_tm_beg(tm, FS_T_CONSOL_AGG, st);
   consol_agg_kernel<<<(v.K + 3) / 4, 128, 0, st>>>(v, S_eff, sc.need, sc.E, sc.agg);
   fs_tm_end(tm, FS_T_CONSOL_AGG, st);
   const size_t smem = sizeof(float2) * v.d.F * TA;
   fs_tm_beg(tm, FS_T_CONSOL_PAIR, st);
-  consol_pair_kernel<<<(v.K + TA - 1) / TA, PAIR_THREADS, smem, st>>>(v, S_eff, M_eff, sc.need,
-                                                                    sc.E, sc.agg, sc.keys);
+  consol_pair_kernel<<<(v.K + TA - 1) / TA, PAIR_THREADS, smem, st>>>(v, S_eff, prm.mem_cap_mb, prm.delta_pct,
+                                                                    sc.need, sc.E, sc.agg, sc.keys);
   fs_tm_end(tm, FS_T_CONSOL_PAIR, st);
   consol_decode_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, S_eff, prm, sc.need, sc.E, sc.agg,
                                                           sc.keys, out);
