@@ -5,18 +5,29 @@ A *step* is one pass of the hot path over one batch of synthetic input (BASELINE
 configs[2], "pod": K=1,024 GPUs, M=64 models, F=64, S=16, B=128, R=65,536 requests):
     fs_set_gpu_state (co-resident summaries)  ->  fs_place_batch (R requests)
     ->  fs_local_config on every GPU.
-`value` = nominal dense placement candidates (R*K*S*F) of all ranks / device time of the step,
-inputs resident in HBM.  `e2e` = the same through the C ABI with pinned HOST buffers (H2D of
-state + requests, D2H of placements + local configs inside the timed region).
-N > 1: tables and GPU state are replicated, every rank scores its own R requests (weak scaling,
-no data-path collective).
+`value` = ELIGIBLE placement candidates of all ranks (every eligible (request, GPU) pair x its free shares x
+F: the candidate set of the dense definition, what the CPU oracle evaluates one by one) / device time of the
+step, inputs resident in HBM; the nominal grid R*K*S*F and what the kernel executed after exact pruning are
+reported beside it.  `e2e` = the same through the C ABI with pinned HOST buffers (H2D of state + requests,
+D2H of placements + local configs inside the timed region).
+The default run (N = 1) then adds, outside the pod leg's timed region: `sustained` (seconds of back-to-back
+replays), `variants` (pod reshaped so that pruning has less or nothing to hold on to), and `aux` (configs[3]
+local sweep, configs[4] consolidation, configs[0]/[1] step times), each checked against the oracle in the run.
+N > 1 (`--gpus N` starts N ranks itself through torch.distributed.run when not already under it): tables and
+GPU state are replicated, every rank scores its own R requests (weak scaling, no data-path collective;
+DESIGN.md "Multi-GPU"); the placement records are all-gathered over NCCL and rank 0 checks them.
 `--impl reference` times the CPU oracle (test infrastructure) on a bounded sample instead.
+`--ncu-import X.ncu-rep --ncu-out profiles/Y.json` turns an ncu capture into the small tracked summary the
+roofline block quotes (no GPU needed).
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
+import math
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -30,24 +41,22 @@ sys.path.insert(0, ROOT)
 from paper_2606_30391_b200 import synth  # noqa: E402
 
 METRIC = "placement_candidate_evals_per_sec"
-UNIT = "candidates/s"
+UNIT = "eligible candidates/s"
 # DESIGN.md §7 "Roofline": lane-operations (one 32-bit load / arithmetic / compare / select on one
 # lane) the method needs per unit of work, for the units the scoring kernel counts itself
 OPS_PER_CANDIDATE = 13.0   # dense definition: 8 fp32 arithmetic + 5 compare/select
-OPS_TILE = 14.0            # per (request, sigma, phi): 4 table loads, 5 fp32, 2 tests, 3 running minima
+OPS_REQUEST = 96.0         # per request: two 16-byte plane-minima records per share lane, three bounds (32 lanes x 3)
+OPS_TILE = 12.0            # per (request, sigma, phi) of a built tile: 4 table values, 5 fp32, test + select, running minimum
 OPS_PAIR_TEST = 18.0       # per (request, GPU) tested: 8-word record, 7 eligibility compares, bound (2 fp32 + compare)
 OPS_TSTAR = 12.0           # per swept pair: deadline threshold T*
 OPS_SWEEP = 2.0            # per swept candidate: compare + predicated min
 OPS_ROW = 4.0              # per swept (pair, phi): A0 load, add, min, subtract/compare share
-OPS_WARM_TEST = 20.0       # per warm pair tested: 12-word item, bound (5 fp32), 3 compares
-OPS_DEF = 14.0             # per candidate scored by the definition: 4 loads, 4 mul, 3 add/sub, 3 compares
-# dram bytes per launch of the scoring kernel and its issue utilisation, from the committed ncu
-# capture of this workload (profiles/; a profiler cannot run inside the timed bench)
-NCU_TRAFFIC_BYTES = 42.45e6
-NCU_NOTE = {"source": "profiles/r01_final_pod.md (ncu --set full of this kernel on this workload)",
-            "sm_throughput_pct_of_peak": 65.1, "issue_active_pct_of_peak": 70.4, "warp_instructions": 199.8e6,
-            "note": "executed instructions; `frac` above counts only the lane-operations the method needs"}
+OPS_WARM_TEST = 30.0       # per warm pair tested: 16-word item, bound (2 table bounds + 4 fp32), 3 compares
+OPS_DEF = 15.0             # per candidate scored by the definition: 4 loads, 4 mul, 4 add/sub, 3 compares
 SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128   # 4 schedulers x 32 lanes (B300_MICROARCH "issue")
+NCU_POD = os.path.join(ROOT, "profiles", "r02_pod_ncu.json")
+NCU_LOCAL = os.path.join(ROOT, "profiles", "r02_local_ncu.json")
+NCU_CONSOL = os.path.join(ROOT, "profiles", "r02_consol_ncu.json")
 
 
 def _peaks():
@@ -60,27 +69,54 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def _alu_peak():
+    peaks, src = _peaks()
+    mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    return SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * mhz * 1e6, mhz, src
+
+
+def _git_sha():
+    try:
+        sha = subprocess.run(["git", "rev-parse", "--short", "HEAD"], cwd=ROOT, capture_output=True, text=True).stdout.strip()
+        return sha or None
+    except OSError:
+        return None
+
+
+def _ncu_block(path):
+    """The tracked summary of an ncu capture (written by --ncu-import), with the commit it was taken at, so that
+    a stale capture shows: the figures are evidence from a profiler run, never measured inside the bench."""
+    if not os.path.exists(path):
+        return {"source": os.path.relpath(path, ROOT), "missing": True}
+    d = json.load(open(path))
+    d["source"] = os.path.relpath(path, ROOT)
+    d["bench_git_sha"] = _git_sha()
+    return d
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, period_ms: int = 100):
         self.rows, self.proc, self.thr = [], None, None
         self.cmd = ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                    "-lms", "100"]
+                    "-lms", str(period_ms)]
 
     def start(self):
         try:
             self.proc = subprocess.Popen(self.cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
-            return
+            return self
+
         def pump():
             for line in self.proc.stdout:
                 self.rows.append([x.strip() for x in line.split(",")])
         self.thr = threading.Thread(target=pump, daemon=True)
         self.thr.start()
+        return self
 
     def stop(self) -> dict:
         if self.proc is None:
@@ -113,24 +149,58 @@ def _dist():
     return ws, rank, lrank
 
 
+def _hist(a, n):
+    """Counts of the values 0..n-1 of an integer array (the chosen-index histograms of SURVEY 8(d))."""
+    a = np.asarray(a).reshape(-1)
+    a = a[(a >= 0) & (a < n)]
+    return np.bincount(a.astype(np.int64), minlength=n).astype(int).tolist()
+
+
+def _top_share(h):
+    t = sum(h)
+    return float(max(h) / t) if t else 0.0
+
+
+WORKLOAD_CFG = {"tiny": "configs[0]", "rack": "configs[1]", "pod": "configs[2]", "local": "configs[3]", "consol": "configs[4]"}
+
+
+def _workload_name(cl):
+    base = cl.name.split("/")[0]
+    tag = f"BASELINE.json {WORKLOAD_CFG[base]}" if base in WORKLOAD_CFG else "custom"
+    return f"{cl.name} ({tag})"
+
+
+def _config(cl, args, ws, graph):
+    return {"workload": f"{_workload_name(cl)}: K={cl.K} GPUs, M={cl.M}, F={cl.F}, S={cl.S}, "
+                        f"B={cl.B}, R={cl.R} requests per rank; step = fs_set_gpu_state + fs_place_batch + "
+                        f"fs_local_config(all GPUs, energy objective, exhaustive splits"
+                        + (", then the minimum-SM split rule" if args.split_modes == "both" else "") + ")"
+                        + ("; the two calls on two streams" if args.overlap else "")
+                        + ("; one CUDA graph per step" if graph else ""),
+            "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B, "R_per_rank": cl.R,
+            "l2": "flushed between timed steps by overwriting a 256 MiB buffer",
+            "parallelism": f"replicated tables+state, requests sharded x{ws}"}
+
+
 def oracle_sample(cl, n_req: int, nthreads: int):
-    """One bounded pass of the hot path through the CPU oracle; returns (seconds, candidates)."""
+    """One bounded pass of the hot path through the CPU oracle; returns (seconds, eligible candidates, GPUs)."""
     import oracle
-    n_gpu = max(1, int(round(cl.K * n_req / cl.R)))
+    n_gpu = max(1, int(round(cl.K * n_req / max(cl.R, 1))))
+    reqs = cl.requests[:n_req]
     t0 = time.perf_counter()
-    oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests[:n_req], nthreads)
+    oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, reqs, nthreads)
     oracle.local_config(cl.lat, cl.pow, cl.states, 0, np.arange(n_gpu, dtype=np.int32), nthreads)
     dt = time.perf_counter() - t0
-    return dt, n_req * cl.K * cl.S * cl.F, n_gpu
+    return dt, synth.eligible_work(cl, reqs)[1], n_gpu
 
 
 def run_reference(args):
     ws, rank, _ = _dist()
     if rank != 0:
         return
-    cl = synth.make_cluster(args.workload)
+    cl = synth.make_cluster(args.workload if args.workload in ("tiny", "rack", "pod") else "pod")
     cores = os.cpu_count() or 1
-    n_req = args.ref_requests
+    n_req = min(args.ref_requests, cl.R)
     for _ in range(args.warmup):
         oracle_sample(cl, max(8, n_req // 8), cores)
     tot, cand, n_gpu = 0.0, 0, 0
@@ -143,20 +213,101 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic", "config": _config(cl, args),
+            "data": "synthetic", "config": _config(cl, args, args.gpus, False),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def _config(cl, args):
-    return {"workload": f"{cl.name} (BASELINE.json configs[2]): K={cl.K} GPUs, M={cl.M}, F={cl.F}, S={cl.S}, "
-                        f"B={cl.B}, R={cl.R} requests per rank; step = fs_set_gpu_state + fs_place_batch + "
-                        f"fs_local_config(all GPUs, energy objective, exhaustive splits" + (", then the minimum-SM split rule" if args.split_modes == "both" else "") + ")" + ("; the two calls on two streams" if args.overlap else "") + ("; one CUDA graph per step" if args.graph else ""),
-            "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B, "R_per_rank": cl.R,
-            "l2": "flushed between timed steps by overwriting a 256 MiB buffer",
-            "parallelism": f"replicated tables+state, requests sharded x{args.gpus}"}
+def _place_shape(cl, place):
+    """What the decisions look like (histograms of the chosen indices in every run)."""
+    ok = place["gpu"] >= 0
+    hp, hs, hb = _hist(place["phi"][ok], cl.F), _hist(place["sigma"][ok], cl.S), _hist(place["beta"][ok], cl.B)
+    return {"placed_frac": float(ok.mean()) if len(ok) else 0.0, "top_phi_share": _top_share(hp),
+            "top_sigma_share": _top_share(hs), "top_beta_share": _top_share(hb),
+            "distinct_gpus": int(len(np.unique(place["gpu"][ok]))),
+            "hist_phi": hp, "hist_sigma": hs, "hist_beta": hb}
+
+
+def _local_shape(cl, res):
+    ok = res["phi"] >= 0
+    live = np.arange(4)[None, :] < cl.states["n_res"][: len(res), None]
+    sel = ok[:, None] & live
+    hp = _hist(res["phi"][ok], cl.F)
+    hs = _hist(res["sigma"][sel], cl.S)
+    busy = cl.states["t"]["q"][: len(res)] > 0
+    hb = _hist(res["beta"][sel[:, :, None] & busy], cl.B)
+    return {"feasible_frac": float(ok.mean()) if len(ok) else 0.0, "top_phi_share": _top_share(hp),
+            "top_sigma_share": _top_share(hs), "top_beta_share": _top_share(hb),
+            "hist_phi": hp, "hist_sigma": hs, "hist_beta": hb}
+
+
+def _useful_ops(cl, ps):
+    """Lane-operations of the units the scoring kernel counted itself (DESIGN.md section 7 per-unit figures)."""
+    return (OPS_REQUEST * ps["requests"] + OPS_TILE * ps["tiles_built"] * cl.S * cl.F
+            + OPS_PAIR_TEST * 32 * ps["chunks_tested"] + OPS_TSTAR * ps["cold_pairs_swept"]
+            + OPS_SWEEP * ps["cold_candidates_swept"] + OPS_ROW * cl.F * ps["cold_pairs_swept"]
+            + OPS_WARM_TEST * ps["warm_pairs_tested"] + OPS_DEF * ps["candidates_scored"])
+
+
+def _place_roofline(cl, ps, score_ms, cand_def, ncu_path=None):
+    alu_peak, mhz, peak_src = _alu_peak()
+    useful = _useful_ops(cl, ps)
+    achieved = useful / (score_ms * 1e-3)
+    nominal = OPS_PER_CANDIDATE * cand_def / (score_ms * 1e-3)
+    executed = ps["cold_candidates_swept"] + ps["candidates_scored"]
+    blk = {"bound": "alu", "kernel": "place_dense_kernel (fs_place_batch scoring + argmin + records)",
+           "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
+           "traffic": None, "useful_lane_ops_per_launch": useful, "kernel_ms": score_ms,
+           "executed_candidates_per_launch": executed,
+           "executed_frac_of_eligible": executed / cand_def if cand_def else None,
+           "dense_definition": {"achieved": nominal / 1e12, "frac": nominal / alu_peak,
+                                "note": f"{OPS_PER_CANDIDATE:g} lane-ops x {cand_def} eligible candidates / kernel time; "
+                                        "above 1 when exact pruning skips most of them: it measures the algorithm, not the kernel"},
+           "note": "achieved = lane-ops of the units the kernel counted itself (DESIGN.md section 7 per-unit "
+                   "figures) / CUDA-event time of the launch; peak = 148 SMs x 128 lanes/clk x "
+                   f"{mhz:.0f} MHz ({peak_src} sm_max_mhz)"}
+    if ps["cold_candidates_swept"] > 4 * ps["candidates_scored"]:
+        # sweep-dominated launch (the bounds cannot prune): the swept candidates against the rate at which an SM
+        # issues the sweep's compare + predicated-min pair (profiles/r01_pipe_rates.md: 31.6 pairs per clock per SM)
+        pair_peak = 31.6 * SM_COUNT * mhz * 1e6
+        rate = ps["cold_candidates_swept"] / (score_ms * 1e-3)
+        blk["sweep_pipe"] = {"achieved": rate / 1e12, "peak": pair_peak / 1e12, "unit": "Tcandidate/s", "frac": rate / pair_peak,
+                             "note": "swept candidates / kernel time against 31.6 compare+predicated-min pairs per clock per SM"}
+    if ncu_path:
+        ncu = _ncu_block(ncu_path)
+        blk["ncu"] = ncu
+        if not ncu.get("missing"):
+            blk["traffic"] = ncu.get("dram_bytes")
+            wi = ncu.get("warp_instructions")
+            if wi:
+                blk["useful_per_issued"] = useful / 32.0 / wi
+    return blk
+
+
+def _tb(torch, dev, a):
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+
+
+def _capture(torch, dev, stream, fn, what):
+    """One CUDA graph of fn(stream); None (and a note on stderr) when capture fails: the JSON line says which
+    path was timed ("graph": true | false), so a direct-launch number is never mistaken for the graph path."""
+    try:
+        cap = torch.cuda.Stream(device=dev)
+        cap.wait_stream(stream)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=cap):
+            fn(torch.cuda.current_stream())
+        stream.wait_stream(cap)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        return g
+    except Exception as e:                              # noqa: BLE001 - reported, and the fallback is flagged
+        print(f"bench.py: CUDA graph capture of {what} failed ({e}); timing direct launches", file=sys.stderr)
+        torch.cuda.synchronize()
+        return None
 
 
 def run_ours(args):
@@ -165,9 +316,11 @@ def run_ours(args):
 
     ws, rank, lrank = _dist()
     dist = None
-    if ws > 1:
+    if ws > 1 or "TORCHELASTIC_RUN_ID" in os.environ:   # under torch.distributed.run, also with a single rank
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")     # the communicator lines (nranks, NVLS) ...
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")   # ... on stderr: stdout carries the one JSON line
         torch.cuda.set_device(lrank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", lrank))
     dev = torch.device("cuda", lrank)
@@ -176,7 +329,7 @@ def run_ours(args):
     if rank > 0:   # every rank scores its own batch
         cl.requests = synth.make_requests(cl.seed + 7919 * rank, cl.R, cl.M)
     ctx = fs.Festina(lrank)
-    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+    tb = lambda a: _tb(torch, dev, a)
     # offline profile tables are loaded once (profiling is offline), not per step
     ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
                       tb(cl.models), cl.params)
@@ -194,23 +347,26 @@ def run_ours(args):
     side = torch.cuda.Stream(device=dev) if args.overlap else None
     ev_state, ev_side = torch.cuda.Event(), torch.cuda.Event()
 
-    def step_device(serial=False, st=None):
+    def step(states, reqs, place, local, local2, pinned, serial=False, st=None):
         st = stream if st is None else st
-        ctx.set_gpu_state(d_states, stream=st)
+        ctx.set_gpu_state(states, stream=st, pinned=pinned)
         if side is None or serial:
-            ctx.place_batch(d_reqs, out=d_place, stream=st)
-            ctx.local_config(0, n=cl.K, out=d_local, stream=st)
+            ctx.place_batch(reqs, out=place, stream=st, pinned=pinned)
+            ctx.local_config(0, n=cl.K, out=local, stream=st, pinned=pinned)
             if both_splits:
-                ctx.local_config(2, n=cl.K, out=d_local2, stream=st)
+                ctx.local_config(2, n=cl.K, out=local2, stream=st, pinned=pinned)
             return
         ev_state.record(st)
         side.wait_event(ev_state)
-        ctx.local_config(0, n=cl.K, out=d_local, stream=side)
+        ctx.local_config(0, n=cl.K, out=local, stream=side, pinned=pinned)
         if both_splits:
-            ctx.local_config(2, n=cl.K, out=d_local2, stream=side)
-        ctx.place_batch(d_reqs, out=d_place, stream=st)
+            ctx.local_config(2, n=cl.K, out=local2, stream=side, pinned=pinned)
+        ctx.place_batch(reqs, out=place, stream=st, pinned=pinned)
         ev_side.record(side)
         st.wait_event(ev_side)
+
+    def step_device(serial=False, st=None):
+        step(d_states, d_reqs, d_place, d_local, d_local2, False, serial, st)
 
     def barrier():
         torch.cuda.synchronize()
@@ -218,34 +374,23 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step_device()
     barrier()
     # The calls are asynchronous and allocation-free after the first step, so a whole step (fork to the second
     # stream and join included) can be captured into a CUDA graph and replayed: one launch per step for the host.
     graph, launches_per_step = None, None
+    lc = ctx.launch_count
+    step_device()
+    launches_per_step = ctx.launch_count - lc
+    torch.cuda.synchronize()
     if args.graph:
-        try:
-            ctx.set_timing(False)                       # event records of the per-kernel timers are not capturable
-            cap = torch.cuda.Stream(device=dev)
-            cap.wait_stream(stream)
-            lc = ctx.launch_count
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph, stream=cap):
-                step_device(st=torch.cuda.current_stream())
-            launches_per_step = ctx.launch_count - lc
-            stream.wait_stream(cap)
-            for _ in range(3):
-                graph.replay()
-            torch.cuda.synchronize()
-        except Exception as e:                          # noqa: BLE001 - fall back to direct launches
-            print(f"bench.py: CUDA graph capture failed ({e}); timing direct launches", file=sys.stderr)
-            graph = None
+        ctx.set_timing(False)                           # event records of the per-kernel timers are not capturable
+        graph = _capture(torch, dev, stream, lambda st: step_device(st=st), "the device step")
         ctx.set_timing(True)
     barrier()
-    sampler = ClockSampler(lrank)
-    sampler.start()
-    l0 = ctx.launch_count
+    sampler = ClockSampler(lrank).start()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     kt = {}
     barrier()
@@ -264,7 +409,7 @@ def run_ours(args):
                 kt.setdefault(k, []).append(v)
     barrier()
     wall = time.perf_counter() - wall0
-    launches = ctx.launch_count - l0 if graph is None else launches_per_step * args.steps
+    launches = launches_per_step * args.steps
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
     # per-kernel durations need the kernels one after the other: when the timed steps overlap the two calls,
     # the same K steps are run once more serially (same inputs, L2 flushed) for kernel_ms and the roofline
@@ -278,79 +423,50 @@ def run_ours(args):
             serial_ms += a.elapsed_time(b)
             for k, v in ctx.get_timing().items():
                 kt.setdefault(k, []).append(v)
-    # work counters: one untimed call of the counting instantiation (same input, same work)
+    # work counters: one untimed call with the kernel's counters switched on (same input, same work)
     ctx.set_work_stats(True)
     ctx.place_batch(d_reqs, out=d_place, stream=stream)
     pstats = ctx.last_place_stats()
     ctx.set_work_stats(False)
-    useful_ops = (OPS_TILE * pstats["requests"] * cl.S * cl.F + OPS_PAIR_TEST * 32 * pstats["chunks_tested"]
-                  + OPS_TSTAR * pstats["cold_pairs_swept"] + OPS_SWEEP * pstats["cold_candidates_swept"]
-                  + OPS_ROW * cl.F * pstats["cold_pairs_swept"] + OPS_WARM_TEST * pstats["warm_pairs_tested"]
-                  + OPS_DEF * pstats["candidates_scored"])
-    # the dense definition's work: every eligible (request, GPU) pair x sm_free x F, counted by the
-    # generic kernel (no pruning) on a second context; also an on-GPU cross-check of the two kernels
-    os.environ["FS_FORCE_GENERIC"] = "1"
-    ctx_g = fs.Festina(lrank)
-    del os.environ["FS_FORCE_GENERIC"]
-    ctx_g.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
-                        tb(cl.models), cl.params)
-    ctx_g.set_gpu_state(d_states, stream=stream)
-    ctx_g.set_work_stats(True)
-    d_place_g = torch.empty_like(d_place)
-    ctx_g.place_batch(d_reqs, out=d_place_g, stream=stream)
-    gstats = ctx_g.last_place_stats()
-    torch.cuda.synchronize()
-    assert torch.equal(d_place_g, d_place), "generic and dense scoring kernels disagree"
-    ctx_g.close()
-    pairs, cand_def = gstats["cold_pairs_eligible"], gstats["candidates_scored"]
+    pairs, cand_def = synth.eligible_work(cl)
 
-    # end to end through the C ABI with pinned host buffers
+    # ---- sustained: seconds of back-to-back replays, no flush, clocks sampled over that window ----------
+    sustained = None
+    if rank == 0 and args.sustained_s > 0:
+        n_rep = max(50, int(math.ceil(args.sustained_s * 1e3 / max(dev_ms / args.steps, 1e-3))))
+        s2 = ClockSampler(lrank, 50).start()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n_rep):
+            if graph is not None:
+                graph.replay()
+            else:
+                step_device()
+        b.record(stream); b.synchronize()
+        sus_ms = a.elapsed_time(b)
+        sustained = {"steps": n_rep, "seconds": sus_ms * 1e-3, "ms_per_step": sus_ms / n_rep,
+                     "value": cand_def * n_rep / (sus_ms * 1e-3), "unit": UNIT, "clocks": s2.stop(),
+                     "note": "back-to-back " + ("graph replays" if graph is not None else "direct steps")
+                             + " of the same step, no L2 flush in between (tables and state stay in the 126 MB L2)"}
+
+    # ---- end to end through the C ABI with pinned host buffers --------------------------------------
     h_states = torch.from_numpy(cl.states.view(np.uint8).reshape(-1).copy()).pin_memory()
     h_reqs = torch.from_numpy(cl.requests.view(np.uint8).reshape(-1).copy()).pin_memory()
     h_place = torch.empty(cl.R * 32, dtype=torch.uint8).pin_memory()
     h_local = torch.empty(cl.K * 48, dtype=torch.uint8).pin_memory()
     h_local2 = torch.empty(cl.K * 48, dtype=torch.uint8).pin_memory()
 
-    # The same step as above with FS_HOST_PINNED buffers: every step copies its inputs (state records, requests)
+    # The same step with FS_HOST_PINNED buffers: every step copies its inputs (state records, requests)
     # from page-locked host memory and its results (placements, local configurations) back; the host waits for
     # the stream before it reads them.  Two streams and one CUDA graph per step, as in the device-resident step.
     def step_host(st=None):
-        st = stream if st is None else st
-        ctx.set_gpu_state(h_states, stream=st, pinned=True)
-        if side is None:
-            ctx.place_batch(h_reqs, out=h_place, stream=st, pinned=True)
-            ctx.local_config(0, n=cl.K, out=h_local, stream=st, pinned=True)
-            if both_splits:
-                ctx.local_config(2, n=cl.K, out=h_local2, stream=st, pinned=True)
-            return
-        ev_state.record(st)
-        side.wait_event(ev_state)
-        ctx.local_config(0, n=cl.K, out=h_local, stream=side, pinned=True)
-        if both_splits:
-            ctx.local_config(2, n=cl.K, out=h_local2, stream=side, pinned=True)
-        ctx.place_batch(h_reqs, out=h_place, stream=st, pinned=True)
-        ev_side.record(side)
-        st.wait_event(ev_side)
+        step(h_states, h_reqs, h_place, h_local, h_local2, True, False, st)
 
     ctx.set_timing(False)
     for _ in range(3):
         step_host()
     torch.cuda.synchronize()
-    hgraph = None
-    if args.graph:
-        try:
-            cap = torch.cuda.Stream(device=dev)
-            cap.wait_stream(stream)
-            hgraph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(hgraph, stream=cap):
-                step_host(st=torch.cuda.current_stream())
-            stream.wait_stream(cap)
-            for _ in range(3):
-                hgraph.replay()
-            torch.cuda.synchronize()
-        except Exception as e:                          # noqa: BLE001 - fall back to direct calls
-            print(f"bench.py: CUDA graph capture of the host-buffer step failed ({e}); timing direct calls", file=sys.stderr)
-            hgraph = None
+    hgraph = _capture(torch, dev, stream, lambda st: step_host(st=st), "the host-buffer step") if args.graph else None
     barrier()
     e2e_t = 0.0
     for _ in range(args.steps):
@@ -366,34 +482,52 @@ def run_ours(args):
         e2e_t += time.perf_counter() - t0
     clocks = sampler.stop()
     assert np.array_equal(h_place.numpy(), d_place.cpu().numpy()), "host and device paths disagree"
+    assert np.array_equal(h_local.numpy(), d_local.cpu().numpy()), "host and device paths disagree (local)"
+
+    # ---- N > 1: the placement records of all ranks, gathered on the device over NCCL; rank 0 recomputes
+    # every rank's batch on its own GPU and compares the bytes
+    gathered_ok = None
+    if dist is not None:
+        from paper_2606_30391_b200 import shard
+        allrec = shard.gather_records(d_place, [cl.R] * ws, dist, dtype=synth.PLACEMENT_DT)
+        if rank == 0:
+            gathered_ok = len(allrec) == ws * cl.R
+            d_chk = torch.empty_like(d_place)
+            for r in range(ws):
+                rq = cl.requests if r == 0 else synth.make_requests(cl.seed + 7919 * r, cl.R, cl.M)
+                ctx.place_batch(tb(rq), out=d_chk, stream=stream)
+                torch.cuda.synchronize()
+                gathered_ok = gathered_ok and np.array_equal(d_chk.cpu().numpy().view(synth.PLACEMENT_DT),
+                                                             allrec[r * cl.R:(r + 1) * cl.R])
 
     t = torch.tensor([dev_ms, e2e_t * 1e3, wall * 1e3], dtype=torch.float64, device=dev)
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dev_ms, e2e_ms, wall_ms = (float(x) for x in t.cpu())
     if rank != 0:
+        ctx.close()
         if dist is not None:
             dist.destroy_process_group()
         return
     grid_cands = cl.R * cl.K * cl.S * cl.F
     steps = args.steps
-    value = ws * grid_cands * steps / (dev_ms * 1e-3)
-    peaks, peak_src = _peaks()
-    sm_clk_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
-    alu_peak = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * sm_clk_hz          # lane-instructions / s
     score_ms = float(np.mean(kt.get("place_score", [float("nan")])))
-    achieved = useful_ops / (score_ms * 1e-3)
-    nominal = OPS_PER_CANDIDATE * cand_def / (score_ms * 1e-3)
     place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
-    ok = place["gpu"] >= 0
+    local = d_local.cpu().numpy().view(synth.LOCAL_CFG_DT)
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": dev_ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": _config(cl, args),
+        "metric": METRIC, "value": ws * cand_def * steps / (dev_ms * 1e-3), "unit": UNIT, "n_gpus": ws, "steps": steps,
+        "warmup": warm, "ms_per_step": dev_ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": _config(cl, args, ws, graph is not None),
+        "graph": {"device_step": graph is not None, "host_step": hgraph is not None},
         "decisions_per_sec": ws * (cl.R + cl.K) * steps / (dev_ms * 1e-3),
         "placement_decisions_per_sec": ws * cl.R * steps / (dev_ms * 1e-3),
+        "nominal_grid_candidates_per_sec": ws * grid_cands * steps / (dev_ms * 1e-3),
+        "executed_candidates_per_sec": ws * (pstats["cold_candidates_swept"] + pstats["candidates_scored"]) * steps / (dev_ms * 1e-3),
         "nominal_candidates_per_step": grid_cands, "eligible_candidates_per_step": cand_def,
         "eligible_pairs_per_step": pairs, "place_stats": pstats,
+        "value_note": "value = eligible candidates (the dense definition's candidate set, what the oracle evaluates one by "
+                      "one) / step time; the kernel reaches the same argmin after scoring executed_candidates of them "
+                      "(exact branch and bound), so value measures the method on this workload, roofline.frac the kernel",
         "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
         "serial": {"ms_per_step": serial_ms / steps,
                    "note": ("timed steps run fs_place_batch and fs_local_config on two streams"
@@ -402,39 +536,91 @@ def run_ours(args):
                               "right after" if (args.overlap or graph is not None) else
                             "timed steps are serial: kernel_ms comes from them")},
         "wall_ms_per_step_incl_flush": wall_ms / steps,
-        "e2e": {"value": ws * grid_cands * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
+        "e2e": {"value": ws * cand_def * steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / steps,
                 "h2d_bytes_per_step": cl.K * 128 + cl.R * 32, "d2h_bytes_per_step": cl.R * 32 + cl.K * 48 * (2 if both_splits else 1),
                 "mode": "FS_HOST_PINNED buffers (page-locked host memory): state records and local configurations by "
                         "copy engine, requests read and placement records written over PCIe by the scoring kernel itself"
-                        + (", two streams" if side is not None else "") + (", one CUDA graph per step" if hgraph is not None else "")
+                        + (", two streams" if side is not None else "") + (", one CUDA graph per step" if hgraph is not None else ", direct calls")
                         + "; host wall clock around the step incl. the final stream synchronisation"},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": "place_dense_kernel (fs_place_batch scoring + argmin)",
-                     "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tlane-op/s",
-                     "frac": achieved / alu_peak, "traffic": NCU_TRAFFIC_BYTES,
-                     "useful_lane_ops_per_launch": useful_ops, "kernel_ms": score_ms,
-                     "dense_definition": {"achieved": nominal / 1e12, "frac": nominal / alu_peak,
-                                          "note": f"{OPS_PER_CANDIDATE:g} lane-ops x {cand_def} eligible candidates "
-                                                  "(counted by the unpruned generic kernel); above 1 because "
-                                                  "exact pruning skips most of them"},
-                     "ncu": NCU_NOTE,
-                     "note": "achieved = lane-ops of the units the kernel counted itself (DESIGN.md section 7 "
-                             "per-unit figures) / CUDA-event time of the launch; peak = 148 SMs x 128 lanes/clk x "
-                             f"{sm_clk_hz / 1e6:.0f} MHz ({peak_src} sm_max_mhz); traffic from the committed ncu capture"},
-        "degeneracy": {"placed_frac": float(ok.mean()),
-                       "top_phi_share": float(np.bincount(place["phi"][ok]).max() / max(ok.sum(), 1)),
-                       "distinct_gpus": int(len(np.unique(place["gpu"][ok])))},
+        "roofline": _place_roofline(cl, pstats, score_ms, cand_def, NCU_POD),
+        "degeneracy": _place_shape(cl, place),
+        "local_shape": _local_shape(cl, local),
     }
-    if ws == 1 and not args.no_cpu_baseline:
-        cores = os.cpu_count() or 1
-        dt, c, n_gpu = oracle_sample(cl, args.cpu_requests, cores)
-        line["cpu_baseline"] = {"value": c / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{args.cpu_requests} of {cl.R} requests x all {cl.K} GPUs + "
-                                          f"{n_gpu} GPUs local config, {dt:.1f} s"}
+    if sustained is not None:
+        line["sustained"] = sustained
+    if gathered_ok is not None:
+        line["gathered_records_ok"] = bool(gathered_ok)
+        assert gathered_ok, "records gathered over NCCL differ from the recomputation on rank 0"
+    if ws == 1:
+        ctx.set_timing(True)
+        if args.variants:
+            line["variants"] = run_variants(args, torch, dev, ctx, flush)
+        if args.aux:
+            line["aux"] = {w: run_aux_leg(args, torch, dev, w, flush) for w in ("local", "consol")}
+            line["aux"].update({w: run_small_leg(args, torch, dev, w, flush) for w in ("tiny", "rack")})
+        if not args.no_cpu_baseline:
+            cores = os.cpu_count() or 1
+            dt, c, n_gpu = oracle_sample(cl, args.cpu_requests, cores)
+            line["cpu_baseline"] = {"value": c / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{args.cpu_requests} of {cl.R} requests x all {cl.K} GPUs + "
+                                              f"{n_gpu} GPUs local config, {dt:.1f} s"}
     print(json.dumps(line), flush=True)
+    ctx.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+def run_variants(args, torch, dev, ctx, flush):
+    """configs[2] reshaped so that the bounds prune less (or nothing): the scoring kernel timed on each, with its
+    work counters, its roofline fraction and the shape of the decisions; every variant is checked against the
+    oracle on a sample of its requests in this run."""
+    import oracle
+    out = {}
+    stream = torch.cuda.current_stream()
+    cores = os.cpu_count() or 1
+    for name in synth.VARIANTS:
+        cl = synth.make_variant(args.workload, name)
+        tb = lambda a: _tb(torch, dev, a)
+        ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                          tb(cl.models), cl.params)
+        d_states, d_reqs = tb(cl.states), tb(cl.requests)
+        d_place = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+        n_steps = max(3, args.steps // 2) if name != "identical_gpus" else 3
+        ts, step_ms = [], []
+        for i in range(3 + n_steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctx.set_gpu_state(d_states, stream=stream)
+            ctx.place_batch(d_reqs, out=d_place, stream=stream)
+            b.record(stream); b.synchronize()
+            if i >= 3:
+                ts.append(ctx.get_timing()["place_score"]); step_ms.append(a.elapsed_time(b))
+        ctx.set_work_stats(True)
+        ctx.place_batch(d_reqs, out=d_place, stream=stream)
+        ps = ctx.last_place_stats()
+        ctx.set_work_stats(False)
+        place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
+        idx = np.arange(0, cl.R, max(1, cl.R // args.variant_sample))
+        ref = oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests[idx], cores)
+        same = all(np.array_equal(place[idx][f], ref[f]) for f in ("gpu", "sigma", "phi", "beta", "f_req", "flat")) and \
+            np.array_equal(place[idx]["energy_mj"].view(np.uint32), ref["energy_mj"].view(np.uint32))
+        assert same, f"variant {name}: CUDA and oracle disagree on the sample"
+        pairs, cand_def = synth.eligible_work(cl)
+        score_ms = float(np.mean(ts))
+        shape = _place_shape(cl, place)
+        for k in ("hist_sigma", "hist_beta"):
+            shape.pop(k)
+        out[name] = {"place_score_ms": score_ms, "ms_per_step": float(np.mean(step_ms)), "steps": n_steps,
+                     "step": "fs_set_gpu_state + fs_place_batch, L2 flushed between steps",
+                     "value": cand_def / (float(np.mean(step_ms)) * 1e-3), "unit": UNIT,
+                     "eligible_candidates_per_step": cand_def, "place_stats": ps,
+                     "roofline": _place_roofline(cl, ps, score_ms, cand_def),
+                     "degeneracy": shape,
+                     "oracle_check": f"{len(idx)} requests (every {max(1, cl.R // args.variant_sample)}th) identical to the oracle"}
+    return out
 
 
 def _slot_evals(cl) -> int:
@@ -444,51 +630,44 @@ def _slot_evals(cl) -> int:
     return int((np.minimum(q, cl.B) * live[:, :, None]).sum()) * cl.F * cl.S
 
 
-def run_aux(args):
-    """--workload local (BASELINE.json configs[3]) / consol (configs[4]): the other two entry points at
-    their own full-size configs, same JSON contract.  1 GPU."""
-    import torch
+def run_aux_leg(args, torch, dev, workload, flush):
+    """configs[3] (`local`) / configs[4] (`consol`): the other two entry points at their own full-size configs.
+    Returns the result object (also printed as its own line by --workload local|consol)."""
     import paper_2606_30391_b200 as fs
     import oracle
-    ws, rank, lrank = _dist()
-    assert ws == 1, "the local / consol workloads are single-GPU bench lines"
-    dev = torch.device("cuda", lrank)
-    torch.cuda.set_device(dev)
-    cl = synth.make_cluster(args.workload)
-    ctx = fs.Festina(lrank)
-    tb = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.uint8).reshape(-1)).to(dev)
+    cl = synth.make_cluster(workload)
+    ctx = fs.Festina(dev.index or 0)
+    tb = lambda a: _tb(torch, dev, a)
     ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
                       tb(cl.models), cl.params)
     d_states = tb(cl.states)
-    local = args.workload == "local"
+    local = workload == "local"
     rec = 48 if local else 16
     d_out = torch.empty(cl.K * rec, dtype=torch.uint8, device=dev)
     h_states = torch.from_numpy(cl.states.view(np.uint8).reshape(-1).copy()).pin_memory()
     h_out = torch.empty(cl.K * rec, dtype=torch.uint8).pin_memory()
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
     ctx.set_timing(True)
     flags = fs.FS_OBJ_POWER | fs.FS_SPLIT_EXHAUSTIVE      # configs[3]: "minimum-power feasible config"
 
-    def step(states, out):
-        ctx.set_gpu_state(states, stream=stream)
+    def step(states, out, pinned, st):
+        ctx.set_gpu_state(states, stream=st, pinned=pinned)
         if local:
-            ctx.local_config(flags, n=cl.K, out=out, stream=stream)
+            ctx.local_config(flags, n=cl.K, out=out, stream=st, pinned=pinned)
         else:
-            ctx.consolidate(out=out, stream=stream)
+            ctx.consolidate(out=out, stream=st, pinned=pinned)
 
     warm = max(args.warmup, 3)
     for _ in range(warm):
-        step(d_states, d_out)
+        step(d_states, d_out, False, stream)
     torch.cuda.synchronize()
-    sampler = ClockSampler(lrank)
-    sampler.start()
+    sampler = ClockSampler(dev.index or 0).start()
     l0 = ctx.launch_count
     kt, dev_ms = {}, 0.0
     for _ in range(args.steps):
         flush.zero_()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream); step(d_states, d_out); b.record(stream); b.synchronize()
+        a.record(stream); step(d_states, d_out, False, stream); b.record(stream); b.synchronize()
         dev_ms += a.elapsed_time(b)
         for k, v in ctx.get_timing().items():
             kt.setdefault(k, []).append(v)
@@ -496,32 +675,10 @@ def run_aux(args):
     # end to end: the same step on FS_HOST_PINNED buffers (page-locked host memory, the calls enqueue and return,
     # the host waits for the stream before it reads the results), captured once into a CUDA graph
     ctx.set_timing(False)
-
-    def step_host():
-        ctx.set_gpu_state(h_states, stream=torch.cuda.current_stream(), pinned=True)
-        if local:
-            ctx.local_config(flags, n=cl.K, out=h_out, stream=torch.cuda.current_stream(), pinned=True)
-        else:
-            ctx.consolidate(out=h_out, stream=torch.cuda.current_stream(), pinned=True)
-
     for _ in range(3):
-        step_host()
+        step(h_states, h_out, True, stream)
     torch.cuda.synchronize()
-    hgraph = None
-    if args.graph:
-        try:
-            cap = torch.cuda.Stream(device=dev)
-            cap.wait_stream(stream)
-            hgraph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(hgraph, stream=cap):
-                step_host()
-            stream.wait_stream(cap)
-            for _ in range(3):
-                hgraph.replay()
-            torch.cuda.synchronize()
-        except Exception as e:                          # noqa: BLE001 - fall back to direct calls
-            print(f"bench.py: CUDA graph capture of the host-buffer step failed ({e}); timing direct calls", file=sys.stderr)
-            hgraph = None
+    hgraph = _capture(torch, dev, stream, lambda st: step(h_states, h_out, True, st), f"the {workload} host-buffer step") if args.graph else None
     e2e_t = 0.0
     for _ in range(args.steps):
         flush.zero_(); h_out.zero_(); torch.cuda.synchronize()
@@ -529,73 +686,206 @@ def run_aux(args):
         if hgraph is not None:
             hgraph.replay()
         else:
-            step_host()
+            step(h_states, h_out, True, stream)
         torch.cuda.synchronize()
         e2e_t += time.perf_counter() - t0
-    assert np.array_equal(h_out.numpy(), d_out.cpu().numpy()), "host and device paths disagree"
     clocks = sampler.stop()
     assert np.array_equal(h_out.numpy(), d_out.cpu().numpy()), "host and device paths disagree"
-    peaks, peak_src = _peaks()
-    alu_peak = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    alu_peak, mhz, peak_src = _alu_peak()
     cores = os.cpu_count() or 1
     if local:
         units, unit_name, metric = _slot_evals(cl), "slot evals/s", "local_slot_evals_per_sec"
-        kname, kms, ops = "local_slot_grouped_kernel (a7)", float(np.mean(kt["local_slot"])), 5.0
+        kname, kms, ops, slots = "local_slot_grouped_kernel (a7)", float(np.mean(kt["local_slot"])), 5.0, 8.0
         ops_note = ("5 lane-ops per (slot, phi, sigma, beta) under the power objective: 2 table values, "
                     "rounds*LAT, deadline compare, cost compare/select (6 under the energy objective)")
         res = d_out.cpu().numpy().view(synth.LOCAL_CFG_DT)
-        degeneracy = {"feasible_frac": float((res["phi"] >= 0).mean()),
-                      "top_phi_share": float(np.bincount(res["phi"][res["phi"] >= 0]).max() / max((res["phi"] >= 0).sum(), 1))}
-        n_s = args.cpu_gpus
+        shape = _local_shape(cl, res)
         t0 = time.perf_counter()
-        ref = oracle.local_config(cl.lat, cl.pow, cl.states, flags, np.arange(n_s, dtype=np.int32), cores)
+        ref = oracle.local_config(cl.lat, cl.pow, cl.states, flags, None, cores)
         dt = time.perf_counter() - t0
-        assert np.array_equal(ref["flat"], res["flat"][:n_s]), "CUDA and oracle disagree on the sample"
-        sub = synth.Cluster(**{**cl.__dict__, "states": cl.states[:n_s], "K": n_s})
-        cpu = {"value": _slot_evals(sub) / dt, "unit": unit_name, "cores": cores, "kind": "oracle",
-               "sample": f"GPUs 0..{n_s - 1} of {cl.K}, {dt:.1f} s"}
-        work = (f"local (BASELINE.json configs[3]): K={cl.K} GPUs, 2-4 co-residents, queue depths U{{0..256}}, "
+        assert np.array_equal(ref["flat"], res["flat"]) and np.array_equal(ref["phi"], res["phi"]) and \
+            np.array_equal(ref["beta"], res["beta"]), "CUDA and oracle disagree"
+        cpu = {"value": units / dt, "unit": unit_name, "cores": cores, "kind": "oracle",
+               "sample": f"the whole config (all {cl.K} GPUs, compared in full), {dt:.1f} s"}
+        work = (f"{_workload_name(cl)}: K={cl.K} GPUs, 2-4 co-residents, queue depths U{{0..256}}, "
                 f"F={cl.F} x all SM splits (S={cl.S}) x batch 1..{cl.B}; step = fs_set_gpu_state + "
                 "fs_local_config(all GPUs, power objective, exhaustive splits)")
-        decisions = cl.K
+        ncu_path = NCU_LOCAL
     else:
         units, unit_name, metric = cl.K * cl.K * cl.F, "pair-frequency evals/s", "consol_pair_freq_evals_per_sec"
-        kname, kms, ops = "consol_pair_kernel (a10)", float(np.mean(kt["consol_pair"])), 8.0
+        kname, kms, ops, slots = "consol_pair_kernel (a10)", float(np.mean(kt["consol_pair"])), 8.0, 5.5
         ops_note = ("8 lane-ops per (source, destination, phi): 2 fp32 + 2 small-int values, int add + compare, "
-                    "fp32 add, min (SURVEY 8(d))")
+                    "fp32 add, min (SURVEY 8(d)); the four values are on-chip reads the kernel amortises")
         res = d_out.cpu().numpy().view(synth.CONSOL_DT)
-        degeneracy = {"has_destination_frac": float((res["dst"] >= 0).mean()),
-                      "distinct_destinations": int(len(np.unique(res["dst"][res["dst"] >= 0])))}
+        shape = {"has_destination_frac": float((res["dst"] >= 0).mean()),
+                 "distinct_destinations": int(len(np.unique(res["dst"][res["dst"] >= 0]))),
+                 "hist_phi": _hist(res["phi"][res["dst"] >= 0], cl.F)}
         p = cl.params
         t0 = time.perf_counter()
         ref = oracle.consolidate(cl.lat, cl.pow, cl.models, cl.states, p.p_idle_w, p.horizon_ms, p.mem_cap_mb,
                                  p.delta_pct, cores)
         dt = time.perf_counter() - t0
-        assert np.array_equal(ref["dst"], res["dst"]), "CUDA and oracle disagree"
+        assert np.array_equal(ref["dst"], res["dst"]) and np.array_equal(ref["phi"], res["phi"]), "CUDA and oracle disagree"
         cpu = {"value": units / dt, "unit": unit_name, "cores": cores, "kind": "oracle",
-               "sample": f"the whole config ({cl.K} sources x {cl.K} destinations), {dt:.1f} s"}
-        work = (f"consol (BASELINE.json configs[4]): K={cl.K} GPUs, M={cl.M}, 1-2 tenants, load ~ Beta(2,5); "
+               "sample": f"the whole config ({cl.K} sources x {cl.K} destinations, compared in full), {dt:.1f} s"}
+        work = (f"{_workload_name(cl)}: K={cl.K} GPUs, M={cl.M}, 1-2 tenants, load ~ Beta(2,5); "
                 f"step = fs_set_gpu_state + fs_consolidate ({cl.K * cl.K} pairs x {cl.F} frequencies)")
-        decisions = cl.K
+        ncu_path = NCU_CONSOL
     steps = args.steps
     achieved = ops * units / (kms * 1e-3)
+    # issue slots: the exhaustive kernels spend one half-rate compare and one half-rate predicated min per unit
+    # (profiles/r01_pipe_rates.md: 2 issue slots each) beside their full-rate arithmetic
+    pipe = slots * units / (kms * 1e-3)
     line = {"metric": metric, "value": units * steps / (dev_ms * 1e-3), "unit": unit_name, "n_gpus": 1,
             "steps": steps, "warmup": warm, "ms_per_step": dev_ms / steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": work, "K": cl.K, "M": cl.M, "F": cl.F, "S": cl.S, "B": cl.B,
                        "l2": "flushed between timed steps by overwriting a 256 MiB buffer"},
-            "decisions_per_sec": decisions * steps / (dev_ms * 1e-3),
+            "graph": {"device_step": False, "host_step": hgraph is not None},
+            "decisions_per_sec": cl.K * steps / (dev_ms * 1e-3),
             "kernel_ms": {k: float(np.mean(v)) for k, v in kt.items()},
             "e2e": {"value": units * steps / e2e_t, "unit": unit_name, "ms_per_step": 1e3 * e2e_t / steps,
                     "h2d_bytes_per_step": cl.K * 128, "d2h_bytes_per_step": cl.K * rec},
             "gpu_launches": int(launches), "clocks": clocks,
             "roofline": {"bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": alu_peak / 1e12,
                          "unit": "Tlane-op/s", "frac": achieved / alu_peak, "traffic": None, "kernel_ms": kms,
+                         "peak_pipe": {"issue_slots_per_unit": slots, "achieved": pipe / 1e12, "frac": pipe / alu_peak,
+                                       "note": "issue slots the kernel's instruction mix needs per unit (half-rate compare "
+                                               "and predicated min count 2 each) x units / kernel time / the same peak"},
+                         "ncu": _ncu_block(ncu_path),
                          "note": ops_note + f"; x {units} units / CUDA-event time of the kernel; peak = 148 SMs x "
                                  f"128 lanes/clk x sm_max_mhz ({peak_src})"},
-            "degeneracy": degeneracy, "cpu_baseline": cpu}
-    print(json.dumps(line), flush=True)
+            "degeneracy": shape, "cpu_baseline": cpu}
+    if not line["roofline"]["ncu"].get("missing"):
+        line["roofline"]["traffic"] = line["roofline"]["ncu"].get("dram_bytes")
     ctx.close()
+    return line
+
+
+def run_small_leg(args, torch, dev, workload, flush):
+    """configs[0] / configs[1]: the pod step at the two small configs (latency-bound: no roofline claim), the
+    placements and local configurations compared with the oracle in full."""
+    import paper_2606_30391_b200 as fs
+    import oracle
+    cl = synth.make_cluster(workload)
+    ctx = fs.Festina(dev.index or 0)
+    tb = lambda a: _tb(torch, dev, a)
+    ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                      tb(cl.models), cl.params)
+    d_states, d_reqs = tb(cl.states), tb(cl.requests)
+    d_place = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+    d_local = torch.empty(cl.K * 48, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(st):
+        ctx.set_gpu_state(d_states, stream=st)
+        ctx.place_batch(d_reqs, out=d_place, stream=st)
+        ctx.local_config(0, n=cl.K, out=d_local, stream=st)
+
+    for _ in range(3):
+        step(stream)
+    torch.cuda.synchronize()
+    graph = _capture(torch, dev, stream, step, f"the {workload} step") if args.graph else None
+    ms = 0.0
+    for _ in range(args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        if graph is not None:
+            graph.replay()
+        else:
+            step(stream)
+        b.record(stream); b.synchronize()
+        ms += a.elapsed_time(b)
+    cores = os.cpu_count() or 1
+    place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
+    local = d_local.cpu().numpy().view(synth.LOCAL_CFG_DT)
+    t0 = time.perf_counter()
+    ref = oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests, cores)
+    lref = oracle.local_config(cl.lat, cl.pow, cl.states, 0, None, cores)
+    dt = time.perf_counter() - t0
+    assert np.array_equal(ref["flat"], place["flat"]) and np.array_equal(ref["energy_mj"].view(np.uint32), place["energy_mj"].view(np.uint32))
+    assert np.array_equal(lref["flat"], local["flat"]) and np.array_equal(lref["beta"], local["beta"])
+    pairs, cand = synth.eligible_work(cl)
+    shape = _place_shape(cl, place)
+    shape.pop("hist_beta")
+    ctx.close()
+    return {"workload": f"{_workload_name(cl)}: K={cl.K}, M={cl.M}, F={cl.F}, S={cl.S}, B={cl.B}, R={cl.R}",
+            "ms_per_step": ms / args.steps, "graph": graph is not None,
+            "value": cand * args.steps / (ms * 1e-3), "unit": UNIT,
+            "decisions_per_sec": (cl.R + cl.K) * args.steps / (ms * 1e-3), "eligible_candidates_per_step": cand,
+            "cpu_baseline": {"value": cand / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"the whole config, compared in full, {dt:.2f} s"},
+            "degeneracy": shape, "note": "latency-bound at this size: no roofline claim"}
+
+
+def ncu_import(rep, out_path, command):
+    """`ncu -i rep --page raw --csv` -> the small tracked JSON summary the roofline blocks quote (per kernel launch
+    in the report; the first one is what bench.py reads).  Runs anywhere ncu is installed: no GPU needed."""
+    raw = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    rows = list(csv.reader(raw.splitlines()))
+    hdr = rows[0]
+    want = {"kernel": "Kernel Name", "duration_ns": "gpu__time_duration.sum",
+            "sm_throughput_pct": "sm__throughput.avg.pct_of_peak_sustained_elapsed",
+            "issue_active_pct": "smsp__issue_active.avg.pct_of_peak_sustained_active",
+            "warp_instructions": "smsp__inst_executed.sum",
+            "warps_active_pct": "sm__warps_active.avg.pct_of_peak_sustained_active",
+            "dram_read_bytes": "dram__bytes_read.sum", "dram_write_bytes": "dram__bytes_write.sum",
+            "pipe_alu_pct": "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active",
+            "pipe_fma_pct": "sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active",
+            "pipe_lsu_pct": "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active",
+            "l1tex_throughput_pct": "l1tex__throughput.avg.pct_of_peak_sustained_elapsed",
+            "lts_throughput_pct": "lts__throughput.avg.pct_of_peak_sustained_elapsed",
+            "registers_per_thread": "launch__registers_per_thread", "grid": "launch__grid_size", "block": "launch__block_size",
+            "sm_clock_ghz": "sm__cycles_elapsed.avg.per_second"}
+    units = dict(zip(hdr, rows[1]))
+    scale = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "byte": 1.0, "us": 1e3, "ms": 1e6, "ns": 1.0, "s": 1e9}
+    launches = []
+    for r in rows[2:]:
+        d = dict(zip(hdr, r))
+        o = {}
+        for k, m in want.items():
+            if m not in d:
+                continue
+            v = d[m]
+            if k == "kernel":
+                o[k] = v.split("(")[0][-120:]
+                continue
+            try:
+                x = float(v.replace(",", ""))
+            except ValueError:
+                continue
+            if k.endswith("_bytes") or k == "duration_ns":
+                x *= scale.get(units.get(m, ""), 1.0)
+            o[k] = x
+        stalls = {k[len("smsp__average_warps_issue_stalled_"):-len("_per_issue_active.ratio")]: float(v)
+                  for k, v in d.items() if k.startswith("smsp__average_warps_issue_stalled_") and k.endswith("_per_issue_active.ratio") and v}
+        tot = sum(stalls.values()) or 1.0
+        o["stall_pct"] = {k: round(100 * v / tot, 1) for k, v in sorted(stalls.items(), key=lambda x: -x[1])[:8]}
+        if "dram_read_bytes" in o:
+            o["dram_bytes"] = o["dram_read_bytes"] + o.get("dram_write_bytes", 0.0)
+        launches.append(o)
+    if not launches:
+        raise SystemExit(f"no kernel launch in {rep}")
+    dirty = bool(subprocess.run(["git", "status", "--porcelain", "--", "paper_2606_30391_b200"], cwd=ROOT, capture_output=True, text=True).stdout.strip())
+    summary = dict(launches[0])
+    summary.update({"captured_at_git_sha": _git_sha(), "sources_modified_since_that_commit": dirty,
+                    "command": command, "report": os.path.basename(rep), "launches_in_report": len(launches),
+                    "note": "figures of a run under the profiler (cold caches, serialised, ~40 replays): evidence for shares "
+                            "and counters, never a bench value"})
+    if len(launches) > 1:
+        summary["other_launches"] = launches[1:]
+    json.dump(summary, open(out_path, "w"), indent=1)
+    print(f"wrote {out_path}: {summary.get('kernel')} {summary.get('duration_ns', 0) / 1e3:.1f} us, "
+          f"{summary.get('warp_instructions', 0):.0f} warp instructions")
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
 
 
 def main():
@@ -607,17 +897,44 @@ def main():
     ap.add_argument("--workload", default="pod", choices=list(synth.CONFIGS))
     ap.add_argument("--cpu-requests", type=int, default=12288, help="oracle sample of the cpu_baseline leg")
     ap.add_argument("--ref-requests", type=int, default=1024, help="oracle sample per step of --impl reference")
-    ap.add_argument("--cpu-gpus", type=int, default=4096, help="oracle sample (GPUs) of --workload local")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--graph", type=int, default=1, help="1: replay the device step from a CUDA graph")
     ap.add_argument("--split-modes", default="exhaustive", choices=["exhaustive", "both"],
                     help="pod: fs_local_config once (all splits) or twice (all splits, then the per-task minimum-SM rule)")
     ap.add_argument("--overlap", type=int, default=1, help="1: fs_local_config on a second stream beside fs_place_batch")
+    ap.add_argument("--variants", type=int, default=1, help="1: time the scoring kernel on the reshaped pod workloads too")
+    ap.add_argument("--variant-sample", type=int, default=128, help="requests per variant recomputed by the oracle")
+    ap.add_argument("--aux", type=int, default=1, help="1: add the configs[3] / configs[4] / configs[0] / configs[1] legs")
+    ap.add_argument("--sustained-s", type=float, default=2.0, help="seconds of back-to-back replays for `sustained` (0: off)")
+    ap.add_argument("--ncu-import", default=None, help="an .ncu-rep to summarise (with --ncu-out); nothing is run on a GPU")
+    ap.add_argument("--ncu-out", default=None)
+    ap.add_argument("--ncu-cmd", default="", help="the ncu command line that made the report (recorded in the summary)")
     args = ap.parse_args()
+    if args.ncu_import:
+        ncu_import(args.ncu_import, args.ncu_out or NCU_POD, args.ncu_cmd)
+        return
     if args.impl == "reference":
         run_reference(args)
-    elif args.workload in ("local", "consol"):
-        run_aux(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N`: start the N ranks here (one process per GPU, NCCL), exactly as the driver's
+        # torch.distributed.run command line would
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        os.execv(sys.executable, cmd)
+    if args.workload in ("local", "consol"):
+        import torch
+        ws, rank, lrank = _dist()
+        if rank != 0:
+            return
+        dev = torch.device("cuda", lrank)
+        torch.cuda.set_device(dev)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        print(json.dumps(run_aux_leg(args, torch, dev, args.workload, flush)), flush=True)
     else:
         run_ours(args)
 

@@ -331,9 +331,11 @@ uint64_t fs_launch_count(const fs_ctx* ctx);
  *   out[1] cold (request, GPU) pairs found eligible      out[2] cold pairs swept after pruning
  *   out[3] cold candidates swept (sum of sm_free*F)      out[4] warm (model resident) pairs tested
  *   out[5] pairs scored candidate by candidate with the definition (warm pairs + tie recovery)
- *   out[6] candidates scored that way                    out[7] requests processed (x GPU slices) */
+ *   out[6] candidates scored that way                    out[7] requests processed (x GPU slices)
+ *   out[8] requests for which the (sigma, phi) tile was built (a cold pair could still win)        */
+#define FS_NSTATS 9
 int fs_set_work_stats(fs_ctx* ctx, int on);
-int fs_last_place_stats(fs_ctx* ctx, uint64_t out[8]);
+int fs_last_place_stats(fs_ctx* ctx, uint64_t out[FS_NSTATS]);
 
 /* Per-kernel device timing for measurement (bench.py's roofline line).  fs_set_timing(ctx, 1)
  * makes every later call record CUDA event pairs on its stream around its kernels;

@@ -351,10 +351,10 @@ class Festina:
 
     def last_place_stats(self) -> dict:
         """Work counters of the last fs_place_batch run with set_work_stats(True) (festina_eval.h)."""
-        o = (C.c_uint64 * 8)()
-        self._check(lib().fs_last_place_stats(self._h, o), "fs_last_place_stats")
         names = ("chunks_tested", "cold_pairs_eligible", "cold_pairs_swept", "cold_candidates_swept",
-                 "warm_pairs_tested", "pairs_scored", "candidates_scored", "requests")
+                 "warm_pairs_tested", "pairs_scored", "candidates_scored", "requests", "tiles_built")
+        o = (C.c_uint64 * len(names))()                  # FS_NSTATS
+        self._check(lib().fs_last_place_stats(self._h, o), "fs_last_place_stats")
         return {n: int(o[i]) for i, n in enumerate(names)}
 
     def set_timing(self, on: bool = True):

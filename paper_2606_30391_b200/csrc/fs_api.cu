@@ -161,13 +161,13 @@ int fs_create(fs_ctx** out, int cuda_device) {
   if (cudaSetDevice(cuda_device) != cudaSuccess ||
       cudaHostAlloc((void**)&c->flag_host, sizeof(int) * FS_NFLAGS, cudaHostAllocMapped) != cudaSuccess ||
       cudaHostGetDevicePointer((void**)&c->flag_dev, c->flag_host, 0) != cudaSuccess ||
-      cudaMalloc((void**)&c->stats, 8 * sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMalloc((void**)&c->stats, FS_NSTATS * sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return FS_ERR_CUDA;
   }
   std::memset(c->flag_host, 0, sizeof(int) * FS_NFLAGS);
-  cudaMemset(c->stats, 0, 8 * sizeof(unsigned long long));
+  cudaMemset(c->stats, 0, FS_NSTATS * sizeof(unsigned long long));
   fsk_local_smem_attr();
   fsk_place_smem_attr();
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
@@ -704,12 +704,12 @@ int fs_set_work_stats(fs_ctx* c, int on) {
   return FS_OK;
 }
 
-int fs_last_place_stats(fs_ctx* c, uint64_t out[8]) {
+int fs_last_place_stats(fs_ctx* c, uint64_t out[FS_NSTATS]) {
   if (!c || !out) return FS_ERR_ARG;
-  unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  unsigned long long h[FS_NSTATS] = {};
   FS_CUDA(c, cudaSetDevice(c->dev));
   FS_CUDA(c, cudaMemcpy(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost));
-  for (int i = 0; i < 8; ++i) out[i] = h[i];
+  for (int i = 0; i < FS_NSTATS; ++i) out[i] = h[i];
   return FS_OK;
 }
 

@@ -210,7 +210,7 @@ __device__ __forceinline__ void st_tile(float2* p, const float (&x)[NPHI], const
 }
 
 // work counters of a counting launch (fs_set_work_stats): per warp in shared memory, flushed per request
-enum { ST_CHUNKS = 0, ST_ELIG, ST_SWEPT, ST_CSWEPT, ST_WITEMS, ST_SCORED, ST_CSCORED, ST_REQ };
+enum { ST_CHUNKS = 0, ST_ELIG, ST_SWEPT, ST_CSWEPT, ST_WITEMS, ST_SCORED, ST_CSCORED, ST_REQ, ST_TILES, ST_N };
 
 template <int NPHI, bool VEC, bool COLS>
 __global__ void __launch_bounds__(DENSE_MAXW * 32, 1)
@@ -240,7 +240,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   uint64_t* w_bar = reinterpret_cast<uint64_t*>(s_warp + DENSE_BAR_OFF);
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_warp + DENSE_CNT_OFF);
   float2* tile = reinterpret_cast<float2*>(s_warp + DENSE_TILE_OFF);
-  if (lane == 0) { fs_mbar_init(w_bar, 1); fs_mbar_fence_init(); if (stats) { for (int i = 0; i < 8; ++i) s_cnt[i] = 0u; } }
+  if (lane == 0) { fs_mbar_init(w_bar, 1); fs_mbar_fence_init(); if (stats) { for (int i = 0; i < ST_N; ++i) s_cnt[i] = 0u; } }
   __syncwarp();
 
   const double* dsuf = v.dsuf + 1 + c0;
@@ -341,6 +341,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             }
             if (cold) {
               // ---- the request's tile: {t0, er} per (share, frequency), and the EXACT prefix minima of er
+              if (stats && lane == 0) s_cnt[ST_TILES] += 1u;
               const LaneLP q_lp1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, 0) + cb0, phi0, Fc);
               __syncwarp();
               if (bulk) {
@@ -601,7 +602,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     }
     if (stats) {
       __syncwarp();
-      if (lane < 8) { const uint32_t x = lane == ST_REQ ? 1u : s_cnt[lane]; if (x) atomicAdd(&stats[lane], (unsigned long long)x); s_cnt[lane] = 0u; }
+      if (lane < ST_N) { const uint32_t x = lane == ST_REQ ? 1u : s_cnt[lane]; if (x) atomicAdd(&stats[lane], (unsigned long long)x); s_cnt[lane] = 0u; }
       __syncwarp();
     }
     // ---- advance: the next request has landed in s_req
@@ -1252,7 +1253,7 @@ int fsk_place(const FsView& v, int R, const fs_request* reqs, fs_placement* out,
               const FsPlaceScratch& sc, cudaStream_t st, FsTimers* tm) {
   if (R <= 0) return 0;
   int launches = 0;
-  if (sc.count_work) cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * 8, st);
+  if (sc.count_work) cudaMemsetAsync(sc.stats, 0, sizeof(unsigned long long) * FS_NSTATS, st);
   if (v.K <= 0) {
     cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)R, st);
     place_decode_kernel<<<(R + 7) / 8, 256, 0, st>>>(v, R, reqs, sc.keys, out);

@@ -835,18 +835,24 @@ def test_step_is_capturable_into_a_cuda_graph(ctx):
     cmp.assert_local_equal(dl.cpu().numpy().view(synth.LOCAL_CFG_DT), _oracle_local(cl, 0))
 
 
-@pytest.mark.parametrize("variant", ["dynamic_power_x4", "cold_starts_feasible"])
+@pytest.mark.parametrize("variant", ["ties", "identical_gpus"])
+def test_rack_tie_variants_full(ctx, variant):
+    """configs[1] with tables quantised to a few powers of two and every SLO relaxed (ties inside a GPU), and with
+    eight GPU records repeated (exact ties ACROSS GPUs: no bound is strict, every GPU of the best kind is swept);
+    every tie must fall to the lowest flat index; compared in full."""
+    cl = synth.make_variant("rack", variant)
+    ctx.load_cluster(cl)
+    cmp.assert_placement_equal(ctx.place_batch(cl.requests), _oracle_place(cl))
+
+
+@pytest.mark.parametrize("variant", list(synth.VARIANTS))
 def test_pod_workload_variants_sampled(ctx, variant):
     """configs[2] with a less degenerate shape: 4x the dynamic power (chosen frequencies spread over the levels)
     or cheap weight loads (cold starts meet the TTFT deadline, so the sorted cold scan does the work)."""
-    cl = synth.make_cluster("pod")
-    if variant == "dynamic_power_x4":
-        cl.pow = (cl.pow + 3.0 * (cl.pow - cl.pow[:, :, :1])).astype(np.float32)
-    else:
-        cl.models["load_ms"] *= 0.05
+    cl = synth.make_variant("pod", variant)
     ctx.load_cluster(cl)
     got = ctx.place_batch(cl.requests)
-    idx = np.arange(0, cl.R, 256)
+    idx = np.arange(0, cl.R, 256 if variant in ("dynamic_power_x4", "cold_starts_feasible") else 1024)
     cmp.assert_placement_equal(got[idx], _oracle_place(cl, cl.requests[idx]))
     ok = got["gpu"] >= 0
     if variant == "dynamic_power_x4":
@@ -975,3 +981,33 @@ def test_dispatch_without_gpus_scales_out(fs):
     got2, after = c.dispatch_commit(cl.requests)
     assert (got2["gpu"] == -1).all() and len(after) == 0
     c.close()
+
+
+# ---- the N > 1 result gather on an NCCL group (one rank: what a single GPU can exercise) ---------------------
+def test_gather_records_on_an_nccl_group(tmp_path):
+    """shard.gather_records with a CUDA byte tensor (the buffer a FS_DEVICE call wrote) on the nccl backend."""
+    import subprocess
+    import sys
+    import textwrap
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = textwrap.dedent(f"""
+        import os, sys, numpy as np, torch, torch.distributed as dist
+        sys.path.insert(0, {root!r})
+        from paper_2606_30391_b200 import shard, synth
+        import paper_2606_30391_b200 as fs
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29631")
+        torch.cuda.set_device(0)
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+        cl = synth.make_custom(seed=77, K=13, M=4, F=8, S=8, B=8, R=101, lo=1, hi=3)
+        ctx = fs.Festina(0); ctx.load_cluster(cl)
+        dev = torch.device("cuda", 0)
+        d_req = torch.from_numpy(cl.requests.view(np.uint8).reshape(-1).copy()).to(dev)
+        d_out = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+        ctx.place_batch(d_req, out=d_out); torch.cuda.synchronize()
+        full = shard.gather_records(d_out, [cl.R], dist, dtype=synth.PLACEMENT_DT)
+        host = shard.gather_records(ctx.place_batch(cl.requests), [cl.R], dist)
+        assert full.tobytes() == host.tobytes() == d_out.cpu().numpy().tobytes()
+        dist.destroy_process_group(); print("gather ok")
+    """)
+    p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300)
+    assert p.returncode == 0 and "gather ok" in p.stdout, (p.stdout + p.stderr)[-3000:]

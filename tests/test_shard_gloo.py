@@ -36,6 +36,10 @@ def _worker(rank, world, port, out_dir):
     lmine = oracle.local_config(cl.lat, cl.pow, cl.states, 0, np.arange(glo, ghi, dtype=np.int32))
     lsizes = [shard.shard_range(cl.K, r, world)[1] - shard.shard_range(cl.K, r, world)[0] for r in range(world)]
     lfull = shard.gather_records(lmine, lsizes, dist)
+    # the same exchange from a torch byte tensor (what a FS_DEVICE call leaves behind), with the record dtype
+    import torch
+    tfull = shard.gather_records(torch.from_numpy(mine.view(np.uint8).reshape(-1).copy()), sizes, dist, dtype=mine.dtype)
+    assert tfull.tobytes() == full.tobytes()
     if rank == 0:
         ref = oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests)
         lref = oracle.local_config(cl.lat, cl.pow, cl.states, 0)
