@@ -40,7 +40,7 @@ struct fs_ctx {
   bool zero_copy = true;   // FS_ZERO_COPY=0 in the environment: bulk copies for FS_HOST_PINNED too
   size_t a1_cap = 0; unsigned char* a1_buf = nullptr; size_t pl_cap = 0; unsigned char* pl_buf = nullptr;
   // consolidation scratch
-  size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float4* agg = nullptr;
+  size_t consol_cap = 0; uint8_t* need = nullptr; float* E = nullptr; float2* E2 = nullptr; uint32_t* T2 = nullptr; float4* agg = nullptr;
   unsigned long long* ckeys = nullptr; fs_consol_out* consol_dev = nullptr;
   // diagnostics
   int* flag_host = nullptr; int* flag_dev = nullptr;
@@ -183,7 +183,7 @@ int fs_destroy(fs_ctx* c) {
   void* ptrs[] = {c->lat, c->pow, c->lpT, c->pmin, c->freq, c->models, c->comp, c->comp_n, c->states,
                   c->ginfo, c->gA, c->grec, c->gsort, c->dsort, c->dsuf, c->gA0, c->ctr, c->warm_off, c->warm_cursor, c->warm_item, c->keys, c->stats,
                   c->reqs_dev, c->place_dev, c->bin_off, c->bin_cursor, c->keylist, c->nkeys, c->lslots, c->G, c->ids_dev, c->local_dev, c->need, c->E,
-                  c->agg, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf, c->pl_buf};
+                  c->agg, c->E2, c->T2, c->ckeys, c->consol_dev, c->bt_ids, c->bt_off, c->bt_tasks, c->bt_out, c->a1_buf, c->pl_buf};
   bool ok = true;
   for (void* p : ptrs) if (p) ok = (cudaFree(p) == cudaSuccess) && ok;
   if (c->flag_host) ok = (cudaFreeHost(c->flag_host) == cudaSuccess) && ok;
@@ -382,12 +382,14 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
   if (c->K == 0) return pending;
   const size_t kf = (size_t)c->K * c->d.F;
   if (kf > c->consol_cap) {
+    const size_t kp = (size_t)c->K * ((c->d.F + 1) / 2 + 1);   // frequency pairs + one row: the pair kernel prefetches one trip ahead
     FS_TRY(grow(c, c->need, kf)); FS_TRY(grow(c, c->E, kf)); FS_TRY(grow(c, c->agg, (size_t)c->K));
+    FS_TRY(grow(c, c->E2, kp)); FS_TRY(grow(c, c->T2, kp));
     FS_TRY(grow(c, c->ckeys, (size_t)c->K)); FS_TRY(grow(c, c->consol_dev, (size_t)c->K));
     c->consol_cap = kf;
   }
   fs_consol_out* d_out = space != FS_DEVICE ? c->consol_dev : out;
-  FsConsolScratch sc{c->need, c->E, c->agg, c->ckeys};
+  FsConsolScratch sc{c->need, c->E, c->E2, c->T2, c->agg, c->ckeys};
   c->launches += fsk_consolidate(view_of(c), c->prm, d_out, sc, st, c->timing ? &c->tm : nullptr);
   FS_TRY(check_kernel(c));
   if (space != FS_DEVICE) {

@@ -6,6 +6,8 @@
 //   C*_g   = min_phi { E_g[phi] : need_g[phi] <= S_eff }
 //   C*_ab  = min_phi { fl(E_b[phi]+E_a[phi]) : need_a[phi]+need_b[phi] <= S_eff }  (lowest phi)
 //   score(a->b) = fl(C*_ab - C*_b);   dst(a) = argmin_b (score, b)  as one 64-bit key
+#include <cuda_fp16.h>
+
 #include "fs_kernels.h"
 
 namespace {
@@ -89,21 +91,43 @@ __global__ void __launch_bounds__(128) consol_agg_kernel(FsView v, int S_eff,
   }
 }
 
+// ---- what the pair kernel streams per destination: per frequency PAIR one {E[phi], E[phi+1]} and one packed
+// pair of binary16 values S_eff - need (small integers: exact); a frequency past F-1 is never feasible.
+// One more row than ceil(F/2) is allocated: the pair kernel's prefetch of the trip after the last needs no clamp.
+__global__ void consol_pack_kernel(int K, int F, int S_eff, const uint8_t* __restrict__ need, const float* __restrict__ E,
+                                   float2* __restrict__ E2, uint32_t* __restrict__ T2) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x, pp = blockIdx.y;
+  if (b >= K) return;
+  const int p0 = 2 * pp, p1 = 2 * pp + 1;
+  const bool h1 = p1 < F;
+  const float e1 = h1 ? E[(size_t)p1 * K + b] : FS_INF;
+  const int n0 = (int)need[(size_t)p0 * K + b], n1 = h1 ? (int)need[(size_t)p1 * K + b] : FS_NEED_INF;
+  const __half2 t = __halves2half2(__int2half_rn(S_eff - n0), __int2half_rn(S_eff - n1));
+  E2[(size_t)pp * K + b] = make_float2(E[(size_t)p0 * K + b], e1);
+  T2[(size_t)pp * K + b] = *reinterpret_cast<const uint32_t*>(&t);
+}
+
 // ---- a10: pair scoring; one block = TA sources x all destinations ----------------------------
 __global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
     FsView v, int S_eff, float mem_cap_mb, int delta_pct, const uint8_t* __restrict__ need, const float* __restrict__ E,
+    const float2* __restrict__ E2, const uint32_t* __restrict__ T2,
     const float4* __restrict__ agg, unsigned long long* __restrict__ keys) {
   extern __shared__ unsigned char smem_raw[];
   // M_eff = fl(fl(cap * (100 - delta)) / 100): the 5 % margin on memory (R:s19)
   const float M_eff = __fdiv_rn(__fmul_rn(mem_cap_mb, (float)(100 - delta_pct)), 100.0f);
   const int F = v.d.F, K = v.K;
-  float2* sEN = reinterpret_cast<float2*>(smem_raw);               // [F][TA] {E_a, need_a as int bits}: one LDS.64
+  // [ceil(F/2)][TA] {E_a[phi], E_a[phi+1], need_a of both as two binary16 values, -}: one LDS.128 per source and
+  // frequency pair, read by broadcast; a frequency past F-1 is never feasible (E = INF, need = FS_NEED_INF)
+  float4* sEN = reinterpret_cast<float4*>(smem_raw);
   __shared__ unsigned long long sred[TA][PAIR_THREADS / 32];
-  const int a0 = blockIdx.x * TA;
-  for (int x = threadIdx.x; x < F * TA; x += blockDim.x) {
-    const int phi = x / TA, a = a0 + x % TA;
-    sEN[x] = make_float2(a < K ? E[(size_t)phi * K + a] : FS_INF,
-                         __int_as_float(a < K ? (int)need[(size_t)phi * K + a] : FS_NEED_INF));
+  const int a0 = blockIdx.x * TA, FP = (F + 1) / 2;
+  for (int x = threadIdx.x; x < FP * TA; x += blockDim.x) {
+    const int pp = x / TA, a = a0 + x % TA, p0 = 2 * pp, p1 = 2 * pp + 1;
+    const bool h0 = a < K, h1 = a < K && p1 < F;
+    const float e0 = h0 ? E[(size_t)p0 * K + a] : FS_INF, e1 = h1 ? E[(size_t)p1 * K + a] : FS_INF;
+    const int n0 = h0 ? (int)need[(size_t)p0 * K + a] : FS_NEED_INF, n1 = h1 ? (int)need[(size_t)p1 * K + a] : FS_NEED_INF;
+    const __half2 nn = __halves2half2(__int2half_rn(n0), __int2half_rn(n1));     // small integers: exact
+    sEN[x] = make_float4(e0, e1, __uint_as_float(*reinterpret_cast<const uint32_t*>(&nn)), 0.0f);
   }
   __syncthreads();
   float4 ag[TA];
@@ -114,26 +138,64 @@ __global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
   for (int t = 0; t < TA; ++t) best[t] = FS_KEY_NONE;
   // two destinations per thread and trip: the broadcast read of a source's (E, need) serves both; per
   // (source, destination, phi) one add, one integer compare and one predicated min
-  for (int b0 = threadIdx.x; b0 < K; b0 += 2 * blockDim.x) {
+  // blockIdx.y = a slice of the destinations (finer blocks: the grid is several waves deep and its tail short);
+  // the slices' minima meet in keys[] by atomicMin
+  const int per = (K + (int)gridDim.y - 1) / (int)gridDim.y;
+  const int bs = blockIdx.y * per, be = min(K, bs + per);
+  for (int b0 = bs + threadIdx.x; b0 < be; b0 += 2 * blockDim.x) {
     const int b1 = b0 + blockDim.x;
-    const bool two = b1 < K;
+    const bool two = b1 < be;
     const int b1c = two ? b1 : b0;
     float cab0[TA], cab1[TA];
 #pragma unroll
     for (int t = 0; t < TA; ++t) cab0[t] = cab1[t] = FS_INF;
-    for (int phi = 0; phi < F; ++phi) {
-      const float e0 = E[(size_t)phi * K + b0], e1 = E[(size_t)phi * K + b1c];
-      const int thr0 = S_eff - (int)need[(size_t)phi * K + b0], thr1 = S_eff - (int)need[(size_t)phi * K + b1c];
+    // two frequencies per trip, software-pipelined: the eight values of the NEXT trip (E and need of both
+    // destinations) are requested before the current trip's 2 x TA x 2 candidates are scored, so the loads'
+    // latency hides behind the arithmetic (the kernel waited on them for 40 % of its issue slots before)
+    // Two frequencies per trip.  Per (source, destination, frequency pair): ONE packed binary16 compare gives both
+    // feasibility predicates (need_a + need_b <= S_eff  <=>  need_a <= S_eff - need_b; HSETP2), two adds, two
+    // selects of +INF and one three-input min (FMNMX3): 3.25 instructions per (pair, frequency) instead of 4, and
+    // half the work of the ALU pipe, which bound this kernel.
+    // The destinations' values come packed per frequency pair (consol_pack_kernel): one 64-bit and one 32-bit load
+    // per destination and trip, on running pointers.  Software-pipelined: the next trip's values are requested
+    // before this trip is scored (one row of padding behind the last pair: no clamp).
+    float ec[2][2]; uint32_t tc[2];                      // E [phi in trip][destination]; S_eff - need of both phis, packed, [destination]
+    const float2* pe0 = E2 + b0; const float2* pe1 = E2 + b1c;
+    const uint32_t* pt0 = T2 + b0; const uint32_t* pt1 = T2 + b1c;
+#define FS_PAIR_LOAD(EC, TC)                                                                              \
+    {                                                                                                     \
+      const float2 x0 = *pe0, x1 = *pe1;                                                                  \
+      EC[0][0] = x0.x; EC[1][0] = x0.y; EC[0][1] = x1.x; EC[1][1] = x1.y; TC[0] = *pt0; TC[1] = *pt1;     \
+    }
+    FS_PAIR_LOAD(ec, tc)
+    const float4* sp = sEN;
+    for (int pp = 0; pp < FP; ++pp) {
+      pe0 += K; pe1 += K; pt0 += K; pt1 += K;
+      float en_[2][2]; uint32_t tn_[2];
+      FS_PAIR_LOAD(en_, tn_)
 #pragma unroll
       for (int t = 0; t < TA; ++t) {
-        const float2 en = sEN[phi * TA + t];
-        const int na = __float_as_int(en.y);
-        asm("{.reg .pred p; setp.le.s32 p, %1, %2; @p min.f32 %0, %0, %3;}"    // INF never wins
-            : "+f"(cab0[t]) : "r"(na), "r"(thr0), "f"(__fadd_rn(e0, en.x)));
-        asm("{.reg .pred p; setp.le.s32 p, %1, %2; @p min.f32 %0, %0, %3;}"
-            : "+f"(cab1[t]) : "r"(na), "r"(thr1), "f"(__fadd_rn(e1, en.x)));
+        const float4 en = sp[t];
+        const uint32_t na2 = __float_as_uint(en.z);
+        asm("{.reg .pred p, q; .reg .f32 y0, y1;\n\t"
+            "setp.le.f16x2 p|q, %3, %4;\n\t"
+            "selp.f32 y0, %1, 0f7F800000, p;\n\t"
+            "selp.f32 y1, %2, 0f7F800000, q;\n\t"
+            "min.f32 %0, %0, y0, y1;}"
+            : "+f"(cab0[t]) : "f"(__fadd_rn(ec[0][0], en.x)), "f"(__fadd_rn(ec[1][0], en.y)), "r"(na2), "r"(tc[0]));
+        asm("{.reg .pred p, q; .reg .f32 y0, y1;\n\t"
+            "setp.le.f16x2 p|q, %3, %4;\n\t"
+            "selp.f32 y0, %1, 0f7F800000, p;\n\t"
+            "selp.f32 y1, %2, 0f7F800000, q;\n\t"
+            "min.f32 %0, %0, y0, y1;}"
+            : "+f"(cab1[t]) : "f"(__fadd_rn(ec[0][1], en.x)), "f"(__fadd_rn(ec[1][1], en.y)), "r"(na2), "r"(tc[1]));
       }
+      sp += TA;
+#pragma unroll
+      for (int u = 0; u < 2; ++u) { ec[u][0] = en_[u][0]; ec[u][1] = en_[u][1]; }
+      tc[0] = tn_[0]; tc[1] = tn_[1];
     }
+#undef FS_PAIR_LOAD
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       if (h == 1 && !two) break;
@@ -163,7 +225,7 @@ __global__ void __launch_bounds__(PAIR_THREADS) consol_pair_kernel(
   if (threadIdx.x < TA && a0 + threadIdx.x < K) {
     unsigned long long kk = FS_KEY_NONE;
     for (int w = 0; w < PAIR_THREADS / 32; ++w) kk = sred[threadIdx.x][w] < kk ? sred[threadIdx.x][w] : kk;
-    keys[a0 + threadIdx.x] = kk;
+    if (kk != FS_KEY_NONE) atomicMin(&keys[a0 + threadIdx.x], kk);
   }
 }
 
@@ -204,12 +266,15 @@ int fsk_consolidate(const FsView& v, const fs_params& prm, fs_consol_out* out,
   fs_tm_beg(tm, FS_T_CONSOL_AGG, st);
   consol_agg_kernel<<<(v.K + 3) / 4, 128, 0, st>>>(v, S_eff, sc.need, sc.E, sc.agg);
   fs_tm_end(tm, FS_T_CONSOL_AGG, st);
-  const size_t smem = sizeof(float2) * v.d.F * TA;
+  const size_t smem = sizeof(float4) * ((v.d.F + 1) / 2) * TA;
   fs_tm_beg(tm, FS_T_CONSOL_PAIR, st);
-  consol_pair_kernel<<<(v.K + TA - 1) / TA, PAIR_THREADS, smem, st>>>(v, S_eff, prm.mem_cap_mb, prm.delta_pct,
-                                                                    sc.need, sc.E, sc.agg, sc.keys);
+  consol_pack_kernel<<<dim3((v.K + 255) / 256, (v.d.F + 1) / 2), 256, 0, st>>>(v.K, v.d.F, S_eff, sc.need, sc.E, sc.E2, sc.T2);
+  cudaMemsetAsync(sc.keys, 0xFF, sizeof(unsigned long long) * (size_t)v.K, st);
+  const int nds = max(1, min(8, v.K / (4 * PAIR_THREADS)));          // destination slices: >= 2 trips of 2 x 256 each
+  consol_pair_kernel<<<dim3((v.K + TA - 1) / TA, nds), PAIR_THREADS, smem, st>>>(v, S_eff, prm.mem_cap_mb, prm.delta_pct,
+                                                                    sc.need, sc.E, sc.E2, sc.T2, sc.agg, sc.keys);
   fs_tm_end(tm, FS_T_CONSOL_PAIR, st);
   consol_decode_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, S_eff, prm, sc.need, sc.E, sc.agg,
                                                           sc.keys, out);
-  return 3;
+  return 4;
 }

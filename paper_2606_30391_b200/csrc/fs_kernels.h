@@ -92,6 +92,8 @@ int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs
 struct FsConsolScratch {
   uint8_t* need;     // [F][K]  sum of minimum shares per frequency, FS_NEED_INF = none
   float* E;          // [F][K]  slot-order energy at those shares
+  float2* E2;        // [ceil(F/2)+1][K]  {E[phi], E[phi+1]} per frequency pair (what the pair kernel streams)
+  uint32_t* T2;      // [ceil(F/2)+1][K]  S_eff - need of the pair as two binary16 values
   float4* agg;       // [K]     {mem, C*, mig, n_res as float bits}
   unsigned long long* keys;  // [K] per-source argmin key (score, dst)
 };
