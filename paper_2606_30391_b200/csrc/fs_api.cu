@@ -347,7 +347,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
     c->n_cap = n;
   }
   if (c->d.M > c->bin_m_cap) {
-    FS_TRY(grow(c, c->bin_off, (size_t)c->d.M * 16 + 1)); FS_TRY(grow(c, c->bin_cursor, (size_t)c->d.M * 16));
+    FS_TRY(grow(c, c->bin_off, (size_t)c->d.M * 2 * FS_LOCAL_QB + 1)); FS_TRY(grow(c, c->bin_cursor, (size_t)c->d.M * 2 * FS_LOCAL_QB));
     FS_TRY(grow(c, c->keylist, (size_t)c->d.M * 2)); FS_TRY(grow(c, c->nkeys, (size_t)1));
     c->bin_m_cap = c->d.M;
   }

@@ -52,9 +52,10 @@ struct __align__(16) FsGpuRec {
 static_assert(sizeof(FsGpuRec) == 32, "FsGpuRec layout");
 // Prefix minima of one plane (model, phase, batch bucket) over shares <= s and all phi (fs_tables.cu)
 struct __align__(16) FsPlaneMin {
-  double lp;                // min of the exact product LAT*POW
+  float lpf;                // min of the exact product LAT*POW, times (1 - 2^-22), rounded DOWN to binary32
   float lmin;               // min LAT
-  float pmax;               // max POW
+  float eta;                // 2^-149 * (max POW + 1), rounded UP
+  float _pad;
 };
 static_assert(sizeof(FsPlaneMin) == 16, "FsPlaneMin layout");
 // One (GPU k, tenant slot j) that hosts a model: what a request of that model needs to bound and
@@ -65,8 +66,8 @@ struct __align__(16) FsWarmItem {
   int32_t sm_free;
   float t_avail_ms, mem_free_mb, e_cur;
   float a_min;              // min over phi of A[k][1+j][phi]
-  double lp1;               // FsPlaneMin of plane (model, decode, br1) at share sm_free - 1
-  float l1_min, p1_max;
+  float lp1f, eta1, l1_min; // FsPlaneMin of plane (model, decode, br1) at share sm_free - 1
+  uint32_t _pad0;
   int32_t f_cur;            // F_curr of the GPU
   uint32_t magic;           // ceil(2^32 / (br1+1)) for br1 >= 1 (0: br1 == 0): rounds by multiply-high
   uint32_t _pad[2];
@@ -82,8 +83,9 @@ __device__ __forceinline__ size_t fs_idx(const FsDimsDev& d, int m, int p, int f
   return ((((size_t)m * 2 + p) * d.F + f) * d.S + s) * d.B + b;
 }
 // plane layout    [M][2][B][S][F]  (phi fastest): one (sigma,phi) plane per (model,phase,beta)
+// (the plane's index fits 32 bits: M <= 32767, B <= 256; one widening multiply by S*F <= 8192 forms the offset)
 __device__ __forceinline__ size_t fs_plane(const FsDimsDev& d, int m, int p, int b) {
-  return (((size_t)m * 2 + p) * d.B + b) * (size_t)d.S * d.F;
+  return (size_t)(uint32_t)((m * 2 + p) * d.B + b) * (size_t)(uint32_t)(d.S * d.F);
 }
 
 // ---- arithmetic ---------------------------------------------------------------------------
@@ -103,13 +105,18 @@ __device__ __forceinline__ float fs_unorderable(uint32_t o) {
 __device__ __forceinline__ unsigned long long fs_make_key(float v, uint32_t flat) {
   return ((unsigned long long)fs_orderable(v) << 32) | flat;
 }
+// warp-wide minimum of a 64-bit key by two 32-bit reductions (redux.sync): the high words first, then the low
+// words of the lanes that hold the minimal high word (all 32 lanes must call it)
+__device__ __forceinline__ uint32_t fs_redux_min_u32(uint32_t x) {
+  uint32_t r;
+  asm volatile("redux.sync.min.u32 %0, %1, 0xffffffff;" : "=r"(r) : "r"(x));
+  return r;
+}
 __device__ __forceinline__ unsigned long long fs_warp_min_key(unsigned long long k) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    unsigned long long other = __shfl_xor_sync(0xffffffffu, k, o);
-    k = other < k ? other : k;
-  }
-  return k;
+  const uint32_t hi = (uint32_t)(k >> 32), lo = (uint32_t)k;
+  const uint32_t mh = fs_redux_min_u32(hi);
+  const uint32_t ml = fs_redux_min_u32(hi == mh ? lo : 0xFFFFFFFFu);
+  return ((unsigned long long)mh << 32) | ml;
 }
 
 // ceil(q / n) for q < 2^24, 1 <= n <= 256 by multiply-high: magic = ceil(2^32 / n) for n >= 2 (0 stands for
@@ -123,12 +130,13 @@ __device__ __forceinline__ uint32_t fs_ceil_div_magic(uint32_t q, uint32_t magic
 
 // A lower bound on e = fl(fl(fr*LAT)*POW) of EVERY entry of a plane prefix, fr >= 0 an integer below 2^24:
 // with u = 2^-24, eta = 2^-150 one rounding obeys fl(z) >= z(1-u) - eta for every z >= 0 (half an ulp, normal
-// or subnormal), hence e >= fr*LAT*POW*(1-u)^2 - eta*(POW+1) >= fr*lp*(1-2u) - eta*(pmax+1).  Evaluated in
-// binary64 with twice that slack and rounded down; never negative.  Exactness of the kernel's results does not
-// depend on how tight this is, only on its being a lower bound.
-__device__ __forceinline__ float fs_energy_lb(float fr, double lp, float pmax) {
-  const double x = (double)fr * lp * (1.0 - 0x1p-22) - 0x1p-149 * ((double)pmax + 1.0);
-  return x > 0.0 ? __double2float_rd(x) : 0.0f;
+// or subnormal), hence e >= fr*LAT*POW*(1-u)^2 - eta*(POW+1) >= fr*lp*(1-2u) - eta*(pmax+1), lp = min LAT*POW.
+// The table side (fs_tables.cu) stores lpf <= lp*(1-2^-22) and eta_f >= 2^-149*(pmax+1); here one multiply and one
+// subtract, both rounded DOWN, finish it; never negative.  Exactness of the kernel's results does not depend on
+// how tight this is, only on its being a lower bound.
+__device__ __forceinline__ float fs_energy_lb(float fr, float lpf, float eta_f) {
+  const float x = __fsub_rd(__fmul_rd(fr, lpf), eta_f);
+  return x > 0.0f ? x : 0.0f;
 }
 
 // The shared slot rule (Eq. 1; R:s11), given the two table values.

@@ -72,14 +72,15 @@ int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* 
                          FsWarmItem* items /*[4K]*/, cudaStream_t st);
 
 // fs_local.cu — per-slot batch search + SM-split search
+#define FS_LOCAL_QB 16    // queue-depth buckets per (model, phase) key of the slot search
 struct FsLocalScratch {
   float* G;               // [n][RMAX*2][F*S]  slot cost g_{i,p}[phi][sigma]
   const uint32_t* comp;   // [RMAX][ns_stride] SM splits in lexicographic order, sigma_i in byte i
   const uint32_t* comp_n; // [RMAX] number of splits NS = C(S-1, n_res-1)
   int ns_stride;
   // per-call grouping of the live slots by (model, phase, q bucket)
-  int32_t* bin_off;       // [M*2*8 + 1]
-  int32_t* bin_cursor;    // [M*2*8]
+  int32_t* bin_off;       // [M*2*FS_LOCAL_QB + 1]
+  int32_t* bin_cursor;    // [M*2*FS_LOCAL_QB]
   int32_t* keylist;       // [M*2] non-empty (model, phase) keys
   int32_t* nkeys;         // [1]
   void* slots;            // [n*8] 16-byte slot records

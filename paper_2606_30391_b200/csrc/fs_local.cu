@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
 // multiply-high with a per-beta magic constant (exact for q < 2^24, beta < 256).  Strict '<' in
 // ascending beta keeps the lowest beta on ties, as the definition wants.
 constexpr int LS_TR = 8;          // rows per tile
-constexpr int LS_QB = 8;          // q buckets per key (slots of similar depth share a warp)
+constexpr int LS_QB = FS_LOCAL_QB; // q buckets per key: slots of (nearly) the same depth share a warp, so its lanes stop together
 constexpr int LS_WARPS = 4;
 __constant__ uint32_t c_magic[FS_MAX_B];   // ceil(2^32 / (beta+1)), beta >= 1
 

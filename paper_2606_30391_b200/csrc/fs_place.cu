@@ -19,6 +19,19 @@ struct ReqCtx {
   int br0; uint32_t rounds0; bool valid;
 };
 
+// the same without rounds0 (the caller has a cheaper way to it)
+__device__ __forceinline__ ReqCtx make_req_nodiv(const FsView& v, const fs_request& rq) {
+  ReqCtx c;
+  c.valid = rq.model >= 0 && rq.model < v.d.M && rq.L < (1u << 24) && rq.o_pred < (1u << 24);
+  c.m = c.valid ? rq.model : 0; c.L = rq.L; c.O = (21u * rq.o_pred + 19u) / 20u;
+  c.mem = __fmul_rn(__uint2float_rn(rq.L + c.O), v.models[c.m].kv_mb_per_token);
+  c.slo_ttft = rq.slo_ttft_ms; c.slo_tbt = rq.slo_tbt_ms; c.load_ms = v.models[c.m].load_ms;
+  const uint32_t n0 = rq.L < (uint32_t)v.d.B ? rq.L : (uint32_t)v.d.B;   // min(L,B)
+  c.br0 = n0 ? (int)n0 - 1 : 0;
+  c.rounds0 = 0u;
+  return c;
+}
+
 __device__ __forceinline__ ReqCtx make_req(const FsView& v, const fs_request& rq) {
   ReqCtx c;
   c.valid = rq.model >= 0 && rq.model < v.d.M && rq.L < (1u << 24) && rq.o_pred < (1u << 24);
@@ -125,11 +138,7 @@ __device__ __forceinline__ bool has_model(uint32_t w0, uint32_t w1, uint32_t mm)
   return ((((x0 - 0x00010001u) & ~x0) | ((x1 - 0x00010001u) & ~x1)) & 0x80008000u) != 0u;
 }
 
-__device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) {
-  uint32_t r;
-  asm volatile("redux.sync.min.u32 %0, %1, 0xffffffff;" : "=r"(r) : "r"(x));
-  return r;
-}
+__device__ __forceinline__ uint32_t warp_min_u32(uint32_t x) { return fs_redux_min_u32(x); }
 
 // largest t >= 0 with fl(w + t) <= slo, or -1 if there is none.  fl(w + .) is monotone, so the
 // answer is characterised by g(T) <= slo < g(nextup(T)); a double-precision guess is verified
@@ -252,6 +261,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
   const bool bulk = (d.F & 1) == 0;                      // rows are 16-byte multiples at 16-byte aligned addresses
   const float* a0_lane = v.gA0 + cb0 + phi0;             // rows of gA0 are padded with +INF to FA columns: aligned
   const int ls = min(lane, d.S - 1);                     // lane <-> share for the bounds
+  const uint32_t magicB = fs_magic((uint32_t)d.B);
   uint32_t tile_parity = 0;
   // ---- request tickets: r_cur is being scored, r_nxt is on its way into s_req, the ticket after that is
   // requested while r_cur is scored (ticket -> request -> model info would otherwise be a serial chain of
@@ -273,9 +283,14 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
+    // the ticket after next: lane 0's atomic writes r_nn in place (predicated, no merge of a branch), and nothing
+    // reads it before the volatile shuffle at the end of the request, so the warp never waits for it here
     int r_nn = 0;
-    if (lane == 0) r_nn = (int)atomicAdd(&ctr[sci], 1u);
-    const ReqCtx c = make_req(v, rq);
+    asm volatile("{.reg .pred p; setp.eq.s32 p, %2, 0;\n\t@p atom.global.add.u32 %0, [%1], 1;}"
+                 : "+r"(r_nn) : "l"(ctr + sci), "r"(lane) : "memory");
+    ReqCtx c = make_req_nodiv(v, rq);
+    // rounds0 = ceil(L / min(L, B)): 1 when 0 < L < B, else by multiply-high with the block's constant for B
+    c.rounds0 = c.L < (uint32_t)d.B ? (c.L ? 1u : 0u) : fs_ceil_div_magic(c.L, magicB);
     unsigned long long key = FS_KEY_NONE; int kwin = 0;
     if (!c.valid) {
       if (lane == 0 && sci == 0) fs_raise(v.flag, FS_FLAG_REQUEST);
@@ -285,11 +300,12 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       const float fr0 = __uint2float_rn(c.rounds0), fO = __uint2float_rn(c.O);
       float b_t0, b_e0, b_er;
       {
-        const FsPlaneMin pm0 = v.pmin[(((size_t)c.m * 2 + 0) * d.B + c.br0) * d.S + ls];
-        const FsPlaneMin pm1 = v.pmin[(((size_t)c.m * 2 + 1) * d.B + 0) * d.S + ls];
+        // (32-bit indices: plane index < 2^24, S <= 32)
+        const FsPlaneMin pm0 = v.pmin[(uint32_t)(((c.m * 2 + 0) * d.B + c.br0) * d.S + ls)];
+        const FsPlaneMin pm1 = v.pmin[(uint32_t)(((c.m * 2 + 1) * d.B + 0) * d.S + ls)];
         b_t0 = __fmul_rn(fr0, pm0.lmin);
-        b_e0 = fs_energy_lb(fr0, pm0.lp, pm0.pmax);
-        b_er = (c.O == 0 || pm1.lmin <= c.slo_tbt) ? __fadd_rn(b_e0, fs_energy_lb(fO, pm1.lp, pm1.pmax)) : FS_INF;
+        b_e0 = fs_energy_lb(fr0, pm0.lpf, pm0.eta);
+        b_er = (c.O == 0 || pm1.lmin <= c.slo_tbt) ? __fadd_rn(b_e0, fs_energy_lb(fO, pm1.lpf, pm1.eta)) : FS_INF;
       }
       const LaneLP q_lp0 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 0, c.br0) + cb0, phi0, Fc);
       // an empty prefill / decode slot passes its deadline whatever the wait (slot rule, q == 0)
@@ -479,7 +495,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             if (it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
               have = true; sidx = it.sm_free - 1;
               wr1 = fs_ceil_div_magic(c.O, it.magic);
-              e1lb = fs_energy_lb(__uint2float_rn(wr1), it.lp1, it.p1_max);
+              e1lb = fs_energy_lb(__uint2float_rn(wr1), it.lp1f, it.eta1);
             }
           }
           const float e0lb = __shfl_sync(FULL, b_e0, sidx), t0lb = __shfl_sync(FULL, b_t0, sidx);
@@ -507,6 +523,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           p = make_pair(v, c, v.ginfo[k]);
         }
         if (p.ok) {
+          // the record step reads this GPU's summary if it wins: have it in L1 by then
+          if (wsrc >= 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(v.ginfo + k));
           if (stats && lane == 0) { s_cnt[ST_SCORED] += 1u; s_cnt[ST_CSCORED] += (uint32_t)(p.smf * d.F); }
           const LaneLP w_lp1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, p.br1) + cb0, phi0, Fc);
           const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F + cb0;
@@ -537,7 +555,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       const float e0 = __fmul_rn(t0, b0[BUF][u][i]);                                                   \
       const float e1 = __fmul_rn(__fmul_rn(fr1, a1[BUF][u][i]), b1[BUF][u][i]);                        \
       const float dE = __fsub_rn(__fadd_rn(ar[i], __fadd_rn(e0, e1)), p.ecur);   /* -0 == +0 in every compare below */ \
-      const bool ok = s < p.smf && __fadd_rn(wait_e, t0) <= ttft_e && a1[BUF][u][i] <= tbt_e;          \
+      /* rows past sm_free-1 are copies of the last row (clamped loads): the strict '<' below never takes them */ \
+      const bool ok = __fadd_rn(wait_e, t0) <= ttft_e && a1[BUF][u][i] <= tbt_e;                       \
       if (ok && dE < pb) { pb = dE; pflat = flat0 + (uint32_t)(s * d.F + i); }   /* INF never enters */ \
     }                                                                                                  \
   }

@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
   const FsDimsDev d = v.d;
   const int m = gi.model[i], br1 = gi.br1[i];
   float a_min = FS_INF;
-  FsPlaneMin pm; pm.lp = (double)FS_INF; pm.lmin = FS_INF; pm.pmax = 0.0f;
+  FsPlaneMin pm; pm.lpf = FS_INF; pm.lmin = FS_INF; pm.eta = 0.0f; pm._pad = 0.0f;
   for (int phi = lane; phi < d.F; phi += 32) a_min = fminf(a_min, v.gA[((size_t)k * FS_NVAR + 1 + i) * d.F + phi]);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) a_min = fminf(a_min, __shfl_xor_sync(0xffffffffu, a_min, o));
@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t*
     FsWarmItem it;
     it.k = k; it.j = i; it.br1 = br1; it.sm_free = gi.sm_free;
     it.t_avail_ms = gi.t_avail_ms; it.mem_free_mb = gi.mem_free_mb; it.e_cur = gi.e_cur;
-    it.a_min = a_min; it.lp1 = pm.lp; it.l1_min = pm.lmin; it.p1_max = pm.pmax; it.f_cur = gi.f_cur;
+    it.a_min = a_min; it.lp1f = pm.lpf; it.eta1 = pm.eta; it.l1_min = pm.lmin; it._pad0 = 0u; it.f_cur = gi.f_cur;
     it.magic = fs_magic((uint32_t)max(br1, 0) + 1u); it._pad[0] = it._pad[1] = 0;
     items[off[m] + atomicAdd(&cursor[m], 1)] = it;
   }

@@ -45,8 +45,9 @@ __global__ void __launch_bounds__(256) build_planes_kernel(const float* __restri
 }
 
 // pmin[m][p][b][s] over the plane (m, p, b), shares <= s and all phi: the minimum of the exact product
-// LAT*POW (binary64 holds the product of two binary32 values exactly), the minimum LAT and the maximum POW.
-// fs_energy_lb (fs_common.cuh) turns them into a lower bound on fl(fl(rounds*LAT)*POW) of every such entry.
+// LAT*POW (binary64 holds the product of two binary32 values exactly) shrunk by 2^-22 and rounded down, the
+// minimum LAT, and 2^-149 (max POW + 1) rounded up.  fs_energy_lb (fs_common.cuh) turns them into a lower
+// bound on fl(fl(rounds*LAT)*POW) of every such entry with two binary32 operations.
 __global__ void __launch_bounds__(128) plane_min_kernel(const float2* __restrict__ lpT, FsDimsDev d,
                                                        FsPlaneMin* __restrict__ pmin) {
   const int lane = threadIdx.x & 31;
@@ -67,7 +68,12 @@ __global__ void __launch_bounds__(128) plane_min_kernel(const float2* __restrict
       l = fminf(l, __shfl_xor_sync(0xffffffffu, l, o)); p = fmaxf(p, __shfl_xor_sync(0xffffffffu, p, o));
     }
     mlp = lp < mlp ? lp : mlp; ml = fminf(ml, l); xp = fmaxf(xp, p);
-    if (lane == 0) { FsPlaneMin o; o.lp = mlp; o.lmin = ml; o.pmax = xp; pmin[(size_t)w * d.S + s] = o; }
+    if (lane == 0) {
+      FsPlaneMin o;
+      o.lpf = __double2float_rd(mlp * (1.0 - 0x1p-22)); o.lmin = ml;
+      o.eta = __double2float_ru(0x1p-149 * ((double)xp + 1.0)); o._pad = 0.0f;
+      pmin[(size_t)w * d.S + s] = o;
+    }
   }
 }
 
