@@ -292,6 +292,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
     // rounds0 = ceil(L / min(L, B)): 1 when 0 < L < B, else by multiply-high with the block's constant for B
     c.rounds0 = c.L < (uint32_t)d.B ? (c.L ? 1u : 0u) : fs_ceil_div_magic(c.L, magicB);
     unsigned long long key = FS_KEY_NONE; int kwin = 0;
+    // the lane's warm item of this request: GPU, j | br1 << 8 | sm_free << 16 (0: none), rounds1, T_avail, Ecur
+    int wk = 0; uint32_t wpk = 0, wr1 = 0; float wta = 0.f, wec = 0.f;
     if (!c.valid) {
       if (lane == 0 && sci == 0) fs_raise(v.flag, FS_FLAG_REQUEST);
     } else {
@@ -318,8 +320,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       // attaining the minimum.  One code site serves both.
       //   warm bound:  dE >= fl(fl(a_min + fl(b_e0[sm_free-1] + e1lb)) - Ecur),  e1lb = fs_energy_lb(rounds1, ...)
       int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
-      uint32_t ordl = NONE32; int wk = 0;
-      uint32_t wpk = 0, wr1 = 0; float wta = 0.f, wec = 0.f;   // the lane's item: j | br1 << 8 | sm_free << 16, rounds1, T_avail, Ecur
+      uint32_t ordl = NONE32;
       bool recover = false; float bestW = FS_INF; uint32_t flat = NONE32;
       for (;;) {
         int k = KNONE;
@@ -523,8 +524,6 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           p = make_pair(v, c, v.ginfo[k]);
         }
         if (p.ok) {
-          // the record step reads this GPU's summary if it wins: have it in L1 by then
-          if (wsrc >= 0) asm volatile("prefetch.global.L1 [%0];" ::"l"(v.ginfo + k));
           if (stats && lane == 0) { s_cnt[ST_SCORED] += 1u; s_cnt[ST_CSCORED] += (uint32_t)(p.smf * d.F); }
           const LaneLP w_lp1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, p.br1) + cb0, phi0, Fc);
           const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F + cb0;
@@ -591,7 +590,19 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         const uint32_t fl = (uint32_t)key;
         // the winning GPU is known (kwin); one small division instead of three 32-bit ones
         const int ks = kwin, rem = (int)(fl - (uint32_t)(ks * d.S * d.F)), sgs = rem / d.F, phis = rem - sgs * d.F;
-        const PairCtx p = make_pair(v, c, v.ginfo[ks]);
+        // a warm winner's context is still in the lane that holds its list item (a GPU is listed once per model);
+        // only a cold winner reads the GPU's summary
+        PairCtx p;
+        const unsigned hit = __ballot_sync(FULL, wpk != 0u && wk == ks);
+        if (hit) {
+          const int src = __ffs(hit) - 1;
+          const uint32_t pk = __shfl_sync(FULL, wpk, src);
+          p.ok = true; p.j = (int)(pk & 0xFFu); p.var = p.j + 1; p.br1 = (int)((pk >> 8) & 0xFFu); p.smf = (int)(pk >> 16);
+          p.wait = __shfl_sync(FULL, wta, src); p.ecur = __shfl_sync(FULL, wec, src);
+          p.rounds1 = __shfl_sync(FULL, wr1, src);
+        } else {
+          p = make_pair(v, c, v.ginfo[ks]);
+        }
         const LaneLP q0 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 0, c.br0), phi0, d.F);
         const LaneLP q1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, p.br1), phi0, d.F);
         const float* Ar = v.gA + ((size_t)ks * FS_NVAR + p.var) * d.F;
