@@ -123,13 +123,12 @@ __device__ __forceinline__ Cand eval_cand(const FsView& v, const ReqCtx& c, cons
 //      walks the cold-capable GPUs in ascending d = a_min - Ecur, lane <-> GPU: eligibility and the exact
 //      lower bound fl(fl(a_min + bnd[sm_free]) - Ecur) against the incumbent; the survivors are swept
 //      (compare + predicated min per candidate); the walk stops when no later GPU can win;
-//  (d) re-scores a cold winner once with the definition to recover the lowest flat index attaining
-//      the minimum, and (one slice) writes the placement record.
+//  (d) for a cold winner recovers the lowest flat index attaining the minimum from the tile (first candidate
+//      in flat order whose definition value equals it), and (one slice) writes the placement record.
 // All loops are rolled so that the kernel stays inside the instruction cache.
 // =============================================================================================
 constexpr int DENSE_MAXW = 20;                // warps per block at most (registers: 65536 / 640 = 102 -> 96)
 constexpr int DENSE_SMEM_MAX = 224 * 1024;    // of the 227 KB a block may use
-constexpr int DENSE_S = FS_MAX_S;
 
 // does any of the four 16-bit models packed in (w0, w1) equal m?  (exact "has a zero halfword" test on the
 // XOR; the SIMD-in-a-word video instructions are emulated on this architecture and cost ~30 instructions)
@@ -315,9 +314,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
       // per-lane incumbent (best, bestk), ordered by (dE, GPU index): the scans are not in index order
       float best = FS_INF; int bestk = KNONE;
       uint32_t bflat = NONE32;   // flat index of the lane's incumbent when the definition body found it (warm pairs)
-      // ---- (b), (d) the definition, pair by pair, from the planes: first the WARM pairs (GPUs that already
-      // host model m), best bound first, then once more on a cold winner to recover the lowest flat index
-      // attaining the minimum.  One code site serves both.
+      // ---- (b) the definition, pair by pair, from the planes: the WARM pairs (GPUs that already host model m),
+      // best bound first.
       //   warm bound:  dE >= fl(fl(a_min + fl(b_e0[sm_free-1] + e1lb)) - Ecur),  e1lb = fs_energy_lb(rounds1, ...)
       int ib = warm_off[c.m]; const int ie = warm_off[c.m + 1];
       uint32_t ordl = NONE32;
@@ -485,6 +483,34 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             // lowest flat index, nothing to recover (a GPU is warm or cold for a request, never both)
             if (k != KNONE && best == bestW && bestk == k) flat = bflat;
             if (__any_sync(FULL, flat != NONE32)) k = KNONE;
+            if (k != KNONE) {
+              // a COLD winner (it can only come from a sweep, so the tile holds this request's {t0, er}): the lowest
+              // flat index attaining the minimum is the first (share, frequency) in flat order whose definition value
+              // fl(fl(A0 + er) - Ecur) equals it and whose t0 meets the deadline (t0 <= T*); the same values the
+              // definition computes (er = fl(e0 + e1), INF where the TBT deadline fails), read from the tile
+              const FsGpuInfo gi = v.ginfo[k];
+              const float wait = __fadd_rn(gi.t_avail_ms, c.load_ms);
+              const float Tst = c.L == 0 ? FS_INF : fs_tstar(wait, c.slo_ttft);
+              float arow[NPHI];
+              {
+                const float* ap = a0_lane + (size_t)k * (size_t)FA;
+                if (NPHI == 2) { const float2 t = *reinterpret_cast<const float2*>(ap); arow[0] = t.x; arow[NPHI - 1] = t.y; }
+                else arow[0] = ap[0];
+              }
+              const uint32_t flat0 = (uint32_t)(k * d.S * d.F + cb0 + phi0);
+              for (int s = 0; s < gi.sm_free; ++s) {
+                float tt[NPHI], ee[NPHI];
+                ld_tile<NPHI>(tile + s * FT + phi0, tt, ee);
+                uint32_t f = NONE32;
+#pragma unroll
+                for (int i = NPHI - 1; i >= 0; --i) {
+                  const float dE = __fsub_rn(__fadd_rn(arow[i], ee[i]), gi.e_cur);
+                  if (tt[i] <= Tst && dE == bestW) f = flat0 + (uint32_t)(s * d.F + i);
+                }
+                if (__any_sync(FULL, f != NONE32)) { flat = f; break; }
+              }
+              k = KNONE;
+            }
             break;
           }
           // next 32 items: lane <-> item
@@ -513,17 +539,15 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
         }
         if (k == KNONE) break;                            // no feasible candidate at all, or a warm winner
         // a warm pair's context comes from the item its lane holds (the item passed the memory, bucket and
-        // share tests when it was listed); only the recovery of a cold winner reads the GPU's summary
+        // share tests when it was listed): no dependent load of the GPU's summary
         PairCtx p;
-        if (wsrc >= 0) {
+        {
           const uint32_t pk = __shfl_sync(FULL, wpk, wsrc);
           p.ok = true; p.j = (int)(pk & 0xFFu); p.var = p.j + 1; p.br1 = (int)((pk >> 8) & 0xFFu); p.smf = (int)(pk >> 16);
           p.wait = __shfl_sync(FULL, wta, wsrc); p.ecur = __shfl_sync(FULL, wec, wsrc);
           p.rounds1 = __shfl_sync(FULL, wr1, wsrc);
-        } else {
-          p = make_pair(v, c, v.ginfo[k]);
         }
-        if (p.ok) {
+        {
           if (stats && lane == 0) { s_cnt[ST_SCORED] += 1u; s_cnt[ST_CSCORED] += (uint32_t)(p.smf * d.F); }
           const LaneLP w_lp1 = lane_lp<NPHI, VEC>(v.lpT + fs_plane(d, c.m, 1, p.br1) + cb0, phi0, Fc);
           const float* Ar = v.gA + ((size_t)k * FS_NVAR + p.var) * d.F + cb0;
@@ -535,9 +559,7 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           // two share rows per stage, software-pipelined: the four plane loads of the NEXT stage are issued
           // before the current one is scored, so a stage's latency hides behind the arithmetic of the one
           // before it.  Each lane keeps the minimum of ITS candidates of this pair and the first (lowest flat)
-          // candidate attaining it; merged into the incumbent afterwards, or, in the recovery pass, matched
-          // against the winner's value (the pair's minimum by the definition equals what the sweep found:
-          // monotone rounding).
+          // candidate attaining it; merged into the incumbent afterwards.
           float pb = FS_INF; uint32_t pflat = NONE32;
           const uint32_t flat0 = (uint32_t)(k * d.S * d.F + cb0 + phi0);
           float a0[2][2][NPHI], b0[2][2][NPHI], a1[2][2][NPHI], b1[2][2][NPHI];   // [stage buffer][row][phi]
@@ -570,10 +592,8 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
           }
 #undef FS_BODY_LOAD
 #undef FS_BODY_SCORE
-          if (recover) { if (pb == bestW) flat = pflat; }
-          else if (pb < best || (pb == best && k < bestk)) { best = pb; bestk = k; bflat = pflat; }
+          if (pb < best || (pb == best && k < bestk)) { best = pb; bestk = k; bflat = pflat; }
         }
-        if (recover) break;
       }
       key = flat != NONE32 ? fs_make_key(bestW, flat) : FS_KEY_NONE;
       key = fs_warp_min_key(key);
