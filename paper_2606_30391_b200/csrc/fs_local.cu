@@ -105,7 +105,7 @@ __global__ void local_keys_kernel(const int32_t* __restrict__ off, int nkeys_all
 
 // the body for one phase (P = key & 1): the deadline rule differs (prefill: whole queue; decode: one step), so the
 // candidate loop is compiled once per phase and the block picks its version once
-template <int P, bool OBJ_POWER>
+template <int P, bool OBJ_POWER, bool fill>
 __device__ __forceinline__ void local_slot_body(const FsView& v, const int key, unsigned char* ls_smem, uint64_t& bar,
                                                 const int32_t* __restrict__ off,
                                                 const LocalSlot* __restrict__ slots, float* __restrict__ Gs) {
@@ -129,19 +129,27 @@ __device__ __forceinline__ void local_slot_body(const FsView& v, const int key, 
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int s0 = off[key * LS_QB], s1 = off[(key + 1) * LS_QB];
-  // Rounds of LS_WARPS*32 slots, lane <-> slot.  A last round of fewer than 64 slots spreads them evenly over
-  // the warps and, when a warp gets <= 16 of them, gives each slot G = 2, 4, ... lanes
-  // that split the beta range (groups of four beta, interleaved); their minima are merged by shuffles
-  // (min is exact in any order).  At pod a (model, phase) key has ~40 slots: without this most lanes idle.
+  // Rounds of LS_WARPS*32 slots, lane <-> slot.  In a round that is not full the slots fill whole warps first
+  // (every lane busy) and the remaining r < 32 slots go to one more warp, where each slot gets G = 32 /
+  // pow2ceil(r) lanes that split the beta range (groups of four beta, interleaved; their minima are merged by
+  // shuffles: min is exact in any order): a warp left with 4 slots finishes 8 times sooner instead of running 4
+  // lanes over the whole range (4,096 GPUs: 0.761 -> 0.717 ms).  With `fill` = false (the per-phase launches used for grids
+  // of a few waves) only a round of fewer than 64 slots is split, and it is spread EVENLY over the block's warps,
+  // so that every warp works and the block is short (pod, ~40 slots per key: 0.185 against 0.194 - 0.213 ms).
   for (int start = s0; start < s1; start += LS_WARPS * 32) {
     const int n_round = min(LS_WARPS * 32, s1 - start);
-    int pad = 32, per = 32;
-    if (n_round < 64) {                                 // denser rounds keep lane <-> slot: splitting beta costs
-      per = (n_round + LS_WARPS - 1) / LS_WARPS;        // a second LDS wavefront per row, which only pays
-                                                        // when most lanes would idle otherwise
+    int pad = 32, per = 32, base = warp * 32;
+    if (!fill) {
+      if (n_round < 64) {
+        per = (n_round + LS_WARPS - 1) / LS_WARPS; base = warp * per;
+        pad = 1; while (pad < per) pad <<= 1;
+      }
+    } else if (n_round < LS_WARPS * 32) {
+      const int nfull = n_round >> 5, rem = n_round & 31;
+      per = warp < nfull ? 32 : (warp == nfull ? rem : 0);
       pad = 1; while (pad < per) pad <<= 1;
     }
-    const int G = 32 / pad, grp = lane / pad, sl_ix = warp * per + (lane % pad);
+    const int G = 32 / pad, grp = lane / pad, sl_ix = base + (lane % pad);
     const bool have = (lane % pad) < per && sl_ix < n_round;
     LocalSlot sl_ = have ? slots[start + sl_ix] : LocalSlot{0, 0u, 0.f, 0u};
     const uint32_t nb = have ? (sl_.meta >> 8) : 0u;
@@ -209,9 +217,9 @@ __global__ void __launch_bounds__(LS_WARPS * 32) local_slot_grouped_kernel(
   const int key = keylist[blockIdx.x];
   if (PSEL >= 0) {
     if ((key & 1) != PSEL) return;
-    local_slot_body<(PSEL > 0 ? 1 : 0), OBJ_POWER>(v, key, ls_smem, bar, off, slots, Gs);
-  } else if (key & 1) local_slot_body<1, OBJ_POWER>(v, key, ls_smem, bar, off, slots, Gs);
-  else                local_slot_body<0, OBJ_POWER>(v, key, ls_smem, bar, off, slots, Gs);
+    local_slot_body<(PSEL > 0 ? 1 : 0), OBJ_POWER, false>(v, key, ls_smem, bar, off, slots, Gs);
+  } else if (key & 1) local_slot_body<1, OBJ_POWER, true>(v, key, ls_smem, bar, off, slots, Gs);
+  else                local_slot_body<0, OBJ_POWER, true>(v, key, ls_smem, bar, off, slots, Gs);
 }
 
 // ---- steps 2-3: tenant sums, split search, argmin; one block per GPU -----------------------

@@ -833,6 +833,19 @@ def test_step_is_capturable_into_a_cuda_graph(ctx):
     torch.cuda.synchronize()
     cmp.assert_placement_equal(do.cpu().numpy().view(synth.PLACEMENT_DT), _oracle_place(cl))
     cmp.assert_local_equal(dl.cpu().numpy().view(synth.LOCAL_CFG_DT), _oracle_local(cl, 0))
+    # the next poll: other state records and other requests in the SAME device buffers, the same graph replayed.
+    # fs_set_gpu_state is inside the graph, so the scan order and the per-model lists are rebuilt by the replay
+    # (festina_eval.h: capture fs_set_gpu_state together with the placement calls that follow it)
+    cl2 = synth.make_cluster("rack", seed=11)
+    cl2.lat, cl2.pow, cl2.models = cl.lat, cl.pow, cl.models          # the tables stay those of the context
+    cl2.states["t"]["mem_used_mb"][...] = 0                           # (mem_used is not read by these two calls)
+    ds.copy_(tb(cl2.states)); dr.copy_(tb(cl2.requests))
+    do.zero_(); dl.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    cmp.assert_placement_equal(do.cpu().numpy().view(synth.PLACEMENT_DT), _oracle_place(cl2))
+    cmp.assert_local_equal(dl.cpu().numpy().view(synth.LOCAL_CFG_DT), _oracle_local(cl2, 0))
+    assert not np.array_equal(cl2.states["n_res"], cl.states["n_res"])
 
 
 @pytest.mark.parametrize("variant", ["ties", "identical_gpus"])
