@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(256) local_slot_kernel(FsView v, int n,
 // time: lane <-> slot, sequential over beta, LDS.128 broadcasts of four beta per row, rounds by
 // multiply-high with a per-beta magic constant (exact for q < 2^24, beta < 256).  Strict '<' in
 // ascending beta keeps the lowest beta on ties, as the definition wants.
-constexpr int LS_TR = 8;          // rows per tile
+constexpr int LS_TR = 16;         // rows per tile (a multiple of 8; 2 x 16 x B floats of shared memory: 32 KB at B = 256)
 constexpr int LS_QB = FS_LOCAL_QB; // q buckets per key: slots of (nearly) the same depth share a warp, so its lanes stop together
 constexpr int LS_WARPS = 4;
 __constant__ uint32_t c_magic[FS_MAX_B];   // ceil(2^32 / (beta+1)), beta >= 1
@@ -159,29 +159,37 @@ __device__ __forceinline__ void local_slot_body(const FsView& v, const int key, 
 #pragma unroll
     for (int r = 0; r < LS_TR; ++r) best[r] = FS_INF;
     for (uint32_t b4 = 4u * grp; b4 < maxnb; b4 += 4u * G) {
-      float4 L4[LS_TR], P4[LS_TR];
-#pragma unroll
-      for (int r = 0; r < LS_TR; ++r) {
-        L4[r] = *reinterpret_cast<const float4*>(sl + r * B + b4);
-        P4[r] = *reinterpret_cast<const float4*>(sp + r * B + b4);
-      }
+      // the four betas' round counts and deadlines once per lane and trip, shared by all rows of the tile
+      float fr[4], slo_b[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const uint32_t beta = b4 + u;
         const uint32_t rounds = beta == 0 ? sl_.q : __umulhi(sl_.q + beta, c_magic[beta]);
-        const float fr = __uint2float_rn(rounds);
+        fr[u] = __uint2float_rn(rounds);
         // beta past this slot's range: a deadline nothing meets (tables are > 0)
-        const float slo_b = beta < nb ? sl_.slo : -1.0f;
+        slo_b[u] = beta < nb ? sl_.slo : -1.0f;
+      }
 #pragma unroll
-        for (int r = 0; r < LS_TR; ++r) {
-          const float la = u == 0 ? L4[r].x : u == 1 ? L4[r].y : u == 2 ? L4[r].z : L4[r].w;
-          const float pw = u == 0 ? P4[r].x : u == 1 ? P4[r].y : u == 2 ? P4[r].z : P4[r].w;
-          const float t = __fmul_rn(fr, la);
-          const float cost = OBJ_POWER ? pw : __fmul_rn(t, pw);
-          // one compare + one predicated min per candidate (the ALU pipe binds this kernel);
-          // beta* is recovered for the chosen row only (split kernel)
-          asm("{.reg .pred p; setp.le.f32 p, %1, %2; @p min.f32 %0, %0, %3;}"
-              : "+f"(best[r]) : "f"(P == 0 ? t : la), "f"(slo_b), "f"(cost));
+      for (int rh = 0; rh < LS_TR; rh += 8) {          // eight rows at a time: 16 broadcast LDS.128 in flight
+        float4 L4[8], P4[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          L4[r] = *reinterpret_cast<const float4*>(sl + (rh + r) * B + b4);
+          P4[r] = *reinterpret_cast<const float4*>(sp + (rh + r) * B + b4);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const float la = u == 0 ? L4[r].x : u == 1 ? L4[r].y : u == 2 ? L4[r].z : L4[r].w;
+            const float pw = u == 0 ? P4[r].x : u == 1 ? P4[r].y : u == 2 ? P4[r].z : P4[r].w;
+            const float t = __fmul_rn(fr[u], la);
+            const float cost = OBJ_POWER ? pw : __fmul_rn(t, pw);
+            // one compare + one predicated min per candidate (the ALU pipe binds this kernel);
+            // beta* is recovered for the chosen row only (split kernel)
+            asm("{.reg .pred p; setp.le.f32 p, %1, %2; @p min.f32 %0, %0, %3;}"
+                : "+f"(best[rh + r]) : "f"(P == 0 ? t : la), "f"(slo_b[u]), "f"(cost));
+          }
         }
       }
     }
