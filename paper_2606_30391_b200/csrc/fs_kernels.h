@@ -68,9 +68,6 @@ int fsk_dispatch(const FsView& v, int R, const fs_request* reqs, fs_placement* o
                  const FsWarmItem* witems, cudaStream_t st, FsTimers* tm);
 int fsk_dispatch_commit(const FsView& v, int R, const fs_request* reqs, fs_placement* out, fs_gpu_avail* work,
                         cudaStream_t st, FsTimers* tm);
-int fsk_build_warm_lists(const FsView& v, int32_t* warm_off /*[M+1]*/, int32_t* warm_cursor /*[M]*/,
-                         FsWarmItem* items /*[4K]*/, cudaStream_t st);
-
 // fs_local.cu — per-slot batch search + SM-split search
 #define FS_LOCAL_QB 16    // queue-depth buckets per (model, phase) key of the slot search
 struct FsLocalScratch {

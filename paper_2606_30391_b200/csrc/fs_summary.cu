@@ -174,12 +174,11 @@ __global__ void __launch_bounds__(128) summary_kernel(FsView v, FsGpuInfo* __res
 // only decides how soon a request meets its best GPUs and can stop scanning (fs_place.cu).
 // rank of every record by (key, index): warp <-> record, lanes over the other records' keys
 // (written by the summary kernel), partial counts summed by shuffles
-__global__ void __launch_bounds__(256) order_rank_kernel(const FsGpuRec* __restrict__ grec,
-                                                        const float* __restrict__ okey, int Kpad,
-                                                        FsGpuRec* __restrict__ gsort,
-                                                        double* __restrict__ dsort) {
+__device__ __forceinline__ void order_rank_block(int bid, const FsGpuRec* __restrict__ grec,
+                                                 const float* __restrict__ okey, int Kpad,
+                                                 FsGpuRec* __restrict__ gsort, double* __restrict__ dsort) {
   const int lane = threadIdx.x & 31;
-  const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int i = bid * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (i >= Kpad) return;
   const float key = okey[i];
   int rank = 0;
@@ -203,9 +202,9 @@ __global__ void __launch_bounds__(256) order_rank_kernel(const FsGpuRec* __restr
 // dsuf[0] = max over the capable GPUs of max(a_min, |Ecur|) (INF if any is huge: no early stop);
 // dsuf[1+c] = min of d over sorted positions >= 32*c   (exact suffix minimum, in double);
 // dsuf[2+nchunk] = the earliest T_avail among the capable GPUs
-__global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __restrict__ gsort,
-                                                           const double* __restrict__ dsort, int nchunk,
-                                                           double* __restrict__ dsuf) {
+__device__ __forceinline__ void order_suffix_block(const FsGpuRec* __restrict__ gsort,
+                                                   const double* __restrict__ dsort, int nchunk,
+                                                   double* __restrict__ dsuf) {
   __shared__ double seg[1024];
   __shared__ float smax[32], smin[32];
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -256,8 +255,8 @@ __global__ void __launch_bounds__(1024) order_suffix_kernel(const FsGpuRec* __re
 }
 
 // ---- warm lists: for every model, the (GPU, tenant slot) pairs that host it -----------------
-__global__ void warm_count_kernel(FsView v, int32_t* __restrict__ cnt /*[M+1], zeroed*/) {
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+__device__ __forceinline__ void warm_count_block(int bid, const FsView& v, int32_t* __restrict__ cnt /*[M+1], zeroed*/) {
+  const int k = bid * blockDim.x + threadIdx.x;
   if (k >= v.K) return;
   const FsGpuInfo gi = v.ginfo[k];
   for (int i = 0; i < gi.n_res; ++i) {
@@ -265,6 +264,23 @@ __global__ void warm_count_kernel(FsView v, int32_t* __restrict__ cnt /*[M+1], z
     for (int j = 0; j < i; ++j) first = first && (gi.model[j] != gi.model[i]);
     if (first) atomicAdd(&cnt[gi.model[i] + 1], 1);
   }
+}
+// The placement preparation in three launches instead of five (each is launch latency, not work):
+//   A  blocks [0, nb_rank): rank sort of the scan order;  blocks [nb_rank, ...): count the warm pairs per model
+//   B  block 0: suffix minima of the scan order;          block 1: scan of the per-model counts
+//   C  fill the per-model lists
+__global__ void __launch_bounds__(256) prep_rank_count_kernel(FsView v, int nb_rank, const FsGpuRec* __restrict__ grec,
+                                                             const float* __restrict__ okey, FsGpuRec* __restrict__ gsort,
+                                                             double* __restrict__ dsort, int32_t* __restrict__ cnt) {
+  if ((int)blockIdx.x < nb_rank) order_rank_block((int)blockIdx.x, grec, okey, v.Kpad, gsort, dsort);
+  else warm_count_block((int)blockIdx.x - nb_rank, v, cnt);
+}
+__global__ void __launch_bounds__(1024) prep_suffix_scan_kernel(const FsGpuRec* __restrict__ gsort,
+                                                               const double* __restrict__ dsort, int nchunk,
+                                                               double* __restrict__ dsuf, int32_t* __restrict__ off,
+                                                               int32_t* __restrict__ cursor, int M) {
+  if (blockIdx.x == 0) order_suffix_block(gsort, dsort, nchunk, dsuf);
+  else fs_bucket_scan_block(off, cursor, M);
 }
 // one warp per (GPU, slot): lanes over phi reduce the bounds the placement kernel prunes with
 __global__ void __launch_bounds__(128) warm_fill_kernel(FsView v, const int32_t* __restrict__ off,
@@ -316,19 +332,11 @@ int fsk_place_prepare(const FsView& v, const FsGpuRec* grec, FsGpuRec* gsort, do
   if (v.K <= 0) return 0;
   fs_tm_beg(tm, FS_T_PLACE_WARM, st);
   const float* okey = reinterpret_cast<const float*>(dsuf + v.Kpad / FS_CHUNK + 4);   // written by the summary kernel
-  order_rank_kernel<<<(v.Kpad + 7) / 8, 256, 0, st>>>(grec, okey, v.Kpad, gsort, dsort);
-  order_suffix_kernel<<<1, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf);
-  const int n = fsk_build_warm_lists(v, warm_off, warm_cursor, items, st);
-  fs_tm_end(tm, FS_T_PLACE_WARM, st);
-  return 2 + n;
-}
-
-int fsk_build_warm_lists(const FsView& v, int32_t* warm_off, int32_t* warm_cursor,
-                         FsWarmItem* items, cudaStream_t st) {
-  if (v.K <= 0) return 0;
   cudaMemsetAsync(warm_off, 0, sizeof(int32_t) * (v.d.M + 1), st);
-  warm_count_kernel<<<(v.K + 127) / 128, 128, 0, st>>>(v, warm_off);
-  fs_bucket_scan_kernel<<<1, 1024, 0, st>>>(warm_off, warm_cursor, v.d.M);
+  const int nb_rank = (v.Kpad + 7) / 8, nb_count = (v.K + 255) / 256;
+  prep_rank_count_kernel<<<nb_rank + nb_count, 256, 0, st>>>(v, nb_rank, grec, okey, gsort, dsort, warm_off);
+  prep_suffix_scan_kernel<<<2, 1024, 0, st>>>(gsort, dsort, v.Kpad / FS_CHUNK, dsuf, warm_off, warm_cursor, v.d.M);
   warm_fill_kernel<<<(v.K * FS_RMAX + 3) / 4, 128, 0, st>>>(v, warm_off, warm_cursor, items);
+  fs_tm_end(tm, FS_T_PLACE_WARM, st);
   return 3;
 }
