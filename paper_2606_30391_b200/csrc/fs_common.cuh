@@ -202,7 +202,7 @@ __device__ __forceinline__ void fs_tma_load_1d(void* smem_dst, const void* gsrc,
 }
 
 // ---- counting-sort helper shared by the per-call bucketing passes ---------------------------
-// single-block inclusive scan of off[1..M] in place (off[0] = 0) and cursor[m] = 0
+// single-block (1,024 threads) inclusive scan of off[1..M] in place (off[0] = 0) and cursor[m] = 0
 __device__ __forceinline__ void fs_bucket_scan_block(int32_t* __restrict__ off, int32_t* __restrict__ cursor, int M) {
   __shared__ int32_t part[1024];
   const int t = threadIdx.x, per = (M + 1023) / 1024;
@@ -220,7 +220,4 @@ __device__ __forceinline__ void fs_bucket_scan_block(int32_t* __restrict__ off, 
   int32_t acc = part[t] - sum;
   if (t == 0) off[0] = 0;
   for (int m = lo; m < hi; ++m) { acc += off[m + 1]; off[m + 1] = acc; cursor[m] = 0; }
-}
-static __global__ void __launch_bounds__(1024) fs_bucket_scan_kernel(int32_t* __restrict__ off, int32_t* __restrict__ cursor, int M) {
-  fs_bucket_scan_block(off, cursor, M);
 }

@@ -96,11 +96,14 @@ __global__ void local_bin_fill_kernel(FsView v, int n, const int32_t* __restrict
   LocalSlot o; int bin;
   if (local_slot_of(v, gpu_ids, x >> 3, x & 7, o, bin)) slots[off[bin] + atomicAdd(&cursor[bin], 1)] = o;
 }
-__global__ void local_keys_kernel(const int32_t* __restrict__ off, int nkeys_all, int32_t* __restrict__ keylist,
-                                  int32_t* __restrict__ nkeys) {
-  const int key = blockIdx.x * blockDim.x + threadIdx.x;
-  if (key >= nkeys_all) return;
-  if (off[(key + 1) * LS_QB] > off[key * LS_QB]) keylist[atomicAdd(nkeys, 1)] = key;
+// one block: the scan of the bin counts, then the list of the non-empty (model, phase) keys (one launch, not two)
+__global__ void __launch_bounds__(1024) local_scan_keys_kernel(int32_t* __restrict__ off, int32_t* __restrict__ cursor, int nbins,
+                                                              int nkeys_all, int32_t* __restrict__ keylist,
+                                                              int32_t* __restrict__ nkeys) {
+  fs_bucket_scan_block(off, cursor, nbins);
+  __syncthreads();
+  for (int key = threadIdx.x; key < nkeys_all; key += blockDim.x)
+    if (off[(key + 1) * LS_QB] > off[key * LS_QB]) keylist[atomicAdd(nkeys, 1)] = key;
 }
 
 // the body for one phase (P = key & 1): the deadline rule differs (prefill: whole queue; decode: one step), so the
@@ -434,10 +437,9 @@ int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs
     cudaMemsetAsync(sc.bin_off, 0, sizeof(int32_t) * (size_t)(nbins + 1), st);
     cudaMemsetAsync(sc.nkeys, 0, sizeof(int32_t), st);
     local_bin_count_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(v, n, gpu_ids, sc.bin_off);
-    fs_bucket_scan_kernel<<<1, 1024, 0, st>>>(sc.bin_off, sc.bin_cursor, nbins);
+    local_scan_keys_kernel<<<1, 1024, 0, st>>>(sc.bin_off, sc.bin_cursor, nbins, nkeys_all, sc.keylist, sc.nkeys);
     local_bin_fill_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(v, n, gpu_ids, sc.bin_off, sc.bin_cursor,
                                                                reinterpret_cast<LocalSlot*>(sc.slots));
-    local_keys_kernel<<<(nkeys_all + 255) / 256, 256, 0, st>>>(sc.bin_off, nkeys_all, sc.keylist, sc.nkeys);
     const dim3 grid(min(nkeys_all, nslots), (rows + LS_TR - 1) / LS_TR);
     const size_t smem = sizeof(float) * 2 * LS_TR * v.d.B;
     const LocalSlot* sl = reinterpret_cast<const LocalSlot*>(sc.slots);
@@ -446,10 +448,10 @@ int fsk_local(const FsView& v, int n, const int32_t* gpu_ids, uint32_t flags, fs
     const bool power = flags & FS_OBJ_POWER;
     if (n >= 2048) {
       if (power) FS_LAUNCH_SLOT(true, -1); else FS_LAUNCH_SLOT(false, -1);
-      launches += 5;
+      launches += 4;
     } else {
       if (power) { FS_LAUNCH_SLOT(true, 0); FS_LAUNCH_SLOT(true, 1); } else { FS_LAUNCH_SLOT(false, 0); FS_LAUNCH_SLOT(false, 1); }
-      launches += 6;
+      launches += 5;
     }
 #undef FS_LAUNCH_SLOT
   } else {
