@@ -905,6 +905,12 @@ def _free_port():
     return p
 
 
+def _spawn_cmd(n, argv):
+    """The command line `python bench.py --gpus N` re-executes itself under: one rank per GPU of this node."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + list(argv)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -940,9 +946,7 @@ def main():
         have = torch.cuda.device_count()
         if have < args.gpus:
             raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible")
-        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
-               "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + sys.argv[1:]
-        os.execv(sys.executable, cmd)
+        os.execv(sys.executable, _spawn_cmd(args.gpus, sys.argv[1:]))
     if args.workload in ("local", "consol"):
         import torch
         ws, rank, lrank = _dist()
