@@ -133,27 +133,26 @@ __device__ __forceinline__ void local_slot_body(const FsView& v, const int key, 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int s0 = off[key * LS_QB], s1 = off[(key + 1) * LS_QB];
   // Rounds of LS_WARPS*32 slots, lane <-> slot.  In a round that is not full the slots fill whole warps first
-  // (every lane busy) and the remaining r < 32 slots go to one more warp, where each slot gets G = 32 /
-  // pow2ceil(r) lanes that split the beta range (groups of four beta, interleaved; their minima are merged by
+  // (every lane busy) and the remaining r < 32 slots go to one more warp, where each slot gets G = 32 / r
+  // lanes (at most 8) that split the beta range (groups of four beta, interleaved; their minima are merged by
   // shuffles: min is exact in any order): a warp left with 4 slots finishes 8 times sooner instead of running 4
   // lanes over the whole range (4,096 GPUs: 0.761 -> 0.717 ms).  With `fill` = false (the per-phase launches used for grids
   // of a few waves) only a round of fewer than 64 slots is split, and it is spread EVENLY over the block's warps,
   // so that every warp works and the block is short (pod, ~40 slots per key: 0.185 against 0.194 - 0.213 ms).
   for (int start = s0; start < s1; start += LS_WARPS * 32) {
     const int n_round = min(LS_WARPS * 32, s1 - start);
-    int pad = 32, per = 32, base = warp * 32;
+    int per = 32, base = warp * 32;                     // slots of this warp, and where they start in the round
     if (!fill) {
-      if (n_round < 64) {
-        per = (n_round + LS_WARPS - 1) / LS_WARPS; base = warp * per;
-        pad = 1; while (pad < per) pad <<= 1;
-      }
+      if (n_round < 64) { per = (n_round + LS_WARPS - 1) / LS_WARPS; base = warp * per; }
     } else if (n_round < LS_WARPS * 32) {
       const int nfull = n_round >> 5, rem = n_round & 31;
       per = warp < nfull ? 32 : (warp == nfull ? rem : 0);
-      pad = 1; while (pad < per) pad <<= 1;
     }
-    const int G = 32 / pad, grp = lane / pad, sl_ix = base + (lane % pad);
-    const bool have = (lane % pad) < per && sl_ix < n_round;
+    // a warp with fewer than 17 slots gives each slot G lanes (any G up to 8, not only powers of two: 10 slots
+    // -> 3 groups of 10 lanes) that split the beta range; lanes beyond G * per idle
+    const int G = per > 0 ? min(32 / per, 8) : 1;
+    const int grp = per > 0 ? lane / per : 0, idx = per > 0 ? lane - grp * per : lane, sl_ix = base + idx;
+    const bool have = per > 0 && grp < G && sl_ix < n_round;
     LocalSlot sl_ = have ? slots[start + sl_ix] : LocalSlot{0, 0u, 0.f, 0u};
     const uint32_t nb = have ? (sl_.meta >> 8) : 0u;
     uint32_t maxnb;
@@ -196,9 +195,9 @@ __device__ __forceinline__ void local_slot_body(const FsView& v, const int key, 
         }
       }
     }
-    for (int o2 = pad; o2 < 32; o2 <<= 1) {
+    for (int g = 1; g < G; ++g) {                        // group 0 collects the groups' minima
 #pragma unroll
-      for (int r = 0; r < LS_TR; ++r) best[r] = fminf(best[r], __shfl_xor_sync(0xffffffffu, best[r], o2));
+      for (int r = 0; r < LS_TR; ++r) best[r] = fminf(best[r], __shfl_sync(0xffffffffu, best[r], (idx + g * per) & 31));
     }
     if (have && grp == 0) {
       const size_t o = ((size_t)sl_.gi * (FS_RMAX * 2) + (sl_.meta & 0xFF)) * rows + r0;
