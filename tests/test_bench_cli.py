@@ -42,3 +42,34 @@ def test_tracked_ncu_summaries_are_what_the_roofline_blocks_read():
         assert not blk.get("missing"), path
         assert kernel in blk["kernel"] and blk["warp_instructions"] > 0 and blk["duration_ns"] > 0
         assert blk["command"].startswith("ncu ") and blk["captured_at_git_sha"]
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_default_arm_prints_one_json_line_with_the_contract_keys():
+    """A short run of the product arm on the GPU: one JSON line on stdout carrying the driver's contract keys."""
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3", "--variants", "0",
+                        "--aux", "0", "--sustained-s", "0.2", "--cpu-requests", "256"], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-3000:]
+    lines = [l for l in p.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1, lines[:3]
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "e2e", "gpu_launches", "clocks", "roofline", "cpu_baseline",
+              "graph", "sustained", "degeneracy", "place_stats", "kernel_ms"):
+        assert k in d, k
+    assert d["n_gpus"] == 1 and d["steps"] == 3 and d["warmup"] == 3 and d["dtype"] == "f32" and d["data"] == "synthetic"
+    assert d["value"] > 0 and d["ms_per_step"] > 0 and d["gpu_launches"] > 0 and d["vs_baseline"] is None
+    assert "configs[2]" in d["config"]["workload"] and "workload" in d["config"]
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 1024 * 128 + 65536 * 32 and e["d2h_bytes_per_step"] == 65536 * 32 + 1024 * 48
+    assert e["value"] < d["value"]                       # the copies are inside the end-to-end timed region
+    r = d["roofline"]
+    assert r["bound"] == "alu" and 0 < r["frac"] < 1 and r["peak"] > 0 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert r["traffic"] is None or r["traffic"] > 0
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["unit"] == d["unit"] and c["value"] > 0
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert len(d["degeneracy"]["hist_phi"]) == 64 and len(d["degeneracy"]["hist_sigma"]) == 16 and len(d["degeneracy"]["hist_beta"]) == 128
