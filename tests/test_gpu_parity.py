@@ -1002,13 +1002,15 @@ def test_gather_records_on_an_nccl_group(tmp_path):
     import subprocess
     import sys
     import textwrap
+    import socket
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sk = socket.socket(); sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]; sk.close()
     code = textwrap.dedent(f"""
         import os, sys, numpy as np, torch, torch.distributed as dist
         sys.path.insert(0, {root!r})
         from paper_2606_30391_b200 import shard, synth
         import paper_2606_30391_b200 as fs
-        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29631")
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="{port}")
         torch.cuda.set_device(0)
         dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
         cl = synth.make_custom(seed=77, K=13, M=4, F=8, S=8, B=8, R=101, lo=1, hi=3)
