@@ -306,6 +306,36 @@ int fs_ewr(fs_ctx* ctx, int32_t n, const int32_t* gpu_of, const float* f_mhz, co
 int fs_replace_plan(fs_ctx* ctx, int32_t n, const fs_plan_llm* llms, int32_t s_eff, float m_eff,
                     int32_t* gpu_of, int32_t* summary, int space, void* cuda_stream);
 
+/* fs_replace_plan for callers that must not allocate device memory.
+ *
+ * Everything else in this header hangs off an fs_ctx, and a context allocates: fs_create does, and so does
+ * the first call of each size.  That rules the library out for two kinds of caller.  One is a scheduler that
+ * sits next to a serving engine which claimed almost all of HBM for weights and KV cache when it started:
+ * a cudaMalloc issued later may simply fail.  The other is a control loop sharing the GPU with live
+ * inference: cudaMalloc and cudaFree serialise on the driver's allocator, and cudaFree waits for the whole
+ * device, so either one stalls the streams the scheduler is supposed to leave alone.  This call is for them.
+ * It takes no context and calls no cudaMalloc / cudaFree / cudaHostAlloc nor any routine that allocates; the
+ * kernel's working arrays sit in one array compiled into the library (about 300 KiB), which every GPU that
+ * loads the library keeps until the process exits.  That fixed size is the limit:
+ *   n <= FS_PLAN_STATIC_MAX_N, otherwise FS_ERR_SHAPE ("dims outside the supported range") and nothing runs.
+ *
+ * Same kernel, same results as fs_replace_plan(..., FS_DEVICE, ...):
+ *   llms [n], gpu_of [n], summary [4] : caller-owned memory the CURRENT CUDA device can address (device
+ *   memory, or mapped page-locked host memory); the work is enqueued on `cuda_stream`, which must belong
+ *   to the current device, and the call returns without waiting.  s_eff in 1..FS_MAX_S (else FS_ERR_ARG).
+ *   An LLM with need_units < 1 stays unplaced (gpu_of = -1) as in fs_replace_plan, but with no context there
+ *   is nowhere to keep the sticky FS_ERR_RANGE: check that field yourself if it can be bad.
+ * First call on each device: the library looks up the array's device address (one cudaGetSymbolAddress,
+ * which also makes the runtime load the library's code on that device).  Make that first call early, at
+ * start-up, and before any stream capture begins on that device.
+ * The array is shared by every call in the process.  Nothing in it needs clearing between calls (the kernel
+ * writes each word before reading it), but two calls that overlap on one GPU - different streams, or
+ * different host threads - race on it: keep them on one stream, or order the streams yourself.
+ * Errors: FS_ERR_ARG, FS_ERR_SHAPE, FS_ERR_CUDA (no usable device, or the launch failed).                */
+#define FS_PLAN_STATIC_MAX_N 1024
+int fs_replace_plan_static(int32_t n, const fs_plan_llm* llms, int32_t s_eff, float m_eff,
+                           int32_t* gpu_of, int32_t* summary, void* cuda_stream);
+
 /* Transmission plan: minimum-cost assignment of n sources to n destinations under
  * e_uv = Bytes(u -> v) / BW(u, v), costs in whole microseconds rint(fl(fl(bytes_mb[u] / bw[u][v]) * 1000))
  * (bytes in MB, bw in MB per ms, row-major [n][n], > 0), Kuhn-Munkres, exact in int64.

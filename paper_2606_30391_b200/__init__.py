@@ -23,7 +23,7 @@ FS_OBJ_ENERGY, FS_OBJ_POWER, FS_SPLIT_EXHAUSTIVE, FS_SPLIT_MINSM = 0, 1, 0, 2
 
 # every symbol include/festina_eval.h declares
 SYMBOLS = ("fs_create", "fs_destroy", "fs_load_profiles", "fs_set_gpu_state", "fs_place_batch",
-           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_dispatch_commit", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_migration_plan", "fs_migration_select", "fs_strerror", "fs_last_cuda_error",
+           "fs_local_config", "fs_consolidate", "fs_dispatch", "fs_dispatch_commit", "fs_batch_tasks", "fs_llm_profiles", "fs_ewr", "fs_replace_plan", "fs_replace_plan_static", "fs_migration_plan", "fs_migration_select", "fs_strerror", "fs_last_cuda_error",
            "fs_launch_count", "fs_set_work_stats", "fs_last_place_stats", "fs_set_timing", "fs_get_timing")
 TIMERS = ("place_score", "place_decode", "summary", "local_slot", "local_split", "consol_agg",
           "consol_pair", "place_warm", "batch_tasks", "dispatch")
@@ -68,6 +68,7 @@ def lib() -> C.CDLL:
     L.fs_migration_plan.argtypes = [vp, i32, vp, vp, vp, vp, C.c_int, vp]
     L.fs_migration_select.argtypes = [vp, i32, vp, vp, vp, C.c_int, vp]
     L.fs_replace_plan.argtypes = [vp, i32, vp, i32, C.c_float, vp, vp, C.c_int, vp]
+    L.fs_replace_plan_static.argtypes = [i32, vp, i32, C.c_float, vp, vp, vp]
     L.fs_llm_profiles.argtypes = [vp, i32, vp, vp, C.c_int, vp]
     L.fs_ewr.argtypes = [vp, i32, vp, vp, vp, i32, vp, vp, C.c_int, vp]
     L.fs_dispatch.argtypes = [vp, i32, vp, vp, C.c_int, vp]
@@ -123,6 +124,32 @@ def _stream_ptr(stream) -> C.c_void_p:
     if hasattr(stream, "cuda_stream"):
         return C.c_void_p(stream.cuda_stream)
     return C.c_void_p(int(stream))
+
+
+FS_PLAN_STATIC_MAX_N = 1024   # festina_eval.h
+
+
+def replace_plan_static(llms, s_eff: int, m_eff: float, gpu_of, summary, stream=None) -> None:
+    """fs_replace_plan_static: Algorithm 1 phases 2-3 without a context and without any allocation.
+
+    For a process that cannot (HBM already handed to a serving engine) or must not (cudaMalloc / cudaFree
+    stall the inference streams it shares the GPU with) allocate device memory when it needs a plan.
+    `llms` (n fs_plan_llm records, 16 bytes each), `gpu_of` (n int32) and `summary` (4 int32) are torch CUDA
+    tensors of the caller, on the current device; nothing is copied, the kernel is enqueued on `stream` and
+    the results are valid once that stream has been synchronised.  At most FS_PLAN_STATIC_MAX_N LLMs: the
+    working arrays are a fixed array inside the library, shared by all calls (do not overlap two calls on
+    one GPU).  Raises FestinaError (FS_ERR_SHAPE) beyond that limit."""
+    for t in (llms, gpu_of, summary):
+        assert _is_torch_cuda(t) and t.is_contiguous(), "device tensors only: this path copies nothing"
+    n = llms.numel() * llms.element_size() // 16
+    assert gpu_of.numel() * gpu_of.element_size() >= 4 * n and summary.numel() * summary.element_size() >= 16
+    rc = lib().fs_replace_plan_static(n, C.c_void_p(llms.data_ptr()), int(s_eff), float(m_eff),
+                                      C.c_void_p(gpu_of.data_ptr()), C.c_void_p(summary.data_ptr()), _stream_ptr(stream))
+    if rc != FS_OK:
+        where = "fs_replace_plan_static"
+        if rc == FS_ERR_SHAPE:
+            where += f" (n = {n} LLMs, the built-in scratch array holds at most {FS_PLAN_STATIC_MAX_N})"
+        raise FestinaError(rc, where)
 
 
 class Festina:

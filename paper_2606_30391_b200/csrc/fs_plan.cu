@@ -10,6 +10,8 @@
 // 64-bit (value, index) keys reduced by shuffles, the three orders are rank sorts (lane <-> item).
 // One warp does the whole plan; the per-GPU resident lists hold at most S_eff <= 32 entries, so the
 // waste sums of the swap test are short and are taken by lane 0 in the order the definition fixes.
+#include <mutex>
+
 #include "fs_kernels.h"
 
 namespace {
@@ -210,4 +212,72 @@ int fsk_replace_plan(int n, const fs_plan_llm* llms, int s_eff, float m_eff, voi
   sc.res = (int32_t*)take(sizeof(int32_t) * g * PL_RES);
   replace_plan_kernel<<<1, 32, 0, st>>>(n, llms, s_eff, m_eff, sc, gpu_of, summary, flag);
   return 1;
+}
+
+// ---- fs_replace_plan_static: the same plan without any allocation -------------------------------------
+//
+// Who this is for.  fs_replace_plan lives on an fs_ctx, and both fs_create and the first call of a given
+// size go through cudaMalloc.  Some hosts of this library cannot do that at the moment they want a plan:
+// the scheduler runs inside (or beside) a serving engine that reserved nearly all of HBM for weights and
+// KV cache at start-up, so a late cudaMalloc fails or has to be fought for; and a control loop that shares
+// the GPU with running inference must not call cudaMalloc / cudaFree at all, because both take the
+// driver's allocator lock and cudaFree waits for the whole device, stalling the very streams the scheduler
+// is trying not to disturb.  Those callers get this one entry point: it needs no context and never calls
+// cudaMalloc, cudaFree, cudaHostAlloc or any routine that allocates.  The caller brings the input and the
+// two outputs (device-addressable); the kernel's working arrays (processing order, the BFD bins, the per-GPU
+// room / frequency / resident lists) live in the fixed array below.
+//
+// What it costs.  Every GPU on which this library's code gets loaded holds sizeof(g_plan_static) bytes
+// (about 300 KiB, see the static_assert) from module load until the process exits, whether or not the entry
+// point is ever called.  The size is fixed at build time, hence the limit n <= FS_PLAN_STATIC_MAX_N.
+//
+// `g_plan_static` is a DEVICE symbol.  In host code the name is only a handle for the runtime: taking its
+// address there yields a host address, and a kernel handed that would fault (or, on a system where the GPU can
+// reach host memory, quietly work on the wrong bytes).  The device address comes from cudaGetSymbolAddress,
+// asked once per device with that device current (plan_static_base below).
+constexpr size_t pl_align16(size_t b) { return (b + 15) / 16 * 16; }
+constexpr size_t pl_static_bytes(size_t n) {   // the carve-up of fsk_replace_plan, for n items
+  return 3 * pl_align16(4 * n) + 4 * pl_align16(4 * (2 * n + 1)) + pl_align16(4 * (2 * n + 1) * (size_t)FS_MAX_S);
+}
+constexpr size_t PL_STATIC_HEAD = 256;         // first 256 bytes: the kernel's range-flag words (a sink here)
+constexpr size_t PL_STATIC_BYTES = PL_STATIC_HEAD + pl_static_bytes(FS_PLAN_STATIC_MAX_N);
+static_assert(PL_STATIC_BYTES <= 320 * 1024, "keep the resident scratch modest");
+static __device__ __align__(256) unsigned char g_plan_static[PL_STATIC_BYTES];
+
+namespace {
+constexpr int PL_STATIC_MAX_DEV = 64;
+std::mutex g_plan_static_mu;
+unsigned char* g_plan_static_base[PL_STATIC_MAX_DEV];   // device address of g_plan_static, per device ordinal
+
+// Device address of the scratch array on the CURRENT device (first use on a device: one
+// cudaGetSymbolAddress, which also makes the runtime load this library's code onto that device).
+int plan_static_base(unsigned char** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return FS_ERR_CUDA; }
+  if (dev < 0 || dev >= PL_STATIC_MAX_DEV) return FS_ERR_SHAPE;
+  std::lock_guard<std::mutex> lock(g_plan_static_mu);
+  if (!g_plan_static_base[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_plan_static) != cudaSuccess || !p) { cudaGetLastError(); return FS_ERR_CUDA; }
+    g_plan_static_base[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_plan_static_base[dev];
+  return FS_OK;
+}
+}  // namespace
+
+extern "C" int fs_replace_plan_static(int32_t n, const fs_plan_llm* llms, int32_t s_eff, float m_eff,
+                                      int32_t* gpu_of, int32_t* summary, void* cuda_stream) {
+  if (n < 0 || !summary || (n > 0 && (!llms || !gpu_of)) || s_eff < 1 || s_eff > FS_MAX_S) return FS_ERR_ARG;
+  if (n > FS_PLAN_STATIC_MAX_N) return FS_ERR_SHAPE;     // the resident array is sized for FS_PLAN_STATIC_MAX_N
+  unsigned char* base = nullptr;
+  const int rc = plan_static_base(&base);
+  if (rc != FS_OK) return rc;
+  // Nothing in the array has to start at zero: the kernel writes every word before it reads it (order[] by
+  // the rank sort, a bin's room when the bin is opened, the per-GPU records up to 2n+1 at the top of phase
+  // 3, a resident list only below its count), so whatever the previous call left behind is never seen.
+  fsk_replace_plan(n, llms, s_eff, m_eff, base + PL_STATIC_HEAD, gpu_of, summary, reinterpret_cast<int*>(base),
+                   static_cast<cudaStream_t>(cuda_stream));
+  if (cudaGetLastError() != cudaSuccess) return FS_ERR_CUDA;
+  return FS_OK;
 }
