@@ -119,8 +119,11 @@ __device__ __forceinline__ unsigned long long fs_warp_min_key(unsigned long long
   return ((unsigned long long)mh << 32) | ml;
 }
 
-// ceil(q / n) for q < 2^24, 1 <= n <= 256 by multiply-high: magic = ceil(2^32 / n) for n >= 2 (0 stands for
+// ceil(q / n) for q <= 2^24, 1 <= n <= 256 by multiply-high: magic = ceil(2^32 / n) for n >= 2 (0 stands for
 // n == 1).  floor((q-1)/n) = umulhi(q-1, magic) exactly, because (q-1) * (magic*n - 2^32) < 2^24 * 2^8 = 2^32.
+// Beyond that it can be one too large (n = 255: first at q = 16,909,560), so a caller whose q may exceed 2^24
+// (the padded output length O of a request) tests the range and divides otherwise; tests/test_magic_division.py
+// checks the bound and the first failures.
 __host__ __device__ __forceinline__ uint32_t fs_magic(uint32_t n) {
   return n <= 1u ? 0u : (uint32_t)((0x100000000ull + n - 1u) / n);
 }

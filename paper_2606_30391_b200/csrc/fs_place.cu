@@ -521,7 +521,9 @@ place_dense_kernel(FsView v, int R, const fs_request* __restrict__ reqs,
             it = witems[ix];
             if (it.sm_free >= 1 && it.br1 >= 0 && c.mem <= it.mem_free_mb) {
               have = true; sidx = it.sm_free - 1;
-              wr1 = fs_ceil_div_magic(c.O, it.magic);
+              // O = padded output length reaches (21*(2^24-1)+19)/20 > 2^24, past the range in which the
+              // multiply-high quotient is exact (fs_common.cuh): such a request (warp-uniform) divides for real
+              wr1 = c.O <= (1u << 24) ? fs_ceil_div_magic(c.O, it.magic) : fs_ceil_div(c.O, (uint32_t)it.br1 + 1u);
               e1lb = fs_energy_lb(__uint2float_rn(wr1), it.lp1f, it.eta1);
             }
           }

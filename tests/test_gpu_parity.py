@@ -146,6 +146,38 @@ def test_local_queue_depths_up_to_2_pow_24(ctx, B):
     _check_all(ctx, cl, consol=False)
 
 
+def test_padded_output_lengths_past_2_pow_24(ctx):
+    """o_pred up to 2^24-1 pads to O = (21*o_pred+19)/20 > 2^24, beyond the range in which the placement kernel's
+    multiply-high round count is exact (tests/test_magic_division.py): decode buckets 252 / 255 of a B = 256
+    table joined by requests whose O sits on and around the first values at which the shortcut is one round off
+    (16,909,560 for 255; 17,318,448 for 252), plus prompts L near 2^24 for the prefill shortcut."""
+    cl = synth.make_custom(seed=77, K=24, M=2, F=6, S=4, B=256, R=160, lo=1, hi=2)
+    st = synth.Stream(77, "bigO")
+    cl.states["t"]["beta"][:, :, 1] = np.array([250, 253, 251, 254, 255, 0], dtype=np.uint8)[st.randint(cl.K * 4, 0, 5)].reshape(cl.K, 4)
+    cl.states["t"]["q"][:, :, 1] = 1 + st.randint(cl.K * 4, 0, 1000).reshape(cl.K, 4).astype(np.uint32)
+    cl.states["t"]["sigma"][...] = 0                     # free shares everywhere
+    cl.states["t"]["slo_ms"][...] = 1e30
+    cl.states["mem_free_mb"] = 1e30
+    cl.models["kv_mb_per_token"] = 1e-9
+    cl.requests["slo_ttft_ms"] = 1e30
+    cl.requests["slo_tbt_ms"] = 1e30
+    crit = []
+    for O in (16909560, 17318448, 1 << 24, (1 << 24) + 1, 17616076):
+        crit += [(20 * (O + d)) // 21 + e for d in (-1, 0, 1, 255) for e in (0, 1)]     # o_pred with pad near O
+    o = np.array(crit + list(2 ** 24 - 1 - st.randint(cl.R, 0, 900000)), dtype=np.int64)[:cl.R]
+    cl.requests["o_pred"] = np.clip(o, 0, 2 ** 24 - 1).astype(np.uint32)
+    cl.requests["L"][::3] = (2 ** 24 - 1 - st.randint(len(cl.requests["L"][::3]), 0, 70000)).astype(np.uint32)
+    pad = (21 * cl.requests["o_pred"].astype(np.int64) + 19) // 20
+    assert (pad == 16909560).any() and (pad == 17318448).any() and (pad > 2 ** 24).sum() > 100
+    ctx.load_cluster(cl)
+    got = ctx.place_batch(cl.requests)
+    ref = _oracle_place(cl)
+    cmp.assert_placement_equal(got, ref)
+    warm = cl.states["t"]["model"][got["gpu"], 0] == cl.requests["model"]
+    assert (got["gpu"] >= 0).all() and (got["beta"] >= 251).sum() > 20 and warm.sum() > 20     # joined the deep buckets
+    cmp.assert_placement_equal(ctx.dispatch(cl.requests), _oracle_dispatch(cl))
+
+
 def test_empty_inputs(ctx):
     cl = synth.make_custom(seed=5, K=4, M=2, F=4, S=4, B=4, R=8)
     ctx.load_cluster(cl)
