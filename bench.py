@@ -39,6 +39,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_2606_30391_b200 import synth  # noqa: E402
+import bench_work  # noqa: E402
 
 METRIC = "placement_candidate_evals_per_sec"
 UNIT = "eligible candidates/s"
@@ -83,15 +84,122 @@ def _git_sha():
         return None
 
 
+def _csrc_hash():
+    """sha1 over the kernel sources and the header (names and bytes): what an ncu capture is a capture OF.  Works
+    on the GPU box, where the snapshot has no .git."""
+    import glob
+    import hashlib
+    h = hashlib.sha1()
+    files = sorted(glob.glob(os.path.join(ROOT, "paper_2606_30391_b200", "csrc", "*"))) + [os.path.join(ROOT, "include", "festina_eval.h")]
+    for f in files:
+        h.update(os.path.basename(f).encode()); h.update(open(f, "rb").read())
+    return h.hexdigest()[:12]
+
+
 def _ncu_block(path):
-    """The tracked summary of an ncu capture (written by --ncu-import), with the commit it was taken at, so that
-    a stale capture shows: the figures are evidence from a profiler run, never measured inside the bench."""
+    """The tracked summary of an ncu capture (written by --ncu-import) with the hash of the sources it was taken
+    on beside the hash of the sources now, so that a stale capture shows (`stale`: true / false, None when the
+    summary predates the hash): the figures are evidence from a profiler run, never measured inside the bench."""
     if not os.path.exists(path):
         return {"source": os.path.relpath(path, ROOT), "missing": True}
     d = json.load(open(path))
     d["source"] = os.path.relpath(path, ROOT)
     d["bench_git_sha"] = _git_sha()
+    d["bench_csrc_hash"] = _csrc_hash()
+    d["stale"] = (d["csrc_hash"] != d["bench_csrc_hash"]) if d.get("csrc_hash") else None
+    if d.get("dram_bytes") and d.get("duration_ns"):
+        d["hbm_gbs"] = d["dram_bytes"] / d["duration_ns"]
+        d["hbm_frac"] = d["hbm_gbs"] / float(_peaks()[0].get("hbm_gbs", 6650.0))
     return d
+
+
+LINE_BUDGET = 3000   # bytes: the driver keeps a 3 KB tail of stdout, the contract line has to fit in it
+
+
+def _r(x, n=5):
+    """Floats to n significant digits (the line has a byte budget); everything else unchanged."""
+    if isinstance(x, float) and math.isfinite(x):
+        return float(f"{x:.{n}g}")
+    return x
+
+
+def _roofline_scalars(rf, requests=None):
+    ncu = rf.get("ncu") or {}
+    out = {"bound": rf.get("bound"), "kernel": str(rf.get("kernel", "")).split(" ")[0], "achieved": _r(rf.get("achieved")),
+           "peak": _r(rf.get("peak")), "unit": rf.get("unit"), "frac": _r(rf.get("frac")), "traffic": rf.get("traffic"),
+           "kernel_ms": _r(rf.get("kernel_ms"))}
+    if "survey_formula" in rf:
+        out["survey_formula_frac"] = _r(rf["survey_formula"].get("frac"))
+    if "sweep_pipe" in rf:
+        out["sweep_pipe_frac"] = _r(rf["sweep_pipe"].get("frac"))
+    if ncu and not ncu.get("missing"):
+        out.update({"hbm_frac": _r(ncu.get("hbm_frac")), "hbm_gbs": _r(ncu.get("hbm_gbs")),
+                    "issue_active_pct": _r(ncu.get("issue_active_pct")), "ncu": ncu.get("source"),
+                    "ncu_csrc_hash": ncu.get("csrc_hash"), "ncu_stale": ncu.get("stale")})
+        if requests and ncu.get("warp_instructions"):
+            out["warp_instr_per_request"] = _r(ncu["warp_instructions"] / requests)
+    return out
+
+
+def compact_line(full: dict, detail_path=None) -> dict:
+    """The contract line the driver parses (at most LINE_BUDGET bytes as JSON): the contract keys, `roofline`,
+    `cpu_baseline`, `e2e`, `clocks` and one scalar triple per extra leg.  Histograms, work counters, notes and
+    the whole ncu summaries stay in the detail file (`detail`)."""
+    cfg = dict(full.get("config", {}))
+    cfg["workload"] = str(cfg.get("workload", ""))[:200]
+    for k in ("l2", "parallelism"):
+        if k in cfg:
+            cfg[k] = str(cfg[k])[:60]
+    line = {k: _r(full.get(k)) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step",
+                                         "higher_is_better", "scaling", "vs_baseline", "dtype", "data", "gpu_launches")}
+    line["config"] = cfg
+    ck = full.get("clocks") or {}
+    line["clocks"] = {k: ck.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")}
+    e = full.get("e2e") or {}
+    line["e2e"] = {k: _r(e.get(k)) for k in ("value", "unit", "ms_per_step", "h2d_bytes_per_step", "d2h_bytes_per_step")}
+    if "cpu_baseline" in full:
+        c = full["cpu_baseline"]
+        line["cpu_baseline"] = {"value": _r(c.get("value")), "unit": c.get("unit"), "cores": c.get("cores"),
+                                "kind": c.get("kind"), "sample": str(c.get("sample", ""))[:120]}
+    line["kernel_ms"] = {k: _r(v, 4) for k, v in (full.get("kernel_ms") or {}).items()}
+    if "roofline" in full:
+        line["roofline"] = _roofline_scalars(full["roofline"], (full.get("place_stats") or {}).get("requests"))
+    g = full.get("graph")
+    line["graph"] = bool(g.get("device_step")) if isinstance(g, dict) else bool(g)
+    if "sustained" in full:
+        line["sustained_ms"] = _r(full["sustained"].get("ms_per_step"))
+    if "gathered_records_ok" in full:
+        line["gathered_records_ok"] = full["gathered_records_ok"]
+
+    def triple(leg, ms_key):
+        if not isinstance(leg, dict):
+            return {"ok": False}
+        if leg.get("ok") is False:
+            return {"ok": False, "error": str(leg.get("error", ""))[:80]}
+        t = {"ms": _r(leg.get(ms_key, leg.get("ms_per_step")), 4), "ok": True}
+        if "roofline" in leg:
+            t["frac"] = _r(leg["roofline"].get("frac"), 4)
+        return t
+    if "variants" in full:
+        line["variants"] = {k: triple(v, "place_score_ms") for k, v in full["variants"].items()}
+    if "aux" in full:
+        line["aux"] = {k: triple(v, "ms_per_step") for k, v in full["aux"].items()}
+    if detail_path:
+        line["detail"] = os.path.relpath(detail_path, ROOT) if os.path.isabs(detail_path) else detail_path
+    return line
+
+
+def emit(full: dict, detail_path=None):
+    """Write the full result to the detail file and print the contract line (one line, flushed)."""
+    if detail_path:
+        try:
+            json.dump(full, open(detail_path, "w"), indent=1)
+        except OSError as e:
+            print(f"bench.py: could not write {detail_path}: {e}", file=sys.stderr)
+            detail_path = None
+    text = json.dumps(compact_line(full, detail_path))
+    assert len(text.encode()) <= LINE_BUDGET, f"contract line is {len(text.encode())} bytes (budget {LINE_BUDGET})"
+    print(text, flush=True)
 
 
 class ClockSampler:
@@ -191,7 +299,7 @@ def oracle_sample(cl, n_req: int, nthreads: int):
     oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, reqs, nthreads)
     oracle.local_config(cl.lat, cl.pow, cl.states, 0, np.arange(n_gpu, dtype=np.int32), nthreads)
     dt = time.perf_counter() - t0
-    return dt, synth.eligible_work(cl, reqs)[1], n_gpu
+    return dt, bench_work.eligible_work(cl, reqs)[1], n_gpu
 
 
 def run_reference(args):
@@ -255,32 +363,30 @@ def _place_roofline(cl, ps, score_ms, cand_def, ncu_path=None):
     alu_peak, mhz, peak_src = _alu_peak()
     useful = _useful_ops(cl, ps)
     executed = ps["cold_candidates_swept"] + ps["candidates_scored"]
-    # 13 lane-ops per placement candidate x the candidates this launch evaluated (swept + scored by
-    # the definition) is the algorithmic work; the unit model of DESIGN.md section 7 (every unit the kernel counted,
-    # bounds and record tests included) is reported beside it
+    # frac: the lane-ops of every unit the kernel counted itself, each weighted with what that unit costs (DESIGN.md
+    # section 7: a swept candidate is a compare and a predicated min, a candidate scored by the definition 15, ...)
+    # over the launch's CUDA-event time, against the issue peak.  SURVEY 8(d)'s flat 13 lane-ops x candidates
+    # evaluated charges a swept candidate like a full evaluation (it exceeds 1 on sweep-dominated inputs): it is
+    # kept beside it as survey_formula.
     survey = OPS_PER_CANDIDATE * executed
-    achieved = survey / (score_ms * 1e-3)
+    achieved = useful / (score_ms * 1e-3)
     nominal = OPS_PER_CANDIDATE * cand_def / (score_ms * 1e-3)
     blk = {"bound": "alu", "kernel": "place_dense_kernel (fs_place_batch scoring + argmin + records)",
            "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
-           "traffic": None, "algorithmic_lane_ops_per_launch": survey, "kernel_ms": score_ms,
+           "traffic": None, "algorithmic_lane_ops_per_launch": useful, "kernel_ms": score_ms,
            "executed_candidates_per_launch": executed,
            "executed_frac_of_eligible": executed / cand_def if cand_def else None,
-           "unit_model": {"useful_lane_ops_per_launch": useful, "achieved": useful / (score_ms * 1e-3) / 1e12,
-                          "frac": useful / (score_ms * 1e-3) / alu_peak,
-                          "note": "lane-ops of every unit the kernel counted itself, weighted with DESIGN.md section 7's "
-                                  "per-unit figures (requests, built tiles, records tested, swept pairs and candidates, "
-                                  "warm pairs tested, candidates scored by the definition)"},
+           "survey_formula": {"lane_ops_per_unit": OPS_PER_CANDIDATE, "lane_ops_per_launch": survey,
+                              "achieved": survey / (score_ms * 1e-3) / 1e12, "frac": survey / (score_ms * 1e-3) / alu_peak,
+                              "note": "13 lane-ops (SURVEY 8(d)) x candidates evaluated by this launch (swept + scored by the "
+                                      "definition): over-counts swept candidates, above 1 on sweep-dominated inputs"},
            "dense_definition": {"achieved": nominal / 1e12, "frac": nominal / alu_peak,
                                 "note": f"{OPS_PER_CANDIDATE:g} lane-ops x {cand_def} eligible candidates / kernel time; "
                                         "above 1 when exact pruning skips most of them: it measures the algorithm, not the kernel"},
-           "note": f"achieved = {OPS_PER_CANDIDATE:g} lane-ops (SURVEY 8(d)) x candidates evaluated by this launch / CUDA-event "
-                   "time of the launch; peak = 148 SMs x 128 lanes/clk x "
+           "note": "achieved = lane-ops of the units the kernel counted (requests, built tiles, records tested, swept pairs "
+                   "and candidates, warm pairs tested, candidates scored by the definition; DESIGN.md section 7 per-unit "
+                   "figures) / CUDA-event time of the launch; peak = 148 SMs x 128 lanes/clk x "
                    f"{mhz:.0f} MHz ({peak_src} sm_max_mhz)"}
-    if achieved > alu_peak:
-        blk["frac_note"] = ("above 1: on this input almost every evaluated candidate is a SWEPT one, which costs a compare and "
-                            "a min on the request's tile, not the 13 lane-ops of a full evaluation: unit_model.frac is the "
-                            "honest figure here")
     if ps["cold_candidates_swept"] > 4 * ps["candidates_scored"]:
         # sweep-dominated launch (the bounds cannot prune): the swept candidates against the rate at which an SM
         # issues the sweep's compare + predicated-min pair (profiles/r01_pipe_rates.md: 31.6 pairs per clock per SM)
@@ -293,9 +399,10 @@ def _place_roofline(cl, ps, score_ms, cand_def, ncu_path=None):
         blk["ncu"] = ncu
         if not ncu.get("missing"):
             blk["traffic"] = ncu.get("dram_bytes")
+            blk["hbm_frac"] = ncu.get("hbm_frac")
             wi = ncu.get("warp_instructions")
             if wi:
-                blk["useful_per_issued"] = survey / 32.0 / wi
+                blk["useful_per_issued"] = useful / 32.0 / wi
     return blk
 
 
@@ -441,7 +548,7 @@ def run_ours(args):
     ctx.place_batch(d_reqs, out=d_place, stream=stream)
     pstats = ctx.last_place_stats()
     ctx.set_work_stats(False)
-    pairs, cand_def = synth.eligible_work(cl)
+    pairs, cand_def = bench_work.eligible_work(cl)
 
     # ---- sustained: seconds of back-to-back replays, no flush, clocks sampled over that window ----------
     sustained = None
@@ -566,74 +673,82 @@ def run_ours(args):
     if gathered_ok is not None:
         line["gathered_records_ok"] = bool(gathered_ok)
         assert gathered_ok, "records gathered over NCCL differ from the recomputation on rank 0"
-    if ws == 1:
+    detail = args.detail_out
+    if ws == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        dt, c, n_gpu = oracle_sample(cl, args.cpu_requests, cores)
+        line["cpu_baseline"] = {"value": c / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{args.cpu_requests} of {cl.R} requests x all {cl.K} GPUs + "
+                                          f"{n_gpu} GPUs local config, {dt:.1f} s"}
+    if ws == 1 and (args.variants or args.aux):
+        # the headline first: whatever happens in an extra leg below, this line is already on stdout.  The
+        # enriched line (same pod numbers + one triple per extra leg) is printed last.
+        emit(line, detail)
+
+        def guarded(fn, *a):
+            try:
+                return fn(*a)
+            except Exception as e:                          # noqa: BLE001 - reported in the line and on stderr
+                print(f"bench.py: leg {fn.__name__}{a[-2:-1]} failed: {e!r}", file=sys.stderr)
+                return {"ok": False, "error": repr(e)}
         ctx.set_timing(True)
         if args.variants:
-            line["variants"] = run_variants(args, torch, dev, ctx, flush)
+            line["variants"] = {n: guarded(run_variant, args, torch, dev, ctx, n, flush) for n in bench_work.VARIANTS}
         if args.aux:
-            line["aux"] = {w: run_aux_leg(args, torch, dev, w, flush) for w in ("local", "consol")}
-            line["aux"].update({w: run_small_leg(args, torch, dev, w, flush) for w in ("tiny", "rack")})
-        if not args.no_cpu_baseline:
-            cores = os.cpu_count() or 1
-            dt, c, n_gpu = oracle_sample(cl, args.cpu_requests, cores)
-            line["cpu_baseline"] = {"value": c / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": f"{args.cpu_requests} of {cl.R} requests x all {cl.K} GPUs + "
-                                              f"{n_gpu} GPUs local config, {dt:.1f} s"}
-    print(json.dumps(line), flush=True)
+            line["aux"] = {w: guarded(run_aux_leg, args, torch, dev, w, flush) for w in ("local", "consol")}
+            line["aux"].update({w: guarded(run_small_leg, args, torch, dev, w, flush) for w in ("tiny", "rack")})
+    emit(line, detail)
     ctx.close()
     if dist is not None:
         dist.destroy_process_group()
 
 
-def run_variants(args, torch, dev, ctx, flush):
-    """configs[2] reshaped so that the bounds prune less (or nothing): the scoring kernel timed on each, with its
-    work counters, its roofline fraction and the shape of the decisions; every variant is checked against the
-    oracle on a sample of its requests in this run."""
+def run_variant(args, torch, dev, ctx, name, flush):
+    """configs[2] reshaped so that the bounds prune less (or nothing): the scoring kernel timed on the variant, with
+    its work counters, its roofline fraction and the shape of the decisions; checked against the oracle on a sample
+    of its requests in this run."""
     import oracle
-    out = {}
     stream = torch.cuda.current_stream()
     cores = os.cpu_count() or 1
-    for name in synth.VARIANTS:
-        cl = synth.make_variant(args.workload, name)
-        tb = lambda a: _tb(torch, dev, a)
-        ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
-                          tb(cl.models), cl.params)
-        d_states, d_reqs = tb(cl.states), tb(cl.requests)
-        d_place = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
-        n_steps = max(3, args.steps // 2) if name != "identical_gpus" else 3
-        ts, step_ms = [], []
-        for i in range(3 + n_steps):
-            flush.zero_()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            ctx.set_gpu_state(d_states, stream=stream)
-            ctx.place_batch(d_reqs, out=d_place, stream=stream)
-            b.record(stream); b.synchronize()
-            if i >= 3:
-                ts.append(ctx.get_timing()["place_score"]); step_ms.append(a.elapsed_time(b))
-        ctx.set_work_stats(True)
+    cl = bench_work.make_variant(args.workload, name)
+    tb = lambda a: _tb(torch, dev, a)
+    ctx.load_profiles(torch.from_numpy(cl.lat).to(dev), torch.from_numpy(cl.pow).to(dev), tb(cl.freq_mhz),
+                      tb(cl.models), cl.params)
+    d_states, d_reqs = tb(cl.states), tb(cl.requests)
+    d_place = torch.empty(cl.R * 32, dtype=torch.uint8, device=dev)
+    n_steps = max(3, args.steps // 2) if name != "identical_gpus" else 3
+    ts, step_ms = [], []
+    for i in range(3 + n_steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        ctx.set_gpu_state(d_states, stream=stream)
         ctx.place_batch(d_reqs, out=d_place, stream=stream)
-        ps = ctx.last_place_stats()
-        ctx.set_work_stats(False)
-        place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
-        idx = np.arange(0, cl.R, max(1, cl.R // args.variant_sample))
-        ref = oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests[idx], cores)
-        same = all(np.array_equal(place[idx][f], ref[f]) for f in ("gpu", "sigma", "phi", "beta", "f_req", "flat")) and \
-            np.array_equal(place[idx]["energy_mj"].view(np.uint32), ref["energy_mj"].view(np.uint32))
-        assert same, f"variant {name}: CUDA and oracle disagree on the sample"
-        pairs, cand_def = synth.eligible_work(cl)
-        score_ms = float(np.mean(ts))
-        shape = _place_shape(cl, place)
-        for k in ("hist_sigma", "hist_beta"):
-            shape.pop(k)
-        out[name] = {"place_score_ms": score_ms, "ms_per_step": float(np.mean(step_ms)), "steps": n_steps,
-                     "step": "fs_set_gpu_state + fs_place_batch, L2 flushed between steps",
-                     "value": cand_def / (float(np.mean(step_ms)) * 1e-3), "unit": UNIT,
-                     "eligible_candidates_per_step": cand_def, "place_stats": ps,
-                     "roofline": _place_roofline(cl, ps, score_ms, cand_def),
-                     "degeneracy": shape,
-                     "oracle_check": f"{len(idx)} requests (every {max(1, cl.R // args.variant_sample)}th) identical to the oracle"}
-    return out
+        b.record(stream); b.synchronize()
+        if i >= 3:
+            ts.append(ctx.get_timing()["place_score"]); step_ms.append(a.elapsed_time(b))
+    ctx.set_work_stats(True)
+    ctx.place_batch(d_reqs, out=d_place, stream=stream)
+    ps = ctx.last_place_stats()
+    ctx.set_work_stats(False)
+    place = d_place.cpu().numpy().view(synth.PLACEMENT_DT)
+    idx = np.arange(0, cl.R, max(1, cl.R // args.variant_sample))
+    ref = oracle.place_batch(cl.lat, cl.pow, cl.models, cl.states, cl.requests[idx], cores)
+    same = all(np.array_equal(place[idx][f], ref[f]) for f in ("gpu", "sigma", "phi", "beta", "f_req", "flat")) and \
+        np.array_equal(place[idx]["energy_mj"].view(np.uint32), ref["energy_mj"].view(np.uint32))
+    assert same, f"variant {name}: CUDA and oracle disagree on the sample"
+    pairs, cand_def = bench_work.eligible_work(cl)
+    score_ms = float(np.mean(ts))
+    shape = _place_shape(cl, place)
+    for k in ("hist_sigma", "hist_beta"):
+        shape.pop(k)
+    return {"place_score_ms": score_ms, "ms_per_step": float(np.mean(step_ms)), "steps": n_steps,
+            "step": "fs_set_gpu_state + fs_place_batch, L2 flushed between steps",
+            "value": cand_def / (float(np.mean(step_ms)) * 1e-3), "unit": UNIT,
+            "eligible_candidates_per_step": cand_def, "place_stats": ps,
+            "roofline": _place_roofline(cl, ps, score_ms, cand_def),
+            "degeneracy": shape,
+            "oracle_check": f"{len(idx)} requests (every {max(1, cl.R // args.variant_sample)}th) identical to the oracle"}
 
 
 def _slot_evals(cl) -> int:
@@ -823,7 +938,7 @@ def run_small_leg(args, torch, dev, workload, flush):
     dt = time.perf_counter() - t0
     assert np.array_equal(ref["flat"], place["flat"]) and np.array_equal(ref["energy_mj"].view(np.uint32), place["energy_mj"].view(np.uint32))
     assert np.array_equal(lref["flat"], local["flat"]) and np.array_equal(lref["beta"], local["beta"])
-    pairs, cand = synth.eligible_work(cl)
+    pairs, cand = bench_work.eligible_work(cl)
     shape = _place_shape(cl, place)
     shape.pop("hist_beta")
     ctx.close()
@@ -886,7 +1001,7 @@ def ncu_import(rep, out_path, command):
         raise SystemExit(f"no kernel launch in {rep}")
     dirty = bool(subprocess.run(["git", "status", "--porcelain", "--", "paper_2606_30391_b200"], cwd=ROOT, capture_output=True, text=True).stdout.strip())
     summary = dict(launches[0])
-    summary.update({"captured_at_git_sha": _git_sha(), "sources_modified_since_that_commit": dirty,
+    summary.update({"captured_at_git_sha": _git_sha(), "sources_modified_since_that_commit": dirty, "csrc_hash": _csrc_hash(),
                     "command": command, "report": os.path.basename(rep), "launches_in_report": len(launches),
                     "note": "figures of a run under the profiler (cold caches, serialised, ~40 replays): evidence for shares "
                             "and counters, never a bench value"})
@@ -929,6 +1044,8 @@ def main():
     ap.add_argument("--variant-sample", type=int, default=128, help="requests per variant recomputed by the oracle")
     ap.add_argument("--aux", type=int, default=1, help="1: add the configs[3] / configs[4] / configs[0] / configs[1] legs")
     ap.add_argument("--sustained-s", type=float, default=2.0, help="seconds of back-to-back replays for `sustained` (0: off)")
+    ap.add_argument("--detail-out", default=os.path.join(ROOT, "bench_detail.json"),
+                    help="where the full result goes (histograms, work counters, notes, ncu summaries); stdout carries the contract line only")
     ap.add_argument("--ncu-import", default=None, help="an .ncu-rep to summarise (with --ncu-out); nothing is run on a GPU")
     ap.add_argument("--ncu-out", default=None)
     ap.add_argument("--ncu-cmd", default="", help="the ncu command line that made the report (recorded in the summary)")
@@ -955,7 +1072,7 @@ def main():
         dev = torch.device("cuda", lrank)
         torch.cuda.set_device(dev)
         flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-        print(json.dumps(run_aux_leg(args, torch, dev, args.workload, flush)), flush=True)
+        emit(run_aux_leg(args, torch, dev, args.workload, flush), args.detail_out)
     else:
         run_ours(args)
 

@@ -11,6 +11,7 @@ import fs_compare as cmp
 import fs_util as U
 import oracle
 from paper_2606_30391_b200 import synth
+import bench_work
 
 pytestmark = pytest.mark.gpu
 
@@ -885,16 +886,16 @@ def test_rack_tie_variants_full(ctx, variant):
     """configs[1] with tables quantised to a few powers of two and every SLO relaxed (ties inside a GPU), and with
     eight GPU records repeated (exact ties ACROSS GPUs: no bound is strict, every GPU of the best kind is swept);
     every tie must fall to the lowest flat index; compared in full."""
-    cl = synth.make_variant("rack", variant)
+    cl = bench_work.make_variant("rack", variant)
     ctx.load_cluster(cl)
     cmp.assert_placement_equal(ctx.place_batch(cl.requests), _oracle_place(cl))
 
 
-@pytest.mark.parametrize("variant", list(synth.VARIANTS))
+@pytest.mark.parametrize("variant", list(bench_work.VARIANTS))
 def test_pod_workload_variants_sampled(ctx, variant):
     """configs[2] with a less degenerate shape: 4x the dynamic power (chosen frequencies spread over the levels)
     or cheap weight loads (cold starts meet the TTFT deadline, so the sorted cold scan does the work)."""
-    cl = synth.make_variant("pod", variant)
+    cl = bench_work.make_variant("pod", variant)
     ctx.load_cluster(cl)
     got = ctx.place_batch(cl.requests)
     idx = np.arange(0, cl.R, 256 if variant in ("dynamic_power_x4", "cold_starts_feasible") else 1024)

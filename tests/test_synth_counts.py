@@ -1,4 +1,4 @@
-"""synth.eligible_work (the size of the dense definition's candidate set, used by bench.py for its rates)
+"""bench_work.eligible_work (the size of the dense definition's candidate set, used by bench.py for its rates)
 against a plain double loop over (request, GPU), and the workload variants' shapes."""
 from __future__ import annotations
 
@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 
 from paper_2606_30391_b200 import synth
+import bench_work
 
 f32 = np.float32
 
@@ -40,17 +41,17 @@ def test_eligible_work_equals_double_loop(seed):
     cl = synth.make_custom(seed=900 + seed, K=23, M=3, F=5, S=6, B=4, R=57, lo=1, hi=4)
     cl.states["mem_free_mb"][::3] *= 0.05                     # some GPUs too full for most requests
     cl.states["n_res"][1] = 0
-    assert synth.eligible_work(cl) == _loop_count(cl)
+    assert bench_work.eligible_work(cl) == _loop_count(cl)
 
 
 def test_variants_keep_the_shape_and_change_what_they_say():
     base = synth.make_cluster("tiny")
-    for v in synth.VARIANTS:
-        cl = synth.make_variant("tiny", v)
+    for v in bench_work.VARIANTS:
+        cl = bench_work.make_variant("tiny", v)
         assert cl.lat.shape == base.lat.shape and cl.K == base.K and cl.R == base.R
-    assert np.all(synth.make_variant("tiny", "dynamic_power_x4").pow >= base.pow)
-    assert np.all(synth.make_variant("tiny", "cold_starts_feasible").models["load_ms"] < base.models["load_ms"])
-    t = synth.make_variant("tiny", "ties")
+    assert np.all(bench_work.make_variant("tiny", "dynamic_power_x4").pow >= base.pow)
+    assert np.all(bench_work.make_variant("tiny", "cold_starts_feasible").models["load_ms"] < base.models["load_ms"])
+    t = bench_work.make_variant("tiny", "ties")
     assert len(np.unique(t.lat)) <= 3 and len(np.unique(t.pow)) <= 2
     with pytest.raises(ValueError):
-        synth.make_variant("tiny", "nope")
+        bench_work.make_variant("tiny", "nope")
