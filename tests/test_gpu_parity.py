@@ -438,8 +438,8 @@ def test_dispatch_full_size(ctx):
 
 @pytest.mark.parametrize("R", [1, 19, 2959, 11840, 11841, 14799, 20000])
 def test_request_counts_around_the_static_dynamic_boundary(ctx, R):
-    """The scoring kernel assigns all but the last four rounds of requests statically (148 blocks x 20 warps
-    = 2,960 requests per round) and hands out the tail dynamically: every request exactly once at any R."""
+    """The scoring kernel hands requests to its warps by ticket (an atomic counter, two requests ahead); request counts
+    around multiples of a full wave of warps (148 blocks x 20 warps = 2,960): every request exactly once at any R."""
     cl = synth.make_cluster("rack")
     reqs = synth.make_requests(4242 + R, R, cl.M)
     ctx.load_cluster(cl)
@@ -1000,6 +1000,12 @@ def test_hand_computed_coupling_cases_through_cuda(ctx):
     cl = pins._coupled_cluster(beta1=2)
     ctx.load_cluster(cl)
     assert ctx.place_batch(cl.requests)[0]["gpu"] == -1
+    cl = pins._consol_busy_cluster()                    # pair score with busy destinations, by hand
+    ctx.load_cluster(cl)
+    out = ctx.consolidate()
+    for a, (dst, phi, score, saving) in enumerate(pins.CONSOL_BY_HAND):
+        assert (int(out[a]["dst"]), int(out[a]["phi"])) == (dst, phi), a
+        assert out[a]["score_mj"] == np.float32(score) and out[a]["saving_mj"] == np.float32(saving), a
     cl = pins._power_cluster()
     ctx.load_cluster(cl)
     o = ctx.local_config(1 | 2)[0]

@@ -488,6 +488,67 @@ def test_consolidate_margin_delta():
 
 
 # ---------------------------------------------------------------------------------------------
+# Pair score with BUSY destinations, BY HAND (SURVEY 8(c) fs_consolidate steps 1-4; P:46, P:351, P:623;
+# DESIGN s18 "score = extra energy the destination pays").  Six GPUs, F = 2, S = 16 (S_eff = 15), B = 2.
+# Every tenant has an empty prefill queue and 4 decode tokens at bucket beta = 1: 2 rounds x LAT 2.0 = 4 ms,
+# energy = 4 x POW.  A model's table makes it infeasible (LAT 1000 > TBT slack 10) below its minimum share and
+# sets POW = E/4 there (E/8 at larger shares: the rule takes the LOWEST feasible share, not the cheapest).
+#
+#   GPU  tenants (model)   need[phi0, phi1]   E[phi0, phi1]     C*_g (own optimum)      sum of mig_mj
+#   0    2 (0, 1)          4+4, 2+2 = 8, 4    100+50, 300+100   150  at phi 0           30+12 = 42
+#   1    1 (2)             8, 3               1000, 1500        1000 at phi 0           5
+#   2    1 (3)             8, 1               200, 800          200  at phi 0           7
+#   3    1 (4)             8, 1               5000, 5100        5000 at phi 0           9
+#   4    3 (5, 5, 5)       3, 3               3, 3              3    at phi 0 (tie)     6
+#   5    1 (6)             8, 2               7000, 7100        7000 at phi 0           11
+#
+# Source 0 (2 tenants): GPU 4 is out (2 + 3 > 4 tenants) although it would score 153 - 3 = 150.  With every other
+# destination phi 0 needs 8 + 8 = 16 > 15 units, so the merged GPU runs at phi 1 although BOTH run at phi 0 alone:
+#   b=1: 1500+400 = 1900 - 1000 = 900     b=2: 800+400 = 1200 - 200 = 1000    (lowest C*_ab, not the lowest score)
+#   b=3: 5100+400 = 5500 - 5000 = 500     b=5: 7100+400 = 7500 - 7000 = 500   (exact tie: lower index wins)
+#   => dst 3, phi 1, score 500, saving = (100 W x 1000 ms + 150) - (500 + 42) = 99608.
+# Source 1: b=0: 400+1500 - 150 = 1750; b=2: 2300 - 200 = 2100; b=3: 6600 - 5000 = 1600; b=5: 8600 - 7000 = 1600;
+#   b=4 (1 + 3 = 4 tenants: allowed): phi 0 needs 8 + 3 = 11: 3 + 1000 = 1003 - 3 = 1000 => dst 4, phi 0,
+#   saving = 101000 - (1000 + 5) = 99995.
+# Source 4 (3 tenants: only single-tenant destinations): every one of b = 1, 2, 3, 5 costs E_b[0] + 3 - C*_b = 3
+#   => dst 1, phi 0, saving = 100003 - (3 + 6) = 99994.
+# Sources 2, 3, 5 all go to GPU 4 at phi 0: scores 203-3 = 200, 5003-3 = 5000, 7003-3 = 7000;
+#   savings 100200 - 207 = 99993, 105000 - 5009 = 99991, 107000 - 7011 = 99989.
+CONSOL_BY_HAND = [  # (dst, phi, score_mj, saving_mj) per source
+    (3, 1, 500.0, 99608.0), (4, 0, 1000.0, 99995.0), (4, 0, 200.0, 99993.0),
+    (4, 0, 5000.0, 99991.0), (1, 0, 3.0, 99994.0), (4, 0, 7000.0, 99989.0)]
+
+
+def _consol_busy_cluster():
+    need = {0: (4, 2), 1: (4, 2), 2: (8, 3), 3: (8, 1), 4: (8, 1), 5: (1, 1), 6: (8, 2)}
+    energy = {0: (100, 300), 1: (50, 100), 2: (1000, 1500), 3: (200, 800), 4: (5000, 5100), 5: (1, 1), 6: (7000, 7100)}
+    M, F, S, B = 7, 2, 16, 2
+    lat = np.full((M, 2, F, S, B), 3.0, dtype=np.float32)       # bucket 0 and the prefill phase: never read
+    pw = np.full((M, 2, F, S, B), 7.0, dtype=np.float32)
+    for m in range(M):
+        for phi in range(F):
+            lo = need[m][phi] - 1
+            lat[m, 1, phi, :lo, 1] = 1000.0
+            lat[m, 1, phi, lo:, 1] = 2.0
+            pw[m, 1, phi, :, 1] = energy[m][phi] / 8.0
+            pw[m, 1, phi, lo, 1] = energy[m][phi] / 4.0
+    models = mk_models(M)
+    models["mig_mj"] = [30.0, 12.0, 5.0, 7.0, 9.0, 2.0, 11.0]
+    t = lambda m, sg: dict(model=m, sigma=sg, beta=(0, 1), q=(0, 4), slo=(1e9, 10.0), mem=100.0)
+    states = mk_states([mk_state(tenants=[t(0, 5), t(1, 5)]), mk_state(tenants=[t(2, 9)]), mk_state(tenants=[t(3, 9)]),
+                        mk_state(tenants=[t(4, 9)]), mk_state(tenants=[t(5, 1), t(5, 1), t(5, 1)]), mk_state(tenants=[t(6, 9)])])
+    return cluster_from(lat, pw, models, states, mk_requests([]),
+                        synth.Params(p_idle_w=100.0, horizon_ms=1000.0, mem_cap_mb=80000.0, delta_pct=5))
+
+
+def test_consolidate_busy_destinations_by_hand():
+    out = _consol(_consol_busy_cluster())
+    for a, (dst, phi, score, saving) in enumerate(CONSOL_BY_HAND):
+        assert (int(out[a]["dst"]), int(out[a]["phi"])) == (dst, phi), a
+        assert out[a]["score_mj"] == f32(score) and out[a]["saving_mj"] == f32(saving), a
+
+
+# ---------------------------------------------------------------------------------------------
 # Co-resident coupling BY HAND (P:44, P:127, P:265 shared operating point; DESIGN s4): a busy tenant of the
 # request's model (bump: its decode batch grows by the new sequence) and a busy tenant of another model.
 # Every number below is written out; none comes from fs_brute or from the oracle.
