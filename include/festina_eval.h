@@ -53,7 +53,9 @@ typedef enum {
   FS_OK = 0,
   FS_ERR_ARG = -1,   /* NULL pointer, bad enum, bad count                       */
   FS_ERR_SHAPE = -2, /* dims outside the supported range                        */
-  FS_ERR_STATE = -3, /* call order: profiles / GPU state not loaded yet         */
+  FS_ERR_STATE = -3, /* call order: profiles / GPU state not loaded yet; or a call that has to allocate
+                        (first call of these sizes) was made while `cuda_stream` is being captured: run
+                        it once outside the capture first                                          */
   FS_ERR_RANGE = -4, /* an index / value inside device data was out of range    */
   FS_ERR_CUDA = -5,  /* a CUDA runtime call failed (see fs_last_cuda_error)     */
   FS_ERR_NOMEM = -6  /* device or host allocation failed                        */

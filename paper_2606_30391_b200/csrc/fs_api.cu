@@ -47,6 +47,7 @@ struct fs_ctx {
   uint64_t launches = 0; int last_cuda = 0;
   bool timing = false; bool have_events = false; FsTimers tm{};
   int sm_count = 148; bool count_work = false;
+  cudaStream_t cur = nullptr;   // the stream of the API call in progress (grow() asks whether it is being captured)
 };
 
 namespace {
@@ -63,14 +64,25 @@ namespace {
 
 // The new buffer is allocated before the old one is released: after a failed allocation the pointer and the
 // caller's capacity field still describe a valid (old) buffer, and the next call simply tries again.
+// A call that has to grow a buffer allocates and (when it replaces one) waits for the device: neither is legal
+// while the caller's stream is being captured into a graph, and the synchronisation would silently invalidate the
+// capture.  Such a call returns FS_ERR_STATE instead ("run the call once with these sizes before capturing").
 template <class T> int grow(fs_ctx* c, T*& p, size_t n_elems) {
   if (n_elems == 0) n_elems = 1;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(c->cur, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+  if (cap != cudaStreamCaptureStatusNone) return FS_ERR_STATE;
   T* fresh = nullptr;
   FS_CUDA(c, cudaMalloc((void**)&fresh, n_elems * sizeof(T)));
   if (p) {
     // kernels of earlier calls may still read the old buffer on the caller's streams
-    FS_CUDA(c, cudaDeviceSynchronize());
-    FS_CUDA(c, cudaFree(p));
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaFree(p);
+    if (e != cudaSuccess) {                 // keep the old buffer (still described by the caller's capacity field)
+      cudaFree(fresh);
+      c->last_cuda = (int)e; cudaGetLastError();
+      return FS_ERR_CUDA;
+    }
   }
   p = fresh;
   return FS_OK;
@@ -205,7 +217,7 @@ int fs_load_profiles(fs_ctx* c, const fs_dims* dims, const float* lat, const flo
       dims->S > FS_MAX_S || dims->B < 1 || dims->B > FS_MAX_B)
     return FS_ERR_SHAPE;
   if (params->delta_pct < 0 || params->delta_pct > 100) return FS_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   c->have_prof = false; c->have_state = false; c->K = 0; c->consol_cap = 0;
@@ -247,7 +259,7 @@ int fs_set_gpu_state(fs_ctx* c, int32_t K, const fs_gpu_state* states, int space
   if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof) return FS_ERR_STATE;
   if ((unsigned long long)K * c->d.S * c->d.F >= 0xFFFFFFFFull) return FS_ERR_SHAPE;  // flat is 32-bit
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (K > c->k_cap) {
@@ -284,7 +296,7 @@ int fs_place_batch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* o
   if (!c || R < 0 || (R > 0 && (!reqs || !out))) return FS_ERR_ARG;
   if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (R == 0) return pending;
@@ -334,7 +346,7 @@ int fs_local_config(fs_ctx* c, int32_t n, const int32_t* gpu_ids, uint32_t flags
   if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (!gpu_ids && n > c->K) return FS_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (n == 0) return pending;
@@ -376,7 +388,7 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
   if (!c || !space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (c->K > 0 && !out) return FS_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (c->K == 0) return pending;
@@ -385,6 +397,9 @@ int fs_consolidate(fs_ctx* c, fs_consol_out* out, int space, void* cuda_stream) 
     const size_t kp = (size_t)c->K * ((c->d.F + 1) / 2 + 1);   // frequency pairs + one row: the pair kernel prefetches one trip ahead
     FS_TRY(grow(c, c->need, kf)); FS_TRY(grow(c, c->E, kf)); FS_TRY(grow(c, c->agg, (size_t)c->K));
     FS_TRY(grow(c, c->E2, kp)); FS_TRY(grow(c, c->T2, kp));
+    // the pair kernel's software pipeline loads one row past the last frequency pair and discards it: that row
+    // is never written by the pack kernel, so give it defined contents once (no uninitialised read)
+    FS_CUDA(c, cudaMemsetAsync(c->E2, 0, kp * sizeof(*c->E2), st)); FS_CUDA(c, cudaMemsetAsync(c->T2, 0, kp * sizeof(*c->T2), st));
     FS_TRY(grow(c, c->ckeys, (size_t)c->K)); FS_TRY(grow(c, c->consol_dev, (size_t)c->K));
     c->consol_cap = kf;
   }
@@ -408,7 +423,7 @@ int fs_dispatch(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placement* out,
   if (!space_ok(space)) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (c->K >= (1 << 24)) return FS_ERR_SHAPE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (R == 0) return pending;
@@ -446,7 +461,7 @@ int fs_dispatch_commit(fs_ctx* c, int32_t R, const fs_request* reqs, fs_placemen
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
   if (c->K >= (1 << 24)) return FS_ERR_SHAPE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (R == 0 && !after) return pending;
@@ -481,7 +496,7 @@ int fs_llm_profiles(fs_ctx* c, int32_t n, const fs_llm* llms, fs_llm_profile* ou
   if (!c || n < 0 || (n > 0 && (!llms || !out))) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
   if (!c->have_prof) return FS_ERR_STATE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (n == 0) return pending;
@@ -507,7 +522,7 @@ int fs_ewr(fs_ctx* c, int32_t n, const int32_t* gpu_of, const float* f_mhz, cons
            float* f_gpu, double* out3, int space, void* cuda_stream) {
   if (!c || n < 0 || K < 0 || !out3 || (n > 0 && (!gpu_of || !f_mhz || !t_ms)) || (K > 0 && !f_gpu)) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   const int32_t* d_g = gpu_of; const float *d_f = f_mhz, *d_t = t_ms; float* d_fg = f_gpu; double* d_o = out3;
@@ -541,7 +556,7 @@ int fs_replace_plan(fs_ctx* c, int32_t n, const fs_plan_llm* llms, int32_t s_eff
                     int32_t* gpu_of, int32_t* summary, int space, void* cuda_stream) {
   if (!c || n < 0 || !summary || (n > 0 && (!llms || !gpu_of)) || s_eff < 1 || s_eff > FS_MAX_S) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   const size_t sb = fsk_plan_scratch_bytes(n);
@@ -572,7 +587,7 @@ int fs_migration_plan(fs_ctx* c, int32_t n, const float* bytes_mb, const float* 
   if (!c || n < 0 || !total_us || (n > 0 && (!bytes_mb || !bw || !dst_of))) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
   if (n > 1024) return FS_ERR_SHAPE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   const float *d_b = bytes_mb, *d_w = bw; int32_t* d_d = dst_of; long long* d_t = reinterpret_cast<long long*>(total_us);
@@ -603,7 +618,7 @@ int fs_migration_select(fs_ctx* c, int32_t r, const fs_mig_req* reqs, uint8_t* f
                         void* cuda_stream) {
   if (!c || r < 0 || (r > 0 && (!reqs || !flags || !mig_ms))) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (r == 0) return pending;
@@ -632,7 +647,7 @@ int fs_batch_tasks(fs_ctx* c, int32_t n, const int32_t* gpu_ids, const int32_t* 
   if (!c || n < 0 || n_tasks < 0 || (n > 0 && !task_off) || (n_tasks > 0 && (!tasks || !out))) return FS_ERR_ARG;
   if (space != FS_HOST && space != FS_DEVICE) return FS_ERR_ARG;
   if (!c->have_prof || !c->have_state) return FS_ERR_STATE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaStream_t st = (cudaStream_t)cuda_stream; c->cur = st;
   FS_CUDA(c, cudaSetDevice(c->dev));
   const int pending = take_flags(c);
   if (n == 0) return pending;
@@ -662,7 +677,7 @@ const char* fs_strerror(int code) {
     case FS_OK: return "ok";
     case FS_ERR_ARG: return "bad argument";
     case FS_ERR_SHAPE: return "dims outside the supported range";
-    case FS_ERR_STATE: return "profiles or GPU state not loaded";
+    case FS_ERR_STATE: return "profiles or GPU state not loaded (or the call must allocate while its stream is being captured)";
     case FS_ERR_RANGE: return "index or value out of range in device data";
     case FS_ERR_CUDA: return "CUDA runtime error";
     case FS_ERR_NOMEM: return "out of memory";

@@ -881,6 +881,43 @@ def test_step_is_capturable_into_a_cuda_graph(ctx):
     assert not np.array_equal(cl2.states["n_res"], cl.states["n_res"])
 
 
+def test_first_call_of_a_size_inside_a_capture_is_refused_not_allocated(fs):
+    """A call that would have to allocate (and wait for the device) while its stream is being captured returns
+    FS_ERR_STATE and enqueues nothing, instead of invalidating the capture; after one call outside a capture the
+    same call captures and replays."""
+    import torch
+    cl = synth.make_cluster("tiny")
+    c = fs.Festina(0)
+    c.load_cluster(cl)
+    dev = torch.device("cuda", 0)
+    d_reqs = torch.from_numpy(cl.requests.view(np.uint8).reshape(-1).copy()).to(dev)
+    d_out = torch.zeros(cl.R * 32, dtype=torch.uint8, device=dev)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        g.capture_begin()
+        try:
+            with pytest.raises(fs.FestinaError) as e:
+                c.place_batch(d_reqs, out=d_out, stream=s)          # first call with R requests: needs its buffers
+            assert e.value.code == fs.FS_ERR_STATE
+        finally:
+            g.capture_end()
+    torch.cuda.synchronize()
+    c.place_batch(d_reqs, out=d_out, stream=s)                      # outside a capture: allocates
+    torch.cuda.synchronize()
+    g2 = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        g2.capture_begin()
+        c.place_batch(d_reqs, out=d_out, stream=s)
+        g2.capture_end()
+    d_out.zero_()
+    g2.replay()
+    torch.cuda.synchronize()
+    cmp.assert_placement_equal(d_out.cpu().numpy().view(synth.PLACEMENT_DT), _oracle_place(cl))
+    c.close()
+
+
 @pytest.mark.parametrize("variant", ["ties", "identical_gpus"])
 def test_rack_tie_variants_full(ctx, variant):
     """configs[1] with tables quantised to a few powers of two and every SLO relaxed (ties inside a GPU), and with
