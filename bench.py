@@ -55,9 +55,9 @@ OPS_ROW = 4.0              # per swept (pair, phi): A0 load, add, min, subtract/
 OPS_WARM_TEST = 30.0       # per warm pair tested: 16-word item, bound (2 table bounds + 4 fp32), 3 compares
 OPS_DEF = 15.0             # per candidate scored by the definition: 4 loads, 4 mul, 4 add/sub, 3 compares
 SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128   # 4 schedulers x 32 lanes (B300_MICROARCH "issue")
-NCU_POD = os.path.join(ROOT, "profiles", "r02_pod_ncu.json")
-NCU_LOCAL = os.path.join(ROOT, "profiles", "r02_local_ncu.json")
-NCU_CONSOL = os.path.join(ROOT, "profiles", "r02_consol_ncu.json")
+NCU_POD = os.path.join(ROOT, "profiles", "r03_pod_ncu.json")
+NCU_LOCAL = os.path.join(ROOT, "profiles", "r03_local_ncu.json")
+NCU_CONSOL = os.path.join(ROOT, "profiles", "r03_consol_ncu.json")
 
 
 def _peaks():

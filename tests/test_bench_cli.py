@@ -49,9 +49,9 @@ import pytest
 
 def _full_result_like_round_2():
     """A full result dict of the size that broke round 2 (its 27.9 KB one-line JSON overflowed the driver's 3 KB
-    tail): the tracked round-2 detail, which has every leg, histogram and ncu summary."""
+    tail): the tracked detail of a default run, which has every leg, histogram and ncu summary."""
     import bench
-    full = json.load(open(os.path.join(ROOT, "profiles", "r02_bench_pod.json")))
+    full = json.load(open(os.path.join(ROOT, "profiles", "r03_bench_pod.json")))
     full["roofline"]["ncu"] = bench._ncu_block(bench.NCU_POD)     # as a run of today's bench.py embeds it
     return full
 
