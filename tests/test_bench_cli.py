@@ -42,6 +42,9 @@ def test_tracked_ncu_summaries_are_what_the_roofline_blocks_read():
         assert not blk.get("missing"), path
         assert kernel in blk["kernel"] and blk["warp_instructions"] > 0 and blk["duration_ns"] > 0
         assert blk["command"].startswith("ncu ") and blk["captured_at_git_sha"]
+        # taken on the kernel sources as they are now: a later edit of csrc/ or the header must come with new captures
+        assert blk["stale"] is False, (path, blk.get("csrc_hash"), blk["bench_csrc_hash"])
+        assert 0 < blk["hbm_frac"] < 0.2
 
 
 import pytest
