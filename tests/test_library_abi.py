@@ -68,3 +68,22 @@ def test_product_never_imports_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text, f
                 assert "festina_oracle" not in text, f
+
+
+def test_static_plan_entry_point_validates_before_it_touches_cuda():
+    """fs_replace_plan_static (the no-allocation entry point): bad counts and a size beyond the built-in scratch array
+    are refused from the host-visible arguments alone; without a device a well-formed call fails with FS_ERR_CUDA."""
+    import ctypes as C
+    import torch
+    L = fs.lib()
+    one = (C.c_int32 * 4)()
+    buf = (C.c_uint8 * 64)()
+    assert L.fs_replace_plan_static(-1, buf, 8, 1.0, one, one, None) == fs.FS_ERR_ARG
+    assert L.fs_replace_plan_static(1, None, 8, 1.0, one, one, None) == fs.FS_ERR_ARG
+    assert L.fs_replace_plan_static(1, buf, 0, 1.0, one, one, None) == fs.FS_ERR_ARG          # s_eff < 1
+    assert L.fs_replace_plan_static(1, buf, 33, 1.0, one, one, None) == fs.FS_ERR_ARG         # s_eff > FS_MAX_S
+    assert L.fs_replace_plan_static(fs.FS_PLAN_STATIC_MAX_N + 1, buf, 8, 1.0, one, one, None) == fs.FS_ERR_SHAPE
+    text = open(HEADER).read()
+    assert re.search(r"#define\s+FS_PLAN_STATIC_MAX_N\s+%d\b" % fs.FS_PLAN_STATIC_MAX_N, text)
+    if not torch.cuda.is_available():
+        assert L.fs_replace_plan_static(0, None, 8, 1.0, None, one, None) == fs.FS_ERR_CUDA
